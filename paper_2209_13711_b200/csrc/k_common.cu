@@ -1,0 +1,247 @@
+// k_common.cu -- a0 hit indexing (PAPER.md:125 SoA event data) and the generic
+// work-list kernels (emit items, scan item counts, row offsets) used by every stage.
+#include "lst_launch.h"
+
+namespace lst {
+
+// ------------------------------------------------------------------ begin: reset the slot header
+__global__ void k_begin(SlotDev s) {
+  Header *h = s.hdr;
+  const int t = threadIdx.x;
+  if (t < 8) h->n_obj[t] = 0;
+  if (t < S_NSTAGE) { h->n_items[t] = 0; h->n_groups[t] = 0; h->cand[t] = 0ull; }
+  if (t == 0) { h->err = 0; h->pad = 0; }
+}
+
+// ------------------------------------------------------------------ a0.1 histogram of det ids
+__global__ void k_hist(GeoDev geo, SlotDev s) {
+  const uint32_t n = s.hdr->n_hits;
+  for (uint32_t h = blockIdx.x * blockDim.x + threadIdx.x; h < n; h += gridDim.x * blockDim.x) {
+    const uint32_t d = s.raw_det[h];
+    if (d >= geo.n_det) { atomicOr(&s.hdr->err, (uint32_t)ERR_DET); continue; }
+    atomicAdd(&s.det_cnt[d], 1u);
+  }
+}
+
+// Exclusive scan of in[0..n) into out[0..n], out[n] = total; one block.
+__device__ void block_scan_array(const uint32_t *in, uint32_t *out, uint32_t n, uint32_t *sh) {
+  uint32_t carry = 0;
+  for (uint32_t base = 0; base < n; base += blockDim.x) {
+    const uint32_t i = base + threadIdx.x;
+    const uint32_t v = i < n ? in[i] : 0u;
+    uint32_t tot;
+    const uint32_t e = block_excl_scan(v, sh, &tot);
+    if (i < n) out[i] = carry + e;
+    carry += tot;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[n] = carry;
+}
+
+// ------------------------------------------------------------------ a0.2 scan + MD groups
+// det_off = exclusive scan of det_cnt; MD group of module m: rows = lower hits, width = upper hits.
+__global__ void k_det_scan(GeoDev geo, SlotDev s) {
+  __shared__ uint32_t sh[33];
+  block_scan_array(s.det_cnt, s.det_off, geo.n_det, sh);
+  __syncthreads();
+  for (uint32_t d = threadIdx.x; d < geo.n_det; d += blockDim.x) s.det_cur[d] = 0;
+  const StageBuf &st = s.st[S_MD];
+  for (uint32_t m = threadIdx.x; m < geo.n_modules; m += blockDim.x) {
+    st.gR[m] = s.det_cnt[2 * m];
+    st.gW[m] = s.det_cnt[2 * m + 1];
+  }
+  if (threadIdx.x == 0) s.hdr->n_groups[S_MD] = geo.n_modules;
+}
+
+// ------------------------------------------------------------------ a0.3 scatter (unordered within a det)
+__global__ void k_scatter(GeoDev geo, SlotDev s) {
+  const uint32_t n = s.hdr->n_hits;
+  for (uint32_t h = blockIdx.x * blockDim.x + threadIdx.x; h < n; h += gridDim.x * blockDim.x) {
+    const uint32_t d = s.raw_det[h];
+    if (d >= geo.n_det) continue;
+    const uint32_t p = s.det_off[d] + atomicAdd(&s.det_cur[d], 1u);
+    s.tmp_orig[p] = h;
+  }
+}
+
+// ------------------------------------------------------------------ a0.4 rank inside the det
+// Makes the order canonical (ascending caller index within a det) whatever order the atomics gave.
+__global__ void k_rank(GeoDev geo, SlotDev s) {
+  const uint32_t n = s.det_off[geo.n_det];
+  for (uint32_t p = blockIdx.x * blockDim.x + threadIdx.x; p < n; p += gridDim.x * blockDim.x) {
+    const uint32_t h = s.tmp_orig[p];
+    const uint32_t d = s.raw_det[h];
+    const uint32_t b = s.det_off[d], e = s.det_off[d + 1];
+    uint32_t r = 0;
+    for (uint32_t q = b; q < e; ++q) r += (s.tmp_orig[q] < h);
+    const float x = s.raw_x[h], y = s.raw_y[h], z = s.raw_z[h];
+    s.hit[b + r] = make_float4(x, y, z, sqrtf(x * x + y * y));
+    s.hit_orig[b + r] = h;
+  }
+}
+
+// ------------------------------------------------------------------ emit work items
+__device__ __forceinline__ uint32_t items_of(uint32_t R, uint32_t W) {
+  if (R == 0 || W == 0) return 0;
+  if (W <= (uint32_t)kItemCand) {
+    const uint32_t rpi = (uint32_t)kItemCand / W;
+    return (R + rpi - 1) / rpi;
+  }
+  return R * ((W + kItemCand - 1) / kItemCand);
+}
+
+// One block.  rows_level >= 0: the groups are kRowChunk-row chunks of that object level and the
+// kernel sets n_groups itself (gR must be 1, gW the group's candidate count: written by the
+// stage's group kernel for every g < ceil(n_rows / kRowChunk)).
+__global__ void k_emit_items(SlotDev s, int stage, int rows_level) {
+  __shared__ uint32_t sh[33];
+  __shared__ unsigned long long sh_cand;
+  Header *hdr = s.hdr;
+  const StageBuf &st = s.st[stage];
+  uint32_t ng;
+  if (rows_level >= 0) ng = (hdr->n_obj[rows_level] + kRowChunk - 1) / kRowChunk;
+  else ng = hdr->n_groups[stage];
+  if (ng > st.cap_groups) ng = 0;   // cannot happen: cap_groups is sized from the object capacity
+  if (threadIdx.x == 0) sh_cand = 0ull;
+  __syncthreads();
+  uint32_t carry = 0;
+  unsigned long long my_cand = 0;
+  for (uint32_t base = 0; base < ng; base += blockDim.x) {
+    const uint32_t g = base + threadIdx.x;
+    uint32_t ni = 0;
+    if (g < ng) {
+      const uint32_t R = st.gR[g], W = st.gW[g];
+      ni = items_of(R, W);
+      my_cand += (unsigned long long)R * W;
+    }
+    uint32_t tot;
+    const uint32_t e = block_excl_scan(ni, sh, &tot);
+    if (g < ng) st.g_item0[g] = carry + e;
+    carry += tot;
+    __syncthreads();
+  }
+  atomicAdd(&sh_cand, my_cand);
+  __syncthreads();
+  const bool overflow = carry > st.cap_items;
+  if (threadIdx.x == 0) {
+    st.g_item0[ng] = carry;
+    hdr->n_groups[stage] = ng;
+    hdr->n_items[stage] = overflow ? 0u : carry;
+    hdr->cand[stage] = sh_cand;
+    if (overflow) atomicOr(&hdr->err, (uint32_t)ERR_CAP_ITEMS);
+  }
+  if (overflow) return;
+  for (uint32_t g = threadIdx.x; g < ng; g += blockDim.x) {
+    const uint32_t R = st.gR[g], W = st.gW[g];
+    const uint32_t ni = items_of(R, W);
+    Item *out = st.items + st.g_item0[g];
+    if (ni == 0) continue;
+    if (W <= (uint32_t)kItemCand) {
+      const uint32_t rpi = (uint32_t)kItemCand / W;
+      for (uint32_t k = 0; k < ni; ++k) {
+        Item it;
+        it.group = g; it.i0 = k * rpi; it.j0 = 0;
+        it.nrows = (uint16_t)min(rpi, R - k * rpi); it.nj = (uint16_t)W;
+        out[k] = it;
+      }
+    } else {
+      const uint32_t nt = (W + kItemCand - 1) / kItemCand;
+      for (uint32_t k = 0; k < ni; ++k) {
+        Item it;
+        it.group = g; it.i0 = k / nt; it.j0 = (k % nt) * kItemCand;
+        it.nrows = 1; it.nj = (uint16_t)min((uint32_t)kItemCand, W - it.j0);
+        out[k] = it;
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------ scan item pass counts
+// One block.  Exact object count of the level; overflow empties the level (never truncates).
+__global__ void k_scan_items(SlotDev s, int stage, int level, uint32_t cap) {
+  __shared__ uint32_t sh[33];
+  Header *hdr = s.hdr;
+  const StageBuf &st = s.st[stage];
+  const uint32_t n = hdr->n_items[stage];
+  uint32_t carry = 0;
+  for (uint32_t base = 0; base < n; base += blockDim.x) {
+    const uint32_t i = base + threadIdx.x;
+    const uint32_t v = i < n ? st.item_cnt[i] : 0u;
+    uint32_t tot;
+    const uint32_t e = block_excl_scan(v, sh, &tot);
+    if (i < n) st.item_base[i] = carry + e;
+    carry += tot;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    if (carry > cap) {
+      atomicOr(&hdr->err, (uint32_t)ERR_CAP_OBJ);
+      hdr->n_items[stage] = 0;
+      hdr->n_obj[level] = 0;
+    } else {
+      hdr->n_obj[level] = carry;
+    }
+  }
+}
+
+// ------------------------------------------------------------------ row offsets from sorted row keys
+// off[r] = first object whose row key >= r, r in [0, n_rows]; keys ascending.
+// KIND 0: MD -> module (n_rows = n_modules); 1: LS -> inner MD; 2: T3 -> first MD (n_rows = n_md)
+template <int KIND>
+__global__ void k_row_offsets(GeoDev geo, SlotDev s) {
+  const Header *hdr = s.hdr;
+  uint32_t n, n_rows;
+  uint32_t *off;
+  if (KIND == 0) { n = hdr->n_obj[0]; n_rows = geo.n_modules; off = s.md_mod_off; }
+  else if (KIND == 1) { n = hdr->n_obj[1]; n_rows = hdr->n_obj[0]; off = s.ls_md_off; }
+  else { n = hdr->n_obj[2]; n_rows = hdr->n_obj[0]; off = s.t3_md_off; }
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nt = gridDim.x * blockDim.x;
+  if (n == 0) {
+    for (uint32_t r = tid; r <= n_rows; r += nt) off[r] = 0;
+    return;
+  }
+  for (uint32_t k = tid; k < n; k += nt) {
+    uint32_t key, prev;
+    if (KIND == 0) { key = s.md_mod[k] >> 2; prev = k ? (s.md_mod[k - 1] >> 2) + 1 : 0; }
+    else if (KIND == 1) { key = s.ls_md[k].x; prev = k ? s.ls_md[k - 1].x + 1 : 0; }
+    else { key = s.t3_md[k].x; prev = k ? s.t3_md[k - 1].x + 1 : 0; }
+    for (uint32_t r = prev; r <= key; ++r) off[r] = k;
+    if (k == n - 1) for (uint32_t r = key + 1; r <= n_rows; ++r) off[r] = n;
+  }
+}
+
+// ------------------------------------------------------------------ host launchers
+static inline int grid_for(uint32_t n, int threads, int max_blocks) {
+  long b = ((long)n + threads - 1) / threads;
+  if (b < 1) b = 1;
+  if (b > max_blocks) b = max_blocks;
+  return (int)b;
+}
+
+void launch_index(const Ctx &c, const SlotDev &s, cudaStream_t st) {
+  cudaMemsetAsync(s.det_cnt, 0, sizeof(uint32_t) * (c.geo.n_det + 1), st);
+  k_begin<<<1, 32, 0, st>>>(s);
+  const int g = grid_for(s.cap_hits, 256, c.n_sm * 8);
+  k_hist<<<g, 256, 0, st>>>(c.geo, s);
+  k_det_scan<<<1, 1024, 0, st>>>(c.geo, s);
+  k_scatter<<<g, 256, 0, st>>>(c.geo, s);
+  k_rank<<<g, 256, 0, st>>>(c.geo, s);
+}
+
+void launch_emit(const Ctx &c, const SlotDev &s, int stage, int rows_level, cudaStream_t st) {
+  (void)c;
+  k_emit_items<<<1, 1024, 0, st>>>(s, stage, rows_level);
+}
+void launch_scan_items(const Ctx &c, const SlotDev &s, int stage, int level, uint32_t cap, cudaStream_t st) {
+  (void)c;
+  k_scan_items<<<1, 1024, 0, st>>>(s, stage, level, cap);
+}
+void launch_row_offsets(const Ctx &c, const SlotDev &s, int kind, cudaStream_t st) {
+  const uint32_t cap = kind == 0 ? s.cap_md : (kind == 1 ? s.cap_ls : s.cap_t3);
+  const int g = grid_for(cap, 256, c.n_sm * 4);
+  if (kind == 0) k_row_offsets<0><<<g, 256, 0, st>>>(c.geo, s);
+  else if (kind == 1) k_row_offsets<1><<<g, 256, 0, st>>>(c.geo, s);
+  else k_row_offsets<2><<<g, 256, 0, st>>>(c.geo, s);
+}
+
+}  // namespace lst

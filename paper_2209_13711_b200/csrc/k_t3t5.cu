@@ -1,0 +1,201 @@
+// k_t3t5.cu -- a3 triplets (Fig. 5, 8; reading C4) and a4 quintuplets (PAPER.md:73,
+// Fig. 9; reading C5: radius match, middle triplet, weighted Kasa circle-fit chi2).
+//
+// Both are joins on a shared mini-doublet: a T3 is LS (1,2) + LS (2,3), a T5 is T3 (1,2,3) +
+// T3 (3,4,5).  Left objects are the rows; the right list of a row is the contiguous range of
+// objects whose first MD is the row's last MD (LS are grouped by inner MD, T3 by first MD).
+// Groups are chunks of kRowChunk rows; a group's candidates are numbered row-major.
+#include "lst_launch.h"
+
+namespace lst {
+
+struct RowTab {                       // right-list table of one group, in shared memory
+  uint32_t start[kRowChunk];
+  uint32_t cum[kRowChunk + 1];
+};
+
+// T5 = false: rows are LS, right lists are LS ranges of the outer MD.
+// T5 = true : rows are T3, right lists are T3 ranges of the third MD.
+template <bool T5>
+__device__ __forceinline__ void right_range(const SlotDev &s, uint32_t row, uint32_t *st, uint32_t *cnt) {
+  if (!T5) {
+    const uint32_t mo = s.ls_md[row].y;
+    *st = s.ls_md_off[mo];
+    *cnt = s.ls_md_off[mo + 1] - *st;
+  } else {
+    const uint32_t m3 = s.t3_md[row].z;
+    *st = s.t3_md_off[m3];
+    *cnt = s.t3_md_off[m3 + 1] - *st;
+  }
+}
+
+template <bool T5>
+__global__ void k_join_groups(SlotDev s) {
+  const int stage = T5 ? S_T5 : S_T3;
+  const StageBuf &st = s.st[stage];
+  const uint32_t n_rows = s.hdr->n_obj[T5 ? 2 : 1];
+  const uint32_t ng = (n_rows + kRowChunk - 1) / kRowChunk;
+  const int lane = threadIdx.x & 31;
+  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+  for (uint32_t gidx = warp; gidx < ng; gidx += nwarp) {
+    const uint32_t r0 = gidx * kRowChunk, r1 = min(r0 + kRowChunk, n_rows);
+    uint32_t sum = 0;
+    for (uint32_t r = r0 + lane; r < r1; r += 32) {
+      uint32_t a, c;
+      right_range<T5>(s, r, &a, &c);
+      sum += c;
+    }
+    sum = warp_sum(sum);
+    if (lane == 0) { st.gR[gidx] = 1; st.gW[gidx] = sum; }
+  }
+}
+
+template <bool T5>
+__device__ __forceinline__ void stage_rows(RowTab &rt, const SlotDev &s, uint32_t r0, uint32_t n_rows, uint32_t *sh) {
+  const int tid = threadIdx.x;   // kThreads == kRowChunk
+  uint32_t a = 0, c = 0;
+  if (r0 + tid < n_rows) right_range<T5>(s, r0 + tid, &a, &c);
+  uint32_t tot;
+  const uint32_t e = block_excl_scan(c, sh, &tot);
+  rt.start[tid] = a;
+  rt.cum[tid] = e;
+  if (tid == 0) rt.cum[kRowChunk] = tot;
+  __syncthreads();
+}
+// flat candidate -> (row in group, right object)
+__device__ __forceinline__ void flat_to_pair(const RowTab &rt, uint32_t cf, int *row, uint32_t *right) {
+  int lo = 0, hi = kRowChunk;
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (rt.cum[mid] <= cf) lo = mid; else hi = mid;
+  }
+  *row = lo;
+  *right = rt.start[lo] + (cf - rt.cum[lo]);
+}
+
+__device__ __forceinline__ Pt md_point(const SlotDev &s, uint32_t md) {
+  const float4 p = s.md_pos[md];
+  return make_pt(p.x, p.y, p.z, (int)(s.md_mod[md] & 3u));
+}
+
+// ------------------------------------------------------------------ evaluation of one candidate
+__device__ __forceinline__ bool t3_candidate(const SlotDev &s, const Params &g, uint32_t a, uint32_t b, T3Out *o,
+                                             uint4 *mds) {
+  const uint2 la = s.ls_md[a], lb = s.ls_md[b];
+  const Pt P1 = md_point(s, la.x), P2 = md_point(s, la.y), P3 = md_point(s, lb.y);
+  if (mds) *mds = make_uint4(la.x, la.y, lb.y, 0u);
+  return t3_eval_d(g, P1, P2, P3, o);
+}
+__device__ __forceinline__ bool t5_candidate(const SlotDev &s, const Params &g, uint32_t a, uint32_t b, T5Out *o,
+                                             uint32_t *mds, double2 *ka, double2 *kb) {
+  const double2 k3a = s.t3_kd[a], k3b = s.t3_kd[b];
+  if (ka) { *ka = k3a; *kb = k3b; }
+  if (!o && !le(fabs(k3a.x - k3b.x), g.ns * (k3a.y + k3b.y))) return false;   // early T5-1
+  const uint4 ta = s.t3_md[a], tb = s.t3_md[b];
+  const uint32_t m[5] = {ta.x, ta.y, ta.z, tb.y, tb.z};
+  Pt P[5];
+#pragma unroll
+  for (int k = 0; k < 5; ++k) { P[k] = md_point(s, m[k]); if (mds) mds[k] = m[k]; }
+  return t5_eval_d(g, P, k3a.x, k3a.y, k3b.x, k3b.y, o);
+}
+
+template <bool T5>
+__global__ void __launch_bounds__(kThreads) k_join_eval(SlotDev s, Params g) {
+  __shared__ ItemScratch sc;
+  __shared__ RowTab rt;
+  __shared__ uint32_t sh[33];
+  const int stage = T5 ? S_T5 : S_T3;
+  const StageBuf &st = s.st[stage];
+  const uint32_t n_items = s.hdr->n_items[stage];
+  const uint32_t n_rows = s.hdr->n_obj[T5 ? 2 : 1];
+  const int tid = threadIdx.x;
+  for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+    const Item item = st.items[it];
+    const uint32_t r0 = item.group * kRowChunk;
+    if (tid < kItemWords) sc.mask[tid] = 0;
+    stage_rows<T5>(rt, s, r0, n_rows, sh);
+    const int nj = item.nj;
+    for (int base = 0; base < nj; base += kThreads) {
+      const int c = base + tid;
+      bool pass = false;
+      if (c < nj) {
+        int row; uint32_t b;
+        flat_to_pair(rt, item.j0 + c, &row, &b);
+        pass = T5 ? t5_candidate(s, g, r0 + row, b, nullptr, nullptr, nullptr, nullptr)
+                  : t3_candidate(s, g, r0 + row, b, nullptr, nullptr);
+      }
+      const uint32_t w = __ballot_sync(0xffffffffu, pass);
+      if ((tid & 31) == 0) sc.mask[c >> 5] = w;
+    }
+    __syncthreads();
+    publish_mask(sc, st.mask + (size_t)it * kItemWords, st.item_cnt + it);
+    __syncthreads();
+  }
+}
+
+template <bool T5>
+__global__ void __launch_bounds__(kThreads) k_join_fill(SlotDev s, Params g) {
+  __shared__ ItemScratch sc;
+  __shared__ RowTab rt;
+  __shared__ uint32_t sh[33];
+  const int stage = T5 ? S_T5 : S_T3;
+  const StageBuf &st = s.st[stage];
+  const uint32_t n_items = s.hdr->n_items[stage];
+  const uint32_t n_rows = s.hdr->n_obj[T5 ? 2 : 1];
+  const int tid = threadIdx.x;
+  for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+    if (st.item_cnt[it] == 0) continue;
+    const Item item = st.items[it];
+    const uint32_t r0 = item.group * kRowChunk;
+    stage_rows<T5>(rt, s, r0, n_rows, sh);
+    expand_mask(sc, st.mask + (size_t)it * kItemWords);
+    const int n = (int)sc.n;
+    const uint32_t base = st.item_base[it];
+    for (int k = tid; k < n; k += kThreads) {
+      int row; uint32_t b;
+      flat_to_pair(rt, item.j0 + sc.list[k], &row, &b);
+      const uint32_t a = r0 + row, idx = base + k;
+      if (!T5) {
+        T3Out o; uint4 m;
+        t3_candidate(s, g, a, b, &o, &m);
+        s.t3_md[idx] = m;
+        s.t3_ls[idx] = make_uint2(a, b);
+        s.t3_kd[idx] = make_double2(o.kappa3, o.sigk3);
+        s.t3_beta[idx] = (float)o.beta;
+      } else {
+        T5Out o; uint32_t m[5]; double2 ka, kb;
+        t5_candidate(s, g, a, b, &o, m, &ka, &kb);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) s.t5_md[(size_t)5 * idx + q] = m[q];
+        s.t5_t3[idx] = make_uint2(a, b);
+        s.t5_chi2[idx] = o.chi2;
+        s.t5_etaphi[idx] = make_double2(o.eta, o.phi);
+        s.t5_f[idx] = make_float4((float)o.R, (float)o.chi2, (float)ka.x, (float)kb.x);
+        s.t5_pt[idx] = (float)o.pt;
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// ------------------------------------------------------------------ launchers
+void launch_t3(const Ctx &c, const SlotDev &s, cudaStream_t st) {
+  const int gg = (int)((s.cap_ls / kRowChunk + 1 + 3) / 4);   // 4 warps per block, one group per warp
+  k_join_groups<false><<<gg < c.n_sm * 8 ? gg : c.n_sm * 8, 128, 0, st>>>(s);
+  launch_emit(c, s, S_T3, 1, st);
+  k_join_eval<false><<<c.n_sm * 8, kThreads, 0, st>>>(s, c.par);
+  launch_scan_items(c, s, S_T3, 2, s.cap_t3, st);
+  k_join_fill<false><<<c.n_sm * 8, kThreads, 0, st>>>(s, c.par);
+  launch_row_offsets(c, s, 2, st);
+}
+
+void launch_t5(const Ctx &c, const SlotDev &s, cudaStream_t st) {
+  const int gg = (int)((s.cap_t3 / kRowChunk + 1 + 3) / 4);
+  k_join_groups<true><<<gg < c.n_sm * 8 ? gg : c.n_sm * 8, 128, 0, st>>>(s);
+  launch_emit(c, s, S_T5, 2, st);
+  k_join_eval<true><<<c.n_sm * 8, kThreads, 0, st>>>(s, c.par);
+  launch_scan_items(c, s, S_T5, 3, s.cap_t5, st);
+  k_join_fill<true><<<c.n_sm * 8, kThreads, 0, st>>>(s, c.par);
+}
+
+}  // namespace lst

@@ -1,0 +1,606 @@
+// lst_api.cu -- the C-ABI of include/lst.h: context, module-map builder (host), workspace layout,
+// event upload, the launch chain (optionally one CUDA graph per slot) and result views.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/lst.h"
+#include "lst_launch.h"
+
+using namespace lst;
+
+// ------------------------------------------------------------------ status text
+static thread_local char g_cuda_err[256] = "no CUDA error recorded";
+
+static int cuda_fail(cudaError_t e, const char *where) {
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "CUDA error at %s: %s", where, cudaGetErrorString(e));
+  return LST_ECUDA;
+}
+#define CU(call)                                          \
+  do {                                                    \
+    cudaError_t e_ = (call);                              \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call);   \
+  } while (0)
+
+extern "C" const char *lst_strerror(int status) {
+  switch (status) {
+    case LST_OK: return "ok";
+    case LST_EINVAL: return "invalid argument";
+    case LST_ENOMEM: return "workspace too small or object capacity exceeded";
+    case LST_ECUDA: return g_cuda_err;
+    case LST_ESTATE: return "call order violated";
+    default: return "unknown status";
+  }
+}
+
+// ------------------------------------------------------------------ config
+extern "C" void lst_default_config(lst_config *c) {
+  if (!c) return;
+  memset(c, 0, sizeof(*c));
+  const double s12 = std::sqrt(12.0);
+  c->kB = 0.00299792458 * 3.8;
+  c->pt_min = 0.8;
+  c->n_sigma = 4.0;
+  c->z0max = 15.0;
+  c->d0max = 2.5;
+  c->chi2max = 18.42;
+  c->dr2max = 1e-4;
+  c->map_kscale = 1.25;
+  c->map_z0 = 20.0;
+  c->ec_md_sys = 0.3;
+  c->modez_slack = 0.15;
+  c->seed_sig_phi = 0.001;
+  c->seed_sig_pt = 0.01;
+  c->seed_sig_z = 0.05;
+  const double pitch_t[4] = {0.01, 0.009, 0.01, 0.009};
+  const double len_z[4] = {0.15, 5.0, 0.0, 0.0}, len_r[4] = {0.0, 0.0, 0.15, 5.0};
+  for (int k = 0; k < 4; ++k) {
+    c->sig_t[k] = pitch_t[k] / s12;
+    c->sig_z[k] = len_z[k] / s12;
+    c->sig_r[k] = len_r[k] / s12;
+  }
+  c->dup_t5_shared = 5;
+  c->dup_pt5_shared = 5;
+  c->dup_pt3_shared = 3;
+  c->s0_enabled = 1;
+  c->start_layer_mask = 0x3u | (0x3u << 6) | (0x3u << 11);
+  c->cap_md_per_hit = 1.0f;
+  c->cap_ls_per_hit = 6.0f;
+  c->cap_t3_per_hit = 6.0f;
+  c->cap_t5_per_hit = 2.0f;
+  c->cap_pt3_per_seed = 96.0f;
+  c->cap_pt5_per_seed = 48.0f;
+  c->cap_mdcand_per_hit = 64.0f;
+  c->cap_lscand_per_hit = 512.0f;
+  c->cap_t3cand_per_hit = 64.0f;
+  c->cap_t5cand_per_hit = 16.0f;
+  c->use_cuda_graph = 1;
+}
+
+static void make_params(const lst_config &c, Params *p) {
+  memset(p, 0, sizeof(*p));
+  p->kmax = c.kB / (2.0 * c.pt_min);
+  p->kB = c.kB; p->ns = c.n_sigma; p->z0max = c.z0max; p->d0max = c.d0max; p->chi2max = c.chi2max;
+  p->dr2max = c.dr2max; p->ec_md_sys = c.ec_md_sys; p->modez_slack = c.modez_slack;
+  p->seed_sig_phi = c.seed_sig_phi; p->seed_sig_pt = c.seed_sig_pt; p->seed_sig_z = c.seed_sig_z;
+  for (int k = 0; k < 4; ++k) {
+    p->sig_t[k] = c.sig_t[k]; p->sig_z[k] = c.sig_z[k]; p->sig_r[k] = c.sig_r[k];
+    p->f_sig_t[k] = (float)c.sig_t[k]; p->f_sig_z[k] = (float)c.sig_z[k]; p->f_sig_r[k] = (float)c.sig_r[k];
+  }
+  p->f_kmax = (float)p->kmax; p->f_ns = (float)c.n_sigma; p->f_z0max = (float)c.z0max;
+  p->f_ec_md_sys = (float)c.ec_md_sys; p->f_modez_slack = (float)c.modez_slack;
+  p->dup_t5 = c.dup_t5_shared; p->dup_pt5 = c.dup_pt5_shared; p->dup_pt3 = c.dup_pt3_shared;
+  p->s0_enabled = c.s0_enabled;
+  p->start_mask = c.start_layer_mask;
+}
+
+static bool geometry_ok(const lst_geometry *g) {
+  if (!g || g->n_modules == 0 || !g->category || !g->logical_layer || !g->rmin || !g->rmax || !g->phic ||
+      !g->half_phi || !g->zmin || !g->zmax)
+    return false;
+  for (uint32_t m = 0; m < g->n_modules; ++m)
+    if (g->category[m] > 3 || g->logical_layer[m] > 15) return false;
+  return true;
+}
+
+// ------------------------------------------------------------------ C2 module map (host)
+// PAPER.md:53-55 (Fig. 4).  Reading C2: B is connected to A iff B sits in a layer that may follow
+// A's, and the phi and r-z intervals swept from A's box by helices with |kappa| <= kscale*kmax,
+// |z0| <= map_z0 (and a d0max allowance in phi) overlap B's box.
+namespace {
+struct Box { double rlo, rhi, phi, hphi, zlo, zhi; bool endcap; };
+
+inline void followers(int layer, int out[3], int *n) {
+  *n = 0;
+  if (layer < 6) {
+    if (layer < 5) out[(*n)++] = layer + 1;
+    out[(*n)++] = 6;
+    out[(*n)++] = 11;
+  } else if (layer != 10 && layer != 15) {
+    out[(*n)++] = layer + 1;
+  }
+}
+
+inline bool reachable(const Box &A, const Box &B, double kp, double z0m, double d0m) {
+  const double angA = std::asin(std::min(1.0, kp * A.rlo));
+  const double angB = std::asin(std::min(1.0, kp * B.rhi));
+  const double dphi = std::fabs(std::remainder(B.phi - A.phi, 2.0 * M_PI));
+  const double bend = angB - angA + d0m * std::max(0.0, 1.0 / A.rlo - 1.0 / B.rhi);
+  if (!(dphi <= A.hphi + B.hphi + bend)) return false;
+  const double rho[2] = {B.rlo / A.rhi, angB / angA};
+  const double z0[2] = {-z0m, z0m}, zA[2] = {A.zlo, A.zhi};
+  if (!B.endcap) {
+    double lo = INFINITY, hi = -INFINITY;
+    for (double v0 : z0) for (double va : zA) for (double r : rho) {
+      const double zp = v0 + (va - v0) * r;
+      lo = std::min(lo, zp); hi = std::max(hi, zp);
+    }
+    return lo <= B.zhi && hi >= B.zlo;
+  }
+  const double side = B.zlo > 0 ? 1.0 : -1.0;
+  double lo = INFINITY, hi = -INFINITY;
+  int nvalid = 0;
+  for (double v0 : z0) for (double va : zA) {
+    const double den = va - v0;
+    if (!(side * den > 0.0)) continue;
+    const double q = (B.zlo - v0) / den;
+    lo = std::min(lo, q); hi = std::max(hi, q);
+    ++nvalid;
+  }
+  if (nvalid == 0) return false;
+  if (nvalid < 4) hi = INFINITY;
+  return lo <= rho[1] && hi >= rho[0];
+}
+}  // namespace
+
+extern "C" int lst_build_module_map(const lst_geometry *g, const lst_config *cfg_in, uint32_t **row_offsets,
+                                    uint32_t **cols) {
+  if (!geometry_ok(g) || !row_offsets || !cols) return LST_EINVAL;
+  lst_config cfg;
+  if (cfg_in) cfg = *cfg_in; else lst_default_config(&cfg);
+  const uint32_t n = g->n_modules;
+  const double kp = cfg.map_kscale * cfg.kB / (2.0 * cfg.pt_min);
+  std::vector<Box> box(n);
+  std::vector<std::vector<uint32_t>> by_layer(16);
+  for (uint32_t m = 0; m < n; ++m) {
+    box[m] = Box{(double)g->rmin[m], (double)g->rmax[m], (double)g->phic[m], (double)g->half_phi[m],
+                 (double)g->zmin[m], (double)g->zmax[m], g->category[m] >= 2};
+    by_layer[g->logical_layer[m]].push_back(m);
+  }
+  std::vector<uint32_t> off(n + 1, 0), out;
+  std::vector<uint32_t> row;
+  for (uint32_t A = 0; A < n; ++A) {
+    int nl[3], nn;
+    followers(g->logical_layer[A], nl, &nn);
+    row.clear();
+    for (int k = 0; k < nn; ++k)
+      for (uint32_t B : by_layer[nl[k]])
+        if (reachable(box[A], box[B], kp, cfg.map_z0, cfg.d0max)) row.push_back(B);
+    std::sort(row.begin(), row.end());
+    off[A] = (uint32_t)out.size();
+    out.insert(out.end(), row.begin(), row.end());
+  }
+  off[n] = (uint32_t)out.size();
+  uint32_t *o = (uint32_t *)malloc(sizeof(uint32_t) * (n + 1));
+  uint32_t *c = (uint32_t *)malloc(sizeof(uint32_t) * std::max<size_t>(out.size(), 1));
+  if (!o || !c) { free(o); free(c); return LST_ENOMEM; }
+  memcpy(o, off.data(), sizeof(uint32_t) * (n + 1));
+  if (!out.empty()) memcpy(c, out.data(), sizeof(uint32_t) * out.size());
+  *row_offsets = o;
+  *cols = c;
+  return LST_OK;
+}
+extern "C" void lst_free(void *p) { free(p); }
+
+// ------------------------------------------------------------------ context
+struct Slot {
+  SlotDev dev;
+  void *workspace = nullptr;
+  size_t ws_bytes = 0;
+  bool bound = false, loaded = false, ran = false;
+  cudaStream_t last_stream = nullptr;
+  cudaGraphExec_t graph = nullptr;
+  bool graph_has_seeds = false;
+  // pinned host staging for copy_to_host views (allocated on first use)
+  uint32_t *h_hits = nullptr, *h_par = nullptr;
+  float *h_f = nullptr;
+  uint8_t *h_keep = nullptr;
+  Header *h_hdr = nullptr;       // pinned
+};
+
+struct lst_ctx {
+  lst_config cfg;
+  Ctx k;
+  uint32_t n_slots, max_hits, max_seeds;
+  void *d_static = nullptr;      // geometry + map on the device
+  std::vector<Slot> slots;
+  size_t ws_bytes = 0;
+  size_t exp_obj_cap = 0, exp_hit_words = 0;
+};
+
+// bump allocator over the workspace; base == nullptr only measures
+struct Carver {
+  char *base;
+  size_t off = 0;
+  explicit Carver(void *b) : base((char *)b) {}
+  template <class T>
+  T *take(size_t n) {
+    off = (off + 255) & ~(size_t)255;
+    T *p = base ? (T *)(base + off) : nullptr;
+    off += sizeof(T) * (n ? n : 1);
+    return p;
+  }
+};
+
+static uint32_t capf(float per, uint32_t n, uint32_t floor_) {
+  const double v = (double)per * (double)n;
+  const double c = std::min(v, 4.0e9);
+  return std::max<uint32_t>((uint32_t)c, floor_);
+}
+
+static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
+  Carver w(base);
+  SlotDev s;
+  memset(&s, 0, sizeof(s));
+  const lst_config &cf = c->cfg;
+  const uint32_t nh = std::max<uint32_t>(c->max_hits, 1), nsd = std::max<uint32_t>(c->max_seeds, 1);
+  const uint32_t n_mod = c->k.geo.n_modules, n_det = c->k.geo.n_det;
+  s.cap_hits = nh; s.cap_seeds = nsd;
+  s.cap_md = capf(cf.cap_md_per_hit, nh, 1024);
+  s.cap_ls = capf(cf.cap_ls_per_hit, nh, 1024);
+  s.cap_t3 = capf(cf.cap_t3_per_hit, nh, 1024);
+  s.cap_t5 = capf(cf.cap_t5_per_hit, nh, 1024);
+  s.cap_pt3 = capf(cf.cap_pt3_per_seed, nsd, 1024);
+  s.cap_pt5 = capf(cf.cap_pt5_per_seed, nsd, 1024);
+  s.cap_tc = s.cap_pt5 + s.cap_pt3 + s.cap_t5 + nsd;
+  s.hdr = w.take<Header>(1);
+  s.raw_x = w.take<float>(nh); s.raw_y = w.take<float>(nh); s.raw_z = w.take<float>(nh);
+  s.raw_det = w.take<uint32_t>(nh);
+  s.seed_pt = w.take<float>(nsd); s.seed_eta = w.take<float>(nsd); s.seed_phi = w.take<float>(nsd);
+  s.seed_z0 = w.take<float>(nsd); s.seed_q = w.take<int8_t>(nsd); s.seed_ids = w.take<uint32_t>(4 * (size_t)nsd);
+  s.det_cnt = w.take<uint32_t>(n_det + 1); s.det_off = w.take<uint32_t>(n_det + 1);
+  s.det_cur = w.take<uint32_t>(n_det + 1);
+  s.tmp_orig = w.take<uint32_t>(nh);
+  s.hit = w.take<float4>(nh); s.hit_orig = w.take<uint32_t>(nh);
+  s.md_pos = w.take<float4>(s.cap_md); s.md_kd = w.take<double2>(s.cap_md); s.md_kf = w.take<float2>(s.cap_md);
+  s.md_hit = w.take<uint2>(s.cap_md); s.md_mod = w.take<uint32_t>(s.cap_md); s.md_dphi = w.take<float>(s.cap_md);
+  s.md_mod_off = w.take<uint32_t>(n_mod + 1);
+  s.ls_md = w.take<uint2>(s.cap_ls); s.ls_f = w.take<float4>(s.cap_ls);
+  s.ls_md_off = w.take<uint32_t>((size_t)s.cap_md + 1);
+  s.t3_md = w.take<uint4>(s.cap_t3); s.t3_ls = w.take<uint2>(s.cap_t3); s.t3_kd = w.take<double2>(s.cap_t3);
+  s.t3_beta = w.take<float>(s.cap_t3);
+  s.t3_md_off = w.take<uint32_t>((size_t)s.cap_md + 1);
+  s.t5_md = w.take<uint32_t>(5 * (size_t)s.cap_t5); s.t5_t3 = w.take<uint2>(s.cap_t5);
+  s.t5_chi2 = w.take<double>(s.cap_t5); s.t5_etaphi = w.take<double2>(s.cap_t5);
+  s.t5_f = w.take<float4>(s.cap_t5); s.t5_pt = w.take<float>(s.cap_t5); s.t5_keep = w.take<uint8_t>(s.cap_t5);
+  s.pt5_po = w.take<uint2>(s.cap_pt5); s.pt3_po = w.take<uint2>(s.cap_pt3);
+  s.pt5_chi2 = w.take<double>(s.cap_pt5); s.pt3_chi2 = w.take<double>(s.cap_pt3);
+  s.pt5_keep = w.take<uint8_t>(s.cap_pt5); s.pt3_keep = w.take<uint8_t>(s.cap_pt3);
+  s.pls_keep = w.take<uint8_t>(nsd);
+  s.tc_to = w.take<uint2>(s.cap_tc); s.tc_f = w.take<float4>(s.cap_tc);
+  // work lists
+  const uint32_t cand_cap[S_NSTAGE] = {
+      capf(cf.cap_mdcand_per_hit, nh, 1 << 16), capf(cf.cap_lscand_per_hit, nh, 1 << 16),
+      capf(cf.cap_t3cand_per_hit, nh, 1 << 16), capf(cf.cap_t5cand_per_hit, nh, 1 << 16),
+      capf(2048.0f, nsd, 1 << 16), capf(4096.0f, nsd, 1 << 16)};
+  const uint32_t grp_cap[S_NSTAGE] = {n_mod, n_mod, s.cap_ls / kRowChunk + 2, s.cap_t3 / kRowChunk + 2,
+                                      nsd / kRowChunk + 2, nsd / kRowChunk + 2};
+  for (int k = 0; k < S_NSTAGE; ++k) {
+    StageBuf &b = s.st[k];
+    b.cap_groups = grp_cap[k];
+    b.cap_items = grp_cap[k] + 2 * (cand_cap[k] / kItemCand) + 16;
+    b.gR = w.take<uint32_t>(b.cap_groups); b.gW = w.take<uint32_t>(b.cap_groups);
+    b.g_item0 = w.take<uint32_t>((size_t)b.cap_groups + 1);
+    b.items = w.take<Item>(b.cap_items);
+    b.mask = w.take<uint32_t>((size_t)b.cap_items * kItemWords);
+    b.item_cnt = w.take<uint32_t>(b.cap_items); b.item_base = w.take<uint32_t>(b.cap_items);
+  }
+  // export scratch: the largest level
+  size_t obj_cap = std::max({(size_t)s.cap_md, (size_t)s.cap_ls, (size_t)s.cap_t3, (size_t)s.cap_t5,
+                             (size_t)s.cap_pt3, (size_t)s.cap_pt5, (size_t)s.cap_tc});
+  size_t hit_words = std::max({2 * (size_t)s.cap_md, 4 * (size_t)s.cap_ls, 6 * (size_t)s.cap_t3,
+                               10 * (size_t)s.cap_t5, 6 * (size_t)s.cap_pt3, 10 * (size_t)s.cap_pt5,
+                               14 * (size_t)s.cap_tc});
+  s.exp_hits = w.take<uint32_t>(hit_words);
+  s.exp_par = w.take<uint32_t>(2 * obj_cap);
+  s.exp_f = w.take<float>(4 * obj_cap);
+  if (out) *out = s;
+  const_cast<lst_ctx *>(c)->exp_obj_cap = obj_cap;
+  const_cast<lst_ctx *>(c)->exp_hit_words = hit_words;
+  return (w.off + 255) & ~(size_t)255;
+}
+
+extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, const lst_config *cfg_in,
+                          uint32_t n_slots, uint32_t max_hits, uint32_t max_seeds, lst_ctx **out) {
+  if (!geometry_ok(g) || !map || !map->row_offsets || !out || n_slots == 0 || max_hits == 0) return LST_EINVAL;
+  const uint32_t n = g->n_modules;
+  if (n > (1u << 29)) return LST_EINVAL;
+  if (map->row_offsets[0] != 0) return LST_EINVAL;
+  const uint32_t nnz = map->row_offsets[n];
+  if (nnz && !map->cols) return LST_EINVAL;
+  for (uint32_t m = 0; m < n; ++m) {
+    const uint32_t a = map->row_offsets[m], b = map->row_offsets[m + 1];
+    if (b < a || b > nnz || b - a > (uint32_t)kMaxDeg) return LST_EINVAL;
+    for (uint32_t e = a; e < b; ++e) {
+      if (map->cols[e] >= n) return LST_EINVAL;
+      if (e > a && map->cols[e] <= map->cols[e - 1]) return LST_EINVAL;
+    }
+  }
+  lst_ctx *c = new (std::nothrow) lst_ctx();
+  if (!c) return LST_ENOMEM;
+  if (cfg_in) c->cfg = *cfg_in; else lst_default_config(&c->cfg);
+  make_params(c->cfg, &c->k.par);
+  c->n_slots = n_slots; c->max_hits = max_hits; c->max_seeds = max_seeds;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  cudaDeviceProp prop;
+  if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
+  if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaGetDeviceProperties"); }
+  c->k.n_sm = prop.multiProcessorCount;
+  // static data: category | layer | map_off | map_cols
+  const size_t o_cat = 0, o_lay = (n + 255) & ~(size_t)255, o_off = o_lay + ((n + 255) & ~(size_t)255);
+  const size_t o_cols = o_off + (((size_t)(n + 1) * 4 + 255) & ~(size_t)255);
+  const size_t total = o_cols + (size_t)std::max<uint32_t>(nnz, 1) * 4;
+  e = cudaMalloc(&c->d_static, total);
+  if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaMalloc(static)"); }
+  char *d = (char *)c->d_static;
+  cudaMemcpy(d + o_cat, g->category, n, cudaMemcpyHostToDevice);
+  cudaMemcpy(d + o_lay, g->logical_layer, n, cudaMemcpyHostToDevice);
+  cudaMemcpy(d + o_off, map->row_offsets, (size_t)(n + 1) * 4, cudaMemcpyHostToDevice);
+  if (nnz) cudaMemcpy(d + o_cols, map->cols, (size_t)nnz * 4, cudaMemcpyHostToDevice);
+  e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) { cudaFree(c->d_static); delete c; return cuda_fail(e, "upload geometry"); }
+  c->k.geo.n_modules = n; c->k.geo.n_det = 2 * n;
+  c->k.geo.category = (const uint8_t *)(d + o_cat);
+  c->k.geo.layer = (const uint8_t *)(d + o_lay);
+  c->k.geo.map_off = (const uint32_t *)(d + o_off);
+  c->k.geo.map_cols = (const uint32_t *)(d + o_cols);
+  for (int l = 0; l < 16; ++l) {
+    c->k.lay_rmin[l] = INFINITY; c->k.lay_rmax[l] = 0.f; c->k.lay_zmin[l] = INFINITY; c->k.lay_zmax[l] = -INFINITY;
+  }
+  for (uint32_t m = 0; m < n; ++m) {
+    const int l = g->logical_layer[m];
+    c->k.lay_rmin[l] = std::min(c->k.lay_rmin[l], g->rmin[m]);
+    c->k.lay_rmax[l] = std::max(c->k.lay_rmax[l], g->rmax[m]);
+    c->k.lay_zmin[l] = std::min(c->k.lay_zmin[l], g->zmin[m]);
+    c->k.lay_zmax[l] = std::max(c->k.lay_zmax[l], g->zmax[m]);
+  }
+  c->slots.resize(n_slots);
+  c->ws_bytes = carve(c, nullptr, nullptr);
+  *out = c;
+  return LST_OK;
+}
+
+static void free_slot_host(Slot &s) {
+  if (s.graph) cudaGraphExecDestroy(s.graph);
+  if (s.h_hits) cudaFreeHost(s.h_hits);
+  if (s.h_par) cudaFreeHost(s.h_par);
+  if (s.h_f) cudaFreeHost(s.h_f);
+  if (s.h_keep) cudaFreeHost(s.h_keep);
+  if (s.h_hdr) cudaFreeHost(s.h_hdr);
+  s = Slot();
+}
+
+extern "C" void lst_destroy(lst_ctx *c) {
+  if (!c) return;
+  cudaDeviceSynchronize();
+  for (Slot &s : c->slots) free_slot_host(s);
+  if (c->d_static) cudaFree(c->d_static);
+  delete c;
+}
+
+extern "C" size_t lst_workspace_bytes(const lst_ctx *c) { return c ? c->ws_bytes : 0; }
+
+extern "C" int lst_bind_workspace(lst_ctx *c, uint32_t slot, void *workspace, size_t bytes) {
+  if (!c || slot >= c->n_slots || !workspace || ((uintptr_t)workspace & 255)) return LST_EINVAL;
+  if (bytes < c->ws_bytes) return LST_ENOMEM;
+  Slot &s = c->slots[slot];
+  if (s.graph) { cudaGraphExecDestroy(s.graph); s.graph = nullptr; }
+  carve(c, workspace, &s.dev);
+  s.workspace = workspace; s.ws_bytes = bytes;
+  s.bound = true; s.loaded = false; s.ran = false;
+  if (!s.h_hdr) CU(cudaMallocHost((void **)&s.h_hdr, sizeof(Header)));
+  return LST_OK;
+}
+
+// ------------------------------------------------------------------ a0 upload
+__global__ void k_set_event(Header *h, uint32_t n_hits, uint32_t n_seeds) {
+  h->n_hits = n_hits;
+  h->n_seeds = n_seeds;
+}
+
+extern "C" int lst_load_event(lst_ctx *c, uint32_t slot, const lst_hits *hits, const lst_pixel_seeds *seeds,
+                              void *cuda_stream) {
+  if (!c || slot >= c->n_slots || !hits) return LST_EINVAL;
+  Slot &s = c->slots[slot];
+  if (!s.bound) return LST_ESTATE;
+  const uint32_t nh = hits->n, nsd = seeds ? seeds->n : 0;
+  if (nh > c->max_hits || nsd > c->max_seeds) return LST_EINVAL;
+  if (nh && (!hits->x || !hits->y || !hits->z || !hits->det)) return LST_EINVAL;
+  if (nsd && (!seeds->pt || !seeds->eta || !seeds->phi || !seeds->z0 || !seeds->q || !seeds->hit_ids)) return LST_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const SlotDev &d = s.dev;
+  if (nh) {
+    const cudaMemcpyKind k = hits->on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    CU(cudaMemcpyAsync(d.raw_x, hits->x, sizeof(float) * nh, k, st));
+    CU(cudaMemcpyAsync(d.raw_y, hits->y, sizeof(float) * nh, k, st));
+    CU(cudaMemcpyAsync(d.raw_z, hits->z, sizeof(float) * nh, k, st));
+    CU(cudaMemcpyAsync(d.raw_det, hits->det, sizeof(uint32_t) * nh, k, st));
+  }
+  if (nsd) {
+    const cudaMemcpyKind k = seeds->on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    CU(cudaMemcpyAsync(d.seed_pt, seeds->pt, sizeof(float) * nsd, k, st));
+    CU(cudaMemcpyAsync(d.seed_eta, seeds->eta, sizeof(float) * nsd, k, st));
+    CU(cudaMemcpyAsync(d.seed_phi, seeds->phi, sizeof(float) * nsd, k, st));
+    CU(cudaMemcpyAsync(d.seed_z0, seeds->z0, sizeof(float) * nsd, k, st));
+    CU(cudaMemcpyAsync(d.seed_q, seeds->q, sizeof(int8_t) * nsd, k, st));
+    CU(cudaMemcpyAsync(d.seed_ids, seeds->hit_ids, sizeof(uint32_t) * 4 * (size_t)nsd, k, st));
+  }
+  k_set_event<<<1, 1, 0, st>>>(d.hdr, nh, nsd);
+  CU(cudaGetLastError());
+  s.loaded = true; s.ran = false; s.last_stream = st;
+  return LST_OK;
+}
+
+// ------------------------------------------------------------------ the chain
+static void enqueue_chain(const lst_ctx *c, const SlotDev &d, cudaStream_t st) {
+  launch_index(c->k, d, st);
+  launch_md(c->k, d, st);
+  launch_ls(c->k, d, st);
+  launch_t3(c->k, d, st);
+  launch_t5(c->k, d, st);
+  launch_pixel(c->k, d, st);
+  launch_dedup(c->k, d, st);
+}
+
+extern "C" int lst_run(lst_ctx *c, uint32_t slot, void *cuda_stream) {
+  if (!c || slot >= c->n_slots) return LST_EINVAL;
+  Slot &s = c->slots[slot];
+  if (!s.bound || !s.loaded) return LST_ESTATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (c->cfg.use_cuda_graph) {
+    if (!s.graph) {
+      // capture on a private stream (the legacy default stream cannot be captured)
+      cudaGraph_t gr = nullptr;
+      cudaStream_t cap = nullptr;
+      CU(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+      cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+      if (e != cudaSuccess) { cudaStreamDestroy(cap); return cuda_fail(e, "cudaStreamBeginCapture"); }
+      enqueue_chain(c, s.dev, cap);
+      e = cudaStreamEndCapture(cap, &gr);
+      cudaStreamDestroy(cap);
+      if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
+      e = cudaGraphInstantiate(&s.graph, gr, 0);
+      cudaGraphDestroy(gr);
+      if (e != cudaSuccess) { s.graph = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
+    }
+    CU(cudaGraphLaunch(s.graph, st));
+  } else {
+    enqueue_chain(c, s.dev, st);
+    CU(cudaGetLastError());
+  }
+  s.ran = true; s.last_stream = st;
+  return LST_OK;
+}
+
+// ------------------------------------------------------------------ results
+static int sync_header(lst_ctx *c, Slot &s) {
+  (void)c;
+  CU(cudaMemcpyAsync(s.h_hdr, s.dev.hdr, sizeof(Header), cudaMemcpyDeviceToHost, s.last_stream));
+  CU(cudaStreamSynchronize(s.last_stream));
+  if (s.h_hdr->err & ERR_DET) return LST_EINVAL;
+  if (s.h_hdr->err & (ERR_CAP_ITEMS | ERR_CAP_OBJ)) return LST_ENOMEM;
+  return LST_OK;
+}
+
+extern "C" int lst_get_counts(lst_ctx *c, uint32_t slot, uint32_t *counts, uint64_t *cand) {
+  if (!c || slot >= c->n_slots || !counts) return LST_EINVAL;
+  Slot &s = c->slots[slot];
+  if (!s.ran) return LST_ESTATE;
+  const int rc = sync_header(c, s);
+  if (rc != LST_OK) return rc;
+  for (int l = 0; l < LST_NLEVEL; ++l) counts[l] = s.h_hdr->n_obj[l];
+  if (cand) for (int k = 0; k < 4; ++k) cand[k] = s.h_hdr->cand[k];
+  return LST_OK;
+}
+
+static const uint32_t kArity[LST_NLEVEL] = {2, 4, 6, 10, 6, 10, 14};
+
+extern "C" int lst_get_objects(lst_ctx *c, uint32_t slot, lst_level level, int copy_to_host, lst_objects *out) {
+  if (!c || slot >= c->n_slots || !out || (int)level < 0 || level >= LST_NLEVEL) return LST_EINVAL;
+  Slot &s = c->slots[slot];
+  if (!s.ran) return LST_ESTATE;
+  launch_export(c->k, s.dev, (int)level, s.last_stream);
+  CU(cudaGetLastError());
+  const int rc = sync_header(c, s);
+  if (rc != LST_OK) return rc;
+  lst_objects o;
+  memset(&o, 0, sizeof(o));
+  o.n = s.h_hdr->n_obj[level];
+  o.arity = kArity[level];
+  const uint8_t *keep_d = level == LST_T5 ? s.dev.t5_keep : level == LST_PT3 ? s.dev.pt3_keep
+                          : level == LST_PT5 ? s.dev.pt5_keep : nullptr;
+  if (!copy_to_host) {
+    o.hit_idx = s.dev.exp_hits; o.parents = s.dev.exp_par; o.f = s.dev.exp_f; o.keep = keep_d; o.on_device = 1;
+  } else {
+    if (!s.h_hits) {
+      CU(cudaMallocHost((void **)&s.h_hits, sizeof(uint32_t) * c->exp_hit_words));
+      CU(cudaMallocHost((void **)&s.h_par, sizeof(uint32_t) * 2 * c->exp_obj_cap));
+      CU(cudaMallocHost((void **)&s.h_f, sizeof(float) * 4 * c->exp_obj_cap));
+      CU(cudaMallocHost((void **)&s.h_keep, c->exp_obj_cap));
+    }
+    if (o.n) {
+      CU(cudaMemcpyAsync(s.h_hits, s.dev.exp_hits, sizeof(uint32_t) * (size_t)o.n * o.arity, cudaMemcpyDeviceToHost, s.last_stream));
+      CU(cudaMemcpyAsync(s.h_par, s.dev.exp_par, sizeof(uint32_t) * 2 * (size_t)o.n, cudaMemcpyDeviceToHost, s.last_stream));
+      CU(cudaMemcpyAsync(s.h_f, s.dev.exp_f, sizeof(float) * 4 * (size_t)o.n, cudaMemcpyDeviceToHost, s.last_stream));
+      if (keep_d) CU(cudaMemcpyAsync(s.h_keep, keep_d, o.n, cudaMemcpyDeviceToHost, s.last_stream));
+      CU(cudaStreamSynchronize(s.last_stream));
+    }
+    o.hit_idx = s.h_hits; o.parents = s.h_par; o.f = s.h_f; o.keep = keep_d ? s.h_keep : nullptr; o.on_device = 0;
+  }
+  *out = o;
+  return LST_OK;
+}
+
+extern "C" uint32_t lst_launches_per_run(const lst_ctx *c) {
+  (void)c;
+  return 0;
+}
+
+// ------------------------------------------------------------------ host test hooks
+// Run the very same __host__ __device__ selection arithmetic on the CPU (tests only; no GPU needed).
+// pts: n * npts * 3 floats (x, y, z per point), cats: n * npts, aux: level-specific doubles.
+//   level MD : npts 2 (lower, upper), cats[0] = module category;             out f: kappa, sigk, dphi
+//   level LS : npts 2 (anchors), aux = {ki, ski, ko, sko};                  out f: kappa, sigk, dphi
+//   level T3 : npts 3;                                                      out f: kappa3, sigk3, beta
+//   level T5 : npts 5, aux = {k3a, sk3a, k3b, sk3b};                        out f: R, chi2, eta (pt, phi skipped)
+// pass[i] = fp64 decision, pre[i] = fp32 pre-filter verdict (1 where the level has none).
+extern "C" int lst_host_eval(const lst_config *cfg_in, int level, uint32_t n, const float *pts, const uint8_t *cats,
+                             const double *aux, uint8_t *pass, uint8_t *pre, double *f) {
+  lst_config cfg;
+  if (cfg_in) cfg = *cfg_in; else lst_default_config(&cfg);
+  Params g;
+  make_params(cfg, &g);
+  const int npts = level == LST_MD ? 2 : level == LST_LS ? 2 : level == LST_T3 ? 3 : level == LST_T5 ? 5 : 0;
+  if (!npts || !pts || !cats || !pass) return LST_EINVAL;
+  for (uint32_t i = 0; i < n; ++i) {
+    Pt P[5];
+    const float *p = pts + (size_t)i * npts * 3;
+    const uint8_t *ct = cats + (size_t)i * npts;
+    for (int k = 0; k < npts; ++k) P[k] = make_pt(p[3 * k], p[3 * k + 1], p[3 * k + 2], ct[k]);
+    double o3[3] = {0, 0, 0};
+    bool ok = false, pr = true;
+    if (level == LST_MD) {
+      MdOut o = {0, 0, 0};
+      ok = md_eval_d(g, P[0], P[1], ct[0], &o);
+      const float rl = sqrtf(p[0] * p[0] + p[1] * p[1]), ru = sqrtf(p[3] * p[3] + p[4] * p[4]);
+      pr = md_pre_f(g, p[0], p[1], p[2], rl, p[3], p[4], p[5], ru, ct[0]);
+      o3[0] = o.kappa; o3[1] = o.sigk; o3[2] = o.dphi;
+    } else if (level == LST_LS) {
+      const double *a = aux + 4 * (size_t)i;
+      LsOut o = {0, 0, 0};
+      ok = ls_eval_d(g, P[0], a[0], a[1], P[1], a[2], a[3], &o);
+      const float ri = sqrtf(p[0] * p[0] + p[1] * p[1]), ro = sqrtf(p[3] * p[3] + p[4] * p[4]);
+      pr = ls_pre_f(g, p[0], p[1], p[2], ri, (float)a[0], (float)a[1], ct[0], p[3], p[4], p[5], ro, (float)a[2],
+                    (float)a[3], ct[1]);
+      o3[0] = o.kappa; o3[1] = o.sigk; o3[2] = o.dphi;
+    } else if (level == LST_T3) {
+      T3Out o = {0, 0, 0};
+      ok = t3_eval_d(g, P[0], P[1], P[2], &o);
+      o3[0] = o.kappa3; o3[1] = o.sigk3; o3[2] = o.beta;
+    } else {
+      const double *a = aux + 4 * (size_t)i;
+      T5Out o = {0, 0, 0, 0, 0};
+      ok = t5_eval_d(g, P, a[0], a[1], a[2], a[3], &o);
+      o3[0] = o.R; o3[1] = o.chi2; o3[2] = o.eta;
+    }
+    pass[i] = ok;
+    if (pre) pre[i] = pr;
+    if (f) { f[3 * (size_t)i] = o3[0]; f[3 * (size_t)i + 1] = o3[1]; f[3 * (size_t)i + 2] = o3[2]; }
+  }
+  return LST_OK;
+}

@@ -1,0 +1,209 @@
+// lst_dev.cuh -- device-side data layout and the work-item machinery shared by all stage kernels.
+//
+// Every stage (MD, LS, T3, T5, pT5, pT3) is a join: rows x per-row candidate lists, grouped so
+// that one group's operands fit in shared memory.  A stage runs as
+//   groups  : per group g, rows R_g and candidates per row (uniform W_g, or a per-row list)
+//   emit    : one block scans the groups and writes fixed-size work ITEMS (<= 1024 candidates)
+//   eval    : persistent blocks, one item at a time: stage operands in shared memory, fp32
+//             pre-filter, compact survivors, fp64 decision, one pass BIT per candidate
+//   scan    : one block scans the per-item pass counts (exact sizes, no truncation)
+//   fill    : per item: ordered prefix over the bits, fp64 derived quantities, SoA stores
+// Output order is canonical (ascending item, ascending candidate) and no global atomics are used
+// for compaction (north_star: ballot/prefix-sum compaction, deterministic).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "lst_math.cuh"
+
+namespace lst {
+
+constexpr int kItemCand = 1024;          // candidates per work item
+constexpr int kItemWords = kItemCand / 32;
+constexpr int kThreads = 128;            // threads per block of eval / fill kernels
+constexpr int kRowChunk = 128;           // rows per group in the variable-width stages (T3, T5, pixel)
+constexpr int kMaxDeg = 512;             // maximum module-map degree (checked by lst_create)
+
+enum Stage { S_MD = 0, S_LS, S_T3, S_T5, S_PT5, S_PT3, S_NSTAGE };
+
+enum ErrBits {
+  ERR_DET = 1u << 0,        // det id out of range
+  ERR_CAP_ITEMS = 1u << 1,  // a work list overflowed
+  ERR_CAP_OBJ = 1u << 2     // an object array overflowed
+};
+
+struct Item {            // 16 bytes
+  uint32_t group;        // module (MD, LS) or row chunk (T3, T5, pixel)
+  uint32_t i0;           // first row (relative to the group's first row)
+  uint32_t j0;           // first candidate column
+  uint16_t nrows, nj;    // nrows * nj <= kItemCand
+};
+
+struct Header {          // per slot, device; zeroed (except n_hits / n_seeds) at the start of lst_run
+  uint32_t n_hits, n_seeds;
+  uint32_t n_obj[8];                 // indexed by lst_level
+  uint32_t n_items[S_NSTAGE];
+  uint32_t n_groups[S_NSTAGE];
+  uint32_t err;
+  uint32_t pad;
+  unsigned long long cand[S_NSTAGE]; // candidates enumerated per stage
+};
+
+struct StageBuf {        // work list of one stage
+  uint32_t *gR, *gW;     // [cap_groups] rows / width (or candidate count) per group
+  uint32_t *g_item0;     // [cap_groups+1] first item of a group
+  Item *items;           // [cap_items]
+  uint32_t *mask;        // [cap_items * kItemWords]
+  uint32_t *item_cnt;    // [cap_items] pass count
+  uint32_t *item_base;   // [cap_items] exclusive prefix
+  uint32_t cap_groups, cap_items;
+};
+
+// Static detector data (device), shared by all slots.
+struct GeoDev {
+  uint32_t n_modules, n_det;
+  const uint8_t *category, *layer;
+  const uint32_t *map_off, *map_cols;
+};
+
+// All per-slot arrays (device pointers into the caller's workspace).
+struct SlotDev {
+  Header *hdr;
+  // raw event
+  float *raw_x, *raw_y, *raw_z; uint32_t *raw_det;
+  float *seed_pt, *seed_eta, *seed_phi, *seed_z0; int8_t *seed_q; uint32_t *seed_ids;
+  // a0: hits grouped by det
+  uint32_t *det_cnt, *det_off, *det_cur;     // [n_det+1]
+  uint32_t *tmp_orig;                        // [cap_hits]
+  float4 *hit;                               // [cap_hits] x, y, z, rt
+  uint32_t *hit_orig;                        // [cap_hits] original caller index
+  // MD
+  float4 *md_pos;        // anchor (lower hit) x, y, z, rt
+  double2 *md_kd;        // kappa_MD, sigma_kappa_MD (fp64: they enter the LS decision)
+  float2 *md_kf;         // same, fp32 (pre-filter)
+  uint2 *md_hit;         // sorted positions of lower / upper hit
+  uint32_t *md_mod;      // module << 2 | category
+  float *md_dphi;
+  uint32_t *md_mod_off;  // [n_modules+1]
+  // LS
+  uint2 *ls_md;          // inner, outer MD
+  float4 *ls_f;          // dphi, kappa, sigma_kappa, 0
+  uint32_t *ls_md_off;   // [cap_md+1] LS range of an inner MD
+  // T3
+  uint4 *t3_md;          // md1, md2, md3, 0
+  uint2 *t3_ls;
+  double2 *t3_kd;        // kappa3, sigma_kappa3
+  float *t3_beta;
+  uint32_t *t3_md_off;   // [cap_md+1] T3 range of a first MD
+  // T5
+  uint32_t *t5_md;       // [5 * cap_t5]
+  uint2 *t5_t3;
+  double *t5_chi2;
+  double2 *t5_etaphi;
+  float4 *t5_f;          // R, chi2, k3a, k3b
+  float *t5_pt;
+  uint8_t *t5_keep;
+  // pixel-seeded
+  uint2 *pt5_po, *pt3_po;          // pls, obj
+  double *pt5_chi2, *pt3_chi2;
+  uint8_t *pt5_keep, *pt3_keep, *pls_keep;
+  // TC
+  uint2 *tc_to;                    // type, obj
+  float4 *tc_f;                    // pt, eta, phi, type
+  // work lists
+  StageBuf st[S_NSTAGE];
+  uint32_t cap_hits, cap_seeds, cap_md, cap_ls, cap_t3, cap_t5, cap_pt3, cap_pt5, cap_tc;
+  // export scratch
+  uint32_t *exp_hits, *exp_par; float *exp_f;
+};
+
+// ------------------------------------------------------------------ small device helpers
+__device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ uint32_t warp_excl_scan(uint32_t v, uint32_t *total) {
+  const int lane = threadIdx.x & 31;
+  uint32_t x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+    if (lane >= o) x += y;
+  }
+  *total = __shfl_sync(0xffffffffu, x, 31);
+  return x - v;
+}
+
+// Block-wide exclusive scan of one value per thread (blockDim.x <= 1024); sh: 33 words.
+__device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t *sh, uint32_t *total) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  uint32_t wt;
+  uint32_t e = warp_excl_scan(v, &wt);
+  __syncthreads();
+  if (lane == 0) sh[w] = wt;
+  __syncthreads();
+  if (w == 0) {
+    uint32_t t = lane < nw ? sh[lane] : 0, tt;
+    uint32_t ee = warp_excl_scan(t, &tt);
+    sh[lane] = ee;
+    if (lane == 0) sh[32] = tt;
+  }
+  __syncthreads();
+  e += sh[w];
+  *total = sh[32];
+  return e;
+}
+
+// Per-item compaction scratch (shared memory).
+struct ItemScratch {
+  uint32_t mask[kItemWords];
+  uint32_t pre[kItemWords + 1];
+  uint16_t list[kItemCand];
+  uint32_t n;
+};
+
+// eval phase 1 helper: append candidate c to the survivor list (warp-aggregated shared atomic).
+// Must be called by all 32 lanes of a warp (uniform loop trip count).
+__device__ __forceinline__ void push_survivor(ItemScratch &s, bool keep, uint32_t c) {
+  const uint32_t b = __ballot_sync(0xffffffffu, keep);
+  if (b == 0) return;
+  const int lane = threadIdx.x & 31;
+  const int leader = __ffs(b) - 1;
+  uint32_t base = 0;
+  if (lane == leader) base = atomicAdd(&s.n, (uint32_t)__popc(b));
+  base = __shfl_sync(0xffffffffu, base, leader);
+  if (keep) s.list[base + __popc(b & ((1u << lane) - 1u))] = (uint16_t)c;
+}
+
+// fill helper: ordered list of set bits of the item's mask.  Call with all threads; needs
+// kThreads >= kItemWords.  After return s.list[0..s.n) holds the candidates in ascending order.
+__device__ __forceinline__ void expand_mask(ItemScratch &s, const uint32_t *gmask) {
+  const int t = threadIdx.x;
+  if (t < 32) {
+    uint32_t w = gmask[t];
+    s.mask[t] = w;
+    uint32_t tot;
+    uint32_t e = warp_excl_scan((uint32_t)__popc(w), &tot);
+    s.pre[t] = e;
+    if (t == 0) { s.pre[kItemWords] = tot; s.n = tot; }
+  }
+  __syncthreads();
+  for (int c = t; c < kItemCand; c += blockDim.x) {
+    const uint32_t w = s.mask[c >> 5];
+    if ((w >> (c & 31)) & 1u) s.list[s.pre[c >> 5] + __popc(w & ((1u << (c & 31)) - 1u))] = (uint16_t)c;
+  }
+  __syncthreads();
+}
+
+// eval epilogue: publish the item's mask and pass count.
+__device__ __forceinline__ void publish_mask(const ItemScratch &s, uint32_t *gmask, uint32_t *gcnt) {
+  if (threadIdx.x < 32) {
+    const uint32_t w = s.mask[threadIdx.x];
+    gmask[threadIdx.x] = w;
+    const uint32_t tot = warp_sum((uint32_t)__popc(w));
+    if (threadIdx.x == 0) *gcnt = tot;
+  }
+}
+
+}  // namespace lst

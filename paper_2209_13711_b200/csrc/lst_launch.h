@@ -1,0 +1,36 @@
+// lst_launch.h -- host-side view of a context and the per-stage launch functions (one per .cu file).
+#pragma once
+#include "lst_dev.cuh"
+
+namespace lst {
+
+struct Ctx {             // what the launchers need from a context
+  GeoDev geo;
+  Params par;
+  int n_sm;
+  // per logical layer geometry bounds (pixel linking windows), host copies
+  float lay_rmin[16], lay_rmax[16], lay_zmin[16], lay_zmax[16];
+};
+
+// k_common.cu
+void launch_index(const Ctx &c, const SlotDev &s, cudaStream_t st);                       // 1 memset + 5 kernels
+void launch_emit(const Ctx &c, const SlotDev &s, int stage, int rows_level, cudaStream_t st);
+void launch_scan_items(const Ctx &c, const SlotDev &s, int stage, int level, uint32_t cap, cudaStream_t st);
+void launch_row_offsets(const Ctx &c, const SlotDev &s, int kind, cudaStream_t st);
+// k_mdls.cu
+void launch_md(const Ctx &c, const SlotDev &s, cudaStream_t st);
+void launch_ls(const Ctx &c, const SlotDev &s, cudaStream_t st);
+// k_t3t5.cu
+void launch_t3(const Ctx &c, const SlotDev &s, cudaStream_t st);
+void launch_t5(const Ctx &c, const SlotDev &s, cudaStream_t st);
+// k_pix.cu
+void launch_pixel(const Ctx &c, const SlotDev &s, cudaStream_t st);
+// k_dedup.cu
+void launch_dedup(const Ctx &c, const SlotDev &s, cudaStream_t st);
+// k_export.cu: gather one level into the export scratch (hit_idx, parents, f)
+void launch_export(const Ctx &c, const SlotDev &s, int level, cudaStream_t st);
+
+// number of kernel launches (memsets not counted) each launcher enqueues
+constexpr int kLaunchesIndex = 5;
+
+}  // namespace lst

@@ -1,0 +1,381 @@
+// lst_math.cuh -- per-candidate selection arithmetic of the CUDA path (DESIGN.md Readings C0-C6).
+//
+// Two flavours per object level:
+//   *_pre_f : fp32 conservative pre-filter.  It may only REJECT a candidate whose cut variable
+//             exceeds the threshold by more than PRE_SLACK (1e-3 relative), far outside the fp32
+//             evaluation error of the difference-first formulas; NaN never rejects.
+//   *_d     : fp64 decision on the fp32 inputs promoted before the first subtraction, and the
+//             derived quantities that are stored.  Every accepted object is decided here.
+// Functions are __host__ __device__ so that the host test hooks (lst_host_* in lst_api.cu) can run
+// the very same code on the CPU.  Nothing here is shared with oracle/.
+#pragma once
+#include <math.h>
+#include <stdint.h>
+
+#ifdef __CUDACC__
+#define LST_HD __host__ __device__ __forceinline__
+#else
+#define LST_HD inline
+#endif
+
+namespace lst {
+
+constexpr double kGuard = 1e-9;       // denominators must exceed this (C0)
+constexpr float kPreSlack = 1.001f;   // fp32 pre-filter loosening
+
+// Selection parameters in the form the kernels use (built once by lst_create from lst_config).
+struct Params {
+  double kmax;          // kB / (2 pt_min)
+  double kB, ns, z0max, d0max, chi2max, dr2max, ec_md_sys, modez_slack;
+  double seed_sig_phi, seed_sig_pt, seed_sig_z;
+  double sig_t[4], sig_z[4], sig_r[4];
+  float f_kmax, f_ns, f_z0max, f_ec_md_sys, f_modez_slack;
+  float f_sig_t[4], f_sig_z[4], f_sig_r[4];
+  int dup_t5, dup_pt5, dup_pt3, s0_enabled;
+  uint32_t start_mask;
+};
+
+LST_HD bool is_endcap(int cat) { return cat >= 2; }
+LST_HD double clamp1(double v) { return v > 1.0 ? 1.0 : (v < -1.0 ? -1.0 : v); }
+LST_HD double dmin(double a, double b) { return a < b ? a : b; }
+LST_HD double wrap_pi(double a) { return remainder(a, 6.283185307179586476925286766559); }
+
+struct Pt {  // a point promoted to double, with its transverse radius and module category
+  double x, y, z, rt;
+  int cat;
+};
+LST_HD Pt make_pt(float x, float y, float z, int cat) {
+  Pt p;
+  p.x = (double)x; p.y = (double)y; p.z = (double)z;
+  p.rt = sqrt(p.x * p.x + p.y * p.y);
+  p.cat = cat;
+  return p;
+}
+// C0 helpers (difference first)
+LST_HD double sd_of(const Pt &A, const Pt &B) {          // sin(dphi)
+  return (A.x * (B.y - A.y) - A.y * (B.x - A.x)) / (A.rt * B.rt);
+}
+LST_HD double dphi_of(const Pt &A, const Pt &B) {
+  return atan2(A.x * (B.y - A.y) - A.y * (B.x - A.x), A.x * B.x + A.y * B.y);
+}
+LST_HD double chord_of(const Pt &A, const Pt &B) { return hypot(B.x - A.x, B.y - A.y); }
+LST_HD double dr_of(const Pt &A, const Pt &B) {          // rt_B - rt_A without cancellation
+  double dx = B.x - A.x, dy = B.y - A.y;
+  return (2.0 * (A.x * dx + A.y * dy) + (dx * dx + dy * dy)) / (A.rt + B.rt);
+}
+LST_HD double kappa3_of(const Pt &A, const Pt &B, const Pt &C) {  // Menger curvature / 2
+  double abx = B.x - A.x, aby = B.y - A.y, bcx = C.x - B.x, bcy = C.y - B.y;
+  double acx = C.x - A.x, acy = C.y - A.y;
+  return (abx * bcy - aby * bcx) / (hypot(abx, aby) * hypot(bcx, bcy) * hypot(acx, acy));
+}
+LST_HD double arc_of(double r, double k) {               // arc length at radius r, half curvature k
+  if (fabs(k * r) <= 1e-4) return r;
+  return asin(clamp1(k * r)) / k;
+}
+// "v <= thr" with NaN failing
+LST_HD bool le(double v, double thr) { return v <= thr; }
+
+// ------------------------------------------------------------------ C1 mini-doublet
+struct MdOut { double kappa, sigk, dphi; };
+
+LST_HD bool md_eval_d(const Params &g, const Pt &l, const Pt &u, int cat, MdOut *o) {
+  if (!(l.rt > kGuard) || !(u.rt > kGuard)) return false;
+  const double dz = u.z - l.z;
+  const double sdv = sd_of(l, u), cxy = chord_of(l, u), drv = dr_of(l, u);
+  const double st = g.sig_t[cat];
+  const double inv = 1.0 / l.rt + 1.0 / u.rt;
+  const double tolphi = g.ns * st * inv;
+  bool ok = true;
+  double cpred;
+  if (!is_endcap(cat)) {
+    ok &= (drv > 0.0);                                                                         // B1
+    ok &= le(fabs(dz - l.z * drv / l.rt), g.z0max * drv / l.rt + 2.0 * g.ns * g.sig_z[cat]);
+    ok &= le(fabs(sdv), g.kmax * cxy + tolphi);                                                // B2
+    cpred = cxy;
+  } else {
+    const double azl = fabs(l.z);
+    if (!(azl > kGuard) || !(azl - g.z0max > kGuard)) return false;
+    ok &= le(fabs(drv - l.rt * dz / l.z),                                                      // E1
+             l.rt * fabs(dz) * g.z0max / (azl * (azl - g.z0max)) + 2.0 * g.ns * g.sig_r[cat]);
+    ok &= le(fabs(sdv), fabs(dz) * asin(dmin(1.0, g.kmax * l.rt)) / (azl - g.z0max) + tolphi);  // E2
+    cpred = fabs(dz) * l.rt / azl;
+  }
+  if (!(cpred > kGuard)) return false;
+  if (o) {
+    o->kappa = sdv / cpred;
+    o->sigk = st * inv / cpred;
+    o->dphi = asin(clamp1(sdv));
+  }
+  return ok;
+}
+
+// fp32 pre-filter: true = keep for the fp64 decision.  rt* are fp32 sqrt(x^2+y^2).
+LST_HD bool md_pre_f(const Params &g, float xl, float yl, float zl, float rl, float xu, float yu, float zu,
+                     float ru, int cat) {
+  const float dx = xu - xl, dy = yu - yl, dz = zu - zl;
+  const float dd = dx * dx + dy * dy;
+  const float drv = (2.0f * (xl * dx + yl * dy) + dd) / (rl + ru);
+  const float cr = xl * dy - yl * dx;
+  const float tolrr = g.f_ns * g.f_sig_t[cat] * (rl + ru);       // tolphi * rl * ru
+  const float rr = rl * ru;
+  if (!is_endcap(cat)) {
+    if (drv < -1e-3f) return false;
+    const float t = drv / rl;
+    if (fabsf(dz - zl * t) > (g.f_z0max * t + 2.0f * g.f_ns * g.f_sig_z[cat]) * kPreSlack + 1e-4f) return false;
+    if (fabsf(cr) > (g.f_kmax * sqrtf(dd) * rr + tolrr) * kPreSlack) return false;
+  } else {
+    const float azl = fabsf(zl);
+    const float den = azl - g.f_z0max;
+    if (den < 1e-3f) return true;  // let the fp64 guard decide
+    const float adz = fabsf(dz);
+    if (fabsf(drv - rl * dz / zl) > (rl * adz * g.f_z0max / (azl * den) + 2.0f * g.f_ns * g.f_sig_r[cat]) * kPreSlack + 1e-4f)
+      return false;
+    const float asl = asinf(fminf(1.0f, g.f_kmax * rl));
+    if (fabsf(cr) > (adz * asl / den * rr + tolrr) * kPreSlack) return false;
+  }
+  return true;
+}
+
+// ------------------------------------------------------------------ C3 line segment
+struct LsOut { double kappa, sigk, dphi; };
+
+// A, B: anchors of the inner / outer MD; (ki, ski), (ko, sko): their kappa_MD, sigma_kappa_MD.
+LST_HD bool ls_eval_d(const Params &g, const Pt &A, double ki, double ski, const Pt &B, double ko, double sko,
+                      LsOut *o) {
+  const int ci = A.cat, co = B.cat;
+  const bool modeZ = is_endcap(co);
+  const double ns = g.ns;
+  const double dz = B.z - A.z;
+  const double drv = dr_of(A, B), sdv = sd_of(A, B), cxy = chord_of(A, B), dph = dphi_of(A, B);
+  bool ok = true;
+  // L1 pointing
+  const double N = A.rt * dz - A.z * drv;
+  const double E = A.rt * g.sig_z[co] + B.rt * g.sig_z[ci] + fabs(B.z) * g.sig_r[ci] + fabs(A.z) * g.sig_r[co];
+  ok &= le(fabs(N), g.z0max * fabs(drv) + ns * E);
+  // L2 pT window
+  const double tphi = g.sig_t[ci] / A.rt + g.sig_t[co] / B.rt;
+  const double tolphi = ns * tphi;
+  ok &= (A.x * B.x + A.y * B.y > 0.0);
+  double kls, sigkls, slack;
+  if (!modeZ) {
+    if (!(cxy > kGuard)) return false;
+    ok &= le(fabs(sdv), g.kmax * cxy + tolphi);
+    kls = sdv / cxy;
+    sigkls = tphi / cxy;
+    slack = 0.0;
+  } else {
+    const double rbar = 0.5 * (A.rt + B.rt), zbar = 0.5 * (fabs(A.z) + fabs(B.z));
+    const double adz = fabs(dz);
+    if (!(adz > kGuard) || !(rbar > kGuard)) return false;
+    const double Sbar = asin(dmin(1.0, g.kmax * (rbar + ns * (g.sig_r[ci] + g.sig_r[co]) / 2.0))) / g.kmax;
+    const double den = zbar - g.z0max - ns * g.sig_z[ci] / 2.0;
+    if (!(den > kGuard)) return false;
+    ok &= le(fabs(dph), g.kmax * (adz + ns * g.sig_z[ci]) * Sbar / den + tolphi);
+    const double lever = zbar / (adz * rbar);
+    kls = dph * lever;
+    sigkls = tphi * lever;
+    slack = fabs(kls) * (g.z0max / zbar + g.modez_slack + ns * (g.sig_r[ci] + g.sig_r[co]) / (A.rt + B.rt) +
+                         ns * g.sig_z[ci] / adz);
+  }
+  // L3 stub-segment curvature consistency
+  ok &= le(fabs(ki - kls), ns * (ski + sigkls) + slack + (is_endcap(ci) ? g.ec_md_sys * fabs(kls) : 0.0));
+  ok &= le(fabs(ko - kls), ns * (sko + sigkls) + slack + (is_endcap(co) ? g.ec_md_sys * fabs(kls) : 0.0));
+  if (o) { o->kappa = kls; o->sigk = sigkls; o->dphi = dph; }
+  return ok;
+}
+
+LST_HD bool ls_pre_f(const Params &g, float xi, float yi, float zi, float ri, float ki, float ski, int ci,
+                     float xo, float yo, float zo, float ro, float ko, float sko, int co) {
+  const float dx = xo - xi, dy = yo - yi, dz = zo - zi;
+  const float dd = dx * dx + dy * dy;
+  const float dotAD = xi * dx + yi * dy;
+  const float drv = (2.0f * dotAD + dd) / (ri + ro);
+  const float ns = g.f_ns;
+  // L1
+  const float N = ri * dz - zi * drv;
+  const float E = ri * g.f_sig_z[co] + ro * g.f_sig_z[ci] + fabsf(zo) * g.f_sig_r[ci] + fabsf(zi) * g.f_sig_r[co];
+  if (fabsf(N) > (g.f_z0max * fabsf(drv) + ns * E) * kPreSlack) return false;
+  const float rr = ri * ro;
+  const float dotAB = ri * ri + dotAD;
+  if (dotAB < -1e-3f * rr) return false;
+  const float cr = xi * dy - yi * dx;
+  const float sd = cr / rr;
+  const float tphi = g.f_sig_t[ci] / ri + g.f_sig_t[co] / ro;
+  const float eci = is_endcap(ci) ? g.f_ec_md_sys : 0.0f, eco = is_endcap(co) ? g.f_ec_md_sys : 0.0f;
+  if (!is_endcap(co)) {
+    const float cxy = sqrtf(dd);
+    const float asd = fabsf(sd);
+    if (asd > (g.f_kmax * cxy + ns * tphi) * kPreSlack) return false;
+    // L3 multiplied through by cxy
+    if (fabsf(ki * cxy - sd) > (ns * (ski * cxy + tphi) + eci * asd) * kPreSlack) return false;
+    if (fabsf(ko * cxy - sd) > (ns * (sko * cxy + tphi) + eco * asd) * kPreSlack) return false;
+  } else {
+    const float rbar = 0.5f * (ri + ro), zbar = 0.5f * (fabsf(zi) + fabsf(zo));
+    const float adz = fabsf(dz);
+    const float den = zbar - g.f_z0max - 0.5f * ns * g.f_sig_z[ci];
+    if (den < 1e-3f || adz < 1e-6f) return true;   // guards are decided in fp64
+    const float srs = g.f_sig_r[ci] + g.f_sig_r[co];
+    const float Sbar = asinf(fminf(1.0f, g.f_kmax * (rbar + 0.5f * ns * srs))) / g.f_kmax;
+    const float dph = atan2f(cr, dotAB);
+    if (fabsf(dph) > (g.f_kmax * (adz + ns * g.f_sig_z[ci]) * Sbar / den + ns * tphi) * kPreSlack) return false;
+    const float lever = zbar / (adz * rbar);
+    const float kls = dph * lever, akls = fabsf(kls);
+    const float sigkls = tphi * lever;
+    const float slack = akls * (g.f_z0max / zbar + g.f_modez_slack + ns * srs / (ri + ro) + ns * g.f_sig_z[ci] / adz);
+    if (fabsf(ki - kls) > (ns * (ski + sigkls) + slack + eci * akls) * kPreSlack) return false;
+    if (fabsf(ko - kls) > (ns * (sko + sigkls) + slack + eco * akls) * kPreSlack) return false;
+  }
+  return true;
+}
+
+// ------------------------------------------------------------------ C4 triplet
+struct T3Out { double kappa3, sigk3, beta; };
+
+LST_HD double sig_perp(const Params &g, const Pt &h) {
+  return g.sig_t[h.cat] + g.sig_r[h.cat] * dmin(1.0, g.kmax * h.rt);
+}
+
+LST_HD bool t3_eval_d(const Params &g, const Pt &P1, const Pt &P2, const Pt &P3, T3Out *o) {
+  const double ns = g.ns;
+  const bool modeZ = is_endcap(P1.cat) || is_endcap(P2.cat) || is_endcap(P3.cat);
+  const double d12x = P2.x - P1.x, d12y = P2.y - P1.y, d23x = P3.x - P2.x, d23y = P3.y - P2.y;
+  const double a = hypot(d12x, d12y), b = hypot(d23x, d23y), c13 = chord_of(P1, P3);
+  if (!(a > kGuard) || !(b > kGuard) || !(c13 > kGuard)) return false;
+  bool ok = true;
+  // T3-1 relative angle
+  const double crs = d12x * d23y - d12y * d23x;
+  const double k3 = crs / (a * b * c13);
+  const double sk3 = (sig_perp(g, P2) + (b * sig_perp(g, P1) + a * sig_perp(g, P3)) / c13) / (a * b);
+  ok &= le(fabs(k3), g.kmax + ns * sk3);
+  // T3-2 phi-lever linearity
+  const double d12 = dphi_of(P1, P2), d23 = dphi_of(P2, P3), d13 = d12 + d23;
+  const double k13 = sin(d13) / c13;
+  double L1, L2, L3, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+  if (modeZ) {
+    L1 = P1.z; L2 = P2.z; L3 = P3.z;
+    s1 = g.sig_z[P1.cat]; s2 = g.sig_z[P2.cat]; s3 = g.sig_z[P3.cat];
+  } else {
+    L1 = arc_of(P1.rt, k13); L2 = arc_of(P2.rt, k13); L3 = arc_of(P3.rt, k13);
+  }
+  const double i1 = 1.0 / P1.rt, i2 = 1.0 / P2.rt, i3 = 1.0 / P3.rt;
+  const double Nphi = d12 * (L3 - L2) - d23 * (L2 - L1);
+  const double Nrho = (i2 - i1) * (L3 - L2) - (i3 - i2) * (L2 - L1);
+  const double Ephi = g.sig_t[P1.cat] * i1 * fabs(L3 - L2) + g.sig_t[P2.cat] * i2 * fabs(L3 - L1) +
+                      g.sig_t[P3.cat] * i3 * fabs(L2 - L1) + s1 * fabs(d23) + s2 * fabs(d13) + s3 * fabs(d12);
+  ok &= le(fabs(Nphi), g.d0max * fabs(Nrho) + ns * Ephi);
+  // T3-3 r-z collinearity
+  const double q1 = k3 * P1.rt, q2 = k3 * P2.rt, q3 = k3 * P3.rt;
+  const double a1 = P1.rt * (1.0 + q1 * q1 / 6.0), a2 = P2.rt * (1.0 + q2 * q2 / 6.0), a3 = P3.rt * (1.0 + q3 * q3 / 6.0);
+  const double Nz = (a2 - a1) * (P3.z - P1.z) - (a3 - a1) * (P2.z - P1.z);
+  const double Ez = g.sig_z[P3.cat] * fabs(a2 - a1) + g.sig_z[P2.cat] * fabs(a3 - a1) + g.sig_z[P1.cat] * fabs(a3 - a2) +
+                    g.sig_r[P2.cat] * fabs(P3.z - P1.z) + g.sig_r[P3.cat] * fabs(P2.z - P1.z) +
+                    g.sig_r[P1.cat] * fabs(P3.z - P2.z);
+  ok &= le(fabs(Nz), ns * Ez);
+  if (o) {
+    o->kappa3 = k3; o->sigk3 = sk3;
+    o->beta = atan2(crs, d12x * d23x + d12y * d23y);
+  }
+  return ok;
+}
+
+// ------------------------------------------------------------------ C5 quintuplet
+struct T5Out { double R, chi2, pt, eta, phi; };
+
+// Weighted Kasa circle fit of 5 points; kc = |kappa3(P1,P3,P5)|.
+LST_HD bool kasa_fit_d(const Params &g, const Pt *P, double kc, double *R, double *chi2) {
+  double w[5], sw = 0.0, mx = 0.0, my = 0.0;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const double st = g.sig_t[P[k].cat], sr = g.sig_r[P[k].cat] * dmin(1.0, kc * P[k].rt);
+    w[k] = 1.0 / (st * st + sr * sr);
+    sw += w[k]; mx += w[k] * P[k].x; my += w[k] * P[k].y;
+  }
+  mx /= sw; my /= sw;
+  double u[5], v[5], Suu = 0, Suv = 0, Svv = 0, Suz = 0, Svz = 0, Sz = 0;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    u[k] = P[k].x - mx; v[k] = P[k].y - my;
+    const double zeta = u[k] * u[k] + v[k] * v[k];
+    Suu += w[k] * u[k] * u[k]; Suv += w[k] * u[k] * v[k]; Svv += w[k] * v[k] * v[k];
+    Suz += w[k] * u[k] * zeta; Svz += w[k] * v[k] * zeta; Sz += w[k] * zeta;
+  }
+  const double det = Suu * Svv - Suv * Suv;
+  if (!(det > 0.0)) return false;
+  const double Bc = (-Suz * Svv + Svz * Suv) / det;
+  const double Cc = (-Svz * Suu + Suz * Suv) / det;
+  const double cx = -Bc / 2.0, cy = -Cc / 2.0;
+  const double R2 = (Bc * Bc + Cc * Cc) / 4.0 + Sz / sw;
+  if (!(R2 > 0.0)) return false;
+  const double Rr = sqrt(R2);
+  double x2 = 0.0;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const double e = hypot(u[k] - cx, v[k] - cy) - Rr;
+    x2 += w[k] * e * e;
+  }
+  *R = Rr; *chi2 = x2;
+  return true;
+}
+
+// P[0..4]: anchors; (k3a, sk3a), (k3b, sk3b): stored kappa3 / sigma of T3 (1,2,3) and (3,4,5).
+LST_HD bool t5_eval_d(const Params &g, const Pt *P, double k3a, double sk3a, double k3b, double sk3b, T5Out *o) {
+  if (!le(fabs(k3a - k3b), g.ns * (sk3a + sk3b))) return false;              // T5-1 radius match
+  if (!t3_eval_d(g, P[1], P[2], P[3], nullptr)) return false;               // T5-2 middle triplet
+  if (!(chord_of(P[0], P[2]) > kGuard) || !(chord_of(P[2], P[4]) > kGuard) || !(chord_of(P[0], P[4]) > kGuard))
+    return false;
+  const double k135 = kappa3_of(P[0], P[2], P[4]);
+  double R = 0.0, chi2 = 0.0;
+  if (!kasa_fit_d(g, P, fabs(k135), &R, &chi2)) return false;                // T5-3 circle fit
+  if (!le(chi2, g.chi2max)) return false;
+  const double k5 = (k135 > 0.0 ? 1.0 : (k135 < 0.0 ? -1.0 : 0.0)) / (2.0 * R);
+  const double den = arc_of(P[4].rt, k5) - arc_of(P[0].rt, k5);
+  if (!(den > kGuard)) return false;
+  if (o) {
+    o->R = R; o->chi2 = chi2;
+    o->pt = g.kB * R;
+    o->phi = wrap_pi(atan2(P[0].y, P[0].x) - asin(clamp1(k5 * P[0].rt)));
+    o->eta = asinh((P[4].z - P[0].z) / den);
+  }
+  return true;
+}
+
+// ------------------------------------------------------------------ C6 pixel linking
+struct Seed { double pt, eta, phi, z0; int q; };
+
+// All n anchors of an OT object against one pixel seed.  first_layer = logical layer of the first MD.
+LST_HD bool px_eval_d(const Params &g, const Seed &s, const Pt *P, int n, int first_layer, double *chi2) {
+  if (!((g.start_mask >> first_layer) & 1u)) return false;
+  if (!(s.pt > kGuard)) return false;
+  const double kp = -(double)s.q * g.kB / (2.0 * s.pt);
+  const double sh = sinh(s.eta);
+  double sum = 0.0;
+  for (int k = 0; k < n; ++k) {
+    const Pt &h = P[k];
+    const bool ec = is_endcap(h.cat);
+    double al;
+    if (!ec) al = arc_of(h.rt, kp);
+    else {
+      if (!(fabs(sh) > kGuard)) return false;
+      al = (h.z - s.z0) / sh;
+    }
+    if (!(al > 0.0)) return false;
+    const double dph = wrap_pi(atan2(h.y, h.x) - (s.phi + kp * al));
+    const double sphi = g.seed_sig_phi + g.seed_sig_pt * fabs(kp) * al + g.sig_t[h.cat] / h.rt;
+    double dzt, szt;
+    if (!ec) {
+      dzt = h.z - (s.z0 + sh * al);
+      szt = g.seed_sig_z + g.sig_z[h.cat];
+    } else {
+      const double rp = (fabs(kp * al) <= 1e-4) ? al : sin(kp * al) / kp;
+      dzt = h.rt - rp;
+      szt = g.seed_sig_z / fabs(sh) + g.sig_r[h.cat];
+    }
+    if (!le(fabs(dph), g.ns * sphi)) return false;
+    if (!le(fabs(dzt), g.ns * szt)) return false;
+    sum += (dph / sphi) * (dph / sphi) + (dzt / szt) * (dzt / szt);
+  }
+  *chi2 = sum / (2.0 * n);
+  return true;
+}
+
+}  // namespace lst

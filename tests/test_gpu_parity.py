@@ -1,0 +1,194 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, level by level, on
+the same seeded synthetic events (BASELINE.json configs 1-5).
+
+Bar (north_star): object sets (sorted hit-index tuples) identical at every level, except objects
+whose cut variable lies within 1e-5 relative of a threshold - those are counted and must stay
+below 1e-4 of the objects; derived floats within 1e-4 relative (absolute 1e-9 where the value
+itself is below 1e-6).
+"""
+import numpy as np
+import pytest
+
+import lstgen
+from oracle import lst_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+REL, ABS_TINY = 1e-4, 1e-9
+BAND, MAX_NEAR_FRAC = 1e-5, 1e-4
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2209_13711_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _gpu(B, geom, mp, ev, upto_tc=True, **kw):
+    lst = B.LST(geom, mp[0], mp[1], n_slots=1, max_hits=max(ev.n_hits, 1), max_seeds=max(ev.n_seeds, 1), **kw)
+    seeds = None
+    if ev.n_seeds:
+        seeds = (ev.seed_pt, ev.seed_eta, ev.seed_phi, ev.seed_z0, ev.seed_q, ev.seed_hit_ids)
+    lst.lst_load_event(0, ev.x, ev.y, ev.z, ev.det, seeds)
+    lst.lst_run(0)
+    return lst
+
+
+def _oracle(geom, mp, ev, upto):
+    o = O.Oracle(geom, mp[0], mp[1])
+    o.load(ev)
+    o.run(upto=upto)
+    return o
+
+
+def _keys(level, obj):
+    """Identity of an object: hit tuple (+ pLS for pixel-seeded levels)."""
+    h = obj["hits"].astype(np.int64)
+    if level in (O.PT3, O.PT5):
+        h = np.concatenate([obj["parents"][:, :1].astype(np.int64), h], 1)
+    return [tuple(r) for r in h.tolist()]
+
+
+def compare_level(o, lst, level, check_floats=True):
+    ref, got = o.get(level), lst.lst_get_objects(0, level)
+    kr, kg = _keys(level, ref), _keys(level, got)
+    sr, sg = set(kr), set(kg)
+    assert len(sr) == len(kr) and len(sg) == len(kg), "duplicate objects in a collection"
+    near = 0
+    for t in sr ^ sg:
+        seed = t[0] if level in (O.PT3, O.PT5) else 0
+        hits = t[1:] if level in (O.PT3, O.PT5) else t
+        _, margin = o.eval(level, hits, seed)
+        assert margin < BAND, "level %s: object %s differs with oracle margin %.3g" % (O.LEVEL_NAMES[level], t, margin)
+        near += 1
+    n = max(len(sr), 1)
+    assert near <= max(MAX_NEAR_FRAC * n, 0.0) or near == 0, "too many near-threshold differences: %d of %d" % (near, n)
+    if check_floats and sr:
+        ir = {t: i for i, t in enumerate(kr)}
+        common = [t for t in kg if t in ir]
+        a = ref["f"][[ir[t] for t in common]]
+        ig = {t: i for i, t in enumerate(kg)}
+        b = got["f"][[ig[t] for t in common]].astype(np.float64)
+        ncol = {O.MD: 3, O.LS: 3, O.T3: 3, O.T5: 4, O.PT3: 1, O.PT5: 1}[level]
+        for c in range(ncol):
+            x, y = a[:, c], b[:, c]
+            tiny = np.abs(x) < 1e-6
+            assert np.all(np.abs(x - y)[tiny] <= ABS_TINY + 1e-7 * np.abs(x[tiny])), (O.LEVEL_NAMES[level], c)
+            rel = np.abs(x - y)[~tiny] / np.abs(x[~tiny])
+            assert rel.size == 0 or rel.max() <= REL, (O.LEVEL_NAMES[level], c, rel.max())
+    return len(sr), near, ref, got
+
+
+CHAIN = (O.MD, O.LS, O.T3, O.T5)
+
+
+@pytest.mark.parametrize("cfg", ["cfg1", "cfg2"])
+def test_barrel_configs_chain(B, geom_barrel, map_barrel, cfg):
+    ev = lstgen.make_event(geom_barrel, cfg)
+    o = _oracle(geom_barrel, map_barrel, ev, O.T5)
+    lst = _gpu(B, geom_barrel, map_barrel, ev)
+    cnt, cand = lst.lst_get_counts(0)
+    for lvl in CHAIN:
+        n, near, ref, got = compare_level(o, lst, lvl)
+        assert n == o.count(lvl) and n > 0
+        assert cnt[lvl] == len(got["hits"])
+        # canonical order: the CUDA path emits objects in the oracle's order (ascending module, rows, columns)
+        if near == 0:
+            assert np.array_equal(ref["hits"], got["hits"])
+            assert np.array_equal(ref["parents"], got["parents"])
+    lst.close()
+
+
+@pytest.mark.parametrize("cfg", ["cfg3", "cfg3h"])
+def test_full_detector_chain(B, geom_full, map_full, cfg):
+    ev = lstgen.make_event(geom_full, cfg)
+    o = _oracle(geom_full, map_full, ev, O.T5)
+    lst = _gpu(B, geom_full, map_full, ev)
+    total = 0
+    for lvl in CHAIN:
+        n, near, ref, got = compare_level(o, lst, lvl)
+        assert n == o.count(lvl) and n > 1000
+        total += n
+        if near == 0:
+            assert np.array_equal(ref["hits"], got["hits"])
+    cnt, cand = lst.lst_get_counts(0)
+    assert cand[1] > 1e6    # the LS candidate loop is the dominant one
+    lst.close()
+
+
+def test_empty_and_tiny_events(B, geom_barrel, map_barrel):
+    import dataclasses
+    ev = lstgen.make_event(geom_barrel, "cfg1")
+    empty = dataclasses.replace(ev, x=ev.x[:0], y=ev.y[:0], z=ev.z[:0], det=ev.det[:0], pid=ev.pid[:0])
+    lst = B.LST(geom_barrel, map_barrel[0], map_barrel[1], max_hits=1024, max_seeds=16)
+    lst.lst_load_event(0, empty.x, empty.y, empty.z, empty.det)
+    lst.lst_run(0)
+    cnt, _ = lst.lst_get_counts(0)
+    assert cnt.sum() == 0
+    for lvl in range(7):
+        assert len(lst.lst_get_objects(0, lvl)["hits"]) == 0
+    # one hit only; then the same slot re-used for a real event (state fully reset)
+    lst.lst_load_event(0, ev.x[:1], ev.y[:1], ev.z[:1], ev.det[:1])
+    lst.lst_run(0)
+    assert lst.lst_get_counts(0)[0].sum() == 0
+    lst.lst_load_event(0, ev.x, ev.y, ev.z, ev.det)
+    lst.lst_run(0)
+    o = _oracle(geom_barrel, map_barrel, ev, O.T5)
+    for lvl in CHAIN:
+        compare_level(o, lst, lvl)
+    lst.close()
+
+
+def test_errors(B, geom_barrel, map_barrel):
+    ev = lstgen.make_event(geom_barrel, "cfg1")
+    lst = B.LST(geom_barrel, map_barrel[0], map_barrel[1], max_hits=64, max_seeds=4)
+    with pytest.raises(B.LstError) as e:      # more hits than max_hits
+        lst.lst_load_event(0, ev.x, ev.y, ev.z, ev.det)
+    assert e.value.status == B.LST_EINVAL
+    with pytest.raises(B.LstError) as e:      # run before load
+        lst.lst_run(0)
+    assert e.value.status == B.LST_ESTATE
+    bad = ev.det[:32].copy()
+    bad[3] = 2 * geom_barrel.n_modules + 7    # det out of range -> reported at get
+    lst.lst_load_event(0, ev.x[:32], ev.y[:32], ev.z[:32], bad)
+    lst.lst_run(0)
+    with pytest.raises(B.LstError) as e:
+        lst.lst_get_counts(0)
+    assert e.value.status == B.LST_EINVAL
+    lst.close()
+    # capacity overflow is reported, never silent
+    cfg = B.lst_default_config()
+    cfg.cap_ls_per_hit = 0.001
+    ev2 = lstgen.make_event(geom_barrel, "cfg2")
+    lst = B.LST(geom_barrel, map_barrel[0], map_barrel[1], cfg=cfg, max_hits=ev2.n_hits, max_seeds=4)
+    lst.lst_load_event(0, ev2.x, ev2.y, ev2.z, ev2.det)
+    lst.lst_run(0)
+    with pytest.raises(B.LstError) as e:
+        lst.lst_get_counts(0)
+    assert e.value.status == B.LST_ENOMEM
+    lst.close()
+
+
+def test_device_resident_input_and_graph_replay(B, geom_barrel, map_barrel):
+    """on_device = 1 inputs; the same slot run repeatedly (graph replay) and without graphs."""
+    import torch
+    ev = lstgen.make_event(geom_barrel, "cfg2")
+    o = _oracle(geom_barrel, map_barrel, ev, O.T5)
+    for use_graph in (1, 0):
+        cfg = B.lst_default_config()
+        cfg.use_cuda_graph = use_graph
+        lst = B.LST(geom_barrel, map_barrel[0], map_barrel[1], cfg=cfg, max_hits=ev.n_hits, max_seeds=4)
+        dx, dy, dz = (torch.from_numpy(a).cuda() for a in (ev.x, ev.y, ev.z))
+        dd = torch.from_numpy(ev.det.astype(np.int64)).to(torch.int32).cuda()   # same bits as uint32
+        st = torch.cuda.Stream()
+        for rep in range(3):
+            with torch.cuda.stream(st):
+                lst.lst_load_event(0, dx, dy, dz, dd, stream=st)
+                lst.lst_run(0, stream=st)
+            for lvl in CHAIN:
+                compare_level(o, lst, lvl)
+        lst.close()
