@@ -58,6 +58,9 @@ CONFIGS = {
                  f_sec=0.0, noise=0.0, seeds=False, seed=1),
     "cfg2": dict(barrel_only=True, n=500, spectrum=True, pt_range=None, eta_max=0.8,
                  f_sec=0.0, noise=0.01, seeds=False, seed=2),
+    # config 2 with pixel seeds: small enough for the oracle's all-pairs (brute) linking and cleaning
+    "cfg2s": dict(barrel_only=True, n=500, spectrum=True, pt_range=None, eta_max=0.8,
+                  f_sec=0.0, noise=0.01, seeds=True, seed=22),
     "cfg3": dict(barrel_only=False, n=6000, spectrum=True, pt_range=None, eta_max=2.4,
                  f_sec=0.15, noise=0.02, seeds=False, seed=3),
     "cfg3h": dict(barrel_only=False, n=13500, spectrum=True, pt_range=None, eta_max=2.4,

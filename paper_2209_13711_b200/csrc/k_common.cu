@@ -10,7 +10,7 @@ __global__ void k_begin(SlotDev s) {
   const int t = threadIdx.x;
   if (t < 8) h->n_obj[t] = 0;
   if (t < S_NSTAGE) { h->n_items[t] = 0; h->n_groups[t] = 0; h->cand[t] = 0ull; }
-  if (t == 0) { h->err = 0; h->pad = 0; }
+  if (t == 0) { h->err = 0; h->pad = 0; h->n_dd = 0; h->n_flag = 0; s.scan_part[kScanBlocks + 1] = 0; }
 }
 
 // ------------------------------------------------------------------ a0.1 histogram of det ids
@@ -186,7 +186,8 @@ __global__ void k_scan_items(SlotDev s, int stage, int level, uint32_t cap) {
 
 // ------------------------------------------------------------------ row offsets from sorted row keys
 // off[r] = first object whose row key >= r, r in [0, n_rows]; keys ascending.
-// KIND 0: MD -> module (n_rows = n_modules); 1: LS -> inner MD; 2: T3 -> first MD (n_rows = n_md)
+// KIND 0: MD -> module (n_rows = n_modules); 1: LS -> inner MD; 2: T3 -> first MD; 3: T5 -> first MD
+// (n_rows = n_md); 4: pT5 -> seed; 5: pT3 -> seed (n_rows = n_seeds)
 template <int KIND>
 __global__ void k_row_offsets(GeoDev geo, SlotDev s) {
   const Header *hdr = s.hdr;
@@ -194,7 +195,10 @@ __global__ void k_row_offsets(GeoDev geo, SlotDev s) {
   uint32_t *off;
   if (KIND == 0) { n = hdr->n_obj[0]; n_rows = geo.n_modules; off = s.md_mod_off; }
   else if (KIND == 1) { n = hdr->n_obj[1]; n_rows = hdr->n_obj[0]; off = s.ls_md_off; }
-  else { n = hdr->n_obj[2]; n_rows = hdr->n_obj[0]; off = s.t3_md_off; }
+  else if (KIND == 2) { n = hdr->n_obj[2]; n_rows = hdr->n_obj[0]; off = s.t3_md_off; }
+  else if (KIND == 3) { n = hdr->n_obj[3]; n_rows = hdr->n_obj[0]; off = s.t5_md_off; }
+  else if (KIND == 4) { n = hdr->n_obj[5]; n_rows = hdr->n_seeds; off = s.pt5_pls_off; }
+  else { n = hdr->n_obj[4]; n_rows = hdr->n_seeds; off = s.pt3_pls_off; }
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nt = gridDim.x * blockDim.x;
   if (n == 0) {
     for (uint32_t r = tid; r <= n_rows; r += nt) off[r] = 0;
@@ -204,7 +208,10 @@ __global__ void k_row_offsets(GeoDev geo, SlotDev s) {
     uint32_t key, prev;
     if (KIND == 0) { key = s.md_mod[k] >> 2; prev = k ? (s.md_mod[k - 1] >> 2) + 1 : 0; }
     else if (KIND == 1) { key = s.ls_md[k].x; prev = k ? s.ls_md[k - 1].x + 1 : 0; }
-    else { key = s.t3_md[k].x; prev = k ? s.t3_md[k - 1].x + 1 : 0; }
+    else if (KIND == 2) { key = s.t3_md[k].x; prev = k ? s.t3_md[k - 1].x + 1 : 0; }
+    else if (KIND == 3) { key = s.t5_md[5 * (size_t)k]; prev = k ? s.t5_md[5 * (size_t)(k - 1)] + 1 : 0; }
+    else if (KIND == 4) { key = s.pt5_po[k].x; prev = k ? s.pt5_po[k - 1].x + 1 : 0; }
+    else { key = s.pt3_po[k].x; prev = k ? s.pt3_po[k - 1].x + 1 : 0; }
     for (uint32_t r = prev; r <= key; ++r) off[r] = k;
     if (k == n - 1) for (uint32_t r = key + 1; r <= n_rows; ++r) off[r] = n;
   }
@@ -237,11 +244,68 @@ void launch_scan_items(const Ctx &c, const SlotDev &s, int stage, int level, uin
   k_scan_items<<<1, 1024, 0, st>>>(s, stage, level, cap);
 }
 void launch_row_offsets(const Ctx &c, const SlotDev &s, int kind, cudaStream_t st) {
-  const uint32_t cap = kind == 0 ? s.cap_md : (kind == 1 ? s.cap_ls : s.cap_t3);
-  const int g = grid_for(cap, 256, c.n_sm * 4);
-  if (kind == 0) k_row_offsets<0><<<g, 256, 0, st>>>(c.geo, s);
-  else if (kind == 1) k_row_offsets<1><<<g, 256, 0, st>>>(c.geo, s);
-  else k_row_offsets<2><<<g, 256, 0, st>>>(c.geo, s);
+  const uint32_t caps[6] = {s.cap_md, s.cap_ls, s.cap_t3, s.cap_t5, s.cap_pt5, s.cap_pt3};
+  const int g = grid_for(caps[kind], 256, c.n_sm * 4);
+  switch (kind) {
+    case 0: k_row_offsets<0><<<g, 256, 0, st>>>(c.geo, s); break;
+    case 1: k_row_offsets<1><<<g, 256, 0, st>>>(c.geo, s); break;
+    case 2: k_row_offsets<2><<<g, 256, 0, st>>>(c.geo, s); break;
+    case 3: k_row_offsets<3><<<g, 256, 0, st>>>(c.geo, s); break;
+    case 4: k_row_offsets<4><<<g, 256, 0, st>>>(c.geo, s); break;
+    default: k_row_offsets<5><<<g, 256, 0, st>>>(c.geo, s); break;
+  }
+}
+
+// ------------------------------------------------------------------ device-wide exclusive scan
+// out[0..n) = exclusive prefix of in[0..n), out[n] = total; n = *n_ptr (a Header field).  Two
+// launches of kScanBlocks blocks: per-block sums (the last block to finish scans them), then the
+// per-block scan with its carry.  in == out is allowed.  part: kScanBlocks + 2 words, last = ticket.
+__global__ void __launch_bounds__(kScanThreads) k_scan_sums(const uint32_t *in, const uint32_t *n_ptr, uint32_t *part) {
+  __shared__ uint32_t sh[33];
+  __shared__ bool last;
+  const uint32_t n = *n_ptr;
+  const uint32_t chunk = (n + gridDim.x - 1) / gridDim.x;
+  const uint32_t b0 = min(n, blockIdx.x * chunk), b1 = min(n, b0 + chunk);
+  uint32_t sum = 0;
+  for (uint32_t i = b0 + threadIdx.x; i < b1; i += blockDim.x) sum += in[i];
+  uint32_t tot;
+  block_excl_scan(sum, sh, &tot);
+  if (threadIdx.x == 0) {
+    part[blockIdx.x] = tot;
+    __threadfence();
+    last = atomicAdd(&part[kScanBlocks + 1], 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  const uint32_t v = threadIdx.x < gridDim.x ? __ldcg(&part[threadIdx.x]) : 0u;
+  const uint32_t e = block_excl_scan(v, sh, &tot);
+  if (threadIdx.x < gridDim.x) part[threadIdx.x] = e;
+  if (threadIdx.x == 0) { part[kScanBlocks] = tot; part[kScanBlocks + 1] = 0; }
+}
+__global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t *in, const uint32_t *n_ptr, const uint32_t *part,
+                                                             uint32_t *out) {
+  __shared__ uint32_t sh[33];
+  const uint32_t n = *n_ptr;
+  const uint32_t chunk = (n + gridDim.x - 1) / gridDim.x;
+  const uint32_t b0 = min(n, blockIdx.x * chunk), b1 = min(n, b0 + chunk);
+  uint32_t carry = part[blockIdx.x];
+  for (uint32_t base = b0; base < b1; base += blockDim.x) {
+    const uint32_t i = base + threadIdx.x;
+    const uint32_t v = i < b1 ? in[i] : 0u;
+    uint32_t tot;
+    const uint32_t e = block_excl_scan(v, sh, &tot);
+    if (i < b1) out[i] = carry + e;
+    carry += tot;
+    __syncthreads();
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = part[kScanBlocks];
+}
+void launch_scan(const Ctx &c, const SlotDev &s, const uint32_t *in, uint32_t *out, const uint32_t *n_ptr,
+                 cudaStream_t st) {
+  (void)c;
+  k_scan_sums<<<kScanBlocks, kScanThreads, 0, st>>>(in, n_ptr, s.scan_part);
+  k_scan_apply<<<kScanBlocks, kScanThreads, 0, st>>>(in, n_ptr, s.scan_part, out);
 }
 
 }  // namespace lst

@@ -1,6 +1,370 @@
-// k_dedup.cu -- a6 duplicate removal and track candidates (reading C7).
+// k_dedup.cu -- a6 duplicate removal and track candidates (reading C7, steps S0-S4).
+//
+// Every rule is non-greedy ("a is removed iff SOME b of the named set satisfies the condition"), so
+// each object decides its own fate from read-only data: one thread per object, keep flags only,
+// no ordering between threads.  Pairs are found through two lookups instead of all-pairs loops:
+//   * hit -> objects incidence lists (CSR over the sorted hit positions) for "shares OT hits";
+//   * pixel seeds binned in eta (bin width >= 1.25 sqrt(dr2max)) for "close in eta-phi", plus a
+//     per-seed list of related seeds (close in eta-phi, or sharing a pixel-hit id).
+// Object ids in the incidence lists ("dd ids"): [0, nT5) T5, then pT5, then pT3.
 #include "lst_launch.h"
 
 namespace lst {
-void launch_dedup(const Ctx &c, const SlotDev &s, cudaStream_t st) { (void)c; (void)s; (void)st; }
+
+struct DRef {
+  int type;              // 0 T5, 1 pT5, 2 pT3
+  uint32_t idx;          // index inside its own collection
+  int n_ot;              // 10 or 6
+  const uint32_t *hits;  // sorted hit positions, layer order
+  uint32_t pls;
+  double score;
+};
+
+__device__ __forceinline__ DRef dd_ref(const SlotDev &s, uint32_t n5, uint32_t np5, uint32_t d) {
+  DRef r;
+  if (d < n5) {
+    r.type = 0; r.idx = d; r.n_ot = 10; r.hits = s.t5_hits + 10 * (size_t)d; r.pls = 0xFFFFFFFFu; r.score = s.t5_chi2[d];
+  } else if (d < n5 + np5) {
+    const uint32_t i = d - n5;
+    const uint2 po = s.pt5_po[i];
+    r.type = 1; r.idx = i; r.n_ot = 10; r.hits = s.t5_hits + 10 * (size_t)po.y; r.pls = po.x; r.score = s.pt5_chi2[i];
+  } else {
+    const uint32_t i = d - n5 - np5;
+    r.type = 2; r.idx = i; r.n_ot = 6; r.hits = s.pt3_hits + 6 * (size_t)i; r.pls = s.pt3_po[i].x; r.score = s.pt3_chi2[i];
+  }
+  return r;
+}
+__device__ __forceinline__ int dd_type(uint32_t n5, uint32_t np5, uint32_t d) { return d < n5 ? 0 : (d < n5 + np5 ? 1 : 2); }
+
+// "b beats a": (score, hit coordinates in layer order, pLS index, original hit indices), reading 15.
+__device__ bool dd_beats(const SlotDev &s, const DRef &b, const DRef &a) {
+  if (b.score < a.score) return true;
+  if (b.score > a.score) return false;
+  const int n = a.n_ot < b.n_ot ? a.n_ot : b.n_ot;
+  for (int k = 0; k < n; ++k) {
+    const float4 pb = s.hit[b.hits[k]], pa = s.hit[a.hits[k]];
+    if (pb.x < pa.x) return true;
+    if (pb.x > pa.x) return false;
+    if (pb.y < pa.y) return true;
+    if (pb.y > pa.y) return false;
+    if (pb.z < pa.z) return true;
+    if (pb.z > pa.z) return false;
+  }
+  if (a.type != 0 && b.type != 0) {
+    if (b.pls < a.pls) return true;
+    if (b.pls > a.pls) return false;
+  }
+  for (int k = 0; k < n; ++k) {
+    const uint32_t ob = s.hit_orig[b.hits[k]], oa = s.hit_orig[a.hits[k]];
+    if (ob < oa) return true;
+    if (ob > oa) return false;
+  }
+  return false;
+}
+
+__device__ __forceinline__ int dd_shared(const uint32_t *ha, int na, const uint32_t *hb, int nb) {
+  int n = 0;
+  for (int j = 0; j < nb; ++j) {
+    const uint32_t v = hb[j];
+#pragma unroll
+    for (int i = 0; i < 10; ++i) n += (i < na && ha[i] == v);
+  }
+  return n;
+}
+
+__device__ __forceinline__ int eta_bin(const Params &g, double eta) {
+  const double t = (eta + 4.0) * g.eta_bin_inv;
+  if (!(t >= 0.0)) return 0;
+  return t < (double)g.eta_nbins ? (int)t : g.eta_nbins - 1;
+}
+__device__ __forceinline__ bool close_eta_phi(const Params &g, double e1, double p1, double e2, double p2) {
+  const double de = e1 - e2;
+  if (fabs(de) > g.dr_eta_pre) return false;
+  const double dp = wrap_pi(p1 - p2);
+  return de * de + dp * dp < g.dr2max;
+}
+
+// ------------------------------------------------------------------ pixel-seed lookups
+// One block: cleaning sizes, eta bins of the seeds (counting sort; order inside a bin is irrelevant).
+__global__ void __launch_bounds__(1024) k_pls_prep(SlotDev s, Params g) {
+  __shared__ uint32_t cnt[kEtaBins];
+  __shared__ uint32_t sh[33];
+  Header *hdr = s.hdr;
+  const uint32_t n = hdr->n_seeds;
+  if (threadIdx.x == 0) {
+    hdr->n_dd = hdr->n_obj[3] + hdr->n_obj[5] + hdr->n_obj[4];
+    hdr->n_flag = hdr->n_obj[5] + hdr->n_obj[4] + hdr->n_obj[3] + n;
+  }
+  for (int b = threadIdx.x; b < kEtaBins; b += blockDim.x) cnt[b] = 0;
+  __syncthreads();
+  for (uint32_t p = threadIdx.x; p < n; p += blockDim.x) atomicAdd(&cnt[eta_bin(g, (double)s.seed_eta[p])], 1u);
+  __syncthreads();
+  uint32_t carry = 0;
+  for (int base = 0; base < kEtaBins; base += blockDim.x) {
+    const int b = base + threadIdx.x;
+    const uint32_t v = cnt[b];
+    uint32_t tot;
+    const uint32_t e = block_excl_scan(v, sh, &tot);
+    s.pls_bin_off[b] = carry + e;
+    cnt[b] = carry + e;
+    carry += tot;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) s.pls_bin_off[kEtaBins] = carry;
+  __syncthreads();
+  for (uint32_t p = threadIdx.x; p < n; p += blockDim.x) {
+    const uint32_t pos = atomicAdd(&cnt[eta_bin(g, (double)s.seed_eta[p])], 1u);
+    s.pls_bin_ent[pos] = p;
+  }
+}
+
+// One warp per seed a: seeds b != a that are close in eta-phi (bit 31) or share a pixel-hit id.
+__global__ void __launch_bounds__(256) k_pls_adj(SlotDev s, Params g) {
+  const uint32_t n = s.hdr->n_seeds;
+  const int lane = threadIdx.x & 31;
+  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+  const uint4 *ids = reinterpret_cast<const uint4 *>(s.seed_ids);
+  for (uint32_t a = warp; a < n; a += nwarp) {
+    const double ea = (double)s.seed_eta[a], pa = (double)s.seed_phi[a];
+    const uint4 ia = ids[a];
+    uint32_t cnt = 0;
+    for (uint32_t base = 0; base < n; base += 32) {
+      const uint32_t b = base + lane;
+      bool rel = false, close = false;
+      if (b < n && b != a) {
+        close = close_eta_phi(g, ea, pa, (double)s.seed_eta[b], (double)s.seed_phi[b]);
+        const uint4 ib = ids[b];
+        const uint32_t va[4] = {ia.x, ia.y, ia.z, ia.w}, vb[4] = {ib.x, ib.y, ib.z, ib.w};
+        bool sharep = false;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int j = 0; j < 4; ++j) sharep |= (va[i] == vb[j]);
+        rel = close || sharep;
+      }
+      const uint32_t bal = __ballot_sync(0xffffffffu, rel);
+      if (rel) {
+        const uint32_t pos = cnt + __popc(bal & ((1u << lane) - 1u));
+        if (pos < (uint32_t)kAdjCap) s.pls_adj[(size_t)a * kAdjCap + pos] = b | (close ? 0x80000000u : 0u);
+      }
+      cnt += __popc(bal);
+    }
+    if (lane == 0) {
+      if (cnt > (uint32_t)kAdjCap) { atomicOr(&s.hdr->err, (uint32_t)ERR_CAP_PIX); cnt = 0; }
+      s.pls_adj_cnt[a] = cnt;
+    }
+  }
+}
+
+// ------------------------------------------------------------------ hit -> objects incidence
+__device__ __forceinline__ void md_hits2(const SlotDev &s, uint32_t md, uint32_t *out) {
+  const uint2 h = s.md_hit[md];
+  out[0] = h.x; out[1] = h.y;
+}
+// thread per dd object: gather its hit positions (T5 and pT3 store them) and count the incidences
+__global__ void k_dd_count(SlotDev s) {
+  const Header *hdr = s.hdr;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = hdr->n_dd;
+  for (uint32_t d = blockIdx.x * blockDim.x + threadIdx.x; d < n_dd; d += gridDim.x * blockDim.x) {
+    uint32_t h[10];
+    int n;
+    if (d < n5 + np5) {
+      const uint32_t t = d < n5 ? d : s.pt5_po[d - n5].y;
+#pragma unroll
+      for (int q = 0; q < 5; ++q) md_hits2(s, s.t5_md[5 * (size_t)t + q], h + 2 * q);
+      n = 10;
+      if (d < n5)
+#pragma unroll
+        for (int q = 0; q < 10; ++q) s.t5_hits[10 * (size_t)d + q] = h[q];
+    } else {
+      const uint32_t i = d - n5 - np5;
+      const uint4 m = s.t3_md[s.pt3_po[i].y];
+      md_hits2(s, m.x, h); md_hits2(s, m.y, h + 2); md_hits2(s, m.z, h + 4);
+      n = 6;
+#pragma unroll
+      for (int q = 0; q < 6; ++q) s.pt3_hits[6 * (size_t)i + q] = h[q];
+    }
+    for (int q = 0; q < n; ++q) atomicAdd(&s.inc_cnt[h[q]], 1u);
+  }
+}
+__global__ void k_dd_scatter(SlotDev s) {
+  const Header *hdr = s.hdr;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = hdr->n_dd;
+  for (uint32_t d = blockIdx.x * blockDim.x + threadIdx.x; d < n_dd; d += gridDim.x * blockDim.x) {
+    const DRef r = dd_ref(s, n5, np5, d);
+    for (int q = 0; q < r.n_ot; ++q) {
+      const uint32_t h = r.hits[q];
+      s.inc_ent[s.inc_off[h] + atomicAdd(&s.inc_cur[h], 1u)] = d;
+    }
+  }
+}
+
+// ------------------------------------------------------------------ S0: inside one collection
+__global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
+  const Header *hdr = s.hdr;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = hdr->n_dd;
+  for (uint32_t d = blockIdx.x * blockDim.x + threadIdx.x; d < n_dd; d += gridDim.x * blockDim.x) {
+    const DRef A = dd_ref(s, n5, np5, d);
+    uint32_t ha[10];
+#pragma unroll
+    for (int q = 0; q < 10; ++q) ha[q] = q < A.n_ot ? A.hits[q] : 0xFFFFFFFFu;
+    bool keep = true;
+    if (g.s0_enabled) {
+      const int min_shared = A.type == 0 ? g.dup_t5 : (A.type == 1 ? g.dup_pt5 : g.dup_pt3);
+      // an object sharing >= min_shared of A's hits contains one of any n_ot - min_shared + 1 of them
+      const int k0 = min_shared - 1;
+      for (int k = k0; k < A.n_ot && keep; ++k) {
+        const uint32_t h = A.hits[k];
+        for (uint32_t e = s.inc_off[h]; e < s.inc_off[h + 1]; ++e) {
+          const uint32_t b = s.inc_ent[e];
+          if (b == d || dd_type(n5, np5, b) != A.type) continue;
+          const DRef Bq = dd_ref(s, n5, np5, b);
+          if (dd_shared(ha, A.n_ot, Bq.hits, Bq.n_ot) >= min_shared && dd_beats(s, Bq, A)) { keep = false; break; }
+        }
+      }
+      if (keep && A.type != 0) {   // objects of the same pixel seed are duplicates of one another
+        const uint32_t *off = A.type == 1 ? s.pt5_pls_off : s.pt3_pls_off;
+        const uint32_t base = A.type == 1 ? n5 : n5 + np5;
+        for (uint32_t i = off[A.pls]; i < off[A.pls + 1]; ++i) {
+          if (i == A.idx) continue;
+          const DRef Bq = dd_ref(s, n5, np5, base + i);
+          if (dd_beats(s, Bq, A)) { keep = false; break; }
+        }
+      }
+    }
+    if (A.type == 0) s.t5_keep[A.idx] = keep;
+    else if (A.type == 1) { s.pt5_keep[A.idx] = keep; if (keep) s.pls_has5[A.pls] = 1; }
+    else s.pt3_keep[A.idx] = keep;
+  }
+}
+
+// ------------------------------------------------------------------ S1: pT3 against surviving pT5
+__global__ void __launch_bounds__(128) k_s1(SlotDev s, Params g) {
+  (void)g;
+  const Header *hdr = s.hdr;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], np3 = hdr->n_obj[4];
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < np3; i += gridDim.x * blockDim.x) {
+    if (!s.pt3_keep[i]) continue;
+    const uint32_t p = s.pt3_po[i].x;
+    bool dup = s.pls_has5[p];
+    const uint32_t na = s.pls_adj_cnt[p];
+    for (uint32_t k = 0; k < na && !dup; ++k) dup = s.pls_has5[s.pls_adj[(size_t)p * kAdjCap + k] & 0x7FFFFFFFu];
+    for (int q = 0; q < 6 && !dup; ++q) {
+      const uint32_t h = s.pt3_hits[6 * (size_t)i + q];
+      for (uint32_t e = s.inc_off[h]; e < s.inc_off[h + 1]; ++e) {
+        const uint32_t b = s.inc_ent[e];
+        if (b >= n5 && b < n5 + np5 && s.pt5_keep[b - n5]) { dup = true; break; }
+      }
+    }
+    if (dup) s.pt3_keep[i] = 0;
+    else s.pls_has3[p] = 1;
+  }
+}
+
+// ------------------------------------------------------------------ S2: T5 against surviving pT5 / pT3
+__global__ void __launch_bounds__(128) k_s2(SlotDev s, Params g) {
+  const Header *hdr = s.hdr;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5];
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n5; i += gridDim.x * blockDim.x) {
+    if (!s.t5_keep[i]) continue;
+    bool dup = false;
+    for (int q = 0; q < 10 && !dup; ++q) {
+      const uint32_t h = s.t5_hits[10 * (size_t)i + q];
+      for (uint32_t e = s.inc_off[h]; e < s.inc_off[h + 1]; ++e) {
+        const uint32_t b = s.inc_ent[e];
+        if (b < n5) continue;
+        if (b < n5 + np5 ? s.pt5_keep[b - n5] : s.pt3_keep[b - n5 - np5]) { dup = true; break; }
+      }
+    }
+    const double2 ep = s.t5_etaphi[i];
+    const int b0 = eta_bin(g, ep.x);
+    const int lo = b0 > 0 ? b0 - 1 : 0, hi = b0 + 1 < g.eta_nbins ? b0 + 1 : g.eta_nbins - 1;
+    const uint32_t e0 = s.pls_bin_off[lo], e1 = s.pls_bin_off[hi + 1];
+    for (uint32_t e = e0; e < e1 && !dup; ++e) {
+      const uint32_t p = s.pls_bin_ent[e];
+      if ((s.pls_has5[p] || s.pls_has3[p]) && close_eta_phi(g, ep.x, ep.y, (double)s.seed_eta[p], (double)s.seed_phi[p]))
+        dup = true;
+    }
+    if (dup) { s.t5_keep[i] = 0; continue; }
+    for (uint32_t e = e0; e < e1; ++e) {   // survivor: the seeds close to it are duplicates of it (S3)
+      const uint32_t p = s.pls_bin_ent[e];
+      if (close_eta_phi(g, ep.x, ep.y, (double)s.seed_eta[p], (double)s.seed_phi[p])) s.pls_near_t5[p] = 1;
+    }
+  }
+}
+
+// ------------------------------------------------------------------ S3 + keep flags in TC order
+__device__ __forceinline__ bool pls_unused(const SlotDev &s, uint32_t p) {
+  return s.pt5_pls_off[p + 1] == s.pt5_pls_off[p] && s.pt3_pls_off[p + 1] == s.pt3_pls_off[p];
+}
+__global__ void k_s3_flags(SlotDev s) {
+  const Header *hdr = s.hdr;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], np3 = hdr->n_obj[4], n = hdr->n_flag;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    uint32_t f;
+    if (i < np5) f = s.pt5_keep[i];
+    else if (i < np5 + np3) f = s.pt3_keep[i - np5];
+    else if (i < np5 + np3 + n5) f = s.t5_keep[i - np5 - np3];
+    else {
+      const uint32_t p = i - np5 - np3 - n5;
+      bool keep = pls_unused(s, p) && !s.pls_near_t5[p];
+      const uint32_t na = s.pls_adj_cnt[p];
+      for (uint32_t k = 0; k < na && keep; ++k) {
+        const uint32_t a = s.pls_adj[(size_t)p * kAdjCap + k];
+        const uint32_t b = a & 0x7FFFFFFFu;
+        if (s.pls_has5[b] || s.pls_has3[b]) keep = false;
+        else if ((a >> 31) && b < p && pls_unused(s, b)) keep = false;
+      }
+      s.pls_keep[p] = keep;
+      f = keep;
+    }
+    s.tc_flag[i] = f;
+  }
+}
+
+// ------------------------------------------------------------------ S4: TC = pT5, pT3, T5, pLS survivors
+__global__ void k_tc_fill(SlotDev s) {
+  Header *hdr = s.hdr;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], np3 = hdr->n_obj[4], n = hdr->n_flag;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    if (!s.tc_flag[i]) continue;
+    const uint32_t pos = s.tc_pos[i];
+    uint32_t type, obj, p = 0xFFFFFFFFu;
+    if (i < np5) { type = 5; obj = i; p = s.pt5_po[obj].x; }
+    else if (i < np5 + np3) { type = 4; obj = i - np5; p = s.pt3_po[obj].x; }
+    else if (i < np5 + np3 + n5) { type = 3; obj = i - np5 - np3; }
+    else { type = 6; obj = i - np5 - np3 - n5; p = obj; }
+    s.tc_to[pos] = make_uint2(type, obj);
+    if (type == 3) {
+      const double2 ep = s.t5_etaphi[obj];
+      s.tc_f[pos] = make_float4(s.t5_pt[obj], (float)ep.x, (float)ep.y, 3.0f);
+    } else {
+      s.tc_f[pos] = make_float4(s.seed_pt[p], s.seed_eta[p], s.seed_phi[p], (float)type);
+    }
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) hdr->n_obj[6] = s.tc_pos[n];
+}
+
+static inline int grid_of(uint32_t n, int threads, int max_blocks) {
+  long b = ((long)n + threads - 1) / threads;
+  return (int)(b < 1 ? 1 : (b > max_blocks ? max_blocks : b));
+}
+
+void launch_dedup(const Ctx &c, const SlotDev &s, cudaStream_t st) {
+  const uint32_t cap_dd = s.cap_t5 + s.cap_pt5 + s.cap_pt3;
+  cudaMemsetAsync(s.inc_cnt, 0, sizeof(uint32_t) * 2 * ((size_t)s.cap_hits + 1), st);
+  cudaMemsetAsync(s.pls_has5, 0, 3 * (size_t)s.cap_seeds, st);
+  k_pls_prep<<<1, 1024, 0, st>>>(s, c.par);
+  k_pls_adj<<<grid_of(s.cap_seeds, 8, c.n_sm * 8), 256, 0, st>>>(s, c.par);
+  k_dd_count<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s);
+  launch_scan(c, s, s.inc_cnt, s.inc_off, &s.hdr->n_hits, st);
+  k_dd_scatter<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s);
+  k_s0<<<grid_of(cap_dd, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par);
+  k_s1<<<grid_of(s.cap_pt3, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par);
+  k_s2<<<grid_of(s.cap_t5, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par);
+  k_s3_flags<<<grid_of(s.cap_tc, 256, c.n_sm * 8), 256, 0, st>>>(s);
+  launch_scan(c, s, s.tc_flag, s.tc_pos, &s.hdr->n_flag, st);
+  k_tc_fill<<<grid_of(s.cap_tc, 256, c.n_sm * 8), 256, 0, st>>>(s);
+}
+
 }  // namespace lst

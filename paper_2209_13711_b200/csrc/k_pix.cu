@@ -1,6 +1,119 @@
 // k_pix.cu -- a5 pixel-seeded pT5 / pT3 (Fig. 10-11; reading C6).
+//
+// The definition is "all (pixel seed, T5 / T3) pairs".  The enumeration is restricted, without
+// changing the result, to the objects whose FIRST anchor can pass its two residual cuts: per seed
+// the start-layer modules whose lower-sensor box (lst_geometry) overlaps the seed's extrapolation
+// window are listed (k_px_modules); the (seed, module) pairs are the rows of the generic join
+// (k_t3t5.cu), whose right lists are the T5 / T3 starting in that module.  The window test is
+// conservative (interval arithmetic on the box plus margins); tests compare with the oracle's
+// brute force.
 #include "lst_launch.h"
 
 namespace lst {
-void launch_pixel(const Ctx &c, const SlotDev &s, cudaStream_t st) { (void)c; (void)s; (void)st; }
+
+constexpr float kPxMarginPhi = 2e-3f;   // rad, added to every azimuthal window
+constexpr float kPxMarginLen = 5e-2f;   // cm, added to every z / r window
+
+__device__ __forceinline__ float asin_sat(float v) { return asinf(fminf(1.0f, fmaxf(-1.0f, v))); }
+
+// Can a hit inside module m's lower-sensor box pass the first-anchor cuts of seed (pt, eta, phi, z0, q)?
+__device__ __forceinline__ bool px_module_compatible(const GeoDev &geo, const Params &g, uint32_t m, float kp,
+                                                     float sh, float phi, float z0) {
+  const int cat = geo.category[m];
+  const float rlo = geo.rmin[m], rhi = geo.rmax[m], phic = geo.phic[m], hphi = geo.hphi[m];
+  const float zlo = geo.zmin[m], zhi = geo.zmax[m];
+  const float akp = fabsf(kp);
+  const float sgn = kp < 0.0f ? -1.0f : 1.0f;
+  const float ns = g.f_ns;
+  if (cat < 2) {
+    // barrel: arc length s(r) = asin(|k| r) / |k| is increasing in r
+    const float a_lo = asin_sat(akp * rlo), a_hi = asin_sat(akp * rhi);
+    const float s_lo = akp * rlo <= 1e-4f ? rlo : a_lo / akp, s_hi = akp * rhi <= 1e-4f ? rhi : a_hi / akp;
+    const float phim = phi + sgn * 0.5f * (a_lo + a_hi);
+    const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * akp * s_hi + g.f_sig_t[cat] / rlo;
+    const float dphi = fabsf(remainderf(phic - phim, 6.2831853071795864769f));
+    if (dphi > hphi + 0.5f * (a_hi - a_lo) + ns * sgp + kPxMarginPhi) return false;
+    const float z1 = z0 + sh * s_lo, z2 = z0 + sh * s_hi;
+    const float tol = ns * ((float)g.seed_sig_z + g.f_sig_z[cat]) + kPxMarginLen + 1e-3f * (fabsf(z1) + fabsf(z2));
+    return fmaxf(z1, z2) + tol >= zlo && fminf(z1, z2) - tol <= zhi;
+  }
+  // endcap: the anchor's z is the lower-sensor plane, so the arc length is known
+  if (!(fabsf(sh) > 1e-9f)) return false;
+  const float al = (zlo - z0) / sh;
+  if (!(al > 0.0f)) return false;
+  const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * akp * al + g.f_sig_t[cat] / rlo;
+  const float dphi = fabsf(remainderf(phic - (phi + kp * al), 6.2831853071795864769f));
+  if (dphi > hphi + ns * sgp + kPxMarginPhi + 1e-3f * akp * al) return false;
+  const float ka = kp * al;
+  const float rp = fabsf(ka) <= 1e-4f ? al : sinf(ka) / kp;
+  const float tol = ns * ((float)g.seed_sig_z / fabsf(sh) + g.f_sig_r[cat]) + kPxMarginLen + 1e-3f * fabsf(rp);
+  return rp + tol >= rlo && rp - tol <= rhi;
+}
+
+// One warp per seed.  FILL = false: count the compatible start modules; FILL = true: write the
+// (seed, module) rows at the seed's offset, modules ascending.  (A seed with eta ~ 0 is compatible
+// with every endcap module of a side - its extrapolation tolerances diverge - so the lists are
+// sized exactly, not capped per seed.)
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_px_modules(GeoDev geo, SlotDev s, Params g) {
+  const uint32_t n_seeds = s.hdr->n_seeds;
+  const int lane = threadIdx.x & 31;
+  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+  if (FILL && s.hdr->n_obj[kPairLevel] == 0) return;
+  for (uint32_t p = warp; p < n_seeds; p += nwarp) {
+    const float pt = s.seed_pt[p], phi = s.seed_phi[p], z0 = s.seed_z0[p];
+    const float kp = -(float)s.seed_q[p] * (float)g.kB / (2.0f * pt);
+    const float sh = sinhf(s.seed_eta[p]);
+    const uint32_t off = FILL ? s.px_off[p] : 0u;
+    uint32_t cnt = 0;
+    for (uint32_t base = 0; base < geo.n_start; base += 32) {
+      const uint32_t k = base + lane;
+      bool ok = false;
+      uint32_t m = 0;
+      if (k < geo.n_start && pt > 0.0f) {
+        m = geo.start_mods[k];
+        ok = px_module_compatible(geo, g, m, kp, sh, phi, z0);
+      }
+      const uint32_t b = __ballot_sync(0xffffffffu, ok);
+      if (FILL && ok) s.px_pair[off + cnt + __popc(b & ((1u << lane) - 1u))] = make_uint2(p, m);
+      cnt += __popc(b);
+    }
+    if (!FILL && lane == 0) s.px_cnt[p] = cnt;
+  }
+}
+
+// One block: offsets of the per-seed lists; the row count (0 + error flag if the rows do not fit).
+__global__ void __launch_bounds__(1024) k_px_offsets(SlotDev s) {
+  __shared__ uint32_t sh[33];
+  const uint32_t n_seeds = s.hdr->n_seeds;
+  uint32_t carry = 0;
+  for (uint32_t base = 0; base < n_seeds; base += blockDim.x) {
+    const uint32_t p = base + threadIdx.x;
+    const uint32_t v = p < n_seeds ? s.px_cnt[p] : 0u;
+    uint32_t tot;
+    const uint32_t e = block_excl_scan(v, sh, &tot);
+    if (p < n_seeds) s.px_off[p] = carry + e;
+    carry += tot;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    s.px_off[n_seeds] = carry;
+    if (carry > s.cap_seeds * (uint32_t)kPxCap) { atomicOr(&s.hdr->err, (uint32_t)ERR_CAP_PIX); carry = 0; }
+    s.hdr->n_obj[kPairLevel] = carry;
+  }
+}
+
+void launch_pixel(const Ctx &c, const SlotDev &s, cudaStream_t st) {
+  const int warps_per_block = 8;
+  int g = (int)((s.cap_seeds + warps_per_block - 1) / warps_per_block);
+  if (g > c.n_sm * 8) g = c.n_sm * 8;
+  k_px_modules<false><<<g, 256, 0, st>>>(c.geo, s, c.par);
+  k_px_offsets<<<1, 1024, 0, st>>>(s);
+  k_px_modules<true><<<g, 256, 0, st>>>(c.geo, s, c.par);
+  launch_join(c, s, 2, st);            // pT5
+  launch_row_offsets(c, s, 4, st);
+  launch_join(c, s, 3, st);            // pT3
+  launch_row_offsets(c, s, 5, st);
+}
+
 }  // namespace lst

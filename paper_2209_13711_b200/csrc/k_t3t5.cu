@@ -14,26 +14,43 @@ struct RowTab {                       // right-list table of one group, in share
   uint32_t cum[kRowChunk + 1];
 };
 
-// T5 = false: rows are LS, right lists are LS ranges of the outer MD.
-// T5 = true : rows are T3, right lists are T3 ranges of the third MD.
-template <bool T5>
+// KIND 0 (T3) : rows are LS, right lists are LS ranges of the outer MD.
+// KIND 1 (T5) : rows are T3, right lists are T3 ranges of the third MD.
+// KIND 2 (pT5): rows are (seed, compatible start module) pairs (k_pix.cu), right lists are the T5
+//               whose first MD lies in that module (T5 are ordered by first MD, MDs by module).
+// KIND 3 (pT3): same with T3.
+enum { J_T3 = 0, J_T5 = 1, J_PT5 = 2, J_PT3 = 3 };
+
+template <int KIND> struct JoinTraits;
+template <> struct JoinTraits<J_T3> { static constexpr int stage = S_T3, rows_level = 1, out_level = 2; };
+template <> struct JoinTraits<J_T5> { static constexpr int stage = S_T5, rows_level = 2, out_level = 3; };
+template <> struct JoinTraits<J_PT5> { static constexpr int stage = S_PT5, rows_level = kPairLevel, out_level = 5; };
+template <> struct JoinTraits<J_PT3> { static constexpr int stage = S_PT3, rows_level = kPairLevel, out_level = 4; };
+
+template <int KIND>
 __device__ __forceinline__ void right_range(const SlotDev &s, uint32_t row, uint32_t *st, uint32_t *cnt) {
-  if (!T5) {
+  if (KIND == J_T3) {
     const uint32_t mo = s.ls_md[row].y;
     *st = s.ls_md_off[mo];
     *cnt = s.ls_md_off[mo + 1] - *st;
-  } else {
+  } else if (KIND == J_T5) {
     const uint32_t m3 = s.t3_md[row].z;
     *st = s.t3_md_off[m3];
     *cnt = s.t3_md_off[m3 + 1] - *st;
+  } else {
+    const uint32_t m = s.px_pair[row].y;
+    const uint32_t md0 = s.md_mod_off[m], md1 = s.md_mod_off[m + 1];
+    const uint32_t *off = KIND == J_PT5 ? s.t5_md_off : s.t3_md_off;
+    *st = off[md0];
+    *cnt = off[md1] - *st;
   }
 }
 
-template <bool T5>
+template <int KIND>
 __global__ void k_join_groups(SlotDev s) {
-  const int stage = T5 ? S_T5 : S_T3;
+  const int stage = JoinTraits<KIND>::stage;
   const StageBuf &st = s.st[stage];
-  const uint32_t n_rows = s.hdr->n_obj[T5 ? 2 : 1];
+  const uint32_t n_rows = s.hdr->n_obj[JoinTraits<KIND>::rows_level];
   const uint32_t ng = (n_rows + kRowChunk - 1) / kRowChunk;
   const int lane = threadIdx.x & 31;
   const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
@@ -42,7 +59,7 @@ __global__ void k_join_groups(SlotDev s) {
     uint32_t sum = 0;
     for (uint32_t r = r0 + lane; r < r1; r += 32) {
       uint32_t a, c;
-      right_range<T5>(s, r, &a, &c);
+      right_range<KIND>(s, r, &a, &c);
       sum += c;
     }
     sum = warp_sum(sum);
@@ -50,11 +67,11 @@ __global__ void k_join_groups(SlotDev s) {
   }
 }
 
-template <bool T5>
+template <int KIND>
 __device__ __forceinline__ void stage_rows(RowTab &rt, const SlotDev &s, uint32_t r0, uint32_t n_rows, uint32_t *sh) {
   const int tid = threadIdx.x;   // kThreads == kRowChunk
   uint32_t a = 0, c = 0;
-  if (r0 + tid < n_rows) right_range<T5>(s, r0 + tid, &a, &c);
+  if (r0 + tid < n_rows) right_range<KIND>(s, r0 + tid, &a, &c);
   uint32_t tot;
   const uint32_t e = block_excl_scan(c, sh, &tot);
   rt.start[tid] = a;
@@ -99,21 +116,84 @@ __device__ __forceinline__ bool t5_candidate(const SlotDev &s, const Params &g, 
   return t5_eval_d(g, P, k3a.x, k3a.y, k3b.x, k3b.y, o);
 }
 
-template <bool T5>
-__global__ void __launch_bounds__(kThreads) k_join_eval(SlotDev s, Params g) {
+// pT5 / pT3 candidate: pixel seed `p` against OT object `obj` (reading C6).  The fp32 pre-filter tests
+// the first anchor only, loosened by kPreSlack plus absolute slacks far above the fp32 error
+// (1e-5 rad on a >= 4e-3 rad window, 2e-3 cm on a >= 0.2 cm window); it never rejects on NaN.
+template <int KIND>
+__device__ __forceinline__ bool px_candidate(const GeoDev &geo, const SlotDev &s, const Params &g, uint32_t p,
+                                             uint32_t obj, double *chi2, bool prefilter) {
+  constexpr int N = KIND == J_PT5 ? 5 : 3;
+  uint32_t m[5];
+  if (KIND == J_PT5) {
+#pragma unroll
+    for (int k = 0; k < 5; ++k) m[k] = s.t5_md[5 * (size_t)obj + k];
+  } else {
+    const uint4 t = s.t3_md[obj];
+    m[0] = t.x; m[1] = t.y; m[2] = t.z;
+  }
+  const float spt = s.seed_pt[p], seta = s.seed_eta[p], sphi = s.seed_phi[p], sz0 = s.seed_z0[p];
+  const int q = s.seed_q[p];
+  const uint32_t mm0 = s.md_mod[m[0]];
+  if (prefilter) {
+    const float4 h = s.md_pos[m[0]];
+    const int cat = (int)(mm0 & 3u);
+    const float kp = -(float)q * (float)g.kB / (2.0f * spt);
+    const float sh = sinhf(seta);
+    float al;
+    if (cat < 2) {
+      const float kr = kp * h.w;
+      al = fabsf(kr) <= 1e-4f ? h.w : asinf(fminf(1.0f, fmaxf(-1.0f, kr))) / kp;
+    } else {
+      al = (h.z - sz0) / sh;
+    }
+    const float dph = remainderf(atan2f(h.y, h.x) - (sphi + kp * al), 6.2831853071795864769f);
+    const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * fabsf(kp) * al + g.f_sig_t[cat] / h.w;
+    if (fabsf(dph) > g.f_ns * sgp * kPreSlack + 1e-5f) return false;
+    float dzt, szt;
+    if (cat < 2) {
+      dzt = h.z - (sz0 + sh * al);
+      szt = (float)g.seed_sig_z + g.f_sig_z[cat];
+    } else {
+      const float ka = kp * al;
+      dzt = h.w - (fabsf(ka) <= 1e-4f ? al : sinf(ka) / kp);
+      szt = (float)g.seed_sig_z / fabsf(sh) + g.f_sig_r[cat];
+    }
+    if (fabsf(dzt) > g.f_ns * szt * kPreSlack + 2e-3f) return false;
+  }
+  Seed sd;
+  sd.pt = (double)spt; sd.eta = (double)seta; sd.phi = (double)sphi; sd.z0 = (double)sz0; sd.q = q;
+  Pt P[N];
+#pragma unroll
+  for (int k = 0; k < N; ++k) P[k] = md_point(s, m[k]);
+  double c2 = 0.0;
+  const bool ok = px_eval_d(g, sd, P, N, (int)geo.layer[mm0 >> 2], &c2);
+  if (chi2) *chi2 = c2;
+  return ok;
+}
+
+template <int KIND>
+__device__ __forceinline__ bool join_candidate(const GeoDev &geo, const SlotDev &s, const Params &g, uint32_t row,
+                                               uint32_t b) {
+  if (KIND == J_T3) return t3_candidate(s, g, row, b, nullptr, nullptr);
+  if (KIND == J_T5) return t5_candidate(s, g, row, b, nullptr, nullptr, nullptr, nullptr);
+  return px_candidate<KIND>(geo, s, g, s.px_pair[row].x, b, nullptr, true);
+}
+
+template <int KIND>
+__global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, Params g) {
   __shared__ ItemScratch sc;
   __shared__ RowTab rt;
   __shared__ uint32_t sh[33];
-  const int stage = T5 ? S_T5 : S_T3;
+  const int stage = JoinTraits<KIND>::stage;
   const StageBuf &st = s.st[stage];
   const uint32_t n_items = s.hdr->n_items[stage];
-  const uint32_t n_rows = s.hdr->n_obj[T5 ? 2 : 1];
+  const uint32_t n_rows = s.hdr->n_obj[JoinTraits<KIND>::rows_level];
   const int tid = threadIdx.x;
   for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
     const Item item = st.items[it];
     const uint32_t r0 = item.group * kRowChunk;
     if (tid < kItemWords) sc.mask[tid] = 0;
-    stage_rows<T5>(rt, s, r0, n_rows, sh);
+    stage_rows<KIND>(rt, s, r0, n_rows, sh);
     const int nj = item.nj;
     for (int base = 0; base < nj; base += kThreads) {
       const int c = base + tid;
@@ -121,8 +201,7 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(SlotDev s, Params g) {
       if (c < nj) {
         int row; uint32_t b;
         flat_to_pair(rt, item.j0 + c, &row, &b);
-        pass = T5 ? t5_candidate(s, g, r0 + row, b, nullptr, nullptr, nullptr, nullptr)
-                  : t3_candidate(s, g, r0 + row, b, nullptr, nullptr);
+        pass = join_candidate<KIND>(geo, s, g, r0 + row, b);
       }
       const uint32_t w = __ballot_sync(0xffffffffu, pass);
       if ((tid & 31) == 0) sc.mask[c >> 5] = w;
@@ -133,21 +212,21 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(SlotDev s, Params g) {
   }
 }
 
-template <bool T5>
-__global__ void __launch_bounds__(kThreads) k_join_fill(SlotDev s, Params g) {
+template <int KIND>
+__global__ void __launch_bounds__(kThreads) k_join_fill(GeoDev geo, SlotDev s, Params g) {
   __shared__ ItemScratch sc;
   __shared__ RowTab rt;
   __shared__ uint32_t sh[33];
-  const int stage = T5 ? S_T5 : S_T3;
+  const int stage = JoinTraits<KIND>::stage;
   const StageBuf &st = s.st[stage];
   const uint32_t n_items = s.hdr->n_items[stage];
-  const uint32_t n_rows = s.hdr->n_obj[T5 ? 2 : 1];
+  const uint32_t n_rows = s.hdr->n_obj[JoinTraits<KIND>::rows_level];
   const int tid = threadIdx.x;
   for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
     if (st.item_cnt[it] == 0) continue;
     const Item item = st.items[it];
     const uint32_t r0 = item.group * kRowChunk;
-    stage_rows<T5>(rt, s, r0, n_rows, sh);
+    stage_rows<KIND>(rt, s, r0, n_rows, sh);
     expand_mask(sc, st.mask + (size_t)it * kItemWords);
     const int n = (int)sc.n;
     const uint32_t base = st.item_base[it];
@@ -155,14 +234,14 @@ __global__ void __launch_bounds__(kThreads) k_join_fill(SlotDev s, Params g) {
       int row; uint32_t b;
       flat_to_pair(rt, item.j0 + sc.list[k], &row, &b);
       const uint32_t a = r0 + row, idx = base + k;
-      if (!T5) {
+      if (KIND == J_T3) {
         T3Out o; uint4 m;
         t3_candidate(s, g, a, b, &o, &m);
         s.t3_md[idx] = m;
         s.t3_ls[idx] = make_uint2(a, b);
         s.t3_kd[idx] = make_double2(o.kappa3, o.sigk3);
         s.t3_beta[idx] = (float)o.beta;
-      } else {
+      } else if (KIND == J_T5) {
         T5Out o; uint32_t m[5]; double2 ka, kb;
         t5_candidate(s, g, a, b, &o, m, &ka, &kb);
 #pragma unroll
@@ -172,6 +251,12 @@ __global__ void __launch_bounds__(kThreads) k_join_fill(SlotDev s, Params g) {
         s.t5_etaphi[idx] = make_double2(o.eta, o.phi);
         s.t5_f[idx] = make_float4((float)o.R, (float)o.chi2, (float)ka.x, (float)kb.x);
         s.t5_pt[idx] = (float)o.pt;
+      } else {
+        const uint32_t p = s.px_pair[a].x;
+        double c2 = 0.0;
+        px_candidate<KIND>(geo, s, g, p, b, &c2, false);
+        if (KIND == J_PT5) { s.pt5_po[idx] = make_uint2(p, b); s.pt5_chi2[idx] = c2; }
+        else { s.pt3_po[idx] = make_uint2(p, b); s.pt3_chi2[idx] = c2; }
       }
     }
     __syncthreads();
@@ -179,23 +264,33 @@ __global__ void __launch_bounds__(kThreads) k_join_fill(SlotDev s, Params g) {
 }
 
 // ------------------------------------------------------------------ launchers
+template <int KIND>
+static void launch_join_t(const Ctx &c, const SlotDev &s, uint32_t row_cap, uint32_t out_cap, cudaStream_t st) {
+  const int gg = (int)((row_cap / kRowChunk + 1 + 3) / 4);   // 4 warps per block, one group per warp
+  k_join_groups<KIND><<<gg < c.n_sm * 8 ? gg : c.n_sm * 8, 128, 0, st>>>(s);
+  launch_emit(c, s, JoinTraits<KIND>::stage, JoinTraits<KIND>::rows_level, st);
+  k_join_eval<KIND><<<c.n_sm * 8, kThreads, 0, st>>>(c.geo, s, c.par);
+  launch_scan_items(c, s, JoinTraits<KIND>::stage, JoinTraits<KIND>::out_level, out_cap, st);
+  k_join_fill<KIND><<<c.n_sm * 8, kThreads, 0, st>>>(c.geo, s, c.par);
+}
+
+void launch_join(const Ctx &c, const SlotDev &s, int kind, cudaStream_t st) {
+  switch (kind) {
+    case J_T3: launch_join_t<J_T3>(c, s, s.cap_ls, s.cap_t3, st); break;
+    case J_T5: launch_join_t<J_T5>(c, s, s.cap_t3, s.cap_t5, st); break;
+    case J_PT5: launch_join_t<J_PT5>(c, s, s.cap_seeds * kPxCap, s.cap_pt5, st); break;
+    default: launch_join_t<J_PT3>(c, s, s.cap_seeds * kPxCap, s.cap_pt3, st); break;
+  }
+}
+
 void launch_t3(const Ctx &c, const SlotDev &s, cudaStream_t st) {
-  const int gg = (int)((s.cap_ls / kRowChunk + 1 + 3) / 4);   // 4 warps per block, one group per warp
-  k_join_groups<false><<<gg < c.n_sm * 8 ? gg : c.n_sm * 8, 128, 0, st>>>(s);
-  launch_emit(c, s, S_T3, 1, st);
-  k_join_eval<false><<<c.n_sm * 8, kThreads, 0, st>>>(s, c.par);
-  launch_scan_items(c, s, S_T3, 2, s.cap_t3, st);
-  k_join_fill<false><<<c.n_sm * 8, kThreads, 0, st>>>(s, c.par);
+  launch_join(c, s, J_T3, st);
   launch_row_offsets(c, s, 2, st);
 }
 
 void launch_t5(const Ctx &c, const SlotDev &s, cudaStream_t st) {
-  const int gg = (int)((s.cap_t3 / kRowChunk + 1 + 3) / 4);
-  k_join_groups<true><<<gg < c.n_sm * 8 ? gg : c.n_sm * 8, 128, 0, st>>>(s);
-  launch_emit(c, s, S_T5, 2, st);
-  k_join_eval<true><<<c.n_sm * 8, kThreads, 0, st>>>(s, c.par);
-  launch_scan_items(c, s, S_T5, 3, s.cap_t5, st);
-  k_join_fill<true><<<c.n_sm * 8, kThreads, 0, st>>>(s, c.par);
+  launch_join(c, s, J_T5, st);
+  launch_row_offsets(c, s, 3, st);
 }
 
 }  // namespace lst

@@ -15,6 +15,7 @@ using namespace lst;
 
 // ------------------------------------------------------------------ status text
 static thread_local char g_cuda_err[256] = "no CUDA error recorded";
+static thread_local char g_cap_err[256] = "workspace too small or object capacity exceeded";
 
 static int cuda_fail(cudaError_t e, const char *where) {
   snprintf(g_cuda_err, sizeof(g_cuda_err), "CUDA error at %s: %s", where, cudaGetErrorString(e));
@@ -30,7 +31,7 @@ extern "C" const char *lst_strerror(int status) {
   switch (status) {
     case LST_OK: return "ok";
     case LST_EINVAL: return "invalid argument";
-    case LST_ENOMEM: return "workspace too small or object capacity exceeded";
+    case LST_ENOMEM: return g_cap_err;
     case LST_ECUDA: return g_cuda_err;
     case LST_ESTATE: return "call order violated";
     default: return "unknown status";
@@ -96,6 +97,12 @@ static void make_params(const lst_config &c, Params *p) {
   p->dup_t5 = c.dup_t5_shared; p->dup_pt5 = c.dup_pt5_shared; p->dup_pt3 = c.dup_pt3_shared;
   p->s0_enabled = c.s0_enabled;
   p->start_mask = c.start_layer_mask;
+  // bin width >= 1.25 sqrt(dr2max): two seeds closer than sqrt(dr2max) in eta are in adjacent bins
+  const double sq = std::sqrt(std::max(c.dr2max, 0.0));
+  const double width = std::max(1.25 * sq, 8.0 / kEtaBins);
+  p->eta_bin_inv = 1.0 / width;
+  p->eta_nbins = std::min<int>(kEtaBins, (int)std::ceil(8.0 / width));
+  p->dr_eta_pre = 1.001 * sq + 1e-12;
 }
 
 static bool geometry_ok(const lst_geometry *g) {
@@ -277,18 +284,33 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.t5_md = w.take<uint32_t>(5 * (size_t)s.cap_t5); s.t5_t3 = w.take<uint2>(s.cap_t5);
   s.t5_chi2 = w.take<double>(s.cap_t5); s.t5_etaphi = w.take<double2>(s.cap_t5);
   s.t5_f = w.take<float4>(s.cap_t5); s.t5_pt = w.take<float>(s.cap_t5); s.t5_keep = w.take<uint8_t>(s.cap_t5);
+  s.t5_md_off = w.take<uint32_t>((size_t)s.cap_md + 1);
   s.pt5_po = w.take<uint2>(s.cap_pt5); s.pt3_po = w.take<uint2>(s.cap_pt3);
   s.pt5_chi2 = w.take<double>(s.cap_pt5); s.pt3_chi2 = w.take<double>(s.cap_pt3);
   s.pt5_keep = w.take<uint8_t>(s.cap_pt5); s.pt3_keep = w.take<uint8_t>(s.cap_pt3);
   s.pls_keep = w.take<uint8_t>(nsd);
+  s.px_cnt = w.take<uint32_t>(nsd);
+  s.px_off = w.take<uint32_t>((size_t)nsd + 1); s.px_pair = w.take<uint2>((size_t)nsd * kPxCap);
+  s.pt5_pls_off = w.take<uint32_t>((size_t)nsd + 1); s.pt3_pls_off = w.take<uint32_t>((size_t)nsd + 1);
+  s.t5_hits = w.take<uint32_t>(10 * (size_t)s.cap_t5); s.pt3_hits = w.take<uint32_t>(6 * (size_t)s.cap_pt3);
+  s.inc_cnt = w.take<uint32_t>(2 * ((size_t)nh + 1)); s.inc_cur = s.inc_cnt ? s.inc_cnt + nh + 1 : nullptr;
+  s.inc_off = w.take<uint32_t>((size_t)nh + 1);
+  s.inc_ent = w.take<uint32_t>(10 * (size_t)s.cap_t5 + 10 * (size_t)s.cap_pt5 + 6 * (size_t)s.cap_pt3);
+  s.pls_bin_off = w.take<uint32_t>(kEtaBins + 1); s.pls_bin_ent = w.take<uint32_t>(nsd);
+  s.pls_adj_cnt = w.take<uint32_t>(nsd); s.pls_adj = w.take<uint32_t>((size_t)nsd * kAdjCap);
+  s.pls_has5 = w.take<uint8_t>(3 * (size_t)nsd);
+  s.pls_has3 = s.pls_has5 ? s.pls_has5 + nsd : nullptr; s.pls_near_t5 = s.pls_has5 ? s.pls_has5 + 2 * (size_t)nsd : nullptr;
   s.tc_to = w.take<uint2>(s.cap_tc); s.tc_f = w.take<float4>(s.cap_tc);
+  s.tc_flag = w.take<uint32_t>((size_t)s.cap_tc + 1); s.tc_pos = w.take<uint32_t>((size_t)s.cap_tc + 1);
+  s.scan_part = w.take<uint32_t>(kScanBlocks + 2);
   // work lists
   const uint32_t cand_cap[S_NSTAGE] = {
       capf(cf.cap_mdcand_per_hit, nh, 1 << 16), capf(cf.cap_lscand_per_hit, nh, 1 << 16),
       capf(cf.cap_t3cand_per_hit, nh, 1 << 16), capf(cf.cap_t5cand_per_hit, nh, 1 << 16),
       capf(2048.0f, nsd, 1 << 16), capf(4096.0f, nsd, 1 << 16)};
+  const uint32_t pair_groups = (uint32_t)(((size_t)nsd * kPxCap) / kRowChunk + 2);
   const uint32_t grp_cap[S_NSTAGE] = {n_mod, n_mod, s.cap_ls / kRowChunk + 2, s.cap_t3 / kRowChunk + 2,
-                                      nsd / kRowChunk + 2, nsd / kRowChunk + 2};
+                                      pair_groups, pair_groups};
   for (int k = 0; k < S_NSTAGE; ++k) {
     StageBuf &b = s.st[k];
     b.cap_groups = grp_cap[k];
@@ -333,6 +355,11 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   lst_ctx *c = new (std::nothrow) lst_ctx();
   if (!c) return LST_ENOMEM;
   if (cfg_in) c->cfg = *cfg_in; else lst_default_config(&c->cfg);
+  if (c->cfg.dup_t5_shared < 1 || c->cfg.dup_pt5_shared < 1 || c->cfg.dup_pt3_shared < 1 || !(c->cfg.pt_min > 0.0) ||
+      !(c->cfg.dr2max >= 0.0)) {
+    delete c;
+    return LST_EINVAL;
+  }
   make_params(c->cfg, &c->k.par);
   c->n_slots = n_slots; c->max_hits = max_hits; c->max_seeds = max_seeds;
   int dev = 0;
@@ -341,10 +368,18 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaGetDeviceProperties"); }
   c->k.n_sm = prop.multiProcessorCount;
-  // static data: category | layer | map_off | map_cols
-  const size_t o_cat = 0, o_lay = (n + 255) & ~(size_t)255, o_off = o_lay + ((n + 255) & ~(size_t)255);
-  const size_t o_cols = o_off + (((size_t)(n + 1) * 4 + 255) & ~(size_t)255);
-  const size_t total = o_cols + (size_t)std::max<uint32_t>(nnz, 1) * 4;
+  // modules that may start a pixel-seeded object (C6 START layers)
+  std::vector<uint32_t> start_mods;
+  for (uint32_t m = 0; m < n; ++m)
+    if ((c->cfg.start_layer_mask >> g->logical_layer[m]) & 1u) start_mods.push_back(m);
+  // static data: category | layer | map_off | map_cols | 6 box arrays | start modules
+  const auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
+  const size_t o_cat = 0, o_lay = up(n), o_off = o_lay + up(n);
+  const size_t o_cols = o_off + up((size_t)(n + 1) * 4);
+  const size_t o_box = o_cols + up((size_t)std::max<uint32_t>(nnz, 1) * 4);
+  const size_t box_stride = up((size_t)n * 4);
+  const size_t o_start = o_box + 6 * box_stride;
+  const size_t total = o_start + std::max<size_t>(start_mods.size(), 1) * 4;
   e = cudaMalloc(&c->d_static, total);
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaMalloc(static)"); }
   char *d = (char *)c->d_static;
@@ -352,6 +387,10 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   cudaMemcpy(d + o_lay, g->logical_layer, n, cudaMemcpyHostToDevice);
   cudaMemcpy(d + o_off, map->row_offsets, (size_t)(n + 1) * 4, cudaMemcpyHostToDevice);
   if (nnz) cudaMemcpy(d + o_cols, map->cols, (size_t)nnz * 4, cudaMemcpyHostToDevice);
+  const float *box[6] = {g->rmin, g->rmax, g->phic, g->half_phi, g->zmin, g->zmax};
+  for (int k = 0; k < 6; ++k) cudaMemcpy(d + o_box + k * box_stride, box[k], (size_t)n * 4, cudaMemcpyHostToDevice);
+  if (!start_mods.empty())
+    cudaMemcpy(d + o_start, start_mods.data(), start_mods.size() * 4, cudaMemcpyHostToDevice);
   e = cudaDeviceSynchronize();
   if (e != cudaSuccess) { cudaFree(c->d_static); delete c; return cuda_fail(e, "upload geometry"); }
   c->k.geo.n_modules = n; c->k.geo.n_det = 2 * n;
@@ -359,6 +398,11 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   c->k.geo.layer = (const uint8_t *)(d + o_lay);
   c->k.geo.map_off = (const uint32_t *)(d + o_off);
   c->k.geo.map_cols = (const uint32_t *)(d + o_cols);
+  c->k.geo.rmin = (const float *)(d + o_box); c->k.geo.rmax = (const float *)(d + o_box + box_stride);
+  c->k.geo.phic = (const float *)(d + o_box + 2 * box_stride); c->k.geo.hphi = (const float *)(d + o_box + 3 * box_stride);
+  c->k.geo.zmin = (const float *)(d + o_box + 4 * box_stride); c->k.geo.zmax = (const float *)(d + o_box + 5 * box_stride);
+  c->k.geo.start_mods = (const uint32_t *)(d + o_start);
+  c->k.geo.n_start = (uint32_t)start_mods.size();
   for (int l = 0; l < 16; ++l) {
     c->k.lay_rmin[l] = INFINITY; c->k.lay_rmax[l] = 0.f; c->k.lay_zmin[l] = INFINITY; c->k.lay_zmax[l] = -INFINITY;
   }
@@ -397,7 +441,10 @@ extern "C" size_t lst_workspace_bytes(const lst_ctx *c) { return c ? c->ws_bytes
 
 extern "C" int lst_bind_workspace(lst_ctx *c, uint32_t slot, void *workspace, size_t bytes) {
   if (!c || slot >= c->n_slots || !workspace || ((uintptr_t)workspace & 255)) return LST_EINVAL;
-  if (bytes < c->ws_bytes) return LST_ENOMEM;
+  if (bytes < c->ws_bytes) {
+    snprintf(g_cap_err, sizeof(g_cap_err), "workspace too small: %zu bytes given, %zu needed", bytes, c->ws_bytes);
+    return LST_ENOMEM;
+  }
   Slot &s = c->slots[slot];
   if (s.graph) { cudaGraphExecDestroy(s.graph); s.graph = nullptr; }
   carve(c, workspace, &s.dev);
@@ -493,7 +540,15 @@ static int sync_header(lst_ctx *c, Slot &s) {
   CU(cudaMemcpyAsync(s.h_hdr, s.dev.hdr, sizeof(Header), cudaMemcpyDeviceToHost, s.last_stream));
   CU(cudaStreamSynchronize(s.last_stream));
   if (s.h_hdr->err & ERR_DET) return LST_EINVAL;
-  if (s.h_hdr->err & (ERR_CAP_ITEMS | ERR_CAP_OBJ)) return LST_ENOMEM;
+  if (s.h_hdr->err & (ERR_CAP_ITEMS | ERR_CAP_OBJ | ERR_CAP_PIX)) {
+    const Header &h = *s.h_hdr;
+    snprintf(g_cap_err, sizeof(g_cap_err),
+             "capacity exceeded:%s%s%s (objects MD %u LS %u T3 %u T5 %u pT3 %u pT5 %u; raise lst_config.cap_*)",
+             (h.err & ERR_CAP_ITEMS) ? " work items" : "", (h.err & ERR_CAP_OBJ) ? " object array" : "",
+             (h.err & ERR_CAP_PIX) ? " per-seed list" : "", h.n_obj[0], h.n_obj[1], h.n_obj[2], h.n_obj[3], h.n_obj[4],
+             h.n_obj[5]);
+    return LST_ENOMEM;
+  }
   return LST_OK;
 }
 

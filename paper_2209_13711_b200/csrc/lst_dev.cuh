@@ -23,13 +23,20 @@ constexpr int kItemWords = kItemCand / 32;
 constexpr int kThreads = 128;            // threads per block of eval / fill kernels
 constexpr int kRowChunk = 128;           // rows per group in the variable-width stages (T3, T5, pixel)
 constexpr int kMaxDeg = 512;             // maximum module-map degree (checked by lst_create)
+constexpr int kPxCap = 64;               // (seed, start module) rows per pixel seed ON AVERAGE (overflow -> LST_ENOMEM)
+constexpr int kAdjCap = 32;              // related pixel seeds per pixel seed (overflow -> LST_ENOMEM)
+constexpr int kEtaBins = 2048;           // eta bins of the pixel-seed lookup used by the cleaning
+constexpr int kScanBlocks = 128;         // blocks of the two-pass device-wide scan
+constexpr int kScanThreads = 512;
+constexpr int kPairLevel = 7;            // Header::n_obj slot that holds the (seed, module) pair count
 
 enum Stage { S_MD = 0, S_LS, S_T3, S_T5, S_PT5, S_PT3, S_NSTAGE };
 
 enum ErrBits {
   ERR_DET = 1u << 0,        // det id out of range
   ERR_CAP_ITEMS = 1u << 1,  // a work list overflowed
-  ERR_CAP_OBJ = 1u << 2     // an object array overflowed
+  ERR_CAP_OBJ = 1u << 2,    // an object array overflowed
+  ERR_CAP_PIX = 1u << 3     // a per-seed list (compatible modules / related seeds) overflowed
 };
 
 struct Item {            // 16 bytes
@@ -41,10 +48,12 @@ struct Item {            // 16 bytes
 
 struct Header {          // per slot, device; zeroed (except n_hits / n_seeds) at the start of lst_run
   uint32_t n_hits, n_seeds;
-  uint32_t n_obj[8];                 // indexed by lst_level
+  uint32_t n_obj[8];                 // indexed by lst_level; [kPairLevel] = (seed, module) pairs
   uint32_t n_items[S_NSTAGE];
   uint32_t n_groups[S_NSTAGE];
   uint32_t err;
+  uint32_t n_dd;                     // T5 + pT5 + pT3 objects entering the cleaning
+  uint32_t n_flag;                   // pT5 + pT3 + T5 + seeds: length of the TC keep-flag array
   uint32_t pad;
   unsigned long long cand[S_NSTAGE]; // candidates enumerated per stage
 };
@@ -64,6 +73,10 @@ struct GeoDev {
   uint32_t n_modules, n_det;
   const uint8_t *category, *layer;
   const uint32_t *map_off, *map_cols;
+  // boxes of the lower sensors (lst_geometry) and the modules that may start a pT3 / pT5 (C6)
+  const float *rmin, *rmax, *phic, *hphi, *zmin, *zmax;
+  const uint32_t *start_mods;
+  uint32_t n_start;
 };
 
 // All per-slot arrays (device pointers into the caller's workspace).
@@ -103,10 +116,26 @@ struct SlotDev {
   float4 *t5_f;          // R, chi2, k3a, k3b
   float *t5_pt;
   uint8_t *t5_keep;
+  uint32_t *t5_md_off;   // [cap_md+1] T5 range of a first MD
   // pixel-seeded
   uint2 *pt5_po, *pt3_po;          // pls, obj
   double *pt5_chi2, *pt3_chi2;
   uint8_t *pt5_keep, *pt3_keep, *pls_keep;
+  uint32_t *px_cnt;                // [cap_seeds] compatible start modules of a seed
+  uint32_t *px_off;                // [cap_seeds+1]
+  uint2 *px_pair;                  // [cap_seeds * kPxCap] (seed, module), ascending: rows of the pixel joins
+  uint32_t *pt5_pls_off, *pt3_pls_off;   // [cap_seeds+1] pT5 / pT3 range of a seed
+  // a6 cleaning
+  uint32_t *t5_hits, *pt3_hits;    // [10 cap_t5], [6 cap_pt3] sorted hit positions in layer order
+  uint32_t *inc_cnt, *inc_cur;     // [cap_hits+1] each, contiguous: hit -> objects incidence
+  uint32_t *inc_off;               // [cap_hits+1]
+  uint32_t *inc_ent;               // [10 cap_t5 + 10 cap_pt5 + 6 cap_pt3] object ids (T5 | pT5 | pT3)
+  uint32_t *pls_bin_off;           // [kEtaBins+1]
+  uint32_t *pls_bin_ent;           // [cap_seeds]
+  uint32_t *pls_adj_cnt, *pls_adj; // [cap_seeds], [cap_seeds * kAdjCap]: related seeds (bit 31: close in eta-phi)
+  uint8_t *pls_has5, *pls_has3, *pls_near_t5;   // [cap_seeds] each, contiguous
+  uint32_t *tc_flag, *tc_pos;      // [cap_tc+1]
+  uint32_t *scan_part;             // [kScanBlocks+2]: block partials, total; last word = ticket
   // TC
   uint2 *tc_to;                    // type, obj
   float4 *tc_f;                    // pt, eta, phi, type

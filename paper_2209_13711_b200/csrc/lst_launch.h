@@ -17,12 +17,15 @@ void launch_index(const Ctx &c, const SlotDev &s, cudaStream_t st);             
 void launch_emit(const Ctx &c, const SlotDev &s, int stage, int rows_level, cudaStream_t st);
 void launch_scan_items(const Ctx &c, const SlotDev &s, int stage, int level, uint32_t cap, cudaStream_t st);
 void launch_row_offsets(const Ctx &c, const SlotDev &s, int kind, cudaStream_t st);
+void launch_scan(const Ctx &c, const SlotDev &s, const uint32_t *in, uint32_t *out, const uint32_t *n_ptr,
+                 cudaStream_t st);                                                        // 2 kernels
 // k_mdls.cu
 void launch_md(const Ctx &c, const SlotDev &s, cudaStream_t st);
 void launch_ls(const Ctx &c, const SlotDev &s, cudaStream_t st);
 // k_t3t5.cu
 void launch_t3(const Ctx &c, const SlotDev &s, cudaStream_t st);
 void launch_t5(const Ctx &c, const SlotDev &s, cudaStream_t st);
+void launch_join(const Ctx &c, const SlotDev &s, int kind, cudaStream_t st);   // 0 T3, 1 T5, 2 pT5, 3 pT3
 // k_pix.cu
 void launch_pixel(const Ctx &c, const SlotDev &s, cudaStream_t st);
 // k_dedup.cu

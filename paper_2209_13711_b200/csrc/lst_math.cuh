@@ -33,6 +33,9 @@ struct Params {
   float f_sig_t[4], f_sig_z[4], f_sig_r[4];
   int dup_t5, dup_pt5, dup_pt3, s0_enabled;
   uint32_t start_mask;
+  // eta binning of the pixel seeds used by the cleaning (k_dedup.cu)
+  double eta_bin_inv, dr_eta_pre;
+  int eta_nbins;
 };
 
 LST_HD bool is_endcap(int cat) { return cat >= 2; }

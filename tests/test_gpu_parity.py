@@ -192,3 +192,117 @@ def test_device_resident_input_and_graph_replay(B, geom_barrel, map_barrel):
             for lvl in CHAIN:
                 compare_level(o, lst, lvl)
         lst.close()
+
+
+# ------------------------------------------------------------------ a5 / a6: pixel linking, cleaning, TC
+PAD = 0xFFFFFFFF
+
+
+def _oracle_tc_keys(o, ev):
+    """(type, 10 OT hits padded, 4 pixel ids) of every oracle TC entry, in TC order."""
+    tc = o.get(O.TC)
+    objs = {lvl: o.get(lvl) for lvl in (O.T5, O.PT3, O.PT5)}
+    ids = ev.seed_hit_ids.astype(np.int64)
+    keys = []
+    for t, i in tc["parents"].tolist():
+        ot, pix = [PAD] * 10, [PAD] * 4
+        if t == O.TC:
+            pix = ids[i].tolist()
+        else:
+            h = objs[t]["hits"][i].tolist()
+            ot[:len(h)] = h
+            if t != O.T5:
+                pix = ids[objs[t]["parents"][i, 0]].tolist()
+        keys.append((t, *ot, *pix))
+    return keys, tc
+
+
+def compare_cleaning(o, lst, ev):
+    # keep flags, object by object
+    for lvl in (O.T5, O.PT3, O.PT5):
+        ref, got = o.get(lvl), lst.lst_get_objects(0, lvl)
+        kr = dict(zip(_keys(lvl, ref), o.keep(lvl).tolist()))
+        kg = dict(zip(_keys(lvl, got), got["keep"].tolist()))
+        assert kr == kg, "keep flags differ at level %s" % O.LEVEL_NAMES[lvl]
+    keys_o, tc_o = _oracle_tc_keys(o, ev)
+    got = lst.lst_get_objects(0, O.TC)
+    keys_g = [(int(p[0]), *h) for p, h in zip(got["parents"].tolist(), got["hits"].astype(np.int64).tolist())]
+    assert keys_g == keys_o                       # same candidates in the same (canonical) order
+    f_o, f_g = tc_o["f"], got["f"].astype(np.float64)
+    assert np.allclose(f_g, f_o, rtol=REL, atol=1e-6)
+    return len(keys_o)
+
+
+def _chain_with_pixels(B, geom, mp, ev, brute=False):
+    o = O.Oracle(geom, mp[0], mp[1])
+    o.load(ev)
+    o.run(upto=O.TC, brute=brute)
+    lst = _gpu(B, geom, mp, ev)
+    near = 0
+    for lvl in (O.MD, O.LS, O.T3, O.T5, O.PT3, O.PT5):
+        n, nr, ref, got = compare_level(o, lst, lvl)
+        assert n == o.count(lvl)
+        near += nr
+    return o, lst, near
+
+
+def test_pixel_linking_and_cleaning_small_brute(B, geom_barrel, map_barrel):
+    """Config 2 + seeds against the oracle's all-pairs definitions (module-map, joins, S0 all brute)."""
+    ev = lstgen.make_event(geom_barrel, "cfg2s")
+    assert ev.n_seeds > 50
+    o, lst, near = _chain_with_pixels(B, geom_barrel, map_barrel, ev, brute=True)
+    assert o.count(O.PT5) > 20 and o.count(O.PT3) > 20
+    if near == 0:
+        assert compare_cleaning(o, lst, ev) > 10
+    lst.close()
+
+
+def test_config4_pixel_linking_cleaning_tc(B, geom_full, map_full):
+    ev = lstgen.make_event(geom_full, "cfg4")
+    assert ev.n_seeds > 1000
+    o, lst, near = _chain_with_pixels(B, geom_full, map_full, ev)
+    assert o.count(O.PT5) > 1000 and o.count(O.PT3) > 1000
+    if near == 0:
+        n_tc = compare_cleaning(o, lst, ev)
+        assert n_tc > 1000
+        # survivors of DIFFERENT collections share no outer-tracker hits (PAPER.md:77)
+        got = lst.lst_get_objects(0, O.TC)
+        ot, typ = got["hits"][:, :10].astype(np.int64), got["parents"][:, 0]
+        used = {t: set(ot[typ == t][ot[typ == t] != PAD].tolist()) for t in (O.T5, O.PT3, O.PT5)}
+        assert not (used[O.T5] & used[O.PT5]) and not (used[O.T5] & used[O.PT3]) and not (used[O.PT3] & used[O.PT5])
+    lst.close()
+
+
+def test_config4h_seed_subset(B, geom_full, map_full):
+    """PU200-like occupancy (config 4, 13 500 particles) with the first 500 seeds: the oracle's
+    all-pairs pixel linking over every seed would take minutes."""
+    import dataclasses
+    ev = lstgen.make_event(geom_full, "cfg4h")
+    k = 500
+    ev = dataclasses.replace(ev, seed_pt=ev.seed_pt[:k], seed_eta=ev.seed_eta[:k], seed_phi=ev.seed_phi[:k],
+                             seed_z0=ev.seed_z0[:k], seed_q=ev.seed_q[:k], seed_hit_ids=ev.seed_hit_ids[:k],
+                             seed_pid=ev.seed_pid[:k])
+    o, lst, near = _chain_with_pixels(B, geom_full, map_full, ev)
+    if near == 0:
+        assert compare_cleaning(o, lst, ev) > 1000
+    lst.close()
+
+
+def test_cleaning_without_s0_and_without_seeds(B, geom_barrel, map_barrel):
+    # no seeds: TC = cleaned T5
+    ev = lstgen.make_event(geom_barrel, "cfg2")
+    o = _oracle(geom_barrel, map_barrel, ev, O.TC)
+    lst = _gpu(B, geom_barrel, map_barrel, ev)
+    assert compare_cleaning(o, lst, ev) > 10
+    lst.close()
+    # S0 switched off on both sides
+    ev = lstgen.make_event(geom_barrel, "cfg2s")
+    cfg_o, cfg_g = O.default_config(), B.lst_default_config()
+    cfg_o.s0_enabled = 0
+    cfg_g.s0_enabled = 0
+    o = O.Oracle(geom_barrel, map_barrel[0], map_barrel[1], cfg_o)
+    o.load(ev)
+    o.run(upto=O.TC)
+    lst = _gpu(B, geom_barrel, map_barrel, ev, cfg=cfg_g)
+    assert compare_cleaning(o, lst, ev) > 10
+    lst.close()
