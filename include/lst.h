@@ -180,8 +180,18 @@ int lst_get_objects(lst_ctx *ctx, uint32_t slot, lst_level level, int copy_to_ho
  * MD, LS, T3, T5 (uint64[4]). */
 int lst_get_counts(lst_ctx *ctx, uint32_t slot, uint32_t *counts, uint64_t *cand);
 
-/* Number of kernels one lst_run launches (for launch accounting in benchmarks). */
+/* Number of kernels the last lst_run / lst_run_timed of this context enqueued (or captured into
+ * its graph); 0 before the first run.  For launch accounting in benchmarks. */
 uint32_t lst_launches_per_run(const lst_ctx *ctx);
+
+/* Measurement aid (per-kernel ms): the same chain as lst_run, launched without a
+ * CUDA graph with one CUDA event after every kernel, then synchronised.  names[k] (HOST array of
+ * max_kernels pointers to static strings, may be NULL) and ms[k] (HOST, may be NULL) receive the
+ * kernel name and its duration on the stream (launch gap included); *n_kernels the number of
+ * kernels in the chain (may exceed max_kernels; only max_kernels entries are written).
+ * The objects it leaves in the slot are those of lst_run. */
+int lst_run_timed(lst_ctx *ctx, uint32_t slot, void *cuda_stream, uint32_t max_kernels, const char **names,
+                  float *ms, uint32_t *n_kernels);
 
 const char *lst_strerror(int status);
 

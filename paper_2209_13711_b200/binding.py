@@ -22,7 +22,7 @@ LEVEL_NAMES = ("MD", "LS", "T3", "T5", "PT3", "PT5", "TC")
 
 EXPORTS = ("lst_default_config", "lst_build_module_map", "lst_free", "lst_create", "lst_destroy",
            "lst_workspace_bytes", "lst_bind_workspace", "lst_load_event", "lst_run", "lst_get_objects",
-           "lst_get_counts", "lst_launches_per_run", "lst_strerror", "lst_host_eval")
+           "lst_get_counts", "lst_launches_per_run", "lst_run_timed", "lst_strerror", "lst_host_eval")
 
 
 class lst_config(C.Structure):
@@ -99,6 +99,7 @@ def lib():
         L.lst_get_counts.argtypes = [vp, u32, vp, vp]
         L.lst_launches_per_run.argtypes = [vp]
         L.lst_launches_per_run.restype = u32
+        L.lst_run_timed.argtypes = [vp, u32, vp, u32, vp, vp, C.POINTER(u32)]
         L.lst_strerror.argtypes = [C.c_int]
         L.lst_strerror.restype = C.c_char_p
         L.lst_host_eval.argtypes = [C.POINTER(lst_config), C.c_int, u32, vp, vp, vp, vp, vp, vp]
@@ -234,6 +235,17 @@ class LST:
 
     def lst_run(self, slot, stream=None):
         _check(lib().lst_run(self._h, slot, self._stream_ptr(stream)), "lst_run")
+
+    def lst_run_timed(self, slot, stream=None):
+        """-> list of (kernel name, ms) of one un-graphed, event-bracketed pass of the chain."""
+        cap = 96
+        names = (C.c_char_p * cap)()
+        ms = np.zeros(cap, np.float32)
+        n = C.c_uint32(0)
+        _check(lib().lst_run_timed(self._h, slot, self._stream_ptr(stream), cap, C.cast(names, C.c_void_p), _p(ms),
+                                   C.byref(n)), "lst_run_timed")
+        k = min(int(n.value), cap)
+        return [(names[i].decode(), float(ms[i])) for i in range(k)]
 
     def lst_get_counts(self, slot):
         cnt = np.zeros(LST_NLEVEL, np.uint32)

@@ -227,32 +227,34 @@ static inline int grid_for(uint32_t n, int threads, int max_blocks) {
 
 void launch_index(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   cudaMemsetAsync(s.det_cnt, 0, sizeof(uint32_t) * (c.geo.n_det + 1), st);
-  k_begin<<<1, 32, 0, st>>>(s);
+  k_begin<<<1, 32, 0, st>>>(s); LST_MARK(c, st, "k_begin");
   const int g = grid_for(s.cap_hits, 256, c.n_sm * 8);
-  k_hist<<<g, 256, 0, st>>>(c.geo, s);
-  k_det_scan<<<1, 1024, 0, st>>>(c.geo, s);
-  k_scatter<<<g, 256, 0, st>>>(c.geo, s);
-  k_rank<<<g, 256, 0, st>>>(c.geo, s);
+  k_hist<<<g, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_hist");
+  k_det_scan<<<1, 1024, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_det_scan");
+  k_scatter<<<g, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_scatter");
+  k_rank<<<g, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_rank");
 }
 
+static const char *const kEmitName[S_NSTAGE] = {"k_emit_items[MD]", "k_emit_items[LS]", "k_emit_items[T3]",
+                                                  "k_emit_items[T5]", "k_emit_items[pT5]", "k_emit_items[pT3]"};
+static const char *const kScanName[S_NSTAGE] = {"k_scan_items[MD]", "k_scan_items[LS]", "k_scan_items[T3]",
+                                                  "k_scan_items[T5]", "k_scan_items[pT5]", "k_scan_items[pT3]"};
 void launch_emit(const Ctx &c, const SlotDev &s, int stage, int rows_level, cudaStream_t st) {
-  (void)c;
-  k_emit_items<<<1, 1024, 0, st>>>(s, stage, rows_level);
+  k_emit_items<<<1, 1024, 0, st>>>(s, stage, rows_level); LST_MARK(c, st, kEmitName[stage]);
 }
 void launch_scan_items(const Ctx &c, const SlotDev &s, int stage, int level, uint32_t cap, cudaStream_t st) {
-  (void)c;
-  k_scan_items<<<1, 1024, 0, st>>>(s, stage, level, cap);
+  k_scan_items<<<1, 1024, 0, st>>>(s, stage, level, cap); LST_MARK(c, st, kScanName[stage]);
 }
 void launch_row_offsets(const Ctx &c, const SlotDev &s, int kind, cudaStream_t st) {
   const uint32_t caps[6] = {s.cap_md, s.cap_ls, s.cap_t3, s.cap_t5, s.cap_pt5, s.cap_pt3};
   const int g = grid_for(caps[kind], 256, c.n_sm * 4);
   switch (kind) {
-    case 0: k_row_offsets<0><<<g, 256, 0, st>>>(c.geo, s); break;
-    case 1: k_row_offsets<1><<<g, 256, 0, st>>>(c.geo, s); break;
-    case 2: k_row_offsets<2><<<g, 256, 0, st>>>(c.geo, s); break;
-    case 3: k_row_offsets<3><<<g, 256, 0, st>>>(c.geo, s); break;
-    case 4: k_row_offsets<4><<<g, 256, 0, st>>>(c.geo, s); break;
-    default: k_row_offsets<5><<<g, 256, 0, st>>>(c.geo, s); break;
+    case 0: k_row_offsets<0><<<g, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_row_offsets[MD]"); break;
+    case 1: k_row_offsets<1><<<g, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_row_offsets[LS]"); break;
+    case 2: k_row_offsets<2><<<g, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_row_offsets[T3]"); break;
+    case 3: k_row_offsets<3><<<g, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_row_offsets[T5]"); break;
+    case 4: k_row_offsets<4><<<g, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_row_offsets[pT5]"); break;
+    default: k_row_offsets<5><<<g, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_row_offsets[pT3]"); break;
   }
 }
 
@@ -303,9 +305,8 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t *in,
 }
 void launch_scan(const Ctx &c, const SlotDev &s, const uint32_t *in, uint32_t *out, const uint32_t *n_ptr,
                  cudaStream_t st) {
-  (void)c;
-  k_scan_sums<<<kScanBlocks, kScanThreads, 0, st>>>(in, n_ptr, s.scan_part);
-  k_scan_apply<<<kScanBlocks, kScanThreads, 0, st>>>(in, n_ptr, s.scan_part, out);
+  k_scan_sums<<<kScanBlocks, kScanThreads, 0, st>>>(in, n_ptr, s.scan_part); LST_MARK(c, st, "k_scan_sums");
+  k_scan_apply<<<kScanBlocks, kScanThreads, 0, st>>>(in, n_ptr, s.scan_part, out); LST_MARK(c, st, "k_scan_apply");
 }
 
 }  // namespace lst

@@ -354,17 +354,17 @@ void launch_dedup(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   const uint32_t cap_dd = s.cap_t5 + s.cap_pt5 + s.cap_pt3;
   cudaMemsetAsync(s.inc_cnt, 0, sizeof(uint32_t) * 2 * ((size_t)s.cap_hits + 1), st);
   cudaMemsetAsync(s.pls_has5, 0, 3 * (size_t)s.cap_seeds, st);
-  k_pls_prep<<<1, 1024, 0, st>>>(s, c.par);
-  k_pls_adj<<<grid_of(s.cap_seeds, 8, c.n_sm * 8), 256, 0, st>>>(s, c.par);
-  k_dd_count<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s);
+  k_pls_prep<<<1, 1024, 0, st>>>(s, c.par); LST_MARK(c, st, "k_pls_prep");
+  k_pls_adj<<<grid_of(s.cap_seeds, 8, c.n_sm * 8), 256, 0, st>>>(s, c.par); LST_MARK(c, st, "k_pls_adj");
+  k_dd_count<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_dd_count");
   launch_scan(c, s, s.inc_cnt, s.inc_off, &s.hdr->n_hits, st);
-  k_dd_scatter<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s);
-  k_s0<<<grid_of(cap_dd, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par);
-  k_s1<<<grid_of(s.cap_pt3, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par);
-  k_s2<<<grid_of(s.cap_t5, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par);
-  k_s3_flags<<<grid_of(s.cap_tc, 256, c.n_sm * 8), 256, 0, st>>>(s);
+  k_dd_scatter<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_dd_scatter");
+  k_s0<<<grid_of(cap_dd, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s0");
+  k_s1<<<grid_of(s.cap_pt3, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s1");
+  k_s2<<<grid_of(s.cap_t5, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s2");
+  k_s3_flags<<<grid_of(s.cap_tc, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_s3_flags");
   launch_scan(c, s, s.tc_flag, s.tc_pos, &s.hdr->n_flag, st);
-  k_tc_fill<<<grid_of(s.cap_tc, 256, c.n_sm * 8), 256, 0, st>>>(s);
+  k_tc_fill<<<grid_of(s.cap_tc, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_tc_fill");
 }
 
 }  // namespace lst

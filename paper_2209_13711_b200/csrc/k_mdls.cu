@@ -237,18 +237,18 @@ static inline int persistent_grid(const Ctx &c, int per_sm) { return c.n_sm * pe
 
 void launch_md(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   launch_emit(c, s, S_MD, -1, st);
-  k_md_eval<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par);
+  k_md_eval<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_md_eval");
   launch_scan_items(c, s, S_MD, 0, s.cap_md, st);
-  k_md_fill<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par);
+  k_md_fill<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_md_fill");
   launch_row_offsets(c, s, 0, st);
 }
 
 void launch_ls(const Ctx &c, const SlotDev &s, cudaStream_t st) {
-  k_ls_groups<<<(c.geo.n_modules + 127) / 128, 128, 0, st>>>(c.geo, s);
+  k_ls_groups<<<(c.geo.n_modules + 127) / 128, 128, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_ls_groups");
   launch_emit(c, s, S_LS, -1, st);
-  k_ls_eval<<<persistent_grid(c, 5), kThreads, 0, st>>>(c.geo, s, c.par);
+  k_ls_eval<<<persistent_grid(c, 5), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_ls_eval");
   launch_scan_items(c, s, S_LS, 1, s.cap_ls, st);
-  k_ls_fill<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par);
+  k_ls_fill<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_ls_fill");
   launch_row_offsets(c, s, 1, st);
 }
 

@@ -107,9 +107,9 @@ void launch_pixel(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   const int warps_per_block = 8;
   int g = (int)((s.cap_seeds + warps_per_block - 1) / warps_per_block);
   if (g > c.n_sm * 8) g = c.n_sm * 8;
-  k_px_modules<false><<<g, 256, 0, st>>>(c.geo, s, c.par);
-  k_px_offsets<<<1, 1024, 0, st>>>(s);
-  k_px_modules<true><<<g, 256, 0, st>>>(c.geo, s, c.par);
+  k_px_modules<false><<<g, 256, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_px_modules<false>");
+  k_px_offsets<<<1, 1024, 0, st>>>(s); LST_MARK(c, st, "k_px_offsets");
+  k_px_modules<true><<<g, 256, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_px_modules<true>");
   launch_join(c, s, 2, st);            // pT5
   launch_row_offsets(c, s, 4, st);
   launch_join(c, s, 3, st);            // pT3

@@ -22,10 +22,18 @@ struct RowTab {                       // right-list table of one group, in share
 enum { J_T3 = 0, J_T5 = 1, J_PT5 = 2, J_PT3 = 3 };
 
 template <int KIND> struct JoinTraits;
-template <> struct JoinTraits<J_T3> { static constexpr int stage = S_T3, rows_level = 1, out_level = 2; };
-template <> struct JoinTraits<J_T5> { static constexpr int stage = S_T5, rows_level = 2, out_level = 3; };
-template <> struct JoinTraits<J_PT5> { static constexpr int stage = S_PT5, rows_level = kPairLevel, out_level = 5; };
-template <> struct JoinTraits<J_PT3> { static constexpr int stage = S_PT3, rows_level = kPairLevel, out_level = 4; };
+template <> struct JoinTraits<J_T3> {
+  static constexpr const char *n_groups = "k_join_groups[T3]", *n_eval = "k_join_eval[T3]", *n_fill = "k_join_fill[T3]";
+  static constexpr int stage = S_T3, rows_level = 1, out_level = 2; };
+template <> struct JoinTraits<J_T5> {
+  static constexpr const char *n_groups = "k_join_groups[T5]", *n_eval = "k_join_eval[T5]", *n_fill = "k_join_fill[T5]";
+  static constexpr int stage = S_T5, rows_level = 2, out_level = 3; };
+template <> struct JoinTraits<J_PT5> {
+  static constexpr const char *n_groups = "k_join_groups[pT5]", *n_eval = "k_join_eval[pT5]", *n_fill = "k_join_fill[pT5]";
+  static constexpr int stage = S_PT5, rows_level = kPairLevel, out_level = 5; };
+template <> struct JoinTraits<J_PT3> {
+  static constexpr const char *n_groups = "k_join_groups[pT3]", *n_eval = "k_join_eval[pT3]", *n_fill = "k_join_fill[pT3]";
+  static constexpr int stage = S_PT3, rows_level = kPairLevel, out_level = 4; };
 
 template <int KIND>
 __device__ __forceinline__ void right_range(const SlotDev &s, uint32_t row, uint32_t *st, uint32_t *cnt) {
@@ -267,11 +275,11 @@ __global__ void __launch_bounds__(kThreads) k_join_fill(GeoDev geo, SlotDev s, P
 template <int KIND>
 static void launch_join_t(const Ctx &c, const SlotDev &s, uint32_t row_cap, uint32_t out_cap, cudaStream_t st) {
   const int gg = (int)((row_cap / kRowChunk + 1 + 3) / 4);   // 4 warps per block, one group per warp
-  k_join_groups<KIND><<<gg < c.n_sm * 8 ? gg : c.n_sm * 8, 128, 0, st>>>(s);
+  k_join_groups<KIND><<<gg < c.n_sm * 8 ? gg : c.n_sm * 8, 128, 0, st>>>(s); LST_MARK(c, st, JoinTraits<KIND>::n_groups);
   launch_emit(c, s, JoinTraits<KIND>::stage, JoinTraits<KIND>::rows_level, st);
-  k_join_eval<KIND><<<c.n_sm * 8, kThreads, 0, st>>>(c.geo, s, c.par);
+  k_join_eval<KIND><<<c.n_sm * 8, kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, JoinTraits<KIND>::n_eval);
   launch_scan_items(c, s, JoinTraits<KIND>::stage, JoinTraits<KIND>::out_level, out_cap, st);
-  k_join_fill<KIND><<<c.n_sm * 8, kThreads, 0, st>>>(c.geo, s, c.par);
+  k_join_fill<KIND><<<c.n_sm * 8, kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, JoinTraits<KIND>::n_fill);
 }
 
 void launch_join(const Ctx &c, const SlotDev &s, int kind, cudaStream_t st) {

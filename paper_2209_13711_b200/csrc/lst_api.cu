@@ -227,6 +227,9 @@ struct lst_ctx {
   std::vector<Slot> slots;
   size_t ws_bytes = 0;
   size_t exp_obj_cap = 0, exp_hit_words = 0;
+  uint32_t launches = 0;         // kernels enqueued by the last chain (graph capture or direct)
+  Recorder timed;                // lst_run_timed: events created on first use
+  bool timed_ready = false;
 };
 
 // bump allocator over the workspace; base == nullptr only measures
@@ -419,6 +422,10 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   return LST_OK;
 }
 
+static void free_timed(lst_ctx *c) {
+  if (c->timed_ready) for (int k = 0; k <= Recorder::kMax; ++k) cudaEventDestroy(c->timed.ev[k]);
+  c->timed_ready = false;
+}
 static void free_slot_host(Slot &s) {
   if (s.graph) cudaGraphExecDestroy(s.graph);
   if (s.h_hits) cudaFreeHost(s.h_hits);
@@ -433,6 +440,7 @@ extern "C" void lst_destroy(lst_ctx *c) {
   if (!c) return;
   cudaDeviceSynchronize();
   for (Slot &s : c->slots) free_slot_host(s);
+  free_timed(c);
   if (c->d_static) cudaFree(c->d_static);
   delete c;
 }
@@ -494,7 +502,15 @@ extern "C" int lst_load_event(lst_ctx *c, uint32_t slot, const lst_hits *hits, c
 }
 
 // ------------------------------------------------------------------ the chain
+static void enqueue_stages(const lst_ctx *c, const SlotDev &d, cudaStream_t st);
 static void enqueue_chain(const lst_ctx *c, const SlotDev &d, cudaStream_t st) {
+  Recorder count_only;
+  if (!c->k.rec) c->k.rec = &count_only;
+  enqueue_stages(c, d, st);
+  const_cast<lst_ctx *>(c)->launches = (uint32_t)c->k.rec->n;
+  if (c->k.rec == &count_only) c->k.rec = nullptr;
+}
+static void enqueue_stages(const lst_ctx *c, const SlotDev &d, cudaStream_t st) {
   launch_index(c->k, d, st);
   launch_md(c->k, d, st);
   launch_ls(c->k, d, st);
@@ -601,9 +617,38 @@ extern "C" int lst_get_objects(lst_ctx *c, uint32_t slot, lst_level level, int c
   return LST_OK;
 }
 
-extern "C" uint32_t lst_launches_per_run(const lst_ctx *c) {
-  (void)c;
-  return 0;
+extern "C" uint32_t lst_launches_per_run(const lst_ctx *c) { return c ? c->launches : 0; }
+
+// The chain without a graph, one CUDA event after every kernel; synchronises the stream.
+extern "C" int lst_run_timed(lst_ctx *c, uint32_t slot, void *cuda_stream, uint32_t max_kernels, const char **names,
+                             float *ms, uint32_t *n_kernels) {
+  if (!c || slot >= c->n_slots || !n_kernels) return LST_EINVAL;
+  Slot &s = c->slots[slot];
+  if (!s.bound || !s.loaded) return LST_ESTATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  Recorder &r = c->timed;
+  if (!c->timed_ready) {
+    for (int k = 0; k <= Recorder::kMax; ++k) CU(cudaEventCreate(&r.ev[k]));
+    c->timed_ready = true;
+  }
+  r.timed = true;
+  r.n = 0;
+  CU(cudaEventRecord(r.ev[0], st));
+  c->k.rec = &r;
+  enqueue_chain(c, s.dev, st);
+  c->k.rec = nullptr;
+  CU(cudaGetLastError());
+  s.ran = true; s.last_stream = st;
+  CU(cudaStreamSynchronize(st));
+  const uint32_t n = std::min<uint32_t>((uint32_t)r.n, max_kernels);
+  for (uint32_t k = 0; k < n; ++k) {
+    float t = 0.f;
+    CU(cudaEventElapsedTime(&t, r.ev[k], r.ev[k + 1]));
+    if (ms) ms[k] = t;
+    if (names) names[k] = r.name[k];
+  }
+  *n_kernels = (uint32_t)r.n;
+  return LST_OK;
 }
 
 // ------------------------------------------------------------------ host test hooks

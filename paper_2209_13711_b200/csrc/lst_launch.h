@@ -4,7 +4,27 @@
 
 namespace lst {
 
+// Launch recorder: counts the kernels a chain enqueues and, when `timed`, drops a CUDA event after
+// each one so that lst_run_timed can report per-kernel durations (bench.py, profiles/).
+struct Recorder {
+  static constexpr int kMax = 96;
+  bool timed = false;
+  int n = 0;
+  const char *name[kMax];
+  cudaEvent_t ev[kMax + 1];   // ev[0] = before the first kernel; created by the owner when timed
+};
+#define LST_MARK(ctx, stream, kname)                                                   \
+  do {                                                                                 \
+    Recorder *r_ = (ctx).rec;                                                          \
+    if (r_ && r_->n < Recorder::kMax) {                                                \
+      r_->name[r_->n] = (kname);                                                       \
+      ++r_->n;                                                                         \
+      if (r_->timed) cudaEventRecord(r_->ev[r_->n], (stream));                         \
+    }                                                                                  \
+  } while (0)
+
 struct Ctx {             // what the launchers need from a context
+  mutable Recorder *rec = nullptr;
   GeoDev geo;
   Params par;
   int n_sm;
