@@ -131,28 +131,28 @@ __global__ void k_emit_items(SlotDev s, int stage, int rows_level) {
     if (overflow) atomicOr(&hdr->err, (uint32_t)ERR_CAP_ITEMS);
   }
   if (overflow) return;
-  for (uint32_t g = threadIdx.x; g < ng; g += blockDim.x) {
+  // one thread per ITEM (a heavy module owns hundreds of items): find its group in g_item0
+  __syncthreads();
+  for (uint32_t i = threadIdx.x; i < carry; i += blockDim.x) {
+    uint32_t lo = 0, hi = ng;            // last g with g_item0[g] <= i (empty groups repeat an offset)
+    while (hi - lo > 1) {
+      const uint32_t mid = (lo + hi) >> 1;
+      if (st.g_item0[mid] <= i) lo = mid; else hi = mid;
+    }
+    const uint32_t g = lo, k = i - st.g_item0[g];
     const uint32_t R = st.gR[g], W = st.gW[g];
-    const uint32_t ni = items_of(R, W);
-    Item *out = st.items + st.g_item0[g];
-    if (ni == 0) continue;
+    Item it;
+    it.group = g;
     if (W <= (uint32_t)kItemCand) {
       const uint32_t rpi = (uint32_t)kItemCand / W;
-      for (uint32_t k = 0; k < ni; ++k) {
-        Item it;
-        it.group = g; it.i0 = k * rpi; it.j0 = 0;
-        it.nrows = (uint16_t)min(rpi, R - k * rpi); it.nj = (uint16_t)W;
-        out[k] = it;
-      }
+      it.i0 = k * rpi; it.j0 = 0;
+      it.nrows = (uint16_t)min(rpi, R - k * rpi); it.nj = (uint16_t)W;
     } else {
       const uint32_t nt = (W + kItemCand - 1) / kItemCand;
-      for (uint32_t k = 0; k < ni; ++k) {
-        Item it;
-        it.group = g; it.i0 = k / nt; it.j0 = (k % nt) * kItemCand;
-        it.nrows = 1; it.nj = (uint16_t)min((uint32_t)kItemCand, W - it.j0);
-        out[k] = it;
-      }
+      it.i0 = k / nt; it.j0 = (k % nt) * kItemCand;
+      it.nrows = 1; it.nj = (uint16_t)min((uint32_t)kItemCand, W - it.j0);
     }
+    st.items[i] = it;
   }
 }
 
@@ -213,8 +213,16 @@ __global__ void k_row_offsets(GeoDev geo, SlotDev s) {
     else if (KIND == 4) { key = s.pt5_po[k].x; prev = k ? s.pt5_po[k - 1].x + 1 : 0; }
     else { key = s.pt3_po[k].x; prev = k ? s.pt3_po[k - 1].x + 1 : 0; }
     for (uint32_t r = prev; r <= key; ++r) off[r] = k;
-    if (k == n - 1) for (uint32_t r = key + 1; r <= n_rows; ++r) off[r] = n;
   }
+  // rows after the last key (outer-layer MDs start no T3 / T5: a long tail)
+  uint32_t last;
+  if (KIND == 0) last = s.md_mod[n - 1] >> 2;
+  else if (KIND == 1) last = s.ls_md[n - 1].x;
+  else if (KIND == 2) last = s.t3_md[n - 1].x;
+  else if (KIND == 3) last = s.t5_md[5 * (size_t)(n - 1)];
+  else if (KIND == 4) last = s.pt5_po[n - 1].x;
+  else last = s.pt3_po[n - 1].x;
+  for (uint32_t r = last + 1 + tid; r <= n_rows; r += nt) off[r] = n;
 }
 
 // ------------------------------------------------------------------ host launchers

@@ -200,41 +200,73 @@ __global__ void k_dd_scatter(SlotDev s) {
 }
 
 // ------------------------------------------------------------------ S0: inside one collection
+// One WARP per object A.  An object sharing >= min_shared of A's n_ot hits contains at least one of
+// any n_ot - min_shared + 1 of them, so only the incidence lists of hits k0..n_ot-1 are searched;
+// the lists are flattened into one index space that the lanes stride (their lengths are very
+// uneven: inner-layer hits sit in hundreds of objects), and the cheap tests (type, score) come
+// before B's hit row is loaded.
+__device__ __forceinline__ double dd_score(const SlotDev &s, uint32_t n5, uint32_t np5, uint32_t d) {
+  return d < n5 ? s.t5_chi2[d] : (d < n5 + np5 ? s.pt5_chi2[d - n5] : s.pt3_chi2[d - n5 - np5]);
+}
 __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
   const Header *hdr = s.hdr;
   const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = hdr->n_dd;
-  for (uint32_t d = blockIdx.x * blockDim.x + threadIdx.x; d < n_dd; d += gridDim.x * blockDim.x) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+  for (uint32_t d = warp; d < n_dd; d += nwarp) {
     const DRef A = dd_ref(s, n5, np5, d);
     uint32_t ha[10];
 #pragma unroll
     for (int q = 0; q < 10; ++q) ha[q] = q < A.n_ot ? A.hits[q] : 0xFFFFFFFFu;
-    bool keep = true;
+    bool beaten = false;
     if (g.s0_enabled) {
       const int min_shared = A.type == 0 ? g.dup_t5 : (A.type == 1 ? g.dup_pt5 : g.dup_pt3);
-      // an object sharing >= min_shared of A's hits contains one of any n_ot - min_shared + 1 of them
       const int k0 = min_shared - 1;
-      for (int k = k0; k < A.n_ot && keep; ++k) {
-        const uint32_t h = A.hits[k];
-        for (uint32_t e = s.inc_off[h]; e < s.inc_off[h + 1]; ++e) {
-          const uint32_t b = s.inc_ent[e];
-          if (b == d || dd_type(n5, np5, b) != A.type) continue;
-          const DRef Bq = dd_ref(s, n5, np5, b);
-          if (dd_shared(ha, A.n_ot, Bq.hits, Bq.n_ot) >= min_shared && dd_beats(s, Bq, A)) { keep = false; break; }
-        }
+      uint32_t beg[10], pre[11];
+      pre[0] = 0;
+#pragma unroll
+      for (int q = 0; q < 10; ++q) {
+        uint32_t len = 0;
+        beg[q] = 0;
+        if (q >= k0 && q < A.n_ot) { beg[q] = s.inc_off[ha[q]]; len = s.inc_off[ha[q] + 1] - beg[q]; }
+        pre[q + 1] = pre[q] + len;
       }
-      if (keep && A.type != 0) {   // objects of the same pixel seed are duplicates of one another
+      const uint32_t total = pre[10];
+      for (uint32_t base = 0; base < total && !beaten; base += 32) {
+        const uint32_t i = base + lane;
+        bool hit = false;
+        if (i < total) {
+          uint32_t e = 0;
+#pragma unroll
+          for (int q = 0; q < 10; ++q)
+            if (i >= pre[q] && i < pre[q + 1]) e = beg[q] + (i - pre[q]);
+          const uint32_t b = s.inc_ent[e];
+          if (b != d && dd_type(n5, np5, b) == A.type && !(dd_score(s, n5, np5, b) > A.score)) {
+            const DRef Bq = dd_ref(s, n5, np5, b);
+            hit = dd_shared(ha, A.n_ot, Bq.hits, Bq.n_ot) >= min_shared && dd_beats(s, Bq, A);
+          }
+        }
+        beaten = __any_sync(0xffffffffu, hit);
+      }
+      if (!beaten && A.type != 0) {   // objects of the same pixel seed are duplicates of one another
         const uint32_t *off = A.type == 1 ? s.pt5_pls_off : s.pt3_pls_off;
-        const uint32_t base = A.type == 1 ? n5 : n5 + np5;
-        for (uint32_t i = off[A.pls]; i < off[A.pls + 1]; ++i) {
-          if (i == A.idx) continue;
-          const DRef Bq = dd_ref(s, n5, np5, base + i);
-          if (dd_beats(s, Bq, A)) { keep = false; break; }
+        const uint32_t dbase = A.type == 1 ? n5 : n5 + np5;
+        const uint32_t i0 = off[A.pls], i1 = off[A.pls + 1];
+        for (uint32_t base = i0; base < i1 && !beaten; base += 32) {
+          const uint32_t i = base + lane;
+          bool hit = false;
+          if (i < i1 && i != A.idx && !(dd_score(s, n5, np5, dbase + i) > A.score))
+            hit = dd_beats(s, dd_ref(s, n5, np5, dbase + i), A);
+          beaten = __any_sync(0xffffffffu, hit);
         }
       }
     }
-    if (A.type == 0) s.t5_keep[A.idx] = keep;
-    else if (A.type == 1) { s.pt5_keep[A.idx] = keep; if (keep) s.pls_has5[A.pls] = 1; }
-    else s.pt3_keep[A.idx] = keep;
+    if (lane == 0) {
+      const bool keep = !beaten;
+      if (A.type == 0) s.t5_keep[A.idx] = keep;
+      else if (A.type == 1) { s.pt5_keep[A.idx] = keep; if (keep) s.pls_has5[A.pls] = 1; }
+      else s.pt3_keep[A.idx] = keep;
+    }
   }
 }
 
@@ -359,7 +391,7 @@ void launch_dedup(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   k_dd_count<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_dd_count");
   launch_scan(c, s, s.inc_cnt, s.inc_off, &s.hdr->n_hits, st);
   k_dd_scatter<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_dd_scatter");
-  k_s0<<<grid_of(cap_dd, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s0");
+  k_s0<<<grid_of(cap_dd, 4, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s0");
   k_s1<<<grid_of(s.cap_pt3, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s1");
   k_s2<<<grid_of(s.cap_t5, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s2");
   k_s3_flags<<<grid_of(s.cap_tc, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_s3_flags");
