@@ -9,7 +9,7 @@ __global__ void k_begin(SlotDev s) {
   Header *h = s.hdr;
   const int t = threadIdx.x;
   if (t < 8) h->n_obj[t] = 0;
-  if (t < S_NSTAGE) { h->n_items[t] = 0; h->n_groups[t] = 0; h->cand[t] = 0ull; }
+  if (t < S_NSTAGE) { h->n_items[t] = 0; h->n_groups[t] = 0; h->n_units[t] = 0; h->cand[t] = 0ull; }
   if (t == 0) { h->err = 0; h->pad = 0; h->n_dd = 0; h->n_flag = 0; s.scan_part[kScanBlocks + 1] = 0; }
 }
 
@@ -89,6 +89,15 @@ __device__ __forceinline__ uint32_t items_of(uint32_t R, uint32_t W) {
   }
   return R * ((W + kItemCand - 1) / kItemCand);
 }
+// Work units of a group: the items (q, ct), q = row chunk, ct = column tile, are cut into runs of
+// kUnitItems consecutive q at fixed ct; the items of a unit share their columns (item index of
+// (q, ct) = g_item0 + q * n_ct + ct; unit u of the group: ct = u % n_ct, q0 = (u / n_ct) * kUnitItems).
+__device__ __forceinline__ uint32_t units_of(uint32_t R, uint32_t W) {
+  if (R == 0 || W == 0) return 0;
+  const uint32_t nct = W <= (uint32_t)kItemCand ? 1u : (W + kItemCand - 1) / kItemCand;
+  const uint32_t nq = items_of(R, W) / nct;
+  return nct * ((nq + kUnitItems - 1) / kUnitItems);
+}
 
 // One block.  rows_level >= 0: the groups are kRowChunk-row chunks of that object level and the
 // kernel sets n_groups itself (gR must be 1, gW the group's candidate count: written by the
@@ -104,14 +113,15 @@ __global__ void k_emit_items(SlotDev s, int stage, int rows_level) {
   if (ng > st.cap_groups) ng = 0;   // cannot happen: cap_groups is sized from the object capacity
   if (threadIdx.x == 0) sh_cand = 0ull;
   __syncthreads();
-  uint32_t carry = 0;
+  uint32_t carry = 0, ucarry = 0;
   unsigned long long my_cand = 0;
   for (uint32_t base = 0; base < ng; base += blockDim.x) {
     const uint32_t g = base + threadIdx.x;
-    uint32_t ni = 0;
+    uint32_t ni = 0, nu = 0;
     if (g < ng) {
       const uint32_t R = st.gR[g], W = st.gW[g];
       ni = items_of(R, W);
+      nu = units_of(R, W);
       my_cand += (unsigned long long)R * W;
     }
     uint32_t tot;
@@ -119,14 +129,23 @@ __global__ void k_emit_items(SlotDev s, int stage, int rows_level) {
     if (g < ng) st.g_item0[g] = carry + e;
     carry += tot;
     __syncthreads();
+    const uint32_t eu = block_excl_scan(nu, sh, &tot);
+    if (g < ng) st.g_unit0[g] = ucarry + eu;
+    ucarry += tot;
+    __syncthreads();
   }
-  atomicAdd(&sh_cand, my_cand);
+  // block sum of the candidate counts (64-bit shared atomics are CAS loops: reduce per warp first)
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) my_cand += __shfl_xor_sync(0xffffffffu, my_cand, o);
+  if ((threadIdx.x & 31) == 0) atomicAdd(&sh_cand, my_cand);
   __syncthreads();
   const bool overflow = carry > st.cap_items;
   if (threadIdx.x == 0) {
     st.g_item0[ng] = carry;
+    st.g_unit0[ng] = ucarry;
     hdr->n_groups[stage] = ng;
     hdr->n_items[stage] = overflow ? 0u : carry;
+    hdr->n_units[stage] = overflow ? 0u : ucarry;
     hdr->cand[stage] = sh_cand;
     if (overflow) atomicOr(&hdr->err, (uint32_t)ERR_CAP_ITEMS);
   }
@@ -200,29 +219,23 @@ __global__ void k_row_offsets(GeoDev geo, SlotDev s) {
   else if (KIND == 4) { n = hdr->n_obj[5]; n_rows = hdr->n_seeds; off = s.pt5_pls_off; }
   else { n = hdr->n_obj[4]; n_rows = hdr->n_seeds; off = s.pt3_pls_off; }
   const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nt = gridDim.x * blockDim.x;
-  if (n == 0) {
-    for (uint32_t r = tid; r <= n_rows; r += nt) off[r] = 0;
-    return;
+  // one thread per ROW: lower bound of r in the ascending keys (gaps between keys can be thousands
+  // of rows wide, e.g. outer-layer MDs start no T3 / T5)
+  for (uint32_t r = tid; r <= n_rows; r += nt) {
+    uint32_t lo = 0, hi = n;           // first k in [0, n] with key[k] >= r
+    while (lo < hi) {
+      const uint32_t mid = (lo + hi) >> 1;
+      uint32_t key;
+      if (KIND == 0) key = s.md_mod[mid] >> 2;
+      else if (KIND == 1) key = s.ls_md[mid].x;
+      else if (KIND == 2) key = s.t3_md[mid].x;
+      else if (KIND == 3) key = s.t5_md[5 * (size_t)mid];
+      else if (KIND == 4) key = s.pt5_po[mid].x;
+      else key = s.pt3_po[mid].x;
+      if (key < r) lo = mid + 1; else hi = mid;
+    }
+    off[r] = lo;
   }
-  for (uint32_t k = tid; k < n; k += nt) {
-    uint32_t key, prev;
-    if (KIND == 0) { key = s.md_mod[k] >> 2; prev = k ? (s.md_mod[k - 1] >> 2) + 1 : 0; }
-    else if (KIND == 1) { key = s.ls_md[k].x; prev = k ? s.ls_md[k - 1].x + 1 : 0; }
-    else if (KIND == 2) { key = s.t3_md[k].x; prev = k ? s.t3_md[k - 1].x + 1 : 0; }
-    else if (KIND == 3) { key = s.t5_md[5 * (size_t)k]; prev = k ? s.t5_md[5 * (size_t)(k - 1)] + 1 : 0; }
-    else if (KIND == 4) { key = s.pt5_po[k].x; prev = k ? s.pt5_po[k - 1].x + 1 : 0; }
-    else { key = s.pt3_po[k].x; prev = k ? s.pt3_po[k - 1].x + 1 : 0; }
-    for (uint32_t r = prev; r <= key; ++r) off[r] = k;
-  }
-  // rows after the last key (outer-layer MDs start no T3 / T5: a long tail)
-  uint32_t last;
-  if (KIND == 0) last = s.md_mod[n - 1] >> 2;
-  else if (KIND == 1) last = s.ls_md[n - 1].x;
-  else if (KIND == 2) last = s.t3_md[n - 1].x;
-  else if (KIND == 3) last = s.t5_md[5 * (size_t)(n - 1)];
-  else if (KIND == 4) last = s.pt5_po[n - 1].x;
-  else last = s.pt3_po[n - 1].x;
-  for (uint32_t r = last + 1 + tid; r <= n_rows; r += nt) off[r] = n;
 }
 
 // ------------------------------------------------------------------ host launchers
@@ -254,8 +267,8 @@ void launch_scan_items(const Ctx &c, const SlotDev &s, int stage, int level, uin
   k_scan_items<<<1, 1024, 0, st>>>(s, stage, level, cap); LST_MARK(c, st, kScanName[stage]);
 }
 void launch_row_offsets(const Ctx &c, const SlotDev &s, int kind, cudaStream_t st) {
-  const uint32_t caps[6] = {s.cap_md, s.cap_ls, s.cap_t3, s.cap_t5, s.cap_pt5, s.cap_pt3};
-  const int g = grid_for(caps[kind], 256, c.n_sm * 4);
+  const uint32_t rows[6] = {c.geo.n_modules, s.cap_md, s.cap_md, s.cap_md, s.cap_seeds, s.cap_seeds};
+  const int g = grid_for(rows[kind] + 1, 256, c.n_sm * 4);
   switch (kind) {
     case 0: k_row_offsets<0><<<g, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_row_offsets[MD]"); break;
     case 1: k_row_offsets<1><<<g, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_row_offsets[LS]"); break;

@@ -264,7 +264,14 @@ __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
     if (lane == 0) {
       const bool keep = !beaten;
       if (A.type == 0) s.t5_keep[A.idx] = keep;
-      else if (A.type == 1) { s.pt5_keep[A.idx] = keep; if (keep) s.pls_has5[A.pls] = 1; }
+      else if (A.type == 1) {
+        s.pt5_keep[A.idx] = keep;
+        if (keep) {
+          s.pls_has5[A.pls] = 1;
+#pragma unroll
+          for (int q = 0; q < 10; ++q) s.hit_used5[ha[q]] = 1;   // S1 / S2: "shares a hit with a surviving pT5"
+        }
+      }
       else s.pt3_keep[A.idx] = keep;
     }
   }
@@ -274,39 +281,38 @@ __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
 __global__ void __launch_bounds__(128) k_s1(SlotDev s, Params g) {
   (void)g;
   const Header *hdr = s.hdr;
-  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], np3 = hdr->n_obj[4];
+  const uint32_t np3 = hdr->n_obj[4];
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < np3; i += gridDim.x * blockDim.x) {
     if (!s.pt3_keep[i]) continue;
     const uint32_t p = s.pt3_po[i].x;
     bool dup = s.pls_has5[p];
     const uint32_t na = s.pls_adj_cnt[p];
     for (uint32_t k = 0; k < na && !dup; ++k) dup = s.pls_has5[s.pls_adj[(size_t)p * kAdjCap + k] & 0x7FFFFFFFu];
-    for (int q = 0; q < 6 && !dup; ++q) {
-      const uint32_t h = s.pt3_hits[6 * (size_t)i + q];
-      for (uint32_t e = s.inc_off[h]; e < s.inc_off[h + 1]; ++e) {
-        const uint32_t b = s.inc_ent[e];
-        if (b >= n5 && b < n5 + np5 && s.pt5_keep[b - n5]) { dup = true; break; }
-      }
-    }
+    uint32_t h[6];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) h[q] = s.pt3_hits[6 * (size_t)i + q];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) dup |= (s.hit_used5[h[q]] != 0);
     if (dup) s.pt3_keep[i] = 0;
-    else s.pls_has3[p] = 1;
+    else {
+      s.pls_has3[p] = 1;
+#pragma unroll
+      for (int q = 0; q < 6; ++q) s.hit_used3[h[q]] = 1;
+    }
   }
 }
 
 // ------------------------------------------------------------------ S2: T5 against surviving pT5 / pT3
 __global__ void __launch_bounds__(128) k_s2(SlotDev s, Params g) {
   const Header *hdr = s.hdr;
-  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5];
+  const uint32_t n5 = hdr->n_obj[3];
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n5; i += gridDim.x * blockDim.x) {
     if (!s.t5_keep[i]) continue;
     bool dup = false;
-    for (int q = 0; q < 10 && !dup; ++q) {
+#pragma unroll
+    for (int q = 0; q < 10; ++q) {
       const uint32_t h = s.t5_hits[10 * (size_t)i + q];
-      for (uint32_t e = s.inc_off[h]; e < s.inc_off[h + 1]; ++e) {
-        const uint32_t b = s.inc_ent[e];
-        if (b < n5) continue;
-        if (b < n5 + np5 ? s.pt5_keep[b - n5] : s.pt3_keep[b - n5 - np5]) { dup = true; break; }
-      }
+      dup |= (s.hit_used5[h] | s.hit_used3[h]) != 0;
     }
     const double2 ep = s.t5_etaphi[i];
     const int b0 = eta_bin(g, ep.x);
@@ -386,6 +392,7 @@ void launch_dedup(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   const uint32_t cap_dd = s.cap_t5 + s.cap_pt5 + s.cap_pt3;
   cudaMemsetAsync(s.inc_cnt, 0, sizeof(uint32_t) * 2 * ((size_t)s.cap_hits + 1), st);
   cudaMemsetAsync(s.pls_has5, 0, 3 * (size_t)s.cap_seeds, st);
+  cudaMemsetAsync(s.hit_used5, 0, 2 * (size_t)s.cap_hits, st);
   k_pls_prep<<<1, 1024, 0, st>>>(s, c.par); LST_MARK(c, st, "k_pls_prep");
   k_pls_adj<<<grid_of(s.cap_seeds, 8, c.n_sm * 8), 256, 0, st>>>(s, c.par); LST_MARK(c, st, "k_pls_adj");
   k_dd_count<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_dd_count");

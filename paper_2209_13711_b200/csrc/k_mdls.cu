@@ -144,58 +144,115 @@ __device__ __forceinline__ uint32_t map_col_to_md(const MapRow &mr, uint32_t j) 
   return mr.start[lo] + (j - mr.cum[lo]);
 }
 
+// append candidate c to a survivor list (warp-aggregated shared atomic); all 32 lanes must call
+__device__ __forceinline__ void push_list(uint16_t *list, uint32_t *n, bool keep, uint32_t c) {
+  const uint32_t b = __ballot_sync(0xffffffffu, keep);
+  if (b == 0) return;
+  const int lane = threadIdx.x & 31;
+  const int leader = __ffs(b) - 1;
+  uint32_t base = 0;
+  if (lane == leader) base = atomicAdd(n, (uint32_t)__popc(b));
+  base = __shfl_sync(0xffffffffu, base, leader);
+  if (keep) list[base + __popc(b & ((1u << lane) - 1u))] = (uint16_t)c;
+}
+
+// One block per WORK UNIT (k_emit_items): up to kUnitItems items of module A that share one column
+// tile, i.e. the MDs of the connected modules are staged in shared memory once and re-used for all
+// rows (an inner-barrel module compares each of its ~30 MDs with ~1200 MDs of ~64 neighbours).
+// Per item: tier 1 (ls_tier1_f: no division / sqrt / atan, ~82 % rejected) on every candidate,
+// tier 2 (ls_pre_f, full fp32) on the compacted survivors, fp64 decision on what is left (~3 %).
 __global__ void __launch_bounds__(kThreads) k_ls_eval(GeoDev geo, SlotDev s, Params g) {
   __shared__ ItemScratch sc;
+  __shared__ uint16_t list2[kItemCand];
+  __shared__ uint32_t n2;
   __shared__ MapRow mr;
   __shared__ float4 p_pos[kItemCand + 8];
-  __shared__ float2 p_kf[kItemCand + 8];
-  __shared__ uint32_t p_idx[kItemCand + 8];
-  __shared__ uint8_t p_cat[kItemCand + 8];
+  __shared__ uint32_t p_idc[kItemCand + 8];     // MD index | category << 30
+  __shared__ float4 tab[4];                     // per category: sig_z, sig_r, sig_t
   const StageBuf &st = s.st[S_LS];
-  const uint32_t n_items = s.hdr->n_items[S_LS];
+  const uint32_t n_units = s.hdr->n_units[S_LS], ng = s.hdr->n_groups[S_LS];
   const int tid = threadIdx.x;
-  for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
-    const Item item = st.items[it];
-    const uint32_t A = item.group;
-    const int nr = item.nrows, nj = item.nj;
-    const uint32_t i0 = s.md_mod_off[A] + item.i0;
+  if (tid < 4) tab[tid] = make_float4(g.f_sig_z[tid], g.f_sig_r[tid], g.f_sig_t[tid], 0.0f);
+  for (uint32_t u = blockIdx.x; u < n_units; u += gridDim.x) {
+    uint32_t lo = 0, hi = ng;                   // last group with g_unit0 <= u
+    while (hi - lo > 1) {
+      const uint32_t mid = (lo + hi) >> 1;
+      if (st.g_unit0[mid] <= u) lo = mid; else hi = mid;
+    }
+    const uint32_t A = lo, lu = u - st.g_unit0[A];
+    const uint32_t R = st.gR[A], W = st.gW[A];
+    const uint32_t nct = W <= (uint32_t)kItemCand ? 1u : (W + kItemCand - 1) / kItemCand;
+    const uint32_t rpi = W <= (uint32_t)kItemCand ? (uint32_t)kItemCand / W : 1u;
+    const uint32_t nq = (R + rpi - 1) / rpi;
+    const uint32_t ct = lu % nct, q0 = (lu / nct) * kUnitItems;
+    const uint32_t qn = min((uint32_t)kUnitItems, nq - q0);
+    const uint32_t j0 = ct * kItemCand;
+    const int nj = (int)min((uint32_t)kItemCand, W - j0);
+    const uint32_t md0 = s.md_mod_off[A], item0 = st.g_item0[A];
+    __syncthreads();                            // the previous unit is done with mr / p_pos
     stage_map_row(mr, geo, s, A);
-    if (tid < kItemWords) sc.mask[tid] = 0;
-    if (tid == 0) sc.n = 0;
     __syncthreads();
-    for (int k = tid; k < nr + nj; k += kThreads) {
-      const uint32_t md = k < nr ? i0 + k : map_col_to_md(mr, item.j0 + (k - nr));
-      p_idx[k] = md;
+    for (int k = tid; k < nj; k += kThreads) {
+      const uint32_t md = map_col_to_md(mr, j0 + k);
       p_pos[k] = s.md_pos[md];
-      p_kf[k] = s.md_kf[md];
-      p_cat[k] = (uint8_t)(s.md_mod[md] & 3u);
+      p_idc[k] = md | ((s.md_mod[md] & 3u) << 30);
     }
-    __syncthreads();
-    const int nc = nr * nj;
-    for (int base = 0; base < nc; base += kThreads) {
-      const int c = base + tid;
-      bool keep = false;
-      if (c < nc) {
-        const int r = c / nj, jj = nr + (c - r * nj);
-        const float4 a = p_pos[r], b = p_pos[jj];
-        const float2 ka = p_kf[r], kb = p_kf[jj];
-        keep = ls_pre_f(g, a.x, a.y, a.z, a.w, ka.x, ka.y, p_cat[r], b.x, b.y, b.z, b.w, kb.x, kb.y, p_cat[jj]);
+    const uint32_t inv = (1u << 20) / (uint32_t)nj + 1u;   // c / nj == (c * inv) >> 20 for c * nj < 2^20
+    for (uint32_t qi = 0; qi < qn; ++qi) {
+      const uint32_t q = q0 + qi, it = item0 + q * nct + ct, i0 = q * rpi;
+      const int nr = (int)min(rpi, R - i0);
+      for (int k = tid; k < nr; k += kThreads) {
+        const uint32_t md = md0 + i0 + k;
+        p_pos[nj + k] = s.md_pos[md];
+        p_idc[nj + k] = md | ((s.md_mod[md] & 3u) << 30);
       }
-      push_survivor(sc, keep, (uint32_t)c);
+      if (tid < kItemWords) sc.mask[tid] = 0;
+      if (tid == 0) { sc.n = 0; n2 = 0; }
+      __syncthreads();
+      const int nc = nr * nj;
+      for (int base = 0; base < nc; base += kThreads) {          // tier 1
+        const int c = base + tid;
+        bool keep = false;
+        if (c < nc) {
+          const int r = (int)(((uint32_t)c * inv) >> 20), jj = c - r * nj;
+          const float4 a = p_pos[nj + r], b = p_pos[jj];
+          const uint32_t ca = p_idc[nj + r] >> 30, cb = p_idc[jj] >> 30;
+          const float4 ta = tab[ca], tb = tab[cb];
+          keep = ls_tier1_f(g, a.x, a.y, a.z, a.w, ta.x, ta.y, ta.z, b.x, b.y, b.z, b.w, tb.x, tb.y, tb.z, cb >= 2u);
+        }
+        push_list(sc.list, &sc.n, keep, (uint32_t)c);
+      }
+      __syncthreads();
+      const int n1 = (int)sc.n;
+      for (int base = 0; base < n1; base += kThreads) {          // tier 2
+        const int k = base + tid;
+        bool keep = false;
+        int c = 0;
+        if (k < n1) {
+          c = sc.list[k];
+          const int r = (int)(((uint32_t)c * inv) >> 20), jj = c - r * nj;
+          const float4 a = p_pos[nj + r], b = p_pos[jj];
+          const uint32_t ia = p_idc[nj + r], ib = p_idc[jj];
+          const float2 ka = s.md_kf[ia & 0x3FFFFFFFu], kb = s.md_kf[ib & 0x3FFFFFFFu];
+          keep = ls_pre_f(g, a.x, a.y, a.z, a.w, ka.x, ka.y, (int)(ia >> 30), b.x, b.y, b.z, b.w, kb.x, kb.y, (int)(ib >> 30));
+        }
+        push_list(list2, &n2, keep, (uint32_t)c);
+      }
+      __syncthreads();
+      const int nsv = (int)n2;
+      for (int k = tid; k < nsv; k += kThreads) {                // fp64 decision
+        const int c = list2[k];
+        const int r = (int)(((uint32_t)c * inv) >> 20), jj = c - r * nj;
+        const float4 a = p_pos[nj + r], b = p_pos[jj];
+        const uint32_t ia = p_idc[nj + r], ib = p_idc[jj];
+        const double2 ka = s.md_kd[ia & 0x3FFFFFFFu], kb = s.md_kd[ib & 0x3FFFFFFFu];
+        const Pt pa = make_pt(a.x, a.y, a.z, (int)(ia >> 30)), pb = make_pt(b.x, b.y, b.z, (int)(ib >> 30));
+        if (ls_eval_d(g, pa, ka.x, ka.y, pb, kb.x, kb.y, nullptr)) atomicOr(&sc.mask[c >> 5], 1u << (c & 31));
+      }
+      __syncthreads();
+      publish_mask(sc, st.mask + (size_t)it * kItemWords, st.item_cnt + it);
+      __syncthreads();
     }
-    __syncthreads();
-    const int nsv = (int)sc.n;
-    for (int k = tid; k < nsv; k += kThreads) {
-      const int c = sc.list[k];
-      const int r = c / nj, jj = nr + (c - r * nj);
-      const float4 a = p_pos[r], b = p_pos[jj];
-      const double2 ka = s.md_kd[p_idx[r]], kb = s.md_kd[p_idx[jj]];
-      const Pt pa = make_pt(a.x, a.y, a.z, p_cat[r]), pb = make_pt(b.x, b.y, b.z, p_cat[jj]);
-      if (ls_eval_d(g, pa, ka.x, ka.y, pb, kb.x, kb.y, nullptr)) atomicOr(&sc.mask[c >> 5], 1u << (c & 31));
-    }
-    __syncthreads();
-    publish_mask(sc, st.mask + (size_t)it * kItemWords, st.item_cnt + it);
-    __syncthreads();
   }
 }
 
@@ -246,7 +303,7 @@ void launch_md(const Ctx &c, const SlotDev &s, cudaStream_t st) {
 void launch_ls(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   k_ls_groups<<<(c.geo.n_modules + 127) / 128, 128, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_ls_groups");
   launch_emit(c, s, S_LS, -1, st);
-  k_ls_eval<<<persistent_grid(c, 5), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_ls_eval");
+  k_ls_eval<<<persistent_grid(c, 6), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_ls_eval");
   launch_scan_items(c, s, S_LS, 1, s.cap_ls, st);
   k_ls_fill<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_ls_fill");
   launch_row_offsets(c, s, 1, st);

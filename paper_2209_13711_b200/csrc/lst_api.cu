@@ -303,6 +303,7 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.pls_adj_cnt = w.take<uint32_t>(nsd); s.pls_adj = w.take<uint32_t>((size_t)nsd * kAdjCap);
   s.pls_has5 = w.take<uint8_t>(3 * (size_t)nsd);
   s.pls_has3 = s.pls_has5 ? s.pls_has5 + nsd : nullptr; s.pls_near_t5 = s.pls_has5 ? s.pls_has5 + 2 * (size_t)nsd : nullptr;
+  s.hit_used5 = w.take<uint8_t>(2 * (size_t)nh); s.hit_used3 = s.hit_used5 ? s.hit_used5 + nh : nullptr;
   s.tc_to = w.take<uint2>(s.cap_tc); s.tc_f = w.take<float4>(s.cap_tc);
   s.tc_flag = w.take<uint32_t>((size_t)s.cap_tc + 1); s.tc_pos = w.take<uint32_t>((size_t)s.cap_tc + 1);
   s.scan_part = w.take<uint32_t>(kScanBlocks + 2);
@@ -320,6 +321,7 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
     b.cap_items = grp_cap[k] + 2 * (cand_cap[k] / kItemCand) + 16;
     b.gR = w.take<uint32_t>(b.cap_groups); b.gW = w.take<uint32_t>(b.cap_groups);
     b.g_item0 = w.take<uint32_t>((size_t)b.cap_groups + 1);
+    b.g_unit0 = w.take<uint32_t>((size_t)b.cap_groups + 1);
     b.items = w.take<Item>(b.cap_items);
     b.mask = w.take<uint32_t>((size_t)b.cap_items * kItemWords);
     b.item_cnt = w.take<uint32_t>(b.cap_items); b.item_base = w.take<uint32_t>(b.cap_items);
@@ -665,6 +667,8 @@ extern "C" int lst_host_eval(const lst_config *cfg_in, int level, uint32_t n, co
   if (cfg_in) cfg = *cfg_in; else lst_default_config(&cfg);
   Params g;
   make_params(cfg, &g);
+  const bool tier1_only = level == 101;   // diagnostics: pre = LS tier 1 alone, pass = full fp32 pre-filter
+  if (tier1_only) level = LST_LS;
   const int npts = level == LST_MD ? 2 : level == LST_LS ? 2 : level == LST_T3 ? 3 : level == LST_T5 ? 5 : 0;
   if (!npts || !pts || !cats || !pass) return LST_EINVAL;
   for (uint32_t i = 0; i < n; ++i) {
@@ -685,8 +689,15 @@ extern "C" int lst_host_eval(const lst_config *cfg_in, int level, uint32_t n, co
       LsOut o = {0, 0, 0};
       ok = ls_eval_d(g, P[0], a[0], a[1], P[1], a[2], a[3], &o);
       const float ri = sqrtf(p[0] * p[0] + p[1] * p[1]), ro = sqrtf(p[3] * p[3] + p[4] * p[4]);
-      pr = ls_pre_f(g, p[0], p[1], p[2], ri, (float)a[0], (float)a[1], ct[0], p[3], p[4], p[5], ro, (float)a[2],
+      pr = ls_tier1_f(g, p[0], p[1], p[2], ri, g.f_sig_z[ct[0]], g.f_sig_r[ct[0]], g.f_sig_t[ct[0]], p[3], p[4], p[5], ro,
+                      g.f_sig_z[ct[1]], g.f_sig_r[ct[1]], g.f_sig_t[ct[1]], ct[1] >= 2) &&
+           ls_pre_f(g, p[0], p[1], p[2], ri, (float)a[0], (float)a[1], ct[0], p[3], p[4], p[5], ro, (float)a[2],
                     (float)a[3], ct[1]);
+      if (tier1_only) {
+        ok = pr;
+        pr = ls_tier1_f(g, p[0], p[1], p[2], ri, g.f_sig_z[ct[0]], g.f_sig_r[ct[0]], g.f_sig_t[ct[0]], p[3], p[4], p[5], ro,
+                        g.f_sig_z[ct[1]], g.f_sig_r[ct[1]], g.f_sig_t[ct[1]], ct[1] >= 2);
+      }
       o3[0] = o.kappa; o3[1] = o.sigk; o3[2] = o.dphi;
     } else if (level == LST_T3) {
       T3Out o = {0, 0, 0};

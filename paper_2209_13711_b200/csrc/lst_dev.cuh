@@ -21,6 +21,7 @@ namespace lst {
 constexpr int kItemCand = 1024;          // candidates per work item
 constexpr int kItemWords = kItemCand / 32;
 constexpr int kThreads = 128;            // threads per block of eval / fill kernels
+constexpr int kUnitItems = 8;            // items per work unit (same group, same column tile, consecutive rows)
 constexpr int kRowChunk = 128;           // rows per group in the variable-width stages (T3, T5, pixel)
 constexpr int kMaxDeg = 512;             // maximum module-map degree (checked by lst_create)
 constexpr int kPxCap = 64;               // (seed, start module) rows per pixel seed ON AVERAGE (overflow -> LST_ENOMEM)
@@ -51,6 +52,7 @@ struct Header {          // per slot, device; zeroed (except n_hits / n_seeds) a
   uint32_t n_obj[8];                 // indexed by lst_level; [kPairLevel] = (seed, module) pairs
   uint32_t n_items[S_NSTAGE];
   uint32_t n_groups[S_NSTAGE];
+  uint32_t n_units[S_NSTAGE];        // work units (k_emit_items): item runs that share their columns
   uint32_t err;
   uint32_t n_dd;                     // T5 + pT5 + pT3 objects entering the cleaning
   uint32_t n_flag;                   // pT5 + pT3 + T5 + seeds: length of the TC keep-flag array
@@ -61,6 +63,7 @@ struct Header {          // per slot, device; zeroed (except n_hits / n_seeds) a
 struct StageBuf {        // work list of one stage
   uint32_t *gR, *gW;     // [cap_groups] rows / width (or candidate count) per group
   uint32_t *g_item0;     // [cap_groups+1] first item of a group
+  uint32_t *g_unit0;     // [cap_groups+1] first work unit of a group
   Item *items;           // [cap_items]
   uint32_t *mask;        // [cap_items * kItemWords]
   uint32_t *item_cnt;    // [cap_items] pass count
@@ -134,6 +137,7 @@ struct SlotDev {
   uint32_t *pls_bin_ent;           // [cap_seeds]
   uint32_t *pls_adj_cnt, *pls_adj; // [cap_seeds], [cap_seeds * kAdjCap]: related seeds (bit 31: close in eta-phi)
   uint8_t *pls_has5, *pls_has3, *pls_near_t5;   // [cap_seeds] each, contiguous
+  uint8_t *hit_used5, *hit_used3;  // [cap_hits] each, contiguous: hit belongs to a surviving pT5 / pT3 (S1, S2)
   uint32_t *tc_flag, *tc_pos;      // [cap_tc+1]
   uint32_t *scan_part;             // [kScanBlocks+2]: block partials, total; last word = ticket
   // TC
