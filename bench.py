@@ -254,7 +254,8 @@ def run_ours(a, rank, world, local_rank):
 
     geom = lstgen.build_geometry(False)
     off, cols = B.lst_build_module_map(geom)
-    events = [lstgen.make_event(geom, a.workload, seed=1000 + rank * a.events + i) for i in range(a.events)]
+    from paper_2209_13711_b200 import sharding
+    events = [lstgen.make_event(geom, a.workload, seed=sd) for sd in sharding.event_seeds(rank, world, a.events)]
     max_hits = max(e.n_hits for e in events)
     max_seeds = max(max(e.n_seeds for e in events), 1)
     lst = B.LST(geom, off, cols, n_slots=a.slots, max_hits=max_hits, max_seeds=max_seeds, device=str(dev))
@@ -336,24 +337,21 @@ def run_ours(a, rank, world, local_rank):
         barrier()
         clocks = cs.stop() if sample_clocks else None
         ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = sharding.max_over_ranks(ms, dist if world > 1 else None, dev)
         return ms, clocks
 
     ms, clocks = timed(step_resident, a.warmup, a.steps, True)
     # every slot's last event must have completed without capacity / input errors
     counts = [lst.lst_get_counts(sl) for sl in range(a.slots)]
     launches = lst.launches_per_run() + 1                      # + k_set_event of lst_load_event
-    value = world * a.events * a.steps / (ms * 1e-3)
+    value = sharding.job_events_per_s(world, a.events, a.steps, ms)
 
     e2e = None
     if not a.no_e2e:
         d2h[0] = 0
         ms_e, _ = timed(step_e2e, max(a.warmup, 1), a.steps, False)
         d2h_per_step = d2h[0] / (max(a.warmup, 1) + a.steps)
-        e2e = {"value": world * a.events * a.steps / (ms_e * 1e-3), "unit": UNIT,
+        e2e = {"value": sharding.job_events_per_s(world, a.events, a.steps, ms_e), "unit": UNIT,
                "h2d_bytes_per_step": int(h2d_bytes), "d2h_bytes_per_step": int(d2h_per_step),
                "ms_per_step": ms_e / a.steps,
                "api": "lst_load_event(host pinned SoA) + lst_run + lst_get_objects(LST_TC, copy_to_host=1)"}
