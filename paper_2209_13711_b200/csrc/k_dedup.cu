@@ -5,7 +5,7 @@
 // no ordering between threads.  Pairs are found through two lookups instead of all-pairs loops:
 //   * hit -> objects incidence lists (CSR over the sorted hit positions) for "shares OT hits";
 //   * pixel seeds binned in eta (bin width >= 1.25 sqrt(dr2max)) for "close in eta-phi", plus a
-//     per-seed list of related seeds (close in eta-phi, or sharing a pixel-hit id).
+//     per-seed list of the seeds close to it; a hash set of the pixel-hit ids for "shares a pixel hit".
 // Object ids in the incidence lists ("dd ids"): [0, nT5) T5, then pT5, then pT3.
 #include "lst_launch.h"
 
@@ -94,6 +94,7 @@ __global__ void __launch_bounds__(1024) k_pls_prep(SlotDev s, Params g) {
   if (threadIdx.x == 0) {
     hdr->n_dd = hdr->n_obj[3] + hdr->n_obj[5] + hdr->n_obj[4];
     hdr->n_flag = hdr->n_obj[5] + hdr->n_obj[4] + hdr->n_obj[3] + n;
+    hdr->n_inc = 3 * hdr->n_hits;
   }
   for (int b = threadIdx.x; b < kEtaBins; b += blockDim.x) cnt[b] = 0;
   __syncthreads();
@@ -118,42 +119,55 @@ __global__ void __launch_bounds__(1024) k_pls_prep(SlotDev s, Params g) {
   }
 }
 
-// One warp per seed a: seeds b != a that are close in eta-phi (bit 31) or share a pixel-hit id.
+// Thread per seed a: the seeds b != a close to it in eta-phi, found through the eta bins (a close
+// seed lies in a's bin or a neighbouring one: the bin width exceeds sqrt(dr2max)).
 __global__ void __launch_bounds__(256) k_pls_adj(SlotDev s, Params g) {
   const uint32_t n = s.hdr->n_seeds;
-  const int lane = threadIdx.x & 31;
-  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
-  const uint4 *ids = reinterpret_cast<const uint4 *>(s.seed_ids);
-  for (uint32_t a = warp; a < n; a += nwarp) {
+  for (uint32_t a = blockIdx.x * blockDim.x + threadIdx.x; a < n; a += gridDim.x * blockDim.x) {
     const double ea = (double)s.seed_eta[a], pa = (double)s.seed_phi[a];
-    const uint4 ia = ids[a];
+    const int b0 = eta_bin(g, ea);
+    const int lo = b0 > 0 ? b0 - 1 : 0, hi = b0 + 1 < g.eta_nbins ? b0 + 1 : g.eta_nbins - 1;
+    const uint32_t e0 = s.pls_bin_off[lo], e1 = s.pls_bin_off[hi + 1];
     uint32_t cnt = 0;
-    for (uint32_t base = 0; base < n; base += 32) {
-      const uint32_t b = base + lane;
-      bool rel = false, close = false;
-      if (b < n && b != a) {
-        close = close_eta_phi(g, ea, pa, (double)s.seed_eta[b], (double)s.seed_phi[b]);
-        const uint4 ib = ids[b];
-        const uint32_t va[4] = {ia.x, ia.y, ia.z, ia.w}, vb[4] = {ib.x, ib.y, ib.z, ib.w};
-        bool sharep = false;
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-          for (int j = 0; j < 4; ++j) sharep |= (va[i] == vb[j]);
-        rel = close || sharep;
-      }
-      const uint32_t bal = __ballot_sync(0xffffffffu, rel);
-      if (rel) {
-        const uint32_t pos = cnt + __popc(bal & ((1u << lane) - 1u));
-        if (pos < (uint32_t)kAdjCap) s.pls_adj[(size_t)a * kAdjCap + pos] = b | (close ? 0x80000000u : 0u);
-      }
-      cnt += __popc(bal);
+    for (uint32_t e = e0; e < e1; ++e) {
+      const uint32_t b = s.pls_bin_ent[e];
+      if (b == a || !close_eta_phi(g, ea, pa, (double)s.seed_eta[b], (double)s.seed_phi[b])) continue;
+      if (cnt < (uint32_t)kAdjCap) s.pls_adj[(size_t)a * kAdjCap + cnt] = b;
+      ++cnt;
     }
-    if (lane == 0) {
-      if (cnt > (uint32_t)kAdjCap) { atomicOr(&s.hdr->err, (uint32_t)ERR_CAP_PIX); cnt = 0; }
-      s.pls_adj_cnt[a] = cnt;
-    }
+    if (cnt > (uint32_t)kAdjCap) { atomicOr(&s.hdr->err, (uint32_t)ERR_CAP_PIX); cnt = 0; }
+    s.pls_adj_cnt[a] = cnt;
   }
+}
+
+// "Seeds a and b share a pixel hit" is looked up through the pixel-hit ids themselves: every id
+// is inserted into a hash set (linear probing; at most half full), and a seed remembers the slots of
+// its 4 ids.  Flags per slot (pid_has5 / pid_has3) then answer "does some seed with a surviving
+// pT5 / pT3 contain this pixel hit" without any seed-to-seed list.
+__device__ __forceinline__ uint32_t pid_hash(uint32_t id) { return (id * 0x9E3779B1u) ^ (id >> 15); }
+__global__ void __launch_bounds__(256) k_pid_insert(SlotDev s) {
+  const uint32_t n4 = 4 * s.hdr->n_seeds, mask = s.pid_size - 1;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += gridDim.x * blockDim.x) {
+    const uint32_t id = s.seed_ids[i];
+    const unsigned long long key = (1ull << 32) | id;
+    uint32_t h = pid_hash(id) & mask;
+    for (;;) {
+      const unsigned long long old = atomicCAS(&s.pid_key[h], 0ull, key);
+      if (old == 0ull || old == key) break;
+      h = (h + 1) & mask;
+    }
+    s.pls_slot[i] = h;
+  }
+}
+__device__ __forceinline__ void pid_mark(const SlotDev &s, uint8_t *flag, uint32_t p) {
+  const uint4 sl = reinterpret_cast<const uint4 *>(s.pls_slot)[p];
+  flag[sl.x] = 1; flag[sl.y] = 1; flag[sl.z] = 1; flag[sl.w] = 1;
+}
+__device__ __forceinline__ bool pid_any(const SlotDev &s, uint32_t p, bool with3) {
+  const uint4 sl = reinterpret_cast<const uint4 *>(s.pls_slot)[p];
+  uint32_t v = s.pid_has5[sl.x] | s.pid_has5[sl.y] | s.pid_has5[sl.z] | s.pid_has5[sl.w];
+  if (with3) v |= s.pid_has3[sl.x] | s.pid_has3[sl.y] | s.pid_has3[sl.z] | s.pid_has3[sl.w];
+  return v != 0;
 }
 
 // ------------------------------------------------------------------ hit -> objects incidence
@@ -184,7 +198,8 @@ __global__ void k_dd_count(SlotDev s) {
 #pragma unroll
       for (int q = 0; q < 6; ++q) s.pt3_hits[6 * (size_t)i + q] = h[q];
     }
-    for (int q = 0; q < n; ++q) atomicAdd(&s.inc_cnt[h[q]], 1u);
+    const uint32_t ty = (uint32_t)dd_type(n5, np5, d);
+    for (int q = 0; q < n; ++q) atomicAdd(&s.inc_cnt[3 * h[q] + ty], 1u);
   }
 }
 __global__ void k_dd_scatter(SlotDev s) {
@@ -193,7 +208,7 @@ __global__ void k_dd_scatter(SlotDev s) {
   for (uint32_t d = blockIdx.x * blockDim.x + threadIdx.x; d < n_dd; d += gridDim.x * blockDim.x) {
     const DRef r = dd_ref(s, n5, np5, d);
     for (int q = 0; q < r.n_ot; ++q) {
-      const uint32_t h = r.hits[q];
+      const uint32_t h = 3 * r.hits[q] + (uint32_t)r.type;
       s.inc_ent[s.inc_off[h] + atomicAdd(&s.inc_cur[h], 1u)] = d;
     }
   }
@@ -201,49 +216,75 @@ __global__ void k_dd_scatter(SlotDev s) {
 
 // ------------------------------------------------------------------ S0: inside one collection
 // One WARP per object A.  An object sharing >= min_shared of A's n_ot hits contains at least one of
-// any n_ot - min_shared + 1 of them, so only the incidence lists of hits k0..n_ot-1 are searched;
-// the lists are flattened into one index space that the lanes stride (their lengths are very
-// uneven: inner-layer hits sit in hundreds of objects), and the cheap tests (type, score) come
-// before B's hit row is loaded.
+// any n_ot - min_shared + 1 of them, so only the incidence lists (of A's own type) of hits
+// k0..n_ot-1 are searched; the lists are flattened into one index space that the lanes stride
+// (their lengths are very uneven: inner-layer hits sit in hundreds of objects).  Per entry B the
+// cheap tests come first: score(B) <= score(A), then a NECESSARY condition for ">= min_shared
+// shared hits" -- the number of B's hits whose hash bit is set in A's 64-bit hit signature -- and
+// only then the exact hit-set intersection and the full "B beats A" order.
 __device__ __forceinline__ double dd_score(const SlotDev &s, uint32_t n5, uint32_t np5, uint32_t d) {
   return d < n5 ? s.t5_chi2[d] : (d < n5 + np5 ? s.pt5_chi2[d - n5] : s.pt3_chi2[d - n5 - np5]);
 }
 __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
+  __shared__ uint32_t sh_pre[4][12], sh_beg[4][12];
   const Header *hdr = s.hdr;
   const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = hdr->n_dd;
-  const int lane = threadIdx.x & 31;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+  uint32_t *pre = sh_pre[wib], *beg = sh_beg[wib];
   for (uint32_t d = warp; d < n_dd; d += nwarp) {
     const DRef A = dd_ref(s, n5, np5, d);
     uint32_t ha[10];
+    unsigned long long sigA = 0ull;
 #pragma unroll
-    for (int q = 0; q < 10; ++q) ha[q] = q < A.n_ot ? A.hits[q] : 0xFFFFFFFFu;
+    for (int q = 0; q < 10; ++q) {
+      ha[q] = q < A.n_ot ? A.hits[q] : 0xFFFFFFFFu;
+      if (q < A.n_ot) sigA |= 1ull << (ha[q] & 63u);
+    }
     bool beaten = false;
     if (g.s0_enabled) {
       const int min_shared = A.type == 0 ? g.dup_t5 : (A.type == 1 ? g.dup_pt5 : g.dup_pt3);
-      const int k0 = min_shared - 1;
-      uint32_t beg[10], pre[11];
-      pre[0] = 0;
-#pragma unroll
-      for (int q = 0; q < 10; ++q) {
-        uint32_t len = 0;
-        beg[q] = 0;
-        if (q >= k0 && q < A.n_ot) { beg[q] = s.inc_off[ha[q]]; len = s.inc_off[ha[q] + 1] - beg[q]; }
-        pre[q + 1] = pre[q] + len;
+      const int k0 = min_shared - 1, nl = A.n_ot > k0 ? A.n_ot - k0 : 0;   // lists searched: hits k0 .. n_ot-1
+      {
+        uint32_t len = 0, b0 = 0;
+        if (lane < nl) {
+          const uint32_t row = 3 * A.hits[k0 + lane] + (uint32_t)A.type;
+          b0 = s.inc_off[row]; len = s.inc_off[row + 1] - b0;
+        }
+        uint32_t tot;
+        const uint32_t ex = warp_excl_scan(len, &tot);
+        __syncwarp();
+        if (lane < 11) { pre[lane] = ex; beg[lane] = b0; }      // lanes >= nl: pre = total
+        __syncwarp();
       }
-      const uint32_t total = pre[10];
+      const int nlc = nl < 10 ? nl : 10;
+      const uint32_t total = pre[nlc];
+      const double *score_arr = A.type == 0 ? s.t5_chi2 : (A.type == 1 ? s.pt5_chi2 : s.pt3_chi2);
+      const uint32_t dbase = A.type == 0 ? 0u : (A.type == 1 ? n5 : n5 + np5);
+      int cur = 0;
       for (uint32_t base = 0; base < total && !beaten; base += 32) {
         const uint32_t i = base + lane;
         bool hit = false;
         if (i < total) {
-          uint32_t e = 0;
+          while (i >= pre[cur + 1]) ++cur;
+          const uint32_t b = s.inc_ent[beg[cur] + (i - pre[cur])];
+          if (b != d && !(score_arr[b - dbase] > A.score)) {
+            const uint32_t *hb = A.type == 0 ? s.t5_hits + 10 * (size_t)b
+                               : (A.type == 1 ? s.t5_hits + 10 * (size_t)s.pt5_po[b - dbase].y
+                                              : s.pt3_hits + 6 * (size_t)(b - dbase));
+            const uint2 *hb2 = reinterpret_cast<const uint2 *>(hb);
+            int cnt = 0;
 #pragma unroll
-          for (int q = 0; q < 10; ++q)
-            if (i >= pre[q] && i < pre[q + 1]) e = beg[q] + (i - pre[q]);
-          const uint32_t b = s.inc_ent[e];
-          if (b != d && dd_type(n5, np5, b) == A.type && !(dd_score(s, n5, np5, b) > A.score)) {
-            const DRef Bq = dd_ref(s, n5, np5, b);
-            hit = dd_shared(ha, A.n_ot, Bq.hits, Bq.n_ot) >= min_shared && dd_beats(s, Bq, A);
+            for (int q = 0; q < 5; ++q) {
+              if (2 * q < A.n_ot) {
+                const uint2 v = hb2[q];
+                cnt += (int)((sigA >> (v.x & 63u)) & 1ull) + (int)((sigA >> (v.y & 63u)) & 1ull);
+              }
+            }
+            if (cnt >= min_shared) {
+              const DRef Bq = dd_ref(s, n5, np5, b);
+              hit = dd_shared(ha, A.n_ot, Bq.hits, Bq.n_ot) >= min_shared && dd_beats(s, Bq, A);
+            }
           }
         }
         beaten = __any_sync(0xffffffffu, hit);
@@ -268,6 +309,7 @@ __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
         s.pt5_keep[A.idx] = keep;
         if (keep) {
           s.pls_has5[A.pls] = 1;
+          pid_mark(s, s.pid_has5, A.pls);
 #pragma unroll
           for (int q = 0; q < 10; ++q) s.hit_used5[ha[q]] = 1;   // S1 / S2: "shares a hit with a surviving pT5"
         }
@@ -285,9 +327,9 @@ __global__ void __launch_bounds__(128) k_s1(SlotDev s, Params g) {
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < np3; i += gridDim.x * blockDim.x) {
     if (!s.pt3_keep[i]) continue;
     const uint32_t p = s.pt3_po[i].x;
-    bool dup = s.pls_has5[p];
+    bool dup = s.pls_has5[p] || pid_any(s, p, false);
     const uint32_t na = s.pls_adj_cnt[p];
-    for (uint32_t k = 0; k < na && !dup; ++k) dup = s.pls_has5[s.pls_adj[(size_t)p * kAdjCap + k] & 0x7FFFFFFFu];
+    for (uint32_t k = 0; k < na && !dup; ++k) dup = s.pls_has5[s.pls_adj[(size_t)p * kAdjCap + k]];
     uint32_t h[6];
 #pragma unroll
     for (int q = 0; q < 6; ++q) h[q] = s.pt3_hits[6 * (size_t)i + q];
@@ -296,6 +338,7 @@ __global__ void __launch_bounds__(128) k_s1(SlotDev s, Params g) {
     if (dup) s.pt3_keep[i] = 0;
     else {
       s.pls_has3[p] = 1;
+      pid_mark(s, s.pid_has3, p);
 #pragma unroll
       for (int q = 0; q < 6; ++q) s.hit_used3[h[q]] = 1;
     }
@@ -345,13 +388,12 @@ __global__ void k_s3_flags(SlotDev s) {
     else if (i < np5 + np3 + n5) f = s.t5_keep[i - np5 - np3];
     else {
       const uint32_t p = i - np5 - np3 - n5;
-      bool keep = pls_unused(s, p) && !s.pls_near_t5[p];
+      bool keep = pls_unused(s, p) && !s.pls_near_t5[p] && !pid_any(s, p, true);
       const uint32_t na = s.pls_adj_cnt[p];
       for (uint32_t k = 0; k < na && keep; ++k) {
-        const uint32_t a = s.pls_adj[(size_t)p * kAdjCap + k];
-        const uint32_t b = a & 0x7FFFFFFFu;
+        const uint32_t b = s.pls_adj[(size_t)p * kAdjCap + k];
         if (s.pls_has5[b] || s.pls_has3[b]) keep = false;
-        else if ((a >> 31) && b < p && pls_unused(s, b)) keep = false;
+        else if (b < p && pls_unused(s, b)) keep = false;
       }
       s.pls_keep[p] = keep;
       f = keep;
@@ -390,13 +432,16 @@ static inline int grid_of(uint32_t n, int threads, int max_blocks) {
 
 void launch_dedup(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   const uint32_t cap_dd = s.cap_t5 + s.cap_pt5 + s.cap_pt3;
-  cudaMemsetAsync(s.inc_cnt, 0, sizeof(uint32_t) * 2 * ((size_t)s.cap_hits + 1), st);
+  cudaMemsetAsync(s.inc_cnt, 0, sizeof(uint32_t) * 2 * (3 * (size_t)s.cap_hits + 1), st);
   cudaMemsetAsync(s.pls_has5, 0, 3 * (size_t)s.cap_seeds, st);
   cudaMemsetAsync(s.hit_used5, 0, 2 * (size_t)s.cap_hits, st);
   k_pls_prep<<<1, 1024, 0, st>>>(s, c.par); LST_MARK(c, st, "k_pls_prep");
-  k_pls_adj<<<grid_of(s.cap_seeds, 8, c.n_sm * 8), 256, 0, st>>>(s, c.par); LST_MARK(c, st, "k_pls_adj");
+  cudaMemsetAsync(s.pid_key, 0, sizeof(unsigned long long) * (size_t)s.pid_size, st);
+  cudaMemsetAsync(s.pid_has5, 0, 2 * (size_t)s.pid_size, st);
+  k_pls_adj<<<grid_of(s.cap_seeds, 256, c.n_sm * 8), 256, 0, st>>>(s, c.par); LST_MARK(c, st, "k_pls_adj");
+  k_pid_insert<<<grid_of(4 * s.cap_seeds, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_pid_insert");
   k_dd_count<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_dd_count");
-  launch_scan(c, s, s.inc_cnt, s.inc_off, &s.hdr->n_hits, st);
+  launch_scan(c, s, s.inc_cnt, s.inc_off, &s.hdr->n_inc, st);
   k_dd_scatter<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_dd_scatter");
   k_s0<<<grid_of(cap_dd, 4, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s0");
   k_s1<<<grid_of(s.cap_pt3, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s1");

@@ -80,6 +80,7 @@ __global__ void __launch_bounds__(kThreads) k_md_fill(GeoDev geo, SlotDev s, Par
       s.md_hit[idx] = make_uint2(hl, hu);
       s.md_mod[idx] = (m << 2) | (uint32_t)cat;
       s.md_dphi[idx] = (float)o.dphi;
+      s.md_phi[idx] = atan2f(l.y, l.x);
     }
     __syncthreads();
   }

@@ -16,22 +16,35 @@ constexpr float kPxMarginLen = 5e-2f;   // cm, added to every z / r window
 
 __device__ __forceinline__ float asin_sat(float v) { return asinf(fminf(1.0f, fmaxf(-1.0f, v))); }
 
-// Can a hit inside module m's lower-sensor box pass the first-anchor cuts of seed (pt, eta, phi, z0, q)?
-__device__ __forceinline__ bool px_module_compatible(const GeoDev &geo, const Params &g, uint32_t m, float kp,
-                                                     float sh, float phi, float z0) {
-  const int cat = geo.category[m];
-  const float rlo = geo.rmin[m], rhi = geo.rmax[m], phic = geo.phic[m], hphi = geo.hphi[m];
-  const float zlo = geo.zmin[m], zhi = geo.zmax[m];
+__device__ __forceinline__ float wrap_f(float d) {   // to [-pi, pi]; error ~1e-7 |d|, far below kPxMarginPhi
+  return d - 6.2831853071795864769f * rintf(d * 0.15915494309189533577f);
+}
+
+// Can a hit inside a start module's lower-sensor box pass the first-anchor cuts of seed
+// (kp, sinh eta, phi, z0)?  b1 = {phic, hphi, rmin, rmax}, b2 = {zmin, zmax, category, -}.
+// A cheap necessary condition on the azimuth comes first (no inverse trigonometric function:
+// asin(x) <= x + (pi/2 - 1) x^3 on [0, 1]); it removes > 90 % of the (seed, module) pairs.
+__device__ __forceinline__ bool px_module_compatible(const Params &g, float4 b1, float4 b2, float kp, float sh,
+                                                     float phi, float z0) {
+  const int cat = (int)b2.z;
+  const float phic = b1.x, hphi = b1.y, rlo = b1.z, rhi = b1.w;
+  const float zlo = b2.x, zhi = b2.y;
   const float akp = fabsf(kp);
   const float sgn = kp < 0.0f ? -1.0f : 1.0f;
   const float ns = g.f_ns;
+  const float d0 = wrap_f(phic - phi);
   if (cat < 2) {
+    {
+      const float x = fminf(1.0f, akp * rhi);
+      const float ub = x + 0.5708f * x * x * x;   // >= asin(x) >= |kp| s(r) for every r in the box
+      const float sgp_ub = (float)g.seed_sig_phi + (float)g.seed_sig_pt * ub + g.f_sig_t[cat] / rlo;
+      if (fabsf(d0) > (hphi + ub + ns * sgp_ub) * kPreSlack + kPxMarginPhi + 1e-4f) return false;
+    }
     // barrel: arc length s(r) = asin(|k| r) / |k| is increasing in r
     const float a_lo = asin_sat(akp * rlo), a_hi = asin_sat(akp * rhi);
     const float s_lo = akp * rlo <= 1e-4f ? rlo : a_lo / akp, s_hi = akp * rhi <= 1e-4f ? rhi : a_hi / akp;
-    const float phim = phi + sgn * 0.5f * (a_lo + a_hi);
     const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * akp * s_hi + g.f_sig_t[cat] / rlo;
-    const float dphi = fabsf(remainderf(phic - phim, 6.2831853071795864769f));
+    const float dphi = fabsf(wrap_f(d0 - sgn * 0.5f * (a_lo + a_hi)));
     if (dphi > hphi + 0.5f * (a_hi - a_lo) + ns * sgp + kPxMarginPhi) return false;
     const float z1 = z0 + sh * s_lo, z2 = z0 + sh * s_hi;
     const float tol = ns * ((float)g.seed_sig_z + g.f_sig_z[cat]) + kPxMarginLen + 1e-3f * (fabsf(z1) + fabsf(z2));
@@ -42,7 +55,7 @@ __device__ __forceinline__ bool px_module_compatible(const GeoDev &geo, const Pa
   const float al = (zlo - z0) / sh;
   if (!(al > 0.0f)) return false;
   const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * akp * al + g.f_sig_t[cat] / rlo;
-  const float dphi = fabsf(remainderf(phic - (phi + kp * al), 6.2831853071795864769f));
+  const float dphi = fabsf(wrap_f(d0 - kp * al));
   if (dphi > hphi + ns * sgp + kPxMarginPhi + 1e-3f * akp * al) return false;
   const float ka = kp * al;
   const float rp = fabsf(ka) <= 1e-4f ? al : sinf(ka) / kp;
@@ -50,35 +63,97 @@ __device__ __forceinline__ bool px_module_compatible(const GeoDev &geo, const Pa
   return rp + tol >= rlo && rp - tol <= rhi;
 }
 
-// One warp per seed.  FILL = false: count the compatible start modules; FILL = true: write the
-// (seed, module) rows at the seed's offset, modules ascending.  (A seed with eta ~ 0 is compatible
-// with every endcap module of a side - its extrapolation tolerances diverge - so the lists are
-// sized exactly, not capped per seed.)
+// Stage 1 of the (seed, start module) test: the azimuthal window only, cheap and necessary.
+// Barrel: |phic - phi| against the widest window any r in the box allows (asin(x) <= x + (pi/2 - 1) x^3);
+// endcap: the exact azimuthal test (the arc length is fixed by the plane's z; inv_sh = 1 / sinh eta).
+__device__ __forceinline__ bool px_module_phi(const Params &g, float4 b1, float4 b2, float kp, float inv_sh,
+                                              float phi, float z0) {
+  const float akp = fabsf(kp);
+  const float d0 = wrap_f(b1.x - phi);
+  if (b2.z < 2.0f) {
+    const float x = fminf(1.0f, akp * b1.w);
+    const float ub = x + 0.5708f * x * x * x;
+    const float sgp_ub = (float)g.seed_sig_phi + (float)g.seed_sig_pt * ub + b2.w;
+    return !(fabsf(d0) > (b1.y + ub + g.f_ns * sgp_ub) * kPreSlack + kPxMarginPhi + 1e-4f);
+  }
+  const float al = (b2.x - z0) * inv_sh;
+  if (!(al > 0.0f)) return false;
+  const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * akp * al + b2.w;
+  return !(fabsf(wrap_f(d0 - kp * al)) > (b1.y + g.f_ns * sgp) * kPreSlack + kPxMarginPhi + 2e-3f * akp * al + 1e-4f);
+}
+
+// One warp per seed.  FILL = false: test every start module, keep one bit per (seed, module) and
+// count them: stage 1 (px_module_phi) on all modules, its survivors (~5 %) queued per warp and put
+// through the full test 32 at a time.  FILL = true: expand the bits into the (seed, module) rows at
+// the seed's offset, modules ascending.  (A seed with eta ~ 0 is compatible with every endcap
+// module of a side - its extrapolation tolerances diverge - so the lists are sized exactly, not
+// capped per seed.)  Dynamic shared memory: 8 warps x (nw words of bits + 64 queue entries).
 template <bool FILL>
 __global__ void __launch_bounds__(256) k_px_modules(GeoDev geo, SlotDev s, Params g) {
+  extern __shared__ uint32_t px_sh[];
   const uint32_t n_seeds = s.hdr->n_seeds;
-  const int lane = threadIdx.x & 31;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+  const uint32_t nw = (geo.n_start + 31) / 32;
   if (FILL && s.hdr->n_obj[kPairLevel] == 0) return;
+  uint32_t *wbits = px_sh + (size_t)wib * (nw + 64), *queue = wbits + nw;
   for (uint32_t p = warp; p < n_seeds; p += nwarp) {
-    const float pt = s.seed_pt[p], phi = s.seed_phi[p], z0 = s.seed_z0[p];
-    const float kp = -(float)s.seed_q[p] * (float)g.kB / (2.0f * pt);
-    const float sh = sinhf(s.seed_eta[p]);
-    const uint32_t off = FILL ? s.px_off[p] : 0u;
-    uint32_t cnt = 0;
-    for (uint32_t base = 0; base < geo.n_start; base += 32) {
-      const uint32_t k = base + lane;
-      bool ok = false;
-      uint32_t m = 0;
-      if (k < geo.n_start && pt > 0.0f) {
-        m = geo.start_mods[k];
-        ok = px_module_compatible(geo, g, m, kp, sh, phi, z0);
+    uint32_t *bits = s.px_bits + (size_t)p * nw;
+    if (FILL) {
+      uint32_t pos = s.px_off[p];
+      for (uint32_t w = 0; w < nw; ++w) {
+        const uint32_t b = bits[w];
+        if ((b >> lane) & 1u)
+          s.px_pair[pos + __popc(b & ((1u << lane) - 1u))] = make_uint2(p, geo.start_mods[w * 32 + lane]);
+        pos += __popc(b);
       }
-      const uint32_t b = __ballot_sync(0xffffffffu, ok);
-      if (FILL && ok) s.px_pair[off + cnt + __popc(b & ((1u << lane) - 1u))] = make_uint2(p, m);
-      cnt += __popc(b);
+    } else {
+      const float pt = s.seed_pt[p], phi = s.seed_phi[p], z0 = s.seed_z0[p];
+      const float kp = -(float)s.seed_q[p] * (float)g.kB / (2.0f * pt);
+      const float sh = sinhf(s.seed_eta[p]);
+      const float inv_sh = 1.0f / sh;
+      const bool seed_ok = fabsf(sh) > 1e-9f;   // endcap planes are unreachable for sinh eta ~ 0
+      for (uint32_t w = lane; w < nw; w += 32) wbits[w] = 0;
+      __syncwarp();
+      uint32_t nq = 0;
+      for (uint32_t w = 0; w <= nw; ++w) {
+        if (w < nw) {
+          const uint32_t k = w * 32 + lane;
+          bool ok = false;
+          if (k < geo.n_start && pt > 0.0f) {
+            const float4 b1 = geo.start_box[k], b2 = geo.start_box2[k];
+            ok = (b2.z < 2.0f || seed_ok) && px_module_phi(g, b1, b2, kp, inv_sh, phi, z0);
+          }
+          const uint32_t b = __ballot_sync(0xffffffffu, ok);
+          if (ok) queue[nq + __popc(b & ((1u << lane) - 1u))] = k;
+          nq += __popc(b);
+          __syncwarp();
+        }
+        if (nq >= 32 || (w == nw && nq > 0)) {
+          const uint32_t take = nq < 32 ? nq : 32;
+          if ((uint32_t)lane < take) {
+            const uint32_t k = queue[lane];
+            if (px_module_compatible(g, geo.start_box[k], geo.start_box2[k], kp, sh, phi, z0))
+              atomicOr(&wbits[k >> 5], 1u << (k & 31));
+          }
+          __syncwarp();
+          const uint32_t mv = (uint32_t)lane + 32 < nq ? queue[lane + 32] : 0u;
+          __syncwarp();
+          if ((uint32_t)lane + 32 < nq) queue[lane] = mv;
+          nq -= take;
+          __syncwarp();
+        }
+      }
+      uint32_t cnt = 0;
+      for (uint32_t w = lane; w < nw; w += 32) {
+        const uint32_t b = wbits[w];
+        bits[w] = b;
+        cnt += __popc(b);
+      }
+      cnt = warp_sum(cnt);
+      if (lane == 0) s.px_cnt[p] = cnt;
+      __syncwarp();
     }
-    if (!FILL && lane == 0) s.px_cnt[p] = cnt;
   }
 }
 
@@ -107,7 +182,9 @@ void launch_pixel(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   const int warps_per_block = 8;
   int g = (int)((s.cap_seeds + warps_per_block - 1) / warps_per_block);
   if (g > c.n_sm * 8) g = c.n_sm * 8;
-  k_px_modules<false><<<g, 256, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_px_modules<false>");
+  const size_t shb = 8 * ((size_t)(c.geo.n_start + 31) / 32 + 64) * sizeof(uint32_t);
+  if (shb > 48 * 1024) cudaFuncSetAttribute(k_px_modules<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shb);
+  k_px_modules<false><<<g, 256, shb, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_px_modules<false>");
   k_px_offsets<<<1, 1024, 0, st>>>(s); LST_MARK(c, st, "k_px_offsets");
   k_px_modules<true><<<g, 256, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_px_modules<true>");
   launch_join(c, s, 2, st);            // pT5

@@ -124,12 +124,44 @@ __device__ __forceinline__ bool t5_candidate(const SlotDev &s, const Params &g, 
   return t5_eval_d(g, P, k3a.x, k3a.y, k3b.x, k3b.y, o);
 }
 
-// pT5 / pT3 candidate: pixel seed `p` against OT object `obj` (reading C6).  The fp32 pre-filter tests
+// pT5 / pT3 candidate: pixel seed against OT object `obj` (reading C6).  The fp32 pre-filter tests
 // the first anchor only, loosened by kPreSlack plus absolute slacks far above the fp32 error
 // (1e-5 rad on a >= 4e-3 rad window, 2e-3 cm on a >= 0.2 cm window); it never rejects on NaN.
+// sp = {kappa_p, sinh eta, phi, z0} of the seed, computed once per row (stage_seeds).
+template <int KIND>
+__device__ __forceinline__ bool px_pre_f(const SlotDev &s, const Params &g, float4 sp, uint32_t obj) {
+  const uint32_t m0 = KIND == J_PT5 ? s.t5_md[5 * (size_t)obj] : s.t3_md[obj].x;
+  const float4 h = s.md_pos[m0];
+  const int cat = (int)(s.md_mod[m0] & 3u);
+  const float kp = sp.x, sh = sp.y;
+  float al;
+  if (cat < 2) {
+    const float kr = kp * h.w;
+    al = fabsf(kr) <= 1e-4f ? h.w : asinf(fminf(1.0f, fmaxf(-1.0f, kr))) / kp;
+  } else {
+    al = (h.z - sp.w) / sh;
+  }
+  const float d = s.md_phi[m0] - (sp.z + kp * al);
+  const float dph = d - 6.2831853071795864769f * rintf(d * 0.15915494309189533577f);
+  const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * fabsf(kp) * al + g.f_sig_t[cat] / h.w;
+  if (fabsf(dph) > g.f_ns * sgp * kPreSlack + 1e-5f) return false;
+  float dzt, szt;
+  if (cat < 2) {
+    dzt = h.z - (sp.w + sh * al);
+    szt = (float)g.seed_sig_z + g.f_sig_z[cat];
+  } else {
+    const float ka = kp * al;
+    dzt = h.w - (fabsf(ka) <= 1e-4f ? al : sinf(ka) / kp);
+    szt = (float)g.seed_sig_z / fabsf(sh) + g.f_sig_r[cat];
+  }
+  if (fabsf(dzt) > g.f_ns * szt * kPreSlack + 2e-3f) return false;
+  return true;
+}
+
+// fp64 decision (and chi2_pix) of one (seed, object) pair.
 template <int KIND>
 __device__ __forceinline__ bool px_candidate(const GeoDev &geo, const SlotDev &s, const Params &g, uint32_t p,
-                                             uint32_t obj, double *chi2, bool prefilter) {
+                                             uint32_t obj, double *chi2) {
   constexpr int N = KIND == J_PT5 ? 5 : 3;
   uint32_t m[5];
   if (KIND == J_PT5) {
@@ -139,52 +171,52 @@ __device__ __forceinline__ bool px_candidate(const GeoDev &geo, const SlotDev &s
     const uint4 t = s.t3_md[obj];
     m[0] = t.x; m[1] = t.y; m[2] = t.z;
   }
-  const float spt = s.seed_pt[p], seta = s.seed_eta[p], sphi = s.seed_phi[p], sz0 = s.seed_z0[p];
-  const int q = s.seed_q[p];
-  const uint32_t mm0 = s.md_mod[m[0]];
-  if (prefilter) {
-    const float4 h = s.md_pos[m[0]];
-    const int cat = (int)(mm0 & 3u);
-    const float kp = -(float)q * (float)g.kB / (2.0f * spt);
-    const float sh = sinhf(seta);
-    float al;
-    if (cat < 2) {
-      const float kr = kp * h.w;
-      al = fabsf(kr) <= 1e-4f ? h.w : asinf(fminf(1.0f, fmaxf(-1.0f, kr))) / kp;
-    } else {
-      al = (h.z - sz0) / sh;
-    }
-    const float dph = remainderf(atan2f(h.y, h.x) - (sphi + kp * al), 6.2831853071795864769f);
-    const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * fabsf(kp) * al + g.f_sig_t[cat] / h.w;
-    if (fabsf(dph) > g.f_ns * sgp * kPreSlack + 1e-5f) return false;
-    float dzt, szt;
-    if (cat < 2) {
-      dzt = h.z - (sz0 + sh * al);
-      szt = (float)g.seed_sig_z + g.f_sig_z[cat];
-    } else {
-      const float ka = kp * al;
-      dzt = h.w - (fabsf(ka) <= 1e-4f ? al : sinf(ka) / kp);
-      szt = (float)g.seed_sig_z / fabsf(sh) + g.f_sig_r[cat];
-    }
-    if (fabsf(dzt) > g.f_ns * szt * kPreSlack + 2e-3f) return false;
-  }
   Seed sd;
-  sd.pt = (double)spt; sd.eta = (double)seta; sd.phi = (double)sphi; sd.z0 = (double)sz0; sd.q = q;
+  sd.pt = (double)s.seed_pt[p]; sd.eta = (double)s.seed_eta[p]; sd.phi = (double)s.seed_phi[p];
+  sd.z0 = (double)s.seed_z0[p]; sd.q = s.seed_q[p];
   Pt P[N];
 #pragma unroll
   for (int k = 0; k < N; ++k) P[k] = md_point(s, m[k]);
   double c2 = 0.0;
-  const bool ok = px_eval_d(g, sd, P, N, (int)geo.layer[mm0 >> 2], &c2);
+  const bool ok = px_eval_d(g, sd, P, N, (int)geo.layer[s.md_mod[m[0]] >> 2], &c2);
   if (chi2) *chi2 = c2;
   return ok;
 }
 
+// per-row seed parameters of the pixel joins: {kappa_p, sinh eta, phi, z0}
+__device__ __forceinline__ void stage_seeds(float4 *rowseed, const SlotDev &s, const Params &g, uint32_t r0,
+                                            uint32_t n_rows) {
+  const int tid = threadIdx.x;   // kThreads == kRowChunk
+  float4 v = make_float4(0.f, 1.f, 0.f, 0.f);
+  if (r0 + tid < n_rows) {
+    const uint32_t p = s.px_pair[r0 + tid].x;
+    v.x = -(float)s.seed_q[p] * (float)g.kB / (2.0f * s.seed_pt[p]);
+    v.y = sinhf(s.seed_eta[p]);
+    v.z = s.seed_phi[p];
+    v.w = s.seed_z0[p];
+  }
+  rowseed[tid] = v;
+}
+
+// Phase 1 of a join candidate: a cheap necessary condition evaluated on every candidate (T5: the
+// radius match T5-1 on the stored kappa3; pixel: the fp32 first-anchor pre-filter).  T3 has none.
+template <int KIND>
+__device__ __forceinline__ bool join_phase1(const SlotDev &s, const Params &g, uint32_t row, uint32_t b,
+                                            const float4 *rowseed, int lrow) {
+  if (KIND == J_T3) return true;
+  if (KIND == J_T5) {
+    const double2 k3a = s.t3_kd[row], k3b = s.t3_kd[b];
+    return le(fabs(k3a.x - k3b.x), g.ns * (k3a.y + k3b.y));
+  }
+  return px_pre_f<KIND>(s, g, rowseed[lrow], b);
+}
+// Phase 2: the fp64 decision.
 template <int KIND>
 __device__ __forceinline__ bool join_candidate(const GeoDev &geo, const SlotDev &s, const Params &g, uint32_t row,
                                                uint32_t b) {
   if (KIND == J_T3) return t3_candidate(s, g, row, b, nullptr, nullptr);
   if (KIND == J_T5) return t5_candidate(s, g, row, b, nullptr, nullptr, nullptr, nullptr);
-  return px_candidate<KIND>(geo, s, g, s.px_pair[row].x, b, nullptr, true);
+  return px_candidate<KIND>(geo, s, g, s.px_pair[row].x, b, nullptr);
 }
 
 template <int KIND>
@@ -192,6 +224,7 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
   __shared__ ItemScratch sc;
   __shared__ RowTab rt;
   __shared__ uint32_t sh[33];
+  __shared__ float4 rowseed[(KIND == J_PT5 || KIND == J_PT3) ? kRowChunk : 1];
   const int stage = JoinTraits<KIND>::stage;
   const StageBuf &st = s.st[stage];
   const uint32_t n_items = s.hdr->n_items[stage];
@@ -201,18 +234,42 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
     const Item item = st.items[it];
     const uint32_t r0 = item.group * kRowChunk;
     if (tid < kItemWords) sc.mask[tid] = 0;
+    if (tid == 0) sc.n = 0;
+    if (KIND == J_PT5 || KIND == J_PT3) stage_seeds(rowseed, s, g, r0, n_rows);
     stage_rows<KIND>(rt, s, r0, n_rows, sh);
     const int nj = item.nj;
-    for (int base = 0; base < nj; base += kThreads) {
-      const int c = base + tid;
-      bool pass = false;
-      if (c < nj) {
+    if (KIND == J_T3) {
+      for (int base = 0; base < nj; base += kThreads) {
+        const int c = base + tid;
+        bool pass = false;
+        if (c < nj) {
+          int row; uint32_t b;
+          flat_to_pair(rt, item.j0 + c, &row, &b);
+          pass = join_candidate<KIND>(geo, s, g, r0 + row, b);
+        }
+        const uint32_t w = __ballot_sync(0xffffffffu, pass);
+        if ((tid & 31) == 0) sc.mask[c >> 5] = w;
+      }
+    } else {
+      // phase 1 on every candidate, survivors compacted; phase 2 (fp64) on the dense survivor list
+      for (int base = 0; base < nj; base += kThreads) {
+        const int c = base + tid;
+        bool keep = false;
+        if (c < nj) {
+          int row; uint32_t b;
+          flat_to_pair(rt, item.j0 + c, &row, &b);
+          keep = join_phase1<KIND>(s, g, r0 + row, b, rowseed, row);
+        }
+        push_survivor(sc, keep, (uint32_t)c);
+      }
+      __syncthreads();
+      const int nsv = (int)sc.n;
+      for (int k = tid; k < nsv; k += kThreads) {
+        const int c = sc.list[k];
         int row; uint32_t b;
         flat_to_pair(rt, item.j0 + c, &row, &b);
-        pass = join_candidate<KIND>(geo, s, g, r0 + row, b);
+        if (join_candidate<KIND>(geo, s, g, r0 + row, b)) atomicOr(&sc.mask[c >> 5], 1u << (c & 31));
       }
-      const uint32_t w = __ballot_sync(0xffffffffu, pass);
-      if ((tid & 31) == 0) sc.mask[c >> 5] = w;
     }
     __syncthreads();
     publish_mask(sc, st.mask + (size_t)it * kItemWords, st.item_cnt + it);
@@ -262,7 +319,7 @@ __global__ void __launch_bounds__(kThreads) k_join_fill(GeoDev geo, SlotDev s, P
       } else {
         const uint32_t p = s.px_pair[a].x;
         double c2 = 0.0;
-        px_candidate<KIND>(geo, s, g, p, b, &c2, false);
+        px_candidate<KIND>(geo, s, g, p, b, &c2);
         if (KIND == J_PT5) { s.pt5_po[idx] = make_uint2(p, b); s.pt5_chi2[idx] = c2; }
         else { s.pt3_po[idx] = make_uint2(p, b); s.pt3_chi2[idx] = c2; }
       }

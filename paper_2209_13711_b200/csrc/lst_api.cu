@@ -278,6 +278,7 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.hit = w.take<float4>(nh); s.hit_orig = w.take<uint32_t>(nh);
   s.md_pos = w.take<float4>(s.cap_md); s.md_kd = w.take<double2>(s.cap_md); s.md_kf = w.take<float2>(s.cap_md);
   s.md_hit = w.take<uint2>(s.cap_md); s.md_mod = w.take<uint32_t>(s.cap_md); s.md_dphi = w.take<float>(s.cap_md);
+  s.md_phi = w.take<float>(s.cap_md);
   s.md_mod_off = w.take<uint32_t>(n_mod + 1);
   s.ls_md = w.take<uint2>(s.cap_ls); s.ls_f = w.take<float4>(s.cap_ls);
   s.ls_md_off = w.take<uint32_t>((size_t)s.cap_md + 1);
@@ -293,14 +294,20 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.pt5_keep = w.take<uint8_t>(s.cap_pt5); s.pt3_keep = w.take<uint8_t>(s.cap_pt3);
   s.pls_keep = w.take<uint8_t>(nsd);
   s.px_cnt = w.take<uint32_t>(nsd);
+  s.px_bits = w.take<uint32_t>((size_t)nsd * ((c->k.geo.n_start + 31) / 32));
   s.px_off = w.take<uint32_t>((size_t)nsd + 1); s.px_pair = w.take<uint2>((size_t)nsd * kPxCap);
   s.pt5_pls_off = w.take<uint32_t>((size_t)nsd + 1); s.pt3_pls_off = w.take<uint32_t>((size_t)nsd + 1);
   s.t5_hits = w.take<uint32_t>(10 * (size_t)s.cap_t5); s.pt3_hits = w.take<uint32_t>(6 * (size_t)s.cap_pt3);
-  s.inc_cnt = w.take<uint32_t>(2 * ((size_t)nh + 1)); s.inc_cur = s.inc_cnt ? s.inc_cnt + nh + 1 : nullptr;
-  s.inc_off = w.take<uint32_t>((size_t)nh + 1);
+  s.inc_cnt = w.take<uint32_t>(2 * (3 * (size_t)nh + 1)); s.inc_cur = s.inc_cnt ? s.inc_cnt + 3 * (size_t)nh + 1 : nullptr;
+  s.inc_off = w.take<uint32_t>(3 * (size_t)nh + 1);
   s.inc_ent = w.take<uint32_t>(10 * (size_t)s.cap_t5 + 10 * (size_t)s.cap_pt5 + 6 * (size_t)s.cap_pt3);
   s.pls_bin_off = w.take<uint32_t>(kEtaBins + 1); s.pls_bin_ent = w.take<uint32_t>(nsd);
   s.pls_adj_cnt = w.take<uint32_t>(nsd); s.pls_adj = w.take<uint32_t>((size_t)nsd * kAdjCap);
+  s.pid_size = 64;
+  while (s.pid_size < 8 * (size_t)nsd && s.pid_size < (1u << 31)) s.pid_size <<= 1;
+  s.pid_key = w.take<unsigned long long>(s.pid_size);
+  s.pls_slot = w.take<uint32_t>(4 * (size_t)nsd);
+  s.pid_has5 = w.take<uint8_t>(2 * (size_t)s.pid_size); s.pid_has3 = s.pid_has5 ? s.pid_has5 + s.pid_size : nullptr;
   s.pls_has5 = w.take<uint8_t>(3 * (size_t)nsd);
   s.pls_has3 = s.pls_has5 ? s.pls_has5 + nsd : nullptr; s.pls_near_t5 = s.pls_has5 ? s.pls_has5 + 2 * (size_t)nsd : nullptr;
   s.hit_used5 = w.take<uint8_t>(2 * (size_t)nh); s.hit_used3 = s.hit_used5 ? s.hit_used5 + nh : nullptr;
@@ -384,7 +391,8 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   const size_t o_box = o_cols + up((size_t)std::max<uint32_t>(nnz, 1) * 4);
   const size_t box_stride = up((size_t)n * 4);
   const size_t o_start = o_box + 6 * box_stride;
-  const size_t total = o_start + std::max<size_t>(start_mods.size(), 1) * 4;
+  const size_t o_sbox = o_start + up(std::max<size_t>(start_mods.size(), 1) * 4);
+  const size_t total = o_sbox + 2 * up(std::max<size_t>(start_mods.size(), 1) * 16);
   e = cudaMalloc(&c->d_static, total);
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaMalloc(static)"); }
   char *d = (char *)c->d_static;
@@ -396,6 +404,21 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   for (int k = 0; k < 6; ++k) cudaMemcpy(d + o_box + k * box_stride, box[k], (size_t)n * 4, cudaMemcpyHostToDevice);
   if (!start_mods.empty())
     cudaMemcpy(d + o_start, start_mods.data(), start_mods.size() * 4, cudaMemcpyHostToDevice);
+  {
+    std::vector<float> sb(8 * std::max<size_t>(start_mods.size(), 1), 0.0f);
+    float *b1 = sb.data(), *b2 = sb.data() + 4 * std::max<size_t>(start_mods.size(), 1);
+    for (size_t k = 0; k < start_mods.size(); ++k) {
+      const uint32_t m = start_mods[k];
+      b1[4 * k] = g->phic[m]; b1[4 * k + 1] = g->half_phi[m]; b1[4 * k + 2] = g->rmin[m]; b1[4 * k + 3] = g->rmax[m];
+      b2[4 * k] = g->zmin[m]; b2[4 * k + 1] = g->zmax[m]; b2[4 * k + 2] = (float)g->category[m];
+      b2[4 * k + 3] = c->k.par.f_sig_t[g->category[m] & 3] / g->rmin[m];
+    }
+    const size_t nb = std::max<size_t>(start_mods.size(), 1) * 16;
+    cudaMemcpy(d + o_sbox, b1, nb, cudaMemcpyHostToDevice);
+    cudaMemcpy(d + o_sbox + up(nb), b2, nb, cudaMemcpyHostToDevice);
+    c->k.geo.start_box = (const float4 *)(d + o_sbox);
+    c->k.geo.start_box2 = (const float4 *)(d + o_sbox + up(nb));
+  }
   e = cudaDeviceSynchronize();
   if (e != cudaSuccess) { cudaFree(c->d_static); delete c; return cuda_fail(e, "upload geometry"); }
   c->k.geo.n_modules = n; c->k.geo.n_det = 2 * n;
@@ -577,7 +600,7 @@ extern "C" int lst_get_counts(lst_ctx *c, uint32_t slot, uint32_t *counts, uint6
   const int rc = sync_header(c, s);
   if (rc != LST_OK) return rc;
   for (int l = 0; l < LST_NLEVEL; ++l) counts[l] = s.h_hdr->n_obj[l];
-  if (cand) for (int k = 0; k < 4; ++k) cand[k] = s.h_hdr->cand[k];
+  if (cand) for (int k = 0; k < S_NSTAGE; ++k) cand[k] = s.h_hdr->cand[k];
   return LST_OK;
 }
 

@@ -56,7 +56,7 @@ struct Header {          // per slot, device; zeroed (except n_hits / n_seeds) a
   uint32_t err;
   uint32_t n_dd;                     // T5 + pT5 + pT3 objects entering the cleaning
   uint32_t n_flag;                   // pT5 + pT3 + T5 + seeds: length of the TC keep-flag array
-  uint32_t pad;
+  uint32_t n_inc;                    // 3 * n_hits: rows of the (hit, object type) -> objects incidence
   unsigned long long cand[S_NSTAGE]; // candidates enumerated per stage
 };
 
@@ -79,6 +79,8 @@ struct GeoDev {
   // boxes of the lower sensors (lst_geometry) and the modules that may start a pT3 / pT5 (C6)
   const float *rmin, *rmax, *phic, *hphi, *zmin, *zmax;
   const uint32_t *start_mods;
+  // the same modules' boxes packed for k_px_modules: {phic, hphi, rmin, rmax}, {zmin, zmax, category, sig_t / rmin}
+  const float4 *start_box, *start_box2;
   uint32_t n_start;
 };
 
@@ -100,6 +102,7 @@ struct SlotDev {
   uint2 *md_hit;         // sorted positions of lower / upper hit
   uint32_t *md_mod;      // module << 2 | category
   float *md_dphi;
+  float *md_phi;         // azimuth of the anchor, fp32 (pixel-linking pre-filter)
   uint32_t *md_mod_off;  // [n_modules+1]
   // LS
   uint2 *ls_md;          // inner, outer MD
@@ -125,17 +128,24 @@ struct SlotDev {
   double *pt5_chi2, *pt3_chi2;
   uint8_t *pt5_keep, *pt3_keep, *pls_keep;
   uint32_t *px_cnt;                // [cap_seeds] compatible start modules of a seed
+  uint32_t *px_bits;               // [cap_seeds * ceil(n_start / 32)] one bit per (seed, start module)
   uint32_t *px_off;                // [cap_seeds+1]
   uint2 *px_pair;                  // [cap_seeds * kPxCap] (seed, module), ascending: rows of the pixel joins
   uint32_t *pt5_pls_off, *pt3_pls_off;   // [cap_seeds+1] pT5 / pT3 range of a seed
   // a6 cleaning
   uint32_t *t5_hits, *pt3_hits;    // [10 cap_t5], [6 cap_pt3] sorted hit positions in layer order
-  uint32_t *inc_cnt, *inc_cur;     // [cap_hits+1] each, contiguous: hit -> objects incidence
-  uint32_t *inc_off;               // [cap_hits+1]
+  uint32_t *inc_cnt, *inc_cur;     // [3 cap_hits+1] each, contiguous: (hit, type) -> objects incidence, row 3 h + type
+  uint32_t *inc_off;               // [3 cap_hits+1]
   uint32_t *inc_ent;               // [10 cap_t5 + 10 cap_pt5 + 6 cap_pt3] object ids (T5 | pT5 | pT3)
   uint32_t *pls_bin_off;           // [kEtaBins+1]
   uint32_t *pls_bin_ent;           // [cap_seeds]
-  uint32_t *pls_adj_cnt, *pls_adj; // [cap_seeds], [cap_seeds * kAdjCap]: related seeds (bit 31: close in eta-phi)
+  uint32_t *pls_adj_cnt, *pls_adj; // [cap_seeds], [cap_seeds * kAdjCap]: seeds close in eta-phi to a seed
+  // pixel-hit ids: open-addressing hash set (key = 1 << 32 | id, 0 = empty), the slot of each of a
+  // seed's 4 ids, and per slot "some surviving pT5 / pT3 uses a seed with this pixel hit"
+  unsigned long long *pid_key;     // [pid_size]
+  uint32_t *pls_slot;              // [4 * cap_seeds]
+  uint8_t *pid_has5, *pid_has3;    // [pid_size] each, contiguous
+  uint32_t pid_size;               // power of two >= 8 * cap_seeds
   uint8_t *pls_has5, *pls_has3, *pls_near_t5;   // [cap_seeds] each, contiguous
   uint8_t *hit_used5, *hit_used3;  // [cap_hits] each, contiguous: hit belongs to a surviving pT5 / pT3 (S1, S2)
   uint32_t *tc_flag, *tc_pos;      // [cap_tc+1]
@@ -210,7 +220,7 @@ __device__ __forceinline__ void push_survivor(ItemScratch &s, bool keep, uint32_
 }
 
 // fill helper: ordered list of set bits of the item's mask.  Call with all threads; needs
-// kThreads >= kItemWords.  After return s.list[0..s.n) holds the candidates in ascending order.
+// kThreads >= 4 * kItemWords.  After return s.list[0..s.n) holds the candidates in ascending order.
 __device__ __forceinline__ void expand_mask(ItemScratch &s, const uint32_t *gmask) {
   const int t = threadIdx.x;
   if (t < 32) {
@@ -222,9 +232,18 @@ __device__ __forceinline__ void expand_mask(ItemScratch &s, const uint32_t *gmas
     if (t == 0) { s.pre[kItemWords] = tot; s.n = tot; }
   }
   __syncthreads();
-  for (int c = t; c < kItemCand; c += blockDim.x) {
-    const uint32_t w = s.mask[c >> 5];
-    if ((w >> (c & 31)) & 1u) s.list[s.pre[c >> 5] + __popc(w & ((1u << (c & 31)) - 1u))] = (uint16_t)c;
+  {   // 4 threads per mask word, each walks the set bits of one byte (items are sparse: ~2 % pass)
+    const int wd = t >> 2, by = t & 3;
+    if (wd < kItemWords) {
+      const uint32_t w = s.mask[wd];
+      uint32_t bits = (w >> (8 * by)) & 0xFFu;
+      uint32_t pos = s.pre[wd] + __popc(w & ((1u << (8 * by)) - 1u));
+      while (bits) {
+        const int b = __ffs(bits) - 1;
+        bits &= bits - 1;
+        s.list[pos++] = (uint16_t)(wd * 32 + 8 * by + b);
+      }
+    }
   }
   __syncthreads();
 }
