@@ -219,46 +219,52 @@ __global__ void k_dd_scatter(SlotDev s) {
 // any n_ot - min_shared + 1 of them, so only the incidence lists (of A's own type) of hits
 // k0..n_ot-1 are searched; the lists are flattened into one index space that the lanes stride
 // (their lengths are very uneven: inner-layer hits sit in hundreds of objects).  Per entry B the
-// cheap tests come first: score(B) <= score(A), then a NECESSARY condition for ">= min_shared
-// shared hits" -- the number of B's hits whose hash bit is set in A's 64-bit hit signature -- and
-// only then the exact hit-set intersection and the full "B beats A" order.
+// cheap test comes first (score(B) <= score(A)); the shared-hit count is exact and costs one
+// shared-memory lookup per hit of B: A's hits sit in a 256-slot table per warp (slot = hit & 255;
+// an A whose hits collide in the table - ~16 % - counts with the 10 x 10 comparison instead).
+constexpr int kS0Slots = 256;
 __device__ __forceinline__ double dd_score(const SlotDev &s, uint32_t n5, uint32_t np5, uint32_t d) {
   return d < n5 ? s.t5_chi2[d] : (d < n5 + np5 ? s.pt5_chi2[d - n5] : s.pt3_chi2[d - n5 - np5]);
 }
 __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
   __shared__ uint32_t sh_pre[4][12], sh_beg[4][12];
+  __shared__ uint32_t sh_tab[4][kS0Slots];
   const Header *hdr = s.hdr;
   const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = hdr->n_dd;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
-  uint32_t *pre = sh_pre[wib], *beg = sh_beg[wib];
+  uint32_t *pre = sh_pre[wib], *beg = sh_beg[wib], *tab = sh_tab[wib];
+  for (int k = lane; k < kS0Slots; k += 32) tab[k] = 0xFFFFFFFFu;
+  __syncwarp();
   for (uint32_t d = warp; d < n_dd; d += nwarp) {
     const DRef A = dd_ref(s, n5, np5, d);
-    uint32_t ha[10];
-    unsigned long long sigA = 0ull;
-#pragma unroll
-    for (int q = 0; q < 10; ++q) {
-      ha[q] = q < A.n_ot ? A.hits[q] : 0xFFFFFFFFu;
-      if (q < A.n_ot) sigA |= 1ull << (ha[q] & 63u);
-    }
+    // lane q < n_ot owns hit q of A
+    const uint32_t my_hit = lane < A.n_ot ? A.hits[lane] : 0xFFFFFFFFu;
     bool beaten = false;
     if (g.s0_enabled) {
       const int min_shared = A.type == 0 ? g.dup_t5 : (A.type == 1 ? g.dup_pt5 : g.dup_pt3);
       const int k0 = min_shared - 1, nl = A.n_ot > k0 ? A.n_ot - k0 : 0;   // lists searched: hits k0 .. n_ot-1
+      // table of A's hits; collisions (two hits of A in one slot) -> exact comparison path
+      const uint32_t slot = my_hit & (kS0Slots - 1);
+      const uint32_t same = __match_any_sync(0xffffffffu, lane < A.n_ot ? slot : 0x10000u + lane);
+      const bool collide = __any_sync(0xffffffffu, lane < A.n_ot && __popc(same) > 1);
+      if (lane < A.n_ot) tab[slot] = my_hit;
       {
         uint32_t len = 0, b0 = 0;
-        if (lane < nl) {
-          const uint32_t row = 3 * A.hits[k0 + lane] + (uint32_t)A.type;
+        if (lane >= k0 && lane < A.n_ot) {
+          const uint32_t row = 3 * my_hit + (uint32_t)A.type;
           b0 = s.inc_off[row]; len = s.inc_off[row + 1] - b0;
         }
+        // lists in lanes k0 .. n_ot-1: shift them down to lanes 0 .. nl-1
+        len = __shfl_down_sync(0xffffffffu, len, k0);
+        b0 = __shfl_down_sync(0xffffffffu, b0, k0);
+        if (lane >= nl) len = 0;
         uint32_t tot;
         const uint32_t ex = warp_excl_scan(len, &tot);
-        __syncwarp();
         if (lane < 11) { pre[lane] = ex; beg[lane] = b0; }      // lanes >= nl: pre = total
         __syncwarp();
       }
-      const int nlc = nl < 10 ? nl : 10;
-      const uint32_t total = pre[nlc];
+      const uint32_t total = pre[nl < 10 ? nl : 10];
       const double *score_arr = A.type == 0 ? s.t5_chi2 : (A.type == 1 ? s.pt5_chi2 : s.pt3_chi2);
       const uint32_t dbase = A.type == 0 ? 0u : (A.type == 1 ? n5 : n5 + np5);
       int cur = 0;
@@ -269,26 +275,34 @@ __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
           while (i >= pre[cur + 1]) ++cur;
           const uint32_t b = s.inc_ent[beg[cur] + (i - pre[cur])];
           if (b != d && !(score_arr[b - dbase] > A.score)) {
-            const uint32_t *hb = A.type == 0 ? s.t5_hits + 10 * (size_t)b
-                               : (A.type == 1 ? s.t5_hits + 10 * (size_t)s.pt5_po[b - dbase].y
-                                              : s.pt3_hits + 6 * (size_t)(b - dbase));
-            const uint2 *hb2 = reinterpret_cast<const uint2 *>(hb);
-            int cnt = 0;
+            int cnt;
+            if (!collide) {
+              const uint32_t *hb = A.type == 0 ? s.t5_hits + 10 * (size_t)b
+                                 : (A.type == 1 ? s.t5_hits + 10 * (size_t)s.pt5_po[b - dbase].y
+                                                : s.pt3_hits + 6 * (size_t)(b - dbase));
+              const uint2 *hb2 = reinterpret_cast<const uint2 *>(hb);
+              cnt = 0;
 #pragma unroll
-            for (int q = 0; q < 5; ++q) {
-              if (2 * q < A.n_ot) {
-                const uint2 v = hb2[q];
-                cnt += (int)((sigA >> (v.x & 63u)) & 1ull) + (int)((sigA >> (v.y & 63u)) & 1ull);
+              for (int q = 0; q < 5; ++q) {
+                if (2 * q < A.n_ot) {
+                  const uint2 v = hb2[q];
+                  cnt += (int)(tab[v.x & (kS0Slots - 1)] == v.x) + (int)(tab[v.y & (kS0Slots - 1)] == v.y);
+                }
               }
-            }
-            if (cnt >= min_shared) {
+            } else {
+              uint32_t ha[10];
+#pragma unroll
+              for (int q = 0; q < 10; ++q) ha[q] = q < A.n_ot ? A.hits[q] : 0xFFFFFFFFu;
               const DRef Bq = dd_ref(s, n5, np5, b);
-              hit = dd_shared(ha, A.n_ot, Bq.hits, Bq.n_ot) >= min_shared && dd_beats(s, Bq, A);
+              cnt = dd_shared(ha, A.n_ot, Bq.hits, Bq.n_ot);
             }
+            if (cnt >= min_shared) hit = dd_beats(s, dd_ref(s, n5, np5, b), A);
           }
         }
         beaten = __any_sync(0xffffffffu, hit);
       }
+      __syncwarp();
+      if (lane < A.n_ot) tab[slot] = 0xFFFFFFFFu;                 // leave the table empty for the next object
       if (!beaten && A.type != 0) {   // objects of the same pixel seed are duplicates of one another
         const uint32_t *off = A.type == 1 ? s.pt5_pls_off : s.pt3_pls_off;
         const uint32_t dbase = A.type == 1 ? n5 : n5 + np5;
@@ -310,8 +324,7 @@ __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
         if (keep) {
           s.pls_has5[A.pls] = 1;
           pid_mark(s, s.pid_has5, A.pls);
-#pragma unroll
-          for (int q = 0; q < 10; ++q) s.hit_used5[ha[q]] = 1;   // S1 / S2: "shares a hit with a surviving pT5"
+          for (int q = 0; q < 10; ++q) s.hit_used5[A.hits[q]] = 1;   // S1 / S2: "shares a hit with a surviving pT5"
         }
       }
       else s.pt3_keep[A.idx] = keep;

@@ -12,6 +12,7 @@ namespace lst {
 struct RowTab {                       // right-list table of one group, in shared memory
   uint32_t start[kRowChunk];
   uint32_t cum[kRowChunk + 1];
+  uint32_t hint[kItemWords];          // row of the item's candidates 0, 32, 64, ... (stage_hints)
 };
 
 // KIND 0 (T3) : rows are LS, right lists are LS ranges of the outer MD.
@@ -98,6 +99,26 @@ __device__ __forceinline__ void flat_to_pair(const RowTab &rt, uint32_t cf, int 
   *right = rt.start[lo] + (cf - rt.cum[lo]);
 }
 
+// Per item: the row of every 32nd candidate, so that a candidate finds its row by a short linear
+// walk (rows are ~100 candidates wide) instead of a 7-step binary search.
+__device__ __forceinline__ void stage_hints(RowTab &rt, uint32_t j0) {
+  if (threadIdx.x < kItemWords) {
+    const uint32_t cf = j0 + 32u * threadIdx.x;
+    int row = 0;
+    if (cf < rt.cum[kRowChunk]) { uint32_t b; flat_to_pair(rt, cf, &row, &b); }
+    rt.hint[threadIdx.x] = (uint32_t)row;
+  }
+  __syncthreads();
+}
+// candidate c of the item (flat index cf = j0 + c < total) -> (row in group, right object)
+__device__ __forceinline__ void item_to_pair(const RowTab &rt, uint32_t j0, int c, int *row, uint32_t *right) {
+  const uint32_t cf = j0 + (uint32_t)c;
+  int r = (int)rt.hint[c >> 5];
+  while (rt.cum[r + 1] <= cf) ++r;
+  *row = r;
+  *right = rt.start[r] + (cf - rt.cum[r]);
+}
+
 __device__ __forceinline__ Pt md_point(const SlotDev &s, uint32_t md) {
   const float4 p = s.md_pos[md];
   return make_pt(p.x, p.y, p.z, (int)(s.md_mod[md] & 3u));
@@ -137,13 +158,13 @@ __device__ __forceinline__ bool px_pre_f(const SlotDev &s, const Params &g, floa
   float al;
   if (cat < 2) {
     const float kr = kp * h.w;
-    al = fabsf(kr) <= 1e-4f ? h.w : asinf(fminf(1.0f, fmaxf(-1.0f, kr))) / kp;
+    al = fabsf(kr) <= 1e-4f ? h.w : __fdividef(asinf(fminf(1.0f, fmaxf(-1.0f, kr))), kp);
   } else {
-    al = (h.z - sp.w) / sh;
+    al = __fdividef(h.z - sp.w, sh);
   }
   const float d = s.md_phi[m0] - (sp.z + kp * al);
   const float dph = d - 6.2831853071795864769f * rintf(d * 0.15915494309189533577f);
-  const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * fabsf(kp) * al + g.f_sig_t[cat] / h.w;
+  const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * fabsf(kp) * al + __fdividef(g.f_sig_t[cat], h.w);
   if (fabsf(dph) > g.f_ns * sgp * kPreSlack + 1e-5f) return false;
   float dzt, szt;
   if (cat < 2) {
@@ -151,8 +172,8 @@ __device__ __forceinline__ bool px_pre_f(const SlotDev &s, const Params &g, floa
     szt = (float)g.seed_sig_z + g.f_sig_z[cat];
   } else {
     const float ka = kp * al;
-    dzt = h.w - (fabsf(ka) <= 1e-4f ? al : sinf(ka) / kp);
-    szt = (float)g.seed_sig_z / fabsf(sh) + g.f_sig_r[cat];
+    dzt = h.w - (fabsf(ka) <= 1e-4f ? al : __fdividef(sinf(ka), kp));
+    szt = __fdividef((float)g.seed_sig_z, fabsf(sh)) + g.f_sig_r[cat];
   }
   if (fabsf(dzt) > g.f_ns * szt * kPreSlack + 2e-3f) return false;
   return true;
@@ -237,6 +258,7 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
     if (tid == 0) sc.n = 0;
     if (KIND == J_PT5 || KIND == J_PT3) stage_seeds(rowseed, s, g, r0, n_rows);
     stage_rows<KIND>(rt, s, r0, n_rows, sh);
+    stage_hints(rt, item.j0);
     const int nj = item.nj;
     if (KIND == J_T3) {
       for (int base = 0; base < nj; base += kThreads) {
@@ -244,7 +266,7 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
         bool pass = false;
         if (c < nj) {
           int row; uint32_t b;
-          flat_to_pair(rt, item.j0 + c, &row, &b);
+          item_to_pair(rt, item.j0, c, &row, &b);
           pass = join_candidate<KIND>(geo, s, g, r0 + row, b);
         }
         const uint32_t w = __ballot_sync(0xffffffffu, pass);
@@ -257,7 +279,7 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
         bool keep = false;
         if (c < nj) {
           int row; uint32_t b;
-          flat_to_pair(rt, item.j0 + c, &row, &b);
+          item_to_pair(rt, item.j0, c, &row, &b);
           keep = join_phase1<KIND>(s, g, r0 + row, b, rowseed, row);
         }
         push_survivor(sc, keep, (uint32_t)c);
@@ -267,7 +289,7 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
       for (int k = tid; k < nsv; k += kThreads) {
         const int c = sc.list[k];
         int row; uint32_t b;
-        flat_to_pair(rt, item.j0 + c, &row, &b);
+        item_to_pair(rt, item.j0, c, &row, &b);
         if (join_candidate<KIND>(geo, s, g, r0 + row, b)) atomicOr(&sc.mask[c >> 5], 1u << (c & 31));
       }
     }
@@ -292,12 +314,13 @@ __global__ void __launch_bounds__(kThreads) k_join_fill(GeoDev geo, SlotDev s, P
     const Item item = st.items[it];
     const uint32_t r0 = item.group * kRowChunk;
     stage_rows<KIND>(rt, s, r0, n_rows, sh);
+    stage_hints(rt, item.j0);
     expand_mask(sc, st.mask + (size_t)it * kItemWords);
     const int n = (int)sc.n;
     const uint32_t base = st.item_base[it];
     for (int k = tid; k < n; k += kThreads) {
       int row; uint32_t b;
-      flat_to_pair(rt, item.j0 + sc.list[k], &row, &b);
+      item_to_pair(rt, item.j0, (int)sc.list[k], &row, &b);
       const uint32_t a = r0 + row, idx = base + k;
       if (KIND == J_T3) {
         T3Out o; uint4 m;

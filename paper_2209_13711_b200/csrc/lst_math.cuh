@@ -42,6 +42,30 @@ LST_HD bool is_endcap(int cat) { return cat >= 2; }
 LST_HD double clamp1(double v) { return v > 1.0 ? 1.0 : (v < -1.0 ? -1.0 : v); }
 LST_HD double dmin(double a, double b) { return a < b ? a : b; }
 LST_HD double wrap_pi(double a) { return remainder(a, 6.283185307179586476925286766559); }
+// sqrt(a^2 + b^2): coordinates are centimetres (|a|, |b| < 1e4), so no overflow / underflow handling.
+LST_HD double hyp(double a, double b) { return sqrt(a * a + b * b); }
+// atan2 for the small angles between neighbouring anchors (every LS has |sin dphi| <~ 0.2 and a
+// positive dot product): for x > 0, |y| <= x / 4 the odd series in t = y / x, 11 terms, truncation
+// error < 3e-15 relative; anything else goes to libm.  The north_star contract needs cut variables
+// to 1e-5 of their thresholds, which this exceeds by ten orders of magnitude.
+LST_HD double atan2_small(double y, double x) {
+  if (x > 0.0 && fabs(y) <= 0.25 * x) {
+    const double t = y / x, u = t * t;
+    double p = 1.0 / 21.0;
+    p = -1.0 / 19.0 + u * p;
+    p = 1.0 / 17.0 + u * p;
+    p = -1.0 / 15.0 + u * p;
+    p = 1.0 / 13.0 + u * p;
+    p = -1.0 / 11.0 + u * p;
+    p = 1.0 / 9.0 + u * p;
+    p = -1.0 / 7.0 + u * p;
+    p = 1.0 / 5.0 + u * p;
+    p = -1.0 / 3.0 + u * p;
+    p = 1.0 + u * p;
+    return t * p;
+  }
+  return atan2(y, x);
+}
 
 struct Pt {  // a point promoted to double, with its transverse radius and module category
   double x, y, z, rt;
@@ -59,9 +83,9 @@ LST_HD double sd_of(const Pt &A, const Pt &B) {          // sin(dphi)
   return (A.x * (B.y - A.y) - A.y * (B.x - A.x)) / (A.rt * B.rt);
 }
 LST_HD double dphi_of(const Pt &A, const Pt &B) {
-  return atan2(A.x * (B.y - A.y) - A.y * (B.x - A.x), A.x * B.x + A.y * B.y);
+  return atan2_small(A.x * (B.y - A.y) - A.y * (B.x - A.x), A.x * B.x + A.y * B.y);
 }
-LST_HD double chord_of(const Pt &A, const Pt &B) { return hypot(B.x - A.x, B.y - A.y); }
+LST_HD double chord_of(const Pt &A, const Pt &B) { return hyp(B.x - A.x, B.y - A.y); }
 LST_HD double dr_of(const Pt &A, const Pt &B) {          // rt_B - rt_A without cancellation
   double dx = B.x - A.x, dy = B.y - A.y;
   return (2.0 * (A.x * dx + A.y * dy) + (dx * dx + dy * dy)) / (A.rt + B.rt);
@@ -69,7 +93,7 @@ LST_HD double dr_of(const Pt &A, const Pt &B) {          // rt_B - rt_A without 
 LST_HD double kappa3_of(const Pt &A, const Pt &B, const Pt &C) {  // Menger curvature / 2
   double abx = B.x - A.x, aby = B.y - A.y, bcx = C.x - B.x, bcy = C.y - B.y;
   double acx = C.x - A.x, acy = C.y - A.y;
-  return (abx * bcy - aby * bcx) / (hypot(abx, aby) * hypot(bcx, bcy) * hypot(acx, acy));
+  return (abx * bcy - aby * bcx) / (hyp(abx, aby) * hyp(bcx, bcy) * hyp(acx, acy));
 }
 LST_HD double arc_of(double r, double k) {               // arc length at radius r, half curvature k
   if (fabs(k * r) <= 1e-4) return r;
@@ -275,7 +299,7 @@ LST_HD bool t3_eval_d(const Params &g, const Pt &P1, const Pt &P2, const Pt &P3,
   const double ns = g.ns;
   const bool modeZ = is_endcap(P1.cat) || is_endcap(P2.cat) || is_endcap(P3.cat);
   const double d12x = P2.x - P1.x, d12y = P2.y - P1.y, d23x = P3.x - P2.x, d23y = P3.y - P2.y;
-  const double a = hypot(d12x, d12y), b = hypot(d23x, d23y), c13 = chord_of(P1, P3);
+  const double a = hyp(d12x, d12y), b = hyp(d23x, d23y), c13 = chord_of(P1, P3);
   if (!(a > kGuard) || !(b > kGuard) || !(c13 > kGuard)) return false;
   bool ok = true;
   // T3-1 relative angle
@@ -309,7 +333,7 @@ LST_HD bool t3_eval_d(const Params &g, const Pt &P1, const Pt &P2, const Pt &P3,
   ok &= le(fabs(Nz), ns * Ez);
   if (o) {
     o->kappa3 = k3; o->sigk3 = sk3;
-    o->beta = atan2(crs, d12x * d23x + d12y * d23y);
+    o->beta = atan2_small(crs, d12x * d23x + d12y * d23y);
   }
   return ok;
 }
@@ -346,7 +370,7 @@ LST_HD bool kasa_fit_d(const Params &g, const Pt *P, double kc, double *R, doubl
   double x2 = 0.0;
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
-    const double e = hypot(u[k] - cx, v[k] - cy) - Rr;
+    const double e = hyp(u[k] - cx, v[k] - cy) - Rr;
     x2 += w[k] * e * e;
   }
   *R = Rr; *chi2 = x2;
