@@ -9,7 +9,7 @@ __global__ void k_begin(SlotDev s) {
   Header *h = s.hdr;
   const int t = threadIdx.x;
   if (t < 8) h->n_obj[t] = 0;
-  if (t < S_NSTAGE) { h->n_items[t] = 0; h->n_groups[t] = 0; h->n_units[t] = 0; h->cand[t] = 0ull; }
+  if (t < S_NSTAGE) { h->n_items[t] = 0; h->n_groups[t] = 0; h->n_units[t] = 0; h->next_unit[t] = 0; h->pool_used[t] = 0; h->cand[t] = 0ull; }
   if (t == 0) { h->err = 0; h->n_inc = 0; h->n_dd = 0; h->n_flag = 0; s.scan_part[kScanBlocks + 1] = 0; }
 }
 
@@ -83,20 +83,17 @@ __global__ void k_rank(GeoDev geo, SlotDev s) {
 // ------------------------------------------------------------------ emit work items
 __device__ __forceinline__ uint32_t items_of(uint32_t R, uint32_t W) {
   if (R == 0 || W == 0) return 0;
-  if (W <= (uint32_t)kItemCand) {
-    const uint32_t rpi = (uint32_t)kItemCand / W;
-    return (R + rpi - 1) / rpi;
-  }
-  return R * ((W + kItemCand - 1) / kItemCand);
+  const uint32_t rpi = item_rpi(W);
+  return ((R + rpi - 1) / rpi) * item_nct(W);
 }
 // Work units of a group: the items (q, ct), q = row chunk, ct = column tile, are cut into runs of
 // kUnitItems consecutive q at fixed ct; the items of a unit share their columns (item index of
-// (q, ct) = g_item0 + q * n_ct + ct; unit u of the group: ct = u % n_ct, q0 = (u / n_ct) * kUnitItems).
+// (q, ct) = g_item0 + q * n_ct + ct; unit u of the group: ct = u % n_ct, q0 = (u / n_ct) * unit_items(W)).
 __device__ __forceinline__ uint32_t units_of(uint32_t R, uint32_t W) {
   if (R == 0 || W == 0) return 0;
-  const uint32_t nct = W <= (uint32_t)kItemCand ? 1u : (W + kItemCand - 1) / kItemCand;
+  const uint32_t nct = item_nct(W), ipu = unit_items(W);
   const uint32_t nq = items_of(R, W) / nct;
-  return nct * ((nq + kUnitItems - 1) / kUnitItems);
+  return nct * ((nq + ipu - 1) / ipu);
 }
 
 // One block.  rows_level >= 0: the groups are kRowChunk-row chunks of that object level and the
@@ -163,7 +160,7 @@ __global__ void k_emit_items(SlotDev s, int stage, int rows_level) {
     Item it;
     it.group = g;
     if (W <= (uint32_t)kItemCand) {
-      const uint32_t rpi = (uint32_t)kItemCand / W;
+      const uint32_t rpi = item_rpi(W);
       it.i0 = k * rpi; it.j0 = 0;
       it.nrows = (uint16_t)min(rpi, R - k * rpi); it.nj = (uint16_t)W;
     } else {
@@ -172,6 +169,14 @@ __global__ void k_emit_items(SlotDev s, int stage, int rows_level) {
       it.nrows = 1; it.nj = (uint16_t)min((uint32_t)kItemCand, W - it.j0);
     }
     st.items[i] = it;
+  }
+  for (uint32_t u = threadIdx.x; u < ucarry; u += blockDim.x) {   // one thread per UNIT: its group
+    uint32_t lo = 0, hi = ng;
+    while (hi - lo > 1) {
+      const uint32_t mid = (lo + hi) >> 1;
+      if (st.g_unit0[mid] <= u) lo = mid; else hi = mid;
+    }
+    st.unit_group[u] = lo;
   }
 }
 

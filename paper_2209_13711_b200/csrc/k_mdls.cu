@@ -37,52 +37,54 @@ __global__ void __launch_bounds__(kThreads) k_md_eval(GeoDev geo, SlotDev s, Par
     }
     __syncthreads();
     const int nsv = (int)sc.n;
-    for (int k = tid; k < nsv; k += kThreads) {
-      const int c = sc.list[k];
-      const int r = c / nj, jj = c - r * nj;
-      const float4 l = pool[r], u = pool[nr + jj];
-      const Pt pl = make_pt(l.x, l.y, l.z, cat), pu = make_pt(u.x, u.y, u.z, cat);
-      if (md_eval_d(g, pl, pu, cat, nullptr)) atomicOr(&sc.mask[c >> 5], 1u << (c & 31));
+    for (int base = 0; base < nsv; base += kThreads) {     // fp64 decision; results go to the pool
+      const int k = base + tid;
+      bool pass = false;
+      int c = 0;
+      MdOut o;
+      if (k < nsv) {
+        c = sc.list[k];
+        const int r = c / nj, jj = c - r * nj;
+        const float4 l = pool[r], u = pool[nr + jj];
+        const Pt pl = make_pt(l.x, l.y, l.z, cat), pu = make_pt(u.x, u.y, u.z, cat);
+        pass = md_eval_d(g, pl, pu, cat, &o);
+      }
+      const uint32_t pos = pool_reserve(s.hdr, st, S_MD, pass);
+      if (pass) atomicOr(&sc.mask[c >> 5], 1u << (c & 31));
+      if (pos != 0xFFFFFFFFu) {
+        st.pkey[pos] = it * (uint32_t)kItemCand + (uint32_t)c;
+        st.p_d2[pos] = make_double2(o.kappa, o.sigk);
+        st.p_f4[pos] = make_float4((float)o.dphi, 0.f, 0.f, 0.f);
+      }
     }
     __syncthreads();
-    publish_mask(sc, st.mask + (size_t)it * kItemWords, st.item_cnt + it);
+    publish_mask(sc, st, it);
     __syncthreads();
   }
 }
 
-__global__ void __launch_bounds__(kThreads) k_md_fill(GeoDev geo, SlotDev s, Params g) {
-  __shared__ ItemScratch sc;
+// One thread per pool entry: canonical position, the cheap fields re-derived from the item.
+__global__ void __launch_bounds__(256) k_md_fill(GeoDev geo, SlotDev s) {
   const StageBuf &st = s.st[S_MD];
-  const uint32_t n_items = s.hdr->n_items[S_MD];
-  const int tid = threadIdx.x;
-  for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
-    if (st.item_cnt[it] == 0) continue;   // uniform per block
+  const Header *hdr = s.hdr;
+  if (hdr->n_obj[0] == 0) return;                            // nothing built, or overflow (level emptied)
+  const uint32_t n = hdr->pool_used[S_MD];
+  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+    uint32_t it, c;
+    const uint32_t idx = pool_target(st, st.pkey[j], &it, &c);
     const Item item = st.items[it];
     const uint32_t m = item.group;
-    const int cat = geo.category[m];
-    const uint32_t lo0 = s.det_off[2 * m] + item.i0, up0 = s.det_off[2 * m + 1] + item.j0;
-    const int nj = item.nj;
-    expand_mask(sc, st.mask + (size_t)it * kItemWords);
-    const int n = (int)sc.n;
-    const uint32_t base = st.item_base[it];
-    for (int k = tid; k < n; k += kThreads) {
-      const int c = sc.list[k];
-      const int r = c / nj, jj = c - r * nj;
-      const uint32_t hl = lo0 + r, hu = up0 + jj;
-      const float4 l = s.hit[hl], u = s.hit[hu];
-      const Pt pl = make_pt(l.x, l.y, l.z, cat), pu = make_pt(u.x, u.y, u.z, cat);
-      MdOut o;
-      md_eval_d(g, pl, pu, cat, &o);
-      const uint32_t idx = base + k;
-      s.md_pos[idx] = l;
-      s.md_kd[idx] = make_double2(o.kappa, o.sigk);
-      s.md_kf[idx] = make_float2((float)o.kappa, (float)o.sigk);
-      s.md_hit[idx] = make_uint2(hl, hu);
-      s.md_mod[idx] = (m << 2) | (uint32_t)cat;
-      s.md_dphi[idx] = (float)o.dphi;
-      s.md_phi[idx] = atan2f(l.y, l.x);
-    }
-    __syncthreads();
+    const uint32_t nj = item.nj, r = c / nj, jj = c - r * nj;
+    const uint32_t hl = s.det_off[2 * m] + item.i0 + r, hu = s.det_off[2 * m + 1] + item.j0 + jj;
+    const float4 l = s.hit[hl];
+    const double2 kd = st.p_d2[j];
+    s.md_pos[idx] = l;
+    s.md_kd[idx] = kd;
+    s.md_kf[idx] = make_float2((float)kd.x, (float)kd.y);
+    s.md_hit[idx] = make_uint2(hl, hu);
+    s.md_mod[idx] = (m << 2) | (uint32_t)geo.category[m];
+    s.md_dphi[idx] = st.p_f4[j].x;
+    s.md_phi[idx] = atan2f(l.y, l.x);
   }
 }
 
@@ -145,148 +147,152 @@ __device__ __forceinline__ uint32_t map_col_to_md(const MapRow &mr, uint32_t j) 
   return mr.start[lo] + (j - mr.cum[lo]);
 }
 
-// append candidate c to a survivor list (warp-aggregated shared atomic); all 32 lanes must call
-__device__ __forceinline__ void push_list(uint16_t *list, uint32_t *n, bool keep, uint32_t c) {
-  const uint32_t b = __ballot_sync(0xffffffffu, keep);
-  if (b == 0) return;
-  const int lane = threadIdx.x & 31;
-  const int leader = __ffs(b) - 1;
-  uint32_t base = 0;
-  if (lane == leader) base = atomicAdd(n, (uint32_t)__popc(b));
-  base = __shfl_sync(0xffffffffu, base, leader);
-  if (keep) list[base + __popc(b & ((1u << lane) - 1u))] = (uint16_t)c;
+// One block per WORK UNIT (k_emit_items): up to kUnitItems items of module A that share one column
+// tile; the MDs of the connected modules (columns) and the unit's rows are staged in shared memory
+// once (an inner-barrel module compares each of its ~30 MDs with ~1200 MDs of ~64 neighbours).
+// After the staging the warps work independently, without block barriers: a warp owns 32 columns
+// (kept in registers) and walks the rows (broadcast reads); three stages connected by warp queues:
+//   tier 1 (ls_tier1_f: no division / sqrt / atan, ~82 % rejected) on every candidate,
+//   tier 2 (ls_pre_f, full fp32) on 32 queued survivors at a time,
+//   the fp64 decision on 32 queued tier-2 survivors at a time (~3 % of the candidates).
+struct LsShared {
+  MapRow mr;
+  float4 c_pos[kItemCand];
+  uint32_t c_idc[kItemCand];          // MD index | category << 30
+  float4 r_pos[kUnitRows];
+  uint32_t r_idc[kUnitRows];
+  uint32_t umask[kUnitItems * kItemWords];
+  uint32_t q1[kThreads / 32][64], q2[kThreads / 32][64];
+  float4 tab[4];                      // per category: sig_z, sig_r, sig_t
+};
+
+// it0: item of the unit's first row chunk; consecutive row chunks are nct items apart.
+__device__ __forceinline__ void ls_stage3(const LsShared &sh, const SlotDev &s, const Params &g, WarpQueue &Q2,
+                                          uint32_t *umask, uint32_t rpi, int nj, uint32_t it0, uint32_t nct) {
+  const StageBuf &st = s.st[S_LS];
+  uint32_t e;
+  bool pass = false;
+  LsOut o;
+  uint32_t mi = 0, mo = 0, q = 0, c = 0;
+  if (Q2.pop(&e)) {
+    const uint32_t r = e & 0xFFu, jj = e >> 8;
+    const float4 a = sh.r_pos[r], b = sh.c_pos[jj];
+    const uint32_t ia = sh.r_idc[r], ib = sh.c_idc[jj];
+    mi = ia & 0x3FFFFFFFu; mo = ib & 0x3FFFFFFFu;
+    const double2 ka = s.md_kd[mi], kb = s.md_kd[mo];
+    const Pt pa = make_pt(a.x, a.y, a.z, (int)(ia >> 30)), pb = make_pt(b.x, b.y, b.z, (int)(ib >> 30));
+    pass = ls_eval_d(g, pa, ka.x, ka.y, pb, kb.x, kb.y, &o);
+    q = r / rpi; c = (r - q * rpi) * (uint32_t)nj + jj;
+  }
+  const uint32_t pos = pool_reserve(s.hdr, st, S_LS, pass);
+  if (pass) atomicOr(&umask[q * kItemWords + (c >> 5)], 1u << (c & 31));
+  if (pos != 0xFFFFFFFFu) {
+    st.pkey[pos] = (it0 + q * nct) * (uint32_t)kItemCand + c;
+    st.p_ab[pos] = make_uint2(mi, mo);
+    st.p_f4[pos] = make_float4((float)o.dphi, (float)o.kappa, (float)o.sigk, 0.0f);
+  }
+}
+__device__ __forceinline__ void ls_stage2(const LsShared &sh, const SlotDev &s, const Params &g, WarpQueue &Q1,
+                                          WarpQueue &Q2, uint32_t *umask, uint32_t rpi, int nj, uint32_t it0,
+                                          uint32_t nct) {
+  uint32_t e = 0;
+  bool keep = false;
+  if (Q1.pop(&e)) {
+    const uint32_t r = e & 0xFFu, jj = e >> 8;
+    const float4 a = sh.r_pos[r], b = sh.c_pos[jj];
+    const uint32_t ia = sh.r_idc[r], ib = sh.c_idc[jj];
+    const float2 ka = s.md_kf[ia & 0x3FFFFFFFu], kb = s.md_kf[ib & 0x3FFFFFFFu];
+    keep = ls_pre_f(g, a.x, a.y, a.z, a.w, ka.x, ka.y, (int)(ia >> 30), b.x, b.y, b.z, b.w, kb.x, kb.y, (int)(ib >> 30));
+  }
+  Q2.push(keep, e);
+  if (Q2.n >= 32u) ls_stage3(sh, s, g, Q2, umask, rpi, nj, it0, nct);
 }
 
-// One block per WORK UNIT (k_emit_items): up to kUnitItems items of module A that share one column
-// tile, i.e. the MDs of the connected modules are staged in shared memory once and re-used for all
-// rows (an inner-barrel module compares each of its ~30 MDs with ~1200 MDs of ~64 neighbours).
-// Per item: tier 1 (ls_tier1_f: no division / sqrt / atan, ~82 % rejected) on every candidate,
-// tier 2 (ls_pre_f, full fp32) on the compacted survivors, fp64 decision on what is left (~3 %).
-__global__ void __launch_bounds__(kThreads) k_ls_eval(GeoDev geo, SlotDev s, Params g) {
-  __shared__ ItemScratch sc;
-  __shared__ uint16_t list2[kItemCand];
-  __shared__ uint32_t n2;
-  __shared__ MapRow mr;
-  __shared__ float4 p_pos[kItemCand + 8];
-  __shared__ uint32_t p_idc[kItemCand + 8];     // MD index | category << 30
-  __shared__ float4 tab[4];                     // per category: sig_z, sig_r, sig_t
+__global__ void __launch_bounds__(kThreads, 6) k_ls_eval(GeoDev geo, SlotDev s, Params g) {
+  __shared__ LsShared sh;
   const StageBuf &st = s.st[S_LS];
-  const uint32_t n_units = s.hdr->n_units[S_LS], ng = s.hdr->n_groups[S_LS];
-  const int tid = threadIdx.x;
-  if (tid < 4) tab[tid] = make_float4(g.f_sig_z[tid], g.f_sig_r[tid], g.f_sig_t[tid], 0.0f);
-  for (uint32_t u = blockIdx.x; u < n_units; u += gridDim.x) {
-    uint32_t lo = 0, hi = ng;                   // last group with g_unit0 <= u
-    while (hi - lo > 1) {
-      const uint32_t mid = (lo + hi) >> 1;
-      if (st.g_unit0[mid] <= u) lo = mid; else hi = mid;
+  const uint32_t n_units = s.hdr->n_units[S_LS];
+  const int tid = threadIdx.x, lane = tid & 31, wib = tid >> 5;
+  constexpr int kWarps = kThreads / 32;
+  if (tid < 4) sh.tab[tid] = make_float4(g.f_sig_z[tid], g.f_sig_r[tid], g.f_sig_t[tid], 0.0f);
+  WarpQueue Q1, Q2;
+  Q1.init(sh.q1[wib]);
+  Q2.init(sh.q2[wib]);
+  __shared__ uint32_t sh_unit[2];
+  for (;;) {
+    __syncthreads();                            // the previous unit is done with the shared arrays
+    if (tid == 0) {                             // units are handed out dynamically (their cost varies 100x)
+      const uint32_t nu = atomicAdd(&s.hdr->next_unit[S_LS], 1u);
+      sh_unit[0] = nu;
+      sh_unit[1] = nu < n_units ? st.unit_group[nu] : 0u;
     }
-    const uint32_t A = lo, lu = u - st.g_unit0[A];
+    __syncthreads();
+    const uint32_t u = sh_unit[0];
+    if (u >= n_units) break;
+    const uint32_t A = sh_unit[1], lu = u - st.g_unit0[A];
     const uint32_t R = st.gR[A], W = st.gW[A];
-    const uint32_t nct = W <= (uint32_t)kItemCand ? 1u : (W + kItemCand - 1) / kItemCand;
-    const uint32_t rpi = W <= (uint32_t)kItemCand ? (uint32_t)kItemCand / W : 1u;
+    const uint32_t nct = item_nct(W), rpi = item_rpi(W), ipu = unit_items(W);
     const uint32_t nq = (R + rpi - 1) / rpi;
-    const uint32_t ct = lu % nct, q0 = (lu / nct) * kUnitItems;
-    const uint32_t qn = min((uint32_t)kUnitItems, nq - q0);
+    const uint32_t ct = lu % nct, q0 = (lu / nct) * ipu;
+    const uint32_t qn = min(ipu, nq - q0);
     const uint32_t j0 = ct * kItemCand;
     const int nj = (int)min((uint32_t)kItemCand, W - j0);
     const uint32_t md0 = s.md_mod_off[A], item0 = st.g_item0[A];
-    __syncthreads();                            // the previous unit is done with mr / p_pos
-    stage_map_row(mr, geo, s, A);
+    const uint32_t row0 = q0 * rpi, it0 = item0 + q0 * nct + ct;
+    const int nrows = (int)min(R - row0, qn * rpi);      // <= kUnitRows
+    stage_map_row(sh.mr, geo, s, A);
+    for (int k = tid; k < nrows; k += kThreads) {
+      const uint32_t md = md0 + row0 + k;
+      sh.r_pos[k] = s.md_pos[md];
+      sh.r_idc[k] = md | ((s.md_mod[md] & 3u) << 30);
+    }
+    for (int k = tid; k < (int)(qn * kItemWords); k += kThreads) sh.umask[k] = 0;
     __syncthreads();
     for (int k = tid; k < nj; k += kThreads) {
-      const uint32_t md = map_col_to_md(mr, j0 + k);
-      p_pos[k] = s.md_pos[md];
-      p_idc[k] = md | ((s.md_mod[md] & 3u) << 30);
+      const uint32_t md = map_col_to_md(sh.mr, j0 + k);
+      sh.c_pos[k] = s.md_pos[md];
+      sh.c_idc[k] = md | ((s.md_mod[md] & 3u) << 30);
     }
-    const uint32_t inv = (1u << 20) / (uint32_t)nj + 1u;   // c / nj == (c * inv) >> 20 for c * nj < 2^20
-    for (uint32_t qi = 0; qi < qn; ++qi) {
-      const uint32_t q = q0 + qi, it = item0 + q * nct + ct, i0 = q * rpi;
-      const int nr = (int)min(rpi, R - i0);
-      for (int k = tid; k < nr; k += kThreads) {
-        const uint32_t md = md0 + i0 + k;
-        p_pos[nj + k] = s.md_pos[md];
-        p_idc[nj + k] = md | ((s.md_mod[md] & 3u) << 30);
+    __syncthreads();
+    // tasks: (32-column chunk, interleaved row group); with few chunks the rows are split over the warps
+    const int nchunk = (nj + 31) >> 5;
+    const int nrg = nchunk >= kWarps ? 1 : kWarps / nchunk;
+    for (int t = wib; t < nchunk * nrg; t += kWarps) {
+      const int chunk = t % nchunk, rg = t / nchunk;
+      const int jj = chunk * 32 + lane;
+      const bool has = jj < nj;
+      const float4 b = sh.c_pos[has ? jj : 0];
+      const uint32_t cb = sh.c_idc[has ? jj : 0] >> 30;
+      const float4 tb = sh.tab[cb];
+      for (int r = rg; r < nrows; r += nrg) {
+        const float4 a = sh.r_pos[r];
+        const float4 ta = sh.tab[sh.r_idc[r] >> 30];
+        const bool keep = has && ls_tier1_f(g, a.x, a.y, a.z, a.w, ta.x, ta.y, ta.z, b.x, b.y, b.z, b.w, tb.x, tb.y, tb.z,
+                                            cb >= 2u);
+        Q1.push(keep, (uint32_t)r | ((uint32_t)jj << 8));
+        if (Q1.n >= 32u) ls_stage2(sh, s, g, Q1, Q2, sh.umask, rpi, nj, it0, nct);
       }
-      if (tid < kItemWords) sc.mask[tid] = 0;
-      if (tid == 0) { sc.n = 0; n2 = 0; }
-      __syncthreads();
-      const int nc = nr * nj;
-      for (int base = 0; base < nc; base += kThreads) {          // tier 1
-        const int c = base + tid;
-        bool keep = false;
-        if (c < nc) {
-          const int r = (int)(((uint32_t)c * inv) >> 20), jj = c - r * nj;
-          const float4 a = p_pos[nj + r], b = p_pos[jj];
-          const uint32_t ca = p_idc[nj + r] >> 30, cb = p_idc[jj] >> 30;
-          const float4 ta = tab[ca], tb = tab[cb];
-          keep = ls_tier1_f(g, a.x, a.y, a.z, a.w, ta.x, ta.y, ta.z, b.x, b.y, b.z, b.w, tb.x, tb.y, tb.z, cb >= 2u);
-        }
-        push_list(sc.list, &sc.n, keep, (uint32_t)c);
-      }
-      __syncthreads();
-      const int n1 = (int)sc.n;
-      for (int base = 0; base < n1; base += kThreads) {          // tier 2
-        const int k = base + tid;
-        bool keep = false;
-        int c = 0;
-        if (k < n1) {
-          c = sc.list[k];
-          const int r = (int)(((uint32_t)c * inv) >> 20), jj = c - r * nj;
-          const float4 a = p_pos[nj + r], b = p_pos[jj];
-          const uint32_t ia = p_idc[nj + r], ib = p_idc[jj];
-          const float2 ka = s.md_kf[ia & 0x3FFFFFFFu], kb = s.md_kf[ib & 0x3FFFFFFFu];
-          keep = ls_pre_f(g, a.x, a.y, a.z, a.w, ka.x, ka.y, (int)(ia >> 30), b.x, b.y, b.z, b.w, kb.x, kb.y, (int)(ib >> 30));
-        }
-        push_list(list2, &n2, keep, (uint32_t)c);
-      }
-      __syncthreads();
-      const int nsv = (int)n2;
-      for (int k = tid; k < nsv; k += kThreads) {                // fp64 decision
-        const int c = list2[k];
-        const int r = (int)(((uint32_t)c * inv) >> 20), jj = c - r * nj;
-        const float4 a = p_pos[nj + r], b = p_pos[jj];
-        const uint32_t ia = p_idc[nj + r], ib = p_idc[jj];
-        const double2 ka = s.md_kd[ia & 0x3FFFFFFFu], kb = s.md_kd[ib & 0x3FFFFFFFu];
-        const Pt pa = make_pt(a.x, a.y, a.z, (int)(ia >> 30)), pb = make_pt(b.x, b.y, b.z, (int)(ib >> 30));
-        if (ls_eval_d(g, pa, ka.x, ka.y, pb, kb.x, kb.y, nullptr)) atomicOr(&sc.mask[c >> 5], 1u << (c & 31));
-      }
-      __syncthreads();
-      publish_mask(sc, st.mask + (size_t)it * kItemWords, st.item_cnt + it);
-      __syncthreads();
+    }
+    while (Q1.n) ls_stage2(sh, s, g, Q1, Q2, sh.umask, rpi, nj, it0, nct);
+    while (Q2.n) ls_stage3(sh, s, g, Q2, sh.umask, rpi, nj, it0, nct);
+    __syncthreads();
+    for (uint32_t qi = wib; qi < qn; qi += kWarps) {          // publish the unit's item masks
+      publish_item(st, it0 + qi * nct, sh.umask[qi * kItemWords + lane]);
     }
   }
 }
 
-__global__ void __launch_bounds__(kThreads) k_ls_fill(GeoDev geo, SlotDev s, Params g) {
-  __shared__ ItemScratch sc;
-  __shared__ MapRow mr;
+// One thread per pool entry: move it to its canonical position.
+__global__ void __launch_bounds__(256) k_ls_fill(SlotDev s) {
   const StageBuf &st = s.st[S_LS];
-  const uint32_t n_items = s.hdr->n_items[S_LS];
-  const int tid = threadIdx.x;
-  for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
-    if (st.item_cnt[it] == 0) continue;
-    const Item item = st.items[it];
-    const uint32_t A = item.group;
-    const int nj = item.nj;
-    const uint32_t i0 = s.md_mod_off[A] + item.i0;
-    stage_map_row(mr, geo, s, A);
-    expand_mask(sc, st.mask + (size_t)it * kItemWords);   // contains the __syncthreads the staging needs
-    const int n = (int)sc.n;
-    const uint32_t base = st.item_base[it];
-    for (int k = tid; k < n; k += kThreads) {
-      const int c = sc.list[k];
-      const int r = c / nj, jj = c - r * nj;
-      const uint32_t mi = i0 + r, mo = map_col_to_md(mr, item.j0 + jj);
-      const float4 a = s.md_pos[mi], b = s.md_pos[mo];
-      const double2 ka = s.md_kd[mi], kb = s.md_kd[mo];
-      const Pt pa = make_pt(a.x, a.y, a.z, s.md_mod[mi] & 3u), pb = make_pt(b.x, b.y, b.z, s.md_mod[mo] & 3u);
-      LsOut o;
-      ls_eval_d(g, pa, ka.x, ka.y, pb, kb.x, kb.y, &o);
-      const uint32_t idx = base + k;
-      s.ls_md[idx] = make_uint2(mi, mo);
-      s.ls_f[idx] = make_float4((float)o.dphi, (float)o.kappa, (float)o.sigk, 0.0f);
-    }
-    __syncthreads();
+  const Header *hdr = s.hdr;
+  if (hdr->n_obj[1] == 0) return;
+  const uint32_t n = hdr->pool_used[S_LS];
+  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+    uint32_t it, c;
+    const uint32_t idx = pool_target(st, st.pkey[j], &it, &c);
+    s.ls_md[idx] = st.p_ab[j];
+    s.ls_f[idx] = st.p_f4[j];
   }
 }
 
@@ -297,16 +303,16 @@ void launch_md(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   launch_emit(c, s, S_MD, -1, st);
   k_md_eval<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_md_eval");
   launch_scan_items(c, s, S_MD, 0, s.cap_md, st);
-  k_md_fill<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_md_fill");
+  k_md_fill<<<persistent_grid(c, 4), 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_md_fill");
   launch_row_offsets(c, s, 0, st);
 }
 
 void launch_ls(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   k_ls_groups<<<(c.geo.n_modules + 127) / 128, 128, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_ls_groups");
   launch_emit(c, s, S_LS, -1, st);
-  k_ls_eval<<<persistent_grid(c, 6), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_ls_eval");
+  k_ls_eval<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_ls_eval");
   launch_scan_items(c, s, S_LS, 1, s.cap_ls, st);
-  k_ls_fill<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_ls_fill");
+  k_ls_fill<<<persistent_grid(c, 4), 256, 0, st>>>(s); LST_MARK(c, st, "k_ls_fill");
   launch_row_offsets(c, s, 1, st);
 }
 

@@ -231,13 +231,48 @@ __device__ __forceinline__ bool join_phase1(const SlotDev &s, const Params &g, u
   }
   return px_pre_f<KIND>(s, g, rowseed[lrow], b);
 }
-// Phase 2: the fp64 decision.
+
+// Phase 2: the fp64 decision of candidate (row, b); an accepted candidate's results go to the
+// stage's pool (all 32 lanes of a warp call; `live` = this lane holds a candidate).
 template <int KIND>
-__device__ __forceinline__ bool join_candidate(const GeoDev &geo, const SlotDev &s, const Params &g, uint32_t row,
-                                               uint32_t b) {
-  if (KIND == J_T3) return t3_candidate(s, g, row, b, nullptr, nullptr);
-  if (KIND == J_T5) return t5_candidate(s, g, row, b, nullptr, nullptr, nullptr, nullptr);
-  return px_candidate<KIND>(geo, s, g, s.px_pair[row].x, b, nullptr);
+__device__ __forceinline__ bool join_phase2(const GeoDev &geo, const SlotDev &s, const Params &g, bool live,
+                                            uint32_t row, uint32_t b, uint32_t key) {
+  const int stage = JoinTraits<KIND>::stage;
+  const StageBuf &st = s.st[stage];
+  bool pass = false;
+  if (KIND == J_T3) {
+    T3Out o;
+    if (live) pass = t3_candidate(s, g, row, b, &o, nullptr);
+    const uint32_t pos = pool_reserve(s.hdr, st, stage, pass);
+    if (pos != 0xFFFFFFFFu) {
+      st.pkey[pos] = key;
+      st.p_ab[pos] = make_uint2(row, b);
+      st.p_d2[pos] = make_double2(o.kappa3, o.sigk3);
+      st.p_f4[pos] = make_float4((float)o.beta, 0.f, 0.f, 0.f);
+    }
+  } else if (KIND == J_T5) {
+    T5Out o;
+    if (live) pass = t5_candidate(s, g, row, b, &o, nullptr, nullptr, nullptr);
+    const uint32_t pos = pool_reserve(s.hdr, st, stage, pass);
+    if (pos != 0xFFFFFFFFu) {
+      st.pkey[pos] = key;
+      st.p_ab[pos] = make_uint2(row, b);
+      st.p_d2[pos] = make_double2(o.eta, o.phi);
+      st.p_d2b[pos] = make_double2(o.chi2, o.R);
+      st.p_f4[pos] = make_float4((float)o.pt, 0.f, 0.f, 0.f);
+    }
+  } else {
+    double c2 = 0.0;
+    const uint32_t p = live ? s.px_pair[row].x : 0u;
+    if (live) pass = px_candidate<KIND>(geo, s, g, p, b, &c2);
+    const uint32_t pos = pool_reserve(s.hdr, st, stage, pass);
+    if (pos != 0xFFFFFFFFu) {
+      st.pkey[pos] = key;
+      st.p_ab[pos] = make_uint2(p, b);
+      st.p_d2[pos] = make_double2(c2, 0.0);
+    }
+  }
+  return pass;
 }
 
 template <int KIND>
@@ -254,6 +289,7 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
   for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
     const Item item = st.items[it];
     const uint32_t r0 = item.group * kRowChunk;
+    const uint32_t key0 = it * (uint32_t)kItemCand;
     if (tid < kItemWords) sc.mask[tid] = 0;
     if (tid == 0) sc.n = 0;
     if (KIND == J_PT5 || KIND == J_PT3) stage_seeds(rowseed, s, g, r0, n_rows);
@@ -263,12 +299,9 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
     if (KIND == J_T3) {
       for (int base = 0; base < nj; base += kThreads) {
         const int c = base + tid;
-        bool pass = false;
-        if (c < nj) {
-          int row; uint32_t b;
-          item_to_pair(rt, item.j0, c, &row, &b);
-          pass = join_candidate<KIND>(geo, s, g, r0 + row, b);
-        }
+        int row = 0; uint32_t b = 0;
+        if (c < nj) item_to_pair(rt, item.j0, c, &row, &b);
+        const bool pass = join_phase2<KIND>(geo, s, g, c < nj, r0 + row, b, key0 + (uint32_t)c);
         const uint32_t w = __ballot_sync(0xffffffffu, pass);
         if ((tid & 31) == 0) sc.mask[c >> 5] = w;
       }
@@ -286,68 +319,54 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
       }
       __syncthreads();
       const int nsv = (int)sc.n;
-      for (int k = tid; k < nsv; k += kThreads) {
-        const int c = sc.list[k];
-        int row; uint32_t b;
-        item_to_pair(rt, item.j0, c, &row, &b);
-        if (join_candidate<KIND>(geo, s, g, r0 + row, b)) atomicOr(&sc.mask[c >> 5], 1u << (c & 31));
+      for (int base = 0; base < nsv; base += kThreads) {
+        const int k = base + tid;
+        int c = 0, row = 0; uint32_t b = 0;
+        if (k < nsv) { c = sc.list[k]; item_to_pair(rt, item.j0, c, &row, &b); }
+        if (join_phase2<KIND>(geo, s, g, k < nsv, r0 + row, b, key0 + (uint32_t)c))
+          atomicOr(&sc.mask[c >> 5], 1u << (c & 31));
       }
     }
     __syncthreads();
-    publish_mask(sc, st.mask + (size_t)it * kItemWords, st.item_cnt + it);
+    publish_mask(sc, st, it);
     __syncthreads();
   }
 }
 
+// One thread per pool entry: canonical position; constituent indices re-read from the inputs.
 template <int KIND>
-__global__ void __launch_bounds__(kThreads) k_join_fill(GeoDev geo, SlotDev s, Params g) {
-  __shared__ ItemScratch sc;
-  __shared__ RowTab rt;
-  __shared__ uint32_t sh[33];
+__global__ void __launch_bounds__(256) k_join_fill(SlotDev s) {
   const int stage = JoinTraits<KIND>::stage;
   const StageBuf &st = s.st[stage];
-  const uint32_t n_items = s.hdr->n_items[stage];
-  const uint32_t n_rows = s.hdr->n_obj[JoinTraits<KIND>::rows_level];
-  const int tid = threadIdx.x;
-  for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
-    if (st.item_cnt[it] == 0) continue;
-    const Item item = st.items[it];
-    const uint32_t r0 = item.group * kRowChunk;
-    stage_rows<KIND>(rt, s, r0, n_rows, sh);
-    stage_hints(rt, item.j0);
-    expand_mask(sc, st.mask + (size_t)it * kItemWords);
-    const int n = (int)sc.n;
-    const uint32_t base = st.item_base[it];
-    for (int k = tid; k < n; k += kThreads) {
-      int row; uint32_t b;
-      item_to_pair(rt, item.j0, (int)sc.list[k], &row, &b);
-      const uint32_t a = r0 + row, idx = base + k;
-      if (KIND == J_T3) {
-        T3Out o; uint4 m;
-        t3_candidate(s, g, a, b, &o, &m);
-        s.t3_md[idx] = m;
-        s.t3_ls[idx] = make_uint2(a, b);
-        s.t3_kd[idx] = make_double2(o.kappa3, o.sigk3);
-        s.t3_beta[idx] = (float)o.beta;
-      } else if (KIND == J_T5) {
-        T5Out o; uint32_t m[5]; double2 ka, kb;
-        t5_candidate(s, g, a, b, &o, m, &ka, &kb);
+  const Header *hdr = s.hdr;
+  if (hdr->n_obj[JoinTraits<KIND>::out_level] == 0) return;
+  const uint32_t n = hdr->pool_used[stage];
+  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+    uint32_t it, c;
+    const uint32_t idx = pool_target(st, st.pkey[j], &it, &c);
+    const uint2 ab = st.p_ab[j];
+    if (KIND == J_T3) {
+      const uint2 la = s.ls_md[ab.x], lb = s.ls_md[ab.y];
+      s.t3_md[idx] = make_uint4(la.x, la.y, lb.y, 0u);
+      s.t3_ls[idx] = ab;
+      s.t3_kd[idx] = st.p_d2[j];
+      s.t3_beta[idx] = st.p_f4[j].x;
+    } else if (KIND == J_T5) {
+      const uint4 ta = s.t3_md[ab.x], tb = s.t3_md[ab.y];
+      const uint32_t m[5] = {ta.x, ta.y, ta.z, tb.y, tb.z};
 #pragma unroll
-        for (int q = 0; q < 5; ++q) s.t5_md[(size_t)5 * idx + q] = m[q];
-        s.t5_t3[idx] = make_uint2(a, b);
-        s.t5_chi2[idx] = o.chi2;
-        s.t5_etaphi[idx] = make_double2(o.eta, o.phi);
-        s.t5_f[idx] = make_float4((float)o.R, (float)o.chi2, (float)ka.x, (float)kb.x);
-        s.t5_pt[idx] = (float)o.pt;
-      } else {
-        const uint32_t p = s.px_pair[a].x;
-        double c2 = 0.0;
-        px_candidate<KIND>(geo, s, g, p, b, &c2);
-        if (KIND == J_PT5) { s.pt5_po[idx] = make_uint2(p, b); s.pt5_chi2[idx] = c2; }
-        else { s.pt3_po[idx] = make_uint2(p, b); s.pt3_chi2[idx] = c2; }
-      }
+      for (int q = 0; q < 5; ++q) s.t5_md[(size_t)5 * idx + q] = m[q];
+      const double2 cr = st.p_d2b[j];
+      s.t5_t3[idx] = ab;
+      s.t5_chi2[idx] = cr.x;
+      s.t5_etaphi[idx] = st.p_d2[j];
+      s.t5_f[idx] = make_float4((float)cr.y, (float)cr.x, (float)s.t3_kd[ab.x].x, (float)s.t3_kd[ab.y].x);
+      s.t5_pt[idx] = st.p_f4[j].x;
+    } else if (KIND == J_PT5) {
+      s.pt5_po[idx] = ab; s.pt5_chi2[idx] = st.p_d2[j].x;
+    } else {
+      s.pt3_po[idx] = ab; s.pt3_chi2[idx] = st.p_d2[j].x;
     }
-    __syncthreads();
   }
 }
 
@@ -359,7 +378,7 @@ static void launch_join_t(const Ctx &c, const SlotDev &s, uint32_t row_cap, uint
   launch_emit(c, s, JoinTraits<KIND>::stage, JoinTraits<KIND>::rows_level, st);
   k_join_eval<KIND><<<c.n_sm * 8, kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, JoinTraits<KIND>::n_eval);
   launch_scan_items(c, s, JoinTraits<KIND>::stage, JoinTraits<KIND>::out_level, out_cap, st);
-  k_join_fill<KIND><<<c.n_sm * 8, kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, JoinTraits<KIND>::n_fill);
+  k_join_fill<KIND><<<c.n_sm * 4, 256, 0, st>>>(s); LST_MARK(c, st, JoinTraits<KIND>::n_fill);
 }
 
 void launch_join(const Ctx &c, const SlotDev &s, int kind, cudaStream_t st) {

@@ -330,8 +330,17 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
     b.g_item0 = w.take<uint32_t>((size_t)b.cap_groups + 1);
     b.g_unit0 = w.take<uint32_t>((size_t)b.cap_groups + 1);
     b.items = w.take<Item>(b.cap_items);
+    b.unit_group = w.take<uint32_t>(b.cap_items);
     b.mask = w.take<uint32_t>((size_t)b.cap_items * kItemWords);
+    b.wpre = w.take<uint16_t>((size_t)b.cap_items * kItemWords);
     b.item_cnt = w.take<uint32_t>(b.cap_items); b.item_base = w.take<uint32_t>(b.cap_items);
+    const uint32_t pool_cap[S_NSTAGE] = {s.cap_md, s.cap_ls, s.cap_t3, s.cap_t5, s.cap_pt5, s.cap_pt3};
+    b.cap_pool = pool_cap[k];
+    b.pkey = w.take<uint32_t>(b.cap_pool);
+    b.p_ab = w.take<uint2>(b.cap_pool);
+    b.p_d2 = w.take<double2>(b.cap_pool);
+    b.p_d2b = k == S_T5 ? w.take<double2>(b.cap_pool) : nullptr;
+    b.p_f4 = w.take<float4>(b.cap_pool);
   }
   // export scratch: the largest level
   size_t obj_cap = std::max({(size_t)s.cap_md, (size_t)s.cap_ls, (size_t)s.cap_t3, (size_t)s.cap_t5,
@@ -380,6 +389,7 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaGetDeviceProperties"); }
   c->k.n_sm = prop.multiProcessorCount;
+  if (const char *ev = getenv("LST_NSM")) { const int v = atoi(ev); if (v > 0) c->k.n_sm = v; }   // experiment knob
   // modules that may start a pixel-seeded object (C6 START layers)
   std::vector<uint32_t> start_mods;
   for (uint32_t m = 0; m < n; ++m)

@@ -21,7 +21,9 @@ namespace lst {
 constexpr int kItemCand = 1024;          // candidates per work item
 constexpr int kItemWords = kItemCand / 32;
 constexpr int kThreads = 128;            // threads per block of eval / fill kernels
-constexpr int kUnitItems = 8;            // items per work unit (same group, same column tile, consecutive rows)
+constexpr int kUnitItems = 8;            // max items per work unit (same group, same column tile, consecutive rows)
+constexpr int kMaxRpi = 256;             // max rows per item
+constexpr int kUnitRows = 256;           // max rows per work unit
 constexpr int kRowChunk = 128;           // rows per group in the variable-width stages (T3, T5, pixel)
 constexpr int kMaxDeg = 512;             // maximum module-map degree (checked by lst_create)
 constexpr int kPxCap = 64;               // (seed, start module) rows per pixel seed ON AVERAGE (overflow -> LST_ENOMEM)
@@ -40,6 +42,22 @@ enum ErrBits {
   ERR_CAP_PIX = 1u << 3     // a per-seed list (compatible modules / related seeds) overflowed
 };
 
+// Item / unit geometry of a group with R rows and W columns (shared by k_emit_items and the eval
+// kernels).  W <= kItemCand: one column tile, item_rpi(W) rows per item; else one row per item and
+// ceil(W / kItemCand) column tiles.  A unit = unit_items(W) consecutive row chunks of one column tile.
+__host__ __device__ __forceinline__ uint32_t item_rpi(uint32_t W) {
+  if (W > (uint32_t)kItemCand) return 1u;
+  const uint32_t r = (uint32_t)kItemCand / W;
+  return r > (uint32_t)kMaxRpi ? (uint32_t)kMaxRpi : r;
+}
+__host__ __device__ __forceinline__ uint32_t item_nct(uint32_t W) {
+  return W <= (uint32_t)kItemCand ? 1u : (W + kItemCand - 1) / kItemCand;
+}
+__host__ __device__ __forceinline__ uint32_t unit_items(uint32_t W) {
+  const uint32_t k = (uint32_t)kUnitRows / item_rpi(W);
+  return k < 1u ? 1u : (k > (uint32_t)kUnitItems ? (uint32_t)kUnitItems : k);
+}
+
 struct Item {            // 16 bytes
   uint32_t group;        // module (MD, LS) or row chunk (T3, T5, pixel)
   uint32_t i0;           // first row (relative to the group's first row)
@@ -53,6 +71,8 @@ struct Header {          // per slot, device; zeroed (except n_hits / n_seeds) a
   uint32_t n_items[S_NSTAGE];
   uint32_t n_groups[S_NSTAGE];
   uint32_t n_units[S_NSTAGE];        // work units (k_emit_items): item runs that share their columns
+  uint32_t next_unit[S_NSTAGE];      // dynamic work distribution: next unit to hand out
+  uint32_t pool_used[S_NSTAGE];      // accepted candidates written to the stage's pool so far
   uint32_t err;
   uint32_t n_dd;                     // T5 + pT5 + pT3 objects entering the cleaning
   uint32_t n_flag;                   // pT5 + pT3 + T5 + seeds: length of the TC keep-flag array
@@ -65,10 +85,18 @@ struct StageBuf {        // work list of one stage
   uint32_t *g_item0;     // [cap_groups+1] first item of a group
   uint32_t *g_unit0;     // [cap_groups+1] first work unit of a group
   Item *items;           // [cap_items]
+  uint32_t *unit_group;  // [cap_items] group of a work unit
   uint32_t *mask;        // [cap_items * kItemWords]
+  uint16_t *wpre;        // [cap_items * kItemWords] pass count of the item's words before this one
   uint32_t *item_cnt;    // [cap_items] pass count
   uint32_t *item_base;   // [cap_items] exclusive prefix
-  uint32_t cap_groups, cap_items;
+  // pool: what the eval kernel computed for each accepted candidate, in arrival order; the fill
+  // kernel moves entry j to its canonical position item_base[item] + rank of the candidate
+  uint32_t *pkey;        // [cap_pool] item * kItemCand + candidate
+  uint2 *p_ab;           // [cap_pool] constituent indices
+  double2 *p_d2, *p_d2b; // [cap_pool] fp64 results (p_d2b: T5 only)
+  float4 *p_f4;          // [cap_pool] fp32 results
+  uint32_t cap_groups, cap_items, cap_pool;
 };
 
 // Static detector data (device), shared by all slots.
@@ -198,6 +226,34 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t *sh, ui
   return e;
 }
 
+// Warp-private ring queue (64 entries in shared memory; head / count are warp-uniform registers).
+// A stage pushes its sparse survivors; the next stage pops them 32 at a time, so that the expensive
+// arithmetic always runs on full warps and no block-wide barrier separates the stages.
+struct WarpQueue {
+  uint32_t *q;       // 64 words of shared memory owned by this warp
+  uint32_t head, n;
+  __device__ __forceinline__ void init(uint32_t *mem) { q = mem; head = 0; n = 0; }
+  // all 32 lanes must call; at most 32 entries are added, the caller keeps n <= 32 before a push
+  __device__ __forceinline__ void push(bool keep, uint32_t v) {
+    const uint32_t b = __ballot_sync(0xffffffffu, keep);
+    const int lane = threadIdx.x & 31;
+    if (keep) q[(head + n + __popc(b & ((1u << lane) - 1u))) & 63u] = v;
+    n += __popc(b);
+    __syncwarp();
+  }
+  // pops min(n, 32) entries: lane < count gets one (returns true)
+  __device__ __forceinline__ bool pop(uint32_t *v) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t take = n < 32u ? n : 32u;
+    const bool have = (uint32_t)lane < take;
+    *v = q[(head + lane) & 63u];
+    __syncwarp();
+    head = (head + take) & 63u;
+    n -= take;
+    return have;
+  }
+};
+
 // Per-item compaction scratch (shared memory).
 struct ItemScratch {
   uint32_t mask[kItemWords];
@@ -248,14 +304,41 @@ __device__ __forceinline__ void expand_mask(ItemScratch &s, const uint32_t *gmas
   __syncthreads();
 }
 
-// eval epilogue: publish the item's mask and pass count.
-__device__ __forceinline__ void publish_mask(const ItemScratch &s, uint32_t *gmask, uint32_t *gcnt) {
-  if (threadIdx.x < 32) {
-    const uint32_t w = s.mask[threadIdx.x];
-    gmask[threadIdx.x] = w;
-    const uint32_t tot = warp_sum((uint32_t)__popc(w));
-    if (threadIdx.x == 0) *gcnt = tot;
-  }
+// eval epilogue, one warp: publish an item's mask words (lane = word), their running pass counts
+// and the item's pass count.
+__device__ __forceinline__ void publish_item(const StageBuf &st, uint32_t it, uint32_t w) {
+  const int lane = threadIdx.x & 31;
+  uint32_t tot;
+  const uint32_t e = warp_excl_scan((uint32_t)__popc(w), &tot);
+  st.mask[(size_t)it * kItemWords + lane] = w;
+  st.wpre[(size_t)it * kItemWords + lane] = (uint16_t)e;
+  if (lane == 0) st.item_cnt[it] = tot;
+}
+__device__ __forceinline__ void publish_mask(const ItemScratch &s, const StageBuf &st, uint32_t it) {
+  if (threadIdx.x < 32) publish_item(st, it, s.mask[threadIdx.x]);
+}
+
+// eval: reserve pool entries for the lanes of a warp whose candidate passed (all 32 lanes call).
+// Returns the lane's pool index, or 0xFFFFFFFF (not passed, or the pool is full: flagged, the level
+// is then emptied by k_scan_items, never truncated).
+__device__ __forceinline__ uint32_t pool_reserve(Header *hdr, const StageBuf &st, int stage, bool pass) {
+  const uint32_t b = __ballot_sync(0xffffffffu, pass);
+  if (b == 0) return 0xFFFFFFFFu;
+  const int lane = threadIdx.x & 31, leader = __ffs(b) - 1;
+  uint32_t base = 0;
+  if (lane == leader) base = atomicAdd(&hdr->pool_used[stage], (uint32_t)__popc(b));
+  base = __shfl_sync(0xffffffffu, base, leader);
+  const uint32_t pos = base + __popc(b & ((1u << lane) - 1u));
+  if (!pass) return 0xFFFFFFFFu;
+  if (pos >= st.cap_pool) { atomicOr(&hdr->err, (uint32_t)ERR_CAP_OBJ); return 0xFFFFFFFFu; }
+  return pos;
+}
+// fill: canonical index of pool entry `key` = item * kItemCand + candidate
+__device__ __forceinline__ uint32_t pool_target(const StageBuf &st, uint32_t key, uint32_t *item, uint32_t *cand) {
+  const uint32_t it = key / (uint32_t)kItemCand, c = key % (uint32_t)kItemCand;
+  const size_t w = (size_t)it * kItemWords + (c >> 5);
+  *item = it; *cand = c;
+  return st.item_base[it] + st.wpre[w] + __popc(st.mask[w] & ((1u << (c & 31)) - 1u));
 }
 
 }  // namespace lst
