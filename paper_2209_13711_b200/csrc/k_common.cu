@@ -9,7 +9,7 @@ __global__ void k_begin(SlotDev s) {
   Header *h = s.hdr;
   const int t = threadIdx.x;
   if (t < 8) h->n_obj[t] = 0;
-  if (t < S_NSTAGE) { h->n_items[t] = 0; h->n_groups[t] = 0; h->n_units[t] = 0; h->next_unit[t] = 0; h->pool_used[t] = 0; h->cand[t] = 0ull; }
+  if (t < S_NSTAGE) { h->n_items[t] = 0; h->n_groups[t] = 0; h->n_units[t] = 0; h->next_unit[t] = 0; h->pool_used[t] = 0; h->cl_used[t] = 0; h->cand[t] = 0ull; }
   if (t == 0) { h->err = 0; h->n_inc = 0; h->n_dd = 0; h->n_flag = 0; s.scan_part[kScanBlocks + 1] = 0; }
 }
 
@@ -178,6 +178,21 @@ __global__ void k_emit_items(SlotDev s, int stage, int rows_level) {
     }
     st.unit_group[u] = lo;
   }
+}
+
+// ------------------------------------------------------------------ per-item pass counts from the masks
+// One warp per item (stages whose decide kernel sets the mask bits with global atomics).
+__global__ void __launch_bounds__(256) k_item_counts(SlotDev s, int stage) {
+  const StageBuf &st = s.st[stage];
+  const uint32_t n = s.hdr->n_items[stage];
+  const int lane = threadIdx.x & 31;
+  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+  for (uint32_t it = warp; it < n; it += nwarp) publish_item(st, it, st.mask[(size_t)it * kItemWords + lane]);
+}
+void launch_item_counts(const Ctx &c, const SlotDev &s, int stage, cudaStream_t st) {
+  static const char *const nm[S_NSTAGE] = {"k_item_counts[MD]", "k_item_counts[LS]", "k_item_counts[T3]",
+                                           "k_item_counts[T5]", "k_item_counts[pT5]", "k_item_counts[pT3]"};
+  k_item_counts<<<c.n_sm * 2, 256, 0, st>>>(s, stage); LST_MARK(c, st, nm[stage]);
 }
 
 // ------------------------------------------------------------------ scan item pass counts

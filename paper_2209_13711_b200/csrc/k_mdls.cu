@@ -161,63 +161,38 @@ struct LsShared {
   uint32_t c_idc[kItemCand];          // MD index | category << 30
   float4 r_pos[kUnitRows];
   uint32_t r_idc[kUnitRows];
-  uint32_t umask[kUnitItems * kItemWords];
-  uint32_t q1[kThreads / 32][64], q2[kThreads / 32][64];
+  uint32_t q1[kThreads / 32][64];
   float4 tab[4];                      // per category: sig_z, sig_r, sig_t
 };
 
+// Tier 2 on up to 32 queued tier-1 survivors; what passes goes to the stage's candidate list.
 // it0: item of the unit's first row chunk; consecutive row chunks are nct items apart.
-__device__ __forceinline__ void ls_stage3(const LsShared &sh, const SlotDev &s, const Params &g, WarpQueue &Q2,
-                                          uint32_t *umask, uint32_t rpi, int nj, uint32_t it0, uint32_t nct) {
-  const StageBuf &st = s.st[S_LS];
-  uint32_t e;
-  bool pass = false;
-  LsOut o;
-  uint32_t mi = 0, mo = 0, q = 0, c = 0;
-  if (Q2.pop(&e)) {
-    const uint32_t r = e & 0xFFu, jj = e >> 8;
-    const float4 a = sh.r_pos[r], b = sh.c_pos[jj];
-    const uint32_t ia = sh.r_idc[r], ib = sh.c_idc[jj];
-    mi = ia & 0x3FFFFFFFu; mo = ib & 0x3FFFFFFFu;
-    const double2 ka = s.md_kd[mi], kb = s.md_kd[mo];
-    const Pt pa = make_pt(a.x, a.y, a.z, (int)(ia >> 30)), pb = make_pt(b.x, b.y, b.z, (int)(ib >> 30));
-    pass = ls_eval_d(g, pa, ka.x, ka.y, pb, kb.x, kb.y, &o);
-    q = r / rpi; c = (r - q * rpi) * (uint32_t)nj + jj;
-  }
-  const uint32_t pos = pool_reserve(s.hdr, st, S_LS, pass);
-  if (pass) atomicOr(&umask[q * kItemWords + (c >> 5)], 1u << (c & 31));
-  if (pos != 0xFFFFFFFFu) {
-    st.pkey[pos] = (it0 + q * nct) * (uint32_t)kItemCand + c;
-    st.p_ab[pos] = make_uint2(mi, mo);
-    st.p_f4[pos] = make_float4((float)o.dphi, (float)o.kappa, (float)o.sigk, 0.0f);
-  }
-}
 __device__ __forceinline__ void ls_stage2(const LsShared &sh, const SlotDev &s, const Params &g, WarpQueue &Q1,
-                                          WarpQueue &Q2, uint32_t *umask, uint32_t rpi, int nj, uint32_t it0,
-                                          uint32_t nct) {
-  uint32_t e = 0;
+                                          uint32_t rpi, int nj, uint32_t it0, uint32_t nct) {
+  uint32_t e = 0, mi = 0, mo = 0, key = 0;
   bool keep = false;
   if (Q1.pop(&e)) {
     const uint32_t r = e & 0xFFu, jj = e >> 8;
     const float4 a = sh.r_pos[r], b = sh.c_pos[jj];
     const uint32_t ia = sh.r_idc[r], ib = sh.c_idc[jj];
-    const float2 ka = s.md_kf[ia & 0x3FFFFFFFu], kb = s.md_kf[ib & 0x3FFFFFFFu];
+    mi = ia & 0x3FFFFFFFu; mo = ib & 0x3FFFFFFFu;
+    const float2 ka = s.md_kf[mi], kb = s.md_kf[mo];
     keep = ls_pre_f(g, a.x, a.y, a.z, a.w, ka.x, ka.y, (int)(ia >> 30), b.x, b.y, b.z, b.w, kb.x, kb.y, (int)(ib >> 30));
+    const uint32_t q = r / rpi, c = (r - q * rpi) * (uint32_t)nj + jj;
+    key = (it0 + q * nct) * (uint32_t)kItemCand + c;
   }
-  Q2.push(keep, e);
-  if (Q2.n >= 32u) ls_stage3(sh, s, g, Q2, umask, rpi, nj, it0, nct);
+  cl_append(s.hdr, s.st[S_LS], S_LS, keep, key, make_uint2(mi, mo));
 }
 
-__global__ void __launch_bounds__(kThreads, 6) k_ls_eval(GeoDev geo, SlotDev s, Params g) {
+__global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, Params g) {
   __shared__ LsShared sh;
   const StageBuf &st = s.st[S_LS];
   const uint32_t n_units = s.hdr->n_units[S_LS];
   const int tid = threadIdx.x, lane = tid & 31, wib = tid >> 5;
   constexpr int kWarps = kThreads / 32;
   if (tid < 4) sh.tab[tid] = make_float4(g.f_sig_z[tid], g.f_sig_r[tid], g.f_sig_t[tid], 0.0f);
-  WarpQueue Q1, Q2;
+  WarpQueue Q1;
   Q1.init(sh.q1[wib]);
-  Q2.init(sh.q2[wib]);
   __shared__ uint32_t sh_unit[2];
   for (;;) {
     __syncthreads();                            // the previous unit is done with the shared arrays
@@ -246,7 +221,8 @@ __global__ void __launch_bounds__(kThreads, 6) k_ls_eval(GeoDev geo, SlotDev s, 
       sh.r_pos[k] = s.md_pos[md];
       sh.r_idc[k] = md | ((s.md_mod[md] & 3u) << 30);
     }
-    for (int k = tid; k < (int)(qn * kItemWords); k += kThreads) sh.umask[k] = 0;
+    for (int k = tid; k < (int)(qn * kItemWords); k += kThreads)      // the decide kernel ORs the pass bits in
+      st.mask[(size_t)(it0 + (k / kItemWords) * nct) * kItemWords + (k % kItemWords)] = 0;
     __syncthreads();
     for (int k = tid; k < nj; k += kThreads) {
       const uint32_t md = map_col_to_md(sh.mr, j0 + k);
@@ -270,14 +246,38 @@ __global__ void __launch_bounds__(kThreads, 6) k_ls_eval(GeoDev geo, SlotDev s, 
         const bool keep = has && ls_tier1_f(g, a.x, a.y, a.z, a.w, ta.x, ta.y, ta.z, b.x, b.y, b.z, b.w, tb.x, tb.y, tb.z,
                                             cb >= 2u);
         Q1.push(keep, (uint32_t)r | ((uint32_t)jj << 8));
-        if (Q1.n >= 32u) ls_stage2(sh, s, g, Q1, Q2, sh.umask, rpi, nj, it0, nct);
+        if (Q1.n >= 32u) ls_stage2(sh, s, g, Q1, rpi, nj, it0, nct);
       }
     }
-    while (Q1.n) ls_stage2(sh, s, g, Q1, Q2, sh.umask, rpi, nj, it0, nct);
-    while (Q2.n) ls_stage3(sh, s, g, Q2, sh.umask, rpi, nj, it0, nct);
-    __syncthreads();
-    for (uint32_t qi = wib; qi < qn; qi += kWarps) {          // publish the unit's item masks
-      publish_item(st, it0 + qi * nct, sh.umask[qi * kItemWords + lane]);
+    while (Q1.n) ls_stage2(sh, s, g, Q1, rpi, nj, it0, nct);
+  }
+}
+
+// fp64 decision of the listed candidates, one thread each (dense warps, no staging); an accepted
+// candidate sets its pass bit and writes its results to the pool.
+__global__ void __launch_bounds__(128) k_ls_decide(SlotDev s, Params g) {
+  const StageBuf &st = s.st[S_LS];
+  Header *hdr = s.hdr;
+  const uint32_t n = min(hdr->cl_used[S_LS], st.cap_cl);
+  const uint32_t nround = (n + 31u) & ~31u;
+  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < nround; j += gridDim.x * blockDim.x) {
+    bool pass = false;
+    LsOut o;
+    uint32_t key = 0;
+    uint2 ab = make_uint2(0u, 0u);
+    if (j < n) {
+      key = st.cl_key[j]; ab = st.cl_ab[j];
+      const float4 a = s.md_pos[ab.x], b = s.md_pos[ab.y];
+      const double2 ka = s.md_kd[ab.x], kb = s.md_kd[ab.y];
+      const Pt pa = make_pt(a.x, a.y, a.z, (int)(s.md_mod[ab.x] & 3u)), pb = make_pt(b.x, b.y, b.z, (int)(s.md_mod[ab.y] & 3u));
+      pass = ls_eval_d(g, pa, ka.x, ka.y, pb, kb.x, kb.y, &o);
+    }
+    const uint32_t pos = pool_reserve(hdr, st, S_LS, pass);
+    if (pass) atomicOr(&st.mask[(size_t)(key / kItemCand) * kItemWords + ((key % kItemCand) >> 5)], 1u << (key & 31u));
+    if (pos != 0xFFFFFFFFu) {
+      st.pkey[pos] = key;
+      st.p_ab[pos] = ab;
+      st.p_f4[pos] = make_float4((float)o.dphi, (float)o.kappa, (float)o.sigk, 0.0f);
     }
   }
 }
@@ -311,6 +311,8 @@ void launch_ls(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   k_ls_groups<<<(c.geo.n_modules + 127) / 128, 128, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_ls_groups");
   launch_emit(c, s, S_LS, -1, st);
   k_ls_eval<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_ls_eval");
+  k_ls_decide<<<persistent_grid(c, 4), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_ls_decide");
+  launch_item_counts(c, s, S_LS, st);
   launch_scan_items(c, s, S_LS, 1, s.cap_ls, st);
   k_ls_fill<<<persistent_grid(c, 4), 256, 0, st>>>(s); LST_MARK(c, st, "k_ls_fill");
   launch_row_offsets(c, s, 1, st);

@@ -24,16 +24,16 @@ enum { J_T3 = 0, J_T5 = 1, J_PT5 = 2, J_PT3 = 3 };
 
 template <int KIND> struct JoinTraits;
 template <> struct JoinTraits<J_T3> {
-  static constexpr const char *n_groups = "k_join_groups[T3]", *n_eval = "k_join_eval[T3]", *n_fill = "k_join_fill[T3]";
+  static constexpr const char *n_groups = "k_join_groups[T3]", *n_eval = "k_join_eval[T3]", *n_decide = "k_join_decide[T3]", *n_fill = "k_join_fill[T3]";
   static constexpr int stage = S_T3, rows_level = 1, out_level = 2; };
 template <> struct JoinTraits<J_T5> {
-  static constexpr const char *n_groups = "k_join_groups[T5]", *n_eval = "k_join_eval[T5]", *n_fill = "k_join_fill[T5]";
+  static constexpr const char *n_groups = "k_join_groups[T5]", *n_eval = "k_join_eval[T5]", *n_decide = "k_join_decide[T5]", *n_fill = "k_join_fill[T5]";
   static constexpr int stage = S_T5, rows_level = 2, out_level = 3; };
 template <> struct JoinTraits<J_PT5> {
-  static constexpr const char *n_groups = "k_join_groups[pT5]", *n_eval = "k_join_eval[pT5]", *n_fill = "k_join_fill[pT5]";
+  static constexpr const char *n_groups = "k_join_groups[pT5]", *n_eval = "k_join_eval[pT5]", *n_decide = "k_join_decide[pT5]", *n_fill = "k_join_fill[pT5]";
   static constexpr int stage = S_PT5, rows_level = kPairLevel, out_level = 5; };
 template <> struct JoinTraits<J_PT3> {
-  static constexpr const char *n_groups = "k_join_groups[pT3]", *n_eval = "k_join_eval[pT3]", *n_fill = "k_join_fill[pT3]";
+  static constexpr const char *n_groups = "k_join_groups[pT3]", *n_eval = "k_join_eval[pT3]", *n_decide = "k_join_decide[pT3]", *n_fill = "k_join_fill[pT3]";
   static constexpr int stage = S_PT3, rows_level = kPairLevel, out_level = 4; };
 
 template <int KIND>
@@ -219,68 +219,35 @@ __device__ __forceinline__ void stage_seeds(float4 *rowseed, const SlotDev &s, c
   rowseed[tid] = v;
 }
 
-// Phase 1 of a join candidate: a cheap necessary condition evaluated on every candidate (T5: the
-// radius match T5-1 on the stored kappa3; pixel: the fp32 first-anchor pre-filter).  T3 has none.
+// Phase 1 of a join candidate: a cheap necessary condition evaluated on every candidate (T3: the
+// fp32 pre-filter t3_pre_f; T5: the radius match T5-1 on the stored kappa3; pixel: the fp32
+// first-anchor pre-filter).  *ab = the pair handed to the decide kernel.
 template <int KIND>
 __device__ __forceinline__ bool join_phase1(const SlotDev &s, const Params &g, uint32_t row, uint32_t b,
-                                            const float4 *rowseed, int lrow) {
-  if (KIND == J_T3) return true;
+                                            const float4 *rowseed, int lrow, uint2 *ab) {
+  *ab = make_uint2(row, b);
+  if (KIND == J_T3) {
+    const uint2 la = s.ls_md[row], lb = s.ls_md[b];
+    const float4 p1 = s.md_pos[la.x], p2 = s.md_pos[la.y], p3 = s.md_pos[lb.y];
+    const int c1 = (int)(s.md_mod[la.x] & 3u), c2 = (int)(s.md_mod[la.y] & 3u), c3 = (int)(s.md_mod[lb.y] & 3u);
+    return t3_pre_f(g, p1.x, p1.y, p1.z, p1.w, c1, p2.x, p2.y, p2.z, p2.w, c2, p3.x, p3.y, p3.z, p3.w, c3);
+  }
   if (KIND == J_T5) {
     const double2 k3a = s.t3_kd[row], k3b = s.t3_kd[b];
     return le(fabs(k3a.x - k3b.x), g.ns * (k3a.y + k3b.y));
   }
+  ab->x = s.px_pair[row].x;     // the seed
   return px_pre_f<KIND>(s, g, rowseed[lrow], b);
 }
 
-// Phase 2: the fp64 decision of candidate (row, b); an accepted candidate's results go to the
-// stage's pool (all 32 lanes of a warp call; `live` = this lane holds a candidate).
-template <int KIND>
-__device__ __forceinline__ bool join_phase2(const GeoDev &geo, const SlotDev &s, const Params &g, bool live,
-                                            uint32_t row, uint32_t b, uint32_t key) {
-  const int stage = JoinTraits<KIND>::stage;
-  const StageBuf &st = s.st[stage];
-  bool pass = false;
-  if (KIND == J_T3) {
-    T3Out o;
-    if (live) pass = t3_candidate(s, g, row, b, &o, nullptr);
-    const uint32_t pos = pool_reserve(s.hdr, st, stage, pass);
-    if (pos != 0xFFFFFFFFu) {
-      st.pkey[pos] = key;
-      st.p_ab[pos] = make_uint2(row, b);
-      st.p_d2[pos] = make_double2(o.kappa3, o.sigk3);
-      st.p_f4[pos] = make_float4((float)o.beta, 0.f, 0.f, 0.f);
-    }
-  } else if (KIND == J_T5) {
-    T5Out o;
-    if (live) pass = t5_candidate(s, g, row, b, &o, nullptr, nullptr, nullptr);
-    const uint32_t pos = pool_reserve(s.hdr, st, stage, pass);
-    if (pos != 0xFFFFFFFFu) {
-      st.pkey[pos] = key;
-      st.p_ab[pos] = make_uint2(row, b);
-      st.p_d2[pos] = make_double2(o.eta, o.phi);
-      st.p_d2b[pos] = make_double2(o.chi2, o.R);
-      st.p_f4[pos] = make_float4((float)o.pt, 0.f, 0.f, 0.f);
-    }
-  } else {
-    double c2 = 0.0;
-    const uint32_t p = live ? s.px_pair[row].x : 0u;
-    if (live) pass = px_candidate<KIND>(geo, s, g, p, b, &c2);
-    const uint32_t pos = pool_reserve(s.hdr, st, stage, pass);
-    if (pos != 0xFFFFFFFFu) {
-      st.pkey[pos] = key;
-      st.p_ab[pos] = make_uint2(p, b);
-      st.p_d2[pos] = make_double2(c2, 0.0);
-    }
-  }
-  return pass;
-}
-
+// Pre-filter kernel: every candidate of every item through phase 1; survivors go to the stage's
+// candidate list.  One barrier-free candidate loop per item after the row table is staged.
 template <int KIND>
 __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, Params g) {
-  __shared__ ItemScratch sc;
   __shared__ RowTab rt;
   __shared__ uint32_t sh[33];
   __shared__ float4 rowseed[(KIND == J_PT5 || KIND == J_PT3) ? kRowChunk : 1];
+  (void)geo;
   const int stage = JoinTraits<KIND>::stage;
   const StageBuf &st = s.st[stage];
   const uint32_t n_items = s.hdr->n_items[stage];
@@ -290,46 +257,72 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
     const Item item = st.items[it];
     const uint32_t r0 = item.group * kRowChunk;
     const uint32_t key0 = it * (uint32_t)kItemCand;
-    if (tid < kItemWords) sc.mask[tid] = 0;
-    if (tid == 0) sc.n = 0;
+    if (tid < kItemWords) st.mask[(size_t)it * kItemWords + tid] = 0;   // the decide kernel ORs the pass bits in
     if (KIND == J_PT5 || KIND == J_PT3) stage_seeds(rowseed, s, g, r0, n_rows);
     stage_rows<KIND>(rt, s, r0, n_rows, sh);
     stage_hints(rt, item.j0);
     const int nj = item.nj;
-    if (KIND == J_T3) {
-      for (int base = 0; base < nj; base += kThreads) {
-        const int c = base + tid;
-        int row = 0; uint32_t b = 0;
-        if (c < nj) item_to_pair(rt, item.j0, c, &row, &b);
-        const bool pass = join_phase2<KIND>(geo, s, g, c < nj, r0 + row, b, key0 + (uint32_t)c);
-        const uint32_t w = __ballot_sync(0xffffffffu, pass);
-        if ((tid & 31) == 0) sc.mask[c >> 5] = w;
+    for (int base = 0; base < nj; base += kThreads) {
+      const int c = base + tid;
+      bool keep = false;
+      uint2 ab = make_uint2(0u, 0u);
+      if (c < nj) {
+        int row; uint32_t b;
+        item_to_pair(rt, item.j0, c, &row, &b);
+        keep = join_phase1<KIND>(s, g, r0 + row, b, rowseed, row, &ab);
       }
-    } else {
-      // phase 1 on every candidate, survivors compacted; phase 2 (fp64) on the dense survivor list
-      for (int base = 0; base < nj; base += kThreads) {
-        const int c = base + tid;
-        bool keep = false;
-        if (c < nj) {
-          int row; uint32_t b;
-          item_to_pair(rt, item.j0, c, &row, &b);
-          keep = join_phase1<KIND>(s, g, r0 + row, b, rowseed, row);
-        }
-        push_survivor(sc, keep, (uint32_t)c);
-      }
-      __syncthreads();
-      const int nsv = (int)sc.n;
-      for (int base = 0; base < nsv; base += kThreads) {
-        const int k = base + tid;
-        int c = 0, row = 0; uint32_t b = 0;
-        if (k < nsv) { c = sc.list[k]; item_to_pair(rt, item.j0, c, &row, &b); }
-        if (join_phase2<KIND>(geo, s, g, k < nsv, r0 + row, b, key0 + (uint32_t)c))
-          atomicOr(&sc.mask[c >> 5], 1u << (c & 31));
-      }
+      cl_append(s.hdr, st, stage, keep, key0 + (uint32_t)c, ab);
     }
     __syncthreads();
-    publish_mask(sc, st, it);
-    __syncthreads();
+  }
+}
+
+// Decide kernel: the fp64 decision of the listed candidates, one thread each (dense warps, no
+// staging); an accepted candidate sets its pass bit and writes its results to the stage's pool.
+template <int KIND>
+__global__ void __launch_bounds__(128) k_join_decide(GeoDev geo, SlotDev s, Params g) {
+  const int stage = JoinTraits<KIND>::stage;
+  const StageBuf &st = s.st[stage];
+  Header *hdr = s.hdr;
+  const uint32_t n = min(hdr->cl_used[stage], st.cap_cl);
+  const uint32_t nround = (n + 31u) & ~31u;
+  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < nround; j += gridDim.x * blockDim.x) {
+    const bool live = j < n;
+    const uint32_t key = live ? st.cl_key[j] : 0u;
+    const uint2 ab = live ? st.cl_ab[j] : make_uint2(0u, 0u);
+    bool pass = false;
+    if (KIND == J_T3) {
+      T3Out o;
+      if (live) pass = t3_candidate(s, g, ab.x, ab.y, &o, nullptr);
+      const uint32_t pos = pool_reserve(hdr, st, stage, pass);
+      if (pos != 0xFFFFFFFFu) {
+        st.pkey[pos] = key;
+        st.p_ab[pos] = ab;
+        st.p_d2[pos] = make_double2(o.kappa3, o.sigk3);
+        st.p_f4[pos] = make_float4((float)o.beta, 0.f, 0.f, 0.f);
+      }
+    } else if (KIND == J_T5) {
+      T5Out o;
+      if (live) pass = t5_candidate(s, g, ab.x, ab.y, &o, nullptr, nullptr, nullptr);
+      const uint32_t pos = pool_reserve(hdr, st, stage, pass);
+      if (pos != 0xFFFFFFFFu) {
+        st.pkey[pos] = key;
+        st.p_ab[pos] = ab;
+        st.p_d2[pos] = make_double2(o.eta, o.phi);
+        st.p_d2b[pos] = make_double2(o.chi2, o.R);
+        st.p_f4[pos] = make_float4((float)o.pt, 0.f, 0.f, 0.f);
+      }
+    } else {
+      double c2 = 0.0;
+      if (live) pass = px_candidate<KIND>(geo, s, g, ab.x, ab.y, &c2);
+      const uint32_t pos = pool_reserve(hdr, st, stage, pass);
+      if (pos != 0xFFFFFFFFu) {
+        st.pkey[pos] = key;
+        st.p_ab[pos] = ab;
+        st.p_d2[pos] = make_double2(c2, 0.0);
+      }
+    }
+    if (pass) atomicOr(&st.mask[(size_t)(key / kItemCand) * kItemWords + ((key % kItemCand) >> 5)], 1u << (key & 31u));
   }
 }
 
@@ -376,7 +369,9 @@ static void launch_join_t(const Ctx &c, const SlotDev &s, uint32_t row_cap, uint
   const int gg = (int)((row_cap / kRowChunk + 1 + 3) / 4);   // 4 warps per block, one group per warp
   k_join_groups<KIND><<<gg < c.n_sm * 8 ? gg : c.n_sm * 8, 128, 0, st>>>(s); LST_MARK(c, st, JoinTraits<KIND>::n_groups);
   launch_emit(c, s, JoinTraits<KIND>::stage, JoinTraits<KIND>::rows_level, st);
-  k_join_eval<KIND><<<c.n_sm * 8, kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, JoinTraits<KIND>::n_eval);
+  k_join_eval<KIND><<<c.n_sm * 16, kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, JoinTraits<KIND>::n_eval);
+  k_join_decide<KIND><<<c.n_sm * 4, 128, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, JoinTraits<KIND>::n_decide);
+  launch_item_counts(c, s, JoinTraits<KIND>::stage, st);
   launch_scan_items(c, s, JoinTraits<KIND>::stage, JoinTraits<KIND>::out_level, out_cap, st);
   k_join_fill<KIND><<<c.n_sm * 4, 256, 0, st>>>(s); LST_MARK(c, st, JoinTraits<KIND>::n_fill);
 }

@@ -341,6 +341,9 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
     b.p_d2 = w.take<double2>(b.cap_pool);
     b.p_d2b = k == S_T5 ? w.take<double2>(b.cap_pool) : nullptr;
     b.p_f4 = w.take<float4>(b.cap_pool);
+    b.cap_cl = 2 * b.cap_pool + 4096;
+    b.cl_key = w.take<uint32_t>(b.cap_cl);
+    b.cl_ab = w.take<uint2>(b.cap_cl);
   }
   // export scratch: the largest level
   size_t obj_cap = std::max({(size_t)s.cap_md, (size_t)s.cap_ls, (size_t)s.cap_t3, (size_t)s.cap_t5,
@@ -735,6 +738,8 @@ extern "C" int lst_host_eval(const lst_config *cfg_in, int level, uint32_t n, co
     } else if (level == LST_T3) {
       T3Out o = {0, 0, 0};
       ok = t3_eval_d(g, P[0], P[1], P[2], &o);
+      pr = t3_pre_f(g, p[0], p[1], p[2], sqrtf(p[0] * p[0] + p[1] * p[1]), ct[0], p[3], p[4], p[5],
+                    sqrtf(p[3] * p[3] + p[4] * p[4]), ct[1], p[6], p[7], p[8], sqrtf(p[6] * p[6] + p[7] * p[7]), ct[2]);
       o3[0] = o.kappa3; o3[1] = o.sigk3; o3[2] = o.beta;
     } else {
       const double *a = aux + 4 * (size_t)i;

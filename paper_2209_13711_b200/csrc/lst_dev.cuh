@@ -73,6 +73,7 @@ struct Header {          // per slot, device; zeroed (except n_hits / n_seeds) a
   uint32_t n_units[S_NSTAGE];        // work units (k_emit_items): item runs that share their columns
   uint32_t next_unit[S_NSTAGE];      // dynamic work distribution: next unit to hand out
   uint32_t pool_used[S_NSTAGE];      // accepted candidates written to the stage's pool so far
+  uint32_t cl_used[S_NSTAGE];        // pre-filter survivors appended to the stage's candidate list
   uint32_t err;
   uint32_t n_dd;                     // T5 + pT5 + pT3 objects entering the cleaning
   uint32_t n_flag;                   // pT5 + pT3 + T5 + seeds: length of the TC keep-flag array
@@ -96,7 +97,10 @@ struct StageBuf {        // work list of one stage
   uint2 *p_ab;           // [cap_pool] constituent indices
   double2 *p_d2, *p_d2b; // [cap_pool] fp64 results (p_d2b: T5 only)
   float4 *p_f4;          // [cap_pool] fp32 results
-  uint32_t cap_groups, cap_items, cap_pool;
+  // candidate list: survivors of the cheap pre-filter kernel, decided in fp64 by the decide kernel
+  uint32_t *cl_key;      // [cap_cl] item * kItemCand + candidate
+  uint2 *cl_ab;          // [cap_cl] the pair (row object, column object)
+  uint32_t cap_groups, cap_items, cap_pool, cap_cl;
 };
 
 // Static detector data (device), shared by all slots.
@@ -333,6 +337,21 @@ __device__ __forceinline__ uint32_t pool_reserve(Header *hdr, const StageBuf &st
   if (pos >= st.cap_pool) { atomicOr(&hdr->err, (uint32_t)ERR_CAP_OBJ); return 0xFFFFFFFFu; }
   return pos;
 }
+// pre-filter kernels: append the surviving lanes' candidates to the stage's list (all 32 lanes call)
+__device__ __forceinline__ void cl_append(Header *hdr, const StageBuf &st, int stage, bool keep, uint32_t key, uint2 ab) {
+  const uint32_t b = __ballot_sync(0xffffffffu, keep);
+  if (b == 0) return;
+  const int lane = threadIdx.x & 31, leader = __ffs(b) - 1;
+  uint32_t base = 0;
+  if (lane == leader) base = atomicAdd(&hdr->cl_used[stage], (uint32_t)__popc(b));
+  base = __shfl_sync(0xffffffffu, base, leader);
+  const uint32_t pos = base + __popc(b & ((1u << lane) - 1u));
+  if (!keep) return;
+  if (pos >= st.cap_cl) { atomicOr(&hdr->err, (uint32_t)ERR_CAP_ITEMS); return; }
+  st.cl_key[pos] = key;
+  st.cl_ab[pos] = ab;
+}
+
 // fill: canonical index of pool entry `key` = item * kItemCand + candidate
 __device__ __forceinline__ uint32_t pool_target(const StageBuf &st, uint32_t key, uint32_t *item, uint32_t *cand) {
   const uint32_t it = key / (uint32_t)kItemCand, c = key % (uint32_t)kItemCand;

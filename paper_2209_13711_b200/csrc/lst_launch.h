@@ -35,6 +35,7 @@ struct Ctx {             // what the launchers need from a context
 // k_common.cu
 void launch_index(const Ctx &c, const SlotDev &s, cudaStream_t st);                       // 1 memset + 5 kernels
 void launch_emit(const Ctx &c, const SlotDev &s, int stage, int rows_level, cudaStream_t st);
+void launch_item_counts(const Ctx &c, const SlotDev &s, int stage, cudaStream_t st);
 void launch_scan_items(const Ctx &c, const SlotDev &s, int stage, int level, uint32_t cap, cudaStream_t st);
 void launch_row_offsets(const Ctx &c, const SlotDev &s, int kind, cudaStream_t st);
 void launch_scan(const Ctx &c, const SlotDev &s, const uint32_t *in, uint32_t *out, const uint32_t *n_ptr,

@@ -338,6 +338,57 @@ LST_HD bool t3_eval_d(const Params &g, const Pt &P1, const Pt &P2, const Pt &P3,
   return ok;
 }
 
+// fp32 pre-filter of a triplet: T3-1 (multiplied through by a b c13, no division) and T3-3, both
+// without trigonometry; T3-2 (second differences of angles) is left to the fp64 decision.  Loosened
+// by kPreSlack and, for T3-3, an absolute 0.02 cm^2 (fp32 error of N is < 2e-3; N_sigma E >= ~8).
+LST_HD bool t3_pre_f(const Params &g, float x1, float y1, float z1, float r1, int c1, float x2, float y2, float z2,
+                     float r2, int c2, float x3, float y3, float z3, float r3, int c3) {
+  const float d12x = x2 - x1, d12y = y2 - y1, d23x = x3 - x2, d23y = y3 - y2, d13x = x3 - x1, d13y = y3 - y1;
+  const float a2 = d12x * d12x + d12y * d12y, b2 = d23x * d23x + d23y * d23y, c2q = d13x * d13x + d13y * d13y;
+  if (!(a2 > 1e-10f) || !(b2 > 1e-10f) || !(c2q > 1e-10f)) return true;   // guards are decided in fp64
+  const float a = sqrtf(a2), b = sqrtf(b2), c13 = sqrtf(c2q);
+  const float crs = d12x * d23y - d12y * d23x;
+  const float sp1 = g.f_sig_t[c1] + g.f_sig_r[c1] * fminf(1.0f, g.f_kmax * r1);
+  const float sp2 = g.f_sig_t[c2] + g.f_sig_r[c2] * fminf(1.0f, g.f_kmax * r2);
+  const float sp3 = g.f_sig_t[c3] + g.f_sig_r[c3] * fminf(1.0f, g.f_kmax * r3);
+  const float abc = a * b * c13;
+  if (fabsf(crs) > (g.f_kmax * abc + g.f_ns * (sp2 * c13 + b * sp1 + a * sp3)) * kPreSlack) return false;   // T3-1
+  const float k3 = crs / abc;
+  const float q1 = k3 * r1, q2 = k3 * r2, q3 = k3 * r3;
+  const float s21 = (r2 - r1) + (r2 * q2 * q2 - r1 * q1 * q1) * (1.0f / 6.0f);
+  const float s31 = (r3 - r1) + (r3 * q3 * q3 - r1 * q1 * q1) * (1.0f / 6.0f);
+  const float s32 = s31 - s21;
+  const float z31 = z3 - z1, z21 = z2 - z1, z32 = z3 - z2;
+  const float N = s21 * z31 - s31 * z21;
+  const float E = g.f_sig_z[c3] * fabsf(s21) + g.f_sig_z[c2] * fabsf(s31) + g.f_sig_z[c1] * fabsf(s32) +
+                  g.f_sig_r[c2] * fabsf(z31) + g.f_sig_r[c3] * fabsf(z21) + g.f_sig_r[c1] * fabsf(z32);
+  if (fabsf(N) > g.f_ns * E * kPreSlack + 0.02f) return false;                                              // T3-3
+  // T3-2 in fp32: its error (~5e-6, from atan2f / asinf and the products) is three orders of magnitude
+  // below the smallest threshold (~5e-3); loosened by 1 % and 2e-4 absolute.
+  const float d12 = atan2f(x1 * d12y - y1 * d12x, x1 * x2 + y1 * y2);
+  const float d23 = atan2f(x2 * d23y - y2 * d23x, x2 * x3 + y2 * y3);
+  const float d13 = d12 + d23;
+  float L1, L2, L3, sl1 = 0.0f, sl2 = 0.0f, sl3 = 0.0f;
+  if (c1 >= 2 || c2 >= 2 || c3 >= 2) {
+    L1 = z1; L2 = z2; L3 = z3;
+    sl1 = g.f_sig_z[c1]; sl2 = g.f_sig_z[c2]; sl3 = g.f_sig_z[c3];
+  } else {
+    const float k13 = sinf(d13) / c13;
+    const float u1 = k13 * r1, u2 = k13 * r2, u3 = k13 * r3;
+    L1 = fabsf(u1) <= 1e-4f ? r1 : asinf(fminf(1.0f, fmaxf(-1.0f, u1))) / k13;
+    L2 = fabsf(u2) <= 1e-4f ? r2 : asinf(fminf(1.0f, fmaxf(-1.0f, u2))) / k13;
+    L3 = fabsf(u3) <= 1e-4f ? r3 : asinf(fminf(1.0f, fmaxf(-1.0f, u3))) / k13;
+  }
+  const float i1 = 1.0f / r1, i2 = 1.0f / r2, i3 = 1.0f / r3;
+  const float L32 = L3 - L2, L21 = L2 - L1, L31 = L3 - L1;
+  const float Nphi = d12 * L32 - d23 * L21;
+  const float Nrho = (i2 - i1) * L32 - (i3 - i2) * L21;
+  const float Ephi = g.f_sig_t[c1] * i1 * fabsf(L32) + g.f_sig_t[c2] * i2 * fabsf(L31) + g.f_sig_t[c3] * i3 * fabsf(L21) +
+                     sl1 * fabsf(d23) + sl2 * fabsf(d13) + sl3 * fabsf(d12);
+  if (fabsf(Nphi) > ((float)g.d0max * fabsf(Nrho) + g.f_ns * Ephi) * 1.01f + 2e-4f) return false;           // T3-2
+  return true;
+}
+
 // ------------------------------------------------------------------ C5 quintuplet
 struct T5Out { double R, chi2, pt, eta, phi; };
 

@@ -169,10 +169,13 @@ def test_t3_t5_arithmetic_equals_oracle(geom_full, small_full):
     aa, bb = np.concatenate(aa), np.concatenate(bb)
     m = np.stack([lp[aa, 0], lp[aa, 1], lp[bb, 1]], 1)
     pts = xyz[m].reshape(len(m), 9)
-    ok, _, f = B.lst_host_eval(B.LST_T3, pts, cat[m])
+    ok, pre, f = B.lst_host_eval(B.LST_T3, pts, cat[m])
     want = set(map(tuple, t3["parents"].tolist()))
     got = set(zip(aa[ok].tolist(), bb[ok].tolist()))
     assert got == want and len(want) > 500
+    assert not (ok & ~pre).any(), "fp32 pre-filter rejected an accepted T3"
+    print("T3 pre-filter keeps %.3f of the candidates, %.3f pass" % (pre.mean(), ok.mean()))
+    assert pre.mean() < 0.9                      # and it does filter
     idx = {t: k for k, t in enumerate(zip(aa.tolist(), bb.tolist()))}
     sel = np.array([idx[t] for t in map(tuple, t3["parents"].tolist())])
     assert np.allclose(f[sel, 0], t3["f"][:, 1], rtol=1e-9, atol=0)      # kappa3
