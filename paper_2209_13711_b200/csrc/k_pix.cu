@@ -20,32 +20,24 @@ __device__ __forceinline__ float wrap_f(float d) {   // to [-pi, pi]; error ~1e-
   return d - 6.2831853071795864769f * rintf(d * 0.15915494309189533577f);
 }
 
-// Can a hit inside a start module's lower-sensor box pass the first-anchor cuts of seed
-// (kp, sinh eta, phi, z0)?  b1 = {phic, hphi, rmin, rmax}, b2 = {zmin, zmax, category, -}.
-// A cheap necessary condition on the azimuth comes first (no inverse trigonometric function:
-// asin(x) <= x + (pi/2 - 1) x^3 on [0, 1]); it removes > 90 % of the (seed, module) pairs.
-__device__ __forceinline__ bool px_module_compatible(const Params &g, float4 b1, float4 b2, float kp, float sh,
-                                                     float phi, float z0) {
-  const int cat = (int)b2.z;
-  const float phic = b1.x, hphi = b1.y, rlo = b1.z, rhi = b1.w;
-  const float zlo = b2.x, zhi = b2.y;
+// Can a hit inside a ROW of start modules (same box up to phic) pass the first-anchor cuts of seed
+// (kp, sinh eta, phi, z0)?  Everything except the module's phic is decided here; for a compatible
+// row the azimuthal window |wrap(phic - *centre)| <= *halfw selects its modules.
+// r1 = {hphi, rmin, rmax, category}, r2 = {zmin, zmax, sig_t / rmin, -}.
+__device__ __forceinline__ bool px_row_window(const Params &g, float4 r1, float4 r2, float kp, float sh, float phi,
+                                              float z0, float *centre, float *halfw) {
+  const int cat = (int)r1.w;
+  const float hphi = r1.x, rlo = r1.y, rhi = r1.z, zlo = r2.x, zhi = r2.y;
   const float akp = fabsf(kp);
   const float sgn = kp < 0.0f ? -1.0f : 1.0f;
   const float ns = g.f_ns;
-  const float d0 = wrap_f(phic - phi);
   if (cat < 2) {
-    {
-      const float x = fminf(1.0f, akp * rhi);
-      const float ub = x + 0.5708f * x * x * x;   // >= asin(x) >= |kp| s(r) for every r in the box
-      const float sgp_ub = (float)g.seed_sig_phi + (float)g.seed_sig_pt * ub + g.f_sig_t[cat] / rlo;
-      if (fabsf(d0) > (hphi + ub + ns * sgp_ub) * kPreSlack + kPxMarginPhi + 1e-4f) return false;
-    }
     // barrel: arc length s(r) = asin(|k| r) / |k| is increasing in r
     const float a_lo = asin_sat(akp * rlo), a_hi = asin_sat(akp * rhi);
     const float s_lo = akp * rlo <= 1e-4f ? rlo : a_lo / akp, s_hi = akp * rhi <= 1e-4f ? rhi : a_hi / akp;
-    const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * akp * s_hi + g.f_sig_t[cat] / rlo;
-    const float dphi = fabsf(wrap_f(d0 - sgn * 0.5f * (a_lo + a_hi)));
-    if (dphi > hphi + 0.5f * (a_hi - a_lo) + ns * sgp + kPxMarginPhi) return false;
+    const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * akp * s_hi + r2.z;
+    *centre = phi + sgn * 0.5f * (a_lo + a_hi);
+    *halfw = hphi + 0.5f * (a_hi - a_lo) + ns * sgp + kPxMarginPhi;
     const float z1 = z0 + sh * s_lo, z2 = z0 + sh * s_hi;
     const float tol = ns * ((float)g.seed_sig_z + g.f_sig_z[cat]) + kPxMarginLen + 1e-3f * (fabsf(z1) + fabsf(z2));
     return fmaxf(z1, z2) + tol >= zlo && fminf(z1, z2) - tol <= zhi;
@@ -54,40 +46,21 @@ __device__ __forceinline__ bool px_module_compatible(const Params &g, float4 b1,
   if (!(fabsf(sh) > 1e-9f)) return false;
   const float al = (zlo - z0) / sh;
   if (!(al > 0.0f)) return false;
-  const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * akp * al + g.f_sig_t[cat] / rlo;
-  const float dphi = fabsf(wrap_f(d0 - kp * al));
-  if (dphi > hphi + ns * sgp + kPxMarginPhi + 1e-3f * akp * al) return false;
+  const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * akp * al + r2.z;
+  *centre = phi + kp * al;
+  *halfw = hphi + ns * sgp + kPxMarginPhi + 1e-3f * akp * al;
   const float ka = kp * al;
   const float rp = fabsf(ka) <= 1e-4f ? al : sinf(ka) / kp;
   const float tol = ns * ((float)g.seed_sig_z / fabsf(sh) + g.f_sig_r[cat]) + kPxMarginLen + 1e-3f * fabsf(rp);
   return rp + tol >= rlo && rp - tol <= rhi;
 }
 
-// Stage 1 of the (seed, start module) test: the azimuthal window only, cheap and necessary.
-// Barrel: |phic - phi| against the widest window any r in the box allows (asin(x) <= x + (pi/2 - 1) x^3);
-// endcap: the exact azimuthal test (the arc length is fixed by the plane's z; inv_sh = 1 / sinh eta).
-__device__ __forceinline__ bool px_module_phi(const Params &g, float4 b1, float4 b2, float kp, float inv_sh,
-                                              float phi, float z0) {
-  const float akp = fabsf(kp);
-  const float d0 = wrap_f(b1.x - phi);
-  if (b2.z < 2.0f) {
-    const float x = fminf(1.0f, akp * b1.w);
-    const float ub = x + 0.5708f * x * x * x;
-    const float sgp_ub = (float)g.seed_sig_phi + (float)g.seed_sig_pt * ub + b2.w;
-    return !(fabsf(d0) > (b1.y + ub + g.f_ns * sgp_ub) * kPreSlack + kPxMarginPhi + 1e-4f);
-  }
-  const float al = (b2.x - z0) * inv_sh;
-  if (!(al > 0.0f)) return false;
-  const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * akp * al + b2.w;
-  return !(fabsf(wrap_f(d0 - kp * al)) > (b1.y + g.f_ns * sgp) * kPreSlack + kPxMarginPhi + 2e-3f * akp * al + 1e-4f);
-}
-
-// One warp per seed.  FILL = false: test every start module, keep one bit per (seed, module) and
-// count them: stage 1 (px_module_phi) on all modules, its survivors (~5 %) queued per warp and put
-// through the full test 32 at a time.  FILL = true: expand the bits into the (seed, module) rows at
-// the seed's offset, modules ascending.  (A seed with eta ~ 0 is compatible with every endcap
-// module of a side - its extrapolation tolerances diverge - so the lists are sized exactly, not
-// capped per seed.)  Dynamic shared memory: 8 warps x (nw words of bits + 64 queue entries).
+// One warp per seed.  FILL = false: one bit per (seed, start module): the lanes test the module
+// ROWS (32 at a time); for every compatible row the warp walks the row's modules and keeps those
+// inside the azimuthal window.  FILL = true: expand the bits into the (seed, module) rows at the
+// seed's offset, modules ascending.  (A seed with eta ~ 0 is compatible with every endcap module of
+// a side - its extrapolation tolerances diverge - so the lists are sized exactly, not capped per
+// seed.)  Dynamic shared memory: 8 warps x nw words of bits.
 template <bool FILL>
 __global__ void __launch_bounds__(256) k_px_modules(GeoDev geo, SlotDev s, Params g) {
   extern __shared__ uint32_t px_sh[];
@@ -96,7 +69,7 @@ __global__ void __launch_bounds__(256) k_px_modules(GeoDev geo, SlotDev s, Param
   const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
   const uint32_t nw = (geo.n_start + 31) / 32;
   if (FILL && s.hdr->n_obj[kPairLevel] == 0) return;
-  uint32_t *wbits = px_sh + (size_t)wib * (nw + 64), *queue = wbits + nw;
+  uint32_t *wbits = px_sh + (size_t)wib * nw;
   for (uint32_t p = warp; p < n_seeds; p += nwarp) {
     uint32_t *bits = s.px_bits + (size_t)p * nw;
     if (FILL) {
@@ -111,39 +84,28 @@ __global__ void __launch_bounds__(256) k_px_modules(GeoDev geo, SlotDev s, Param
       const float pt = s.seed_pt[p], phi = s.seed_phi[p], z0 = s.seed_z0[p];
       const float kp = -(float)s.seed_q[p] * (float)g.kB / (2.0f * pt);
       const float sh = sinhf(s.seed_eta[p]);
-      const float inv_sh = 1.0f / sh;
-      const bool seed_ok = fabsf(sh) > 1e-9f;   // endcap planes are unreachable for sinh eta ~ 0
       for (uint32_t w = lane; w < nw; w += 32) wbits[w] = 0;
       __syncwarp();
-      uint32_t nq = 0;
-      for (uint32_t w = 0; w <= nw; ++w) {
-        if (w < nw) {
-          const uint32_t k = w * 32 + lane;
-          bool ok = false;
-          if (k < geo.n_start && pt > 0.0f) {
-            const float4 b1 = geo.start_box[k], b2 = geo.start_box2[k];
-            ok = (b2.z < 2.0f || seed_ok) && px_module_phi(g, b1, b2, kp, inv_sh, phi, z0);
-          }
-          const uint32_t b = __ballot_sync(0xffffffffu, ok);
-          if (ok) queue[nq + __popc(b & ((1u << lane) - 1u))] = k;
-          nq += __popc(b);
-          __syncwarp();
-        }
-        if (nq >= 32 || (w == nw && nq > 0)) {
-          const uint32_t take = nq < 32 ? nq : 32;
-          if ((uint32_t)lane < take) {
-            const uint32_t k = queue[lane];
-            if (px_module_compatible(g, geo.start_box[k], geo.start_box2[k], kp, sh, phi, z0))
+      for (uint32_t rb = 0; rb < geo.n_prow; rb += 32) {
+        const uint32_t r = rb + lane;
+        float centre = 0.0f, halfw = 0.0f;
+        bool ok = false;
+        if (r < geo.n_prow && pt > 0.0f) ok = px_row_window(g, geo.prow_b1[r], geo.prow_b2[r], kp, sh, phi, z0, &centre, &halfw);
+        uint32_t live = __ballot_sync(0xffffffffu, ok);
+        while (live) {                                   // warp-uniform loop over the compatible rows
+          const int src = __ffs(live) - 1;
+          live &= live - 1;
+          const float c = __shfl_sync(0xffffffffu, centre, src), hw = __shfl_sync(0xffffffffu, halfw, src);
+          const uint32_t m0 = geo.prow_off[rb + src], m1 = geo.prow_off[rb + src + 1];
+          for (uint32_t m = m0 + lane; m < m1; m += 32) {
+            if (!(fabsf(wrap_f(geo.prow_phic[m] - c)) > hw)) {
+              const uint32_t k = geo.prow_k[m];
               atomicOr(&wbits[k >> 5], 1u << (k & 31));
+            }
           }
-          __syncwarp();
-          const uint32_t mv = (uint32_t)lane + 32 < nq ? queue[lane + 32] : 0u;
-          __syncwarp();
-          if ((uint32_t)lane + 32 < nq) queue[lane] = mv;
-          nq -= take;
-          __syncwarp();
         }
       }
+      __syncwarp();
       uint32_t cnt = 0;
       for (uint32_t w = lane; w < nw; w += 32) {
         const uint32_t b = wbits[w];
@@ -182,7 +144,7 @@ void launch_pixel(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   const int warps_per_block = 8;
   int g = (int)((s.cap_seeds + warps_per_block - 1) / warps_per_block);
   if (g > c.n_sm * 8) g = c.n_sm * 8;
-  const size_t shb = 8 * ((size_t)(c.geo.n_start + 31) / 32 + 64) * sizeof(uint32_t);
+  const size_t shb = 8 * ((size_t)(c.geo.n_start + 31) / 32) * sizeof(uint32_t);
   if (shb > 48 * 1024) cudaFuncSetAttribute(k_px_modules<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shb);
   k_px_modules<false><<<g, 256, shb, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_px_modules<false>");
   k_px_offsets<<<1, 1024, 0, st>>>(s); LST_MARK(c, st, "k_px_offsets");

@@ -405,7 +405,43 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   const size_t box_stride = up((size_t)n * 4);
   const size_t o_start = o_box + 6 * box_stride;
   const size_t o_sbox = o_start + up(std::max<size_t>(start_mods.size(), 1) * 4);
-  const size_t total = o_sbox + 2 * up(std::max<size_t>(start_mods.size(), 1) * 16);
+  // rows of start modules (same box up to phic)
+  std::vector<uint32_t> prow_off, prow_k;
+  std::vector<float> prow_phic, prow_b;   // prow_b: 8 floats per row
+  {
+    std::vector<uint32_t> order(start_mods.size());
+    for (size_t k = 0; k < order.size(); ++k) order[k] = (uint32_t)k;
+    auto key_less = [&](uint32_t ka, uint32_t kb) {
+      const uint32_t a = start_mods[ka], b = start_mods[kb];
+      if (g->category[a] != g->category[b]) return g->category[a] < g->category[b];
+      if (g->rmin[a] != g->rmin[b]) return g->rmin[a] < g->rmin[b];
+      if (g->rmax[a] != g->rmax[b]) return g->rmax[a] < g->rmax[b];
+      if (g->zmin[a] != g->zmin[b]) return g->zmin[a] < g->zmin[b];
+      if (g->zmax[a] != g->zmax[b]) return g->zmax[a] < g->zmax[b];
+      if (g->half_phi[a] != g->half_phi[b]) return g->half_phi[a] < g->half_phi[b];
+      return false;
+    };
+    std::stable_sort(order.begin(), order.end(), key_less);
+    for (size_t i = 0; i < order.size(); ++i) {
+      if (i == 0 || key_less(order[i - 1], order[i])) {
+        const uint32_t m = start_mods[order[i]];
+        prow_off.push_back((uint32_t)i);
+        const float b8[8] = {g->half_phi[m], g->rmin[m], g->rmax[m], (float)g->category[m], g->zmin[m], g->zmax[m],
+                             c->k.par.f_sig_t[g->category[m] & 3] / g->rmin[m], 0.0f};
+        prow_b.insert(prow_b.end(), b8, b8 + 8);
+      }
+      prow_k.push_back(order[i]);
+      prow_phic.push_back(g->phic[start_mods[order[i]]]);
+    }
+    prow_off.push_back((uint32_t)order.size());
+  }
+  const size_t n_prow = prow_off.size() - 1;
+  const size_t o_prow = o_sbox + 2 * up(std::max<size_t>(start_mods.size(), 1) * 16);
+  const size_t o_prow2 = o_prow + up(std::max<size_t>(n_prow, 1) * 16);
+  const size_t o_poff = o_prow2 + up(std::max<size_t>(n_prow, 1) * 16);
+  const size_t o_pk = o_poff + up((n_prow + 1) * 4);
+  const size_t o_pphi = o_pk + up(std::max<size_t>(prow_k.size(), 1) * 4);
+  const size_t total = o_pphi + up(std::max<size_t>(prow_phic.size(), 1) * 4);
   e = cudaMalloc(&c->d_static, total);
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaMalloc(static)"); }
   char *d = (char *)c->d_static;
@@ -431,6 +467,20 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
     cudaMemcpy(d + o_sbox + up(nb), b2, nb, cudaMemcpyHostToDevice);
     c->k.geo.start_box = (const float4 *)(d + o_sbox);
     c->k.geo.start_box2 = (const float4 *)(d + o_sbox + up(nb));
+    std::vector<float> r1(4 * std::max<size_t>(n_prow, 1), 0.0f), r2(4 * std::max<size_t>(n_prow, 1), 0.0f);
+    for (size_t r = 0; r < n_prow; ++r)
+      for (int q = 0; q < 4; ++q) { r1[4 * r + q] = prow_b[8 * r + q]; r2[4 * r + q] = prow_b[8 * r + 4 + q]; }
+    cudaMemcpy(d + o_prow, r1.data(), r1.size() * 4, cudaMemcpyHostToDevice);
+    cudaMemcpy(d + o_prow2, r2.data(), r2.size() * 4, cudaMemcpyHostToDevice);
+    cudaMemcpy(d + o_poff, prow_off.data(), prow_off.size() * 4, cudaMemcpyHostToDevice);
+    if (!prow_k.empty()) {
+      cudaMemcpy(d + o_pk, prow_k.data(), prow_k.size() * 4, cudaMemcpyHostToDevice);
+      cudaMemcpy(d + o_pphi, prow_phic.data(), prow_phic.size() * 4, cudaMemcpyHostToDevice);
+    }
+    c->k.geo.prow_b1 = (const float4 *)(d + o_prow); c->k.geo.prow_b2 = (const float4 *)(d + o_prow2);
+    c->k.geo.prow_off = (const uint32_t *)(d + o_poff); c->k.geo.prow_k = (const uint32_t *)(d + o_pk);
+    c->k.geo.prow_phic = (const float *)(d + o_pphi);
+    c->k.geo.n_prow = (uint32_t)n_prow;
   }
   e = cudaDeviceSynchronize();
   if (e != cudaSuccess) { cudaFree(c->d_static); delete c; return cuda_fail(e, "upload geometry"); }

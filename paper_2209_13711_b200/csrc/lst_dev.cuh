@@ -114,6 +114,14 @@ struct GeoDev {
   // the same modules' boxes packed for k_px_modules: {phic, hphi, rmin, rmax}, {zmin, zmax, category, sig_t / rmin}
   const float4 *start_box, *start_box2;
   uint32_t n_start;
+  // start modules grouped into "rows": modules that differ only in phic (same category, r, z and
+  // half_phi box, e.g. one z-row of a barrel layer or one ring of a disk).  prow_b1 = {hphi, rmin,
+  // rmax, category}, prow_b2 = {zmin, zmax, sig_t / rmin, 0}; members prow_off[r] .. prow_off[r+1]:
+  // prow_k = index into start_mods, prow_phic = its phic.
+  const float4 *prow_b1, *prow_b2;
+  const uint32_t *prow_off, *prow_k;
+  const float *prow_phic;
+  uint32_t n_prow;
 };
 
 // All per-slot arrays (device pointers into the caller's workspace).
