@@ -216,8 +216,8 @@ __global__ void k_dd_scatter(SlotDev s) {
 
 // ------------------------------------------------------------------ S0: inside one collection
 // One WARP per object A.  An object sharing >= min_shared of A's n_ot hits contains at least one of
-// any n_ot - min_shared + 1 of them, so only the incidence lists (of A's own type) of hits
-// k0..n_ot-1 are searched; the lists are flattened into one index space that the lanes stride
+// any n_ot - min_shared + 1 of them, so only the n_ot - min_shared + 1 shortest incidence lists (of
+// A's own type) are searched; the lists are flattened into one index space that the lanes stride
 // (their lengths are very uneven: inner-layer hits sit in hundreds of objects).  Per entry B the
 // cheap test comes first (score(B) <= score(A)); the shared-hit count is exact and costs one
 // shared-memory lookup per hit of B: A's hits sit in a 256-slot table per warp (slot = hit & 255;
@@ -250,18 +250,25 @@ __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
       const bool collide = __any_sync(0xffffffffu, lane < A.n_ot && __popc(same) > 1);
       if (lane < A.n_ot) tab[slot] = my_hit;
       {
+        // the nl SHORTEST of A's n_ot incidence lists are searched (any nl of them will do)
         uint32_t len = 0, b0 = 0;
-        if (lane >= k0 && lane < A.n_ot) {
+        if (lane < A.n_ot) {
           const uint32_t row = 3 * my_hit + (uint32_t)A.type;
           b0 = s.inc_off[row]; len = s.inc_off[row + 1] - b0;
         }
-        // lists in lanes k0 .. n_ot-1: shift them down to lanes 0 .. nl-1
-        len = __shfl_down_sync(0xffffffffu, len, k0);
-        b0 = __shfl_down_sync(0xffffffffu, b0, k0);
-        if (lane >= nl) len = 0;
+        int rank = 0;
+#pragma unroll
+        for (int j = 0; j < 10; ++j) {
+          const uint32_t lj = __shfl_sync(0xffffffffu, len, j);
+          rank += (int)(j < A.n_ot && (lj < len || (lj == len && j < lane)));
+        }
+        if (lane < A.n_ot && rank < nl) { beg[rank] = b0; pre[rank] = len; }
+        __syncwarp();
+        const uint32_t l2 = lane < nl ? pre[lane] : 0u;
         uint32_t tot;
-        const uint32_t ex = warp_excl_scan(len, &tot);
-        if (lane < 11) { pre[lane] = ex; beg[lane] = b0; }      // lanes >= nl: pre = total
+        const uint32_t ex = warp_excl_scan(l2, &tot);
+        __syncwarp();
+        if (lane < 11) pre[lane] = ex;                          // lanes >= nl: pre = total
         __syncwarp();
       }
       const uint32_t total = pre[nl < 10 ? nl : 10];

@@ -23,6 +23,14 @@ namespace lst {
 constexpr double kGuard = 1e-9;       // denominators must exceed this (C0)
 constexpr float kPreSlack = 1.001f;   // fp32 pre-filter loosening
 
+// Division inside the fp32 pre-filters: the 2-ulp approximate divide on the device (the pre-filters
+// are loosened by 1e-3 relative, 4 orders of magnitude more), the plain one on the host.
+#ifdef __CUDA_ARCH__
+#define LST_FDIV(a, b) __fdividef((a), (b))
+#else
+#define LST_FDIV(a, b) ((a) / (b))
+#endif
+
 // Selection parameters in the form the kernels use (built once by lst_create from lst_config).
 struct Params {
   double kmax;          // kB / (2 pt_min)
@@ -216,7 +224,7 @@ LST_HD bool ls_pre_f(const Params &g, float xi, float yi, float zi, float ri, fl
   const float dx = xo - xi, dy = yo - yi, dz = zo - zi;
   const float dd = dx * dx + dy * dy;
   const float dotAD = xi * dx + yi * dy;
-  const float drv = (2.0f * dotAD + dd) / (ri + ro);
+  const float drv = LST_FDIV(2.0f * dotAD + dd, ri + ro);
   const float ns = g.f_ns;
   // L1
   const float N = ri * dz - zi * drv;
@@ -226,8 +234,8 @@ LST_HD bool ls_pre_f(const Params &g, float xi, float yi, float zi, float ri, fl
   const float dotAB = ri * ri + dotAD;
   if (dotAB < -1e-3f * rr) return false;
   const float cr = xi * dy - yi * dx;
-  const float sd = cr / rr;
-  const float tphi = g.f_sig_t[ci] / ri + g.f_sig_t[co] / ro;
+  const float sd = LST_FDIV(cr, rr);
+  const float tphi = LST_FDIV(g.f_sig_t[ci], ri) + LST_FDIV(g.f_sig_t[co], ro);
   const float eci = is_endcap(ci) ? g.f_ec_md_sys : 0.0f, eco = is_endcap(co) ? g.f_ec_md_sys : 0.0f;
   if (!is_endcap(co)) {
     const float cxy = sqrtf(dd);
@@ -242,13 +250,13 @@ LST_HD bool ls_pre_f(const Params &g, float xi, float yi, float zi, float ri, fl
     const float den = zbar - g.f_z0max - 0.5f * ns * g.f_sig_z[ci];
     if (den < 1e-3f || adz < 1e-6f) return true;   // guards are decided in fp64
     const float srs = g.f_sig_r[ci] + g.f_sig_r[co];
-    const float Sbar = asinf(fminf(1.0f, g.f_kmax * (rbar + 0.5f * ns * srs))) / g.f_kmax;
+    const float Sbar = LST_FDIV(asinf(fminf(1.0f, g.f_kmax * (rbar + 0.5f * ns * srs))), g.f_kmax);
     const float dph = atan2f(cr, dotAB);
-    if (fabsf(dph) > (g.f_kmax * (adz + ns * g.f_sig_z[ci]) * Sbar / den + ns * tphi) * kPreSlack) return false;
-    const float lever = zbar / (adz * rbar);
+    if (fabsf(dph) > (LST_FDIV(g.f_kmax * (adz + ns * g.f_sig_z[ci]) * Sbar, den) + ns * tphi) * kPreSlack) return false;
+    const float lever = LST_FDIV(zbar, adz * rbar);
     const float kls = dph * lever, akls = fabsf(kls);
     const float sigkls = tphi * lever;
-    const float slack = akls * (g.f_z0max / zbar + g.f_modez_slack + ns * srs / (ri + ro) + ns * g.f_sig_z[ci] / adz);
+    const float slack = akls * (LST_FDIV(g.f_z0max, zbar) + g.f_modez_slack + LST_FDIV(ns * srs, ri + ro) + LST_FDIV(ns * g.f_sig_z[ci], adz));
     if (fabsf(ki - kls) > (ns * (ski + sigkls) + slack + eci * akls) * kPreSlack) return false;
     if (fabsf(ko - kls) > (ns * (sko + sigkls) + slack + eco * akls) * kPreSlack) return false;
   }
@@ -353,7 +361,7 @@ LST_HD bool t3_pre_f(const Params &g, float x1, float y1, float z1, float r1, in
   const float sp3 = g.f_sig_t[c3] + g.f_sig_r[c3] * fminf(1.0f, g.f_kmax * r3);
   const float abc = a * b * c13;
   if (fabsf(crs) > (g.f_kmax * abc + g.f_ns * (sp2 * c13 + b * sp1 + a * sp3)) * kPreSlack) return false;   // T3-1
-  const float k3 = crs / abc;
+  const float k3 = LST_FDIV(crs, abc);
   const float q1 = k3 * r1, q2 = k3 * r2, q3 = k3 * r3;
   const float s21 = (r2 - r1) + (r2 * q2 * q2 - r1 * q1 * q1) * (1.0f / 6.0f);
   const float s31 = (r3 - r1) + (r3 * q3 * q3 - r1 * q1 * q1) * (1.0f / 6.0f);
@@ -373,13 +381,13 @@ LST_HD bool t3_pre_f(const Params &g, float x1, float y1, float z1, float r1, in
     L1 = z1; L2 = z2; L3 = z3;
     sl1 = g.f_sig_z[c1]; sl2 = g.f_sig_z[c2]; sl3 = g.f_sig_z[c3];
   } else {
-    const float k13 = sinf(d13) / c13;
+    const float k13 = LST_FDIV(sinf(d13), c13);
     const float u1 = k13 * r1, u2 = k13 * r2, u3 = k13 * r3;
-    L1 = fabsf(u1) <= 1e-4f ? r1 : asinf(fminf(1.0f, fmaxf(-1.0f, u1))) / k13;
-    L2 = fabsf(u2) <= 1e-4f ? r2 : asinf(fminf(1.0f, fmaxf(-1.0f, u2))) / k13;
-    L3 = fabsf(u3) <= 1e-4f ? r3 : asinf(fminf(1.0f, fmaxf(-1.0f, u3))) / k13;
+    L1 = fabsf(u1) <= 1e-4f ? r1 : LST_FDIV(asinf(fminf(1.0f, fmaxf(-1.0f, u1))), k13);
+    L2 = fabsf(u2) <= 1e-4f ? r2 : LST_FDIV(asinf(fminf(1.0f, fmaxf(-1.0f, u2))), k13);
+    L3 = fabsf(u3) <= 1e-4f ? r3 : LST_FDIV(asinf(fminf(1.0f, fmaxf(-1.0f, u3))), k13);
   }
-  const float i1 = 1.0f / r1, i2 = 1.0f / r2, i3 = 1.0f / r3;
+  const float i1 = LST_FDIV(1.0f, r1), i2 = LST_FDIV(1.0f, r2), i3 = LST_FDIV(1.0f, r3);
   const float L32 = L3 - L2, L21 = L2 - L1, L31 = L3 - L1;
   const float Nphi = d12 * L32 - d23 * L21;
   const float Nrho = (i2 - i1) * L32 - (i3 - i2) * L21;
