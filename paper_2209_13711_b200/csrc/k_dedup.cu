@@ -37,9 +37,14 @@ __device__ __forceinline__ DRef dd_ref(const SlotDev &s, uint32_t n5, uint32_t n
 __device__ __forceinline__ int dd_type(uint32_t n5, uint32_t np5, uint32_t d) { return d < n5 ? 0 : (d < n5 + np5 ? 1 : 2); }
 
 // "b beats a": (score, hit coordinates in layer order, pLS index, original hit indices), reading 15.
-__device__ bool dd_beats(const SlotDev &s, const DRef &b, const DRef &a) {
+// the tie-break of equal scores (rare: kept out of line so that its loads are not speculated)
+__device__ __noinline__ bool dd_beats_tie(const SlotDev &s, const DRef &b, const DRef &a);
+__device__ __forceinline__ bool dd_beats(const SlotDev &s, const DRef &b, const DRef &a) {
   if (b.score < a.score) return true;
   if (b.score > a.score) return false;
+  return dd_beats_tie(s, b, a);
+}
+__device__ __noinline__ bool dd_beats_tie(const SlotDev &s, const DRef &b, const DRef &a) {
   const int n = a.n_ot < b.n_ot ? a.n_ot : b.n_ot;
   for (int k = 0; k < n; ++k) {
     const float4 pb = s.hit[b.hits[k]], pa = s.hit[a.hits[k]];
@@ -256,12 +261,11 @@ __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
           const uint32_t row = 3 * my_hit + (uint32_t)A.type;
           b0 = s.inc_off[row]; len = s.inc_off[row + 1] - b0;
         }
+        // rank of this lane's list by (length, lane): keys are unique, lanes >= n_ot sort last
+        const uint32_t mykey = lane < A.n_ot ? ((len < (1u << 27) ? len : (1u << 27) - 1u) << 4) | (uint32_t)lane : 0xFFFFFFFFu;
         int rank = 0;
 #pragma unroll
-        for (int j = 0; j < 10; ++j) {
-          const uint32_t lj = __shfl_sync(0xffffffffu, len, j);
-          rank += (int)(j < A.n_ot && (lj < len || (lj == len && j < lane)));
-        }
+        for (int j = 0; j < 10; ++j) rank += (int)(__shfl_sync(0xffffffffu, mykey, j) < mykey);
         if (lane < A.n_ot && rank < nl) { beg[rank] = b0; pre[rank] = len; }
         __syncwarp();
         const uint32_t l2 = lane < nl ? pre[lane] : 0u;

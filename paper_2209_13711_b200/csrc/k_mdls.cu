@@ -5,61 +5,71 @@
 namespace lst {
 
 // =================================================================== MD
-// Work item = (module, rows of lower hits, columns of upper hits).  Both sensors' hits are staged in
-// shared memory; every (lower, upper) pair goes through the fp32 pre-filter, survivors are compacted
-// and decided in fp64.
-__global__ void __launch_bounds__(kThreads) k_md_eval(GeoDev geo, SlotDev s, Params g) {
-  __shared__ ItemScratch sc;
-  __shared__ float4 pool[kItemCand + 8];
+// Work item = (module, rows of lower hits, columns of upper hits), <= 1024 pairs (typically ~100).
+// k_md_eval: one WARP per item, no staging and no barriers: every (lower, upper) pair goes through
+// the fp32 pre-filter, the survivors are appended to the stage's candidate list.
+// k_md_decide: one thread per listed pair, fp64 decision; accepted pairs set their pass bit and
+// write kappa, sigma_kappa and dphi to the pool.
+__global__ void __launch_bounds__(256) k_md_eval(GeoDev geo, SlotDev s, Params g) {
+  __shared__ ClStage cl_mem[256 / 32];
   const StageBuf &st = s.st[S_MD];
   const uint32_t n_items = s.hdr->n_items[S_MD];
-  const int tid = threadIdx.x;
-  for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+  ClBuf cl;
+  cl.init(&cl_mem[threadIdx.x >> 5]);
+  constexpr int kSlices = 8, kSliceCand = kItemCand / kSlices;   // a warp task = 128 candidates of an item
+  for (uint32_t w = warp; w < n_items * kSlices; w += nwarp) {
+    const uint32_t it = w / kSlices, sl = w % kSlices;
     const Item item = st.items[it];
+    const int nj = item.nj, nc = item.nrows * nj;
+    if (sl == 0) st.mask[(size_t)it * kItemWords + lane] = 0;  // the decide kernel ORs the pass bits in
+    if ((int)(sl * kSliceCand) >= nc) continue;
     const uint32_t m = item.group;
     const int cat = geo.category[m];
     const uint32_t lo0 = s.det_off[2 * m] + item.i0, up0 = s.det_off[2 * m + 1] + item.j0;
-    const int nr = item.nrows, nj = item.nj;
-    for (int k = tid; k < nr + nj; k += kThreads) pool[k] = k < nr ? s.hit[lo0 + k] : s.hit[up0 + (k - nr)];
-    if (tid < kItemWords) sc.mask[tid] = 0;
-    if (tid == 0) sc.n = 0;
-    __syncthreads();
-    const int nc = nr * nj;
-    for (int base = 0; base < nc; base += kThreads) {
-      const int c = base + tid;
+    const uint32_t inv = (1u << 20) / (uint32_t)nj + 1u;      // c / nj == (c * inv) >> 20 for c * nj < 2^20
+    const int c_end = min(nc, (int)((sl + 1) * kSliceCand));
+    for (int base = (int)(sl * kSliceCand); base < c_end; base += 32) {
+      const int c = base + lane;
       bool keep = false;
-      if (c < nc) {
-        const int r = c / nj, jj = c - r * nj;
-        const float4 l = pool[r], u = pool[nr + jj];
+      uint32_t hl = 0, hu = 0;
+      if (c < c_end) {
+        const int r = (int)(((uint32_t)c * inv) >> 20), jj = c - r * nj;
+        hl = lo0 + r; hu = up0 + jj;
+        const float4 l = s.hit[hl], u = s.hit[hu];
         keep = md_pre_f(g, l.x, l.y, l.z, l.w, u.x, u.y, u.z, u.w, cat);
       }
-      push_survivor(sc, keep, (uint32_t)c);
+      cl.push(s.hdr, st, S_MD, keep, it * (uint32_t)kItemCand + (uint32_t)c, make_uint2(hl, hu));
     }
-    __syncthreads();
-    const int nsv = (int)sc.n;
-    for (int base = 0; base < nsv; base += kThreads) {     // fp64 decision; results go to the pool
-      const int k = base + tid;
-      bool pass = false;
-      int c = 0;
-      MdOut o;
-      if (k < nsv) {
-        c = sc.list[k];
-        const int r = c / nj, jj = c - r * nj;
-        const float4 l = pool[r], u = pool[nr + jj];
-        const Pt pl = make_pt(l.x, l.y, l.z, cat), pu = make_pt(u.x, u.y, u.z, cat);
-        pass = md_eval_d(g, pl, pu, cat, &o);
-      }
-      const uint32_t pos = pool_reserve(s.hdr, st, S_MD, pass);
-      if (pass) atomicOr(&sc.mask[c >> 5], 1u << (c & 31));
-      if (pos != 0xFFFFFFFFu) {
-        st.pkey[pos] = it * (uint32_t)kItemCand + (uint32_t)c;
-        st.p_d2[pos] = make_double2(o.kappa, o.sigk);
-        st.p_f4[pos] = make_float4((float)o.dphi, 0.f, 0.f, 0.f);
-      }
+  }
+  cl.flush_all(s.hdr, st, S_MD);
+}
+
+__global__ void __launch_bounds__(128) k_md_decide(GeoDev geo, SlotDev s, Params g) {
+  const StageBuf &st = s.st[S_MD];
+  Header *hdr = s.hdr;
+  const uint32_t n = min(hdr->cl_used[S_MD], st.cap_cl);
+  const uint32_t nround = (n + 31u) & ~31u;
+  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < nround; j += gridDim.x * blockDim.x) {
+    bool pass = false;
+    MdOut o;
+    uint32_t key = 0;
+    if (j < n) {
+      key = st.cl_key[j];
+      const uint2 ab = st.cl_ab[j];
+      const int cat = geo.category[st.items[key / kItemCand].group];
+      const float4 l = s.hit[ab.x], u = s.hit[ab.y];
+      const Pt pl = make_pt(l.x, l.y, l.z, cat), pu = make_pt(u.x, u.y, u.z, cat);
+      pass = md_eval_d(g, pl, pu, cat, &o);
     }
-    __syncthreads();
-    publish_mask(sc, st, it);
-    __syncthreads();
+    const uint32_t pos = pool_reserve(hdr, st, S_MD, pass);
+    if (pass) atomicOr(&st.mask[(size_t)(key / kItemCand) * kItemWords + ((key % kItemCand) >> 5)], 1u << (key & 31u));
+    if (pos != 0xFFFFFFFFu) {
+      st.pkey[pos] = key;
+      st.p_d2[pos] = make_double2(o.kappa, o.sigk);
+      st.p_f4[pos] = make_float4((float)o.dphi, 0.f, 0.f, 0.f);
+    }
   }
 }
 
@@ -162,13 +172,14 @@ struct LsShared {
   float4 r_pos[kUnitRows];
   uint32_t r_idc[kUnitRows];
   uint32_t q1[kThreads / 32][64];
+  ClStage cl[kThreads / 32];
   float4 tab[4];                      // per category: sig_z, sig_r, sig_t
 };
 
 // Tier 2 on up to 32 queued tier-1 survivors; what passes goes to the stage's candidate list.
 // it0: item of the unit's first row chunk; consecutive row chunks are nct items apart.
 __device__ __forceinline__ void ls_stage2(const LsShared &sh, const SlotDev &s, const Params &g, WarpQueue &Q1,
-                                          uint32_t rpi, int nj, uint32_t it0, uint32_t nct) {
+                                          ClBuf &cl, uint32_t rpi, int nj, uint32_t it0, uint32_t nct) {
   uint32_t e = 0, mi = 0, mo = 0, key = 0;
   bool keep = false;
   if (Q1.pop(&e)) {
@@ -181,7 +192,7 @@ __device__ __forceinline__ void ls_stage2(const LsShared &sh, const SlotDev &s, 
     const uint32_t q = r / rpi, c = (r - q * rpi) * (uint32_t)nj + jj;
     key = (it0 + q * nct) * (uint32_t)kItemCand + c;
   }
-  cl_append(s.hdr, s.st[S_LS], S_LS, keep, key, make_uint2(mi, mo));
+  cl.push(s.hdr, s.st[S_LS], S_LS, keep, key, make_uint2(mi, mo));
 }
 
 __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, Params g) {
@@ -193,6 +204,8 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
   if (tid < 4) sh.tab[tid] = make_float4(g.f_sig_z[tid], g.f_sig_r[tid], g.f_sig_t[tid], 0.0f);
   WarpQueue Q1;
   Q1.init(sh.q1[wib]);
+  ClBuf cl;
+  cl.init(&sh.cl[wib]);
   __shared__ uint32_t sh_unit[2];
   for (;;) {
     __syncthreads();                            // the previous unit is done with the shared arrays
@@ -240,17 +253,26 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
       const float4 b = sh.c_pos[has ? jj : 0];
       const uint32_t cb = sh.c_idc[has ? jj : 0] >> 30;
       const float4 tb = sh.tab[cb];
-      for (int r = rg; r < nrows; r += nrg) {
-        const float4 a = sh.r_pos[r];
-        const float4 ta = sh.tab[sh.r_idc[r] >> 30];
-        const bool keep = has && ls_tier1_f(g, a.x, a.y, a.z, a.w, ta.x, ta.y, ta.z, b.x, b.y, b.z, b.w, tb.x, tb.y, tb.z,
-                                            cb >= 2u);
-        Q1.push(keep, (uint32_t)r | ((uint32_t)jj << 8));
-        if (Q1.n >= 32u) ls_stage2(sh, s, g, Q1, rpi, nj, it0, nct);
+      // the 32 columns of a chunk nearly always share their mode (same or neighbouring modules):
+      // a warp-uniform mode lets the compiler drop the other mode's arithmetic from the loop
+      const bool all_z = __all_sync(0xffffffffu, !has || cb >= 2u), all_r = __all_sync(0xffffffffu, !has || cb < 2u);
+#define LST_LS_ROWS(OEC)                                                                                             \
+      for (int r = rg; r < nrows; r += nrg) {                                                                        \
+        const float4 a = sh.r_pos[r];                                                                                \
+        const float4 ta = sh.tab[sh.r_idc[r] >> 30];                                                                 \
+        const bool keep = has && ls_tier1_f(g, a.x, a.y, a.z, a.w, ta.x, ta.y, ta.z, b.x, b.y, b.z, b.w, tb.x, tb.y, \
+                                            tb.z, (OEC));                                                            \
+        Q1.push(keep, (uint32_t)r | ((uint32_t)jj << 8));                                                            \
+        if (Q1.n >= 32u) ls_stage2(sh, s, g, Q1, cl, rpi, nj, it0, nct);                                                 \
       }
+      if (all_r) { LST_LS_ROWS(false) }
+      else if (all_z) { LST_LS_ROWS(true) }
+      else { LST_LS_ROWS(cb >= 2u) }
+#undef LST_LS_ROWS
     }
-    while (Q1.n) ls_stage2(sh, s, g, Q1, rpi, nj, it0, nct);
+    while (Q1.n) ls_stage2(sh, s, g, Q1, cl, rpi, nj, it0, nct);
   }
+  cl.flush_all(s.hdr, st, S_LS);
 }
 
 // fp64 decision of the listed candidates, one thread each (dense warps, no staging); an accepted
@@ -301,7 +323,9 @@ static inline int persistent_grid(const Ctx &c, int per_sm) { return c.n_sm * pe
 
 void launch_md(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   launch_emit(c, s, S_MD, -1, st);
-  k_md_eval<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_md_eval");
+  k_md_eval<<<persistent_grid(c, 8), 256, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_md_eval");
+  k_md_decide<<<persistent_grid(c, 4), 128, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_md_decide");
+  launch_item_counts(c, s, S_MD, st);
   launch_scan_items(c, s, S_MD, 0, s.cap_md, st);
   k_md_fill<<<persistent_grid(c, 4), 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_md_fill");
   launch_row_offsets(c, s, 0, st);

@@ -247,7 +247,10 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
   __shared__ RowTab rt;
   __shared__ uint32_t sh[33];
   __shared__ float4 rowseed[(KIND == J_PT5 || KIND == J_PT3) ? kRowChunk : 1];
+  __shared__ ClStage cl_mem[kThreads / 32];
   (void)geo;
+  ClBuf cl;
+  cl.init(&cl_mem[threadIdx.x >> 5]);
   const int stage = JoinTraits<KIND>::stage;
   const StageBuf &st = s.st[stage];
   const uint32_t n_items = s.hdr->n_items[stage];
@@ -271,10 +274,11 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
         item_to_pair(rt, item.j0, c, &row, &b);
         keep = join_phase1<KIND>(s, g, r0 + row, b, rowseed, row, &ab);
       }
-      cl_append(s.hdr, st, stage, keep, key0 + (uint32_t)c, ab);
+      cl.push(s.hdr, st, stage, keep, key0 + (uint32_t)c, ab);
     }
     __syncthreads();
   }
+  cl.flush_all(s.hdr, st, stage);
 }
 
 // Decide kernel: the fp64 decision of the listed candidates, one thread each (dense warps, no

@@ -21,7 +21,7 @@ namespace lst {
 constexpr int kItemCand = 1024;          // candidates per work item
 constexpr int kItemWords = kItemCand / 32;
 constexpr int kThreads = 128;            // threads per block of eval / fill kernels
-constexpr int kUnitItems = 8;            // max items per work unit (same group, same column tile, consecutive rows)
+constexpr int kUnitItems = 16;           // max items per work unit (same group, same column tile, consecutive rows)
 constexpr int kMaxRpi = 256;             // max rows per item
 constexpr int kUnitRows = 256;           // max rows per work unit
 constexpr int kRowChunk = 128;           // rows per group in the variable-width stages (T3, T5, pixel)
@@ -248,6 +248,7 @@ struct WarpQueue {
   // all 32 lanes must call; at most 32 entries are added, the caller keeps n <= 32 before a push
   __device__ __forceinline__ void push(bool keep, uint32_t v) {
     const uint32_t b = __ballot_sync(0xffffffffu, keep);
+    if (b == 0) return;
     const int lane = threadIdx.x & 31;
     if (keep) q[(head + n + __popc(b & ((1u << lane) - 1u))) & 63u] = v;
     n += __popc(b);
@@ -359,6 +360,50 @@ __device__ __forceinline__ void cl_append(Header *hdr, const StageBuf &st, int s
   st.cl_key[pos] = key;
   st.cl_ab[pos] = ab;
 }
+
+// Warp-private staging of candidate-list entries (ring of 64 in shared memory): the sparse
+// survivors of many pre-filter iterations are appended 32 at a time, i.e. one atomic on the list
+// counter per 32 entries (the counter is a single address: per-iteration atomics serialise in L2).
+struct ClStage {
+  uint32_t key[64];
+  uint2 ab[64];
+};
+struct ClBuf {
+  ClStage *m;
+  uint32_t head, n;
+  __device__ __forceinline__ void init(ClStage *mem) { m = mem; head = 0; n = 0; }
+  // all 32 lanes call; flushes a full batch when one is ready
+  __device__ __forceinline__ void push(Header *hdr, const StageBuf &st, int stage, bool keep, uint32_t key, uint2 ab) {
+    const uint32_t b = __ballot_sync(0xffffffffu, keep);
+    if (b == 0) return;
+    const int lane = threadIdx.x & 31;
+    if (keep) {
+      const uint32_t p = (head + n + __popc(b & ((1u << lane) - 1u))) & 63u;
+      m->key[p] = key; m->ab[p] = ab;
+    }
+    n += __popc(b);
+    __syncwarp();
+    if (n >= 32u) flush32(hdr, st, stage);
+  }
+  __device__ __forceinline__ void flush32(Header *hdr, const StageBuf &st, int stage) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t take = n < 32u ? n : 32u;
+    uint32_t base = 0;
+    if (lane == 0) base = atomicAdd(&hdr->cl_used[stage], take);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if ((uint32_t)lane < take) {
+      const uint32_t p = (head + lane) & 63u, pos = base + lane;
+      if (pos < st.cap_cl) { st.cl_key[pos] = m->key[p]; st.cl_ab[pos] = m->ab[p]; }
+      else atomicOr(&hdr->err, (uint32_t)ERR_CAP_ITEMS);
+    }
+    __syncwarp();
+    head = (head + take) & 63u;
+    n -= take;
+  }
+  __device__ __forceinline__ void flush_all(Header *hdr, const StageBuf &st, int stage) {
+    while (n) flush32(hdr, st, stage);
+  }
+};
 
 // fill: canonical index of pool entry `key` = item * kItemCand + candidate
 __device__ __forceinline__ uint32_t pool_target(const StageBuf &st, uint32_t key, uint32_t *item, uint32_t *cand) {

@@ -270,28 +270,27 @@ LST_HD bool ls_pre_f(const Params &g, float xi, float yi, float zi, float ri, fl
 // of the inner (i) / outer (o) MD's module category; oec: outer module is an endcap module.
 LST_HD bool ls_tier1_f(const Params &g, float xi, float yi, float zi, float ri, float szi, float sri, float sti,
                        float xo, float yo, float zo, float ro, float szo, float sro, float sto, bool oec) {
-  const float dx = xo - xi, dy = yo - yi, dz = zo - zi;
-  const float dd = dx * dx + dy * dy;
-  const float dotAD = xi * dx + yi * dy;
-  const float P = 2.0f * dotAD + dd;          // drv * (ri + ro)
-  const float S = ri + ro;
+  // L1: rt_i dz - z_i drv with drv = rt_o - rt_i is the r-z cross product rt_i z_o - z_i rt_o
+  // (the fp32 error of the stored radii, ~1e-5 cm, is 1e-5 of the threshold z0max |drv| >= ~100 cm^2)
   const float ns = g.f_ns;
   const float azi = fabsf(zi), azo = fabsf(zo);
   const float E = ri * szo + ro * szi + azo * sri + azi * sro;
-  bool keep = !(fabsf(ri * dz * S - zi * P) > (g.f_z0max * fabsf(P) + ns * E * S) * kPreSlack);     // L1
+  bool keep = !(fabsf(ri * zo - zi * ro) > (g.f_z0max * fabsf(ro - ri) + ns * E) * kPreSlack);              // L1
   const float rr = ri * ro;
-  keep &= !(ri * ri + dotAD < -1e-3f * rr);
-  const float acr = fabsf(xi * dy - yi * dx);
+  keep &= !(xi * xo + yi * yo < -1e-3f * rr);
+  const float acr = fabsf(xi * yo - yi * xo);   // |cross(A, D)| = |cross(A, B)|
   const float T = ns * (sti * ro + sto * ri);   // tolphi * rr
   if (!oec) {
+    const float dx = xo - xi, dy = yo - yi;
+    const float dd = dx * dx + dy * dy;
     const float e = acr - T * kPreSlack;
     const float kk = g.f_kmax * kPreSlack;
     keep &= !(e > 0.0f && e * e > kk * kk * dd * rr * rr);                                           // L2, mode R
   } else {
-    const float x = fminf(1.0f, g.f_kmax * (0.5f * S + 0.5f * ns * (sri + sro)));
+    const float x = fminf(1.0f, g.f_kmax * (0.5f * (ri + ro) + 0.5f * ns * (sri + sro)));
     const float ub = x + 0.5708f * x * x * x;
     const float den = 0.5f * (azi + azo) - g.f_z0max - 0.5f * ns * szi;
-    if (den >= 1e-3f) keep &= !(acr * den > ((fabsf(dz) + ns * szi) * ub * rr + T * den) * kPreSlack);   // L2, mode Z
+    if (den >= 1e-3f) keep &= !(acr * den > ((fabsf(zo - zi) + ns * szi) * ub * rr + T * den) * kPreSlack);   // L2, mode Z
   }
   return keep;
 }
