@@ -68,6 +68,26 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def alu_peak_gops():
+    """fp32 lane-operations per second of the plain ALUs: SMs x 128 FP32 lanes x max SM clock (DESIGN.md 7;
+    unit counts from B200_PROFILING.md / blackwell guide: 4 sub-partitions x 32 lanes per SM)."""
+    import torch
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    mhz, src = 1965.0, "nominal 1965 MHz"
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            mhz, src = float(json.load(open(p))["sm_max_mhz"]), "MEASURED_PEAKS.json sm_max_mhz"
+        except Exception:
+            pass
+    return n_sm * 128 * mhz * 1e6 / 1e9, "%d SMs x 128 fp32 lanes x %.0f MHz (%s), FMA = 1 op" % (n_sm, mhz, src)
+
+
+# DRAM bytes (read + write) of one launch of the dominant kernel from the ncu --set full capture
+# summarised in profiles/ (the file is named in the roofline object); None for other kernels.
+NCU_TRAFFIC = {"k_ls_eval": (None, None)}
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md)."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -138,23 +158,46 @@ def algorithmic_bytes(name, n):
         "k_det_scan": 4 * 2 * nmod * 3 + 8 * nmod,
         "k_scatter": 4 * n["hits"] * 2 + 4 * 2 * nmod,
         "k_rank": (B_HIT_IN + B_HIT + 4) * n["hits"],
-        "k_md_eval": 16 * n["hits"] + bits(0),
-        "k_md_fill": bits(0) + (2 * 16 + B_MD) * n["md"],
+        # pre-filter kernels read their operands once and append (key, pair) = 12 B per survivor;
+        # decide kernels read the list and the operands of the survivors, write pool entries;
+        # fill kernels move pool entries (payload) to the canonical arrays
+        "k_md_eval": 16 * n["hits"] + 12 * n["surv"][0],
+        "k_md_decide": (12 + 32) * n["surv"][0] + bits(0) + 36 * n["md"],
+        "k_md_fill": 36 * n["md"] + bits(0) + B_MD * n["md"],
         "k_ls_groups": 4 * (nnz + 3 * nmod),
-        "k_ls_eval": B_MD_PRE * n["md"] + 4 * (nnz + 2 * nmod) + bits(1),
-        "k_ls_fill": bits(1) + B_LS * n["ls"] + (16 + 16 + 4) * n["md"],
-        "k_join_eval[T3]": 8 * n["ls"] + (16 + 4 + 4) * n["md"] + bits(2),
-        "k_join_fill[T3]": bits(2) + 8 * n["ls"] + 20 * n["md"] + B_T3 * n["t3"],
-        "k_join_eval[T5]": (16 + 16) * n["t3"] + 20 * n["md"] + bits(3),
-        "k_join_fill[T5]": bits(3) + 32 * n["t3"] + 20 * n["md"] + B_T5 * n["t5"],
-        "k_join_eval[pT5]": B_SEED * n["seeds"] + 20 * n["t5"] + 20 * n["md"],
-        "k_join_fill[pT5]": B_PT * n["pt5"] + 20 * n["t5"],
-        "k_join_eval[pT3]": B_SEED * n["seeds"] + 16 * n["t3"] + 20 * n["md"],
-        "k_join_fill[pT3]": B_PT * n["pt3"] + 16 * n["t3"],
+        "k_ls_eval": B_MD_PRE * n["md"] + 4 * (nnz + 2 * nmod) + 12 * n["surv"][1],
+        "k_ls_decide": (12 + 2 * 36) * n["surv"][1] + bits(1) + 28 * n["ls"],
+        "k_ls_fill": 28 * n["ls"] + bits(1) + B_LS * n["ls"],
+        "k_join_eval[T3]": 8 * n["ls"] + (16 + 4) * n["md"] + 12 * n["surv"][2],
+        "k_join_decide[T3]": (12 + 16) * n["surv"][2] + bits(2) + 48 * n["t3"],
+        "k_join_fill[T3]": 48 * n["t3"] + bits(2) + B_T3 * n["t3"],
+        "k_join_eval[T5]": 16 * n["t3"] + 12 * n["surv"][3],
+        "k_join_decide[T5]": (12 + 64) * n["surv"][3] + bits(3) + 64 * n["t5"],
+        "k_join_fill[T5]": 64 * n["t5"] + bits(3) + B_T5 * n["t5"],
+        "k_join_eval[pT5]": B_SEED * n["seeds"] + 4 * n["t5"] + 24 * n["md"] + 12 * n["surv"][4],
+        "k_join_decide[pT5]": (12 + 40) * n["surv"][4] + 28 * n["pt5"],
+        "k_join_fill[pT5]": 28 * n["pt5"] + B_PT * n["pt5"],
+        "k_join_eval[pT3]": B_SEED * n["seeds"] + 16 * n["t3"] + 24 * n["md"] + 12 * n["surv"][5],
+        "k_join_decide[pT3]": (12 + 32) * n["surv"][5] + 28 * n["pt3"],
+        "k_join_fill[pT3]": 28 * n["pt3"] + B_PT * n["pt3"],
         "k_s0": (40 + 8 + 1) * n["t5"] + (8 + 8 + 1) * (n["pt5"] + n["pt3"]),
         "k_tc_fill": B_TC * n["tc"] + 4 * (n["t5"] + n["pt5"] + n["pt3"] + n["seeds"]),
     }
     return t.get(name)
+
+
+# Arithmetic work of the pre-filter kernels in fp32 lane-operations per candidate (FMA = 1 op),
+# counted from the formulas of lst_math.cuh: the candidate loops are bound by
+# the plain fp32 ALUs / issue slots, not by memory.
+OPS_PER_CAND = {"k_md_eval": (0, 27), "k_ls_eval": (1, 36), "k_join_eval[T3]": (2, 128),
+                "k_join_eval[T5]": (3, 4), "k_join_eval[pT5]": (4, 34), "k_join_eval[pT3]": (5, 34)}
+
+
+def algorithmic_ops(name, n):
+    if name not in OPS_PER_CAND:
+        return None
+    k, ops = OPS_PER_CAND[name]
+    return ops * n["cand"][k]
 
 
 def event_totals_bytes(n):
@@ -358,7 +401,7 @@ def run_ours(a, rank, world, local_rank):
     return lst, geom, events, devt, streams, counts, ms, clocks, value, launches, e2e, (off, cols)
 
 
-def kernel_table(lst, B, devt, streams, a, geom, nnz, peak):
+def kernel_table(lst, B, devt, streams, a, geom, nnz, peak, alu_peak):
     """Per-kernel ms of one representative event (event 0, slot 0), live, CUDA events on the launching
     stream (lst_run_timed), with L2 flushed before each pass; median of 5 passes."""
     import torch
@@ -376,7 +419,8 @@ def kernel_table(lst, B, devt, streams, a, geom, nnz, peak):
     cnt, cand = lst.lst_get_counts(0)
     n = {"hits": int(h[0].numel()), "seeds": int(s[0].numel()), "md": int(cnt[0]), "ls": int(cnt[1]), "t3": int(cnt[2]),
          "t5": int(cnt[3]), "pt3": int(cnt[4]), "pt5": int(cnt[5]), "tc": int(cnt[6]),
-         "cand": [int(c) for c in cand], "n_modules": int(geom.n_modules), "nnz": int(nnz)}
+         "cand": [int(c) for c in cand[:6]], "surv": [int(c) for c in cand[6:12]],
+         "n_modules": int(geom.n_modules), "nnz": int(nnz)}
     names = [k for k, _ in runs[0]]
     med = np.median(np.array([[m for _, m in r] for r in runs]), axis=0)
     chain_ms = float(med.sum())
@@ -384,10 +428,34 @@ def kernel_table(lst, B, devt, streams, a, geom, nnz, peak):
     for k, m in zip(names, med):
         b = algorithmic_bytes(k, n)
         gbs = (b / (m * 1e-3) / 1e9) if (b is not None and m > 0) else None
+        ops = algorithmic_ops(k, n)
+        gops = (ops / (m * 1e-3) / 1e9) if (ops is not None and m > 0) else None
         rows.append({"kernel": k, "ms": round(float(m), 5), "share": round(float(m) / chain_ms, 4),
                      "alg_bytes": None if b is None else int(b), "gbs": None if gbs is None else round(gbs, 2),
-                     "frac_hbm": None if gbs is None else round(gbs / peak, 5)})
+                     "frac_hbm": None if gbs is None else round(gbs / peak, 5),
+                     "alg_ops": ops, "gops": None if gops is None else round(gops, 1),
+                     "frac_alu": None if gops is None else round(gops / alu_peak, 4)})
     return rows, n, chain_ms
+
+
+def roofline(top, peak, peak_src, alu_peak, alu_src):
+    """Roofline object of the dominant kernel (largest live duration).  The candidate loops are
+    bound by the plain fp32 ALUs: achieved = algorithmic fp32 lane-operations per
+    launch / live duration against SMs x lanes x clock; the HBM view of the same kernel is kept
+    beside it because BASELINE.json's metric asks for it."""
+    traffic, traffic_src = NCU_TRAFFIC.get(top["kernel"], (None, None))
+    if top["gops"] is not None:
+        r = {"bound": "alu", "kernel": top["kernel"], "achieved": top["gops"], "peak": round(alu_peak, 1),
+             "unit": "Gop/s", "frac": top["frac_alu"], "traffic": traffic, "traffic_source": traffic_src,
+             "peak_source": alu_src, "alg_ops_per_launch": top["alg_ops"], "ms_per_launch": top["ms"],
+             "hbm": {"achieved": top["gbs"], "peak": peak, "unit": "GB/s", "frac": top["frac_hbm"],
+                     "alg_bytes_per_launch": top["alg_bytes"], "peak_source": peak_src}}
+    else:
+        r = {"bound": "hbm", "kernel": top["kernel"], "achieved": top["gbs"], "peak": peak, "unit": "GB/s",
+             "frac": top["frac_hbm"], "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+             "alg_bytes_per_launch": top["alg_bytes"], "ms_per_launch": top["ms"],
+             "note": "latency-bound integer / lookup kernel: see DESIGN.md and profiles/"}
+    return r
 
 
 def main():
@@ -401,7 +469,8 @@ def main():
     from paper_2209_13711_b200 import binding as B
     lst, geom, events, devt, streams, counts, ms, clocks, value, launches, e2e, mp = run_ours(a, rank, world, local_rank)
     peak, peak_src = peaks()
-    rows, n, chain_ms = kernel_table(lst, B, devt, streams, a, geom, len(mp[1]), peak)
+    alu_peak, alu_src = alu_peak_gops()
+    rows, n, chain_ms = kernel_table(lst, B, devt, streams, a, geom, len(mp[1]), peak, alu_peak)
     if rank == 0:
         top = max(rows, key=lambda r: r["ms"])
         ws = lst.workspace_bytes
@@ -421,11 +490,7 @@ def main():
             "gpu_launches": int(launches * a.events * a.steps),
             "launches_per_event": int(launches),
             "e2e": e2e,
-            "roofline": {"bound": "hbm", "kernel": top["kernel"], "achieved": top["gbs"], "peak": peak, "unit": "GB/s",
-                         "frac": top["frac_hbm"], "traffic": None, "peak_source": peak_src,
-                         "alg_bytes_per_launch": top["alg_bytes"], "ms_per_launch": top["ms"],
-                         "note": "dominant kernel by time; it is issue-slot (plain ALU) bound, not HBM bound: see "
-                                 "DESIGN.md and profiles/"},
+            "roofline": roofline(top, peak, peak_src, alu_peak, alu_src),
             "chain": {"single_stream_ms_per_event": round(chain_ms, 4), "alg_bytes_per_event": int(total_b),
                       "hbm_floor_ms_per_event": round(total_b / (peak * 1e9) * 1e3, 5),
                       "achieved_gbs_whole_step": round(total_b * a.events * a.steps / (ms * 1e-3) / 1e9, 2)},

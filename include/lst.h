@@ -177,7 +177,8 @@ int lst_get_objects(lst_ctx *ctx, uint32_t slot, lst_level level, int copy_to_ho
 
 /* Per-level object counts of the slot's last run (synchronises); counts: uint32[LST_NLEVEL], HOST.
  * Also cheap way to wait for a slot.  cand (optional, may be NULL): candidates evaluated for
- * MD, LS, T3, T5, pT5, pT3 (uint64[6]). */
+ * MD, LS, T3, T5, pT5, pT3, then the candidates that survived each stage's fp32 pre-filter and were
+ * decided in fp64, same order (uint64[12]). */
 int lst_get_counts(lst_ctx *ctx, uint32_t slot, uint32_t *counts, uint64_t *cand);
 
 /* Number of kernels the last lst_run / lst_run_timed of this context enqueued (or captured into

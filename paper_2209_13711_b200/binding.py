@@ -249,7 +249,7 @@ class LST:
 
     def lst_get_counts(self, slot):
         cnt = np.zeros(LST_NLEVEL, np.uint32)
-        cand = np.zeros(6, np.uint64)
+        cand = np.zeros(12, np.uint64)
         _check(lib().lst_get_counts(self._h, slot, _p(cnt), _p(cand)), "lst_get_counts")
         return cnt, cand
 

@@ -263,7 +263,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
         const bool keep = has && ls_tier1_f(g, a.x, a.y, a.z, a.w, ta.x, ta.y, ta.z, b.x, b.y, b.z, b.w, tb.x, tb.y, \
                                             tb.z, (OEC));                                                            \
         Q1.push(keep, (uint32_t)r | ((uint32_t)jj << 8));                                                            \
-        if (Q1.n >= 32u) ls_stage2(sh, s, g, Q1, cl, rpi, nj, it0, nct);                                                 \
+        if (Q1.n >= 32u) ls_stage2(sh, s, g, Q1, cl, rpi, nj, it0, nct);                                             \
       }
       if (all_r) { LST_LS_ROWS(false) }
       else if (all_z) { LST_LS_ROWS(true) }

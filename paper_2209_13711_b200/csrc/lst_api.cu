@@ -663,7 +663,7 @@ extern "C" int lst_get_counts(lst_ctx *c, uint32_t slot, uint32_t *counts, uint6
   const int rc = sync_header(c, s);
   if (rc != LST_OK) return rc;
   for (int l = 0; l < LST_NLEVEL; ++l) counts[l] = s.h_hdr->n_obj[l];
-  if (cand) for (int k = 0; k < S_NSTAGE; ++k) cand[k] = s.h_hdr->cand[k];
+  if (cand) for (int k = 0; k < S_NSTAGE; ++k) { cand[k] = s.h_hdr->cand[k]; cand[S_NSTAGE + k] = s.h_hdr->cl_used[k]; }
   return LST_OK;
 }
 

@@ -22,8 +22,8 @@ constexpr int kItemCand = 1024;          // candidates per work item
 constexpr int kItemWords = kItemCand / 32;
 constexpr int kThreads = 128;            // threads per block of eval / fill kernels
 constexpr int kUnitItems = 16;           // max items per work unit (same group, same column tile, consecutive rows)
-constexpr int kMaxRpi = 256;             // max rows per item
-constexpr int kUnitRows = 256;           // max rows per work unit
+constexpr int kMaxRpi = 128;             // max rows per item
+constexpr int kUnitRows = 128;           // max rows per work unit
 constexpr int kRowChunk = 128;           // rows per group in the variable-width stages (T3, T5, pixel)
 constexpr int kMaxDeg = 512;             // maximum module-map degree (checked by lst_create)
 constexpr int kPxCap = 64;               // (seed, start module) rows per pixel seed ON AVERAGE (overflow -> LST_ENOMEM)
