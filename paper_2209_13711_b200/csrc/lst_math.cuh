@@ -219,26 +219,19 @@ LST_HD bool ls_eval_d(const Params &g, const Pt &A, double ki, double ski, const
   return ok;
 }
 
+// Tier 2 of the LS pre-filter (full fp32 L2 and L3).  It runs on candidates that passed tier 1
+// (ls_tier1_f: pointing L1 and the positive dot product), which it does not repeat.
 LST_HD bool ls_pre_f(const Params &g, float xi, float yi, float zi, float ri, float ki, float ski, int ci,
                      float xo, float yo, float zo, float ro, float ko, float sko, int co) {
-  const float dx = xo - xi, dy = yo - yi, dz = zo - zi;
-  const float dd = dx * dx + dy * dy;
-  const float dotAD = xi * dx + yi * dy;
-  const float drv = LST_FDIV(2.0f * dotAD + dd, ri + ro);
   const float ns = g.f_ns;
-  // L1
-  const float N = ri * dz - zi * drv;
-  const float E = ri * g.f_sig_z[co] + ro * g.f_sig_z[ci] + fabsf(zo) * g.f_sig_r[ci] + fabsf(zi) * g.f_sig_r[co];
-  if (fabsf(N) > (g.f_z0max * fabsf(drv) + ns * E) * kPreSlack) return false;
   const float rr = ri * ro;
-  const float dotAB = ri * ri + dotAD;
-  if (dotAB < -1e-3f * rr) return false;
-  const float cr = xi * dy - yi * dx;
+  const float cr = xi * yo - yi * xo;       // cross(A, D) = cross(A, B)
   const float sd = LST_FDIV(cr, rr);
   const float tphi = LST_FDIV(g.f_sig_t[ci], ri) + LST_FDIV(g.f_sig_t[co], ro);
   const float eci = is_endcap(ci) ? g.f_ec_md_sys : 0.0f, eco = is_endcap(co) ? g.f_ec_md_sys : 0.0f;
   if (!is_endcap(co)) {
-    const float cxy = sqrtf(dd);
+    const float dx = xo - xi, dy = yo - yi;
+    const float cxy = sqrtf(dx * dx + dy * dy);
     const float asd = fabsf(sd);
     if (asd > (g.f_kmax * cxy + ns * tphi) * kPreSlack) return false;
     // L3 multiplied through by cxy
@@ -246,12 +239,22 @@ LST_HD bool ls_pre_f(const Params &g, float xi, float yi, float zi, float ri, fl
     if (fabsf(ko * cxy - sd) > (ns * (sko * cxy + tphi) + eco * asd) * kPreSlack) return false;
   } else {
     const float rbar = 0.5f * (ri + ro), zbar = 0.5f * (fabsf(zi) + fabsf(zo));
-    const float adz = fabsf(dz);
+    const float adz = fabsf(zo - zi);
     const float den = zbar - g.f_z0max - 0.5f * ns * g.f_sig_z[ci];
     if (den < 1e-3f || adz < 1e-6f) return true;   // guards are decided in fp64
     const float srs = g.f_sig_r[ci] + g.f_sig_r[co];
-    const float Sbar = LST_FDIV(asinf(fminf(1.0f, g.f_kmax * (rbar + 0.5f * ns * srs))), g.f_kmax);
-    const float dph = atan2f(cr, dotAB);
+    // asin(x) <= x + (pi/2 - 1) x^3 on [0, 1]: an upper bound only loosens the L2 window
+    const float xs = fminf(1.0f, g.f_kmax * (rbar + 0.5f * ns * srs));
+    const float Sbar = LST_FDIV(xs + 0.5708f * xs * xs * xs, g.f_kmax);
+    // dphi = atan2(cr, dot): for |cr| <= dot / 4 the odd series to t^7 (error < 2e-6 relative)
+    const float dotAB = xi * xo + yi * yo;
+    float dph;
+    if (dotAB > 0.0f && fabsf(cr) <= 0.25f * dotAB) {
+      const float t = LST_FDIV(cr, dotAB), u = t * t;
+      dph = t * (1.0f + u * (-0.33333333f + u * (0.2f - 0.14285714f * u)));
+    } else {
+      dph = atan2f(cr, dotAB);
+    }
     if (fabsf(dph) > (LST_FDIV(g.f_kmax * (adz + ns * g.f_sig_z[ci]) * Sbar, den) + ns * tphi) * kPreSlack) return false;
     const float lever = LST_FDIV(zbar, adz * rbar);
     const float kls = dph * lever, akls = fabsf(kls);
