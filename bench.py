@@ -85,7 +85,7 @@ def alu_peak_gops():
 
 # DRAM bytes (read + write) of one launch of the dominant kernel from the ncu --set full capture
 # summarised in profiles/ (the file is named in the roofline object); None for other kernels.
-NCU_TRAFFIC = {"k_ls_eval": (None, None)}
+NCU_TRAFFIC = {"k_ls_eval": (3209472, "profiles/r1c_top_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full")}
 
 
 class ClockSampler:
@@ -204,7 +204,8 @@ def event_totals_bytes(n):
     """Whole-chain algorithmic bytes of one event (this layout)."""
     return (B_HIT_IN + B_HIT) * n["hits"] + 16 * n["hits"] + B_MD * n["md"] + B_MD_PRE * n["md"] + 4 * n["nnz"] + \
         2 * B_LS * n["ls"] + 2 * B_T3 * n["t3"] + 2 * B_T5 * n["t5"] + B_SEED * n["seeds"] + \
-        2 * B_PT * (n["pt3"] + n["pt5"]) + B_TC * n["tc"]
+        2 * B_PT * (n["pt3"] + n["pt5"]) + B_TC * n["tc"] + \
+        2 * 12 * sum(n["surv"]) + 2 * (36 * n["md"] + 28 * n["ls"] + 48 * n["t3"] + 64 * n["t5"] + 28 * (n["pt3"] + n["pt5"]))
 
 
 # ------------------------------------------------------------------ the oracle leg (CPU)
