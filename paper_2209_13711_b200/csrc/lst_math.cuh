@@ -246,12 +246,12 @@ LST_HD bool ls_pre_f(const Params &g, float xi, float yi, float zi, float ri, fl
     // asin(x) <= x + (pi/2 - 1) x^3 on [0, 1]: an upper bound only loosens the L2 window
     const float xs = fminf(1.0f, g.f_kmax * (rbar + 0.5f * ns * srs));
     const float Sbar = LST_FDIV(xs + 0.5708f * xs * xs * xs, g.f_kmax);
-    // dphi = atan2(cr, dot): for |cr| <= dot / 4 the odd series to t^7 (error < 2e-6 relative)
+    // dphi = atan2(cr, dot): for |cr| <= dot / 2 the odd series to t^11 (error < 1e-5 relative)
     const float dotAB = xi * xo + yi * yo;
     float dph;
-    if (dotAB > 0.0f && fabsf(cr) <= 0.25f * dotAB) {
+    if (dotAB > 0.0f && fabsf(cr) <= 0.5f * dotAB) {
       const float t = LST_FDIV(cr, dotAB), u = t * t;
-      dph = t * (1.0f + u * (-0.33333333f + u * (0.2f - 0.14285714f * u)));
+      dph = t * (1.0f + u * (-0.33333333f + u * (0.2f + u * (-0.14285714f + u * (0.11111111f - 0.09090909f * u)))));
     } else {
       dph = atan2f(cr, dotAB);
     }
