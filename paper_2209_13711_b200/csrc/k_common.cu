@@ -61,22 +61,33 @@ __global__ void k_scatter(GeoDev geo, SlotDev s) {
     if (d >= geo.n_det) continue;
     const uint32_t p = s.det_off[d] + atomicAdd(&s.det_cur[d], 1u);
     s.tmp_orig[p] = h;
+    const float dphi = atan2f(s.raw_y[h], s.raw_x[h]) - geo.phic[d >> 1];
+    const float key = dphi - 6.2831853071795864769f * rintf(dphi * 0.15915494309189533577f);
+    s.tmp_key[p] = key == key ? key : 0.0f;      // NaN coordinates must not break the ranking
   }
 }
 
 // ------------------------------------------------------------------ a0.4 rank inside the det
-// Makes the order canonical (ascending caller index within a det) whatever order the atomics gave.
+// Makes the order canonical whatever order the atomics gave: inside a det the hits ascend in
+// azimuth relative to the module centre (ties: caller index).  MDs (anchor = lower hit) and the
+// T3 / T5 grouped by first MD are then azimuth-ordered inside a module, which the pixel joins use
+// to cut a (seed, module) row down to the objects inside the seed's azimuthal window.
 __global__ void k_rank(GeoDev geo, SlotDev s) {
   const uint32_t n = s.det_off[geo.n_det];
   for (uint32_t p = blockIdx.x * blockDim.x + threadIdx.x; p < n; p += gridDim.x * blockDim.x) {
     const uint32_t h = s.tmp_orig[p];
     const uint32_t d = s.raw_det[h];
     const uint32_t b = s.det_off[d], e = s.det_off[d + 1];
+    const float key = s.tmp_key[p];
     uint32_t r = 0;
-    for (uint32_t q = b; q < e; ++q) r += (s.tmp_orig[q] < h);
+    for (uint32_t q = b; q < e; ++q) {
+      const float kq = s.tmp_key[q];
+      r += (kq < key || (kq == key && s.tmp_orig[q] < h));
+    }
     const float x = s.raw_x[h], y = s.raw_y[h], z = s.raw_z[h];
     s.hit[b + r] = make_float4(x, y, z, sqrtf(x * x + y * y));
     s.hit_orig[b + r] = h;
+    s.hit_key[b + r] = key;
   }
 }
 

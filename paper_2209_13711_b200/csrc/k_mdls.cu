@@ -95,6 +95,7 @@ __global__ void __launch_bounds__(256) k_md_fill(GeoDev geo, SlotDev s) {
     s.md_mod[idx] = (m << 2) | (uint32_t)geo.category[m];
     s.md_dphi[idx] = st.p_f4[j].x;
     s.md_phi[idx] = atan2f(l.y, l.x);
+    s.md_prel[idx] = s.hit_key[hl];
   }
 }
 

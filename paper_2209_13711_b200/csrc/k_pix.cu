@@ -73,11 +73,23 @@ __global__ void __launch_bounds__(256) k_px_modules(GeoDev geo, SlotDev s, Param
   for (uint32_t p = warp; p < n_seeds; p += nwarp) {
     uint32_t *bits = s.px_bits + (size_t)p * nw;
     if (FILL) {
+      const float pt = s.seed_pt[p], phi = s.seed_phi[p], z0 = s.seed_z0[p];
+      const float kp = -(float)s.seed_q[p] * (float)g.kB / (2.0f * pt);
+      const float sh = sinhf(s.seed_eta[p]);
       uint32_t pos = s.px_off[p];
       for (uint32_t w = 0; w < nw; ++w) {
         const uint32_t b = bits[w];
-        if ((b >> lane) & 1u)
-          s.px_pair[pos + __popc(b & ((1u << lane) - 1u))] = make_uint2(p, geo.start_mods[w * 32 + lane]);
+        if ((b >> lane) & 1u) {
+          const uint32_t k = w * 32 + lane, m = geo.start_mods[k], r = geo.prow_of[k];
+          // the row's window again, now for the azimuth of a first anchor instead of the module
+          // centre: the module's half width drops out
+          float centre = 0.0f, halfw = 0.0f;
+          const float4 r1 = geo.prow_b1[r];
+          px_row_window(g, r1, geo.prow_b2[r], kp, sh, phi, z0, &centre, &halfw);
+          const uint32_t o = pos + __popc(b & ((1u << lane) - 1u));
+          s.px_pair[o] = make_uint2(p, m);
+          s.px_win[o] = make_float2(wrap_f(centre - geo.phic[m]), halfw - r1.x + 1e-4f);
+        }
         pos += __popc(b);
       }
     } else {

@@ -47,8 +47,20 @@ __device__ __forceinline__ void right_range(const SlotDev &s, uint32_t row, uint
     *st = s.t3_md_off[m3];
     *cnt = s.t3_md_off[m3 + 1] - *st;
   } else {
+    // objects whose first MD lies in the row's module AND inside the row's azimuthal window: MDs
+    // ascend in azimuth (relative to the module centre) inside a module, so that is a range
     const uint32_t m = s.px_pair[row].y;
-    const uint32_t md0 = s.md_mod_off[m], md1 = s.md_mod_off[m + 1];
+    uint32_t md0 = s.md_mod_off[m], md1 = s.md_mod_off[m + 1];
+    const float2 win = s.px_win[row];
+    if (win.y < 2.5f) {        // wider windows wrap around: keep the whole module
+      const float lo = win.x - win.y, hi = win.x + win.y;
+      uint32_t a = md0, b = md1;
+      while (a < b) { const uint32_t mid = (a + b) >> 1; if (s.md_prel[mid] < lo) a = mid + 1; else b = mid; }
+      const uint32_t first = a;
+      b = md1;
+      while (a < b) { const uint32_t mid = (a + b) >> 1; if (s.md_prel[mid] <= hi) a = mid + 1; else b = mid; }
+      md0 = first; md1 = a;
+    }
     const uint32_t *off = KIND == J_PT5 ? s.t5_md_off : s.t3_md_off;
     *st = off[md0];
     *cnt = off[md1] - *st;
@@ -234,7 +246,12 @@ __device__ __forceinline__ bool join_phase1(const SlotDev &s, const Params &g, u
   }
   if (KIND == J_T5) {
     const double2 k3a = s.t3_kd[row], k3b = s.t3_kd[b];
-    return le(fabs(k3a.x - k3b.x), g.ns * (k3a.y + k3b.y));
+    if (!le(fabs(k3a.x - k3b.x), g.ns * (k3a.y + k3b.y))) return false;          // T5-1 (exact, fp64)
+    // T5-2: the middle triplet (MD 2, 3, 4) through the fp32 triplet pre-filter
+    const uint4 ta = s.t3_md[row], tb = s.t3_md[b];
+    const float4 p2 = s.md_pos[ta.y], p3 = s.md_pos[ta.z], p4 = s.md_pos[tb.y];
+    const int c2 = (int)(s.md_mod[ta.y] & 3u), c3 = (int)(s.md_mod[ta.z] & 3u), c4 = (int)(s.md_mod[tb.y] & 3u);
+    return t3_pre_f(g, p2.x, p2.y, p2.z, p2.w, c2, p3.x, p3.y, p3.z, p3.w, c3, p4.x, p4.y, p4.z, p4.w, c4);
   }
   ab->x = s.px_pair[row].x;     // the seed
   return px_pre_f<KIND>(s, g, rowseed[lrow], b);

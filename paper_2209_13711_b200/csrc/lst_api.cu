@@ -275,10 +275,11 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.det_cnt = w.take<uint32_t>(n_det + 1); s.det_off = w.take<uint32_t>(n_det + 1);
   s.det_cur = w.take<uint32_t>(n_det + 1);
   s.tmp_orig = w.take<uint32_t>(nh);
+  s.tmp_key = w.take<float>(nh); s.hit_key = w.take<float>(nh);
   s.hit = w.take<float4>(nh); s.hit_orig = w.take<uint32_t>(nh);
   s.md_pos = w.take<float4>(s.cap_md); s.md_kd = w.take<double2>(s.cap_md); s.md_kf = w.take<float2>(s.cap_md);
   s.md_hit = w.take<uint2>(s.cap_md); s.md_mod = w.take<uint32_t>(s.cap_md); s.md_dphi = w.take<float>(s.cap_md);
-  s.md_phi = w.take<float>(s.cap_md);
+  s.md_phi = w.take<float>(s.cap_md); s.md_prel = w.take<float>(s.cap_md);
   s.md_mod_off = w.take<uint32_t>(n_mod + 1);
   s.ls_md = w.take<uint2>(s.cap_ls); s.ls_f = w.take<float4>(s.cap_ls);
   s.ls_md_off = w.take<uint32_t>((size_t)s.cap_md + 1);
@@ -296,6 +297,7 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.px_cnt = w.take<uint32_t>(nsd);
   s.px_bits = w.take<uint32_t>((size_t)nsd * ((c->k.geo.n_start + 31) / 32));
   s.px_off = w.take<uint32_t>((size_t)nsd + 1); s.px_pair = w.take<uint2>((size_t)nsd * kPxCap);
+  s.px_win = w.take<float2>((size_t)nsd * kPxCap);
   s.pt5_pls_off = w.take<uint32_t>((size_t)nsd + 1); s.pt3_pls_off = w.take<uint32_t>((size_t)nsd + 1);
   s.t5_hits = w.take<uint32_t>(10 * (size_t)s.cap_t5); s.pt3_hits = w.take<uint32_t>(6 * (size_t)s.cap_pt3);
   s.inc_cnt = w.take<uint32_t>(2 * (3 * (size_t)nh + 1)); s.inc_cur = s.inc_cnt ? s.inc_cnt + 3 * (size_t)nh + 1 : nullptr;
@@ -441,7 +443,8 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   const size_t o_poff = o_prow2 + up(std::max<size_t>(n_prow, 1) * 16);
   const size_t o_pk = o_poff + up((n_prow + 1) * 4);
   const size_t o_pphi = o_pk + up(std::max<size_t>(prow_k.size(), 1) * 4);
-  const size_t total = o_pphi + up(std::max<size_t>(prow_phic.size(), 1) * 4);
+  const size_t o_pof = o_pphi + up(std::max<size_t>(prow_phic.size(), 1) * 4);
+  const size_t total = o_pof + up(std::max<size_t>(start_mods.size(), 1) * 4);
   e = cudaMalloc(&c->d_static, total);
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaMalloc(static)"); }
   char *d = (char *)c->d_static;
@@ -481,6 +484,11 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
     c->k.geo.prow_off = (const uint32_t *)(d + o_poff); c->k.geo.prow_k = (const uint32_t *)(d + o_pk);
     c->k.geo.prow_phic = (const float *)(d + o_pphi);
     c->k.geo.n_prow = (uint32_t)n_prow;
+    std::vector<uint32_t> prow_of(std::max<size_t>(start_mods.size(), 1), 0u);
+    for (size_t r = 0; r < n_prow; ++r)
+      for (uint32_t i = prow_off[r]; i < prow_off[r + 1]; ++i) prow_of[prow_k[i]] = (uint32_t)r;
+    cudaMemcpy(d + o_pof, prow_of.data(), prow_of.size() * 4, cudaMemcpyHostToDevice);
+    c->k.geo.prow_of = (const uint32_t *)(d + o_pof);
   }
   e = cudaDeviceSynchronize();
   if (e != cudaSuccess) { cudaFree(c->d_static); delete c; return cuda_fail(e, "upload geometry"); }

@@ -121,6 +121,7 @@ struct GeoDev {
   const float4 *prow_b1, *prow_b2;
   const uint32_t *prow_off, *prow_k;
   const float *prow_phic;
+  const uint32_t *prow_of;   // [n_start] row of start module k
   uint32_t n_prow;
 };
 
@@ -133,6 +134,7 @@ struct SlotDev {
   // a0: hits grouped by det
   uint32_t *det_cnt, *det_off, *det_cur;     // [n_det+1]
   uint32_t *tmp_orig;                        // [cap_hits]
+  float *tmp_key, *hit_key;                  // [cap_hits] azimuth relative to the module centre (sort key inside a det)
   float4 *hit;                               // [cap_hits] x, y, z, rt
   uint32_t *hit_orig;                        // [cap_hits] original caller index
   // MD
@@ -143,6 +145,7 @@ struct SlotDev {
   uint32_t *md_mod;      // module << 2 | category
   float *md_dphi;
   float *md_phi;         // azimuth of the anchor, fp32 (pixel-linking pre-filter)
+  float *md_prel;        // the anchor's sort key (azimuth relative to the module centre): ascending inside a module
   uint32_t *md_mod_off;  // [n_modules+1]
   // LS
   uint2 *ls_md;          // inner, outer MD
@@ -171,6 +174,7 @@ struct SlotDev {
   uint32_t *px_bits;               // [cap_seeds * ceil(n_start / 32)] one bit per (seed, start module)
   uint32_t *px_off;                // [cap_seeds+1]
   uint2 *px_pair;                  // [cap_seeds * kPxCap] (seed, module), ascending: rows of the pixel joins
+  float2 *px_win;                  // [cap_seeds * kPxCap] the row's azimuthal window for first anchors: {centre - phic, half width}
   uint32_t *pt5_pls_off, *pt3_pls_off;   // [cap_seeds+1] pT5 / pT3 range of a seed
   // a6 cleaning
   uint32_t *t5_hits, *pt3_hits;    // [10 cap_t5], [6 cap_pt3] sorted hit positions in layer order

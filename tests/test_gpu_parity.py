@@ -92,14 +92,28 @@ def test_barrel_configs_chain(B, geom_barrel, map_barrel, cfg):
     o = _oracle(geom_barrel, map_barrel, ev, O.T5)
     lst = _gpu(B, geom_barrel, map_barrel, ev)
     cnt, cand = lst.lst_get_counts(0)
+    prev = None
     for lvl in CHAIN:
         n, near, ref, got = compare_level(o, lst, lvl)
         assert n == o.count(lvl) and n > 0
         assert cnt[lvl] == len(got["hits"])
-        # canonical order: the CUDA path emits objects in the oracle's order (ascending module, rows, columns)
-        if near == 0:
-            assert np.array_equal(ref["hits"], got["hits"])
-            assert np.array_equal(ref["parents"], got["parents"])
+        # canonical order of the CUDA path: MDs ascend in (module, azimuth of the lower hit
+        # relative to the module centre); every higher level is grouped by its first constituent, and
+        # its parents index the level below
+        h, par = got["hits"].astype(np.int64), got["parents"].astype(np.int64)
+        if lvl == O.MD:
+            mod = ev.det[h[:, 0]].astype(np.int64) >> 1
+            assert np.all(np.diff(mod) >= 0)
+            rel = np.arctan2(ev.y[h[:, 0]].astype(np.float64), ev.x[h[:, 0]].astype(np.float64)) - \
+                np.asarray(geom_barrel.phic, np.float64)[mod]
+            rel = np.remainder(rel + np.pi, 2 * np.pi) - np.pi
+            same = np.diff(mod) == 0
+            assert np.all(np.diff(rel)[same] >= -1e-5)
+        else:
+            assert np.all(np.diff(par[:, 0]) >= 0)
+            ph = prev["hits"].astype(np.int64)
+            assert np.array_equal(h, np.concatenate([ph[par[:, 0]], ph[par[:, 1]][:, (0 if lvl == O.LS else 2):]], 1))
+        prev = got
     lst.close()
 
 
@@ -113,8 +127,8 @@ def test_full_detector_chain(B, geom_full, map_full, cfg):
         n, near, ref, got = compare_level(o, lst, lvl)
         assert n == o.count(lvl) and n > 1000
         total += n
-        if near == 0:
-            assert np.array_equal(ref["hits"], got["hits"])
+        if lvl != O.MD:      # grouped by first constituent (canonical order)
+            assert np.all(np.diff(got["parents"][:, 0].astype(np.int64)) >= 0)
     cnt, cand = lst.lst_get_counts(0)
     assert cand[1] > 1e6    # the LS candidate loop is the dominant one
     lst.close()
@@ -227,8 +241,14 @@ def compare_cleaning(o, lst, ev):
     keys_o, tc_o = _oracle_tc_keys(o, ev)
     got = lst.lst_get_objects(0, O.TC)
     keys_g = [(int(p[0]), *h) for p, h in zip(got["parents"].tolist(), got["hits"].astype(np.int64).tolist())]
-    assert keys_g == keys_o                       # same candidates in the same (canonical) order
-    f_o, f_g = tc_o["f"], got["f"].astype(np.float64)
+    # same candidates; the TC list is ordered pT5, pT3, T5, pLS (S4) on both sides, the order INSIDE a
+    # type is each implementation's object order (the CUDA path's is azimuth-major)
+    assert len(set(keys_g)) == len(keys_g) and set(keys_g) == set(keys_o)
+    rank = {O.PT5: 0, O.PT3: 1, O.T5: 2, O.TC: 3}
+    for keys in (keys_g, keys_o):
+        assert np.all(np.diff([rank[k[0]] for k in keys]) >= 0)
+    io = {k: i for i, k in enumerate(keys_o)}
+    f_o, f_g = tc_o["f"][[io[k] for k in keys_g]], got["f"].astype(np.float64)
     assert np.allclose(f_g, f_o, rtol=REL, atol=1e-6)
     return len(keys_o)
 
