@@ -219,29 +219,192 @@ __global__ void k_dd_scatter(SlotDev s) {
   }
 }
 
+// ------------------------------------------------------------------ S0, same-seed rule
+// "a is removed iff some b of the same pixel seed beats a" and "beats" is a strict total order, so
+// of a seed's pT5 (pT3) exactly the minimum survives this rule.  One thread per object, two passes:
+// the seed's minimum score by atomicMin on the bit pattern of the (non-negative) double, then the
+// objects AT that score settle the tie order by compare-and-swap (anchors are lower hits, so T3 /
+// T5 that differ only in upper hits tie exactly; the tie sets at the minimum are small).
+__global__ void __launch_bounds__(256) k_pls_min(SlotDev s) {
+  const Header *hdr = s.hdr;
+  const uint32_t np5 = hdr->n_obj[5], np3 = hdr->n_obj[4];
+  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < np5 + np3; j += gridDim.x * blockDim.x) {
+    const bool is5 = j < np5;
+    const uint32_t i = is5 ? j : j - np5;
+    const uint32_t p = (is5 ? s.pt5_po : s.pt3_po)[i].x;
+    const double sc = (is5 ? s.pt5_chi2 : s.pt3_chi2)[i];
+    atomicMin((is5 ? s.pls_min5 : s.pls_min3) + p, (unsigned long long)__double_as_longlong(sc));
+  }
+}
+__global__ void __launch_bounds__(256) k_pls_best(SlotDev s) {
+  const Header *hdr = s.hdr;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], np3 = hdr->n_obj[4];
+  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < np5 + np3; j += gridDim.x * blockDim.x) {
+    const bool is5 = j < np5;
+    const uint32_t i = is5 ? j : j - np5;
+    const uint32_t p = (is5 ? s.pt5_po : s.pt3_po)[i].x;
+    const double sc = (is5 ? s.pt5_chi2 : s.pt3_chi2)[i];
+    if ((unsigned long long)__double_as_longlong(sc) != (is5 ? s.pls_min5 : s.pls_min3)[p]) continue;
+    uint32_t *best = (is5 ? s.pls_best5 : s.pls_best3) + p;
+    const uint32_t dbase = is5 ? n5 : n5 + np5;
+    const DRef me = dd_ref(s, n5, np5, dbase + i);
+    uint32_t cur = *(volatile uint32_t *)best;
+    while (cur == 0xFFFFFFFFu || dd_beats_tie(s, me, dd_ref(s, n5, np5, dbase + cur))) {
+      const uint32_t old = atomicCAS(best, cur, i);
+      if (old == cur) break;
+      cur = old;
+    }
+  }
+}
+
 // ------------------------------------------------------------------ S0: inside one collection
-// One WARP per object A.  An object sharing >= min_shared of A's n_ot hits contains at least one of
-// any n_ot - min_shared + 1 of them, so only the n_ot - min_shared + 1 shortest incidence lists (of
-// A's own type) are searched; the lists are flattened into one index space that the lanes stride
-// (their lengths are very uneven: inner-layer hits sit in hundreds of objects).  Per entry B the
+// EIGHT LANES per object A, four objects per warp (most objects are beaten by one of the first few
+// entries they look at, so the per-object set-up dominates; it is shared by four objects here).
+// An object sharing >= min_shared of A's n_ot hits contains at least one of any n_ot - min_shared
+// + 1 of them, so only the n_ot - min_shared + 1 shortest incidence lists (of A's own type) are
+// searched; the lists are flattened into one index space that the 8 lanes stride.  Per entry B the
 // cheap test comes first (score(B) <= score(A)); the shared-hit count is exact and costs one
-// shared-memory lookup per hit of B: A's hits sit in a 256-slot table per warp (slot = hit & 255;
-// an A whose hits collide in the table - ~16 % - counts with the 10 x 10 comparison instead).
-constexpr int kS0Slots = 256;
+// shared-memory lookup per hit of B: A's hits sit in a 128-slot table per group (slot = hit & 127;
+// an A whose hits collide in the table counts with the 10 x 10 comparison instead).
+constexpr int kS0Slots = 128;
+constexpr uint32_t kNoHit = 0xFFFFFFFFu;
+constexpr uint32_t kS0Light = 64;   // entries an 8-lane group looks at before it hands a longer object to k_s0_heavy
 __device__ __forceinline__ double dd_score(const SlotDev &s, uint32_t n5, uint32_t np5, uint32_t d) {
   return d < n5 ? s.t5_chi2[d] : (d < n5 + np5 ? s.pt5_chi2[d - n5] : s.pt3_chi2[d - n5 - np5]);
 }
 __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
-  __shared__ uint32_t sh_pre[4][12], sh_beg[4][12];
-  __shared__ uint32_t sh_tab[4][kS0Slots];
-  const Header *hdr = s.hdr;
+  __shared__ uint32_t sh_pre[16][12], sh_beg[16][12];
+  __shared__ uint32_t sh_tab[16][kS0Slots];
+  Header *hdr = s.hdr;
   const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = hdr->n_dd;
+  const int lane = threadIdx.x & 31, gl = lane & 7, gbase = lane & ~7, gid = threadIdx.x >> 3;
+  const uint32_t gmask = 0xFFu << gbase;
+  const uint32_t group = (blockIdx.x * blockDim.x + threadIdx.x) >> 3, ngroup = (gridDim.x * blockDim.x) >> 3;
+  uint32_t *pre = sh_pre[gid], *beg = sh_beg[gid], *tab = sh_tab[gid];
+  for (int k = gl; k < kS0Slots; k += 8) tab[k] = kNoHit;
+  __syncwarp();
+  for (uint32_t d = group;; d += ngroup) {
+    const bool valid = d < n_dd;
+    if (!__any_sync(0xffffffffu, valid)) break;
+    DRef A;
+    A.type = 0; A.idx = 0; A.n_ot = 0; A.hits = nullptr; A.pls = kNoHit; A.score = 0.0;
+    if (valid) A = dd_ref(s, n5, np5, d);
+    // lane gl owns hits gl and gl + 8 of A
+    const uint32_t h0 = gl < A.n_ot ? A.hits[gl] : kNoHit, h1 = gl + 8 < A.n_ot ? A.hits[gl + 8] : kNoHit;
+    bool beaten = false, defer = false;
+    if (g.s0_enabled) {
+      const int min_shared = A.type == 0 ? g.dup_t5 : (A.type == 1 ? g.dup_pt5 : g.dup_pt3);
+      const int k0 = min_shared - 1, nl = A.n_ot > k0 ? A.n_ot - k0 : 0;   // number of lists searched
+      // table of A's hits; a collision (two hits of A in one slot) -> exact comparison path
+      const uint32_t slot0 = h0 & (kS0Slots - 1), slot1 = h1 & (kS0Slots - 1);
+      if (h0 != kNoHit) tab[slot0] = h0;
+      __syncwarp();
+      if (h1 != kNoHit) tab[slot1] = h1;
+      __syncwarp();
+      const bool bad = (h0 != kNoHit && tab[slot0] != h0) || (h1 != kNoHit && tab[slot1] != h1);
+      const bool collide = (__ballot_sync(0xffffffffu, bad) & gmask) != 0u;
+      {
+        // the nl SHORTEST of A's n_ot incidence lists are searched (any nl of them will do)
+        uint32_t len0 = 0, b0 = 0, len1 = 0, b1 = 0;
+        if (h0 != kNoHit) { const uint32_t row = 3 * h0 + (uint32_t)A.type; b0 = s.inc_off[row]; len0 = s.inc_off[row + 1] - b0; }
+        if (h1 != kNoHit) { const uint32_t row = 3 * h1 + (uint32_t)A.type; b1 = s.inc_off[row]; len1 = s.inc_off[row + 1] - b1; }
+        // rank by (length, hit position): keys are unique, missing hits sort last
+        const uint32_t key0 = h0 != kNoHit ? ((len0 < (1u << 27) ? len0 : (1u << 27) - 1u) << 4) | (uint32_t)gl : kNoHit;
+        const uint32_t key1 = h1 != kNoHit ? ((len1 < (1u << 27) ? len1 : (1u << 27) - 1u) << 4) | (uint32_t)(gl + 8) : kNoHit;
+        int rank0 = 0, rank1 = 0;
+#pragma unroll
+        for (int j = 0; j < 10; ++j) {
+          const uint32_t kj = j < 8 ? __shfl_sync(0xffffffffu, key0, gbase | j) : __shfl_sync(0xffffffffu, key1, gbase | (j - 8));
+          rank0 += (int)(kj < key0); rank1 += (int)(kj < key1);
+        }
+        if (h0 != kNoHit && rank0 < nl) { beg[rank0] = b0; pre[rank0] = len0; }
+        if (h1 != kNoHit && rank1 < nl) { beg[rank1] = b1; pre[rank1] = len1; }
+        __syncwarp();
+        if (gl == 0) {                                           // exclusive prefix of the <= 10 selected lengths
+          uint32_t acc = 0;
+          for (int q = 0; q < nl; ++q) { const uint32_t t = pre[q]; pre[q] = acc; acc += t; }
+          pre[nl] = acc;
+        }
+        __syncwarp();
+      }
+      const uint32_t total = valid ? pre[nl] : 0u;
+      const double *score_arr = A.type == 0 ? s.t5_chi2 : (A.type == 1 ? s.pt5_chi2 : s.pt3_chi2);
+      const uint32_t dbase = A.type == 0 ? 0u : (A.type == 1 ? n5 : n5 + np5);
+      int cur = 0;
+      for (uint32_t base = 0;; base += 8) {
+        if (!beaten && base >= kS0Light && base < total) defer = true;     // a long one: the whole-warp kernel takes it
+        const bool active = !beaten && !defer && base < total;
+        if (!__any_sync(0xffffffffu, active)) break;
+        const uint32_t i = base + gl;
+        bool hit = false;
+        if (active && i < total) {
+          while (i >= pre[cur + 1]) ++cur;
+          const uint32_t b = s.inc_ent[beg[cur] + (i - pre[cur])];
+          if (b != d && !(score_arr[b - dbase] > A.score)) {
+            int cnt;
+            if (!collide) {
+              const uint32_t *hb = A.type == 0 ? s.t5_hits + 10 * (size_t)b
+                                 : (A.type == 1 ? s.t5_hits + 10 * (size_t)s.pt5_po[b - dbase].y
+                                                : s.pt3_hits + 6 * (size_t)(b - dbase));
+              const uint2 *hb2 = reinterpret_cast<const uint2 *>(hb);
+              cnt = 0;
+#pragma unroll
+              for (int q = 0; q < 5; ++q) {
+                if (2 * q < A.n_ot) {
+                  const uint2 v = hb2[q];
+                  cnt += (int)(tab[v.x & (kS0Slots - 1)] == v.x) + (int)(tab[v.y & (kS0Slots - 1)] == v.y);
+                }
+              }
+            } else {
+              uint32_t ha[10];
+#pragma unroll
+              for (int q = 0; q < 10; ++q) ha[q] = q < A.n_ot ? A.hits[q] : kNoHit;
+              const DRef Bq = dd_ref(s, n5, np5, b);
+              cnt = dd_shared(ha, A.n_ot, Bq.hits, Bq.n_ot);
+            }
+            if (cnt >= min_shared) hit = dd_beats(s, dd_ref(s, n5, np5, b), A);
+          }
+        }
+        if ((__ballot_sync(0xffffffffu, hit) & gmask) != 0u) beaten = true;
+      }
+      // objects of the same pixel seed are duplicates of one another: only the seed's best survives
+      if (valid && A.type != 0 && (A.type == 1 ? s.pls_best5 : s.pls_best3)[A.pls] != A.idx) beaten = true;
+      __syncwarp();
+      if (h0 != kNoHit) tab[slot0] = kNoHit;                     // leave the table empty for the next object
+      if (h1 != kNoHit) tab[slot1] = kNoHit;
+      __syncwarp();
+    }
+    if (valid && gl == 0 && defer && !beaten) s.tc_pos[atomicAdd(&hdr->n_heavy, 1u)] = d;
+    if (valid && gl == 0 && !(defer && !beaten)) {
+      const bool keep = !beaten;
+      if (A.type == 0) s.t5_keep[A.idx] = keep;
+      else if (A.type == 1) {
+        s.pt5_keep[A.idx] = keep;
+        if (keep) {
+          s.pls_has5[A.pls] = 1;
+          pid_mark(s, s.pid_has5, A.pls);
+          for (int q = 0; q < 10; ++q) s.hit_used5[A.hits[q]] = 1;   // S1 / S2: "shares a hit with a surviving pT5"
+        }
+      }
+      else s.pt3_keep[A.idx] = keep;
+    }
+  }
+}
+
+// The objects k_s0 deferred (not beaten by their first kS0Light entries and with longer lists: mostly
+// the objects that survive): one WARP per object over the whole flattened list.
+__global__ void __launch_bounds__(128) k_s0_heavy(SlotDev s, Params g) {
+  __shared__ uint32_t sh_pre[4][12], sh_beg[4][12];
+  __shared__ uint32_t sh_tab[4][256];
+  const Header *hdr = s.hdr;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_heavy = hdr->n_heavy;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
   uint32_t *pre = sh_pre[wib], *beg = sh_beg[wib], *tab = sh_tab[wib];
-  for (int k = lane; k < kS0Slots; k += 32) tab[k] = 0xFFFFFFFFu;
+  for (int k = lane; k < 256; k += 32) tab[k] = 0xFFFFFFFFu;
   __syncwarp();
-  for (uint32_t d = warp; d < n_dd; d += nwarp) {
+  for (uint32_t hv = warp; hv < n_heavy; hv += nwarp) {
+    const uint32_t d = s.tc_pos[hv];
     const DRef A = dd_ref(s, n5, np5, d);
     // lane q < n_ot owns hit q of A
     const uint32_t my_hit = lane < A.n_ot ? A.hits[lane] : 0xFFFFFFFFu;
@@ -250,7 +413,7 @@ __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
       const int min_shared = A.type == 0 ? g.dup_t5 : (A.type == 1 ? g.dup_pt5 : g.dup_pt3);
       const int k0 = min_shared - 1, nl = A.n_ot > k0 ? A.n_ot - k0 : 0;   // lists searched: hits k0 .. n_ot-1
       // table of A's hits; collisions (two hits of A in one slot) -> exact comparison path
-      const uint32_t slot = my_hit & (kS0Slots - 1);
+      const uint32_t slot = my_hit & (256 - 1);
       const uint32_t same = __match_any_sync(0xffffffffu, lane < A.n_ot ? slot : 0x10000u + lane);
       const bool collide = __any_sync(0xffffffffu, lane < A.n_ot && __popc(same) > 1);
       if (lane < A.n_ot) tab[slot] = my_hit;
@@ -297,7 +460,7 @@ __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
               for (int q = 0; q < 5; ++q) {
                 if (2 * q < A.n_ot) {
                   const uint2 v = hb2[q];
-                  cnt += (int)(tab[v.x & (kS0Slots - 1)] == v.x) + (int)(tab[v.y & (kS0Slots - 1)] == v.y);
+                  cnt += (int)(tab[v.x & (256 - 1)] == v.x) + (int)(tab[v.y & (256 - 1)] == v.y);
                 }
               }
             } else {
@@ -314,18 +477,8 @@ __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
       }
       __syncwarp();
       if (lane < A.n_ot) tab[slot] = 0xFFFFFFFFu;                 // leave the table empty for the next object
-      if (!beaten && A.type != 0) {   // objects of the same pixel seed are duplicates of one another
-        const uint32_t *off = A.type == 1 ? s.pt5_pls_off : s.pt3_pls_off;
-        const uint32_t dbase = A.type == 1 ? n5 : n5 + np5;
-        const uint32_t i0 = off[A.pls], i1 = off[A.pls + 1];
-        for (uint32_t base = i0; base < i1 && !beaten; base += 32) {
-          const uint32_t i = base + lane;
-          bool hit = false;
-          if (i < i1 && i != A.idx && !(dd_score(s, n5, np5, dbase + i) > A.score))
-            hit = dd_beats(s, dd_ref(s, n5, np5, dbase + i), A);
-          beaten = __any_sync(0xffffffffu, hit);
-        }
-      }
+      // objects of the same pixel seed are duplicates of one another: only the seed's best survives
+      if (!beaten && A.type != 0 && (A.type == 1 ? s.pls_best5 : s.pls_best3)[A.pls] != A.idx) beaten = true;
     }
     if (lane == 0) {
       const bool keep = !beaten;
@@ -467,7 +620,11 @@ void launch_dedup(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   k_dd_count<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_dd_count");
   launch_scan(c, s, s.inc_cnt, s.inc_off, &s.hdr->n_inc, st);
   k_dd_scatter<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_dd_scatter");
-  k_s0<<<grid_of(cap_dd, 4, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s0");
+  cudaMemsetAsync(s.pls_min5, 0xFF, 24 * (size_t)s.cap_seeds, st);      // pls_min5, pls_min3, pls_best5, pls_best3
+  k_pls_min<<<grid_of(s.cap_pt5 + s.cap_pt3, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_pls_min");
+  k_pls_best<<<grid_of(s.cap_pt5 + s.cap_pt3, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_pls_best");
+  k_s0<<<grid_of(cap_dd, 16, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s0");
+  k_s0_heavy<<<grid_of(cap_dd, 4, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s0_heavy");
   k_s1<<<grid_of(s.cap_pt3, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s1");
   k_s2<<<grid_of(s.cap_t5, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s2");
   k_s3_flags<<<grid_of(s.cap_tc, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_s3_flags");

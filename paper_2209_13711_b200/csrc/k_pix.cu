@@ -7,6 +7,8 @@
 // (k_t3t5.cu), whose right lists are the T5 / T3 starting in that module.  The window test is
 // conservative (interval arithmetic on the box plus margins); tests compare with the oracle's
 // brute force.
+#include <algorithm>
+
 #include "lst_launch.h"
 
 namespace lst {
@@ -69,29 +71,40 @@ __global__ void __launch_bounds__(256) k_px_modules(GeoDev geo, SlotDev s, Param
   const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
   const uint32_t nw = (geo.n_start + 31) / 32;
   if (FILL && s.hdr->n_obj[kPairLevel] == 0) return;
-  uint32_t *wbits = px_sh + (size_t)wib * nw;
+  uint32_t *wbits = px_sh + (size_t)wib * (nw > 64u ? nw : 64u);
   for (uint32_t p = warp; p < n_seeds; p += nwarp) {
     uint32_t *bits = s.px_bits + (size_t)p * nw;
     if (FILL) {
       const float pt = s.seed_pt[p], phi = s.seed_phi[p], z0 = s.seed_z0[p];
       const float kp = -(float)s.seed_q[p] * (float)g.kB / (2.0f * pt);
       const float sh = sinhf(s.seed_eta[p]);
+      // the set bits (ascending module) go through a warp queue so that the windows of 32 (seed,
+      // module) rows are computed at a time
       uint32_t pos = s.px_off[p];
-      for (uint32_t w = 0; w < nw; ++w) {
-        const uint32_t b = bits[w];
-        if ((b >> lane) & 1u) {
-          const uint32_t k = w * 32 + lane, m = geo.start_mods[k], r = geo.prow_of[k];
-          // the row's window again, now for the azimuth of a first anchor instead of the module
-          // centre: the module's half width drops out
-          float centre = 0.0f, halfw = 0.0f;
-          const float4 r1 = geo.prow_b1[r];
-          px_row_window(g, r1, geo.prow_b2[r], kp, sh, phi, z0, &centre, &halfw);
-          const uint32_t o = pos + __popc(b & ((1u << lane) - 1u));
-          s.px_pair[o] = make_uint2(p, m);
-          s.px_win[o] = make_float2(wrap_f(centre - geo.phic[m]), halfw - r1.x + 1e-4f);
+      WarpQueue Q;
+      Q.init(wbits);                  // 64 words of this warp's shared area (nw >= 64 is not needed: see launch)
+      for (uint32_t w = 0; w <= nw; ++w) {
+        if (w < nw) {
+          const uint32_t b = bits[w];
+          Q.push(((b >> lane) & 1u) != 0u, w * 32 + lane);
         }
-        pos += __popc(b);
+        while (Q.n >= 32u || (w == nw && Q.n > 0u)) {
+          const uint32_t take = Q.n < 32u ? Q.n : 32u;
+          uint32_t k;
+          if (Q.pop(&k)) {
+            const uint32_t m = geo.start_mods[k], r = geo.prow_of[k];
+            // the row's window again, now for the azimuth of a first anchor instead of the module
+            // centre: the module's half width drops out
+            float centre = 0.0f, halfw = 0.0f;
+            const float4 r1 = geo.prow_b1[r];
+            px_row_window(g, r1, geo.prow_b2[r], kp, sh, phi, z0, &centre, &halfw);
+            s.px_pair[pos + lane] = make_uint2(p, m);
+            s.px_win[pos + lane] = make_float2(wrap_f(centre - geo.phic[m]), halfw - r1.x + 1e-4f);
+          }
+          pos += take;
+        }
       }
+      __syncwarp();
     } else {
       const float pt = s.seed_pt[p], phi = s.seed_phi[p], z0 = s.seed_z0[p];
       const float kp = -(float)s.seed_q[p] * (float)g.kB / (2.0f * pt);
@@ -156,11 +169,14 @@ void launch_pixel(const Ctx &c, const SlotDev &s, cudaStream_t st) {
   const int warps_per_block = 8;
   int g = (int)((s.cap_seeds + warps_per_block - 1) / warps_per_block);
   if (g > c.n_sm * 8) g = c.n_sm * 8;
-  const size_t shb = 8 * ((size_t)(c.geo.n_start + 31) / 32) * sizeof(uint32_t);
-  if (shb > 48 * 1024) cudaFuncSetAttribute(k_px_modules<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shb);
+  const size_t shb = 8 * std::max<size_t>((size_t)(c.geo.n_start + 31) / 32, 64) * sizeof(uint32_t);   // >= 64 words per warp (queue of the fill pass)
+  if (shb > 48 * 1024) {
+    cudaFuncSetAttribute(k_px_modules<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shb);
+    cudaFuncSetAttribute(k_px_modules<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shb);
+  }
   k_px_modules<false><<<g, 256, shb, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_px_modules<false>");
   k_px_offsets<<<1, 1024, 0, st>>>(s); LST_MARK(c, st, "k_px_offsets");
-  k_px_modules<true><<<g, 256, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_px_modules<true>");
+  k_px_modules<true><<<g, 256, shb, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_px_modules<true>");
   launch_join(c, s, 2, st);            // pT5
   launch_row_offsets(c, s, 4, st);
   launch_join(c, s, 3, st);            // pT3

@@ -310,6 +310,10 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.pid_key = w.take<unsigned long long>(s.pid_size);
   s.pls_slot = w.take<uint32_t>(4 * (size_t)nsd);
   s.pid_has5 = w.take<uint8_t>(2 * (size_t)s.pid_size); s.pid_has3 = s.pid_has5 ? s.pid_has5 + s.pid_size : nullptr;
+  s.pls_min5 = w.take<unsigned long long>(3 * (size_t)nsd);      // min5 | min3 | best5, best3
+  s.pls_min3 = s.pls_min5 ? s.pls_min5 + nsd : nullptr;
+  s.pls_best5 = s.pls_min5 ? (uint32_t *)(s.pls_min5 + 2 * (size_t)nsd) : nullptr;
+  s.pls_best3 = s.pls_best5 ? s.pls_best5 + nsd : nullptr;
   s.pls_has5 = w.take<uint8_t>(3 * (size_t)nsd);
   s.pls_has3 = s.pls_has5 ? s.pls_has5 + nsd : nullptr; s.pls_near_t5 = s.pls_has5 ? s.pls_has5 + 2 * (size_t)nsd : nullptr;
   s.hit_used5 = w.take<uint8_t>(2 * (size_t)nh); s.hit_used3 = s.hit_used5 ? s.hit_used5 + nh : nullptr;

@@ -78,6 +78,7 @@ struct Header {          // per slot, device; zeroed (except n_hits / n_seeds) a
   uint32_t n_dd;                     // T5 + pT5 + pT3 objects entering the cleaning
   uint32_t n_flag;                   // pT5 + pT3 + T5 + seeds: length of the TC keep-flag array
   uint32_t n_inc;                    // 3 * n_hits: rows of the (hit, object type) -> objects incidence
+  uint32_t n_heavy;                  // objects k_s0 handed to k_s0_heavy (listed in tc_pos, free until S3)
   unsigned long long cand[S_NSTAGE]; // candidates enumerated per stage
 };
 
@@ -191,6 +192,9 @@ struct SlotDev {
   uint8_t *pid_has5, *pid_has3;    // [pid_size] each, contiguous
   uint32_t pid_size;               // power of two >= 8 * cap_seeds
   uint8_t *pls_has5, *pls_has3, *pls_near_t5;   // [cap_seeds] each, contiguous
+  unsigned long long *pls_min5, *pls_min3;      // [cap_seeds] bit pattern of the seed's minimum pT5 / pT3 score
+  uint32_t *pls_best5, *pls_best3;              // [cap_seeds] the seed's best pT5 / pT3 (index in its collection), or ~0
+                                                // (the four arrays are contiguous: one memset)
   uint8_t *hit_used5, *hit_used3;  // [cap_hits] each, contiguous: hit belongs to a surviving pT5 / pT3 (S1, S2)
   uint32_t *tc_flag, *tc_pos;      // [cap_tc+1]
   uint32_t *scan_part;             // [kScanBlocks+2]: block partials, total; last word = ticket
