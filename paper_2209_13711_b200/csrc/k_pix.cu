@@ -83,12 +83,21 @@ __global__ void __launch_bounds__(256) k_px_modules(GeoDev geo, SlotDev s, Param
       uint32_t pos = s.px_off[p];
       WarpQueue Q;
       Q.init(wbits);                  // 64 words of this warp's shared area (nw >= 64 is not needed: see launch)
-      for (uint32_t w = 0; w <= nw; ++w) {
-        if (w < nw) {
-          const uint32_t b = bits[w];
-          Q.push(((b >> lane) & 1u) != 0u, w * 32 + lane);
-        }
-        while (Q.n >= 32u || (w == nw && Q.n > 0u)) {
+      for (uint32_t wb = 0; wb <= nw; wb += 32) {
+        // 32 words at a time, only the non-empty ones are expanded (a seed reaches ~6 of 2 588 modules)
+        const uint32_t myw = wb + lane < nw ? bits[wb + lane] : 0u;
+        uint32_t nz = __ballot_sync(0xffffffffu, myw != 0u);
+        const bool last = wb + 32 > nw;
+        // expand the next non-empty word until 32 rows are queued (or the seed is finished), then drain
+        for (;;) {
+          if (!(Q.n >= 32u || (last && nz == 0u && Q.n > 0u))) {
+            if (nz == 0u) break;
+            const int src = __ffs(nz) - 1;
+            nz &= nz - 1;
+            const uint32_t b = __shfl_sync(0xffffffffu, myw, src);
+            Q.push(((b >> lane) & 1u) != 0u, (wb + src) * 32 + lane);
+            continue;
+          }
           const uint32_t take = Q.n < 32u ? Q.n : 32u;
           uint32_t k;
           if (Q.pop(&k)) {
