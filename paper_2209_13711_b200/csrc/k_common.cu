@@ -157,10 +157,16 @@ __global__ void k_emit_items(SlotDev s, int stage, int rows_level) {
     hdr->cand[stage] = sh_cand;
     if (overflow) atomicOr(&hdr->err, (uint32_t)ERR_CAP_ITEMS);
   }
-  if (overflow) return;
-  // one thread per ITEM (a heavy module owns hundreds of items): find its group in g_item0
-  __syncthreads();
-  for (uint32_t i = threadIdx.x; i < carry; i += blockDim.x) {
+}
+
+// One thread per ITEM (a heavy module owns hundreds of items) and per UNIT: find its group in the
+// offsets k_emit_items wrote; many blocks (the binary searches are latency bound).
+__global__ void __launch_bounds__(256) k_emit_fill(SlotDev s, int stage) {
+  const Header *hdr = s.hdr;
+  const StageBuf &st = s.st[stage];
+  const uint32_t ng = hdr->n_groups[stage], n_items = hdr->n_items[stage], n_units = hdr->n_units[stage];
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nt = gridDim.x * blockDim.x;
+  for (uint32_t i = tid; i < n_items; i += nt) {
     uint32_t lo = 0, hi = ng;            // last g with g_item0[g] <= i (empty groups repeat an offset)
     while (hi - lo > 1) {
       const uint32_t mid = (lo + hi) >> 1;
@@ -175,13 +181,13 @@ __global__ void k_emit_items(SlotDev s, int stage, int rows_level) {
       it.i0 = k * rpi; it.j0 = 0;
       it.nrows = (uint16_t)min(rpi, R - k * rpi); it.nj = (uint16_t)W;
     } else {
-      const uint32_t nt = (W + kItemCand - 1) / kItemCand;
-      it.i0 = k / nt; it.j0 = (k % nt) * kItemCand;
+      const uint32_t nt2 = (W + kItemCand - 1) / kItemCand;
+      it.i0 = k / nt2; it.j0 = (k % nt2) * kItemCand;
       it.nrows = 1; it.nj = (uint16_t)min((uint32_t)kItemCand, W - it.j0);
     }
     st.items[i] = it;
   }
-  for (uint32_t u = threadIdx.x; u < ucarry; u += blockDim.x) {   // one thread per UNIT: its group
+  for (uint32_t u = tid; u < n_units; u += nt) {   // one thread per UNIT: its group
     uint32_t lo = 0, hi = ng;
     while (hi - lo > 1) {
       const uint32_t mid = (lo + hi) >> 1;
@@ -289,10 +295,13 @@ void launch_index(const Ctx &c, const SlotDev &s, cudaStream_t st) {
 
 static const char *const kEmitName[S_NSTAGE] = {"k_emit_items[MD]", "k_emit_items[LS]", "k_emit_items[T3]",
                                                   "k_emit_items[T5]", "k_emit_items[pT5]", "k_emit_items[pT3]"};
+static const char *const kEmitFillName[S_NSTAGE] = {"k_emit_fill[MD]", "k_emit_fill[LS]", "k_emit_fill[T3]",
+                                                      "k_emit_fill[T5]", "k_emit_fill[pT5]", "k_emit_fill[pT3]"};
 static const char *const kScanName[S_NSTAGE] = {"k_scan_items[MD]", "k_scan_items[LS]", "k_scan_items[T3]",
                                                   "k_scan_items[T5]", "k_scan_items[pT5]", "k_scan_items[pT3]"};
 void launch_emit(const Ctx &c, const SlotDev &s, int stage, int rows_level, cudaStream_t st) {
   k_emit_items<<<1, 1024, 0, st>>>(s, stage, rows_level); LST_MARK(c, st, kEmitName[stage]);
+  k_emit_fill<<<c.n_sm, 256, 0, st>>>(s, stage); LST_MARK(c, st, kEmitFillName[stage]);
 }
 void launch_scan_items(const Ctx &c, const SlotDev &s, int stage, int level, uint32_t cap, cudaStream_t st) {
   k_scan_items<<<1, 1024, 0, st>>>(s, stage, level, cap); LST_MARK(c, st, kScanName[stage]);
