@@ -166,14 +166,19 @@ __device__ __forceinline__ uint32_t map_col_to_md(const MapRow &mr, uint32_t j) 
 //   tier 1 (ls_tier1_f: no division / sqrt / atan, ~82 % rejected) on every candidate,
 //   tier 2 (ls_pre_f, full fp32) on 32 queued survivors at a time,
 //   the fp64 decision on 32 queued tier-2 survivors at a time (~3 % of the candidates).
+struct LsWarpMem {                    // the warps' queues: live only in the candidate phase of a unit
+  uint32_t q1[kThreads / 32][64];
+  ClStage cl[kThreads / 32];
+};
 struct LsShared {
-  MapRow mr;
+  union {                             // the map row is needed only while the columns are staged
+    MapRow mr;
+    LsWarpMem w;
+  };
   float4 c_pos[kItemCand];
   uint32_t c_idc[kItemCand];          // MD index | category << 30
   float4 r_pos[kUnitRows];
   uint32_t r_idc[kUnitRows];
-  uint32_t q1[kThreads / 32][64];
-  ClStage cl[kThreads / 32];
   float4 tab[4];                      // per category: sig_z, sig_r, sig_t
 };
 
@@ -204,9 +209,9 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
   constexpr int kWarps = kThreads / 32;
   if (tid < 4) sh.tab[tid] = make_float4(g.f_sig_z[tid], g.f_sig_r[tid], g.f_sig_t[tid], 0.0f);
   WarpQueue Q1;
-  Q1.init(sh.q1[wib]);
+  Q1.init(sh.w.q1[wib]);
   ClBuf cl;
-  cl.init(&sh.cl[wib]);
+  cl.init(&sh.w.cl[wib]);
   __shared__ uint32_t sh_unit[2];
   for (;;) {
     __syncthreads();                            // the previous unit is done with the shared arrays
@@ -272,8 +277,8 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
 #undef LST_LS_ROWS
     }
     while (Q1.n) ls_stage2(sh, s, g, Q1, cl, rpi, nj, it0, nct);
+    cl.flush_all(s.hdr, st, S_LS);      // the queues' memory is the next unit's map row
   }
-  cl.flush_all(s.hdr, st, S_LS);
 }
 
 // fp64 decision of the listed candidates, one thread each (dense warps, no staging); an accepted
