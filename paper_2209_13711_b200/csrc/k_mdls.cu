@@ -63,39 +63,36 @@ __global__ void __launch_bounds__(128) k_md_decide(GeoDev geo, SlotDev s, Params
       const Pt pl = make_pt(l.x, l.y, l.z, cat), pu = make_pt(u.x, u.y, u.z, cat);
       pass = md_eval_d(g, pl, pu, cat, &o);
     }
-    const uint32_t pos = pool_reserve(hdr, st, S_MD, pass);
-    if (pass) atomicOr(&st.mask[(size_t)(key / kItemCand) * kItemWords + ((key % kItemCand) >> 5)], 1u << (key & 31u));
-    if (pos != 0xFFFFFFFFu) {
-      st.pkey[pos] = key;
-      st.p_d2[pos] = make_double2(o.kappa, o.sigk);
-      st.p_f4[pos] = make_float4((float)o.dphi, 0.f, 0.f, 0.f);
+    if (pass) {
+      atomicOr(&st.mask[(size_t)(key / kItemCand) * kItemWords + ((key % kItemCand) >> 5)], 1u << (key & 31u));
+      st.p_d2[j] = make_double2(o.kappa, o.sigk);
+      st.p_f4[j] = make_float4((float)o.dphi, 0.f, 0.f, 0.f);
     }
   }
 }
 
-// One thread per pool entry: canonical position, the cheap fields re-derived from the item.
+// One thread per listed pair: the accepted ones move to their canonical position.
 __global__ void __launch_bounds__(256) k_md_fill(GeoDev geo, SlotDev s) {
   const StageBuf &st = s.st[S_MD];
   const Header *hdr = s.hdr;
   if (hdr->n_obj[0] == 0) return;                            // nothing built, or overflow (level emptied)
-  const uint32_t n = hdr->pool_used[S_MD];
+  const uint32_t n = min(hdr->cl_used[S_MD], st.cap_cl);
   for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
-    uint32_t it, c;
-    const uint32_t idx = pool_target(st, st.pkey[j], &it, &c);
-    const Item item = st.items[it];
-    const uint32_t m = item.group;
-    const uint32_t nj = item.nj, r = c / nj, jj = c - r * nj;
-    const uint32_t hl = s.det_off[2 * m] + item.i0 + r, hu = s.det_off[2 * m + 1] + item.j0 + jj;
-    const float4 l = s.hit[hl];
+    const uint32_t key = st.cl_key[j];
+    const uint32_t idx = pool_target(st, key);
+    if (idx == 0xFFFFFFFFu) continue;
+    const uint32_t m = st.items[key / kItemCand].group;
+    const uint2 h = st.cl_ab[j];
+    const float4 l = s.hit[h.x];
     const double2 kd = st.p_d2[j];
     s.md_pos[idx] = l;
     s.md_kd[idx] = kd;
     s.md_kf[idx] = make_float2((float)kd.x, (float)kd.y);
-    s.md_hit[idx] = make_uint2(hl, hu);
+    s.md_hit[idx] = h;
     s.md_mod[idx] = (m << 2) | (uint32_t)geo.category[m];
     s.md_dphi[idx] = st.p_f4[j].x;
     s.md_phi[idx] = atan2f(l.y, l.x);
-    s.md_prel[idx] = s.hit_key[hl];
+    s.md_prel[idx] = s.hit_key[h.x];
   }
 }
 
@@ -300,12 +297,9 @@ __global__ void __launch_bounds__(128) k_ls_decide(SlotDev s, Params g) {
       const Pt pa = make_pt(a.x, a.y, a.z, (int)(s.md_mod[ab.x] & 3u)), pb = make_pt(b.x, b.y, b.z, (int)(s.md_mod[ab.y] & 3u));
       pass = ls_eval_d(g, pa, ka.x, ka.y, pb, kb.x, kb.y, &o);
     }
-    const uint32_t pos = pool_reserve(hdr, st, S_LS, pass);
-    if (pass) atomicOr(&st.mask[(size_t)(key / kItemCand) * kItemWords + ((key % kItemCand) >> 5)], 1u << (key & 31u));
-    if (pos != 0xFFFFFFFFu) {
-      st.pkey[pos] = key;
-      st.p_ab[pos] = ab;
-      st.p_f4[pos] = make_float4((float)o.dphi, (float)o.kappa, (float)o.sigk, 0.0f);
+    if (pass) {
+      atomicOr(&st.mask[(size_t)(key / kItemCand) * kItemWords + ((key % kItemCand) >> 5)], 1u << (key & 31u));
+      st.p_f4[j] = make_float4((float)o.dphi, (float)o.kappa, (float)o.sigk, 0.0f);
     }
   }
 }
@@ -315,11 +309,11 @@ __global__ void __launch_bounds__(256) k_ls_fill(SlotDev s) {
   const StageBuf &st = s.st[S_LS];
   const Header *hdr = s.hdr;
   if (hdr->n_obj[1] == 0) return;
-  const uint32_t n = hdr->pool_used[S_LS];
+  const uint32_t n = min(hdr->cl_used[S_LS], st.cap_cl);
   for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
-    uint32_t it, c;
-    const uint32_t idx = pool_target(st, st.pkey[j], &it, &c);
-    s.ls_md[idx] = st.p_ab[j];
+    const uint32_t idx = pool_target(st, st.cl_key[j]);
+    if (idx == 0xFFFFFFFFu) continue;
+    s.ls_md[idx] = st.cl_ab[j];
     s.ls_f[idx] = st.p_f4[j];
   }
 }

@@ -315,33 +315,22 @@ __global__ void __launch_bounds__(128) k_join_decide(GeoDev geo, SlotDev s, Para
     if (KIND == J_T3) {
       T3Out o;
       if (live) pass = t3_candidate(s, g, ab.x, ab.y, &o, nullptr);
-      const uint32_t pos = pool_reserve(hdr, st, stage, pass);
-      if (pos != 0xFFFFFFFFu) {
-        st.pkey[pos] = key;
-        st.p_ab[pos] = ab;
-        st.p_d2[pos] = make_double2(o.kappa3, o.sigk3);
-        st.p_f4[pos] = make_float4((float)o.beta, 0.f, 0.f, 0.f);
+      if (pass) {
+        st.p_d2[j] = make_double2(o.kappa3, o.sigk3);
+        st.p_f4[j] = make_float4((float)o.beta, 0.f, 0.f, 0.f);
       }
     } else if (KIND == J_T5) {
       T5Out o;
       if (live) pass = t5_candidate(s, g, ab.x, ab.y, &o, nullptr, nullptr, nullptr);
-      const uint32_t pos = pool_reserve(hdr, st, stage, pass);
-      if (pos != 0xFFFFFFFFu) {
-        st.pkey[pos] = key;
-        st.p_ab[pos] = ab;
-        st.p_d2[pos] = make_double2(o.eta, o.phi);
-        st.p_d2b[pos] = make_double2(o.chi2, o.R);
-        st.p_f4[pos] = make_float4((float)o.pt, 0.f, 0.f, 0.f);
+      if (pass) {
+        st.p_d2[j] = make_double2(o.eta, o.phi);
+        st.p_d2b[j] = make_double2(o.chi2, o.R);
+        st.p_f4[j] = make_float4((float)o.pt, 0.f, 0.f, 0.f);
       }
     } else {
       double c2 = 0.0;
       if (live) pass = px_candidate<KIND>(geo, s, g, ab.x, ab.y, &c2);
-      const uint32_t pos = pool_reserve(hdr, st, stage, pass);
-      if (pos != 0xFFFFFFFFu) {
-        st.pkey[pos] = key;
-        st.p_ab[pos] = ab;
-        st.p_d2[pos] = make_double2(c2, 0.0);
-      }
+      if (pass) st.p_d2[j] = make_double2(c2, 0.0);
     }
     if (pass) atomicOr(&st.mask[(size_t)(key / kItemCand) * kItemWords + ((key % kItemCand) >> 5)], 1u << (key & 31u));
   }
@@ -354,11 +343,11 @@ __global__ void __launch_bounds__(256) k_join_fill(SlotDev s) {
   const StageBuf &st = s.st[stage];
   const Header *hdr = s.hdr;
   if (hdr->n_obj[JoinTraits<KIND>::out_level] == 0) return;
-  const uint32_t n = hdr->pool_used[stage];
+  const uint32_t n = min(hdr->cl_used[stage], st.cap_cl);
   for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
-    uint32_t it, c;
-    const uint32_t idx = pool_target(st, st.pkey[j], &it, &c);
-    const uint2 ab = st.p_ab[j];
+    const uint32_t idx = pool_target(st, st.cl_key[j]);
+    if (idx == 0xFFFFFFFFu) continue;
+    const uint2 ab = st.cl_ab[j];
     if (KIND == J_T3) {
       const uint2 la = s.ls_md[ab.x], lb = s.ls_md[ab.y];
       s.t3_md[idx] = make_uint4(la.x, la.y, lb.y, 0u);

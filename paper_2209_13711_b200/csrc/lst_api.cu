@@ -342,14 +342,12 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
     b.item_cnt = w.take<uint32_t>(b.cap_items); b.item_base = w.take<uint32_t>(b.cap_items);
     const uint32_t pool_cap[S_NSTAGE] = {s.cap_md, s.cap_ls, s.cap_t3, s.cap_t5, s.cap_pt5, s.cap_pt3};
     b.cap_pool = pool_cap[k];
-    b.pkey = w.take<uint32_t>(b.cap_pool);
-    b.p_ab = w.take<uint2>(b.cap_pool);
-    b.p_d2 = w.take<double2>(b.cap_pool);
-    b.p_d2b = k == S_T5 ? w.take<double2>(b.cap_pool) : nullptr;
-    b.p_f4 = w.take<float4>(b.cap_pool);
     b.cap_cl = 2 * b.cap_pool + 4096;
     b.cl_key = w.take<uint32_t>(b.cap_cl);
     b.cl_ab = w.take<uint2>(b.cap_cl);
+    b.p_d2 = w.take<double2>(b.cap_cl);
+    b.p_d2b = k == S_T5 ? w.take<double2>(b.cap_cl) : nullptr;
+    b.p_f4 = w.take<float4>(b.cap_cl);
   }
   // export scratch: the largest level
   size_t obj_cap = std::max({(size_t)s.cap_md, (size_t)s.cap_ls, (size_t)s.cap_t3, (size_t)s.cap_t5,

@@ -92,12 +92,11 @@ struct StageBuf {        // work list of one stage
   uint16_t *wpre;        // [cap_items * kItemWords] pass count of the item's words before this one
   uint32_t *item_cnt;    // [cap_items] pass count
   uint32_t *item_base;   // [cap_items] exclusive prefix
-  // pool: what the eval kernel computed for each accepted candidate, in arrival order; the fill
-  // kernel moves entry j to its canonical position item_base[item] + rank of the candidate
-  uint32_t *pkey;        // [cap_pool] item * kItemCand + candidate
-  uint2 *p_ab;           // [cap_pool] constituent indices
-  double2 *p_d2, *p_d2b; // [cap_pool] fp64 results (p_d2b: T5 only)
-  float4 *p_f4;          // [cap_pool] fp32 results
+  // pool: what the decide kernel computed for accepted candidate j of the candidate list (same
+  // index j: no counter, no atomics); the fill kernel moves the entries whose pass bit is set to their
+  // canonical position item_base[item] + rank of the candidate
+  double2 *p_d2, *p_d2b; // [cap_cl] fp64 results (p_d2b: T5 only)
+  float4 *p_f4;          // [cap_cl] fp32 results
   // candidate list: survivors of the cheap pre-filter kernel, decided in fp64 by the decide kernel
   uint32_t *cl_key;      // [cap_cl] item * kItemCand + candidate
   uint2 *cl_ab;          // [cap_cl] the pair (row object, column object)
@@ -413,12 +412,14 @@ struct ClBuf {
   }
 };
 
-// fill: canonical index of pool entry `key` = item * kItemCand + candidate
-__device__ __forceinline__ uint32_t pool_target(const StageBuf &st, uint32_t key, uint32_t *item, uint32_t *cand) {
+// fill: canonical index of listed candidate `key` = item * kItemCand + candidate, or 0xFFFFFFFF if
+// the decide kernel did not accept it (its pass bit is clear)
+__device__ __forceinline__ uint32_t pool_target(const StageBuf &st, uint32_t key) {
   const uint32_t it = key / (uint32_t)kItemCand, c = key % (uint32_t)kItemCand;
   const size_t w = (size_t)it * kItemWords + (c >> 5);
-  *item = it; *cand = c;
-  return st.item_base[it] + st.wpre[w] + __popc(st.mask[w] & ((1u << (c & 31)) - 1u));
+  const uint32_t m = st.mask[w];
+  if (!((m >> (c & 31)) & 1u)) return 0xFFFFFFFFu;
+  return st.item_base[it] + st.wpre[w] + __popc(m & ((1u << (c & 31)) - 1u));
 }
 
 }  // namespace lst
