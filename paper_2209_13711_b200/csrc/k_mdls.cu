@@ -11,12 +11,12 @@ namespace lst {
 // k_md_decide: one thread per listed pair, fp64 decision; accepted pairs set their pass bit and
 // write kappa, sigma_kappa and dphi to the pool.
 __global__ void __launch_bounds__(256) k_md_eval(GeoDev geo, SlotDev s, Params g) {
-  __shared__ ClStage cl_mem[256 / 32];
+  __shared__ ClStageT<64> cl_mem[256 / 32];
   const StageBuf &st = s.st[S_MD];
   const uint32_t n_items = s.hdr->n_items[S_MD];
   const int lane = threadIdx.x & 31;
   const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
-  ClBuf cl;
+  ClBufT<64> cl;
   cl.init(&cl_mem[threadIdx.x >> 5]);
   constexpr int kSlices = 8, kSliceCand = kItemCand / kSlices;   // a warp task = 128 candidates of an item
   for (uint32_t w = warp; w < n_items * kSlices; w += nwarp) {

@@ -264,9 +264,9 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
   __shared__ RowTab rt;
   __shared__ uint32_t sh[33];
   __shared__ float4 rowseed[(KIND == J_PT5 || KIND == J_PT3) ? kRowChunk : 1];
-  __shared__ ClStage cl_mem[kThreads / 32];
+  __shared__ ClStageT<64> cl_mem[kThreads / 32];
   (void)geo;
-  ClBuf cl;
+  ClBufT<64> cl;
   cl.init(&cl_mem[threadIdx.x >> 5]);
   const int stage = JoinTraits<KIND>::stage;
   const StageBuf &st = s.st[stage];

@@ -72,7 +72,6 @@ struct Header {          // per slot, device; zeroed (except n_hits / n_seeds) a
   uint32_t n_groups[S_NSTAGE];
   uint32_t n_units[S_NSTAGE];        // work units (k_emit_items): item runs that share their columns
   uint32_t next_unit[S_NSTAGE];      // dynamic work distribution: next unit to hand out
-  uint32_t pool_used[S_NSTAGE];      // accepted candidates written to the stage's pool so far
   uint32_t cl_used[S_NSTAGE];        // pre-filter survivors appended to the stage's candidate list
   uint32_t err;
   uint32_t n_dd;                     // T5 + pT5 + pT3 objects entering the cleaning
@@ -338,79 +337,54 @@ __device__ __forceinline__ void publish_mask(const ItemScratch &s, const StageBu
   if (threadIdx.x < 32) publish_item(st, it, s.mask[threadIdx.x]);
 }
 
-// eval: reserve pool entries for the lanes of a warp whose candidate passed (all 32 lanes call).
-// Returns the lane's pool index, or 0xFFFFFFFF (not passed, or the pool is full: flagged, the level
-// is then emptied by k_scan_items, never truncated).
-__device__ __forceinline__ uint32_t pool_reserve(Header *hdr, const StageBuf &st, int stage, bool pass) {
-  const uint32_t b = __ballot_sync(0xffffffffu, pass);
-  if (b == 0) return 0xFFFFFFFFu;
-  const int lane = threadIdx.x & 31, leader = __ffs(b) - 1;
-  uint32_t base = 0;
-  if (lane == leader) base = atomicAdd(&hdr->pool_used[stage], (uint32_t)__popc(b));
-  base = __shfl_sync(0xffffffffu, base, leader);
-  const uint32_t pos = base + __popc(b & ((1u << lane) - 1u));
-  if (!pass) return 0xFFFFFFFFu;
-  if (pos >= st.cap_pool) { atomicOr(&hdr->err, (uint32_t)ERR_CAP_OBJ); return 0xFFFFFFFFu; }
-  return pos;
-}
-// pre-filter kernels: append the surviving lanes' candidates to the stage's list (all 32 lanes call)
-__device__ __forceinline__ void cl_append(Header *hdr, const StageBuf &st, int stage, bool keep, uint32_t key, uint2 ab) {
-  const uint32_t b = __ballot_sync(0xffffffffu, keep);
-  if (b == 0) return;
-  const int lane = threadIdx.x & 31, leader = __ffs(b) - 1;
-  uint32_t base = 0;
-  if (lane == leader) base = atomicAdd(&hdr->cl_used[stage], (uint32_t)__popc(b));
-  base = __shfl_sync(0xffffffffu, base, leader);
-  const uint32_t pos = base + __popc(b & ((1u << lane) - 1u));
-  if (!keep) return;
-  if (pos >= st.cap_cl) { atomicOr(&hdr->err, (uint32_t)ERR_CAP_ITEMS); return; }
-  st.cl_key[pos] = key;
-  st.cl_ab[pos] = ab;
-}
-
-// Warp-private staging of candidate-list entries (ring of 64 in shared memory): the sparse
-// survivors of many pre-filter iterations are appended 32 at a time, i.e. one atomic on the list
-// counter per 32 entries (the counter is a single address: per-iteration atomics serialise in L2).
-struct ClStage {
-  uint32_t key[64];
-  uint2 ab[64];
+// Warp-private staging of candidate-list entries (ring in shared memory): the sparse survivors of
+// many pre-filter iterations are appended BATCH at a time, i.e. one atomic on the list counter per
+// BATCH entries (the counter is a single address: per-iteration atomics serialise in L2).
+template <int BATCH>                 // 32 or 64; the ring holds BATCH + 32 .. 2 * BATCH entries
+struct ClStageT {
+  uint32_t key[2 * BATCH];
+  uint2 ab[2 * BATCH];
 };
-struct ClBuf {
-  ClStage *m;
+template <int BATCH>
+struct ClBufT {
+  ClStageT<BATCH> *m;
   uint32_t head, n;
-  __device__ __forceinline__ void init(ClStage *mem) { m = mem; head = 0; n = 0; }
+  static constexpr uint32_t kMask = 2 * BATCH - 1;
+  __device__ __forceinline__ void init(ClStageT<BATCH> *mem) { m = mem; head = 0; n = 0; }
   // all 32 lanes call; flushes a full batch when one is ready
   __device__ __forceinline__ void push(Header *hdr, const StageBuf &st, int stage, bool keep, uint32_t key, uint2 ab) {
     const uint32_t b = __ballot_sync(0xffffffffu, keep);
     if (b == 0) return;
     const int lane = threadIdx.x & 31;
     if (keep) {
-      const uint32_t p = (head + n + __popc(b & ((1u << lane) - 1u))) & 63u;
+      const uint32_t p = (head + n + __popc(b & ((1u << lane) - 1u))) & kMask;
       m->key[p] = key; m->ab[p] = ab;
     }
     n += __popc(b);
     __syncwarp();
-    if (n >= 32u) flush32(hdr, st, stage);
+    if (n >= (uint32_t)BATCH) flush(hdr, st, stage);
   }
-  __device__ __forceinline__ void flush32(Header *hdr, const StageBuf &st, int stage) {
+  __device__ __forceinline__ void flush(Header *hdr, const StageBuf &st, int stage) {
     const int lane = threadIdx.x & 31;
-    const uint32_t take = n < 32u ? n : 32u;
+    const uint32_t take = n < (uint32_t)BATCH ? n : (uint32_t)BATCH;
     uint32_t base = 0;
     if (lane == 0) base = atomicAdd(&hdr->cl_used[stage], take);
     base = __shfl_sync(0xffffffffu, base, 0);
-    if ((uint32_t)lane < take) {
-      const uint32_t p = (head + lane) & 63u, pos = base + lane;
+    for (uint32_t k = lane; k < take; k += 32) {
+      const uint32_t p = (head + k) & kMask, pos = base + k;
       if (pos < st.cap_cl) { st.cl_key[pos] = m->key[p]; st.cl_ab[pos] = m->ab[p]; }
       else atomicOr(&hdr->err, (uint32_t)ERR_CAP_ITEMS);
     }
     __syncwarp();
-    head = (head + take) & 63u;
+    head = (head + take) & kMask;
     n -= take;
   }
   __device__ __forceinline__ void flush_all(Header *hdr, const StageBuf &st, int stage) {
-    while (n) flush32(hdr, st, stage);
+    while (n) flush(hdr, st, stage);
   }
 };
+typedef ClStageT<32> ClStage;
+typedef ClBufT<32> ClBuf;
 
 // fill: canonical index of listed candidate `key` = item * kItemCand + candidate, or 0xFFFFFFFF if
 // the decide kernel did not accept it (its pass bit is clear)
