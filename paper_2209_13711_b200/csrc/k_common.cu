@@ -24,18 +24,17 @@ __global__ void k_hist(GeoDev geo, SlotDev s) {
 }
 
 // Exclusive scan of in[0..n) into out[0..n], out[n] = total; one block.
+// Each thread owns a contiguous chunk (serial sum, ONE block scan of the chunk sums, serial write):
+// two barriers in all instead of two per blockDim.x elements.  in == out is allowed.
 __device__ void block_scan_array(const uint32_t *in, uint32_t *out, uint32_t n, uint32_t *sh) {
-  uint32_t carry = 0;
-  for (uint32_t base = 0; base < n; base += blockDim.x) {
-    const uint32_t i = base + threadIdx.x;
-    const uint32_t v = i < n ? in[i] : 0u;
-    uint32_t tot;
-    const uint32_t e = block_excl_scan(v, sh, &tot);
-    if (i < n) out[i] = carry + e;
-    carry += tot;
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) out[n] = carry;
+  const uint32_t chunk = (n + blockDim.x - 1) / blockDim.x;
+  const uint32_t b0 = min(n, threadIdx.x * chunk), b1 = min(n, b0 + chunk);
+  uint32_t sum = 0;
+  for (uint32_t i = b0; i < b1; ++i) sum += in[i];
+  uint32_t tot;
+  uint32_t run = block_excl_scan(sum, sh, &tot);
+  for (uint32_t i = b0; i < b1; ++i) { const uint32_t v = in[i]; out[i] = run; run += v; }
+  if (threadIdx.x == 0) out[n] = tot;
 }
 
 // ------------------------------------------------------------------ a0.2 scan + MD groups
@@ -121,26 +120,26 @@ __global__ void k_emit_items(SlotDev s, int stage, int rows_level) {
   if (ng > st.cap_groups) ng = 0;   // cannot happen: cap_groups is sized from the object capacity
   if (threadIdx.x == 0) sh_cand = 0ull;
   __syncthreads();
-  uint32_t carry = 0, ucarry = 0;
+  // each thread owns a contiguous chunk of groups: serial sums, one block scan per quantity, serial write
   unsigned long long my_cand = 0;
-  for (uint32_t base = 0; base < ng; base += blockDim.x) {
-    const uint32_t g = base + threadIdx.x;
-    uint32_t ni = 0, nu = 0;
-    if (g < ng) {
-      const uint32_t R = st.gR[g], W = st.gW[g];
-      ni = items_of(R, W);
-      nu = units_of(R, W);
-      my_cand += (unsigned long long)R * W;
-    }
-    uint32_t tot;
-    const uint32_t e = block_excl_scan(ni, sh, &tot);
-    if (g < ng) st.g_item0[g] = carry + e;
-    carry += tot;
-    __syncthreads();
-    const uint32_t eu = block_excl_scan(nu, sh, &tot);
-    if (g < ng) st.g_unit0[g] = ucarry + eu;
-    ucarry += tot;
-    __syncthreads();
+  const uint32_t chunk = (ng + blockDim.x - 1) / blockDim.x;
+  const uint32_t g0 = min(ng, threadIdx.x * chunk), g1 = min(ng, g0 + chunk);
+  uint32_t si = 0, su = 0;
+  for (uint32_t g = g0; g < g1; ++g) {
+    const uint32_t R = st.gR[g], W = st.gW[g];
+    si += items_of(R, W);
+    su += units_of(R, W);
+    my_cand += (unsigned long long)R * W;
+  }
+  uint32_t carry, ucarry;
+  uint32_t ri = block_excl_scan(si, sh, &carry);
+  __syncthreads();
+  uint32_t ru = block_excl_scan(su, sh, &ucarry);
+  for (uint32_t g = g0; g < g1; ++g) {
+    const uint32_t R = st.gR[g], W = st.gW[g];
+    st.g_item0[g] = ri; st.g_unit0[g] = ru;
+    ri += items_of(R, W);
+    ru += units_of(R, W);
   }
   // block sum of the candidate counts (64-bit shared atomics are CAS loops: reduce per warp first)
 #pragma unroll
@@ -219,16 +218,13 @@ __global__ void k_scan_items(SlotDev s, int stage, int level, uint32_t cap) {
   Header *hdr = s.hdr;
   const StageBuf &st = s.st[stage];
   const uint32_t n = hdr->n_items[stage];
-  uint32_t carry = 0;
-  for (uint32_t base = 0; base < n; base += blockDim.x) {
-    const uint32_t i = base + threadIdx.x;
-    const uint32_t v = i < n ? st.item_cnt[i] : 0u;
-    uint32_t tot;
-    const uint32_t e = block_excl_scan(v, sh, &tot);
-    if (i < n) st.item_base[i] = carry + e;
-    carry += tot;
-    __syncthreads();
-  }
+  const uint32_t chunk = (n + blockDim.x - 1) / blockDim.x;
+  const uint32_t b0 = min(n, threadIdx.x * chunk), b1 = min(n, b0 + chunk);
+  uint32_t sum = 0;
+  for (uint32_t i = b0; i < b1; ++i) sum += st.item_cnt[i];
+  uint32_t carry;
+  uint32_t run = block_excl_scan(sum, sh, &carry);
+  for (uint32_t i = b0; i < b1; ++i) { st.item_base[i] = run; run += st.item_cnt[i]; }
   if (threadIdx.x == 0) {
     if (carry > cap) {
       atomicOr(&hdr->err, (uint32_t)ERR_CAP_OBJ);
