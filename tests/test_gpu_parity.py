@@ -383,3 +383,81 @@ def test_config5_slots_streams_match_oracle_and_single_slot(B, geom_full, map_fu
     if near == 0:
         assert compare_cleaning(o, _View(), e) > 100
     lst.close()
+
+
+# ------------------------------------------------------------------ full size, bench launch configuration
+def test_config4h_all_seeds_bench_configuration_sampled(B, geom_full, map_full):
+    """The bench workload as bench.py runs it: one cfg4h event with ALL its ~5.9 k seeds on a non-zero
+    slot of an 8-slot context, on its own stream, graph replayed (second run of the slot).  The
+    oracle's all-pairs pixel linking over every seed takes minutes, so the outputs are checked on
+    samples the oracle evaluates one by one: sampled MD / LS / T3 / T5 / pT3 / pT5 objects must be
+    accepted by the oracle (or lie in the 1e-5 band), sampled (seed, T3 / T5) pairs that are NOT in
+    the output must be rejected, and the levels the oracle finishes in seconds (MD..T5) are compared
+    in full."""
+    import torch
+    ev = lstgen.make_event(geom_full, "cfg4h", seed=1000)
+    sd = (ev.seed_pt, ev.seed_eta, ev.seed_phi, ev.seed_z0, ev.seed_q, ev.seed_hit_ids)
+    lst = B.LST(geom_full, map_full[0], map_full[1], n_slots=8, max_hits=ev.n_hits, max_seeds=ev.n_seeds)
+    st = torch.cuda.Stream()
+    slot = 5
+    for _ in range(2):                      # the second run replays the slot's CUDA graph
+        lst.lst_load_event(slot, ev.x, ev.y, ev.z, ev.det, sd, stream=st)
+        lst.lst_run(slot, stream=st)
+    cnt, cand = lst.lst_get_counts(slot)
+    o = O.Oracle(geom_full, map_full[0], map_full[1])
+    o.load(ev)
+    o.run(upto=O.T5)
+    got = {}
+    for lvl in CHAIN:                       # full comparison of what the oracle builds in seconds
+        ref, g = o.get(lvl), lst.lst_get_objects(slot, lvl)
+        got[lvl] = g
+        sr, sg = set(_keys(lvl, ref)), set(_keys(lvl, g))
+        diff = sr ^ sg
+        for t in diff:
+            assert o.eval(lvl, t)[1] < BAND
+        assert len(diff) <= MAX_NEAR_FRAC * max(len(sr), 1)
+        assert cnt[lvl] == len(g["hits"]) > 10000
+    rng = np.random.default_rng(7)
+    near = 0
+    for lvl, base in ((O.PT3, O.T3), (O.PT5, O.T5)):
+        g = lst.lst_get_objects(slot, lvl)
+        h, pls = g["hits"].astype(np.int64), g["parents"][:, 0].astype(np.int64)
+        assert cnt[lvl] == len(h) > 5000
+        keys = set(zip(pls.tolist(), map(tuple, h.tolist())))
+        assert len(keys) == len(h)
+        for i in rng.choice(len(h), 1500, replace=False):            # accepted pairs: the oracle accepts them too
+            ok, margin = o.eval(lvl, h[i], int(pls[i]))
+            if not ok:
+                assert margin < BAND, (O.LEVEL_NAMES[lvl], i, margin)
+                near += 1
+        bh = got[base]["hits"].astype(np.int64)
+        tested = 0
+        while tested < 1500:                                         # pairs not in the output: the oracle rejects them
+            p, j = int(rng.integers(ev.n_seeds)), int(rng.integers(len(bh)))
+            if (p, tuple(bh[j].tolist())) in keys:
+                continue
+            ok, margin = o.eval(lvl, bh[j], p)
+            if ok:
+                assert margin < BAND, (O.LEVEL_NAMES[lvl], p, j, margin)
+                near += 1
+            tested += 1
+        # the neighbours of accepted pairs are the hard negatives: same seed, another object with the same first hit
+        first = {}
+        for j, row in enumerate(bh[:, 0].tolist()):
+            first.setdefault(row, []).append(j)
+        tested = 0
+        for i in rng.permutation(len(h)):
+            for j in first.get(int(h[i, 0]), [])[:4]:
+                k = (int(pls[i]), tuple(bh[j].tolist()))
+                if k in keys:
+                    continue
+                ok, margin = o.eval(lvl, bh[j], int(pls[i]))
+                if ok:
+                    assert margin < BAND, (O.LEVEL_NAMES[lvl], k, margin)
+                    near += 1
+                tested += 1
+            if tested >= 1500:
+                break
+    assert near <= 3
+    assert cnt[O.TC] > 1000
+    lst.close()
