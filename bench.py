@@ -486,7 +486,8 @@ def main():
                              "step vs 126 MB L2" % (in_bytes / 1e6, a.slots, ws / 1e6),
                        "parallelism": "replicas only (no collective)", "objects_event0": {k: n[k] for k in (
                            "hits", "seeds", "md", "ls", "t3", "t5", "pt3", "pt5", "tc")},
-                       "candidates_event0": dict(zip(("md", "ls", "t3", "t5", "pt5", "pt3"), n["cand"][:6]))},
+                       "candidates_event0": dict(zip(("md", "ls", "t3", "t5", "pt5", "pt3"), n["cand"][:6])),
+                       "prefilter_survivors_event0": dict(zip(("md", "ls", "t3", "t5", "pt5", "pt3"), n["surv"][:6]))},
             "clocks": clocks,
             "gpu_launches": int(launches * a.events * a.steps),
             "launches_per_event": int(launches),

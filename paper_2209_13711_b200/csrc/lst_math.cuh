@@ -149,13 +149,13 @@ LST_HD bool md_pre_f(const Params &g, float xl, float yl, float zl, float rl, fl
                      float ru, int cat) {
   const float dx = xu - xl, dy = yu - yl, dz = zu - zl;
   const float dd = dx * dx + dy * dy;
-  const float drv = (2.0f * (xl * dx + yl * dy) + dd) / (rl + ru);
+  const float drv = LST_FDIV(2.0f * (xl * dx + yl * dy) + dd, rl + ru);
   const float cr = xl * dy - yl * dx;
   const float tolrr = g.f_ns * g.f_sig_t[cat] * (rl + ru);       // tolphi * rl * ru
   const float rr = rl * ru;
   if (!is_endcap(cat)) {
     if (drv < -1e-3f) return false;
-    const float t = drv / rl;
+    const float t = LST_FDIV(drv, rl);
     if (fabsf(dz - zl * t) > (g.f_z0max * t + 2.0f * g.f_ns * g.f_sig_z[cat]) * kPreSlack + 1e-4f) return false;
     if (fabsf(cr) > (g.f_kmax * sqrtf(dd) * rr + tolrr) * kPreSlack) return false;
   } else {
@@ -163,10 +163,10 @@ LST_HD bool md_pre_f(const Params &g, float xl, float yl, float zl, float rl, fl
     const float den = azl - g.f_z0max;
     if (den < 1e-3f) return true;  // let the fp64 guard decide
     const float adz = fabsf(dz);
-    if (fabsf(drv - rl * dz / zl) > (rl * adz * g.f_z0max / (azl * den) + 2.0f * g.f_ns * g.f_sig_r[cat]) * kPreSlack + 1e-4f)
+    if (fabsf(drv - LST_FDIV(rl * dz, zl)) > (LST_FDIV(rl * adz * g.f_z0max, azl * den) + 2.0f * g.f_ns * g.f_sig_r[cat]) * kPreSlack + 1e-4f)
       return false;
     const float asl = asinf(fminf(1.0f, g.f_kmax * rl));
-    if (fabsf(cr) > (adz * asl / den * rr + tolrr) * kPreSlack) return false;
+    if (fabsf(cr) > (LST_FDIV(adz * asl, den) * rr + tolrr) * kPreSlack) return false;
   }
   return true;
 }
