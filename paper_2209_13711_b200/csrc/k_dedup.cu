@@ -269,9 +269,6 @@ __global__ void __launch_bounds__(256) k_pls_best(SlotDev s) {
 constexpr int kS0Slots = 128;
 constexpr uint32_t kNoHit = 0xFFFFFFFFu;
 constexpr uint32_t kS0Light = 64;   // entries an 8-lane group looks at before it hands a longer object to k_s0_heavy
-__device__ __forceinline__ double dd_score(const SlotDev &s, uint32_t n5, uint32_t np5, uint32_t d) {
-  return d < n5 ? s.t5_chi2[d] : (d < n5 + np5 ? s.pt5_chi2[d - n5] : s.pt3_chi2[d - n5 - np5]);
-}
 __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
   __shared__ uint32_t sh_pre[16][12], sh_beg[16][12];
   __shared__ uint32_t sh_tab[16][kS0Slots];

@@ -408,7 +408,7 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   const size_t o_box = o_cols + up((size_t)std::max<uint32_t>(nnz, 1) * 4);
   const size_t box_stride = up((size_t)n * 4);
   const size_t o_start = o_box + 6 * box_stride;
-  const size_t o_sbox = o_start + up(std::max<size_t>(start_mods.size(), 1) * 4);
+  const size_t o_sbox = o_start + up(std::max<size_t>(start_mods.size(), 1) * 4);   // rows of start modules follow
   // rows of start modules (same box up to phic)
   std::vector<uint32_t> prow_off, prow_k;
   std::vector<float> prow_phic, prow_b;   // prow_b: 8 floats per row
@@ -440,7 +440,7 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
     prow_off.push_back((uint32_t)order.size());
   }
   const size_t n_prow = prow_off.size() - 1;
-  const size_t o_prow = o_sbox + 2 * up(std::max<size_t>(start_mods.size(), 1) * 16);
+  const size_t o_prow = o_sbox;
   const size_t o_prow2 = o_prow + up(std::max<size_t>(n_prow, 1) * 16);
   const size_t o_poff = o_prow2 + up(std::max<size_t>(n_prow, 1) * 16);
   const size_t o_pk = o_poff + up((n_prow + 1) * 4);
@@ -459,19 +459,6 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   if (!start_mods.empty())
     cudaMemcpy(d + o_start, start_mods.data(), start_mods.size() * 4, cudaMemcpyHostToDevice);
   {
-    std::vector<float> sb(8 * std::max<size_t>(start_mods.size(), 1), 0.0f);
-    float *b1 = sb.data(), *b2 = sb.data() + 4 * std::max<size_t>(start_mods.size(), 1);
-    for (size_t k = 0; k < start_mods.size(); ++k) {
-      const uint32_t m = start_mods[k];
-      b1[4 * k] = g->phic[m]; b1[4 * k + 1] = g->half_phi[m]; b1[4 * k + 2] = g->rmin[m]; b1[4 * k + 3] = g->rmax[m];
-      b2[4 * k] = g->zmin[m]; b2[4 * k + 1] = g->zmax[m]; b2[4 * k + 2] = (float)g->category[m];
-      b2[4 * k + 3] = c->k.par.f_sig_t[g->category[m] & 3] / g->rmin[m];
-    }
-    const size_t nb = std::max<size_t>(start_mods.size(), 1) * 16;
-    cudaMemcpy(d + o_sbox, b1, nb, cudaMemcpyHostToDevice);
-    cudaMemcpy(d + o_sbox + up(nb), b2, nb, cudaMemcpyHostToDevice);
-    c->k.geo.start_box = (const float4 *)(d + o_sbox);
-    c->k.geo.start_box2 = (const float4 *)(d + o_sbox + up(nb));
     std::vector<float> r1(4 * std::max<size_t>(n_prow, 1), 0.0f), r2(4 * std::max<size_t>(n_prow, 1), 0.0f);
     for (size_t r = 0; r < n_prow; ++r)
       for (int q = 0; q < 4; ++q) { r1[4 * r + q] = prow_b[8 * r + q]; r2[4 * r + q] = prow_b[8 * r + 4 + q]; }
@@ -504,16 +491,6 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   c->k.geo.zmin = (const float *)(d + o_box + 4 * box_stride); c->k.geo.zmax = (const float *)(d + o_box + 5 * box_stride);
   c->k.geo.start_mods = (const uint32_t *)(d + o_start);
   c->k.geo.n_start = (uint32_t)start_mods.size();
-  for (int l = 0; l < 16; ++l) {
-    c->k.lay_rmin[l] = INFINITY; c->k.lay_rmax[l] = 0.f; c->k.lay_zmin[l] = INFINITY; c->k.lay_zmax[l] = -INFINITY;
-  }
-  for (uint32_t m = 0; m < n; ++m) {
-    const int l = g->logical_layer[m];
-    c->k.lay_rmin[l] = std::min(c->k.lay_rmin[l], g->rmin[m]);
-    c->k.lay_rmax[l] = std::max(c->k.lay_rmax[l], g->rmax[m]);
-    c->k.lay_zmin[l] = std::min(c->k.lay_zmin[l], g->zmin[m]);
-    c->k.lay_zmax[l] = std::max(c->k.lay_zmax[l], g->zmax[m]);
-  }
   c->slots.resize(n_slots);
   c->ws_bytes = carve(c, nullptr, nullptr);
   *out = c;

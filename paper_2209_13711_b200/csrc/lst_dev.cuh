@@ -3,13 +3,17 @@
 // Every stage (MD, LS, T3, T5, pT5, pT3) is a join: rows x per-row candidate lists, grouped so
 // that one group's operands fit in shared memory.  A stage runs as
 //   groups  : per group g, rows R_g and candidates per row (uniform W_g, or a per-row list)
-//   emit    : one block scans the groups and writes fixed-size work ITEMS (<= 1024 candidates)
-//   eval    : persistent blocks, one item at a time: stage operands in shared memory, fp32
-//             pre-filter, compact survivors, fp64 decision, one pass BIT per candidate
+//   emit    : one block scans the groups (exact offsets), a multi-block kernel writes the
+//             fixed-size work ITEMS (<= 1024 candidates) and work UNITS
+//   eval    : fp32 pre-filter on every candidate; the survivors (item, candidate, pair) are
+//             appended to the stage's candidate list through warp-private staging
+//   decide  : one thread per listed candidate: fp64 decision, pass BIT of the candidate, the
+//             computed quantities into the pool at the candidate's list index
+//   counts  : per-item pass counts and word prefixes from the pass bits
 //   scan    : one block scans the per-item pass counts (exact sizes, no truncation)
-//   fill    : per item: ordered prefix over the bits, fp64 derived quantities, SoA stores
-// Output order is canonical (ascending item, ascending candidate) and no global atomics are used
-// for compaction (north_star: ballot/prefix-sum compaction, deterministic).
+//   fill    : one thread per listed candidate: the accepted ones move to item_base + bit rank
+// Output order is canonical (ascending item, ascending candidate) whatever order the list was
+// appended in; warp ballots / prefix sums do the compaction, the atomics only order scratch lists.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -110,8 +114,6 @@ struct GeoDev {
   // boxes of the lower sensors (lst_geometry) and the modules that may start a pT3 / pT5 (C6)
   const float *rmin, *rmax, *phic, *hphi, *zmin, *zmax;
   const uint32_t *start_mods;
-  // the same modules' boxes packed for k_px_modules: {phic, hphi, rmin, rmax}, {zmin, zmax, category, sig_t / rmin}
-  const float4 *start_box, *start_box2;
   uint32_t n_start;
   // start modules grouped into "rows": modules that differ only in phic (same category, r, z and
   // half_phi box, e.g. one z-row of a barrel layer or one ring of a disk).  prow_b1 = {hphi, rmin,
@@ -273,56 +275,6 @@ struct WarpQueue {
   }
 };
 
-// Per-item compaction scratch (shared memory).
-struct ItemScratch {
-  uint32_t mask[kItemWords];
-  uint32_t pre[kItemWords + 1];
-  uint16_t list[kItemCand];
-  uint32_t n;
-};
-
-// eval phase 1 helper: append candidate c to the survivor list (warp-aggregated shared atomic).
-// Must be called by all 32 lanes of a warp (uniform loop trip count).
-__device__ __forceinline__ void push_survivor(ItemScratch &s, bool keep, uint32_t c) {
-  const uint32_t b = __ballot_sync(0xffffffffu, keep);
-  if (b == 0) return;
-  const int lane = threadIdx.x & 31;
-  const int leader = __ffs(b) - 1;
-  uint32_t base = 0;
-  if (lane == leader) base = atomicAdd(&s.n, (uint32_t)__popc(b));
-  base = __shfl_sync(0xffffffffu, base, leader);
-  if (keep) s.list[base + __popc(b & ((1u << lane) - 1u))] = (uint16_t)c;
-}
-
-// fill helper: ordered list of set bits of the item's mask.  Call with all threads; needs
-// kThreads >= 4 * kItemWords.  After return s.list[0..s.n) holds the candidates in ascending order.
-__device__ __forceinline__ void expand_mask(ItemScratch &s, const uint32_t *gmask) {
-  const int t = threadIdx.x;
-  if (t < 32) {
-    uint32_t w = gmask[t];
-    s.mask[t] = w;
-    uint32_t tot;
-    uint32_t e = warp_excl_scan((uint32_t)__popc(w), &tot);
-    s.pre[t] = e;
-    if (t == 0) { s.pre[kItemWords] = tot; s.n = tot; }
-  }
-  __syncthreads();
-  {   // 4 threads per mask word, each walks the set bits of one byte (items are sparse: ~2 % pass)
-    const int wd = t >> 2, by = t & 3;
-    if (wd < kItemWords) {
-      const uint32_t w = s.mask[wd];
-      uint32_t bits = (w >> (8 * by)) & 0xFFu;
-      uint32_t pos = s.pre[wd] + __popc(w & ((1u << (8 * by)) - 1u));
-      while (bits) {
-        const int b = __ffs(bits) - 1;
-        bits &= bits - 1;
-        s.list[pos++] = (uint16_t)(wd * 32 + 8 * by + b);
-      }
-    }
-  }
-  __syncthreads();
-}
-
 // eval epilogue, one warp: publish an item's mask words (lane = word), their running pass counts
 // and the item's pass count.
 __device__ __forceinline__ void publish_item(const StageBuf &st, uint32_t it, uint32_t w) {
@@ -332,9 +284,6 @@ __device__ __forceinline__ void publish_item(const StageBuf &st, uint32_t it, ui
   st.mask[(size_t)it * kItemWords + lane] = w;
   st.wpre[(size_t)it * kItemWords + lane] = (uint16_t)e;
   if (lane == 0) st.item_cnt[it] = tot;
-}
-__device__ __forceinline__ void publish_mask(const ItemScratch &s, const StageBuf &st, uint32_t it) {
-  if (threadIdx.x < 32) publish_item(st, it, s.mask[threadIdx.x]);
 }
 
 // Warp-private staging of candidate-list entries (ring in shared memory): the sparse survivors of

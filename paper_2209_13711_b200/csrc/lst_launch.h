@@ -28,8 +28,6 @@ struct Ctx {             // what the launchers need from a context
   GeoDev geo;
   Params par;
   int n_sm;
-  // per logical layer geometry bounds (pixel linking windows), host copies
-  float lay_rmin[16], lay_rmax[16], lay_zmin[16], lay_zmax[16];
 };
 
 // k_common.cu
