@@ -190,7 +190,7 @@ def algorithmic_bytes(name, n):
 # counted from the formulas of lst_math.cuh: the candidate loops are bound by
 # the plain fp32 ALUs / issue slots, not by memory.
 OPS_PER_CAND = {"k_md_eval": (0, 27), "k_ls_eval": (1, 36), "k_join_eval[T3]": (2, 128),
-                "k_join_eval[T5]": (3, 4 + 128), "k_join_eval[pT5]": (4, 34), "k_join_eval[pT3]": (5, 34)}
+                "k_join_eval[T5]": (3, 4 + 128), "k_join_eval[pT5]": (4, 68), "k_join_eval[pT3]": (5, 68)}
 
 
 def algorithmic_ops(name, n):

@@ -158,14 +158,13 @@ __device__ __forceinline__ bool t5_candidate(const SlotDev &s, const Params &g, 
 }
 
 // pT5 / pT3 candidate: pixel seed against OT object `obj` (reading C6).  The fp32 pre-filter tests
-// the first anchor only, loosened by kPreSlack plus absolute slacks far above the fp32 error
+// the first and the last anchor, loosened by kPreSlack plus absolute slacks far above the fp32 error
 // (1e-5 rad on a >= 4e-3 rad window, 2e-3 cm on a >= 0.2 cm window); it never rejects on NaN.
 // sp = {kappa_p, sinh eta, phi, z0} of the seed, computed once per row (stage_seeds).
-template <int KIND>
-__device__ __forceinline__ bool px_pre_f(const SlotDev &s, const Params &g, float4 sp, uint32_t obj) {
-  const uint32_t m0 = KIND == J_PT5 ? s.t5_md[5 * (size_t)obj] : s.t3_md[obj].x;
-  const float4 h = s.md_pos[m0];
-  const int cat = (int)(s.md_mod[m0] & 3u);
+// one anchor (MD m) against the seed parameters sp
+__device__ __forceinline__ bool px_anchor_f(const SlotDev &s, const Params &g, float4 sp, uint32_t m) {
+  const float4 h = s.md_pos[m];
+  const int cat = (int)(s.md_mod[m] & 3u);
   const float kp = sp.x, sh = sp.y;
   float al;
   if (cat < 2) {
@@ -174,7 +173,7 @@ __device__ __forceinline__ bool px_pre_f(const SlotDev &s, const Params &g, floa
   } else {
     al = __fdividef(h.z - sp.w, sh);
   }
-  const float d = s.md_phi[m0] - (sp.z + kp * al);
+  const float d = s.md_phi[m] - (sp.z + kp * al);
   const float dph = d - 6.2831853071795864769f * rintf(d * 0.15915494309189533577f);
   const float sgp = (float)g.seed_sig_phi + (float)g.seed_sig_pt * fabsf(kp) * al + __fdividef(g.f_sig_t[cat], h.w);
   if (fabsf(dph) > g.f_ns * sgp * kPreSlack + 1e-5f) return false;
@@ -189,6 +188,15 @@ __device__ __forceinline__ bool px_pre_f(const SlotDev &s, const Params &g, floa
   }
   if (fabsf(dzt) > g.f_ns * szt * kPreSlack + 2e-3f) return false;
   return true;
+}
+// first and last anchor of the object (the last one has the longest lever arm: together they leave
+// the fp64 kernel little more than the accepted pairs)
+template <int KIND>
+__device__ __forceinline__ bool px_pre_f(const SlotDev &s, const Params &g, float4 sp, uint32_t obj) {
+  uint32_t m0, m1;
+  if (KIND == J_PT5) { m0 = s.t5_md[5 * (size_t)obj]; m1 = s.t5_md[5 * (size_t)obj + 4]; }
+  else { const uint4 t = s.t3_md[obj]; m0 = t.x; m1 = t.z; }
+  return px_anchor_f(s, g, sp, m0) && px_anchor_f(s, g, sp, m1);
 }
 
 // fp64 decision (and chi2_pix) of one (seed, object) pair.
