@@ -108,7 +108,20 @@ __global__ void __launch_bounds__(256) k_px_modules(GeoDev geo, SlotDev s, Param
             const float4 r1 = geo.prow_b1[r];
             px_row_window(g, r1, geo.prow_b2[r], kp, sh, phi, z0, &centre, &halfw);
             s.px_pair[pos + lane] = make_uint2(p, m);
-            s.px_win[pos + lane] = make_float2(wrap_f(centre - geo.phic[m]), halfw - r1.x + 1e-4f);
+            // MDs ascend in azimuth (relative to the module centre) inside a module: those inside the
+            // window are a range, found here once per row by two binary searches
+            uint32_t md0 = s.md_mod_off[m], md1 = s.md_mod_off[m + 1];
+            const float wc = wrap_f(centre - geo.phic[m]), ww = halfw - r1.x + 1e-4f;
+            if (ww < 2.5f) {      // wider windows wrap around: keep the whole module
+              const float lo = wc - ww, hi = wc + ww;
+              uint32_t a = md0, b = md1;
+              while (a < b) { const uint32_t mid = (a + b) >> 1; if (s.md_prel[mid] < lo) a = mid + 1; else b = mid; }
+              const uint32_t first = a;
+              b = md1;
+              while (a < b) { const uint32_t mid = (a + b) >> 1; if (s.md_prel[mid] <= hi) a = mid + 1; else b = mid; }
+              md0 = first; md1 = a;
+            }
+            s.px_rng[pos + lane] = make_uint2(md0, md1);
           }
           pos += take;
         }

@@ -47,23 +47,12 @@ __device__ __forceinline__ void right_range(const SlotDev &s, uint32_t row, uint
     *st = s.t3_md_off[m3];
     *cnt = s.t3_md_off[m3 + 1] - *st;
   } else {
-    // objects whose first MD lies in the row's module AND inside the row's azimuthal window: MDs
-    // ascend in azimuth (relative to the module centre) inside a module, so that is a range
-    const uint32_t m = s.px_pair[row].y;
-    uint32_t md0 = s.md_mod_off[m], md1 = s.md_mod_off[m + 1];
-    const float2 win = s.px_win[row];
-    if (win.y < 2.5f) {        // wider windows wrap around: keep the whole module
-      const float lo = win.x - win.y, hi = win.x + win.y;
-      uint32_t a = md0, b = md1;
-      while (a < b) { const uint32_t mid = (a + b) >> 1; if (s.md_prel[mid] < lo) a = mid + 1; else b = mid; }
-      const uint32_t first = a;
-      b = md1;
-      while (a < b) { const uint32_t mid = (a + b) >> 1; if (s.md_prel[mid] <= hi) a = mid + 1; else b = mid; }
-      md0 = first; md1 = a;
-    }
+    // objects whose first MD lies in the row's module AND inside the row's azimuthal window (the MD
+    // range k_px_modules found: objects are grouped by first MD)
+    const uint2 rng = s.px_rng[row];
     const uint32_t *off = KIND == J_PT5 ? s.t5_md_off : s.t3_md_off;
-    *st = off[md0];
-    *cnt = off[md1] - *st;
+    *st = off[rng.x];
+    *cnt = off[rng.y] - *st;
   }
 }
 

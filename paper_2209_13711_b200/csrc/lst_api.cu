@@ -297,7 +297,7 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.px_cnt = w.take<uint32_t>(nsd);
   s.px_bits = w.take<uint32_t>((size_t)nsd * ((c->k.geo.n_start + 31) / 32));
   s.px_off = w.take<uint32_t>((size_t)nsd + 1); s.px_pair = w.take<uint2>((size_t)nsd * kPxCap);
-  s.px_win = w.take<float2>((size_t)nsd * kPxCap);
+  s.px_rng = w.take<uint2>((size_t)nsd * kPxCap);
   s.pt5_pls_off = w.take<uint32_t>((size_t)nsd + 1); s.pt3_pls_off = w.take<uint32_t>((size_t)nsd + 1);
   s.t5_hits = w.take<uint32_t>(10 * (size_t)s.cap_t5); s.pt3_hits = w.take<uint32_t>(6 * (size_t)s.cap_pt3);
   s.inc_cnt = w.take<uint32_t>(2 * (3 * (size_t)nh + 1)); s.inc_cur = s.inc_cnt ? s.inc_cnt + 3 * (size_t)nh + 1 : nullptr;

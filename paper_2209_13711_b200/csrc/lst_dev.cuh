@@ -175,7 +175,7 @@ struct SlotDev {
   uint32_t *px_bits;               // [cap_seeds * ceil(n_start / 32)] one bit per (seed, start module)
   uint32_t *px_off;                // [cap_seeds+1]
   uint2 *px_pair;                  // [cap_seeds * kPxCap] (seed, module), ascending: rows of the pixel joins
-  float2 *px_win;                  // [cap_seeds * kPxCap] the row's azimuthal window for first anchors: {centre - phic, half width}
+  uint2 *px_rng;                   // [cap_seeds * kPxCap] the row's MDs: those of its module inside the seed's azimuthal window
   uint32_t *pt5_pls_off, *pt3_pls_off;   // [cap_seeds+1] pT5 / pT3 range of a seed
   // a6 cleaning
   uint32_t *t5_hits, *pt3_hits;    // [10 cap_t5], [6 cap_pt3] sorted hit positions in layer order
