@@ -270,16 +270,22 @@ __global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, P
   const uint32_t n_items = s.hdr->n_items[stage];
   const uint32_t n_rows = s.hdr->n_obj[JoinTraits<KIND>::rows_level];
   const int tid = threadIdx.x;
-  for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+  // The pixel stages have few items (~700) and a latency-bound candidate loop: an item is split over
+  // kSplit blocks (each stages the rows and takes a quarter of the candidates).
+  constexpr uint32_t kSplit = (KIND == J_PT5 || KIND == J_PT3) ? 4u : 1u;
+  constexpr int kPart = kItemCand / (int)kSplit;
+  for (uint32_t v = blockIdx.x; v < n_items * kSplit; v += gridDim.x) {
+    const uint32_t it = v / kSplit, part = v % kSplit;
     const Item item = st.items[it];
+    if (part != 0 && (int)(part * kPart) >= (int)item.nj) continue;      // uniform per block
     const uint32_t r0 = item.group * kRowChunk;
     const uint32_t key0 = it * (uint32_t)kItemCand;
-    if (tid < kItemWords) st.mask[(size_t)it * kItemWords + tid] = 0;   // the decide kernel ORs the pass bits in
+    if (part == 0 && tid < kItemWords) st.mask[(size_t)it * kItemWords + tid] = 0;   // the decide kernel ORs the pass bits in
     if (KIND == J_PT5 || KIND == J_PT3) stage_seeds(rowseed, s, g, r0, n_rows);
     stage_rows<KIND>(rt, s, r0, n_rows, sh);
     stage_hints(rt, item.j0);
-    const int nj = item.nj;
-    for (int base = 0; base < nj; base += kThreads) {
+    const int nj = min((int)item.nj, (int)((part + 1) * kPart));
+    for (int base = (int)(part * kPart); base < nj; base += kThreads) {
       const int c = base + tid;
       bool keep = false;
       uint2 ab = make_uint2(0u, 0u);
