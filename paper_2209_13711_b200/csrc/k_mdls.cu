@@ -210,12 +210,14 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
   ClBuf cl;
   cl.init(&sh.w.cl[wib]);
   __shared__ uint32_t sh_unit[2];
+  __shared__ int sh_task;                       // next (chunk, row group) task of the unit: warps take them dynamically
   for (;;) {
     __syncthreads();                            // the previous unit is done with the shared arrays
     if (tid == 0) {                             // units are handed out dynamically (their cost varies 100x)
       const uint32_t nu = atomicAdd(&s.hdr->next_unit[S_LS], 1u);
       sh_unit[0] = nu;
       sh_unit[1] = nu < n_units ? st.unit_group[nu] : 0u;
+      sh_task = 0;
     }
     __syncthreads();
     const uint32_t u = sh_unit[0];
@@ -249,7 +251,11 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
     // tasks: (32-column chunk, interleaved row group); with few chunks the rows are split over the warps
     const int nchunk = (nj + 31) >> 5;
     const int nrg = nchunk >= kWarps ? 1 : kWarps / nchunk;
-    for (int t = wib; t < nchunk * nrg; t += kWarps) {
+    for (;;) {
+      int t = 0;
+      if (lane == 0) t = atomicAdd(&sh_task, 1);
+      t = __shfl_sync(0xffffffffu, t, 0);
+      if (t >= nchunk * nrg) break;
       const int chunk = t % nchunk, rg = t / nchunk;
       const int jj = chunk * 32 + lane;
       const bool has = jj < nj;
