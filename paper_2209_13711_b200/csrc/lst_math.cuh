@@ -110,6 +110,16 @@ LST_HD double arc_of(double r, double k) {               // arc length at radius
 // "v <= thr" with NaN failing
 LST_HD bool le(double v, double thr) { return v <= thr; }
 
+// fp32 atan2 for the pre-filters: for x > 0, |y| <= x / 4 the odd series in t = y / x to t^11
+// (truncation < 2e-9 relative, below the fp32 rounding of the result); atan2f otherwise.
+LST_HD float atan2_small_f(float y, float x) {
+  if (x > 0.0f && fabsf(y) <= 0.25f * x) {
+    const float t = LST_FDIV(y, x), u = t * t;
+    return t * (1.0f + u * (-0.33333333f + u * (0.2f + u * (-0.14285714f + u * (0.11111111f - 0.09090909f * u)))));
+  }
+  return atan2f(y, x);
+}
+
 // ------------------------------------------------------------------ C1 mini-doublet
 struct MdOut { double kappa, sigk, dphi; };
 
@@ -375,8 +385,8 @@ LST_HD bool t3_pre_f(const Params &g, float x1, float y1, float z1, float r1, in
   if (fabsf(N) > g.f_ns * E * kPreSlack + 0.02f) return false;                                              // T3-3
   // T3-2 in fp32: its error (~5e-6, from atan2f / asinf and the products) is three orders of magnitude
   // below the smallest threshold (~5e-3); loosened by 1 % and 2e-4 absolute.
-  const float d12 = atan2f(x1 * d12y - y1 * d12x, x1 * x2 + y1 * y2);
-  const float d23 = atan2f(x2 * d23y - y2 * d23x, x2 * x3 + y2 * y3);
+  const float d12 = atan2_small_f(x1 * d12y - y1 * d12x, x1 * x2 + y1 * y2);
+  const float d23 = atan2_small_f(x2 * d23y - y2 * d23x, x2 * x3 + y2 * y3);
   const float d13 = d12 + d23;
   float L1, L2, L3, sl1 = 0.0f, sl2 = 0.0f, sl3 = 0.0f;
   if (c1 >= 2 || c2 >= 2 || c3 >= 2) {
