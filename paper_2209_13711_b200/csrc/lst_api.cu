@@ -228,6 +228,7 @@ struct lst_ctx {
   size_t ws_bytes = 0;
   size_t exp_obj_cap = 0, exp_hit_words = 0;
   uint32_t launches = 0;         // kernels enqueued by the last chain (graph capture or direct)
+  uint32_t map_edges = 0, map_edges_used = 0;   // module-map edges given / kept for the LS enumeration
   Recorder timed;                // lst_run_timed: events created on first use
   bool timed_ready = false;
 };
@@ -364,6 +365,62 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   return (w.off + 255) & ~(size_t)255;
 }
 
+// Can ANY (inner anchor in module A's lower-sensor box, outer anchor in module B's) pass the LS
+// cuts L1 (pointing) and L2 (pT window) of reading C3?  Host, fp64, interval arithmetic on the two
+// boxes, every bound loosened (1e-3 relative, boxes grown by 1e-4 cm / 1e-6 rad for the fp32
+// rounding of the hits): false only for module pairs that cannot hold a line segment.  The module
+// map is built with wider margins (kappa' = 1.25 kappa_max, z0' = 20 cm, a d0 allowance) than the
+// cuts use, so ~21 % of its edges are dead; dropping them from the LS enumeration changes no result.
+// Assumes what lst_geometry states: a lower-sensor hit lies inside its module's box.
+static bool ls_edge_possible(const Params &p, const lst_geometry *g, uint32_t A, uint32_t B) {
+  const double kEps = 1e-3, gl = 1e-4, ga = 1e-6, kPi = 3.14159265358979323846;
+  const int cA = g->category[A] & 3, cB = g->category[B] & 3;
+  const double ri0 = std::max(1e-6, (double)g->rmin[A] - gl), ri1 = (double)g->rmax[A] + gl;
+  const double ro0 = std::max(1e-6, (double)g->rmin[B] - gl), ro1 = (double)g->rmax[B] + gl;
+  const double zi0 = (double)g->zmin[A] - gl, zi1 = (double)g->zmax[A] + gl;
+  const double zo0 = (double)g->zmin[B] - gl, zo1 = (double)g->zmax[B] + gl;
+  // L1: N = rt_i z_o - z_i rt_o is multilinear: its extremes over the boxes are at the corners
+  double Nmin = INFINITY, Nmax = -INFINITY;
+  const double ris[2] = {ri0, ri1}, zis[2] = {zi0, zi1}, ros[2] = {ro0, ro1}, zos[2] = {zo0, zo1};
+  for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) for (int c = 0; c < 2; ++c) for (int d = 0; d < 2; ++d) {
+    const double N = ris[a] * zos[d] - zis[b] * ros[c];
+    Nmin = std::min(Nmin, N); Nmax = std::max(Nmax, N);
+  }
+  const double azi1 = std::max(std::fabs(zi0), std::fabs(zi1)), azo1 = std::max(std::fabs(zo0), std::fabs(zo1));
+  const double Emax = ri1 * p.sig_z[cB] + ro1 * p.sig_z[cA] + azo1 * p.sig_r[cA] + azi1 * p.sig_r[cB];
+  const double drmax = std::max(std::fabs(ro1 - ri0), std::fabs(ro0 - ri1));
+  const double rhs = (p.z0max * drmax + p.ns * Emax) * (1.0 + kEps) + 1e-3;
+  if (!(Nmin <= rhs && Nmax >= -rhs)) return false;
+  // L2: smallest |dphi| the boxes allow against the largest the cut allows
+  const double dphi = std::fabs(std::remainder((double)g->phic[B] - (double)g->phic[A], 2.0 * kPi));
+  const double dmin = std::max(0.0, dphi - (double)g->half_phi[A] - (double)g->half_phi[B] - 2.0 * ga);
+  const double sigt = std::max(std::max(p.sig_t[0], p.sig_t[1]), std::max(p.sig_t[2], p.sig_t[3]));
+  const double tol = p.ns * sigt * (1.0 / ri0 + 1.0 / ro0);
+  double W = kPi;
+  if (cB < 2) {
+    // mode R: a passing pair lies on a circle through the origin of half curvature <= k' = kmax +
+    // tol / chord, where dphi = asin(k' rt_o) - asin(k' rt_i) on the outgoing arc; the returning arc
+    // has dphi < pi/2 only if asin(k' rt_o) + asin(k' rt_i) > pi/2, which k' rt_o <= 0.6 excludes
+    const double cmin = ro0 - ri1;
+    if (cmin > 1.0) {
+      const double k = (p.kmax + tol / cmin) * (1.0 + 2.0 * kEps);
+      if (k * ro1 <= 0.6) W = (std::asin(k * ro1) - std::asin(k * ri0)) * (1.0 + 2.0 * kEps) + 1e-4;
+    }
+  } else {
+    // mode Z: L2 is itself a bound on |dphi|, taken at the extremes of the boxes
+    const double sigr = std::max(std::max(p.sig_r[0], p.sig_r[1]), std::max(p.sig_r[2], p.sig_r[3]));
+    const double azi0 = (zi0 <= 0.0 && zi1 >= 0.0) ? 0.0 : std::min(std::fabs(zi0), std::fabs(zi1));
+    const double azo0 = (zo0 <= 0.0 && zo1 >= 0.0) ? 0.0 : std::min(std::fabs(zo0), std::fabs(zo1));
+    const double dzmax = std::max(std::fabs(zo1 - zi0), std::fabs(zo0 - zi1));
+    const double den = 0.5 * (azi0 + azo0) - p.z0max - 0.5 * p.ns * p.sig_z[cA];
+    if (den > 1.0) {
+      const double x = std::min(1.0, p.kmax * (0.5 * (ri1 + ro1) + p.ns * sigr));
+      W = (p.kmax * (dzmax + p.ns * p.sig_z[cA]) * (std::asin(x) / p.kmax) / den + tol) * (1.0 + 2.0 * kEps) + 1e-4;
+    }
+  }
+  return dmin <= W;
+}
+
 extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, const lst_config *cfg_in,
                           uint32_t n_slots, uint32_t max_hits, uint32_t max_seeds, lst_ctx **out) {
   if (!geometry_ok(g) || !map || !map->row_offsets || !out || n_slots == 0 || max_hits == 0) return LST_EINVAL;
@@ -452,8 +509,19 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   char *d = (char *)c->d_static;
   cudaMemcpy(d + o_cat, g->category, n, cudaMemcpyHostToDevice);
   cudaMemcpy(d + o_lay, g->logical_layer, n, cudaMemcpyHostToDevice);
-  cudaMemcpy(d + o_off, map->row_offsets, (size_t)(n + 1) * 4, cudaMemcpyHostToDevice);
-  if (nnz) cudaMemcpy(d + o_cols, map->cols, (size_t)nnz * 4, cudaMemcpyHostToDevice);
+  {
+    // the LS enumeration walks the map without its dead edges (ls_edge_possible)
+    std::vector<uint32_t> poff(n + 1, 0u), pcols;
+    pcols.reserve(nnz);
+    for (uint32_t m = 0; m < n; ++m) {
+      for (uint32_t e = map->row_offsets[m]; e < map->row_offsets[m + 1]; ++e)
+        if (ls_edge_possible(c->k.par, g, m, map->cols[e])) pcols.push_back(map->cols[e]);
+      poff[m + 1] = (uint32_t)pcols.size();
+    }
+    c->map_edges = nnz; c->map_edges_used = (uint32_t)pcols.size();
+    cudaMemcpy(d + o_off, poff.data(), (size_t)(n + 1) * 4, cudaMemcpyHostToDevice);
+    if (!pcols.empty()) cudaMemcpy(d + o_cols, pcols.data(), pcols.size() * 4, cudaMemcpyHostToDevice);
+  }
   const float *box[6] = {g->rmin, g->rmax, g->phic, g->half_phi, g->zmin, g->zmax};
   for (int k = 0; k < 6; ++k) cudaMemcpy(d + o_box + k * box_stride, box[k], (size_t)n * 4, cudaMemcpyHostToDevice);
   if (!start_mods.empty())
