@@ -85,7 +85,7 @@ def alu_peak_gops():
 
 # DRAM bytes (read + write) of one launch of the dominant kernel from the ncu --set full capture
 # summarised in profiles/ (the file is named in the roofline object); None for other kernels.
-NCU_TRAFFIC = {"k_ls_eval": (3205376, "profiles/r1d_top_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full")}
+NCU_TRAFFIC = {"k_ls_eval": (3004416, "profiles/r1d_top_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full")}
 
 
 class ClockSampler:
