@@ -128,7 +128,19 @@ static double arc_f(double r, double k) {
 
 /* cut bookkeeping: pass &= (v <= thr) (NaN fails); margin = min |v-thr|/|thr| */
 typedef struct { int pass; double margin; } cut_t;
+/* test hook (lsto_test_cuts): while a trace buffer is installed every cut appends the triple
+ * (kind, v, thr) in evaluation order; kind 0 = "v <= thr", 1 = "v > 0" (thr = its scale),
+ * 2 = a guard failed (v = thr = 0).  It records the bookkeeping, it changes no arithmetic. */
+static _Thread_local double *g_trace = NULL;
+static _Thread_local int g_trace_n = 0, g_trace_cap = 0;
+static void trace_push(double kind, double v, double thr) {
+  if (g_trace && g_trace_n + 3 <= g_trace_cap) {
+    g_trace[g_trace_n] = kind; g_trace[g_trace_n + 1] = v; g_trace[g_trace_n + 2] = thr;
+  }
+  if (g_trace) g_trace_n += 3;
+}
 static void cut_le(cut_t *c, double v, double thr) {
+  trace_push(0.0, v, thr);
   if (!(v <= thr)) c->pass = 0;
   double m = fabs(v - thr) / max2(fabs(thr), 1e-300);
   if (!(m >= 0.0)) m = 0.0; /* NaN: treat as on-threshold */
@@ -136,12 +148,13 @@ static void cut_le(cut_t *c, double v, double thr) {
 }
 /* sign requirement v > 0, measured against a natural scale */
 static void cut_pos(cut_t *c, double v, double scale) {
+  trace_push(1.0, v, scale);
   if (!(v > 0.0)) c->pass = 0;
   double m = fabs(v) / max2(fabs(scale), 1e-300);
   if (!(m >= 0.0)) m = 0.0;
   if (m < c->margin) c->margin = m;
 }
-static void cut_fail(cut_t *c) { c->pass = 0; }
+static void cut_fail(cut_t *c) { trace_push(2.0, 0.0, 0.0); c->pass = 0; }
 
 /* ------------------------------------------------------------------ C1 mini-doublets
  * PAPER.md:37 (Fig. 2): a stub is a pair of hits in the two sensors of one pT module inside a
@@ -657,6 +670,105 @@ int lsto_link_pixel(lsto_ctx *c, uint32_t s0, uint32_t s1) {
   return 0;
 }
 
+/* Indexed enumeration of the same (pLS, object) pairs: the definition above is all pairs; here a
+ * pair is visited only if the object's FIRST anchor can pass its own residual cuts.  Per module the
+ * bounding box of the event's MD anchors (rt, azimuth, z: measured from the MDs themselves, so no
+ * premise about the geometry) is tested against the seed's extrapolation window with interval
+ * arithmetic in fp64 and absolute margins (1e-6) far above rounding; objects are then visited in
+ * the same order as the all-pairs loops (T3 / T5 are grouped by first MD, MDs by module), so the
+ * result arrays are IDENTICAL, which tests/test_oracle_pins.py checks against lsto_link_pixel. */
+typedef struct { double rlo, rhi, zlo, zhi, pref, dlo, dhi; int any; } mbox_t;
+
+static int px_box_possible(const lsto_ctx *c, uint32_t p, const mbox_t *b, int cat) {
+  const lsto_config *g = &c->cfg;
+  const double M = 1e-6;
+  double pt = c->spt[p], eta = c->seta[p], phi = c->sphi[p], z0 = c->sz0[p];
+  if (!(pt > GUARD)) return 0;
+  double kp = -(double)c->sq[p] * g->kB / (2.0 * pt), sh = sinh(eta);
+  double s_lo, s_hi;          /* arc-length interval of an anchor inside the box */
+  if (!is_endcap(cat)) {
+    s_lo = arc_f(b->rlo, kp); s_hi = arc_f(b->rhi, kp);      /* increasing in rt */
+  } else {
+    if (!(fabs(sh) > GUARD)) return 0;
+    double a = (b->zlo - z0) / sh, d = (b->zhi - z0) / sh;   /* linear in z */
+    s_lo = min2(a, d); s_hi = max2(a, d);
+  }
+  if (!(s_hi > 0.0)) return 0;
+  if (s_lo < 0.0) s_lo = 0.0;
+  /* azimuth: predicted phi + kp s over [s_lo, s_hi] against the anchors' azimuth interval */
+  double f_lo = phi + min2(kp * s_lo, kp * s_hi), f_hi = phi + max2(kp * s_lo, kp * s_hi);
+  double sphi = g->seed_sig_phi + g->seed_sig_pt * fabs(kp) * s_hi + g->sig_t[cat] / b->rlo;
+  double tol = g->n_sigma * sphi + M;
+  double a_lo = b->pref + b->dlo, a_hi = b->pref + b->dhi;
+  double width = (a_hi - a_lo) + (f_hi - f_lo) + 2.0 * tol;
+  if (width < 2.0 * 3.14159265358979323846) {
+    double mid = wrap_pi(0.5 * (a_lo + a_hi) - 0.5 * (f_lo + f_hi));
+    if (fabs(mid) > 0.5 * width) return 0;
+  }
+  if (!is_endcap(cat)) {
+    double z1 = z0 + sh * s_lo, z2 = z0 + sh * s_hi;
+    double tz = g->n_sigma * (g->seed_sig_z + g->sig_z[cat]) + M;
+    if (min2(z1, z2) - tz > b->zhi || max2(z1, z2) + tz < b->zlo) return 0;
+  } else if (fabs(kp) * s_hi < 1.5) {          /* sin(kp s)/kp increases with s while |kp s| < pi/2 */
+    double r1 = (fabs(kp * s_lo) <= 1e-4) ? s_lo : sin(kp * s_lo) / kp;
+    double r2 = (fabs(kp * s_hi) <= 1e-4) ? s_hi : sin(kp * s_hi) / kp;
+    double tr = g->n_sigma * (g->seed_sig_z / fabs(sh) + g->sig_r[cat]) + M;
+    if (min2(r1, r2) - tr > b->rhi || max2(r1, r2) + tr < b->rlo) return 0;
+  }
+  return 1;
+}
+
+int lsto_link_pixel_indexed(lsto_ctx *c, uint32_t s0, uint32_t s1) {
+  VCLEAR(c->pt5); VCLEAR(c->pt3);
+  if (s1 > c->n_seeds) s1 = c->n_seeds;
+  uint32_t nm = c->n_modules, nmd = c->md.n;
+  mbox_t *box = calloc((size_t)nm + 1, sizeof(mbox_t));
+  uint32_t *mods = malloc(((size_t)nm + 1) * 4), n_start = 0;
+  for (uint32_t m = 0; m < nm; ++m) {
+    if (!((c->cfg.start_layer_mask >> c->layer[m]) & 1u)) continue;
+    uint32_t a = c->md_mod_off[m], b = c->md_mod_off[m + 1];
+    if (a == b) continue;
+    mbox_t *q = &box[m];
+    const pt3 *f = &c->md.v[a].a;
+    q->pref = atan2(f->y, f->x);
+    q->rlo = q->rhi = f->rt; q->zlo = q->zhi = f->z; q->dlo = q->dhi = 0.0; q->any = 1;
+    for (uint32_t i = a + 1; i < b; ++i) {
+      const pt3 *h = &c->md.v[i].a;
+      double d = wrap_pi(atan2(h->y, h->x) - q->pref);
+      q->rlo = min2(q->rlo, h->rt); q->rhi = max2(q->rhi, h->rt);
+      q->zlo = min2(q->zlo, h->z); q->zhi = max2(q->zhi, h->z);
+      q->dlo = min2(q->dlo, d); q->dhi = max2(q->dhi, d);
+    }
+    mods[n_start++] = m;
+  }
+  /* T5 range of a first MD (T5 are built T3 by T3, so they ascend in their first MD) */
+  uint32_t *t5_off = calloc((size_t)nmd + 2, 4);
+  for (uint32_t i = 0; i < c->t5.n; ++i) t5_off[c->t5.v[i].m[0] + 1]++;
+  for (uint32_t i = 0; i < nmd; ++i) t5_off[i + 1] += t5_off[i];
+  for (int five = 1; five >= 0; --five) {
+    for (uint32_t p = s0; p < s1; ++p) {
+      for (uint32_t k = 0; k < n_start; ++k) {
+        uint32_t m = mods[k];
+        if (!px_box_possible(c, p, &box[m], c->category[m])) continue;
+        for (uint32_t i = c->md_mod_off[m]; i < c->md_mod_off[m + 1]; ++i) {
+          uint32_t o0 = five ? t5_off[i] : c->t3_md_off[i], o1 = five ? t5_off[i + 1] : c->t3_md_off[i + 1];
+          for (uint32_t o = o0; o < o1; ++o) {
+            const pt3 *P[5];
+            int n = five ? 5 : 3;
+            const uint32_t *mm = five ? c->t5.v[o].m : c->t3.v[o].m;
+            for (int q = 0; q < n; ++q) P[q] = &c->md.v[mm[q]].a;
+            double chi2 = 0;
+            cut_t r = px_eval(c, p, P, n, c->layer[m], &chi2, 0);
+            if (r.pass) { px_t x = {p, o, chi2, r.margin}; if (five) VPUSH(c->pt5, x); else VPUSH(c->pt3, x); }
+          }
+        }
+      }
+    }
+  }
+  free(box); free(mods); free(t5_off);
+  return 0;
+}
+
 /* ------------------------------------------------------------------ C7 duplicate removal, TC
  * cross-cleaning pT3 vs pT5; T5 vs pT5 + cleaned pT3; unused pLS vs all; close in
  * eta-phi, and objects must not share hits; TC = pT5 + pT3 + T5 + unlinked pLS. */
@@ -725,12 +837,12 @@ static int beats(const lsto_ctx *c, const dobj_t *b, const dobj_t *a) {
   int n = a->n_ot < b->n_ot ? a->n_ot : b->n_ot;
   for (int k = 0; k < n; ++k) {
     uint32_t hb = b->ot[k], ha = a->ot[k];
-    if (c->hx[hb] < c->hx[ha]) return 1; if (c->hx[hb] > c->hx[ha]) return 0;
-    if (c->hy[hb] < c->hy[ha]) return 1; if (c->hy[hb] > c->hy[ha]) return 0;
-    if (c->hz[hb] < c->hz[ha]) return 1; if (c->hz[hb] > c->hz[ha]) return 0;
+    if (c->hx[hb] != c->hx[ha]) return c->hx[hb] < c->hx[ha];
+    if (c->hy[hb] != c->hy[ha]) return c->hy[hb] < c->hy[ha];
+    if (c->hz[hb] != c->hz[ha]) return c->hz[hb] < c->hz[ha];
   }
-  if (a->has_pls && b->has_pls) { if (b->pls < a->pls) return 1; if (b->pls > a->pls) return 0; }
-  for (int k = 0; k < n; ++k) { if (b->ot[k] < a->ot[k]) return 1; if (b->ot[k] > a->ot[k]) return 0; }
+  if (a->has_pls && b->has_pls && b->pls != a->pls) return b->pls < a->pls;
+  for (int k = 0; k < n; ++k) if (b->ot[k] != a->ot[k]) return b->ot[k] < a->ot[k];
   return 0;
 }
 /* cross-cleaning predicate: close in eta-phi OR sharing any hit */
@@ -1000,4 +1112,102 @@ int lsto_test_kasa(const lsto_config *cfg, const double *x, const double *y, con
   for (int k = 0; k < 5; ++k) { p[k].x = x[k]; p[k].y = y[k]; p[k].z = 0; p[k].rt = hypot(x[k], y[k]); p[k].cat = cat[k]; P[k] = &p[k]; }
   double detn = 0;
   return kasa_fit(&c, P, kc, R, chi2, &detn);
+}
+
+/* Evaluate ONE selection function on double inputs (no event, no fp32 rounding) and return every cut
+ * it evaluated as (kind, v, thr) triples in evaluation order (see trace_push).  level: LSTO_MD
+ * (pts = lower, upper; cats[0] = module category), LSTO_LS (pts = anchors i, o; aux = kappa_MD(i),
+ * sigma(i), kappa_MD(o), sigma(o)), LSTO_T3 (3 anchors), LSTO_T5 (5 anchors; aux = kappa3(a),
+ * sigma(a), kappa3(b), sigma(b)), LSTO_PT3 / LSTO_PT5 (3 / 5 anchors; aux = pt, eta, phi, z0, q,
+ * logical layer of the first MD).  out_f (8 doubles): MD / LS {dphi, kappa, sigk}; T3 {beta, kappa3,
+ * sigk3}; T5 {R, chi2, pt, eta, phi}; PT3 / PT5 {chi2_pix}.  Returns pass (0 / 1), -1 on bad level. */
+int lsto_test_cuts(const lsto_config *cfg, int level, const double *pts, const int32_t *cats, const double *aux,
+                   double *out_f, double *trace, int trace_cap, int *n_trace) {
+  lsto_ctx c; memset(&c, 0, sizeof(c));
+  c.cfg = *cfg;
+  c.kmax = cfg->kB / (2.0 * cfg->pt_min);
+  int npts = level == LSTO_MD || level == LSTO_LS ? 2 : (level == LSTO_T3 || level == LSTO_PT3 ? 3 :
+             (level == LSTO_T5 || level == LSTO_PT5 ? 5 : 0));
+  if (!npts) return -1;
+  pt3 p[5]; const pt3 *P[5];
+  for (int k = 0; k < npts; ++k) {
+    p[k].x = pts[3 * k]; p[k].y = pts[3 * k + 1]; p[k].z = pts[3 * k + 2];
+    p[k].rt = sqrt(p[k].x * p[k].x + p[k].y * p[k].y);
+    p[k].cat = cats[level == LSTO_MD ? 0 : k];
+    P[k] = &p[k];
+  }
+  for (int k = 0; k < 8; ++k) out_f[k] = 0.0;
+  g_trace = trace; g_trace_n = 0; g_trace_cap = trace_cap;
+  cut_t r;
+  if (level == LSTO_MD) {
+    md_t o; memset(&o, 0, sizeof(o));
+    r = md_eval(&c, &p[0], &p[1], cats[0], &o);
+    out_f[0] = o.dphi; out_f[1] = o.kappa; out_f[2] = o.sigk;
+  } else if (level == LSTO_LS) {
+    md_t mi, mo; memset(&mi, 0, sizeof(mi)); memset(&mo, 0, sizeof(mo));
+    mi.a = p[0]; mi.kappa = aux[0]; mi.sigk = aux[1];
+    mo.a = p[1]; mo.kappa = aux[2]; mo.sigk = aux[3];
+    ls_t o; memset(&o, 0, sizeof(o));
+    r = ls_eval(&c, &mi, &mo, &o);
+    out_f[0] = o.dphi; out_f[1] = o.kappa; out_f[2] = o.sigk;
+  } else if (level == LSTO_T3) {
+    t3_t o; memset(&o, 0, sizeof(o));
+    r = t3_eval(&c, P[0], P[1], P[2], &o);
+    out_f[0] = o.beta; out_f[1] = o.kappa3; out_f[2] = o.sigk3;
+  } else if (level == LSTO_T5) {
+    t5_t o; memset(&o, 0, sizeof(o));
+    r = t5_eval(&c, P, aux[0], aux[1], aux[2], aux[3], &o);
+    out_f[0] = o.R; out_f[1] = o.chi2; out_f[2] = o.pt; out_f[3] = o.eta; out_f[4] = o.phi;
+  } else {
+    double spt = aux[0], seta = aux[1], sphi = aux[2], sz0 = aux[3];
+    int8_t sq = (int8_t)aux[4];
+    c.spt = &spt; c.seta = &seta; c.sphi = &sphi; c.sz0 = &sz0; c.sq = &sq; c.n_seeds = 1;
+    double chi2 = 0.0;
+    r = px_eval(&c, 0, P, npts, (int)aux[5], &chi2, 1);
+    out_f[0] = chi2;
+  }
+  if (n_trace) *n_trace = g_trace_n / 3;
+  g_trace = NULL; g_trace_n = 0; g_trace_cap = 0;
+  return r.pass;
+}
+
+/* Replace the object collections of the loaded event by hand-built ones, so that lsto_dedup can be
+ * pinned on constructed cases (shared-hit thresholds, Delta R^2 edge, the pLS rules).  MDs are given
+ * by their hit indices; T3 / T5 by MD indices (+ chi2, pt, eta, phi for T5); pT3 / pT5 by (pLS,
+ * object index, chi2_pix), grouped by pLS as lsto_link_pixel builds them. */
+int lsto_test_inject(lsto_ctx *c, uint32_t n_md, const uint32_t *md_hits, uint32_t n_t3, const uint32_t *t3_md,
+                     uint32_t n_t5, const uint32_t *t5_md, const double *t5_kin /* chi2, pt, eta, phi */,
+                     uint32_t n_pt3, const uint32_t *pt3_po, const double *pt3_chi2,
+                     uint32_t n_pt5, const uint32_t *pt5_po, const double *pt5_chi2) {
+  VCLEAR(c->md); VCLEAR(c->ls); VCLEAR(c->t3); VCLEAR(c->t5); VCLEAR(c->pt3); VCLEAR(c->pt5); VCLEAR(c->tc);
+  for (uint32_t i = 0; i < n_md; ++i) {
+    md_t m; memset(&m, 0, sizeof(m));
+    m.hl = md_hits[2 * i]; m.hu = md_hits[2 * i + 1];
+    if (m.hl >= c->n_hits || m.hu >= c->n_hits) return -1;
+    m.module = c->hdet[m.hl] >> 1;
+    m.a = hit_pt(c, m.hl, c->category[m.module]);
+    VPUSH(c->md, m);
+  }
+  for (uint32_t i = 0; i < n_t3; ++i) {
+    t3_t t; memset(&t, 0, sizeof(t));
+    for (int k = 0; k < 3; ++k) { t.m[k] = t3_md[3 * i + k]; if (t.m[k] >= n_md) return -1; }
+    VPUSH(c->t3, t);
+  }
+  for (uint32_t i = 0; i < n_t5; ++i) {
+    t5_t t; memset(&t, 0, sizeof(t));
+    for (int k = 0; k < 5; ++k) { t.m[k] = t5_md[5 * i + k]; if (t.m[k] >= n_md) return -1; }
+    t.chi2 = t5_kin[4 * i]; t.pt = t5_kin[4 * i + 1]; t.eta = t5_kin[4 * i + 2]; t.phi = t5_kin[4 * i + 3];
+    VPUSH(c->t5, t);
+  }
+  for (uint32_t i = 0; i < n_pt3; ++i) {
+    px_t x = {pt3_po[2 * i], pt3_po[2 * i + 1], pt3_chi2[i], 0.0};
+    if (x.pls >= c->n_seeds || x.obj >= n_t3) return -1;
+    VPUSH(c->pt3, x);
+  }
+  for (uint32_t i = 0; i < n_pt5; ++i) {
+    px_t x = {pt5_po[2 * i], pt5_po[2 * i + 1], pt5_chi2[i], 0.0};
+    if (x.pls >= c->n_seeds || x.obj >= n_t5) return -1;
+    VPUSH(c->pt5, x);
+  }
+  return 0;
 }

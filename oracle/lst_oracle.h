@@ -9,11 +9,22 @@
  * other.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
  * reference legs may build, load or call it.
  *
- * Parity pins (tests/test_oracle_pins.py): helix closed forms, noiseless-track chains,
- * pT-threshold edge, brute-force enumeration, permutation invariance, Kasa fit vs an
- * independent geometric fit, dedup order-independence.  "parity unpinned" against the
- * paper's own values: the paper prints no cut value, object count or worked example
- * on data available here.
+ * Parity pins, function by function (DESIGN.md section 3 has the table):
+ *   tests/test_oracle_pins.py        helix closed forms, noiseless-track chains, pT edge of B2 on
+ *                                    generated hits, brute-force enumeration, permutation
+ *                                    invariance, Kasa fit vs an independent geometric fit
+ *   tests/test_oracle_pins2.py       two-sided pins: closed-form EDGE of B2, E2, L2 (mode R and Z),
+ *                                    T3-1, T5-1, chi2max; every tolerance term of B1, E1, L1, L2, L3,
+ *                                    sigma_kappa3, E_phi, E_z, sigma_phi_k, sigma_zeta_k ONE AT A TIME
+ *                                    (the constants are data); closed forms of dphi_MD, beta, mode-Z
+ *                                    kappa_LS, endcap kappa_MD; S0-S3 on hand-built collections;
+ *                                    truth efficiency >= 99 % at every level on smeared events
+ *   tests/test_oracle_restatement.py every cut variable and threshold against a third transcription
+ *                                    of SURVEY.md 8(c) in numpy, on 1e4 candidates per level
+ *   tests/test_oracle_mutations.py   30 single-token mutants of this file are each caught by the pin
+ *                                    named for the mutated function
+ * "parity unpinned" against the paper's own VALUES: the paper prints no cut value, object count
+ * or worked example on data available here.
  */
 #ifndef LST_ORACLE_H
 #define LST_ORACLE_H
@@ -75,7 +86,9 @@ int lsto_build_md(lsto_ctx *c);
 int lsto_build_ls(lsto_ctx *c, int brute);
 int lsto_build_t3(lsto_ctx *c, int brute);
 int lsto_build_t5(lsto_ctx *c, int brute);
-int lsto_link_pixel(lsto_ctx *c, uint32_t seed_begin, uint32_t seed_end); /* pT5 then pT3 */
+int lsto_link_pixel(lsto_ctx *c, uint32_t seed_begin, uint32_t seed_end); /* pT5 then pT3: ALL pairs */
+/* the same pairs through a per-module first-anchor window (identical output; see the .c file) */
+int lsto_link_pixel_indexed(lsto_ctx *c, uint32_t seed_begin, uint32_t seed_end);
 int lsto_dedup(lsto_ctx *c, int brute);                                   /* S0-S4 -> TC    */
 
 uint32_t lsto_count(const lsto_ctx *c, int level);
@@ -102,6 +115,15 @@ int lsto_eval(const lsto_ctx *c, int level, const uint32_t *hits, uint32_t seed,
 void lsto_test_helpers(const double *A, const double *B, const double *C, double k, double *out7);
 int lsto_test_kasa(const lsto_config *cfg, const double *x, const double *y, const int32_t *cat, double kc,
                    double *R, double *chi2);
+
+/* test hooks (pins only): one selection function on double inputs with the trace of its cuts, and
+ * hand-built object collections for lsto_dedup; see the .c file */
+int lsto_test_cuts(const lsto_config *cfg, int level, const double *pts, const int32_t *cats, const double *aux,
+                   double *out_f, double *trace, int trace_cap, int *n_trace);
+int lsto_test_inject(lsto_ctx *c, uint32_t n_md, const uint32_t *md_hits, uint32_t n_t3, const uint32_t *t3_md,
+                     uint32_t n_t5, const uint32_t *t5_md, const double *t5_kin,
+                     uint32_t n_pt3, const uint32_t *pt3_po, const double *pt3_chi2,
+                     uint32_t n_pt5, const uint32_t *pt5_po, const double *pt5_chi2);
 
 /* TC entry types (parents[0] of level LSTO_TC) */
 enum { LSTO_TC_T5 = LSTO_T5, LSTO_TC_PT3 = LSTO_PT3, LSTO_TC_PT5 = LSTO_PT5, LSTO_TC_PLS = LSTO_TC };

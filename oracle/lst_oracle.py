@@ -31,7 +31,10 @@ class Config(C.Structure):
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (-O2, no fast-math, no intrinsics)."""
+    """Compile the oracle with gcc (-O2, no fast-math, no intrinsics).  LST_ORACLE_SO (tests only:
+    tests/test_oracle_mutations.py) names an already built library to load instead."""
+    if os.environ.get("LST_ORACLE_SO"):
+        return os.environ["LST_ORACLE_SO"]
     stale = (not os.path.exists(_SO)) or any(
         os.path.getmtime(p) > os.path.getmtime(_SO) for p in (_SRC, _HDR))
     if force or stale:
@@ -59,6 +62,9 @@ def lib():
         for f in ("lsto_build_ls", "lsto_build_t3", "lsto_build_t5", "lsto_dedup"):
             getattr(L, f).argtypes = [vp, i32]
         L.lsto_link_pixel.argtypes = [vp, u32, u32]
+        L.lsto_link_pixel_indexed.argtypes = [vp, u32, u32]
+        L.lsto_test_cuts.argtypes = [C.POINTER(Config), i32, vp, vp, vp, vp, vp, i32, C.POINTER(i32)]
+        L.lsto_test_inject.argtypes = [vp, u32, vp, u32, vp, u32, vp, vp, u32, vp, vp, u32, vp, vp]
         L.lsto_count.restype = u32
         L.lsto_count.argtypes = [vp, i32]
         L.lsto_arity.restype = u32
@@ -137,7 +143,10 @@ class Oracle:
             raise ValueError("oracle: invalid event (det out of range)")
         self.n_seeds = len(sp)
 
-    def run(self, upto: int = TC, brute: bool = False, seed_range=None):
+    def run(self, upto: int = TC, brute: bool = False, seed_range=None, pixel_indexed: bool = False):
+        """Build the levels up to `upto`.  brute: all-pairs loops instead of the index-driven ones
+        (module map, joins, cleaning).  Pixel linking is all pairs unless pixel_indexed (identical
+        output through a per-module first-anchor window)."""
         L, b = lib(), int(brute)
         L.lsto_build_md(self._h)
         if upto >= LS:
@@ -148,7 +157,7 @@ class Oracle:
             L.lsto_build_t5(self._h, b)
         if upto >= PT3:
             s0, s1 = seed_range if seed_range is not None else (0, self.n_seeds)
-            L.lsto_link_pixel(self._h, s0, s1)
+            (L.lsto_link_pixel_indexed if pixel_indexed else L.lsto_link_pixel)(self._h, s0, s1)
         if upto >= TC:
             L.lsto_dedup(self._h, b)
         return self
@@ -178,6 +187,24 @@ class Oracle:
         assert rc == 0
         return k[:n].astype(bool)
 
+    def dedup(self, brute: bool = False):
+        lib().lsto_dedup(self._h, int(brute))
+        return self
+
+    def inject(self, md_hits, t3_md=(), t5_md=(), t5_kin=(), pt3_po=(), pt3_chi2=(), pt5_po=(), pt5_chi2=()):
+        """Test hook: replace the object collections of the loaded event by hand-built ones
+        (lsto_test_inject) so that dedup() can be pinned on constructed cases."""
+        u = lambda a, w: np.ascontiguousarray(np.asarray(a, dtype=np.uint32).reshape(-1, w))
+        d = lambda a, w: np.ascontiguousarray(np.asarray(a, dtype=np.float64).reshape(-1, w))
+        md, t3, t5, k5 = u(md_hits, 2), u(t3_md, 3), u(t5_md, 5), d(t5_kin, 4)
+        p3, c3, p5, c5 = u(pt3_po, 2), d(pt3_chi2, 1), u(pt5_po, 2), d(pt5_chi2, 1)
+        assert len(t5) == len(k5) and len(p3) == len(c3) and len(p5) == len(c5)
+        rc = lib().lsto_test_inject(self._h, len(md), _p(md), len(t3), _p(t3), len(t5), _p(t5), _p(k5),
+                                    len(p3), _p(p3), _p(c3), len(p5), _p(p5), _p(c5))
+        if rc != 0:
+            raise ValueError("oracle inject: index out of range")
+        return self
+
     def eval(self, level: int, hits, seed: int = 0):
         """Evaluate one candidate given original hit indices -> (passed, margin)."""
         h = np.ascontiguousarray(hits, dtype=np.uint32)
@@ -204,3 +231,22 @@ def kasa(x, y, cat, kc, cfg: Config | None = None):
     R, c2 = C.c_double(0), C.c_double(0)
     ok = lib().lsto_test_kasa(C.byref(cfg), _p(x), _p(y), _p(cat), float(kc), C.byref(R), C.byref(c2))
     return bool(ok), R.value, c2.value
+
+
+
+CUT_LE, CUT_POS, CUT_GUARD = 0, 1, 2
+
+
+def cuts(level: int, pts, cats, aux=None, cfg: Config | None = None):
+    """Test hook (lsto_test_cuts): one selection function on DOUBLE inputs.
+    Returns (passed, f[8], trace) with trace = [(kind, v, thr), ...] in evaluation order."""
+    cfg = cfg or default_config()
+    pts = np.ascontiguousarray(pts, dtype=np.float64).reshape(-1)
+    cats = np.ascontiguousarray(cats, dtype=np.int32).reshape(-1)
+    aux = np.ascontiguousarray(aux if aux is not None else np.zeros(8), dtype=np.float64).reshape(-1)
+    f, tr, n = np.zeros(8), np.zeros(3 * 64), C.c_int32(0)
+    rc = lib().lsto_test_cuts(C.byref(cfg), int(level), _p(pts), _p(cats), _p(aux), _p(f), _p(tr), len(tr), C.byref(n))
+    if rc < 0:
+        raise ValueError("oracle cuts: bad level")
+    assert 3 * n.value <= len(tr)
+    return bool(rc), f, [tuple(tr[3 * k:3 * k + 3]) for k in range(n.value)]
