@@ -9,7 +9,7 @@ __global__ void k_begin(SlotDev s) {
   Header *h = s.hdr;
   const int t = threadIdx.x;
   if (t < 8) h->n_obj[t] = 0;
-  if (t < S_NSTAGE) { h->n_items[t] = 0; h->n_groups[t] = 0; h->n_units[t] = 0; h->next_unit[t] = 0; h->cl_used[t] = 0; h->cand[t] = 0ull; }
+  if (t < S_NSTAGE) { h->n_items[t] = 0; h->n_groups[t] = 0; h->n_units[t] = 0; h->next_unit[t] = 0; h->cl_used[t] = 0; h->cand[t] = 0ull; h->cand_eval[t] = 0ull; }
   if (t == 0) { h->err = 0; h->n_inc = 0; h->n_heavy = 0; h->n_dd = 0; h->n_flag = 0; s.scan_part[kScanBlocks + 1] = 0; }
 }
 

@@ -82,7 +82,8 @@ struct Header {          // per slot, device; zeroed (except n_hits / n_seeds) a
   uint32_t n_flag;                   // pT5 + pT3 + T5 + seeds: length of the TC keep-flag array
   uint32_t n_inc;                    // 3 * n_hits: rows of the (hit, object type) -> objects incidence
   uint32_t n_heavy;                  // objects k_s0 handed to k_s0_heavy (listed in tc_pos, free until S3)
-  unsigned long long cand[S_NSTAGE]; // candidates enumerated per stage
+  unsigned long long cand[S_NSTAGE]; // candidates of the method's definition per stage (rows x connected columns)
+  unsigned long long cand_eval[S_NSTAGE];   // candidates the stage's pre-filter kernel actually evaluated
 };
 
 struct StageBuf {        // work list of one stage
@@ -148,6 +149,7 @@ struct SlotDev {
   float *md_phi;         // azimuth of the anchor, fp32 (pixel-linking pre-filter)
   float *md_prel;        // the anchor's sort key (azimuth relative to the module centre): ascending inside a module
   uint32_t *md_mod_off;  // [n_modules+1]
+  float4 *md_box;        // [n_modules] bounding box of the module's MD anchors: rt min, rt max, z min, z max
   // LS
   uint2 *ls_md;          // inner, outer MD
   float4 *ls_f;          // dphi, kappa, sigma_kappa, 0
@@ -268,6 +270,36 @@ struct WarpQueue {
     const uint32_t take = n < 32u ? n : 32u;
     const bool have = (uint32_t)lane < take;
     *v = q[(head + lane) & 63u];
+    __syncwarp();
+    head = (head + take) & 63u;
+    n -= take;
+    return have;
+  }
+};
+
+// The same with three words per entry (the LS pre-filter carries inner MD, outer MD and candidate key
+// from tier 1 to tier 2 across row boundaries).
+struct WarpQueue3 {
+  uint32_t *q;       // 3 x 64 words of shared memory owned by this warp
+  uint32_t head, n;
+  __device__ __forceinline__ void init(uint32_t *mem) { q = mem; head = 0; n = 0; }
+  __device__ __forceinline__ void push(bool keep, uint32_t a, uint32_t b, uint32_t c) {
+    const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+    if (bal == 0) return;
+    const int lane = threadIdx.x & 31;
+    if (keep) {
+      const uint32_t p = (head + n + __popc(bal & ((1u << lane) - 1u))) & 63u;
+      q[p] = a; q[64 + p] = b; q[128 + p] = c;
+    }
+    n += __popc(bal);
+    __syncwarp();
+  }
+  __device__ __forceinline__ bool pop(uint32_t *a, uint32_t *b, uint32_t *c) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t take = n < 32u ? n : 32u;
+    const bool have = (uint32_t)lane < take;
+    const uint32_t p = (head + lane) & 63u;
+    *a = q[p]; *b = q[64 + p]; *c = q[128 + p];
     __syncwarp();
     head = (head + take) & 63u;
     n -= take;

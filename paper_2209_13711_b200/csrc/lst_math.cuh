@@ -308,6 +308,50 @@ LST_HD bool ls_tier1_f(const Params &g, float xi, float yi, float zi, float ri, 
   return keep;
 }
 
+// Per-(row MD, connected module) window of the LS enumeration.  (ri, zi, ci): the inner anchor;
+// (rlo, rhi, zlo, zhi): bounding box of the ANCHORS of the module's MDs in this event (measured from
+// the MDs, so nothing is assumed about the geometry description); cB: the module's category.
+// Returns false if NO anchor inside the box can pass cut L1 (interval arithmetic on the bilinear
+// r-z cross product: its extremes over the box are at the corners).  Otherwise *W bounds |dphi| of
+// every pair that can pass L2 (and dot > 0); *W > pi means "no bound" (whole module):
+//   mode R: a passing pair lies on a circle through the origin of half curvature k <= kmax + tol /
+//     chord with chord >= rlo - ri; on it dphi = asin(k ro) - asin(k ri) (both points on the outgoing
+//     arc: the mixed outgoing / returning case needs asin(k ro) + asin(k ri) > pi/2 to keep dot > 0,
+//     impossible for k rhi <= 0.6), increasing in k and in ro;
+//   mode Z: L2 is itself a bound on |dphi|, taken at the box extremes.
+// Every bound is loosened by 2e-3 relative and 2e-4 rad (fp32 evaluation error ~1e-6); a NaN never
+// rejects.  It is a NECESSARY condition of ls_tier1_f, hence of the fp64 decision.
+LST_HD bool ls_row_window(const Params &g, float ri, float zi, int ci, float rlo, float rhi, float zlo, float zhi,
+                          int cB, float *W) {
+  const float ns = g.f_ns;
+  const float n1 = ri * zlo - zi * rlo, n2 = ri * zlo - zi * rhi, n3 = ri * zhi - zi * rlo, n4 = ri * zhi - zi * rhi;
+  const float nmin = fminf(fminf(n1, n2), fminf(n3, n4)), nmax = fmaxf(fmaxf(n1, n2), fmaxf(n3, n4));
+  const float azo = fmaxf(fabsf(zlo), fabsf(zhi));
+  const float E = ri * g.f_sig_z[cB] + rhi * g.f_sig_z[ci] + azo * g.f_sig_r[ci] + fabsf(zi) * g.f_sig_r[cB];
+  const float dr = fmaxf(fabsf(rhi - ri), fabsf(rlo - ri));
+  const float rhs = (g.f_z0max * dr + ns * E) * 1.002f + 0.05f;
+  if (nmin > rhs || nmax < -rhs) return false;                                                  // L1
+  const float tol = ns * (LST_FDIV(g.f_sig_t[ci], ri) + LST_FDIV(g.f_sig_t[cB], rlo));
+  float w = 4.0f;
+  if (cB < 2) {
+    const float cmin = rlo - ri;
+    if (cmin > 1.0f) {
+      const float k = (g.f_kmax + LST_FDIV(tol, cmin)) * 1.002f;
+      if (k * rhi <= 0.6f) w = (asinf(k * rhi) - asinf(k * ri)) * 1.002f + 2e-4f;              // L2, mode R
+    }
+  } else {
+    const float azo0 = (zlo <= 0.0f && zhi >= 0.0f) ? 0.0f : fminf(fabsf(zlo), fabsf(zhi));
+    const float dzmax = fmaxf(fabsf(zhi - zi), fabsf(zlo - zi));
+    const float den = 0.5f * (fabsf(zi) + azo0) - g.f_z0max - 0.5f * ns * g.f_sig_z[ci];
+    if (den > 1.0f) {
+      const float x = fminf(1.0f, g.f_kmax * (0.5f * (ri + rhi) + 0.5f * ns * (g.f_sig_r[ci] + g.f_sig_r[cB])));
+      w = (LST_FDIV((dzmax + ns * g.f_sig_z[ci]) * asinf(x), den) + tol) * 1.002f + 2e-4f;     // L2, mode Z
+    }
+  }
+  *W = w;
+  return true;
+}
+
 // ------------------------------------------------------------------ C4 triplet
 struct T3Out { double kappa3, sigk3, beta; };
 
