@@ -420,7 +420,7 @@ def kernel_table(lst, B, devt, streams, a, geom, nnz, peak, alu_peak):
     cnt, cand = lst.lst_get_counts(0)
     n = {"hits": int(h[0].numel()), "seeds": int(s[0].numel()), "md": int(cnt[0]), "ls": int(cnt[1]), "t3": int(cnt[2]),
          "t5": int(cnt[3]), "pt3": int(cnt[4]), "pt5": int(cnt[5]), "tc": int(cnt[6]),
-         "cand": [int(c) for c in cand[:6]], "surv": [int(c) for c in cand[6:12]],
+         "cand": [int(c) for c in cand[:6]], "surv": [int(c) for c in cand[6:12]], "eval": [int(c) for c in cand[12:18]],
          "n_modules": int(geom.n_modules), "nnz": int(nnz)}
     names = [k for k, _ in runs[0]]
     med = np.median(np.array([[m for _, m in r] for r in runs]), axis=0)
@@ -487,6 +487,7 @@ def main():
                        "parallelism": "replicas only (no collective)", "objects_event0": {k: n[k] for k in (
                            "hits", "seeds", "md", "ls", "t3", "t5", "pt3", "pt5", "tc")},
                        "candidates_event0": dict(zip(("md", "ls", "t3", "t5", "pt5", "pt3"), n["cand"][:6])),
+                       "candidates_visited_event0": dict(zip(("md", "ls", "t3", "t5", "pt5", "pt3"), n["eval"][:6])),
                        "prefilter_survivors_event0": dict(zip(("md", "ls", "t3", "t5", "pt5", "pt3"), n["surv"][:6]))},
             "clocks": clocks,
             "gpu_launches": int(launches * a.events * a.steps),

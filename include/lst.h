@@ -70,6 +70,12 @@ typedef struct {
   float cap_pt3_per_seed, cap_pt5_per_seed;
   float cap_mdcand_per_hit, cap_lscand_per_hit, cap_t3cand_per_hit, cap_t5cand_per_hit;
   int32_t use_cuda_graph;  /* 1: lst_run replays one captured CUDA graph per slot               */
+  int32_t enum_pruning;    /* enumeration shortcuts that never change a result (tests compare with 0):
+                              bit 0: lst_create drops the module-map edges whose two lower-sensor boxes
+                                     cannot hold a line segment (uses the boxes of lst_geometry);
+                              bit 1: the LS pre-filter visits, per inner MD and connected module, only
+                                     the MDs inside the azimuthal window / pointing cone that the cuts
+                                     allow (uses the event's own MD positions only).  Default 3.      */
 } lst_config;
 
 /* Detector description, HOST arrays of length n_modules (copied by the callee).  A module is a
@@ -176,9 +182,11 @@ int lst_run(lst_ctx *ctx, uint32_t slot, void *cuda_stream);
 int lst_get_objects(lst_ctx *ctx, uint32_t slot, lst_level level, int copy_to_host, lst_objects *out);
 
 /* Per-level object counts of the slot's last run (synchronises); counts: uint32[LST_NLEVEL], HOST.
- * Also cheap way to wait for a slot.  cand (optional, may be NULL): candidates evaluated for
- * MD, LS, T3, T5, pT5, pT3, then the candidates that survived each stage's fp32 pre-filter and were
- * decided in fp64, same order (uint64[12]). */
+ * Also cheap way to wait for a slot.  cand (optional, may be NULL; uint64[18]), each in the order
+ * MD, LS, T3, T5, pT5, pT3: [0..5] the candidates of the method's definition (e.g. LS: all MD pairs
+ * in map-connected modules), [6..11] those that survived the stage's fp32 pre-filter and were
+ * decided in fp64, [12..17] those the pre-filter kernel actually evaluated (fewer than [0..5] where
+ * the enumeration is restricted to a window, see lst_config.enum_pruning). */
 int lst_get_counts(lst_ctx *ctx, uint32_t slot, uint32_t *counts, uint64_t *cand);
 
 /* Number of kernels the last lst_run / lst_run_timed of this context enqueued (or captured into

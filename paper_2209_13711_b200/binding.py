@@ -22,7 +22,8 @@ LEVEL_NAMES = ("MD", "LS", "T3", "T5", "PT3", "PT5", "TC")
 
 EXPORTS = ("lst_default_config", "lst_build_module_map", "lst_free", "lst_create", "lst_destroy",
            "lst_workspace_bytes", "lst_bind_workspace", "lst_load_event", "lst_run", "lst_get_objects",
-           "lst_get_counts", "lst_launches_per_run", "lst_run_timed", "lst_strerror", "lst_host_eval")
+           "lst_get_counts", "lst_launches_per_run", "lst_run_timed", "lst_strerror")
+TEST_EXPORTS = ("lst_host_eval", "lst_host_ls_window")      # include/lst_test.h
 
 
 class lst_config(C.Structure):
@@ -35,7 +36,7 @@ class lst_config(C.Structure):
         (n, C.c_float) for n in (
             "cap_md_per_hit", "cap_ls_per_hit", "cap_t3_per_hit", "cap_t5_per_hit", "cap_pt3_per_seed",
             "cap_pt5_per_seed", "cap_mdcand_per_hit", "cap_lscand_per_hit", "cap_t3cand_per_hit",
-            "cap_t5cand_per_hit")] + [("use_cuda_graph", C.c_int32)]
+            "cap_t5cand_per_hit")] + [("use_cuda_graph", C.c_int32), ("enum_pruning", C.c_int32)]
 
 
 class lst_geometry(C.Structure):
@@ -103,6 +104,7 @@ def lib():
         L.lst_strerror.argtypes = [C.c_int]
         L.lst_strerror.restype = C.c_char_p
         L.lst_host_eval.argtypes = [C.POINTER(lst_config), C.c_int, u32, vp, vp, vp, vp, vp, vp]
+        L.lst_host_ls_window.argtypes = [C.POINTER(lst_config), u32, vp, vp, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -157,6 +159,18 @@ def lst_host_eval(level, pts, cats, aux=None, cfg: lst_config | None = None):
     _check(lib().lst_host_eval(C.byref(cfg) if cfg is not None else None, level, n, _p(pts), _p(cats), _p(aux),
                                _p(ok), _p(pre), _p(f)), "lst_host_eval")
     return ok.astype(bool), pre.astype(bool), f
+
+
+def lst_host_ls_window(row, row_cat, box, box_cat, cfg: lst_config | None = None):
+    """Test hook: ls_row_window on the host -> (live [n] bool, w [n] f32)."""
+    row = np.ascontiguousarray(row, dtype=np.float32)
+    box = np.ascontiguousarray(box, dtype=np.float32)
+    rc, bc = (np.ascontiguousarray(a, dtype=np.uint8) for a in (row_cat, box_cat))
+    n = row.shape[0]
+    live, w = np.zeros(n, np.uint8), np.zeros(n, np.float32)
+    _check(lib().lst_host_ls_window(C.byref(cfg) if cfg is not None else None, n, _p(row), _p(rc), _p(box), _p(bc),
+                                    _p(live), _p(w)), "lst_host_ls_window")
+    return live.astype(bool), w
 
 
 class LST:
@@ -249,7 +263,7 @@ class LST:
 
     def lst_get_counts(self, slot):
         cnt = np.zeros(LST_NLEVEL, np.uint32)
-        cand = np.zeros(12, np.uint64)
+        cand = np.zeros(18, np.uint64)
         _check(lib().lst_get_counts(self._h, slot, _p(cnt), _p(cand)), "lst_get_counts")
         return cnt, cand
 

@@ -194,6 +194,9 @@ __global__ void __launch_bounds__(256) k_emit_fill(SlotDev s, int stage) {
     }
     st.unit_group[u] = lo;
   }
+  // LS: the pre-filter kernel walks rows, not items, so the pass-bit masks are cleared here
+  if (stage == S_LS)
+    for (size_t w = tid; w < (size_t)n_items * kItemWords; w += nt) st.mask[w] = 0;
 }
 
 // ------------------------------------------------------------------ per-item pass counts from the masks

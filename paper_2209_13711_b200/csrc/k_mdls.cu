@@ -97,191 +97,267 @@ __global__ void __launch_bounds__(256) k_md_fill(GeoDev geo, SlotDev s) {
 }
 
 // =================================================================== LS
-// Group of module A: rows = MDs of A, width W_A = number of MDs in the modules connected to A.
-__global__ void k_ls_groups(GeoDev geo, SlotDev s) {
+// Group of module A: rows = MDs of A, width W_A = number of MDs in the modules connected to A (the
+// candidates of the method's definition: all MD pairs in map-connected modules; a candidate's pass
+// bit sits at (row, column) of that rectangle whatever part of it the enumeration visits).  The same
+// warp also writes A's ModEv record for the per-row windows of k_ls_eval.
+__global__ void __launch_bounds__(256) k_ls_groups(GeoDev geo, SlotDev s) {
   const StageBuf &st = s.st[S_LS];
-  for (uint32_t A = blockIdx.x * blockDim.x + threadIdx.x; A < geo.n_modules; A += gridDim.x * blockDim.x) {
-    const uint32_t R = s.md_mod_off[A + 1] - s.md_mod_off[A];
+  const int lane = threadIdx.x & 31;
+  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+  for (uint32_t A = warp; A < geo.n_modules; A += nwarp) {
+    const uint32_t m0 = s.md_mod_off[A], R = s.md_mod_off[A + 1] - m0;
     uint32_t W = 0;
+    float rlo = 3.0e38f, rhi = -3.0e38f, zlo = 3.0e38f, zhi = -3.0e38f;
+    float pmin = 0.0f, inv_w = 0.0f;
+    uint32_t edge_cnt = 0;
     if (R) {
-      for (uint32_t e = geo.map_off[A]; e < geo.map_off[A + 1]; ++e) {
-        const uint32_t B = geo.map_cols[e];
-        W += s.md_mod_off[B + 1] - s.md_mod_off[B];
+      // the column of A's candidate rectangle at which each connected module's MDs start
+      const uint32_t e0 = geo.map_off[A], e1 = geo.map_off[A + 1];
+      for (uint32_t eb = e0; eb < e1; eb += 32) {
+        const uint32_t e = eb + lane;
+        uint32_t n = 0;
+        if (e < e1) { const uint32_t B = geo.map_cols[e]; n = s.md_mod_off[B + 1] - s.md_mod_off[B]; }
+        uint32_t tot;
+        const uint32_t ex = warp_excl_scan(n, &tot);
+        if (e < e1) s.edge_col0[e] = W + ex;
+        W += tot;
+      }
+      for (uint32_t k = lane; k < R; k += 32) {
+        const float4 p = s.md_pos[m0 + k];
+        rlo = fminf(rlo, p.w); rhi = fmaxf(rhi, p.w); zlo = fminf(zlo, p.z); zhi = fmaxf(zhi, p.z);
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        rlo = fminf(rlo, __shfl_xor_sync(0xffffffffu, rlo, o)); rhi = fmaxf(rhi, __shfl_xor_sync(0xffffffffu, rhi, o));
+        zlo = fminf(zlo, __shfl_xor_sync(0xffffffffu, zlo, o)); zhi = fmaxf(zhi, __shfl_xor_sync(0xffffffffu, zhi, o));
+      }
+      // keys ascend inside a module: lane j counts the MDs below edge j + 1 of kModBins equal bins
+      pmin = s.md_prel[m0];
+      const float span = s.md_prel[m0 + R - 1] - pmin;
+      if (R <= 0xFFFFu && span > 1e-6f) {
+        inv_w = (float)kModBins / span;
+        if (lane < kModBins - 1) {
+          const float edge = pmin + (float)(lane + 1) * (span * (1.0f / (float)kModBins));
+          uint32_t x = m0, y = m0 + R;
+          while (x < y) { const uint32_t mid = (x + y) >> 1; if (s.md_prel[mid] < edge) x = mid + 1; else y = mid; }
+          edge_cnt = x - m0;
+        }
       }
     }
-    st.gR[A] = R;
-    st.gW[A] = W;
+    // assemble the record: lanes 0 .. 13 hold the 14 counts
+    const uint32_t c_even = __shfl_sync(0xffffffffu, edge_cnt, (2 * lane) & 31), c_odd = __shfl_sync(0xffffffffu, edge_cnt, (2 * lane + 1) & 31);
+    uint32_t word = 0;
+    if (lane == 0) word = __float_as_uint(rlo);
+    else if (lane == 1) word = __float_as_uint(rhi);
+    else if (lane == 2) word = __float_as_uint(zlo);
+    else if (lane == 3) word = __float_as_uint(zhi);
+    else if (lane == 4) word = __float_as_uint(pmin);
+    else if (lane == 5) word = __float_as_uint(inv_w);
+    else if (lane == 6) word = __float_as_uint(geo.phic[A]);
+    else if (lane == 7) word = m0;
+    else if (lane == 8) word = R | ((uint32_t)geo.category[A] << 30);
+    if (lane < 7) {   // words 9 .. 15 = cum[0 .. 13]
+      const uint32_t packed = (c_even & 0xFFFFu) | (c_odd << 16);
+      reinterpret_cast<uint32_t *>(&s.mod_ev[A])[9 + lane] = packed;
+    }
+    if (lane < 9) reinterpret_cast<uint32_t *>(&s.mod_ev[A])[lane] = word;
+    if (lane == 0) {
+      st.gR[A] = R;
+      st.gW[A] = W;
+    }
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) s.hdr->n_groups[S_LS] = geo.n_modules;
 }
 
-// Stage the module-map row of A: per connected module its first MD and the running MD count.
-struct MapRow {
-  uint32_t start[kMaxDeg];
-  uint32_t cum[kMaxDeg + 1];
-  int deg;
-};
-__device__ __forceinline__ void stage_map_row(MapRow &mr, const GeoDev &geo, const SlotDev &s, uint32_t A) {
-  const int tid = threadIdx.x;
-  const uint32_t e0 = geo.map_off[A];
-  const int deg = (int)(geo.map_off[A + 1] - e0);
-  if (tid == 0) mr.deg = deg;
-  // deg <= kMaxDeg: sequential warp scan over the row by warp 0
-  if (tid < 32) {
-    uint32_t carry = 0;
-    for (int b = 0; b < deg; b += 32) {
-      const int e = b + tid;
-      uint32_t n = 0, st0 = 0;
-      if (e < deg) {
-        const uint32_t B = geo.map_cols[e0 + e];
-        st0 = s.md_mod_off[B];
-        n = s.md_mod_off[B + 1] - st0;
-      }
-      uint32_t tot;
-      const uint32_t ex = warp_excl_scan(n, &tot);
-      if (e < deg) { mr.start[e] = st0; mr.cum[e] = carry + ex; }
-      carry += tot;
-    }
-    if (tid == 0) mr.cum[deg] = carry;
-  }
+// k_ls_eval: the fp32 pre-filter of the LS stage.  A warp takes kLsGrab consecutive rows (inner MDs)
+// at a time, handed out dynamically.  The definition is "all MDs of the modules connected to the
+// row's module"; the enumeration visits only the MDs that can pass cuts L1 / L2 for THAT row:
+//   * the (row, connected module) pairs of the grabbed rows are flattened over the lanes; a lane tests
+//     the box of its module's MD anchors against its row's pointing cone (L1) and azimuthal window
+//     (L2), ls_row_window, and turns the window into an index range of the module's MDs (they ascend
+//     in azimuth) through the bin counts of the module's ModEv record: no search, one 64-byte load;
+//   * the ranges of 32 pairs are flattened again: lane c takes candidate c of their concatenation
+//     (its segment = number of segment starts <= c, from one __reduce_or_sync of the start bits);
+//   * tier 1 (ls_tier1_f; for an outer MD in a barrel module also L3, ls_l3_modeR_f) on every visited
+//     candidate; mode-R survivors go straight to the stage's candidate list, mode-Z survivors
+//     through a warp queue to ls_pre_f on 32 dense lanes.
+// A candidate's key is that of the full rectangle: key_base(row) + column index in the row's column list.
+constexpr int kLsGrab = 4;
+// count word of edge k (1 <= k <= 14): cum(k) = cum[k - 1] sits in u16 slot k - 1 of the 7 words q2.y .. q3.w
+__device__ __forceinline__ uint32_t bin_cum(const uint4 &q2, const uint4 &q3, int k, uint32_t n) {
+  if (k <= 0) return 0u;
+  if (k >= kModBins) return n;
+  const int wi = (k - 1) >> 1;
+  const uint32_t w = wi == 0 ? q2.y : (wi == 1 ? q2.z : (wi == 2 ? q2.w : (wi == 3 ? q3.x : (wi == 4 ? q3.y : (wi == 5 ? q3.z : q3.w)))));
+  return (k & 1) ? (w & 0xFFFFu) : (w >> 16);
 }
-// column j of A's candidate list -> MD index
-__device__ __forceinline__ uint32_t map_col_to_md(const MapRow &mr, uint32_t j) {
-  int lo = 0, hi = mr.deg;            // find last e with cum[e] <= j
-  while (hi - lo > 1) {
-    const int mid = (lo + hi) >> 1;
-    if (mr.cum[mid] <= j) lo = mid; else hi = mid;
-  }
-  return mr.start[lo] + (j - mr.cum[lo]);
-}
-
-// One block per WORK UNIT (k_emit_items): up to kUnitItems items of module A that share one column
-// tile; the MDs of the connected modules (columns) and the unit's rows are staged in shared memory
-// once (an inner-barrel module compares each of its ~30 MDs with ~1200 MDs of ~64 neighbours).
-// After the staging the warps work independently, without block barriers: a warp owns 32 columns
-// (kept in registers) and walks the rows (broadcast reads); three stages connected by warp queues:
-//   tier 1 (ls_tier1_f: no division / sqrt / atan, ~82 % rejected) on every candidate,
-//   tier 2 (ls_pre_f, full fp32) on 32 queued survivors at a time,
-//   the fp64 decision on 32 queued tier-2 survivors at a time (~3 % of the candidates).
-struct LsWarpMem {                    // the warps' queues: live only in the candidate phase of a unit
-  uint32_t q1[kThreads / 32][64];
-  ClStage cl[kThreads / 32];
-};
-struct LsShared {
-  union {                             // the map row is needed only while the columns are staged
-    MapRow mr;
-    LsWarpMem w;
-  };
-  float4 c_pos[kItemCand];
-  uint32_t c_idc[kItemCand];          // MD index | category << 30
-  float4 r_pos[kUnitRows];
-  uint32_t r_idc[kUnitRows];
-  float4 tab[4];                      // per category: sig_z, sig_r, sig_t
+struct LsWarpSh {
+  uint32_t q1[3 * 64];
+  ClStage cl;
+  uint32_t seg_md[32], seg_key[32], seg_f[32], seg_row[32];
+  float4 r_pos[kLsGrab];             // the grabbed rows: anchor
+  float4 r_aux[kLsGrab];             // phi, kappa_MD, sigma_kappa_MD, category (as float bits)
+  uint32_t r_key[kLsGrab], r_e0[kLsGrab], r_pre[kLsGrab + 1];   // key_base, first map edge, prefix of the degrees
 };
 
-// Tier 2 on up to 32 queued tier-1 survivors; what passes goes to the stage's candidate list.
-// it0: item of the unit's first row chunk; consecutive row chunks are nct items apart.
-__device__ __forceinline__ void ls_stage2(const LsShared &sh, const SlotDev &s, const Params &g, WarpQueue &Q1,
-                                          ClBuf &cl, uint32_t rpi, int nj, uint32_t it0, uint32_t nct) {
-  uint32_t e = 0, mi = 0, mo = 0, key = 0;
+// Tier 2 (mode Z only) on up to 32 queued tier-1 survivors; what passes goes to the stage's candidate list.
+__device__ __forceinline__ void ls_stage2(const SlotDev &s, const Params &g, WarpQueue3 &Q1, ClBuf &cl) {
+  uint32_t mi = 0, mo = 0, key = 0;
   bool keep = false;
-  if (Q1.pop(&e)) {
-    const uint32_t r = e & 0xFFu, jj = e >> 8;
-    const float4 a = sh.r_pos[r], b = sh.c_pos[jj];
-    const uint32_t ia = sh.r_idc[r], ib = sh.c_idc[jj];
-    mi = ia & 0x3FFFFFFFu; mo = ib & 0x3FFFFFFFu;
+  if (Q1.pop(&mi, &mo, &key)) {
+    const float4 a = s.md_pos[mi], b = s.md_pos[mo];
     const float2 ka = s.md_kf[mi], kb = s.md_kf[mo];
-    keep = ls_pre_f(g, a.x, a.y, a.z, a.w, ka.x, ka.y, (int)(ia >> 30), b.x, b.y, b.z, b.w, kb.x, kb.y, (int)(ib >> 30));
-    const uint32_t q = r / rpi, c = (r - q * rpi) * (uint32_t)nj + jj;
-    key = (it0 + q * nct) * (uint32_t)kItemCand + c;
+    keep = ls_pre_f(g, a.x, a.y, a.z, a.w, ka.x, ka.y, (int)(s.md_mod[mi] & 3u), b.x, b.y, b.z, b.w, kb.x, kb.y,
+                    (int)(s.md_mod[mo] & 3u));
   }
   cl.push(s.hdr, s.st[S_LS], S_LS, keep, key, make_uint2(mi, mo));
 }
 
-__global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, Params g) {
-  __shared__ LsShared sh;
+__global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, Params g, int use_windows) {
+  __shared__ LsWarpSh sh_all[kThreads / 32];
+  __shared__ float4 tab[4];                     // per category: sig_z, sig_r, sig_t
   const StageBuf &st = s.st[S_LS];
-  const uint32_t n_units = s.hdr->n_units[S_LS];
-  const int tid = threadIdx.x, lane = tid & 31, wib = tid >> 5;
-  constexpr int kWarps = kThreads / 32;
-  if (tid < 4) sh.tab[tid] = make_float4(g.f_sig_z[tid], g.f_sig_r[tid], g.f_sig_t[tid], 0.0f);
-  WarpQueue Q1;
-  Q1.init(sh.w.q1[wib]);
+  const uint32_t n_md = s.hdr->n_obj[0];
+  const int tid = threadIdx.x, lane = tid & 31;
+  LsWarpSh &sh = sh_all[tid >> 5];
+  if (tid < 4) tab[tid] = make_float4(g.f_sig_z[tid], g.f_sig_r[tid], g.f_sig_t[tid], 0.0f);
+  __syncthreads();
+  WarpQueue3 Q1;
+  Q1.init(sh.q1);
   ClBuf cl;
-  cl.init(&sh.w.cl[wib]);
-  __shared__ uint32_t sh_unit[2];
-  __shared__ int sh_task;                       // next (chunk, row group) task of the unit: warps take them dynamically
+  cl.init(&sh.cl);
+  const uint32_t le_mask = 0xFFFFFFFFu >> (31 - lane);
+  unsigned long long n_eval = 0;
+  const bool live_stage = s.hdr->n_items[S_LS] != 0;     // 0: nothing to do, or the work list overflowed
   for (;;) {
-    __syncthreads();                            // the previous unit is done with the shared arrays
-    if (tid == 0) {                             // units are handed out dynamically (their cost varies 100x)
-      const uint32_t nu = atomicAdd(&s.hdr->next_unit[S_LS], 1u);
-      sh_unit[0] = nu;
-      sh_unit[1] = nu < n_units ? st.unit_group[nu] : 0u;
-      sh_task = 0;
-    }
-    __syncthreads();
-    const uint32_t u = sh_unit[0];
-    if (u >= n_units) break;
-    const uint32_t A = sh_unit[1], lu = u - st.g_unit0[A];
-    const uint32_t R = st.gR[A], W = st.gW[A];
-    const uint32_t nct = item_nct(W), rpi = item_rpi(W), ipu = unit_items(W);
-    const uint32_t nq = (R + rpi - 1) / rpi;
-    const uint32_t ct = lu % nct, q0 = (lu / nct) * ipu;
-    const uint32_t qn = min(ipu, nq - q0);
-    const uint32_t j0 = ct * kItemCand;
-    const int nj = (int)min((uint32_t)kItemCand, W - j0);
-    const uint32_t md0 = s.md_mod_off[A], item0 = st.g_item0[A];
-    const uint32_t row0 = q0 * rpi, it0 = item0 + q0 * nct + ct;
-    const int nrows = (int)min(R - row0, qn * rpi);      // <= kUnitRows
-    stage_map_row(sh.mr, geo, s, A);
-    for (int k = tid; k < nrows; k += kThreads) {
-      const uint32_t md = md0 + row0 + k;
-      sh.r_pos[k] = s.md_pos[md];
-      sh.r_idc[k] = md | ((s.md_mod[md] & 3u) << 30);
-    }
-    for (int k = tid; k < (int)(qn * kItemWords); k += kThreads)      // the decide kernel ORs the pass bits in
-      st.mask[(size_t)(it0 + (k / kItemWords) * nct) * kItemWords + (k % kItemWords)] = 0;
-    __syncthreads();
-    for (int k = tid; k < nj; k += kThreads) {
-      const uint32_t md = map_col_to_md(sh.mr, j0 + k);
-      sh.c_pos[k] = s.md_pos[md];
-      sh.c_idc[k] = md | ((s.md_mod[md] & 3u) << 30);
-    }
-    __syncthreads();
-    // tasks: (32-column chunk, interleaved row group); with few chunks the rows are split over the warps
-    const int nchunk = (nj + 31) >> 5;
-    const int nrg = nchunk >= kWarps ? 1 : kWarps / nchunk;
-    for (;;) {
-      int t = 0;
-      if (lane == 0) t = atomicAdd(&sh_task, 1);
-      t = __shfl_sync(0xffffffffu, t, 0);
-      if (t >= nchunk * nrg) break;
-      const int chunk = t % nchunk, rg = t / nchunk;
-      const int jj = chunk * 32 + lane;
-      const bool has = jj < nj;
-      const float4 b = sh.c_pos[has ? jj : 0];
-      const uint32_t cb = sh.c_idc[has ? jj : 0] >> 30;
-      const float4 tb = sh.tab[cb];
-      // the 32 columns of a chunk nearly always share their mode (same or neighbouring modules):
-      // a warp-uniform mode lets the compiler drop the other mode's arithmetic from the loop
-      const bool all_z = __all_sync(0xffffffffu, !has || cb >= 2u), all_r = __all_sync(0xffffffffu, !has || cb < 2u);
-#define LST_LS_ROWS(OEC)                                                                                             \
-      for (int r = rg; r < nrows; r += nrg) {                                                                        \
-        const float4 a = sh.r_pos[r];                                                                                \
-        const float4 ta = sh.tab[sh.r_idc[r] >> 30];                                                                 \
-        const bool keep = has && ls_tier1_f(g, a.x, a.y, a.z, a.w, ta.x, ta.y, ta.z, b.x, b.y, b.z, b.w, tb.x, tb.y, \
-                                            tb.z, (OEC));                                                            \
-        Q1.push(keep, (uint32_t)r | ((uint32_t)jj << 8));                                                            \
-        if (Q1.n >= 32u) ls_stage2(sh, s, g, Q1, cl, rpi, nj, it0, nct);                                             \
+    uint32_t r0 = 0;
+    if (lane == 0) r0 = atomicAdd(&s.hdr->next_unit[S_LS], (uint32_t)kLsGrab);
+    r0 = __shfl_sync(0xffffffffu, r0, 0);
+    if (r0 >= n_md || !live_stage) break;
+    // ---- lanes 0 .. kLsGrab-1 set up one row each
+    uint32_t deg = 0;
+    if (lane < kLsGrab && r0 + lane < n_md) {
+      const uint32_t i = r0 + lane;
+      const uint32_t mc = s.md_mod[i], A = mc >> 2;
+      const uint32_t W = st.gW[A];
+      if (W) {
+        const float2 kf = s.md_kf[i];
+        const uint32_t r = i - s.md_mod_off[A];
+        uint32_t key_base;
+        if (W <= (uint32_t)kItemCand) {
+          const uint32_t rpi = item_rpi(W), q = r / rpi;
+          key_base = (st.g_item0[A] + q) * (uint32_t)kItemCand + (r - q * rpi) * W;
+        } else {
+          key_base = (st.g_item0[A] + r * item_nct(W)) * (uint32_t)kItemCand;
+        }
+        const uint32_t e0 = geo.map_off[A];
+        deg = geo.map_off[A + 1] - e0;
+        sh.r_pos[lane] = s.md_pos[i];
+        sh.r_aux[lane] = make_float4(s.md_phi[i], kf.x, kf.y, __uint_as_float(mc & 3u));
+        sh.r_key[lane] = key_base;
+        sh.r_e0[lane] = e0;
       }
-      if (all_r) { LST_LS_ROWS(false) }
-      else if (all_z) { LST_LS_ROWS(true) }
-      else { LST_LS_ROWS(cb >= 2u) }
-#undef LST_LS_ROWS
     }
-    while (Q1.n) ls_stage2(sh, s, g, Q1, cl, rpi, nj, it0, nct);
-    cl.flush_all(s.hdr, st, S_LS);      // the queues' memory is the next unit's map row
+    uint32_t P;
+    const uint32_t dpre = warp_excl_scan(deg, &P);
+    if (lane <= kLsGrab) sh.r_pre[lane] = dpre;             // r_pre[kLsGrab] = P (lanes >= kLsGrab have deg 0)
+    __syncwarp();
+    for (uint32_t pb = 0; pb < P; pb += 32) {
+      // ---- lanes = (row, connected module) pairs: the range of the module's MDs the row has to look at
+      const uint32_t pidx = pb + lane;
+      uint32_t md0 = 0, len = 0, cB = 0, kcol = 0, k = 0;
+      if (pidx < P) {
+#pragma unroll
+        for (int q = 1; q < kLsGrab; ++q) k += (sh.r_pre[q] <= pidx);
+        const uint32_t e = sh.r_e0[k] + (pidx - sh.r_pre[k]);
+        const uint4 *rec = reinterpret_cast<const uint4 *>(&s.mod_ev[geo.map_cols[e]]);
+        const uint4 q2 = rec[2];
+        const uint32_t n = q2.x & 0x3FFFFFFFu;
+        if (n) {
+          const uint4 q0 = rec[0], q1 = rec[1], q3 = rec[3];
+          cB = q2.x >> 30;
+          uint32_t lo = 0;
+          len = n;
+          if (use_windows) {
+            const float4 a = sh.r_pos[k], ax = sh.r_aux[k];
+            float w;
+            if (!ls_row_window(g, a.w, a.z, (int)__float_as_uint(ax.w), __uint_as_float(q0.x), __uint_as_float(q0.y),
+                               __uint_as_float(q0.z), __uint_as_float(q0.w), (int)cB, &w)) len = 0;
+            else {
+              const float pmin = __uint_as_float(q1.x), inv_w = __uint_as_float(q1.y);
+              const float d = ax.x - __uint_as_float(q1.z);
+              const float c = d - 6.2831853071795864769f * rintf(d * 0.15915494309189533577f);
+              if (fabsf(c) + w < 3.0f && inv_w > 0.0f) {
+                // no wrap-around inside [c - w, c + w]: the MDs whose key lies in it are a range; its ends
+                // are rounded outwards to the bin edges (1e-5 rad covers the rounding of the edge positions)
+                const float t_lo = (c - w - 1e-5f - pmin) * inv_w, t_hi = (c + w + 1e-5f - pmin) * inv_w;
+                const int k_lo = t_lo >= (float)kModBins ? kModBins : (t_lo > 0.0f ? (int)t_lo : 0);
+                const int k_hi = t_hi >= (float)(kModBins - 1) ? kModBins : (t_hi >= 0.0f ? (int)t_hi + 1 : 0);
+                lo = bin_cum(q2, q3, k_lo, n);
+                const uint32_t hi = bin_cum(q2, q3, k_hi, n);
+                len = hi > lo ? hi - lo : 0u;
+              }
+            }
+          }
+          md0 = q1.w + lo;
+          kcol = sh.r_key[k] + s.edge_col0[e] + lo;
+        }
+      }
+      uint32_t T;
+      const uint32_t fex = warp_excl_scan(len, &T);           // flat offset of the segment's first candidate
+      const uint32_t bal = __ballot_sync(0xffffffffu, len != 0);
+      const uint32_t nseg = __popc(bal);
+      if (len) {
+        const uint32_t pseg = __popc(bal & ((1u << lane) - 1u));
+        sh.seg_md[pseg] = md0 | (cB << 30);
+        sh.seg_key[pseg] = kcol;
+        sh.seg_f[pseg] = fex;
+        sh.seg_row[pseg] = k;
+      }
+      __syncwarp();
+      n_eval += T;
+      // ---- lanes = candidates of the concatenated ranges
+      uint32_t sbefore = 0;                   // segments that start before the current 32 candidates
+      for (uint32_t w0 = 0; w0 < T; w0 += 32) {
+        const uint32_t sidx = sbefore + lane;
+        uint32_t bit = 0;
+        if (sidx < nseg) { const uint32_t f = sh.seg_f[sidx]; if (f < w0 + 32u) bit = 1u << (f - w0); }
+        const uint32_t starts = __reduce_or_sync(0xffffffffu, bit);
+        const uint32_t f = w0 + lane;
+        bool keepR = false, keepZ = false;
+        uint32_t mi = 0, mo = 0, key = 0;
+        if (f < T) {
+          const uint32_t sg = sbefore + __popc(starts & le_mask) - 1u;
+          const uint32_t smd = sh.seg_md[sg], off = f - sh.seg_f[sg], kr = sh.seg_row[sg];
+          mo = (smd & 0x3FFFFFFFu) + off;
+          mi = r0 + kr;
+          key = sh.seg_key[sg] + off;
+          const float4 a = sh.r_pos[kr], ax = sh.r_aux[kr];
+          const float4 b = s.md_pos[mo];
+          const uint32_t ci = __float_as_uint(ax.w), co = smd >> 30;
+          const float4 ta = tab[ci], tb = tab[co];
+          const bool oec = co >= 2u;
+          bool keep = ls_tier1_f(g, a.x, a.y, a.z, a.w, ta.x, ta.y, ta.z, b.x, b.y, b.z, b.w, tb.x, tb.y, tb.z, oec);
+          if (keep && !oec) {
+            const float2 kb = s.md_kf[mo];
+            keep = ls_l3_modeR_f(g, a.x, a.y, a.w, ax.y, ax.z, ta.z, ci >= 2u, b.x, b.y, b.w, kb.x, kb.y, tb.z);
+          }
+          keepR = keep && !oec;
+          keepZ = keep && oec;
+        }
+        sbefore += __popc(starts);
+        cl.push(s.hdr, st, S_LS, keepR, key, make_uint2(mi, mo));
+        Q1.push(keepZ, mi, mo, key);
+        if (Q1.n >= 32u) ls_stage2(s, g, Q1, cl);
+      }
+      __syncwarp();                           // the segment table is rewritten by the next 32 pairs
+    }
+    __syncwarp();                             // ... and the row table by the next grab
   }
+  while (Q1.n) ls_stage2(s, g, Q1, cl);
+  cl.flush_all(s.hdr, st, S_LS);
+  if (lane == 0 && n_eval) atomicAdd(&s.hdr->cand_eval[S_LS], n_eval);     // n_eval is warp-uniform
 }
 
 // fp64 decision of the listed candidates, one thread each (dense warps, no staging); an accepted
@@ -338,9 +414,9 @@ void launch_md(const Ctx &c, const SlotDev &s, cudaStream_t st) {
 }
 
 void launch_ls(const Ctx &c, const SlotDev &s, cudaStream_t st) {
-  k_ls_groups<<<(c.geo.n_modules + 127) / 128, 128, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_ls_groups");
+  k_ls_groups<<<(c.geo.n_modules + 7) / 8, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_ls_groups");
   launch_emit(c, s, S_LS, -1, st);
-  k_ls_eval<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_ls_eval");
+  k_ls_eval<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par, c.ls_windows); LST_MARK(c, st, "k_ls_eval");
   k_ls_decide<<<persistent_grid(c, 4), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_ls_decide");
   launch_item_counts(c, s, S_LS, st);
   launch_scan_items(c, s, S_LS, 1, s.cap_ls, st);

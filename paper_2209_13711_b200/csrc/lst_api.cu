@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "../../include/lst.h"
+#include "../../include/lst_test.h"
 #include "lst_launch.h"
 
 using namespace lst;
@@ -80,6 +81,7 @@ extern "C" void lst_default_config(lst_config *c) {
   c->cap_t3cand_per_hit = 64.0f;
   c->cap_t5cand_per_hit = 16.0f;
   c->use_cuda_graph = 1;
+  c->enum_pruning = 3;
 }
 
 static void make_params(const lst_config &c, Params *p) {
@@ -282,6 +284,8 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.md_hit = w.take<uint2>(s.cap_md); s.md_mod = w.take<uint32_t>(s.cap_md); s.md_dphi = w.take<float>(s.cap_md);
   s.md_phi = w.take<float>(s.cap_md); s.md_prel = w.take<float>(s.cap_md);
   s.md_mod_off = w.take<uint32_t>(n_mod + 1);
+  s.mod_ev = w.take<ModEv>(n_mod);
+  s.edge_col0 = w.take<uint32_t>(std::max<uint32_t>(c->map_edges_used, 1));
   s.ls_md = w.take<uint2>(s.cap_ls); s.ls_f = w.take<float4>(s.cap_ls);
   s.ls_md_off = w.take<uint32_t>((size_t)s.cap_md + 1);
   s.t3_md = w.take<uint4>(s.cap_t3); s.t3_ls = w.take<uint2>(s.cap_t3); s.t3_kd = w.take<double2>(s.cap_t3);
@@ -446,6 +450,7 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
     return LST_EINVAL;
   }
   make_params(c->cfg, &c->k.par);
+  c->k.ls_windows = (c->cfg.enum_pruning & 2) != 0;
   c->n_slots = n_slots; c->max_hits = max_hits; c->max_seeds = max_seeds;
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
@@ -513,9 +518,10 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
     // the LS enumeration walks the map without its dead edges (ls_edge_possible)
     std::vector<uint32_t> poff(n + 1, 0u), pcols;
     pcols.reserve(nnz);
+    const bool drop_dead = (c->cfg.enum_pruning & 1) != 0;
     for (uint32_t m = 0; m < n; ++m) {
       for (uint32_t e = map->row_offsets[m]; e < map->row_offsets[m + 1]; ++e)
-        if (ls_edge_possible(c->k.par, g, m, map->cols[e])) pcols.push_back(map->cols[e]);
+        if (!drop_dead || ls_edge_possible(c->k.par, g, m, map->cols[e])) pcols.push_back(map->cols[e]);
       poff[m + 1] = (uint32_t)pcols.size();
     }
     c->map_edges = nnz; c->map_edges_used = (uint32_t)pcols.size();
@@ -718,7 +724,11 @@ extern "C" int lst_get_counts(lst_ctx *c, uint32_t slot, uint32_t *counts, uint6
   const int rc = sync_header(c, s);
   if (rc != LST_OK) return rc;
   for (int l = 0; l < LST_NLEVEL; ++l) counts[l] = s.h_hdr->n_obj[l];
-  if (cand) for (int k = 0; k < S_NSTAGE; ++k) { cand[k] = s.h_hdr->cand[k]; cand[S_NSTAGE + k] = s.h_hdr->cl_used[k]; }
+  if (cand) for (int k = 0; k < S_NSTAGE; ++k) {
+    cand[k] = s.h_hdr->cand[k];
+    cand[S_NSTAGE + k] = s.h_hdr->cl_used[k];
+    cand[2 * S_NSTAGE + k] = k == S_LS ? s.h_hdr->cand_eval[k] : s.h_hdr->cand[k];
+  }
   return LST_OK;
 }
 
@@ -794,22 +804,14 @@ extern "C" int lst_run_timed(lst_ctx *c, uint32_t slot, void *cuda_stream, uint3
   return LST_OK;
 }
 
-// ------------------------------------------------------------------ host test hooks
+// ------------------------------------------------------------------ host test hooks (include/lst_test.h)
 // Run the very same __host__ __device__ selection arithmetic on the CPU (tests only; no GPU needed).
-// pts: n * npts * 3 floats (x, y, z per point), cats: n * npts, aux: level-specific doubles.
-//   level MD : npts 2 (lower, upper), cats[0] = module category;             out f: kappa, sigk, dphi
-//   level LS : npts 2 (anchors), aux = {ki, ski, ko, sko};                  out f: kappa, sigk, dphi
-//   level T3 : npts 3;                                                      out f: kappa3, sigk3, beta
-//   level T5 : npts 5, aux = {k3a, sk3a, k3b, sk3b};                        out f: R, chi2, eta (pt, phi skipped)
-// pass[i] = fp64 decision, pre[i] = fp32 pre-filter verdict (1 where the level has none).
 extern "C" int lst_host_eval(const lst_config *cfg_in, int level, uint32_t n, const float *pts, const uint8_t *cats,
                              const double *aux, uint8_t *pass, uint8_t *pre, double *f) {
   lst_config cfg;
   if (cfg_in) cfg = *cfg_in; else lst_default_config(&cfg);
   Params g;
   make_params(cfg, &g);
-  const bool tier1_only = level == 101;   // diagnostics: pre = LS tier 1 alone, pass = full fp32 pre-filter
-  if (tier1_only) level = LST_LS;
   const int npts = level == LST_MD ? 2 : level == LST_LS ? 2 : level == LST_T3 ? 3 : level == LST_T5 ? 5 : 0;
   if (!npts || !pts || !cats || !pass) return LST_EINVAL;
   for (uint32_t i = 0; i < n; ++i) {
@@ -830,15 +832,13 @@ extern "C" int lst_host_eval(const lst_config *cfg_in, int level, uint32_t n, co
       LsOut o = {0, 0, 0};
       ok = ls_eval_d(g, P[0], a[0], a[1], P[1], a[2], a[3], &o);
       const float ri = sqrtf(p[0] * p[0] + p[1] * p[1]), ro = sqrtf(p[3] * p[3] + p[4] * p[4]);
+      // what k_ls_eval applies: tier 1, then L3 in its mode-R form or the full mode-Z pre-filter
       pr = ls_tier1_f(g, p[0], p[1], p[2], ri, g.f_sig_z[ct[0]], g.f_sig_r[ct[0]], g.f_sig_t[ct[0]], p[3], p[4], p[5], ro,
                       g.f_sig_z[ct[1]], g.f_sig_r[ct[1]], g.f_sig_t[ct[1]], ct[1] >= 2) &&
-           ls_pre_f(g, p[0], p[1], p[2], ri, (float)a[0], (float)a[1], ct[0], p[3], p[4], p[5], ro, (float)a[2],
-                    (float)a[3], ct[1]);
-      if (tier1_only) {
-        ok = pr;
-        pr = ls_tier1_f(g, p[0], p[1], p[2], ri, g.f_sig_z[ct[0]], g.f_sig_r[ct[0]], g.f_sig_t[ct[0]], p[3], p[4], p[5], ro,
-                        g.f_sig_z[ct[1]], g.f_sig_r[ct[1]], g.f_sig_t[ct[1]], ct[1] >= 2);
-      }
+           (ct[1] < 2 ? ls_l3_modeR_f(g, p[0], p[1], ri, (float)a[0], (float)a[1], g.f_sig_t[ct[0]], ct[0] >= 2, p[3], p[4], ro,
+                                      (float)a[2], (float)a[3], g.f_sig_t[ct[1]])
+                      : ls_pre_f(g, p[0], p[1], p[2], ri, (float)a[0], (float)a[1], ct[0], p[3], p[4], p[5], ro, (float)a[2],
+                                 (float)a[3], ct[1]));
       o3[0] = o.kappa; o3[1] = o.sigk; o3[2] = o.dphi;
     } else if (level == LST_T3) {
       T3Out o = {0, 0, 0};
@@ -855,6 +855,22 @@ extern "C" int lst_host_eval(const lst_config *cfg_in, int level, uint32_t n, co
     pass[i] = ok;
     if (pre) pre[i] = pr;
     if (f) { f[3 * (size_t)i] = o3[0]; f[3 * (size_t)i + 1] = o3[1]; f[3 * (size_t)i + 2] = o3[2]; }
+  }
+  return LST_OK;
+}
+
+extern "C" int lst_host_ls_window(const lst_config *cfg_in, uint32_t n, const float *row, const uint8_t *row_cat,
+                                  const float *box, const uint8_t *box_cat, uint8_t *live, float *w) {
+  if (!row || !row_cat || !box || !box_cat || !live || !w) return LST_EINVAL;
+  lst_config cfg;
+  if (cfg_in) cfg = *cfg_in; else lst_default_config(&cfg);
+  Params g;
+  make_params(cfg, &g);
+  for (uint32_t i = 0; i < n; ++i) {
+    float ww = 4.0f;
+    live[i] = ls_row_window(g, row[2 * i], row[2 * i + 1], row_cat[i] & 3, box[4 * i], box[4 * i + 1], box[4 * i + 2],
+                            box[4 * i + 3], box_cat[i] & 3, &ww);
+    w[i] = ww;
   }
   return LST_OK;
 }

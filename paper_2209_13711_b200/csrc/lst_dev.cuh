@@ -107,6 +107,20 @@ struct StageBuf {        // work list of one stage
   uint32_t cap_groups, cap_items, cap_pool, cap_cl;
 };
 
+// Per module and event (k_ls_groups): everything a row of the LS pre-filter needs about the MDs of a
+// connected module, in one 64-byte record: the bounding box of their anchors, their first index and
+// count, and where their azimuth keys (md_prel, ascending) cross 14 equidistant edges between the
+// smallest and the largest key, so that an azimuthal window becomes an index range with no search.
+constexpr int kModBins = 15;
+struct __align__(16) ModEv {
+  float rlo, rhi, zlo, zhi;        // anchors: rt and z extent
+  float pmin, inv_w, phic;         // smallest key, bins per radian (0: no bin table), the module's centre azimuth
+  uint32_t first;                  // index of the module's first MD
+  uint32_t n_cat;                  // MDs in the module | category << 30
+  uint16_t cum[kModBins - 1];      // cum[j] = MDs with key < pmin + (j + 1) / inv_w
+};
+static_assert(sizeof(ModEv) == 64, "ModEv is one 64-byte record");
+
 // Static detector data (device), shared by all slots.
 struct GeoDev {
   uint32_t n_modules, n_det;
@@ -149,7 +163,8 @@ struct SlotDev {
   float *md_phi;         // azimuth of the anchor, fp32 (pixel-linking pre-filter)
   float *md_prel;        // the anchor's sort key (azimuth relative to the module centre): ascending inside a module
   uint32_t *md_mod_off;  // [n_modules+1]
-  float4 *md_box;        // [n_modules] bounding box of the module's MD anchors: rt min, rt max, z min, z max
+  ModEv *mod_ev;         // [n_modules] what the LS enumeration needs to know about a module's MDs in this event
+  uint32_t *edge_col0;   // [map edges] column of module A's candidate rectangle where the MDs of cols[e] start
   // LS
   uint2 *ls_md;          // inner, outer MD
   float4 *ls_f;          // dphi, kappa, sigma_kappa, 0

@@ -28,6 +28,7 @@ struct Ctx {             // what the launchers need from a context
   GeoDev geo;
   Params par;
   int n_sm;
+  int ls_windows = 1;    // lst_config.enum_pruning bit 1: per-row windows of the LS enumeration
 };
 
 // k_common.cu

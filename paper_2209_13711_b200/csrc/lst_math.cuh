@@ -352,6 +352,25 @@ LST_HD bool ls_row_window(const Params &g, float ri, float zi, int ci, float rlo
   return true;
 }
 
+// Mode-R line segments in one fp32 pass (the tier-1 conditions plus L3): for an outer MD in a barrel
+// module cut L3, |kappa_MD(m) - kappa_LS| <= N_s (sigma_MD(m) + sigma_LS) + 0.3 |kappa_LS| [m endcap],
+// multiplied through by chord * rt_i * rt_o, needs one square root and no division:
+//   |k_m c rr - cr| <= N_s (s_m c rr + tphi rr) + ec_m |cr|,   cr = cross(A, B), c = chord, rr = rt_i rt_o.
+// Same contract as ls_pre_f (may only reject beyond kPreSlack; NaN never rejects): a mode-R candidate
+// that passes ls_tier1_f and this needs no further fp32 test.
+LST_HD bool ls_l3_modeR_f(const Params &g, float xi, float yi, float ri, float ki, float ski, float sti, bool iec,
+                          float xo, float yo, float ro, float ko, float sko, float sto) {
+  const float rr = ri * ro;
+  const float cr = xi * yo - yi * xo;
+  const float dx = xo - xi, dy = yo - yi;
+  const float crr = sqrtf(dx * dx + dy * dy) * rr;
+  const float T = g.f_ns * (sti * ro + sto * ri);            // N_s tphi rr
+  const float eci = iec ? g.f_ec_md_sys * fabsf(cr) : 0.0f;
+  bool keep = !(fabsf(ki * crr - cr) > (g.f_ns * ski * crr + T + eci) * kPreSlack);
+  keep &= !(fabsf(ko * crr - cr) > (g.f_ns * sko * crr + T) * kPreSlack);
+  return keep;
+}
+
 // ------------------------------------------------------------------ C4 triplet
 struct T3Out { double kappa3, sigk3, beta; };
 

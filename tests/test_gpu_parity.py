@@ -139,6 +139,30 @@ def test_full_detector_chain(B, geom_full, map_full, cfg):
     lst.close()
 
 
+def test_enumeration_shortcuts_change_nothing(B, geom_full, map_full):
+    """lst_config.enum_pruning: the dead module-map edges dropped at lst_create (bit 0) and the per-row
+    windows of the LS pre-filter (bit 1) only skip candidates that cannot pass: with both switched
+    off the very same objects come out, in the same order, while far fewer candidates are visited."""
+    ev = lstgen.make_event(geom_full, "cfg3h")
+    out = {}
+    for mode in (0, 1, 2, 3):
+        cfg = B.lst_default_config()
+        cfg.enum_pruning = mode
+        lst = _gpu(B, geom_full, map_full, ev, cfg=cfg)
+        cnt, cand = lst.lst_get_counts(0)
+        out[mode] = (cnt.copy(), cand.copy(), [lst.lst_get_objects(0, lvl) for lvl in CHAIN])
+        lst.close()
+    for mode in (1, 2, 3):
+        assert np.array_equal(out[mode][0], out[0][0])
+        for a, b in zip(out[mode][2], out[0][2]):
+            assert np.array_equal(a["hits"], b["hits"]) and np.array_equal(a["f"], b["f"])
+    full, visited = int(out[0][1][1]), int(out[3][1][12 + 1])
+    assert int(out[0][1][12 + 1]) == full                       # no shortcut: every pair of the definition is visited
+    assert int(out[1][1][1]) < 0.9 * full                       # dead edges shrink the rectangle
+    assert visited < 0.4 * full, (visited, full)                # windows: less than 40 % of the pairs are looked at
+    print("LS candidates: definition %d, dead edges dropped %d, windows %d" % (full, int(out[1][1][1]), visited))
+
+
 def test_empty_and_tiny_events(B, geom_barrel, map_barrel):
     import dataclasses
     ev = lstgen.make_event(geom_barrel, "cfg1")

@@ -25,15 +25,24 @@ def _built():
     lst_build.build()
 
 
-def test_library_exports_every_declared_symbol():
-    hdr = open(os.path.join(ROOT, "include", "lst.h")).read()
+def _declared(header):
+    hdr = open(os.path.join(ROOT, "include", header)).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(lst_[a-z_]+)\s*\(", hdr))
+    return set(re.findall(r"\b(lst_[a-z_0-9]+)\s*\(", hdr))
+
+
+def test_library_exports_every_declared_symbol():
+    declared = _declared("lst.h")
     assert {"lst_create", "lst_load_event", "lst_run", "lst_get_objects"} <= declared
     L = B.lib()
     for name in sorted(declared):
         assert hasattr(L, name), name
-    assert declared <= set(B.EXPORTS)
+    assert declared == set(B.EXPORTS)
+    # the test hooks live in their own header and are not part of the product API
+    hooks = _declared("lst_test.h")
+    assert hooks == set(B.TEST_EXPORTS) and not (hooks & declared)
+    for name in sorted(hooks):
+        assert hasattr(L, name), name
 
 
 def test_default_config_matches_oracle_config():
@@ -203,3 +212,38 @@ def test_t3_t5_arithmetic_equals_oracle(geom_full, small_full):
     assert np.allclose(f[sel, 0], t5["f"][:, 0], rtol=1e-9)              # R
     assert np.allclose(f[sel, 1], t5["f"][:, 1], rtol=1e-6, atol=1e-9)   # chi2
     assert np.allclose(f[sel, 2], o.t5_kin()[:, 1], rtol=1e-9, atol=1e-12)  # eta
+
+
+def test_ls_row_window_never_excludes_an_accepted_pair(geom_full, map_full, small_full):
+    """The per-(inner MD, connected module) window of the LS enumeration (ls_row_window, run on the
+    host): for every LS the oracle accepts, the module box test is live and the pair's azimuth
+    difference lies inside the window; and the window does restrict (most module pairs are cut)."""
+    ev, o = small_full
+    md, xyz, mod, cat = _md_tables(geom_full, ev, o)
+    ls = o.get(O.LS)["parents"].astype(np.int64)
+    rt = np.hypot(xyz[:, 0].astype(np.float64), xyz[:, 1].astype(np.float64)).astype(np.float32)
+    z = xyz[:, 2].astype(np.float32)
+    nm = geom_full.n_modules
+    box = np.zeros((nm, 4), np.float32)
+    box[:, 0] = box[:, 2] = np.inf
+    box[:, 1] = box[:, 3] = -np.inf
+    np.minimum.at(box[:, 0], mod, rt); np.maximum.at(box[:, 1], mod, rt)
+    np.minimum.at(box[:, 2], mod, z); np.maximum.at(box[:, 3], mod, z)
+    i, oo = ls[:, 0], ls[:, 1]
+    live, w = B.lst_host_ls_window(np.stack([rt[i], z[i]], 1), cat[i], box[mod[oo]], cat[oo])
+    assert live.all()
+    phi = np.arctan2(xyz[:, 1].astype(np.float64), xyz[:, 0].astype(np.float64))
+    dphi = np.abs(np.remainder(phi[oo] - phi[i] + np.pi, 2 * np.pi) - np.pi)
+    assert (dphi <= w.astype(np.float64) - 1e-4).all()          # inside, with the 2e-4 margin to spare
+    assert (w < 3.2).mean() > 0.8
+    # all (row, connected module with MDs) pairs: a good part is dropped by the pointing cone alone
+    off, cols = map_full
+    has = np.bincount(mod, minlength=nm) > 0
+    rows, mods = [], []
+    for r in range(0, len(mod), 7):
+        Bs = cols[off[mod[r]]:off[mod[r] + 1]]
+        Bs = Bs[has[Bs]]
+        rows.append(np.full(len(Bs), r)); mods.append(Bs)
+    rows, mods = np.concatenate(rows), np.concatenate(mods).astype(np.int64)
+    live, w = B.lst_host_ls_window(np.stack([rt[rows], z[rows]], 1), cat[rows], box[mods], geom_full.category[mods])
+    assert 0.3 < live.mean() < 0.95
