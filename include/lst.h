@@ -13,7 +13,9 @@
  *   - one context = one detector (+ module map) on the CUDA device current at lst_create();
  *     a context owns n_slots independent event slots; calls on different slots may be issued
  *     on different CUDA streams concurrently ("multi-streaming").  Calls on
- *     one slot must be issued in order load -> run -> get from one host thread at a time.
+ *     one slot must be issued in order load -> run -> get from one host thread at a time;
+ *     different slots may be driven from different host threads (nothing shared is written after
+ *     lst_bind_workspace, which captures the slot's CUDA graph).
  *   - the library never allocates device memory after lst_create(): each slot works inside one
  *     caller-provided workspace (lst_workspace_bytes / lst_bind_workspace).
  */
@@ -28,7 +30,8 @@ extern "C" {
 
 typedef enum {
   LST_OK = 0,
-  LST_EINVAL = -1,  /* null pointer, out-of-range index, unsorted map, det >= 2*n_modules ...  */
+  LST_EINVAL = -1,  /* null pointer, out-of-range index, unsorted map, bad geometry; per event: det >=
+                       2*n_modules, NaN / infinite input, lower-sensor hit outside its module's box  */
   LST_ENOMEM = -2,  /* workspace too small, or an object collection overflowed its capacity     */
   LST_ECUDA = -3,   /* a CUDA call failed (sticky; text via lst_strerror)                       */
   LST_ESTATE = -4   /* call order violated (run before load, get before run, unbound workspace) */
@@ -80,7 +83,13 @@ typedef struct {
 
 /* Detector description, HOST arrays of length n_modules (copied by the callee).  A module is a
  * two-sensor "pT module"; the box is that of its LOWER sensor (nearer the
- * origin).  Hit det ids are det = 2*module + sensor, sensor 0 = lower, 1 = upper. */
+ * origin).  Hit det ids are det = 2*module + sensor, sensor 0 = lower, 1 = upper.
+ * PRECONDITION, checked for every event on the device: each lower-sensor hit lies inside its
+ * module's box (tolerance 5e-5 cm in r and z, 4e-6 rad in azimuth).  lst_create's dead-edge pruning
+ * and the pixel-seed windows are conservative interval arithmetic ON THESE BOXES, so a hit outside
+ * would silently lose objects: such an event is rejected with LST_EINVAL instead.
+ * lst_create / lst_build_module_map return LST_EINVAL unless 0 < rmin <= rmax, zmin <= zmax (equal
+ * and non-zero for endcap categories: the sensor plane), 0 < half_phi <= 0.6 rad, |phic| <= 2 pi. */
 typedef struct {
   uint32_t n_modules;
   const uint8_t *category;       /* 0 bPS, 1 b2S, 2 ePS, 3 e2S                                   */
@@ -119,7 +128,8 @@ typedef struct {
 
 /* A view of one object collection.  Pointers are DEVICE pointers into the slot workspace
  * (copy_to_host = 0) or HOST pointers into library-owned pinned staging (copy_to_host = 1);
- * both stay valid until the next lst_load_event / lst_get_objects(same level) on the slot.
+ * both stay valid until the next lst_load_event or lst_get_objects (ANY level: the staging is one
+ * buffer per slot) on the slot.
  *   hit_idx : n*arity ORIGINAL caller hit indices in layer order, lower hit before upper hit
  *             (arity: MD 2, LS 4, T3 6, T5 10, PT3 6, PT5 10, TC 14 = 10 OT (0xFFFFFFFF padded)
  *             + 4 pixel-hit ids (0xFFFFFFFF if none))
@@ -154,8 +164,9 @@ void lst_free(void *p);
 
 /* Create a context on the current CUDA device: validates and uploads geometry + map (the host
  * arrays may be freed afterwards).  max_hits / max_seeds bound every event of every slot.
- * LST_EINVAL: null / empty geometry, category > 3, layer > 15, map rows not ascending, column
- * out of range, map degree > 512. */
+ * LST_EINVAL: null / empty / inconsistent geometry (see lst_geometry), category > 3, layer > 15, map
+ * rows not ascending, column out of range, map degree > 512, or capacities (lst_config.cap_* x
+ * max_hits / max_seeds) beyond the 32-bit candidate keys (roughly max_hits > 4 M with the defaults). */
 int lst_create(const lst_geometry *geom, const lst_module_map *map, const lst_config *cfg /* NULL */,
                uint32_t n_slots, uint32_t max_hits, uint32_t max_seeds, lst_ctx **out);
 void lst_destroy(lst_ctx *ctx);
@@ -163,13 +174,17 @@ void lst_destroy(lst_ctx *ctx);
 /* Bytes of DEVICE workspace one slot needs (same for every slot). */
 size_t lst_workspace_bytes(const lst_ctx *ctx);
 /* Give slot `slot` its workspace: DEVICE memory, 256-byte aligned, >= lst_workspace_bytes(), owned
- * by the caller and borrowed until lst_destroy or the next bind.  LST_ENOMEM if too small. */
+ * by the caller and borrowed until lst_destroy or the next bind.  LST_ENOMEM if too small.  With
+ * lst_config.use_cuda_graph the slot's chain is captured and instantiated here (the one call after
+ * lst_create that allocates and synchronises); lst_run only replays it. */
 int lst_bind_workspace(lst_ctx *ctx, uint32_t slot, void *workspace, size_t bytes);
 
 /* a0: copy one event into the slot (async on `cuda_stream`, a cudaStream_t passed as void*).
  * seeds may be NULL (no pixel seeds: pT3 / pT5 are empty, TC = cleaned T5).
- * LST_EINVAL: n > max_hits / max_seeds, null array with n > 0.  det range is checked on the
- * device; an out-of-range det makes lst_get_objects return LST_EINVAL. */
+ * LST_EINVAL: n > max_hits / max_seeds, null array with n > 0.  The event's CONTENT is checked on the
+ * device by lst_run (det < 2 n_modules; x, y, z and the seed parameters finite; lower-sensor hits
+ * inside their module's box); a violation makes lst_get_objects / lst_get_counts return LST_EINVAL
+ * (lst_strerror names which), never a silently different result. */
 int lst_load_event(lst_ctx *ctx, uint32_t slot, const lst_hits *hits, const lst_pixel_seeds *seeds,
                    void *cuda_stream);
 
@@ -178,7 +193,7 @@ int lst_load_event(lst_ctx *ctx, uint32_t slot, const lst_hits *hits, const lst_
 int lst_run(lst_ctx *ctx, uint32_t slot, void *cuda_stream);
 
 /* Synchronise the slot's stream and return a view of one level.  LST_ENOMEM if a collection
- * overflowed its capacity, LST_EINVAL if the event had an invalid det id. */
+ * overflowed its capacity, LST_EINVAL if the event was invalid (see lst_load_event). */
 int lst_get_objects(lst_ctx *ctx, uint32_t slot, lst_level level, int copy_to_host, lst_objects *out);
 
 /* Per-level object counts of the slot's last run (synchronises); counts: uint32[LST_NLEVEL], HOST.

@@ -20,6 +20,19 @@ __global__ void k_hist(GeoDev geo, SlotDev s) {
     const uint32_t d = s.raw_det[h];
     if (d >= geo.n_det) { atomicOr(&s.hdr->err, (uint32_t)ERR_DET); continue; }
     atomicAdd(&s.det_cnt[d], 1u);
+    // input validation (include/lst.h): finite coordinates; a lower-sensor hit inside its module's box
+    // (the dead-edge pruning of lst_create and the pixel-seed windows rely on the boxes)
+    const float x = s.raw_x[h], y = s.raw_y[h], z = s.raw_z[h];
+    if (!(fabsf(x) <= 3.0e38f && fabsf(y) <= 3.0e38f && fabsf(z) <= 3.0e38f)) { atomicOr(&s.hdr->err, (uint32_t)ERR_NONFINITE); continue; }
+    if ((d & 1u) == 0u) {
+      const uint32_t m = d >> 1;
+      const float r = sqrtf(x * x + y * y);
+      const float dp = atan2f(y, x) - geo.phic[m];
+      const float dphi = fabsf(dp - 6.2831853071795864769f * rintf(dp * 0.15915494309189533577f));
+      const bool in = r >= geo.rmin[m] - kBoxTolLen && r <= geo.rmax[m] + kBoxTolLen && z >= geo.zmin[m] - kBoxTolLen &&
+                      z <= geo.zmax[m] + kBoxTolLen && dphi <= geo.hphi[m] + kBoxTolPhi + 4e-7f * (fabsf(geo.phic[m]) + 3.2f);
+      if (!in) atomicOr(&s.hdr->err, (uint32_t)ERR_BOX);
+    }
   }
 }
 

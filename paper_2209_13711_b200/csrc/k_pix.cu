@@ -131,6 +131,8 @@ __global__ void __launch_bounds__(256) k_px_modules(GeoDev geo, SlotDev s, Param
       const float pt = s.seed_pt[p], phi = s.seed_phi[p], z0 = s.seed_z0[p];
       const float kp = -(float)s.seed_q[p] * (float)g.kB / (2.0f * pt);
       const float sh = sinhf(s.seed_eta[p]);
+      if (lane == 0 && !(fabsf(pt) <= 3.0e38f && fabsf(s.seed_eta[p]) <= 3.0e38f && fabsf(phi) <= 3.0e38f && fabsf(z0) <= 3.0e38f))
+        atomicOr(&s.hdr->err, (uint32_t)ERR_NONFINITE);
       for (uint32_t w = lane; w < nw; w += 32) wbits[w] = 0;
       __syncwarp();
       for (uint32_t rb = 0; rb < geo.n_prow; rb += 32) {

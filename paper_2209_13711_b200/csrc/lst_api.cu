@@ -1,6 +1,7 @@
 // lst_api.cu -- the C-ABI of include/lst.h: context, module-map builder (host), workspace layout,
 // event upload, the launch chain (optionally one CUDA graph per slot) and result views.
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -17,10 +18,15 @@ using namespace lst;
 // ------------------------------------------------------------------ status text
 static thread_local char g_cuda_err[256] = "no CUDA error recorded";
 static thread_local char g_cap_err[256] = "workspace too small or object capacity exceeded";
+static thread_local char g_inval_err[192] = "invalid argument";
 
 static int cuda_fail(cudaError_t e, const char *where) {
   snprintf(g_cuda_err, sizeof(g_cuda_err), "CUDA error at %s: %s", where, cudaGetErrorString(e));
   return LST_ECUDA;
+}
+static int einval() {
+  snprintf(g_inval_err, sizeof(g_inval_err), "invalid argument");
+  return LST_EINVAL;
 }
 #define CU(call)                                          \
   do {                                                    \
@@ -31,7 +37,7 @@ static int cuda_fail(cudaError_t e, const char *where) {
 extern "C" const char *lst_strerror(int status) {
   switch (status) {
     case LST_OK: return "ok";
-    case LST_EINVAL: return "invalid argument";
+    case LST_EINVAL: return g_inval_err;
     case LST_ENOMEM: return g_cap_err;
     case LST_ECUDA: return g_cuda_err;
     case LST_ESTATE: return "call order violated";
@@ -111,8 +117,15 @@ static bool geometry_ok(const lst_geometry *g) {
   if (!g || g->n_modules == 0 || !g->category || !g->logical_layer || !g->rmin || !g->rmax || !g->phic ||
       !g->half_phi || !g->zmin || !g->zmax)
     return false;
-  for (uint32_t m = 0; m < g->n_modules; ++m)
+  for (uint32_t m = 0; m < g->n_modules; ++m) {
     if (g->category[m] > 3 || g->logical_layer[m] > 15) return false;
+    // a sane box: 0 < rmin <= rmax, zmin <= zmax (equal for an endcap module: the sensor plane, and not
+    // through z = 0), 0 < half_phi <= 0.6 rad (the azimuthal windows assume a module is narrow)
+    if (!(g->rmin[m] > 0.0f) || !(g->rmax[m] >= g->rmin[m]) || !(g->zmax[m] >= g->zmin[m])) return false;
+    if (!(g->half_phi[m] > 0.0f) || !(g->half_phi[m] <= 0.6f) || !(std::fabs(g->phic[m]) <= 6.3f)) return false;
+    if (g->category[m] >= 2 && (g->zmin[m] != g->zmax[m] || g->zmin[m] == 0.0f)) return false;
+    if (!(std::fabs(g->zmin[m]) <= 1e6f) || !(g->rmax[m] <= 1e6f)) return false;
+  }
   return true;
 }
 
@@ -168,7 +181,7 @@ inline bool reachable(const Box &A, const Box &B, double kp, double z0m, double 
 
 extern "C" int lst_build_module_map(const lst_geometry *g, const lst_config *cfg_in, uint32_t **row_offsets,
                                     uint32_t **cols) {
-  if (!geometry_ok(g) || !row_offsets || !cols) return LST_EINVAL;
+  if (!geometry_ok(g) || !row_offsets || !cols) return einval();
   lst_config cfg;
   if (cfg_in) cfg = *cfg_in; else lst_default_config(&cfg);
   const uint32_t n = g->n_modules;
@@ -219,6 +232,7 @@ struct Slot {
   float *h_f = nullptr;
   uint8_t *h_keep = nullptr;
   Header *h_hdr = nullptr;       // pinned
+  Recorder *timed = nullptr;     // lst_run_timed: events created on first use
 };
 
 struct lst_ctx {
@@ -229,10 +243,8 @@ struct lst_ctx {
   std::vector<Slot> slots;
   size_t ws_bytes = 0;
   size_t exp_obj_cap = 0, exp_hit_words = 0;
-  uint32_t launches = 0;         // kernels enqueued by the last chain (graph capture or direct)
+  std::atomic<uint32_t> launches{0};   // kernels of one chain (the same for every slot)
   uint32_t map_edges = 0, map_edges_used = 0;   // module-map edges given / kept for the LS enumeration
-  Recorder timed;                // lst_run_timed: events created on first use
-  bool timed_ready = false;
 };
 
 // bump allocator over the workspace; base == nullptr only measures
@@ -371,13 +383,13 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
 
 // Can ANY (inner anchor in module A's lower-sensor box, outer anchor in module B's) pass the LS
 // cuts L1 (pointing) and L2 (pT window) of reading C3?  Host, fp64, interval arithmetic on the two
-// boxes, every bound loosened (1e-3 relative, boxes grown by 1e-4 cm / 1e-6 rad for the fp32
-// rounding of the hits): false only for module pairs that cannot hold a line segment.  The module
+// boxes, every bound loosened (1e-3 relative, boxes grown by 1e-4 cm / 1e-5 rad: k_hist accepts a
+// lower-sensor hit up to 5e-5 cm / 4e-6 rad outside its box, else the event is LST_EINVAL): false only for module pairs that cannot hold a line segment.  The module
 // map is built with wider margins (kappa' = 1.25 kappa_max, z0' = 20 cm, a d0 allowance) than the
 // cuts use, so ~21 % of its edges are dead; dropping them from the LS enumeration changes no result.
 // Assumes what lst_geometry states: a lower-sensor hit lies inside its module's box.
 static bool ls_edge_possible(const Params &p, const lst_geometry *g, uint32_t A, uint32_t B) {
-  const double kEps = 1e-3, gl = 1e-4, ga = 1e-6, kPi = 3.14159265358979323846;
+  const double kEps = 1e-3, gl = 1e-4, ga = 1e-5, kPi = 3.14159265358979323846;
   const int cA = g->category[A] & 3, cB = g->category[B] & 3;
   const double ri0 = std::max(1e-6, (double)g->rmin[A] - gl), ri1 = (double)g->rmax[A] + gl;
   const double ro0 = std::max(1e-6, (double)g->rmin[B] - gl), ro1 = (double)g->rmax[B] + gl;
@@ -427,18 +439,18 @@ static bool ls_edge_possible(const Params &p, const lst_geometry *g, uint32_t A,
 
 extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, const lst_config *cfg_in,
                           uint32_t n_slots, uint32_t max_hits, uint32_t max_seeds, lst_ctx **out) {
-  if (!geometry_ok(g) || !map || !map->row_offsets || !out || n_slots == 0 || max_hits == 0) return LST_EINVAL;
+  if (!geometry_ok(g) || !map || !map->row_offsets || !out || n_slots == 0 || max_hits == 0) return einval();
   const uint32_t n = g->n_modules;
-  if (n > (1u << 29)) return LST_EINVAL;
-  if (map->row_offsets[0] != 0) return LST_EINVAL;
+  if (n > (1u << 29)) return einval();
+  if (map->row_offsets[0] != 0) return einval();
   const uint32_t nnz = map->row_offsets[n];
-  if (nnz && !map->cols) return LST_EINVAL;
+  if (nnz && !map->cols) return einval();
   for (uint32_t m = 0; m < n; ++m) {
     const uint32_t a = map->row_offsets[m], b = map->row_offsets[m + 1];
-    if (b < a || b > nnz || b - a > (uint32_t)kMaxDeg) return LST_EINVAL;
+    if (b < a || b > nnz || b - a > (uint32_t)kMaxDeg) return einval();
     for (uint32_t e = a; e < b; ++e) {
-      if (map->cols[e] >= n) return LST_EINVAL;
-      if (e > a && map->cols[e] <= map->cols[e - 1]) return LST_EINVAL;
+      if (map->cols[e] >= n) return einval();
+      if (e > a && map->cols[e] <= map->cols[e - 1]) return einval();
     }
   }
   lst_ctx *c = new (std::nothrow) lst_ctx();
@@ -447,7 +459,7 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   if (c->cfg.dup_t5_shared < 1 || c->cfg.dup_pt5_shared < 1 || c->cfg.dup_pt3_shared < 1 || !(c->cfg.pt_min > 0.0) ||
       !(c->cfg.dr2max >= 0.0)) {
     delete c;
-    return LST_EINVAL;
+    return einval();
   }
   make_params(c->cfg, &c->k.par);
   c->k.ls_windows = (c->cfg.enum_pruning & 2) != 0;
@@ -458,7 +470,6 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaGetDeviceProperties"); }
   c->k.n_sm = prop.multiProcessorCount;
-  if (const char *ev = getenv("LST_NSM")) { const int v = atoi(ev); if (v > 0) c->k.n_sm = v; }   // experiment knob
   // modules that may start a pixel-seeded object (C6 START layers)
   std::vector<uint32_t> start_mods;
   for (uint32_t m = 0; m < n; ++m)
@@ -566,15 +577,20 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   c->k.geo.start_mods = (const uint32_t *)(d + o_start);
   c->k.geo.n_start = (uint32_t)start_mods.size();
   c->slots.resize(n_slots);
-  c->ws_bytes = carve(c, nullptr, nullptr);
+  {
+    // candidate keys (item * 1024 + candidate), list positions and the TC index are 32-bit
+    SlotDev probe;
+    c->ws_bytes = carve(c, nullptr, &probe);
+    bool fits = (double)c->cfg.cap_pt5_per_seed * max_seeds + (double)c->cfg.cap_pt3_per_seed * max_seeds +
+                    (double)c->cfg.cap_t5_per_hit * max_hits + max_seeds < 4.0e9;
+    for (int k = 0; k < S_NSTAGE; ++k)
+      fits = fits && (double)probe.st[k].cap_items * kItemCand < 4.29e9 && 2.0 * (double)probe.st[k].cap_pool + 4096.0 < 4.29e9;
+    if (!fits) { cudaFree(c->d_static); delete c; return einval(); }
+  }
   *out = c;
   return LST_OK;
 }
 
-static void free_timed(lst_ctx *c) {
-  if (c->timed_ready) for (int k = 0; k <= Recorder::kMax; ++k) cudaEventDestroy(c->timed.ev[k]);
-  c->timed_ready = false;
-}
 static void free_slot_host(Slot &s) {
   if (s.graph) cudaGraphExecDestroy(s.graph);
   if (s.h_hits) cudaFreeHost(s.h_hits);
@@ -582,6 +598,7 @@ static void free_slot_host(Slot &s) {
   if (s.h_f) cudaFreeHost(s.h_f);
   if (s.h_keep) cudaFreeHost(s.h_keep);
   if (s.h_hdr) cudaFreeHost(s.h_hdr);
+  if (s.timed) { for (int k = 0; k <= Recorder::kMax; ++k) cudaEventDestroy(s.timed->ev[k]); delete s.timed; }
   s = Slot();
 }
 
@@ -589,15 +606,16 @@ extern "C" void lst_destroy(lst_ctx *c) {
   if (!c) return;
   cudaDeviceSynchronize();
   for (Slot &s : c->slots) free_slot_host(s);
-  free_timed(c);
   if (c->d_static) cudaFree(c->d_static);
   delete c;
 }
 
 extern "C" size_t lst_workspace_bytes(const lst_ctx *c) { return c ? c->ws_bytes : 0; }
 
+static int capture_slot_graph(lst_ctx *c, Slot &s);
+
 extern "C" int lst_bind_workspace(lst_ctx *c, uint32_t slot, void *workspace, size_t bytes) {
-  if (!c || slot >= c->n_slots || !workspace || ((uintptr_t)workspace & 255)) return LST_EINVAL;
+  if (!c || slot >= c->n_slots || !workspace || ((uintptr_t)workspace & 255)) return einval();
   if (bytes < c->ws_bytes) {
     snprintf(g_cap_err, sizeof(g_cap_err), "workspace too small: %zu bytes given, %zu needed", bytes, c->ws_bytes);
     return LST_ENOMEM;
@@ -608,6 +626,7 @@ extern "C" int lst_bind_workspace(lst_ctx *c, uint32_t slot, void *workspace, si
   s.workspace = workspace; s.ws_bytes = bytes;
   s.bound = true; s.loaded = false; s.ran = false;
   if (!s.h_hdr) CU(cudaMallocHost((void **)&s.h_hdr, sizeof(Header)));
+  if (c->cfg.use_cuda_graph) return capture_slot_graph(c, s);
   return LST_OK;
 }
 
@@ -619,13 +638,13 @@ __global__ void k_set_event(Header *h, uint32_t n_hits, uint32_t n_seeds) {
 
 extern "C" int lst_load_event(lst_ctx *c, uint32_t slot, const lst_hits *hits, const lst_pixel_seeds *seeds,
                               void *cuda_stream) {
-  if (!c || slot >= c->n_slots || !hits) return LST_EINVAL;
+  if (!c || slot >= c->n_slots || !hits) return einval();
   Slot &s = c->slots[slot];
   if (!s.bound) return LST_ESTATE;
   const uint32_t nh = hits->n, nsd = seeds ? seeds->n : 0;
-  if (nh > c->max_hits || nsd > c->max_seeds) return LST_EINVAL;
-  if (nh && (!hits->x || !hits->y || !hits->z || !hits->det)) return LST_EINVAL;
-  if (nsd && (!seeds->pt || !seeds->eta || !seeds->phi || !seeds->z0 || !seeds->q || !seeds->hit_ids)) return LST_EINVAL;
+  if (nh > c->max_hits || nsd > c->max_seeds) return einval();
+  if (nh && (!hits->x || !hits->y || !hits->z || !hits->det)) return einval();
+  if (nsd && (!seeds->pt || !seeds->eta || !seeds->phi || !seeds->z0 || !seeds->q || !seeds->hit_ids)) return einval();
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const SlotDev &d = s.dev;
   if (nh) {
@@ -651,48 +670,49 @@ extern "C" int lst_load_event(lst_ctx *c, uint32_t slot, const lst_hits *hits, c
 }
 
 // ------------------------------------------------------------------ the chain
-static void enqueue_stages(const lst_ctx *c, const SlotDev &d, cudaStream_t st);
-static void enqueue_chain(const lst_ctx *c, const SlotDev &d, cudaStream_t st) {
+// Enqueue a0 .. a6 of one slot on `st`; rec (may be NULL) counts / times the kernels.
+static int enqueue_chain(const lst_ctx *c, const SlotDev &d, cudaStream_t st, Recorder *rec) {
   Recorder count_only;
-  if (!c->k.rec) c->k.rec = &count_only;
-  enqueue_stages(c, d, st);
-  const_cast<lst_ctx *>(c)->launches = (uint32_t)c->k.rec->n;
-  if (c->k.rec == &count_only) c->k.rec = nullptr;
+  Ctx k = c->k;                    // a private copy: the recorder pointer is per call, not per context
+  k.rec = rec ? rec : &count_only;
+  launch_index(k, d, st);
+  launch_md(k, d, st);
+  launch_ls(k, d, st);
+  launch_t3(k, d, st);
+  launch_t5(k, d, st);
+  launch_pixel(k, d, st);
+  launch_dedup(k, d, st);
+  return k.rec->n;
 }
-static void enqueue_stages(const lst_ctx *c, const SlotDev &d, cudaStream_t st) {
-  launch_index(c->k, d, st);
-  launch_md(c->k, d, st);
-  launch_ls(c->k, d, st);
-  launch_t3(c->k, d, st);
-  launch_t5(c->k, d, st);
-  launch_pixel(c->k, d, st);
-  launch_dedup(c->k, d, st);
+
+// One CUDA graph per slot, captured when the workspace is bound (lst_run then only replays it: no
+// allocation, no capture, nothing shared between slots is written).
+static int capture_slot_graph(lst_ctx *c, Slot &s) {
+  cudaGraph_t gr = nullptr;
+  cudaStream_t cap = nullptr;
+  CU(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));      // the legacy default stream cannot be captured
+  cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+  if (e != cudaSuccess) { cudaStreamDestroy(cap); return cuda_fail(e, "cudaStreamBeginCapture"); }
+  const int n = enqueue_chain(c, s.dev, cap, nullptr);
+  e = cudaStreamEndCapture(cap, &gr);
+  cudaStreamDestroy(cap);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
+  e = cudaGraphInstantiate(&s.graph, gr, 0);
+  cudaGraphDestroy(gr);
+  if (e != cudaSuccess) { s.graph = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
+  c->launches.store((uint32_t)n);
+  return LST_OK;
 }
 
 extern "C" int lst_run(lst_ctx *c, uint32_t slot, void *cuda_stream) {
-  if (!c || slot >= c->n_slots) return LST_EINVAL;
+  if (!c || slot >= c->n_slots) return einval();
   Slot &s = c->slots[slot];
   if (!s.bound || !s.loaded) return LST_ESTATE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (c->cfg.use_cuda_graph) {
-    if (!s.graph) {
-      // capture on a private stream (the legacy default stream cannot be captured)
-      cudaGraph_t gr = nullptr;
-      cudaStream_t cap = nullptr;
-      CU(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
-      cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
-      if (e != cudaSuccess) { cudaStreamDestroy(cap); return cuda_fail(e, "cudaStreamBeginCapture"); }
-      enqueue_chain(c, s.dev, cap);
-      e = cudaStreamEndCapture(cap, &gr);
-      cudaStreamDestroy(cap);
-      if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
-      e = cudaGraphInstantiate(&s.graph, gr, 0);
-      cudaGraphDestroy(gr);
-      if (e != cudaSuccess) { s.graph = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
-    }
+  if (s.graph) {
     CU(cudaGraphLaunch(s.graph, st));
   } else {
-    enqueue_chain(c, s.dev, st);
+    c->launches.store((uint32_t)enqueue_chain(c, s.dev, st, nullptr));
     CU(cudaGetLastError());
   }
   s.ran = true; s.last_stream = st;
@@ -704,7 +724,13 @@ static int sync_header(lst_ctx *c, Slot &s) {
   (void)c;
   CU(cudaMemcpyAsync(s.h_hdr, s.dev.hdr, sizeof(Header), cudaMemcpyDeviceToHost, s.last_stream));
   CU(cudaStreamSynchronize(s.last_stream));
-  if (s.h_hdr->err & ERR_DET) return LST_EINVAL;
+  if (s.h_hdr->err & (ERR_DET | ERR_NONFINITE | ERR_BOX)) {
+    snprintf(g_inval_err, sizeof(g_inval_err), "invalid event:%s%s%s",
+             (s.h_hdr->err & ERR_DET) ? " det id out of range" : "",
+             (s.h_hdr->err & ERR_NONFINITE) ? " NaN / infinite hit coordinate or seed parameter" : "",
+             (s.h_hdr->err & ERR_BOX) ? " lower-sensor hit outside its module's box" : "");
+    return LST_EINVAL;
+  }
   if (s.h_hdr->err & (ERR_CAP_ITEMS | ERR_CAP_OBJ | ERR_CAP_PIX)) {
     const Header &h = *s.h_hdr;
     snprintf(g_cap_err, sizeof(g_cap_err),
@@ -718,7 +744,7 @@ static int sync_header(lst_ctx *c, Slot &s) {
 }
 
 extern "C" int lst_get_counts(lst_ctx *c, uint32_t slot, uint32_t *counts, uint64_t *cand) {
-  if (!c || slot >= c->n_slots || !counts) return LST_EINVAL;
+  if (!c || slot >= c->n_slots || !counts) return einval();
   Slot &s = c->slots[slot];
   if (!s.ran) return LST_ESTATE;
   const int rc = sync_header(c, s);
@@ -735,7 +761,7 @@ extern "C" int lst_get_counts(lst_ctx *c, uint32_t slot, uint32_t *counts, uint6
 static const uint32_t kArity[LST_NLEVEL] = {2, 4, 6, 10, 6, 10, 14};
 
 extern "C" int lst_get_objects(lst_ctx *c, uint32_t slot, lst_level level, int copy_to_host, lst_objects *out) {
-  if (!c || slot >= c->n_slots || !out || (int)level < 0 || level >= LST_NLEVEL) return LST_EINVAL;
+  if (!c || slot >= c->n_slots || !out || (int)level < 0 || level >= LST_NLEVEL) return einval();
   Slot &s = c->slots[slot];
   if (!s.ran) return LST_ESTATE;
   launch_export(c->k, s.dev, (int)level, s.last_stream);
@@ -770,26 +796,25 @@ extern "C" int lst_get_objects(lst_ctx *c, uint32_t slot, lst_level level, int c
   return LST_OK;
 }
 
-extern "C" uint32_t lst_launches_per_run(const lst_ctx *c) { return c ? c->launches : 0; }
+extern "C" uint32_t lst_launches_per_run(const lst_ctx *c) { return c ? c->launches.load() : 0; }
 
 // The chain without a graph, one CUDA event after every kernel; synchronises the stream.
 extern "C" int lst_run_timed(lst_ctx *c, uint32_t slot, void *cuda_stream, uint32_t max_kernels, const char **names,
                              float *ms, uint32_t *n_kernels) {
-  if (!c || slot >= c->n_slots || !n_kernels) return LST_EINVAL;
+  if (!c || slot >= c->n_slots || !n_kernels) return einval();
   Slot &s = c->slots[slot];
   if (!s.bound || !s.loaded) return LST_ESTATE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  Recorder &r = c->timed;
-  if (!c->timed_ready) {
-    for (int k = 0; k <= Recorder::kMax; ++k) CU(cudaEventCreate(&r.ev[k]));
-    c->timed_ready = true;
+  if (!s.timed) {
+    s.timed = new (std::nothrow) Recorder();
+    if (!s.timed) return LST_ENOMEM;
+    for (int k = 0; k <= Recorder::kMax; ++k) CU(cudaEventCreate(&s.timed->ev[k]));
   }
+  Recorder &r = *s.timed;
   r.timed = true;
   r.n = 0;
   CU(cudaEventRecord(r.ev[0], st));
-  c->k.rec = &r;
-  enqueue_chain(c, s.dev, st);
-  c->k.rec = nullptr;
+  c->launches.store((uint32_t)enqueue_chain(c, s.dev, st, &r));
   CU(cudaGetLastError());
   s.ran = true; s.last_stream = st;
   CU(cudaStreamSynchronize(st));
@@ -813,7 +838,7 @@ extern "C" int lst_host_eval(const lst_config *cfg_in, int level, uint32_t n, co
   Params g;
   make_params(cfg, &g);
   const int npts = level == LST_MD ? 2 : level == LST_LS ? 2 : level == LST_T3 ? 3 : level == LST_T5 ? 5 : 0;
-  if (!npts || !pts || !cats || !pass) return LST_EINVAL;
+  if (!npts || !pts || !cats || !pass) return einval();
   for (uint32_t i = 0; i < n; ++i) {
     Pt P[5];
     const float *p = pts + (size_t)i * npts * 3;
@@ -861,7 +886,7 @@ extern "C" int lst_host_eval(const lst_config *cfg_in, int level, uint32_t n, co
 
 extern "C" int lst_host_ls_window(const lst_config *cfg_in, uint32_t n, const float *row, const uint8_t *row_cat,
                                   const float *box, const uint8_t *box_cat, uint8_t *live, float *w) {
-  if (!row || !row_cat || !box || !box_cat || !live || !w) return LST_EINVAL;
+  if (!row || !row_cat || !box || !box_cat || !live || !w) return einval();
   lst_config cfg;
   if (cfg_in) cfg = *cfg_in; else lst_default_config(&cfg);
   Params g;

@@ -43,8 +43,12 @@ enum ErrBits {
   ERR_DET = 1u << 0,        // det id out of range
   ERR_CAP_ITEMS = 1u << 1,  // a work list overflowed
   ERR_CAP_OBJ = 1u << 2,    // an object array overflowed
-  ERR_CAP_PIX = 1u << 3     // a per-seed list (compatible modules / related seeds) overflowed
+  ERR_CAP_PIX = 1u << 3,    // a per-seed list (compatible modules / related seeds) overflowed
+  ERR_NONFINITE = 1u << 4,  // a hit coordinate or a pixel-seed parameter is NaN or infinite
+  ERR_BOX = 1u << 5         // a lower-sensor hit lies outside its module's box (lst_geometry)
 };
+constexpr float kBoxTolLen = 5e-5f;   // cm: half the growth the host-side box arithmetic allows for
+constexpr float kBoxTolPhi = 5e-7f;   // rad (+ the fp32 rounding of the two azimuths, < 4e-6 in all)
 
 // Item / unit geometry of a group with R rows and W columns (shared by k_emit_items and the eval
 // kernels).  W <= kItemCand: one column tile, item_rpi(W) rows per item; else one row per item and

@@ -24,7 +24,7 @@ struct Recorder {
   } while (0)
 
 struct Ctx {             // what the launchers need from a context
-  mutable Recorder *rec = nullptr;
+  Recorder *rec = nullptr;         // set per call (enqueue_chain works on a copy of the context's Ctx)
   GeoDev geo;
   Params par;
   int n_sm;

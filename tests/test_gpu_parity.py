@@ -202,7 +202,49 @@ def test_errors(B, geom_barrel, map_barrel):
     with pytest.raises(B.LstError) as e:
         lst.lst_get_counts(0)
     assert e.value.status == B.LST_EINVAL
+    # NaN / infinite coordinates, non-finite seed parameters, a lower-sensor hit outside its module's box
+    n = 64
+    lo = np.nonzero((ev.det[:n] & 1) == 0)[0]
+    for what in ("nan", "inf", "box_r", "box_phi", "box_z", "seed"):
+        x, y, z = ev.x[:n].copy(), ev.y[:n].copy(), ev.z[:n].copy()
+        seeds = None
+        if what == "nan":
+            y[5] = np.nan
+        elif what == "inf":
+            z[9] = np.inf
+        elif what == "box_r":
+            x[lo[0]] *= 1.01; y[lo[0]] *= 1.01
+        elif what == "box_phi":
+            c, s_ = np.cos(0.5), np.sin(0.5)
+            x[lo[1]], y[lo[1]] = c * x[lo[1]] - s_ * y[lo[1]], s_ * x[lo[1]] + c * y[lo[1]]
+        elif what == "box_z":
+            z[lo[2]] += 11.0
+        else:
+            seeds = (np.array([1.0, np.nan], np.float32), np.zeros(2, np.float32), np.zeros(2, np.float32),
+                     np.zeros(2, np.float32), np.ones(2, np.int8), np.arange(8, dtype=np.uint32).reshape(2, 4))
+        lst.lst_load_event(0, x, y, z, ev.det[:n], seeds)
+        lst.lst_run(0)
+        with pytest.raises(B.LstError) as e:
+            lst.lst_get_counts(0)
+        assert e.value.status == B.LST_EINVAL, what
+        msg = B.lib().lst_strerror(B.LST_EINVAL).decode()
+        assert ("box" in msg) == what.startswith("box") and ("NaN" in msg) == (not what.startswith("box")), (what, msg)
+    # ... and the untouched event is fine afterwards (the slot recovers)
+    lst.lst_load_event(0, ev.x[:n], ev.y[:n], ev.z[:n], ev.det[:n])
+    lst.lst_run(0)
+    lst.lst_get_counts(0)
     lst.close()
+    # inconsistent geometry / capacities beyond the 32-bit keys are refused by lst_create
+    import dataclasses
+    for field, val in (("half_phi", 0.7), ("rmin", -1.0), ("zmax", -1000.0)):
+        arr = getattr(geom_barrel, field).copy()
+        arr[3] = val
+        with pytest.raises(B.LstError) as e:
+            B.LST(dataclasses.replace(geom_barrel, **{field: arr}), map_barrel[0], map_barrel[1], max_hits=64, max_seeds=4)
+        assert e.value.status == B.LST_EINVAL, field
+    with pytest.raises(B.LstError) as e:
+        B.LST(geom_barrel, map_barrel[0], map_barrel[1], max_hits=6_000_000, max_seeds=4)
+    assert e.value.status == B.LST_EINVAL
     # capacity overflow is reported, never silent
     cfg = B.lst_default_config()
     cfg.cap_ls_per_hit = 0.001
@@ -235,6 +277,38 @@ def test_device_resident_input_and_graph_replay(B, geom_barrel, map_barrel):
             for lvl in CHAIN:
                 compare_level(o, lst, lvl)
         lst.close()
+
+
+def test_two_host_threads_on_two_slots(B, geom_barrel, map_barrel):
+    """include/lst.h: different slots may be driven from different host threads (the slot's graph is
+    captured at lst_bind_workspace; lst_run writes nothing shared)."""
+    import threading
+    import torch
+    ev = lstgen.make_event(geom_barrel, "cfg2")
+    o = _oracle(geom_barrel, map_barrel, ev, O.T5)
+    lst = B.LST(geom_barrel, map_barrel[0], map_barrel[1], n_slots=2, max_hits=ev.n_hits, max_seeds=4)
+    assert lst.launches_per_run() > 0                      # known before the first run
+    errs = []
+
+    def drive(slot):
+        try:
+            torch.cuda.set_device(0)
+            st = torch.cuda.Stream()
+            for _ in range(20):
+                lst.lst_load_event(slot, ev.x, ev.y, ev.z, ev.det, stream=st)
+                lst.lst_run(slot, stream=st)
+                cnt, _ = lst.lst_get_counts(slot)
+                assert [int(c) for c in cnt[:4]] == [o.count(l) for l in CHAIN]
+        except Exception as exc:      # noqa: BLE001
+            errs.append(exc)
+    th = [threading.Thread(target=drive, args=(k,)) for k in range(2)]
+    [t.start() for t in th]
+    [t.join() for t in th]
+    assert not errs, errs
+    for slot in range(2):
+        for lvl in CHAIN:
+            compare_level(o, _SlotView(lst, slot), lvl)
+    lst.close()
 
 
 # ------------------------------------------------------------------ a5 / a6: pixel linking, cleaning, TC
