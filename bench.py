@@ -47,6 +47,9 @@ def parse_args():
     ap.add_argument("--workload", default="cfg4h", choices=["cfg4h", "cfg4"])
     ap.add_argument("--events", type=int, default=64)
     ap.add_argument("--slots", type=int, default=8)
+    ap.add_argument("--batch", type=int, default=1, help="events per chain of launches (lst_config.batch_events); slots are "
+                    "grouped `batch` at a time, one stream per group")
+    ap.add_argument("--pdl", type=int, default=1, help="lst_config.use_pdl")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cfg4", action="store_true", help="skip the second, literal config-4 (6000-particle) throughput entry")
@@ -155,8 +158,7 @@ def algorithmic_bytes(name, n):
     bits = lambda k: n["cand"][k] / 8.0          # one pass bit per candidate (+ ~0.4 % item headers)
     nmod, nnz = n["n_modules"], n["nnz"]
     t = {
-        "k_hist": 4 * n["hits"] + 4 * 2 * nmod,
-        "k_det_scan": 4 * 2 * nmod * 3 + 8 * nmod,
+        "k_hist": (16 + 4) * n["hits"] + 4 * 2 * nmod * 3 + 12 * nmod,   # + det scan and MD groups in its last block
         "k_scatter": 4 * n["hits"] * 2 + 4 * 2 * nmod,
         "k_rank": (B_HIT_IN + B_HIT + 4) * n["hits"],
         # pre-filter kernels read their operands once and append (key, pair) = 12 B per survivor;
@@ -175,12 +177,10 @@ def algorithmic_bytes(name, n):
         "k_join_eval[T5]": 16 * n["t3"] + 12 * n["surv"][3],
         "k_join_decide[T5]": (12 + 64) * n["surv"][3] + bits(3) + 64 * n["t5"],
         "k_join_fill[T5]": 64 * n["t5"] + bits(3) + B_T5 * n["t5"],
-        "k_join_eval[pT5]": B_SEED * n["seeds"] + 4 * n["t5"] + 24 * n["md"] + 12 * n["surv"][4],
-        "k_join_decide[pT5]": (12 + 40) * n["surv"][4] + 28 * n["pt5"],
-        "k_join_fill[pT5]": 28 * n["pt5"] + B_PT * n["pt5"],
-        "k_join_eval[pT3]": B_SEED * n["seeds"] + 16 * n["t3"] + 24 * n["md"] + 12 * n["surv"][5],
-        "k_join_decide[pT3]": (12 + 32) * n["surv"][5] + 28 * n["pt3"],
-        "k_join_fill[pT3]": 28 * n["pt3"] + B_PT * n["pt3"],
+        # pT5 and pT3 share their launches (blockIdx.y)
+        "k_px_eval": 2 * B_SEED * n["seeds"] + 4 * n["t5"] + 16 * n["t3"] + 2 * 24 * n["md"] + 12 * (n["surv"][4] + n["surv"][5]),
+        "k_px_decide": (12 + 40) * n["surv"][4] + (12 + 32) * n["surv"][5] + 28 * (n["pt5"] + n["pt3"]),
+        "k_px_fill": (28 + B_PT) * (n["pt5"] + n["pt3"]),
         "k_s0": (40 + 8 + 1) * n["t5"] + (8 + 8 + 1) * (n["pt5"] + n["pt3"]),
         "k_tc_fill": B_TC * n["tc"] + 4 * (n["t5"] + n["pt5"] + n["pt3"] + n["seeds"]),
     }
@@ -191,14 +191,14 @@ def algorithmic_bytes(name, n):
 # counted from the formulas of lst_math.cuh: the candidate loops are bound by
 # the plain fp32 ALUs / issue slots, not by memory.
 OPS_PER_CAND = {"k_md_eval": (0, 27), "k_ls_eval": (1, 36), "k_join_eval[T3]": (2, 128),
-                "k_join_eval[T5]": (3, 4 + 128), "k_join_eval[pT5]": (4, 68), "k_join_eval[pT3]": (5, 68)}
+                "k_join_eval[T5]": (3, 4 + 128), "k_px_eval": ((4, 5), 68)}
 
 
 def algorithmic_ops(name, n):
     if name not in OPS_PER_CAND:
         return None
     k, ops = OPS_PER_CAND[name]
-    return ops * n["cand"][k]
+    return ops * (sum(n["cand"][q] for q in k) if isinstance(k, tuple) else n["cand"][k])
 
 
 def event_totals_bytes(n):
@@ -357,7 +357,10 @@ def run_ours(a, rank, world, local_rank, init_dist=True):
     events = [lstgen.make_event(geom, a.workload, seed=sd) for sd in sharding.event_seeds(rank, world, a.events)]
     max_hits = max(e.n_hits for e in events)
     max_seeds = max(max(e.n_seeds for e in events), 1)
-    lst = B.LST(geom, off, cols, n_slots=a.slots, max_hits=max_hits, max_seeds=max_seeds, device=str(dev))
+    cfg = B.lst_default_config()
+    cfg.use_pdl, cfg.batch_events = a.pdl, a.batch
+    assert a.slots % a.batch == 0 and a.events % a.slots == 0
+    lst = B.LST(geom, off, cols, cfg=cfg, n_slots=a.slots, max_hits=max_hits, max_seeds=max_seeds, device=str(dev))
 
     u32 = lambda x: np.ascontiguousarray(x, dtype=np.uint32)
     host, devt = [], []
@@ -370,7 +373,7 @@ def run_ours(a, rank, world, local_rank, init_dist=True):
     h2d_bytes = sum(sum(t.numel() * t.element_size() for t in h + s) for h, s in host)
     torch.cuda.synchronize()
 
-    streams = [torch.cuda.Stream(device=dev) for _ in range(a.slots)]
+    streams = [torch.cuda.Stream(device=dev) for _ in range(a.slots // a.batch)]    # one stream per group of slots
     main = torch.cuda.current_stream()
 
     def barrier():
@@ -391,14 +394,28 @@ def run_ours(a, rank, world, local_rank, init_dist=True):
             main.wait_event(e)
         ev1.record(main)
 
+    def enqueue(i, src):
+        """event i into its slot; the slot's group is run once its last slot has been loaded"""
+        sl = i % a.slots
+        grp = sl // a.batch
+        h, s = src[i]
+        lst.lst_load_event(sl, h[0], h[1], h[2], h[3], s if len(s[0]) else None, stream=streams[grp])
+        if a.batch == 1:
+            lst.lst_run(sl, stream=streams[grp])
+        elif sl % a.batch == a.batch - 1:
+            lst.lst_run_batch(grp, stream=streams[grp])
+
     def step_resident():
         for i in range(a.events):
-            sl = i % a.slots
-            h, s = devt[i]
-            lst.lst_load_event(sl, h[0], h[1], h[2], h[3], s if s[0].numel() else None, stream=streams[sl])
-            lst.lst_run(sl, stream=streams[sl])
+            enqueue(i, devt)
 
     d2h = [0]
+
+    host_np = []
+    for h, s in host:
+        hn = [as_np(h[0], np.float32), as_np(h[1], np.float32), as_np(h[2], np.float32), as_np(h[3], np.uint32)]
+        sn = [as_np(s[k], np.float32) for k in range(4)] + [as_np(s[4], np.int8), as_np(s[5], np.uint32)]
+        host_np.append((hn, sn))
 
     def step_e2e():
         inflight = []
@@ -406,13 +423,7 @@ def run_ours(a, rank, world, local_rank, init_dist=True):
             sl = i % a.slots
             if len(inflight) == a.slots:
                 d2h[0] += collect(inflight.pop(0))
-            h, s = host[i]
-            hn = [as_np(h[0], np.float32), as_np(h[1], np.float32), as_np(h[2], np.float32), as_np(h[3], np.uint32)]
-            sn = None
-            if s[0].numel():
-                sn = [as_np(s[k], np.float32) for k in range(4)] + [as_np(s[4], np.int8), as_np(s[5], np.uint32)]
-            lst.lst_load_event(sl, hn[0], hn[1], hn[2], hn[3], sn, stream=streams[sl])
-            lst.lst_run(sl, stream=streams[sl])
+            enqueue(i, host_np)
             inflight.append(sl)
         while inflight:
             d2h[0] += collect(inflight.pop(0))
@@ -444,13 +455,13 @@ def run_ours(a, rank, world, local_rank, init_dist=True):
     for i in range(a.events):
         sl = i % a.slots
         h, s = devt[i]
-        lst.lst_load_event(sl, h[0], h[1], h[2], h[3], s if s[0].numel() else None, stream=streams[sl])
-        lst.lst_run(sl, stream=streams[sl])
+        lst.lst_load_event(sl, h[0], h[1], h[2], h[3], s if s[0].numel() else None, stream=streams[sl // a.batch])
+        lst.lst_run(sl, stream=streams[sl // a.batch])
         cnt_i, _ = lst.lst_get_counts(sl)
         assert cnt_i[B.LST_MD] > 0 and cnt_i[B.LST_TC] > 0, "event %d produced no objects" % i
     ms, clocks = timed(step_resident, a.warmup, a.steps, True)
     counts = [lst.lst_get_counts(sl) for sl in range(a.slots)]
-    launches = lst.launches_per_run() + 1                      # + k_set_event of lst_load_event
+    launches = lst.launches_per_run() / a.batch + 1            # one chain serves `batch` events; + k_set_event of lst_load_event
     value = sharding.job_events_per_s(world, a.events, a.steps, ms)
 
     e2e = None
@@ -545,6 +556,7 @@ def main():
             "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32 pre-filter + f64 decisions", "data": "synthetic",
             "config": {"workload": workload_name(a), "events_per_step": a.events, "slots": a.slots,
+                       "batch_events": a.batch, "streams": a.slots // a.batch, "pdl": a.pdl,
                        "l2": "inputs larger than L2: %.0f MB of device-resident events + %d x %.0f MB slot workspaces per "
                              "step vs 126 MB L2" % (in_bytes / 1e6, a.slots, ws / 1e6),
                        "parallelism": "replicas only (no collective)", "objects_event0": {k: n[k] for k in (
@@ -554,7 +566,7 @@ def main():
                        "prefilter_survivors_event0": dict(zip(("md", "ls", "t3", "t5", "pt5", "pt3"), n["surv"][:6]))},
             "clocks": clocks,
             "gpu_launches": int(launches * a.events * a.steps),
-            "launches_per_event": int(launches),
+            "launches_per_event": round(float(launches), 2), "launches_per_chain": int(lst.launches_per_run()),
             "e2e": e2e,
             "roofline": roofline(top, peak, peak_src, alu_peak, alu_src),
             "chain": {"single_stream_ms_per_event": round(chain_ms, 4), "alg_bytes_per_event": int(total_b),

@@ -79,6 +79,13 @@ typedef struct {
                               bit 1: the LS pre-filter visits, per inner MD and connected module, only
                                      the MDs inside the azimuthal window / pointing cone that the cuts
                                      allow (uses the event's own MD positions only).  Default 3.      */
+  int32_t use_pdl;         /* 1: every kernel of the chain but the first is launched with programmatic
+                              stream serialisation (programmatic dependent launch): its blocks may become
+                              resident while the preceding kernel drains; results are identical          */
+  int32_t batch_events;    /* E in [1, 8], default 1: slots are grouped E at a time (group g = slots
+                              [g E, (g + 1) E)) and lst_run_batch runs a whole group as ONE chain of
+                              launches with a grid over (event, work): SURVEY.md 8(f)1, the B200 form of
+                              the paper's multi-streaming                             */
 } lst_config;
 
 /* Detector description, HOST arrays of length n_modules (copied by the callee).  A module is a
@@ -191,6 +198,13 @@ int lst_load_event(lst_ctx *ctx, uint32_t slot, const lst_hits *hits, const lst_
 /* a0-a6: enqueue the whole chain (index hits by det, MD, LS, T3, T5, pT5, pT3, S0-S3, TC) on
  * `cuda_stream`.  No host synchronisation; no allocation.  Sizes stay on the device. */
 int lst_run(lst_ctx *ctx, uint32_t slot, void *cuda_stream);
+
+/* The same chain for all the slots of group `group` (lst_config.batch_events consecutive slots, every
+ * one of them bound and loaded, normally on this same stream) in ONE sequence of launches whose grids
+ * span (event, work); with batch_events = 1 it is lst_run(group).  Results per slot are those of
+ * lst_run.  LST_ESTATE if a slot of the group has no workspace or no event. */
+int lst_run_batch(lst_ctx *ctx, uint32_t group, void *cuda_stream);
+uint32_t lst_batch_events(const lst_ctx *ctx);
 
 /* Synchronise the slot's stream and return a view of one level.  LST_ENOMEM if a collection
  * overflowed its capacity, LST_EINVAL if the event was invalid (see lst_load_event). */

@@ -22,7 +22,7 @@ LEVEL_NAMES = ("MD", "LS", "T3", "T5", "PT3", "PT5", "TC")
 
 EXPORTS = ("lst_default_config", "lst_build_module_map", "lst_free", "lst_create", "lst_destroy",
            "lst_workspace_bytes", "lst_bind_workspace", "lst_load_event", "lst_run", "lst_get_objects",
-           "lst_get_counts", "lst_launches_per_run", "lst_run_timed", "lst_strerror")
+           "lst_get_counts", "lst_launches_per_run", "lst_run_timed", "lst_strerror", "lst_run_batch", "lst_batch_events")
 TEST_EXPORTS = ("lst_host_eval", "lst_host_ls_window")      # include/lst_test.h
 
 
@@ -36,7 +36,8 @@ class lst_config(C.Structure):
         (n, C.c_float) for n in (
             "cap_md_per_hit", "cap_ls_per_hit", "cap_t3_per_hit", "cap_t5_per_hit", "cap_pt3_per_seed",
             "cap_pt5_per_seed", "cap_mdcand_per_hit", "cap_lscand_per_hit", "cap_t3cand_per_hit",
-            "cap_t5cand_per_hit")] + [("use_cuda_graph", C.c_int32), ("enum_pruning", C.c_int32)]
+            "cap_t5cand_per_hit")] + [("use_cuda_graph", C.c_int32), ("enum_pruning", C.c_int32), ("use_pdl", C.c_int32),
+                                   ("batch_events", C.c_int32)]
 
 
 class lst_geometry(C.Structure):
@@ -96,6 +97,9 @@ def lib():
         L.lst_bind_workspace.argtypes = [vp, u32, vp, C.c_size_t]
         L.lst_load_event.argtypes = [vp, u32, C.POINTER(lst_hits), C.POINTER(lst_pixel_seeds), vp]
         L.lst_run.argtypes = [vp, u32, vp]
+        L.lst_run_batch.argtypes = [vp, u32, vp]
+        L.lst_batch_events.argtypes = [vp]
+        L.lst_batch_events.restype = u32
         L.lst_get_objects.argtypes = [vp, u32, C.c_int, C.c_int, C.POINTER(lst_objects)]
         L.lst_get_counts.argtypes = [vp, u32, vp, vp]
         L.lst_launches_per_run.argtypes = [vp]
@@ -249,6 +253,9 @@ class LST:
 
     def lst_run(self, slot, stream=None):
         _check(lib().lst_run(self._h, slot, self._stream_ptr(stream)), "lst_run")
+
+    def lst_run_batch(self, group, stream=None):
+        _check(lib().lst_run_batch(self._h, group, self._stream_ptr(stream)), "lst_run_batch")
 
     def lst_run_timed(self, slot, stream=None):
         """-> list of (kernel name, ms) of one un-graphed, event-bracketed pass of the chain."""

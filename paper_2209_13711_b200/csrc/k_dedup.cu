@@ -77,93 +77,8 @@ __device__ __forceinline__ int dd_shared(const uint32_t *ha, int na, const uint3
   return n;
 }
 
-__device__ __forceinline__ int eta_bin(const Params &g, double eta) {
-  const double t = (eta + 4.0) * g.eta_bin_inv;
-  if (!(t >= 0.0)) return 0;
-  return t < (double)g.eta_nbins ? (int)t : g.eta_nbins - 1;
-}
-__device__ __forceinline__ bool close_eta_phi(const Params &g, double e1, double p1, double e2, double p2) {
-  const double de = e1 - e2;
-  if (fabs(de) > g.dr_eta_pre) return false;
-  const double dp = wrap_pi(p1 - p2);
-  return de * de + dp * dp < g.dr2max;
-}
-
-// ------------------------------------------------------------------ pixel-seed lookups
-// One block: cleaning sizes, eta bins of the seeds (counting sort; order inside a bin is irrelevant).
-__global__ void __launch_bounds__(1024) k_pls_prep(SlotDev s, Params g) {
-  __shared__ uint32_t cnt[kEtaBins];
-  __shared__ uint32_t sh[33];
-  Header *hdr = s.hdr;
-  const uint32_t n = hdr->n_seeds;
-  if (threadIdx.x == 0) {
-    hdr->n_dd = hdr->n_obj[3] + hdr->n_obj[5] + hdr->n_obj[4];
-    hdr->n_flag = hdr->n_obj[5] + hdr->n_obj[4] + hdr->n_obj[3] + n;
-    hdr->n_inc = 3 * hdr->n_hits;
-  }
-  for (int b = threadIdx.x; b < kEtaBins; b += blockDim.x) cnt[b] = 0;
-  __syncthreads();
-  for (uint32_t p = threadIdx.x; p < n; p += blockDim.x) atomicAdd(&cnt[eta_bin(g, (double)s.seed_eta[p])], 1u);
-  __syncthreads();
-  uint32_t carry = 0;
-  for (int base = 0; base < kEtaBins; base += blockDim.x) {
-    const int b = base + threadIdx.x;
-    const uint32_t v = cnt[b];
-    uint32_t tot;
-    const uint32_t e = block_excl_scan(v, sh, &tot);
-    s.pls_bin_off[b] = carry + e;
-    cnt[b] = carry + e;
-    carry += tot;
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) s.pls_bin_off[kEtaBins] = carry;
-  __syncthreads();
-  for (uint32_t p = threadIdx.x; p < n; p += blockDim.x) {
-    const uint32_t pos = atomicAdd(&cnt[eta_bin(g, (double)s.seed_eta[p])], 1u);
-    s.pls_bin_ent[pos] = p;
-  }
-}
-
-// Thread per seed a: the seeds b != a close to it in eta-phi, found through the eta bins (a close
-// seed lies in a's bin or a neighbouring one: the bin width exceeds sqrt(dr2max)).
-__global__ void __launch_bounds__(256) k_pls_adj(SlotDev s, Params g) {
-  const uint32_t n = s.hdr->n_seeds;
-  for (uint32_t a = blockIdx.x * blockDim.x + threadIdx.x; a < n; a += gridDim.x * blockDim.x) {
-    const double ea = (double)s.seed_eta[a], pa = (double)s.seed_phi[a];
-    const int b0 = eta_bin(g, ea);
-    const int lo = b0 > 0 ? b0 - 1 : 0, hi = b0 + 1 < g.eta_nbins ? b0 + 1 : g.eta_nbins - 1;
-    const uint32_t e0 = s.pls_bin_off[lo], e1 = s.pls_bin_off[hi + 1];
-    uint32_t cnt = 0;
-    for (uint32_t e = e0; e < e1; ++e) {
-      const uint32_t b = s.pls_bin_ent[e];
-      if (b == a || !close_eta_phi(g, ea, pa, (double)s.seed_eta[b], (double)s.seed_phi[b])) continue;
-      if (cnt < (uint32_t)kAdjCap) s.pls_adj[(size_t)a * kAdjCap + cnt] = b;
-      ++cnt;
-    }
-    if (cnt > (uint32_t)kAdjCap) { atomicOr(&s.hdr->err, (uint32_t)ERR_CAP_PIX); cnt = 0; }
-    s.pls_adj_cnt[a] = cnt;
-  }
-}
-
-// "Seeds a and b share a pixel hit" is looked up through the pixel-hit ids themselves: every id
-// is inserted into a hash set (linear probing; at most half full), and a seed remembers the slots of
-// its 4 ids.  Flags per slot (pid_has5 / pid_has3) then answer "does some seed with a surviving
-// pT5 / pT3 contain this pixel hit" without any seed-to-seed list.
-__device__ __forceinline__ uint32_t pid_hash(uint32_t id) { return (id * 0x9E3779B1u) ^ (id >> 15); }
-__global__ void __launch_bounds__(256) k_pid_insert(SlotDev s) {
-  const uint32_t n4 = 4 * s.hdr->n_seeds, mask = s.pid_size - 1;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += gridDim.x * blockDim.x) {
-    const uint32_t id = s.seed_ids[i];
-    const unsigned long long key = (1ull << 32) | id;
-    uint32_t h = pid_hash(id) & mask;
-    for (;;) {
-      const unsigned long long old = atomicCAS(&s.pid_key[h], 0ull, key);
-      if (old == 0ull || old == key) break;
-      h = (h + 1) & mask;
-    }
-    s.pls_slot[i] = h;
-  }
-}
+// The pixel-seed lookups (eta bins, seeds close to a seed, the hash set of the pixel-hit ids) are built
+// by the seed kernels of k_pix.cu; here they are only read.
 __device__ __forceinline__ void pid_mark(const SlotDev &s, uint8_t *flag, uint32_t p) {
   const uint4 sl = reinterpret_cast<const uint4 *>(s.pls_slot)[p];
   flag[sl.x] = 1; flag[sl.y] = 1; flag[sl.z] = 1; flag[sl.w] = 1;
@@ -181,9 +96,15 @@ __device__ __forceinline__ void md_hits2(const SlotDev &s, uint32_t md, uint32_t
   out[0] = h.x; out[1] = h.y;
 }
 // thread per dd object: gather its hit positions (T5 and pT3 store them) and count the incidences
-__global__ void k_dd_count(SlotDev s) {
+__global__ void __launch_bounds__(256) k_dd_count(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
+  pdl_enter();
+  LST_SLOT(B);
   const Header *hdr = s.hdr;
-  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = hdr->n_dd;
+  {   // one warp per seed: the seeds close to it in eta-phi (S1, S3)
+    const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+    for (uint32_t a = warp; a < hdr->n_seeds; a += nwarp) pls_adjacent(s, g, a);
+  }
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = n5 + np5 + hdr->n_obj[4];
   for (uint32_t d = blockIdx.x * blockDim.x + threadIdx.x; d < n_dd; d += gridDim.x * blockDim.x) {
     uint32_t h[10];
     int n;
@@ -207,16 +128,26 @@ __global__ void k_dd_count(SlotDev s) {
     for (int q = 0; q < n; ++q) atomicAdd(&s.inc_cnt[3 * h[q] + ty], 1u);
   }
 }
-__global__ void k_dd_scatter(SlotDev s) {
+__device__ __forceinline__ void pls_best_body(const SlotDev &s, uint32_t n5, uint32_t np5, uint32_t np3);
+__global__ void __launch_bounds__(256) k_dd_scatter(const __grid_constant__ Batch B) {
+  pdl_enter();
+  LST_SLOT(B);
   const Header *hdr = s.hdr;
-  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = hdr->n_dd;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], np3 = hdr->n_obj[4], n_dd = n5 + np5 + np3;
   for (uint32_t d = blockIdx.x * blockDim.x + threadIdx.x; d < n_dd; d += gridDim.x * blockDim.x) {
     const DRef r = dd_ref(s, n5, np5, d);
-    for (int q = 0; q < r.n_ot; ++q) {
-      const uint32_t h = 3 * r.hits[q] + (uint32_t)r.type;
-      s.inc_ent[s.inc_off[h] + atomicAdd(&s.inc_cur[h], 1u)] = d;
-    }
+    // the ten (six) rows are independent: all loads, then all atomics, then all stores in flight together
+    uint32_t row[10], pos[10];
+#pragma unroll
+    for (int q = 0; q < 10; ++q) row[q] = q < r.n_ot ? 3 * r.hits[q] + (uint32_t)r.type : 0u;
+#pragma unroll
+    for (int q = 0; q < 10; ++q) pos[q] = q < r.n_ot ? s.inc_off[row[q]] : 0u;
+#pragma unroll
+    for (int q = 0; q < 10; ++q) if (q < r.n_ot) pos[q] += atomicAdd(&s.inc_cur[row[q]], 1u);
+#pragma unroll
+    for (int q = 0; q < 10; ++q) if (q < r.n_ot) s.inc_ent[pos[q]] = d;
   }
+  pls_best_body(s, n5, np5, np3);
 }
 
 // ------------------------------------------------------------------ S0, same-seed rule
@@ -225,20 +156,8 @@ __global__ void k_dd_scatter(SlotDev s) {
 // the seed's minimum score by atomicMin on the bit pattern of the (non-negative) double, then the
 // objects AT that score settle the tie order by compare-and-swap (anchors are lower hits, so T3 /
 // T5 that differ only in upper hits tie exactly; the tie sets at the minimum are small).
-__global__ void __launch_bounds__(256) k_pls_min(SlotDev s) {
-  const Header *hdr = s.hdr;
-  const uint32_t np5 = hdr->n_obj[5], np3 = hdr->n_obj[4];
-  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < np5 + np3; j += gridDim.x * blockDim.x) {
-    const bool is5 = j < np5;
-    const uint32_t i = is5 ? j : j - np5;
-    const uint32_t p = (is5 ? s.pt5_po : s.pt3_po)[i].x;
-    const double sc = (is5 ? s.pt5_chi2 : s.pt3_chi2)[i];
-    atomicMin((is5 ? s.pls_min5 : s.pls_min3) + p, (unsigned long long)__double_as_longlong(sc));
-  }
-}
-__global__ void __launch_bounds__(256) k_pls_best(SlotDev s) {
-  const Header *hdr = s.hdr;
-  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], np3 = hdr->n_obj[4];
+// (the minimum is taken by the fill kernel of the pixel joins, k_t3t5.cu; the tie order here)
+__device__ __forceinline__ void pls_best_body(const SlotDev &s, uint32_t n5, uint32_t np5, uint32_t np3) {
   for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < np5 + np3; j += gridDim.x * blockDim.x) {
     const bool is5 = j < np5;
     const uint32_t i = is5 ? j : j - np5;
@@ -269,20 +188,40 @@ __global__ void __launch_bounds__(256) k_pls_best(SlotDev s) {
 constexpr int kS0Slots = 128;
 constexpr uint32_t kNoHit = 0xFFFFFFFFu;
 constexpr uint32_t kS0Light = 64;   // entries an 8-lane group looks at before it hands a longer object to k_s0_heavy
-__global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
+__global__ void __launch_bounds__(128) k_s0(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
   __shared__ uint32_t sh_pre[16][12], sh_beg[16][12];
   __shared__ uint32_t sh_tab[16][kS0Slots];
+  pdl_enter();
+  LST_SLOT(B);
   Header *hdr = s.hdr;
-  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = hdr->n_dd;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = n5 + np5 + hdr->n_obj[4];
   const int lane = threadIdx.x & 31, gl = lane & 7, gbase = lane & ~7, gid = threadIdx.x >> 3;
   const uint32_t gmask = 0xFFu << gbase;
   const uint32_t group = (blockIdx.x * blockDim.x + threadIdx.x) >> 3, ngroup = (gridDim.x * blockDim.x) >> 3;
   uint32_t *pre = sh_pre[gid], *beg = sh_beg[gid], *tab = sh_tab[gid];
   for (int k = gl; k < kS0Slots; k += 8) tab[k] = kNoHit;
   __syncwarp();
-  for (uint32_t d = group;; d += ngroup) {
-    const bool valid = d < n_dd;
-    if (!__any_sync(0xffffffffu, valid)) break;
+  // Same-seed rule first: of a seed's pT5 (pT3) only its best can survive, whatever the shared-hit search
+  // says, so the others are flagged here and the search below runs on the T5 and on the seeds' best
+  // objects only (work index: [0, n5) T5, then per seed its best pT5, then per seed its best pT3).
+  const uint32_t n_seeds = hdr->n_seeds;
+  if (g.s0_enabled) {
+    const uint32_t np3 = hdr->n_obj[4];
+    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < np5 + np3; j += gridDim.x * blockDim.x) {
+      if (j < np5) { if (s.pls_best5[s.pt5_po[j].x] != j) s.pt5_keep[j] = 0; }
+      else { const uint32_t i = j - np5; if (s.pls_best3[s.pt3_po[i].x] != i) s.pt3_keep[i] = 0; }
+    }
+  }
+  const uint32_t n_work = g.s0_enabled ? n5 + 2u * n_seeds : n_dd;
+  for (uint32_t wk = group;; wk += ngroup) {
+    if (!__any_sync(0xffffffffu, wk < n_work)) break;
+    uint32_t d = wk;
+    bool valid = wk < n_work;
+    if (valid && g.s0_enabled && wk >= n5) {
+      const uint32_t q = wk - n5, best = q < n_seeds ? s.pls_best5[q] : s.pls_best3[q - n_seeds];
+      valid = best != 0xFFFFFFFFu;
+      d = (q < n_seeds ? n5 : n5 + np5) + best;
+    }
     DRef A;
     A.type = 0; A.idx = 0; A.n_ot = 0; A.hits = nullptr; A.pls = kNoHit; A.score = 0.0;
     if (valid) A = dd_ref(s, n5, np5, d);
@@ -389,32 +328,41 @@ __global__ void __launch_bounds__(128) k_s0(SlotDev s, Params g) {
 }
 
 // The objects k_s0 deferred (not beaten by their first kS0Light entries and with longer lists: mostly
-// the objects that survive): one WARP per object over the whole flattened list.
-__global__ void __launch_bounds__(128) k_s0_heavy(SlotDev s, Params g) {
-  __shared__ uint32_t sh_pre[4][12], sh_beg[4][12];
-  __shared__ uint32_t sh_tab[4][256];
+// the objects that survive): one BLOCK per object over the whole flattened list (a hit of a |eta| ~ 0
+// seed's objects is shared by thousands of pT3: the longest lists set the duration, so they get 128
+// lanes), objects handed out dynamically.  Warp 0 sets the object up, all warps stride the list.
+__global__ void __launch_bounds__(128) k_s0_heavy(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
+  __shared__ uint32_t pre[12], beg[12];
+  __shared__ uint32_t tab[256];
+  __shared__ uint32_t sh_hv, sh_collide;
+  pdl_enter();
+  LST_SLOT(B);
   const Header *hdr = s.hdr;
   const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_heavy = hdr->n_heavy;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
-  uint32_t *pre = sh_pre[wib], *beg = sh_beg[wib], *tab = sh_tab[wib];
-  for (int k = lane; k < 256; k += 32) tab[k] = 0xFFFFFFFFu;
-  __syncwarp();
-  for (uint32_t hv = warp; hv < n_heavy; hv += nwarp) {
+  for (int k = threadIdx.x; k < 256; k += blockDim.x) tab[k] = 0xFFFFFFFFu;
+  for (;;) {
+    __syncthreads();                                            // the previous object is done with the shared arrays
+    if (threadIdx.x == 0) sh_hv = atomicAdd(&s.hdr->next_unit[S_T5], 1u);
+    __syncthreads();
+    const uint32_t hv = sh_hv;
+    if (hv >= n_heavy) break;
     const uint32_t d = s.tc_pos[hv];
     const DRef A = dd_ref(s, n5, np5, d);
-    // lane q < n_ot owns hit q of A
-    const uint32_t my_hit = lane < A.n_ot ? A.hits[lane] : 0xFFFFFFFFu;
+    const int min_shared = A.type == 0 ? g.dup_t5 : (A.type == 1 ? g.dup_pt5 : g.dup_pt3);
+    const int k0 = min_shared - 1, nl = A.n_ot > k0 ? A.n_ot - k0 : 0;   // number of lists searched
     bool beaten = false;
     if (g.s0_enabled) {
-      const int min_shared = A.type == 0 ? g.dup_t5 : (A.type == 1 ? g.dup_pt5 : g.dup_pt3);
-      const int k0 = min_shared - 1, nl = A.n_ot > k0 ? A.n_ot - k0 : 0;   // lists searched: hits k0 .. n_ot-1
-      // table of A's hits; collisions (two hits of A in one slot) -> exact comparison path
-      const uint32_t slot = my_hit & (256 - 1);
-      const uint32_t same = __match_any_sync(0xffffffffu, lane < A.n_ot ? slot : 0x10000u + lane);
-      const bool collide = __any_sync(0xffffffffu, lane < A.n_ot && __popc(same) > 1);
-      if (lane < A.n_ot) tab[slot] = my_hit;
-      {
+      uint32_t slot = 0;
+      if (wib == 0) {
+        // lane q < n_ot owns hit q of A: table of A's hits; collisions (two hits of A in one slot) ->
+        // exact comparison path
+        const uint32_t my_hit = lane < A.n_ot ? A.hits[lane] : 0xFFFFFFFFu;
+        slot = my_hit & (256 - 1);
+        const uint32_t same = __match_any_sync(0xffffffffu, lane < A.n_ot ? slot : 0x10000u + lane);
+        const bool collide = __any_sync(0xffffffffu, lane < A.n_ot && __popc(same) > 1);
+        if (lane < A.n_ot) tab[slot] = my_hit;
+        if (lane == 0) sh_collide = collide;
         // the nl SHORTEST of A's n_ot incidence lists are searched (any nl of them will do)
         uint32_t len = 0, b0 = 0;
         if (lane < A.n_ot) {
@@ -433,14 +381,15 @@ __global__ void __launch_bounds__(128) k_s0_heavy(SlotDev s, Params g) {
         const uint32_t ex = warp_excl_scan(l2, &tot);
         __syncwarp();
         if (lane < 11) pre[lane] = ex;                          // lanes >= nl: pre = total
-        __syncwarp();
       }
+      __syncthreads();
+      const bool collide = sh_collide != 0u;
       const uint32_t total = pre[nl < 10 ? nl : 10];
       const double *score_arr = A.type == 0 ? s.t5_chi2 : (A.type == 1 ? s.pt5_chi2 : s.pt3_chi2);
       const uint32_t dbase = A.type == 0 ? 0u : (A.type == 1 ? n5 : n5 + np5);
       int cur = 0;
-      for (uint32_t base = 0; base < total && !beaten; base += 32) {
-        const uint32_t i = base + lane;
+      for (uint32_t base = 0; base < total && !beaten; base += blockDim.x) {
+        const uint32_t i = base + threadIdx.x;
         bool hit = false;
         if (i < total) {
           while (i >= pre[cur + 1]) ++cur;
@@ -470,14 +419,14 @@ __global__ void __launch_bounds__(128) k_s0_heavy(SlotDev s, Params g) {
             if (cnt >= min_shared) hit = dd_beats(s, dd_ref(s, n5, np5, b), A);
           }
         }
-        beaten = __any_sync(0xffffffffu, hit);
+        beaten = __syncthreads_or(hit) != 0;
       }
-      __syncwarp();
-      if (lane < A.n_ot) tab[slot] = 0xFFFFFFFFu;                 // leave the table empty for the next object
+      __syncthreads();
+      if (wib == 0 && lane < A.n_ot) tab[slot] = 0xFFFFFFFFu;     // leave the table empty for the next object
       // objects of the same pixel seed are duplicates of one another: only the seed's best survives
       if (!beaten && A.type != 0 && (A.type == 1 ? s.pls_best5 : s.pls_best3)[A.pls] != A.idx) beaten = true;
     }
-    if (lane == 0) {
+    if (threadIdx.x == 0) {
       const bool keep = !beaten;
       if (A.type == 0) s.t5_keep[A.idx] = keep;
       else if (A.type == 1) {
@@ -494,8 +443,9 @@ __global__ void __launch_bounds__(128) k_s0_heavy(SlotDev s, Params g) {
 }
 
 // ------------------------------------------------------------------ S1: pT3 against surviving pT5
-__global__ void __launch_bounds__(128) k_s1(SlotDev s, Params g) {
-  (void)g;
+__global__ void __launch_bounds__(128) k_s1(const __grid_constant__ Batch B) {
+  pdl_enter();
+  LST_SLOT(B);
   const Header *hdr = s.hdr;
   const uint32_t np3 = hdr->n_obj[4];
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < np3; i += gridDim.x * blockDim.x) {
@@ -520,30 +470,59 @@ __global__ void __launch_bounds__(128) k_s1(SlotDev s, Params g) {
 }
 
 // ------------------------------------------------------------------ S2: T5 against surviving pT5 / pT3
-__global__ void __launch_bounds__(128) k_s2(SlotDev s, Params g) {
+// A warp takes 32 T5 at a time (lane = object: keep flag and the ten hit flags), then the objects
+// still alive one by one, all lanes striding over the seeds of the object's eta bins (the loops over
+// ~30 binned seeds with fp64 distance tests were the latency of the thread-per-object version).
+__global__ void __launch_bounds__(128) k_s2(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
+  pdl_enter();
+  LST_SLOT(B);
   const Header *hdr = s.hdr;
   const uint32_t n5 = hdr->n_obj[3];
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n5; i += gridDim.x * blockDim.x) {
-    if (!s.t5_keep[i]) continue;
-    bool dup = false;
+  const int lane = threadIdx.x & 31;
+  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+  for (uint32_t base = warp * 32; base < n5; base += nwarp * 32) {
+    const uint32_t i = base + lane;
+    bool alive = i < n5 && s.t5_keep[i] != 0;
+    if (alive) {
+      bool dup = false;
 #pragma unroll
-    for (int q = 0; q < 10; ++q) {
-      const uint32_t h = s.t5_hits[10 * (size_t)i + q];
-      dup |= (s.hit_used5[h] | s.hit_used3[h]) != 0;
+      for (int q = 0; q < 10; ++q) {
+        const uint32_t h = s.t5_hits[10 * (size_t)i + q];
+        dup |= (s.hit_used5[h] | s.hit_used3[h]) != 0;
+      }
+      if (dup) { s.t5_keep[i] = 0; alive = false; }
     }
-    const double2 ep = s.t5_etaphi[i];
-    const int b0 = eta_bin(g, ep.x);
-    const int lo = b0 > 0 ? b0 - 1 : 0, hi = b0 + 1 < g.eta_nbins ? b0 + 1 : g.eta_nbins - 1;
-    const uint32_t e0 = s.pls_bin_off[lo], e1 = s.pls_bin_off[hi + 1];
-    for (uint32_t e = e0; e < e1 && !dup; ++e) {
-      const uint32_t p = s.pls_bin_ent[e];
-      if ((s.pls_has5[p] || s.pls_has3[p]) && close_eta_phi(g, ep.x, ep.y, (double)s.seed_eta[p], (double)s.seed_phi[p]))
-        dup = true;
-    }
-    if (dup) { s.t5_keep[i] = 0; continue; }
-    for (uint32_t e = e0; e < e1; ++e) {   // survivor: the seeds close to it are duplicates of it (S3)
-      const uint32_t p = s.pls_bin_ent[e];
-      if (close_eta_phi(g, ep.x, ep.y, (double)s.seed_eta[p], (double)s.seed_phi[p])) s.pls_near_t5[p] = 1;
+    uint32_t todo = __ballot_sync(0xffffffffu, alive);
+    while (todo) {
+      const int src = __ffs(todo) - 1;
+      todo &= todo - 1;
+      const uint32_t o = base + src;
+      const double2 ep = s.t5_etaphi[o];
+      const int b0 = eta_bin(g, ep.x);
+      const int lo = b0 > 0 ? b0 - 1 : 0, hi = b0 + 1 < g.eta_nbins ? b0 + 1 : g.eta_nbins - 1;
+      const uint32_t e0 = s.pls_bin_off[lo], e1 = s.pls_bin_off[hi + 1];
+      bool dup = false;
+      uint32_t near_mask_any = 0;
+      for (uint32_t eb = e0; eb < e1; eb += 32) {
+        const uint32_t e = eb + lane;
+        bool close = false, used = false;
+        if (e < e1) {
+          const uint32_t p = s.pls_bin_ent[e];
+          close = close_eta_phi(g, ep.x, ep.y, (double)s.seed_eta[p], (double)s.seed_phi[p]);
+          used = close && (s.pls_has5[p] || s.pls_has3[p]);
+        }
+        dup |= __any_sync(0xffffffffu, used);
+        near_mask_any |= __ballot_sync(0xffffffffu, close);
+      }
+      if (dup) { if (lane == 0) s.t5_keep[o] = 0; continue; }
+      if (near_mask_any == 0u) continue;
+      for (uint32_t eb = e0; eb < e1; eb += 32) {   // survivor: the seeds close to it are duplicates of it (S3)
+        const uint32_t e = eb + lane;
+        if (e < e1) {
+          const uint32_t p = s.pls_bin_ent[e];
+          if (close_eta_phi(g, ep.x, ep.y, (double)s.seed_eta[p], (double)s.seed_phi[p])) s.pls_near_t5[p] = 1;
+        }
+      }
     }
   }
 }
@@ -552,10 +531,19 @@ __global__ void __launch_bounds__(128) k_s2(SlotDev s, Params g) {
 __device__ __forceinline__ bool pls_unused(const SlotDev &s, uint32_t p) {
   return s.pt5_pls_off[p + 1] == s.pt5_pls_off[p] && s.pt3_pls_off[p + 1] == s.pt3_pls_off[p];
 }
-__global__ void k_s3_flags(SlotDev s) {
-  const Header *hdr = s.hdr;
-  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], np3 = hdr->n_obj[4], n = hdr->n_flag;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+// Block b owns the flags [b C, (b + 1) C), C = ceil(n_flag / gridDim.x); it also counts them, and the
+// last block to finish scans the per-block counts: k_tc_fill (same grid) places a kept entry at its
+// block's offset + its rank inside the block.
+__global__ void __launch_bounds__(256) k_s3_flags(const __grid_constant__ Batch B) {
+  __shared__ uint32_t sh[33];
+  pdl_enter();
+  LST_SLOT(B);
+  Header *hdr = s.hdr;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], np3 = hdr->n_obj[4], n = np5 + np3 + n5 + hdr->n_seeds;
+  const uint32_t C = (n + gridDim.x - 1) / gridDim.x;
+  const uint32_t i0 = min(n, blockIdx.x * C), i1 = min(n, i0 + C);
+  uint32_t mine = 0;
+  for (uint32_t i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
     uint32_t f;
     if (i < np5) f = s.pt5_keep[i];
     else if (i < np5 + np3) f = s.pt3_keep[i - np5];
@@ -573,30 +561,48 @@ __global__ void k_s3_flags(SlotDev s) {
       f = keep;
     }
     s.tc_flag[i] = f;
+    mine += f != 0u;
   }
+  uint32_t tot;
+  block_excl_scan(mine, sh, &tot);
+  if (threadIdx.x == 0) s.flag_blk[blockIdx.x] = tot;
+  if (!last_block(&hdr->ticket[TK_FLAGS], gridDim.x)) return;
+  const uint32_t total = lb_scan_parts(s.flag_blk, gridDim.x, sh);
+  if (threadIdx.x == 0) hdr->n_obj[6] = total;
 }
 
 // ------------------------------------------------------------------ S4: TC = pT5, pT3, T5, pLS survivors
-__global__ void k_tc_fill(SlotDev s) {
-  Header *hdr = s.hdr;
-  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], np3 = hdr->n_obj[4], n = hdr->n_flag;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-    if (!s.tc_flag[i]) continue;
-    const uint32_t pos = s.tc_pos[i];
-    uint32_t type, obj, p = 0xFFFFFFFFu;
-    if (i < np5) { type = 5; obj = i; p = s.pt5_po[obj].x; }
-    else if (i < np5 + np3) { type = 4; obj = i - np5; p = s.pt3_po[obj].x; }
-    else if (i < np5 + np3 + n5) { type = 3; obj = i - np5 - np3; }
-    else { type = 6; obj = i - np5 - np3 - n5; p = obj; }
-    s.tc_to[pos] = make_uint2(type, obj);
-    if (type == 3) {
-      const double2 ep = s.t5_etaphi[obj];
-      s.tc_f[pos] = make_float4(s.t5_pt[obj], (float)ep.x, (float)ep.y, 3.0f);
-    } else {
-      s.tc_f[pos] = make_float4(s.seed_pt[p], s.seed_eta[p], s.seed_phi[p], (float)type);
+__global__ void __launch_bounds__(256) k_tc_fill(const __grid_constant__ Batch B) {
+  __shared__ uint32_t sh[33];
+  pdl_enter();
+  LST_SLOT(B);
+  const Header *hdr = s.hdr;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], np3 = hdr->n_obj[4], n = np5 + np3 + n5 + hdr->n_seeds;
+  const uint32_t C = (n + gridDim.x - 1) / gridDim.x;
+  const uint32_t i0 = min(n, blockIdx.x * C), i1 = min(n, i0 + C);
+  uint32_t carry = s.flag_blk[blockIdx.x];
+  for (uint32_t base = i0; base < i1; base += blockDim.x) {
+    const uint32_t i = base + threadIdx.x;
+    const bool keep = i < i1 && s.tc_flag[i] != 0u;
+    uint32_t tot;
+    const uint32_t pos = carry + block_excl_scan(keep ? 1u : 0u, sh, &tot);
+    carry += tot;
+    if (keep) {
+      uint32_t type, obj, p = 0xFFFFFFFFu;
+      if (i < np5) { type = 5; obj = i; p = s.pt5_po[obj].x; }
+      else if (i < np5 + np3) { type = 4; obj = i - np5; p = s.pt3_po[obj].x; }
+      else if (i < np5 + np3 + n5) { type = 3; obj = i - np5 - np3; }
+      else { type = 6; obj = i - np5 - np3 - n5; p = obj; }
+      s.tc_to[pos] = make_uint2(type, obj);
+      if (type == 3) {
+        const double2 ep = s.t5_etaphi[obj];
+        s.tc_f[pos] = make_float4(s.t5_pt[obj], (float)ep.x, (float)ep.y, 3.0f);
+      } else {
+        s.tc_f[pos] = make_float4(s.seed_pt[p], s.seed_eta[p], s.seed_phi[p], (float)type);
+      }
     }
+    __syncthreads();
   }
-  if (blockIdx.x == 0 && threadIdx.x == 0) hdr->n_obj[6] = s.tc_pos[n];
 }
 
 static inline int grid_of(uint32_t n, int threads, int max_blocks) {
@@ -604,29 +610,20 @@ static inline int grid_of(uint32_t n, int threads, int max_blocks) {
   return (int)(b < 1 ? 1 : (b > max_blocks ? max_blocks : b));
 }
 
-void launch_dedup(const Ctx &c, const SlotDev &s, cudaStream_t st) {
+// The zeroed scratch (incidence counters, seed / hit / pixel-id flags) and the 0xFF-filled per-seed
+// minima are set by the two memsets at the start of the chain (lst_api.cu).
+void launch_dedup(const Ctx &c, const Batch &b, cudaStream_t st) {
+  const SlotDev &s = b.s[0];
   const uint32_t cap_dd = s.cap_t5 + s.cap_pt5 + s.cap_pt3;
-  cudaMemsetAsync(s.inc_cnt, 0, sizeof(uint32_t) * 2 * (3 * (size_t)s.cap_hits + 1), st);
-  cudaMemsetAsync(s.pls_has5, 0, 3 * (size_t)s.cap_seeds, st);
-  cudaMemsetAsync(s.hit_used5, 0, 2 * (size_t)s.cap_hits, st);
-  k_pls_prep<<<1, 1024, 0, st>>>(s, c.par); LST_MARK(c, st, "k_pls_prep");
-  cudaMemsetAsync(s.pid_key, 0, sizeof(unsigned long long) * (size_t)s.pid_size, st);
-  cudaMemsetAsync(s.pid_has5, 0, 2 * (size_t)s.pid_size, st);
-  k_pls_adj<<<grid_of(s.cap_seeds, 256, c.n_sm * 8), 256, 0, st>>>(s, c.par); LST_MARK(c, st, "k_pls_adj");
-  k_pid_insert<<<grid_of(4 * s.cap_seeds, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_pid_insert");
-  k_dd_count<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_dd_count");
-  launch_scan(c, s, s.inc_cnt, s.inc_off, &s.hdr->n_inc, st);
-  k_dd_scatter<<<grid_of(cap_dd, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_dd_scatter");
-  cudaMemsetAsync(s.pls_min5, 0xFF, 24 * (size_t)s.cap_seeds, st);      // pls_min5, pls_min3, pls_best5, pls_best3
-  k_pls_min<<<grid_of(s.cap_pt5 + s.cap_pt3, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_pls_min");
-  k_pls_best<<<grid_of(s.cap_pt5 + s.cap_pt3, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_pls_best");
-  k_s0<<<grid_of(cap_dd, 16, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s0");
-  k_s0_heavy<<<grid_of(cap_dd, 4, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s0_heavy");
-  k_s1<<<grid_of(s.cap_pt3, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s1");
-  k_s2<<<grid_of(s.cap_t5, 128, c.n_sm * 16), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_s2");
-  k_s3_flags<<<grid_of(s.cap_tc, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_s3_flags");
-  launch_scan(c, s, s.tc_flag, s.tc_pos, &s.hdr->n_flag, st);
-  k_tc_fill<<<grid_of(s.cap_tc, 256, c.n_sm * 8), 256, 0, st>>>(s); LST_MARK(c, st, "k_tc_fill");
+  launch_k(c, st, "k_dd_count", k_dd_count, dim3(grid_of(cap_dd, 256, c.n_sm * 8)), 256, 0, false, b, c.par);
+  launch_scan(c, b, 0, st);
+  launch_k(c, st, "k_dd_scatter", k_dd_scatter, dim3(grid_of(cap_dd, 256, c.n_sm * 8)), 256, 0, false, b);
+  launch_k(c, st, "k_s0", k_s0, dim3(grid_of(cap_dd, 16, c.n_sm * 16)), 128, 0, false, b, c.par);
+  launch_k(c, st, "k_s0_heavy", k_s0_heavy, dim3(grid_of(cap_dd, 4, c.n_sm * 16)), 128, 0, false, b, c.par);
+  launch_k(c, st, "k_s1", k_s1, dim3(grid_of(s.cap_pt3, 128, c.n_sm * 16)), 128, 0, false, b);
+  launch_k(c, st, "k_s2", k_s2, dim3(grid_of(s.cap_t5, 128, c.n_sm * 8)), 128, 0, false, b, c.par);
+  launch_k(c, st, "k_s3_flags", k_s3_flags, dim3(kFlagBlocks), 256, 0, false, b);
+  launch_k(c, st, "k_tc_fill", k_tc_fill, dim3(kFlagBlocks), 256, 0, false, b);
 }
 
 }  // namespace lst

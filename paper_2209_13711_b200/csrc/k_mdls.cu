@@ -10,43 +10,63 @@ namespace lst {
 // the fp32 pre-filter, the survivors are appended to the stage's candidate list.
 // k_md_decide: one thread per listed pair, fp64 decision; accepted pairs set their pass bit and
 // write kappa, sigma_kappa and dphi to the pool.
-__global__ void __launch_bounds__(256) k_md_eval(GeoDev geo, SlotDev s, Params g) {
+__global__ void __launch_bounds__(256) k_md_eval(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
+                                                  const __grid_constant__ Params g) {
   __shared__ ClStageT<64> cl_mem[256 / 32];
+  pdl_enter();
+  LST_SLOT(B);
   const StageBuf &st = s.st[S_MD];
-  const uint32_t n_items = s.hdr->n_items[S_MD];
+  const bool live = s.hdr->n_items[S_MD] != 0;      // 0: nothing to do, or the work list overflowed
   const int lane = threadIdx.x & 31;
   const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
   ClBufT<64> cl;
   cl.init(&cl_mem[threadIdx.x >> 5]);
-  constexpr int kSlices = 8, kSliceCand = kItemCand / kSlices;   // a warp task = 128 candidates of an item
-  for (uint32_t w = warp; w < n_items * kSlices; w += nwarp) {
-    const uint32_t it = w / kSlices, sl = w % kSlices;
-    const Item item = st.items[it];
-    const int nj = item.nj, nc = item.nrows * nj;
-    if (sl == 0) st.mask[(size_t)it * kItemWords + lane] = 0;  // the decide kernel ORs the pass bits in
-    if ((int)(sl * kSliceCand) >= nc) continue;
-    const uint32_t m = item.group;
+  constexpr int kSlices = 8, kSliceCand = kItemCand / kSlices;   // a warp task = slice `sl` (128 candidates) of every item of a module
+  const uint32_t n_task = live ? geo.n_modules * kSlices : 0u;
+  for (uint32_t w = warp; w < n_task; w += nwarp) {
+    const uint32_t m = w / kSlices, sl = w % kSlices;
+    const uint32_t R = st.gR[m], W = st.gW[m];
+    if ((unsigned long long)sl * kSliceCand >= (unsigned long long)R * W) continue;           // also R W == 0; a module of several items has R W > kItemCand
+    const uint32_t it0 = st.g_item0[m], rpi = item_rpi(W), nct = item_nct(W);
+    const uint32_t n_it = ((R + rpi - 1) / rpi) * nct;
     const int cat = geo.category[m];
-    const uint32_t lo0 = s.det_off[2 * m] + item.i0, up0 = s.det_off[2 * m + 1] + item.j0;
-    const uint32_t inv = (1u << 20) / (uint32_t)nj + 1u;      // c / nj == (c * inv) >> 20 for c * nj < 2^20
-    const int c_end = min(nc, (int)((sl + 1) * kSliceCand));
-    for (int base = (int)(sl * kSliceCand); base < c_end; base += 32) {
-      const int c = base + lane;
-      bool keep = false;
-      uint32_t hl = 0, hu = 0;
-      if (c < c_end) {
-        const int r = (int)(((uint32_t)c * inv) >> 20), jj = c - r * nj;
-        hl = lo0 + r; hu = up0 + jj;
-        const float4 l = s.hit[hl], u = s.hit[hu];
-        keep = md_pre_f(g, l.x, l.y, l.z, l.w, u.x, u.y, u.z, u.w, cat);
+    const uint32_t lo_m = s.det_off[2 * m], up_m = s.det_off[2 * m + 1];
+    for (uint32_t k = 0; k < n_it; ++k) {
+      const uint32_t it = it0 + k;
+      uint32_t i0, j0;
+      int nrows, nj;
+      if (W <= (uint32_t)kItemCand) { i0 = k * rpi; j0 = 0; nrows = (int)min(rpi, R - i0); nj = (int)W; }
+      else { i0 = k / nct; j0 = (k % nct) * kItemCand; nrows = 1; nj = (int)min((uint32_t)kItemCand, W - j0); }
+      if (sl == 0) {
+        st.mask[(size_t)it * kItemWords + lane] = 0;             // the decide kernel ORs the pass bits in
+        if (lane == 0) st.item_group[it] = m;
       }
-      cl.push(s.hdr, st, S_MD, keep, it * (uint32_t)kItemCand + (uint32_t)c, make_uint2(hl, hu));
+      const int nc = nrows * nj;
+      if ((int)(sl * kSliceCand) >= nc) continue;
+      const uint32_t lo0 = lo_m + i0, up0 = up_m + j0;
+      const uint32_t inv = (1u << 20) / (uint32_t)nj + 1u;      // c / nj == (c * inv) >> 20 for c * nj < 2^20
+      const int c_end = min(nc, (int)((sl + 1) * kSliceCand));
+      for (int base = (int)(sl * kSliceCand); base < c_end; base += 32) {
+        const int c = base + lane;
+        bool keep = false;
+        uint32_t hl = 0, hu = 0;
+        if (c < c_end) {
+          const int r = (int)(((uint32_t)c * inv) >> 20), jj = c - r * nj;
+          hl = lo0 + r; hu = up0 + jj;
+          const float4 l = s.hit[hl], u = s.hit[hu];
+          keep = md_pre_f(g, l.x, l.y, l.z, l.w, u.x, u.y, u.z, u.w, cat);
+        }
+        cl.push(s.hdr, st, S_MD, keep, it * (uint32_t)kItemCand + (uint32_t)c, make_uint2(hl, hu));
+      }
     }
   }
   cl.flush_all(s.hdr, st, S_MD);
 }
 
-__global__ void __launch_bounds__(128) k_md_decide(GeoDev geo, SlotDev s, Params g) {
+__global__ void __launch_bounds__(128) k_md_decide(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
+                                                    const __grid_constant__ Params g) {
+  pdl_enter();
+  LST_SLOT(B);
   const StageBuf &st = s.st[S_MD];
   Header *hdr = s.hdr;
   const uint32_t n = min(hdr->cl_used[S_MD], st.cap_cl);
@@ -58,7 +78,7 @@ __global__ void __launch_bounds__(128) k_md_decide(GeoDev geo, SlotDev s, Params
     if (j < n) {
       key = st.cl_key[j];
       const uint2 ab = st.cl_ab[j];
-      const int cat = geo.category[st.items[key / kItemCand].group];
+      const int cat = geo.category[st.item_group[key / kItemCand]];
       const float4 l = s.hit[ab.x], u = s.hit[ab.y];
       const Pt pl = make_pt(l.x, l.y, l.z, cat), pu = make_pt(u.x, u.y, u.z, cat);
       pass = md_eval_d(g, pl, pu, cat, &o);
@@ -71,17 +91,23 @@ __global__ void __launch_bounds__(128) k_md_decide(GeoDev geo, SlotDev s, Params
   }
 }
 
-// One thread per listed pair: the accepted ones move to their canonical position.
-__global__ void __launch_bounds__(256) k_md_fill(GeoDev geo, SlotDev s) {
+// One thread per listed pair: the accepted ones move to their canonical position.  Then the MD range
+// of every module (md_mod_off) from the rank of the module's first candidate.
+__global__ void __launch_bounds__(256) k_md_fill(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B) {
+  pdl_enter();
+  LST_SLOT(B);
   const StageBuf &st = s.st[S_MD];
   const Header *hdr = s.hdr;
-  if (hdr->n_obj[0] == 0) return;                            // nothing built, or overflow (level emptied)
-  const uint32_t n = min(hdr->cl_used[S_MD], st.cap_cl);
-  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+  const uint32_t n_md = hdr->n_obj[0], n_items = hdr->n_items[S_MD];
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nt = gridDim.x * blockDim.x;
+  for (uint32_t m = tid; m <= geo.n_modules; m += nt)
+    s.md_mod_off[m] = rank_before(st, n_items, n_md, st.g_item0[m] * (uint32_t)kItemCand);
+  const uint32_t n = n_md ? min(hdr->cl_used[S_MD], st.cap_cl) : 0u;     // n_md == 0: nothing built, or overflow (level emptied)
+  for (uint32_t j = tid; j < n; j += nt) {
     const uint32_t key = st.cl_key[j];
     const uint32_t idx = pool_target(st, key);
     if (idx == 0xFFFFFFFFu) continue;
-    const uint32_t m = st.items[key / kItemCand].group;
+    const uint32_t m = st.item_group[key / kItemCand];
     const uint2 h = st.cl_ab[j];
     const float4 l = s.hit[h.x];
     const double2 kd = st.p_d2[j];
@@ -101,11 +127,20 @@ __global__ void __launch_bounds__(256) k_md_fill(GeoDev geo, SlotDev s) {
 // candidates of the method's definition: all MD pairs in map-connected modules; a candidate's pass
 // bit sits at (row, column) of that rectangle whatever part of it the enumeration visits).  The same
 // warp also writes A's ModEv record for the per-row windows of k_ls_eval.
-__global__ void __launch_bounds__(256) k_ls_groups(GeoDev geo, SlotDev s) {
+constexpr int kLsGroupWarps = 8;     // modules per block of k_ls_groups
+__global__ void __launch_bounds__(32 * kLsGroupWarps) k_ls_groups(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B) {
+  __shared__ uint32_t sh_items[kLsGroupWarps];
+  __shared__ unsigned long long sh_cand[kLsGroupWarps];
+  __shared__ uint32_t sh[33];
+  pdl_enter();
+  LST_SLOT(B);
   const StageBuf &st = s.st[S_LS];
-  const int lane = threadIdx.x & 31;
-  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
-  for (uint32_t A = warp; A < geo.n_modules; A += nwarp) {
+  Header *hdr = s.hdr;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const uint32_t A = blockIdx.x * kLsGroupWarps + wib;
+  uint32_t my_items = 0;
+  unsigned long long my_cand = 0;
+  if (A < geo.n_modules) {
     const uint32_t m0 = s.md_mod_off[A], R = s.md_mod_off[A + 1] - m0;
     uint32_t W = 0;
     float rlo = 3.0e38f, rhi = -3.0e38f, zlo = 3.0e38f, zhi = -3.0e38f;
@@ -117,7 +152,7 @@ __global__ void __launch_bounds__(256) k_ls_groups(GeoDev geo, SlotDev s) {
       for (uint32_t eb = e0; eb < e1; eb += 32) {
         const uint32_t e = eb + lane;
         uint32_t n = 0;
-        if (e < e1) { const uint32_t B = geo.map_cols[e]; n = s.md_mod_off[B + 1] - s.md_mod_off[B]; }
+        if (e < e1) { const uint32_t mb = geo.map_cols[e]; n = s.md_mod_off[mb + 1] - s.md_mod_off[mb]; }
         uint32_t tot;
         const uint32_t ex = warp_excl_scan(n, &tot);
         if (e < e1) s.edge_col0[e] = W + ex;
@@ -166,9 +201,36 @@ __global__ void __launch_bounds__(256) k_ls_groups(GeoDev geo, SlotDev s) {
       st.gR[A] = R;
       st.gW[A] = W;
     }
+    my_items = items_of(R, W);
+    my_cand = (unsigned long long)R * W;
   }
-  if (blockIdx.x == 0 && threadIdx.x == 0) s.hdr->n_groups[S_LS] = geo.n_modules;
+  // first item of every group: exclusive prefix inside the block here, across blocks in the last block
+  if (lane == 0) { sh_items[wib] = my_items; sh_cand[wib] = my_cand; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t acc = 0;
+    unsigned long long cs = 0;
+    for (int k = 0; k < kLsGroupWarps; ++k) {
+      const uint32_t g = blockIdx.x * kLsGroupWarps + k;
+      if (g < geo.n_modules) st.g_item0[g] = acc;
+      acc += sh_items[k]; cs += sh_cand[k];
+    }
+    st.gblk[blockIdx.x] = acc;
+    if (cs) atomicAdd(&hdr->cand[S_LS], cs);
+  }
+  if (!last_block(&hdr->ticket[TK_GROUPS + S_LS], gridDim.x)) return;
+  const uint32_t total = lb_scan_parts(st.gblk, gridDim.x, sh);
+  const uint32_t ng = geo.n_modules;
+  lb_add_block_prefix(st.g_item0, ng, st.gblk, kLsGroupWarps);
+  if (threadIdx.x == 0) {
+    const bool overflow = total > st.cap_items;
+    st.g_item0[ng] = total;
+    hdr->n_groups[S_LS] = ng;
+    hdr->n_items[S_LS] = overflow ? 0u : total;
+    if (overflow) atomicOr(&hdr->err, (uint32_t)ERR_CAP_ITEMS);
+  }
 }
+
 
 // k_ls_eval: the fp32 pre-filter of the LS stage.  A warp takes kLsGrab consecutive rows (inner MDs)
 // at a time, handed out dynamically.  The definition is "all MDs of the modules connected to the
@@ -184,6 +246,20 @@ __global__ void __launch_bounds__(256) k_ls_groups(GeoDev geo, SlotDev s) {
 //     through a warp queue to ls_pre_f on 32 dense lanes.
 // A candidate's key is that of the full rectangle: key_base(row) + column index in the row's column list.
 constexpr int kLsGrab = 4;
+// key of the first candidate of row r (relative to its module A, W > 0 columns) and the items the row starts
+__device__ __forceinline__ uint32_t ls_key_base(const StageBuf &st, uint32_t A, uint32_t r, uint32_t W, uint32_t *first_item,
+                                                uint32_t *n_start) {
+  if (W <= (uint32_t)kItemCand) {
+    const uint32_t rpi = item_rpi(W), q = r / rpi, it = st.g_item0[A] + q;
+    *first_item = it;
+    *n_start = (r == q * rpi) ? 1u : 0u;
+    return it * (uint32_t)kItemCand + (r - q * rpi) * W;
+  }
+  const uint32_t nct = item_nct(W), it = st.g_item0[A] + r * nct;
+  *first_item = it;
+  *n_start = nct;
+  return it * (uint32_t)kItemCand;
+}
 // count word of edge k (1 <= k <= 14): cum(k) = cum[k - 1] sits in u16 slot k - 1 of the 7 words q2.y .. q3.w
 __device__ __forceinline__ uint32_t bin_cum(const uint4 &q2, const uint4 &q3, int k, uint32_t n) {
   if (k <= 0) return 0u;
@@ -201,22 +277,28 @@ struct LsWarpSh {
   uint32_t r_key[kLsGrab], r_e0[kLsGrab], r_pre[kLsGrab + 1];   // key_base, first map edge, prefix of the degrees
 };
 
-// Tier 2 (mode Z only) on up to 32 queued tier-1 survivors; what passes goes to the stage's candidate list.
+// Tier 2 on up to 32 queued tier-1 survivors (dense lanes): cut L3 in its square-root-only mode-R form
+// for an outer MD in a barrel module, the full fp32 pre-filter for an outer MD in an endcap module;
+// what passes goes to the stage's candidate list.
 __device__ __forceinline__ void ls_stage2(const SlotDev &s, const Params &g, WarpQueue3 &Q1, ClBuf &cl) {
   uint32_t mi = 0, mo = 0, key = 0;
   bool keep = false;
   if (Q1.pop(&mi, &mo, &key)) {
     const float4 a = s.md_pos[mi], b = s.md_pos[mo];
     const float2 ka = s.md_kf[mi], kb = s.md_kf[mo];
-    keep = ls_pre_f(g, a.x, a.y, a.z, a.w, ka.x, ka.y, (int)(s.md_mod[mi] & 3u), b.x, b.y, b.z, b.w, kb.x, kb.y,
-                    (int)(s.md_mod[mo] & 3u));
+    const int ci = (int)(s.md_mod[mi] & 3u), co = (int)(s.md_mod[mo] & 3u);
+    if (co < 2) keep = ls_l3_modeR_f(g, a.x, a.y, a.w, ka.x, ka.y, g.f_sig_t[ci], ci >= 2, b.x, b.y, b.w, kb.x, kb.y, g.f_sig_t[co]);
+    else keep = ls_pre_f(g, a.x, a.y, a.z, a.w, ka.x, ka.y, ci, b.x, b.y, b.z, b.w, kb.x, kb.y, co);
   }
   cl.push(s.hdr, s.st[S_LS], S_LS, keep, key, make_uint2(mi, mo));
 }
 
-__global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, Params g, int use_windows) {
+__global__ void __launch_bounds__(kThreads, 8) k_ls_eval(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
+                                                         const __grid_constant__ Params g, int use_windows) {
   __shared__ LsWarpSh sh_all[kThreads / 32];
   __shared__ float4 tab[4];                     // per category: sig_z, sig_r, sig_t
+  pdl_enter();
+  LST_SLOT(B);
   const StageBuf &st = s.st[S_LS];
   const uint32_t n_md = s.hdr->n_obj[0];
   const int tid = threadIdx.x, lane = tid & 31;
@@ -236,7 +318,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
     r0 = __shfl_sync(0xffffffffu, r0, 0);
     if (r0 >= n_md || !live_stage) break;
     // ---- lanes 0 .. kLsGrab-1 set up one row each
-    uint32_t deg = 0;
+    uint32_t deg = 0, clr_item = 0, clr_n = 0;
     if (lane < kLsGrab && r0 + lane < n_md) {
       const uint32_t i = r0 + lane;
       const uint32_t mc = s.md_mod[i], A = mc >> 2;
@@ -244,13 +326,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
       if (W) {
         const float2 kf = s.md_kf[i];
         const uint32_t r = i - s.md_mod_off[A];
-        uint32_t key_base;
-        if (W <= (uint32_t)kItemCand) {
-          const uint32_t rpi = item_rpi(W), q = r / rpi;
-          key_base = (st.g_item0[A] + q) * (uint32_t)kItemCand + (r - q * rpi) * W;
-        } else {
-          key_base = (st.g_item0[A] + r * item_nct(W)) * (uint32_t)kItemCand;
-        }
+        const uint32_t key_base = ls_key_base(st, A, r, W, &clr_item, &clr_n);
         const uint32_t e0 = geo.map_off[A];
         deg = geo.map_off[A + 1] - e0;
         sh.r_pos[lane] = s.md_pos[i];
@@ -262,6 +338,12 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
     uint32_t P;
     const uint32_t dpre = warp_excl_scan(deg, &P);
     if (lane <= kLsGrab) sh.r_pre[lane] = dpre;             // r_pre[kLsGrab] = P (lanes >= kLsGrab have deg 0)
+    // the row that starts a work item clears the item's pass bits (the decide kernel ORs them in)
+#pragma unroll
+    for (int q = 0; q < kLsGrab; ++q) {
+      const uint32_t ci = __shfl_sync(0xffffffffu, clr_item, q), cn = __shfl_sync(0xffffffffu, clr_n, q);
+      for (uint32_t w = lane; w < cn * (uint32_t)kItemWords; w += 32) st.mask[(size_t)ci * kItemWords + w] = 0;
+    }
     __syncwarp();
     for (uint32_t pb = 0; pb < P; pb += 32) {
       // ---- lanes = (row, connected module) pairs: the range of the module's MDs the row has to look at
@@ -325,7 +407,7 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
         if (sidx < nseg) { const uint32_t f = sh.seg_f[sidx]; if (f < w0 + 32u) bit = 1u << (f - w0); }
         const uint32_t starts = __reduce_or_sync(0xffffffffu, bit);
         const uint32_t f = w0 + lane;
-        bool keepR = false, keepZ = false;
+        bool keep = false;
         uint32_t mi = 0, mo = 0, key = 0;
         if (f < T) {
           const uint32_t sg = sbefore + __popc(starts & le_mask) - 1u;
@@ -337,18 +419,10 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
           const float4 b = s.md_pos[mo];
           const uint32_t ci = __float_as_uint(ax.w), co = smd >> 30;
           const float4 ta = tab[ci], tb = tab[co];
-          const bool oec = co >= 2u;
-          bool keep = ls_tier1_f(g, a.x, a.y, a.z, a.w, ta.x, ta.y, ta.z, b.x, b.y, b.z, b.w, tb.x, tb.y, tb.z, oec);
-          if (keep && !oec) {
-            const float2 kb = s.md_kf[mo];
-            keep = ls_l3_modeR_f(g, a.x, a.y, a.w, ax.y, ax.z, ta.z, ci >= 2u, b.x, b.y, b.w, kb.x, kb.y, tb.z);
-          }
-          keepR = keep && !oec;
-          keepZ = keep && oec;
+          keep = ls_tier1_f(g, a.x, a.y, a.z, a.w, ta.x, ta.y, ta.z, b.x, b.y, b.z, b.w, tb.x, tb.y, tb.z, co >= 2u);
         }
         sbefore += __popc(starts);
-        cl.push(s.hdr, st, S_LS, keepR, key, make_uint2(mi, mo));
-        Q1.push(keepZ, mi, mo, key);
+        Q1.push(keep, mi, mo, key);
         if (Q1.n >= 32u) ls_stage2(s, g, Q1, cl);
       }
       __syncwarp();                           // the segment table is rewritten by the next 32 pairs
@@ -362,7 +436,9 @@ __global__ void __launch_bounds__(kThreads, 8) k_ls_eval(GeoDev geo, SlotDev s, 
 
 // fp64 decision of the listed candidates, one thread each (dense warps, no staging); an accepted
 // candidate sets its pass bit and writes its results to the pool.
-__global__ void __launch_bounds__(128) k_ls_decide(SlotDev s, Params g) {
+__global__ void __launch_bounds__(128) k_ls_decide(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
+  pdl_enter();
+  LST_SLOT(B);
   const StageBuf &st = s.st[S_LS];
   Header *hdr = s.hdr;
   const uint32_t n = min(hdr->cl_used[S_LS], st.cap_cl);
@@ -386,13 +462,27 @@ __global__ void __launch_bounds__(128) k_ls_decide(SlotDev s, Params g) {
   }
 }
 
-// One thread per pool entry: move it to its canonical position.
-__global__ void __launch_bounds__(256) k_ls_fill(SlotDev s) {
+// One thread per pool entry: move it to its canonical position.  Then the LS range of every inner MD
+// (ls_md_off) from the rank of the row's first candidate.
+__global__ void __launch_bounds__(256) k_ls_fill(const __grid_constant__ Batch B) {
+  pdl_enter();
+  LST_SLOT(B);
   const StageBuf &st = s.st[S_LS];
   const Header *hdr = s.hdr;
-  if (hdr->n_obj[1] == 0) return;
-  const uint32_t n = min(hdr->cl_used[S_LS], st.cap_cl);
-  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+  const uint32_t n_md = hdr->n_obj[0], n_ls = hdr->n_obj[1], n_items = hdr->n_items[S_LS];
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nt = gridDim.x * blockDim.x;
+  for (uint32_t i = tid; i <= n_md; i += nt) {
+    uint32_t off = n_ls;
+    if (i < n_md) {
+      const uint32_t A = s.md_mod[i] >> 2, W = st.gW[A];
+      uint32_t key = st.g_item0[A] * (uint32_t)kItemCand, fi, ns;
+      if (W) key = ls_key_base(st, A, i - s.md_mod_off[A], W, &fi, &ns);
+      off = rank_before(st, n_items, n_ls, key);
+    }
+    s.ls_md_off[i] = off;
+  }
+  const uint32_t n = n_ls ? min(hdr->cl_used[S_LS], st.cap_cl) : 0u;
+  for (uint32_t j = tid; j < n; j += nt) {
     const uint32_t idx = pool_target(st, st.cl_key[j]);
     if (idx == 0xFFFFFFFFu) continue;
     s.ls_md[idx] = st.cl_ab[j];
@@ -403,25 +493,20 @@ __global__ void __launch_bounds__(256) k_ls_fill(SlotDev s) {
 // ------------------------------------------------------------------ launchers
 static inline int persistent_grid(const Ctx &c, int per_sm) { return c.n_sm * per_sm; }
 
-void launch_md(const Ctx &c, const SlotDev &s, cudaStream_t st) {
-  launch_emit(c, s, S_MD, -1, st);
-  k_md_eval<<<persistent_grid(c, 8), 256, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_md_eval");
-  k_md_decide<<<persistent_grid(c, 4), 128, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_md_decide");
-  launch_item_counts(c, s, S_MD, st);
-  launch_scan_items(c, s, S_MD, 0, s.cap_md, st);
-  k_md_fill<<<persistent_grid(c, 4), 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_md_fill");
-  launch_row_offsets(c, s, 0, st);
+void launch_md(const Ctx &c, const Batch &b, cudaStream_t st) {
+  launch_k(c, st, "k_md_eval", k_md_eval, dim3(persistent_grid(c, 8)), 256, 0, false, c.geo, b, c.par);
+  launch_k(c, st, "k_md_decide", k_md_decide, dim3(persistent_grid(c, 4)), 128, 0, false, c.geo, b, c.par);
+  launch_counts(c, b, S_MD, 0, b.s[0].cap_md, false, st);
+  launch_k(c, st, "k_md_fill", k_md_fill, dim3(persistent_grid(c, 4)), 256, 0, false, c.geo, b);
 }
 
-void launch_ls(const Ctx &c, const SlotDev &s, cudaStream_t st) {
-  k_ls_groups<<<(c.geo.n_modules + 7) / 8, 256, 0, st>>>(c.geo, s); LST_MARK(c, st, "k_ls_groups");
-  launch_emit(c, s, S_LS, -1, st);
-  k_ls_eval<<<persistent_grid(c, 8), kThreads, 0, st>>>(c.geo, s, c.par, c.ls_windows); LST_MARK(c, st, "k_ls_eval");
-  k_ls_decide<<<persistent_grid(c, 4), 128, 0, st>>>(s, c.par); LST_MARK(c, st, "k_ls_decide");
-  launch_item_counts(c, s, S_LS, st);
-  launch_scan_items(c, s, S_LS, 1, s.cap_ls, st);
-  k_ls_fill<<<persistent_grid(c, 4), 256, 0, st>>>(s); LST_MARK(c, st, "k_ls_fill");
-  launch_row_offsets(c, s, 1, st);
+void launch_ls(const Ctx &c, const Batch &b, cudaStream_t st) {
+  launch_k(c, st, "k_ls_groups", k_ls_groups, dim3((c.geo.n_modules + kLsGroupWarps - 1) / kLsGroupWarps), 32 * kLsGroupWarps, 0,
+           false, c.geo, b);
+  launch_k(c, st, "k_ls_eval", k_ls_eval, dim3(persistent_grid(c, 8)), kThreads, 0, false, c.geo, b, c.par, c.ls_windows);
+  launch_k(c, st, "k_ls_decide", k_ls_decide, dim3(persistent_grid(c, 4)), 128, 0, false, b, c.par);
+  launch_counts(c, b, S_LS, 1, b.s[0].cap_ls, false, st);
+  launch_k(c, st, "k_ls_fill", k_ls_fill, dim3(persistent_grid(c, 4)), 256, 0, false, b);
 }
 
 }  // namespace lst

@@ -57,6 +57,47 @@ __device__ __forceinline__ bool px_row_window(const Params &g, float4 r1, float4
   return rp + tol >= rlo && rp - tol <= rhi;
 }
 
+// ------------------------------------------------------------------ seed lookups of the cleaning (reading C7)
+// "Seeds a and b share a pixel hit" is looked up through the pixel-hit ids themselves: every id is
+// inserted into a hash set (linear probing; at most half full), and a seed remembers the slots of its
+// 4 ids.  Flags per slot (pid_has5 / pid_has3) then answer "does some seed with a surviving pT5 /
+// pT3 contain this pixel hit" without any seed-to-seed list.
+__device__ __forceinline__ uint32_t pid_hash(uint32_t id) { return (id * 0x9E3779B1u) ^ (id >> 15); }
+__device__ __forceinline__ void pid_insert(const SlotDev &s, uint32_t i) {
+  const uint32_t id = s.seed_ids[i], mask = s.pid_size - 1;
+  const unsigned long long key = (1ull << 32) | id;
+  uint32_t h = pid_hash(id) & mask;
+  for (;;) {
+    const unsigned long long old = atomicCAS(&s.pid_key[h], 0ull, key);
+    if (old == 0ull || old == key) break;
+    h = (h + 1) & mask;
+  }
+  s.pls_slot[i] = h;
+}
+
+// Last block of the seed-preparation kernel: offsets of the per-seed (seed, module) lists and their
+// total (0 + error flag if the rows do not fit), offsets of the eta bins (counted by the seeds' warps).
+__device__ void seed_epilogue(const SlotDev &s) {
+  __shared__ uint32_t sh[33];
+  Header *hdr = s.hdr;
+  const uint32_t n = hdr->n_seeds;
+  block_scan_array(s.px_cnt, s.px_off, n, sh);
+  block_scan_array(s.pls_bin_cnt, s.pls_bin_off, (uint32_t)kEtaBins, sh);
+  if (threadIdx.x == 0) {
+    uint32_t tot = s.px_off[n];
+    if (tot > s.cap_seeds * (uint32_t)kPxCap) { atomicOr(&hdr->err, (uint32_t)ERR_CAP_PIX); tot = 0; }
+    hdr->n_obj[kPairLevel] = tot;
+  }
+}
+
+static inline size_t px_shared_bytes(const Ctx &c) {   // 8 warps x (>= 64 words: the queue of the fill pass)
+  return 8 * std::max<size_t>((size_t)(c.geo.n_start + 31) / 32, 64) * sizeof(uint32_t);
+}
+static inline int px_grid(const Ctx &c, const Batch &b) {
+  int g = (int)((b.s[0].cap_seeds + 7) / 8);
+  return g > c.n_sm * 8 ? c.n_sm * 8 : (g < 1 ? 1 : g);
+}
+
 // One warp per seed.  FILL = false: one bit per (seed, start module): the lanes test the module
 // ROWS (32 at a time); for every compatible row the warp walks the row's modules and keeps those
 // inside the azimuthal window.  FILL = true: expand the bits into the (seed, module) rows at the
@@ -64,17 +105,25 @@ __device__ __forceinline__ bool px_row_window(const Params &g, float4 r1, float4
 // a side - its extrapolation tolerances diverge - so the lists are sized exactly, not capped per
 // seed.)  Dynamic shared memory: 8 warps x nw words of bits.
 template <bool FILL>
-__global__ void __launch_bounds__(256) k_px_modules(GeoDev geo, SlotDev s, Params g) {
+__global__ void __launch_bounds__(256) k_px_modules(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
+                                                     const __grid_constant__ Params g) {
   extern __shared__ uint32_t px_sh[];
+  pdl_enter();
+  LST_SLOT(B);
   const uint32_t n_seeds = s.hdr->n_seeds;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
   const uint32_t nw = (geo.n_start + 31) / 32;
-  if (FILL && s.hdr->n_obj[kPairLevel] == 0) return;
+  const bool have_rows = s.hdr->n_obj[kPairLevel] != 0;      // 0: no compatible module at all, or the rows overflowed
   uint32_t *wbits = px_sh + (size_t)wib * (nw > 64u ? nw : 64u);
   for (uint32_t p = warp; p < n_seeds; p += nwarp) {
     uint32_t *bits = s.px_bits + (size_t)p * nw;
     if (FILL) {
+      if (lane == 0) {      // the seed into its eta bin (the order inside a bin is irrelevant)
+        const int bin = eta_bin(g, (double)s.seed_eta[p]);
+        s.pls_bin_ent[s.pls_bin_off[bin] + atomicAdd(&s.pls_bin_cur[bin], 1u)] = p;
+      }
+      if (!have_rows) continue;
       const float pt = s.seed_pt[p], phi = s.seed_phi[p], z0 = s.seed_z0[p];
       const float kp = -(float)s.seed_q[p] * (float)g.kB / (2.0f * pt);
       const float sh = sinhf(s.seed_eta[p]);
@@ -163,48 +212,26 @@ __global__ void __launch_bounds__(256) k_px_modules(GeoDev geo, SlotDev s, Param
       }
       cnt = warp_sum(cnt);
       if (lane == 0) s.px_cnt[p] = cnt;
+      if (lane < 4) pid_insert(s, 4 * p + lane);
+      if (lane == 4) atomicAdd(&s.pls_bin_cnt[eta_bin(g, (double)s.seed_eta[p])], 1u);
       __syncwarp();
     }
   }
-}
-
-// One block: offsets of the per-seed lists; the row count (0 + error flag if the rows do not fit).
-__global__ void __launch_bounds__(1024) k_px_offsets(SlotDev s) {
-  __shared__ uint32_t sh[33];
-  const uint32_t n_seeds = s.hdr->n_seeds;
-  uint32_t carry = 0;
-  for (uint32_t base = 0; base < n_seeds; base += blockDim.x) {
-    const uint32_t p = base + threadIdx.x;
-    const uint32_t v = p < n_seeds ? s.px_cnt[p] : 0u;
-    uint32_t tot;
-    const uint32_t e = block_excl_scan(v, sh, &tot);
-    if (p < n_seeds) s.px_off[p] = carry + e;
-    carry += tot;
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) {
-    s.px_off[n_seeds] = carry;
-    if (carry > s.cap_seeds * (uint32_t)kPxCap) { atomicOr(&s.hdr->err, (uint32_t)ERR_CAP_PIX); carry = 0; }
-    s.hdr->n_obj[kPairLevel] = carry;
+  if (!FILL) {
+    if (!last_block(&s.hdr->ticket[TK_SEEDS], gridDim.x)) return;
+    seed_epilogue(s);
   }
 }
 
-void launch_pixel(const Ctx &c, const SlotDev &s, cudaStream_t st) {
-  const int warps_per_block = 8;
-  int g = (int)((s.cap_seeds + warps_per_block - 1) / warps_per_block);
-  if (g > c.n_sm * 8) g = c.n_sm * 8;
-  const size_t shb = 8 * std::max<size_t>((size_t)(c.geo.n_start + 31) / 32, 64) * sizeof(uint32_t);   // >= 64 words per warp (queue of the fill pass)
-  if (shb > 48 * 1024) {
-    cudaFuncSetAttribute(k_px_modules<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shb);
-    cudaFuncSetAttribute(k_px_modules<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shb);
-  }
-  k_px_modules<false><<<g, 256, shb, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_px_modules<false>");
-  k_px_offsets<<<1, 1024, 0, st>>>(s); LST_MARK(c, st, "k_px_offsets");
-  k_px_modules<true><<<g, 256, shb, st>>>(c.geo, s, c.par); LST_MARK(c, st, "k_px_modules<true>");
-  launch_join(c, s, 2, st);            // pT5
-  launch_row_offsets(c, s, 4, st);
-  launch_join(c, s, 3, st);            // pT3
-  launch_row_offsets(c, s, 5, st);
+void launch_seed_prep(const Ctx &c, const Batch &b, cudaStream_t st) {
+  const size_t shb = px_shared_bytes(c);
+  if (shb > 48 * 1024) cudaFuncSetAttribute(k_px_modules<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shb);
+  launch_k(c, st, "k_px_modules<false>", k_px_modules<false>, dim3(px_grid(c, b)), 256, shb, false, c.geo, b, c.par);
+}
+void launch_seed_rows(const Ctx &c, const Batch &b, cudaStream_t st) {
+  const size_t shb = px_shared_bytes(c);
+  if (shb > 48 * 1024) cudaFuncSetAttribute(k_px_modules<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shb);
+  launch_k(c, st, "k_px_modules<true>", k_px_modules<true>, dim3(px_grid(c, b)), 256, shb, false, c.geo, b, c.par);
 }
 
 }  // namespace lst

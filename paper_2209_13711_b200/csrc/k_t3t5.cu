@@ -56,37 +56,90 @@ __device__ __forceinline__ void right_range(const SlotDev &s, uint32_t row, uint
   }
 }
 
+// Groups kernel body: one WARP per group (kRowChunk rows), kJoinGroupWarps groups per (virtual) block.
+// Per row: first right object and the number of the group's candidates before the row (row_start,
+// row_cum: the pre-filter kernel stages them, the fill kernel derives the CSR from them).  Per group:
+// its candidate count and work items; first item of every group = exclusive prefix inside the
+// virtual block here, across virtual blocks in the last block to finish.
+constexpr int kJoinGroupWarps = 4;
 template <int KIND>
-__global__ void k_join_groups(SlotDev s) {
+__device__ __forceinline__ void join_groups_body(const SlotDev &s, uint32_t *sh_items, unsigned long long *sh_cand, uint32_t *sh) {
   const int stage = JoinTraits<KIND>::stage;
   const StageBuf &st = s.st[stage];
-  const uint32_t n_rows = s.hdr->n_obj[JoinTraits<KIND>::rows_level];
+  Header *hdr = s.hdr;
+  const uint32_t n_rows = hdr->n_obj[JoinTraits<KIND>::rows_level];
   const uint32_t ng = (n_rows + kRowChunk - 1) / kRowChunk;
-  const int lane = threadIdx.x & 31;
-  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
-  for (uint32_t gidx = warp; gidx < ng; gidx += nwarp) {
-    const uint32_t r0 = gidx * kRowChunk, r1 = min(r0 + kRowChunk, n_rows);
+  const uint32_t nvb = (ng + kJoinGroupWarps - 1) / kJoinGroupWarps;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  for (uint32_t vb = blockIdx.x; vb < nvb; vb += gridDim.x) {
+    const uint32_t gidx = vb * kJoinGroupWarps + wib;
     uint32_t sum = 0;
-    for (uint32_t r = r0 + lane; r < r1; r += 32) {
-      uint32_t a, c;
-      right_range<KIND>(s, r, &a, &c);
-      sum += c;
+    if (gidx < ng) {
+      const uint32_t r0 = gidx * kRowChunk, r1 = min(r0 + kRowChunk, n_rows);
+      for (uint32_t rb = r0; rb < r1; rb += 32) {
+        const uint32_t r = rb + lane;
+        uint32_t a = 0, c = 0;
+        if (r < r1) right_range<KIND>(s, r, &a, &c);
+        uint32_t tot;
+        const uint32_t e = warp_excl_scan(c, &tot);
+        if (r < r1) { st.row_start[r] = a; st.row_cum[r] = sum + e; }
+        sum += tot;
+      }
+      if (lane == 0) { st.gR[gidx] = 1; st.gW[gidx] = sum; }
     }
-    sum = warp_sum(sum);
-    if (lane == 0) { st.gR[gidx] = 1; st.gW[gidx] = sum; }
+    if (lane == 0) { sh_items[wib] = items_of(1u, sum); sh_cand[wib] = sum; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      uint32_t acc = 0;
+      unsigned long long cs = 0;
+      for (int k = 0; k < kJoinGroupWarps; ++k) {
+        const uint32_t g = vb * kJoinGroupWarps + k;
+        if (g < ng) st.g_item0[g] = acc;
+        acc += sh_items[k]; cs += sh_cand[k];
+      }
+      st.gblk[vb] = acc;
+      if (cs) atomicAdd(&hdr->cand[stage], cs);
+    }
+    __syncthreads();
+  }
+  if (!last_block(&hdr->ticket[TK_GROUPS + stage], gridDim.x)) return;
+  const uint32_t total = lb_scan_parts(st.gblk, nvb, sh);
+  lb_add_block_prefix(st.g_item0, ng, st.gblk, kJoinGroupWarps);
+  if (threadIdx.x == 0) {
+    const bool overflow = total > st.cap_items || ng > st.cap_groups;
+    st.g_item0[ng] = total;
+    hdr->n_groups[stage] = ng;
+    hdr->n_items[stage] = overflow ? 0u : total;
+    if (overflow) atomicOr(&hdr->err, (uint32_t)ERR_CAP_ITEMS);
   }
 }
-
 template <int KIND>
-__device__ __forceinline__ void stage_rows(RowTab &rt, const SlotDev &s, uint32_t r0, uint32_t n_rows, uint32_t *sh) {
+__global__ void __launch_bounds__(32 * kJoinGroupWarps) k_join_groups(const __grid_constant__ Batch B) {
+  __shared__ uint32_t sh_items[kJoinGroupWarps];
+  __shared__ unsigned long long sh_cand[kJoinGroupWarps];
+  __shared__ uint32_t sh[33];
+  pdl_enter();
+  LST_SLOT(B);
+  join_groups_body<KIND>(s, sh_items, sh_cand, sh);
+}
+// pT5 (blockIdx.y = 0) and pT3 (1) in one launch
+__global__ void __launch_bounds__(32 * kJoinGroupWarps) k_px_groups(const __grid_constant__ Batch B) {
+  __shared__ uint32_t sh_items[kJoinGroupWarps];
+  __shared__ unsigned long long sh_cand[kJoinGroupWarps];
+  __shared__ uint32_t sh[33];
+  pdl_enter();
+  LST_SLOT(B);
+  if (blockIdx.y == 0) join_groups_body<J_PT5>(s, sh_items, sh_cand, sh);
+  else join_groups_body<J_PT3>(s, sh_items, sh_cand, sh);
+}
+
+// the row table of a group from what the groups kernel stored
+__device__ __forceinline__ void stage_rows(RowTab &rt, const StageBuf &st, uint32_t r0, uint32_t n_rows, uint32_t W) {
   const int tid = threadIdx.x;   // kThreads == kRowChunk
-  uint32_t a = 0, c = 0;
-  if (r0 + tid < n_rows) right_range<KIND>(s, r0 + tid, &a, &c);
-  uint32_t tot;
-  const uint32_t e = block_excl_scan(c, sh, &tot);
-  rt.start[tid] = a;
-  rt.cum[tid] = e;
-  if (tid == 0) rt.cum[kRowChunk] = tot;
+  const bool have = r0 + tid < n_rows;
+  rt.start[tid] = have ? st.row_start[r0 + tid] : 0u;
+  rt.cum[tid] = have ? st.row_cum[r0 + tid] : W;
+  if (tid == 0) rt.cum[kRowChunk] = W;
   __syncthreads();
 }
 // flat candidate -> (row in group, right object)
@@ -213,98 +266,136 @@ __device__ __forceinline__ bool px_candidate(const GeoDev &geo, const SlotDev &s
   return ok;
 }
 
-// per-row seed parameters of the pixel joins: {kappa_p, sinh eta, phi, z0}
-__device__ __forceinline__ void stage_seeds(float4 *rowseed, const SlotDev &s, const Params &g, uint32_t r0,
-                                            uint32_t n_rows) {
+// What a row contributes to every one of its candidates, staged once per group in shared memory
+// (T3: the anchors of the row LS; T5: kappa3 of the row T3 and the anchors of its MDs 2, 3; pixel: the
+// seed parameters {kappa_p, sinh eta, phi, z0} and the seed index).
+struct RowData {
+  float4 ra[kRowChunk], rb[kRowChunk];
+  double2 rk[kRowChunk];
+  uint32_t rc[kRowChunk];            // categories (ca | cb << 2), or the seed index
+};
+template <int KIND>
+__device__ __forceinline__ void stage_rowdata(RowData &rd, const SlotDev &s, const Params &g, uint32_t r0, uint32_t n_rows) {
   const int tid = threadIdx.x;   // kThreads == kRowChunk
-  float4 v = make_float4(0.f, 1.f, 0.f, 0.f);
-  if (r0 + tid < n_rows) {
-    const uint32_t p = s.px_pair[r0 + tid].x;
-    v.x = -(float)s.seed_q[p] * (float)g.kB / (2.0f * s.seed_pt[p]);
-    v.y = sinhf(s.seed_eta[p]);
-    v.z = s.seed_phi[p];
-    v.w = s.seed_z0[p];
+  const uint32_t row = r0 + tid;
+  if (row >= n_rows) return;
+  if (KIND == J_T3) {
+    const uint2 la = s.ls_md[row];
+    rd.ra[tid] = s.md_pos[la.x]; rd.rb[tid] = s.md_pos[la.y];
+    rd.rc[tid] = (s.md_mod[la.x] & 3u) | ((s.md_mod[la.y] & 3u) << 2);
+  } else if (KIND == J_T5) {
+    const uint4 ta = s.t3_md[row];
+    rd.rk[tid] = s.t3_kd[row];
+    rd.ra[tid] = s.md_pos[ta.y]; rd.rb[tid] = s.md_pos[ta.z];
+    rd.rc[tid] = (s.md_mod[ta.y] & 3u) | ((s.md_mod[ta.z] & 3u) << 2);
+  } else {
+    const uint32_t p = s.px_pair[row].x;
+    rd.ra[tid] = make_float4(-(float)s.seed_q[p] * (float)g.kB / (2.0f * s.seed_pt[p]), sinhf(s.seed_eta[p]), s.seed_phi[p], s.seed_z0[p]);
+    rd.rc[tid] = p;
   }
-  rowseed[tid] = v;
 }
 
 // Phase 1 of a join candidate: a cheap necessary condition evaluated on every candidate (T3: the
-// fp32 pre-filter t3_pre_f; T5: the radius match T5-1 on the stored kappa3; pixel: the fp32
-// first-anchor pre-filter).  *ab = the pair handed to the decide kernel.
+// fp32 pre-filter t3_pre_f; T5: the radius match T5-1 on the stored kappa3, then the middle triplet
+// through t3_pre_f; pixel: the fp32 first / last anchor pre-filter).  *ab = the pair handed to the
+// decide kernel.  (Splitting t3_pre_f into a cheap and an expensive part joined by a warp queue was
+// measured and lost: the selective cut is T3-2, the expensive one.)
 template <int KIND>
 __device__ __forceinline__ bool join_phase1(const SlotDev &s, const Params &g, uint32_t row, uint32_t b,
-                                            const float4 *rowseed, int lrow, uint2 *ab) {
+                                            const RowData &rd, int lrow, uint2 *ab) {
   *ab = make_uint2(row, b);
   if (KIND == J_T3) {
-    const uint2 la = s.ls_md[row], lb = s.ls_md[b];
-    const float4 p1 = s.md_pos[la.x], p2 = s.md_pos[la.y], p3 = s.md_pos[lb.y];
-    const int c1 = (int)(s.md_mod[la.x] & 3u), c2 = (int)(s.md_mod[la.y] & 3u), c3 = (int)(s.md_mod[lb.y] & 3u);
-    return t3_pre_f(g, p1.x, p1.y, p1.z, p1.w, c1, p2.x, p2.y, p2.z, p2.w, c2, p3.x, p3.y, p3.z, p3.w, c3);
+    const uint32_t m3 = s.ls_md[b].y;
+    const float4 p1 = rd.ra[lrow], p2 = rd.rb[lrow], p3 = s.md_pos[m3];
+    const uint32_t cc = rd.rc[lrow];
+    return t3_pre_f(g, p1.x, p1.y, p1.z, p1.w, (int)(cc & 3u), p2.x, p2.y, p2.z, p2.w, (int)(cc >> 2), p3.x, p3.y, p3.z, p3.w,
+                    (int)(s.md_mod[m3] & 3u));
   }
   if (KIND == J_T5) {
-    const double2 k3a = s.t3_kd[row], k3b = s.t3_kd[b];
+    const double2 k3a = rd.rk[lrow], k3b = s.t3_kd[b];
     if (!le(fabs(k3a.x - k3b.x), g.ns * (k3a.y + k3b.y))) return false;          // T5-1 (exact, fp64)
     // T5-2: the middle triplet (MD 2, 3, 4) through the fp32 triplet pre-filter
-    const uint4 ta = s.t3_md[row], tb = s.t3_md[b];
-    const float4 p2 = s.md_pos[ta.y], p3 = s.md_pos[ta.z], p4 = s.md_pos[tb.y];
-    const int c2 = (int)(s.md_mod[ta.y] & 3u), c3 = (int)(s.md_mod[ta.z] & 3u), c4 = (int)(s.md_mod[tb.y] & 3u);
-    return t3_pre_f(g, p2.x, p2.y, p2.z, p2.w, c2, p3.x, p3.y, p3.z, p3.w, c3, p4.x, p4.y, p4.z, p4.w, c4);
+    const uint32_t m4 = s.t3_md[b].y;
+    const float4 p2 = rd.ra[lrow], p3 = rd.rb[lrow], p4 = s.md_pos[m4];
+    const uint32_t cc = rd.rc[lrow];
+    return t3_pre_f(g, p2.x, p2.y, p2.z, p2.w, (int)(cc & 3u), p3.x, p3.y, p3.z, p3.w, (int)(cc >> 2), p4.x, p4.y, p4.z, p4.w,
+                    (int)(s.md_mod[m4] & 3u));
   }
-  ab->x = s.px_pair[row].x;     // the seed
-  return px_pre_f<KIND>(s, g, rowseed[lrow], b);
+  ab->x = rd.rc[lrow];          // the seed
+  return px_pre_f<KIND>(s, g, rd.ra[lrow], b);
 }
-
-// Pre-filter kernel: every candidate of every item through phase 1; survivors go to the stage's
-// candidate list.  One barrier-free candidate loop per item after the row table is staged.
+// Pre-filter kernel: every candidate of every group through phase 1; survivors go to the stage's
+// candidate list.  A block takes a group (the pixel stages: a quarter of one, their candidate loops are
+// latency bound and the groups few), stages its row table once and walks its work items (tiles of
+// kItemCand candidates) with one barrier-free candidate loop each.
+struct JoinSh {
+  RowTab rt;
+  RowData rd;
+  ClStageT<64> cl_mem[kThreads / 32];
+};
 template <int KIND>
-__global__ void __launch_bounds__(kThreads) k_join_eval(GeoDev geo, SlotDev s, Params g) {
-  __shared__ RowTab rt;
-  __shared__ uint32_t sh[33];
-  __shared__ float4 rowseed[(KIND == J_PT5 || KIND == J_PT3) ? kRowChunk : 1];
-  __shared__ ClStageT<64> cl_mem[kThreads / 32];
-  (void)geo;
+__device__ __forceinline__ void join_eval_body(const SlotDev &s, const Params &g, JoinSh &m) {
   ClBufT<64> cl;
-  cl.init(&cl_mem[threadIdx.x >> 5]);
+  cl.init(&m.cl_mem[threadIdx.x >> 5]);
   const int stage = JoinTraits<KIND>::stage;
   const StageBuf &st = s.st[stage];
-  const uint32_t n_items = s.hdr->n_items[stage];
+  const bool live = s.hdr->n_items[stage] != 0;            // 0: nothing to do, or the work list overflowed
+  const uint32_t n_groups = live ? s.hdr->n_groups[stage] : 0u;
   const uint32_t n_rows = s.hdr->n_obj[JoinTraits<KIND>::rows_level];
   const int tid = threadIdx.x;
-  // The pixel stages have few items (~700) and a latency-bound candidate loop: an item is split over
-  // kSplit blocks (each stages the rows and takes a quarter of the candidates).
   constexpr uint32_t kSplit = (KIND == J_PT5 || KIND == J_PT3) ? 4u : 1u;
   constexpr int kPart = kItemCand / (int)kSplit;
-  for (uint32_t v = blockIdx.x; v < n_items * kSplit; v += gridDim.x) {
-    const uint32_t it = v / kSplit, part = v % kSplit;
-    const Item item = st.items[it];
-    if (part != 0 && (int)(part * kPart) >= (int)item.nj) continue;      // uniform per block
-    const uint32_t r0 = item.group * kRowChunk;
-    const uint32_t key0 = it * (uint32_t)kItemCand;
-    if (part == 0 && tid < kItemWords) st.mask[(size_t)it * kItemWords + tid] = 0;   // the decide kernel ORs the pass bits in
-    if (KIND == J_PT5 || KIND == J_PT3) stage_seeds(rowseed, s, g, r0, n_rows);
-    stage_rows<KIND>(rt, s, r0, n_rows, sh);
-    stage_hints(rt, item.j0);
-    const int nj = min((int)item.nj, (int)((part + 1) * kPart));
-    for (int base = (int)(part * kPart); base < nj; base += kThreads) {
-      const int c = base + tid;
-      bool keep = false;
-      uint2 ab = make_uint2(0u, 0u);
-      if (c < nj) {
-        int row; uint32_t b;
-        item_to_pair(rt, item.j0, c, &row, &b);
-        keep = join_phase1<KIND>(s, g, r0 + row, b, rowseed, row, &ab);
+  for (uint32_t v = blockIdx.x; v < n_groups * kSplit; v += gridDim.x) {
+    const uint32_t grp = v / kSplit, part = v % kSplit;
+    const uint32_t W = st.gW[grp];
+    if (W == 0 || (part != 0 && W <= part * (uint32_t)kPart)) continue;   // uniform per block
+    const uint32_t r0 = grp * kRowChunk, it0 = st.g_item0[grp];
+    stage_rowdata<KIND>(m.rd, s, g, r0, n_rows);
+    stage_rows(m.rt, st, r0, n_rows, W);
+    for (uint32_t j0 = 0; j0 < W; j0 += kItemCand) {
+      const uint32_t it = it0 + j0 / kItemCand;
+      const int njt = (int)min((uint32_t)kItemCand, W - j0);
+      if (part == 0 && tid < kItemWords) st.mask[(size_t)it * kItemWords + tid] = 0;   // the decide kernel ORs the pass bits in
+      if ((int)(part * kPart) >= njt) continue;
+      stage_hints(m.rt, j0);
+      const uint32_t key0 = it * (uint32_t)kItemCand;
+      const int nj = min(njt, (int)((part + 1) * kPart));
+      for (int base = (int)(part * kPart); base < nj; base += kThreads) {
+        const int c = base + tid;
+        bool keep = false;
+        uint2 ab = make_uint2(0u, 0u);
+        if (c < nj) {
+          int row; uint32_t b;
+          item_to_pair(m.rt, j0, c, &row, &b);
+          keep = join_phase1<KIND>(s, g, r0 + row, b, m.rd, row, &ab);
+        }
+        cl.push(s.hdr, st, stage, keep, key0 + (uint32_t)c, ab);
       }
-      cl.push(s.hdr, st, stage, keep, key0 + (uint32_t)c, ab);
+      __syncthreads();                                       // the hints are rewritten by the next tile
     }
     __syncthreads();
   }
   cl.flush_all(s.hdr, st, stage);
 }
+template <int KIND>
+__global__ void __launch_bounds__(kThreads) k_join_eval(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
+  __shared__ JoinSh m;
+  pdl_enter();
+  LST_SLOT(B);
+  join_eval_body<KIND>(s, g, m);
+}
+__global__ void __launch_bounds__(kThreads) k_px_eval(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
+  __shared__ JoinSh m;
+  pdl_enter();
+  LST_SLOT(B);
+  if (blockIdx.y == 0) join_eval_body<J_PT5>(s, g, m);
+  else join_eval_body<J_PT3>(s, g, m);
+}
 
 // Decide kernel: the fp64 decision of the listed candidates, one thread each (dense warps, no
 // staging); an accepted candidate sets its pass bit and writes its results to the stage's pool.
 template <int KIND>
-__global__ void __launch_bounds__(128) k_join_decide(GeoDev geo, SlotDev s, Params g) {
+__device__ __forceinline__ void join_decide_body(const GeoDev &geo, const SlotDev &s, const Params &g) {
   const int stage = JoinTraits<KIND>::stage;
   const StageBuf &st = s.st[stage];
   Header *hdr = s.hdr;
@@ -338,16 +429,45 @@ __global__ void __launch_bounds__(128) k_join_decide(GeoDev geo, SlotDev s, Para
     if (pass) atomicOr(&st.mask[(size_t)(key / kItemCand) * kItemWords + ((key % kItemCand) >> 5)], 1u << (key & 31u));
   }
 }
-
-// One thread per pool entry: canonical position; constituent indices re-read from the inputs.
 template <int KIND>
-__global__ void __launch_bounds__(256) k_join_fill(SlotDev s) {
+__global__ void __launch_bounds__(128) k_join_decide(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
+                                                      const __grid_constant__ Params g) {
+  pdl_enter();
+  LST_SLOT(B);
+  join_decide_body<KIND>(geo, s, g);
+}
+__global__ void __launch_bounds__(128) k_px_decide(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
+                                                    const __grid_constant__ Params g) {
+  pdl_enter();
+  LST_SLOT(B);
+  if (blockIdx.y == 0) join_decide_body<J_PT5>(geo, s, g);
+  else join_decide_body<J_PT3>(geo, s, g);
+}
+
+// One thread per pool entry: canonical position; constituent indices re-read from the inputs.  Then
+// the level's CSR by first constituent: the objects of index row x (a first MD, or a pixel seed)
+// start at the rank of the first candidate of the first join row that belongs to x.
+template <int KIND>
+__device__ __forceinline__ void join_fill_body(const SlotDev &s) {
   const int stage = JoinTraits<KIND>::stage;
   const StageBuf &st = s.st[stage];
   const Header *hdr = s.hdr;
-  if (hdr->n_obj[JoinTraits<KIND>::out_level] == 0) return;
-  const uint32_t n = min(hdr->cl_used[stage], st.cap_cl);
-  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+  const uint32_t n_out = hdr->n_obj[JoinTraits<KIND>::out_level], n_items = hdr->n_items[stage];
+  const uint32_t n_rows = hdr->n_obj[JoinTraits<KIND>::rows_level];
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nt = gridDim.x * blockDim.x;
+  {
+    const uint32_t n_idx = (KIND == J_T3 || KIND == J_T5) ? hdr->n_obj[0] : hdr->n_seeds;
+    const uint32_t *in_off = KIND == J_T3 ? s.ls_md_off : (KIND == J_T5 ? s.t3_md_off : s.px_off);
+    uint32_t *out_off = KIND == J_T3 ? s.t3_md_off : (KIND == J_T5 ? s.t5_md_off : (KIND == J_PT5 ? s.pt5_pls_off : s.pt3_pls_off));
+    for (uint32_t x = tid; x <= n_idx; x += nt) {
+      const uint32_t a = in_off[x];
+      uint32_t off = n_out;
+      if (a < n_rows && n_items) off = rank_before(st, n_items, n_out, st.g_item0[a / kRowChunk] * (uint32_t)kItemCand + st.row_cum[a]);
+      out_off[x] = off;
+    }
+  }
+  const uint32_t n = n_out ? min(hdr->cl_used[stage], st.cap_cl) : 0u;
+  for (uint32_t j = tid; j < n; j += nt) {
     const uint32_t idx = pool_target(st, st.cl_key[j]);
     if (idx == 0xFFFFFFFFu) continue;
     const uint2 ab = st.cl_ab[j];
@@ -368,44 +488,52 @@ __global__ void __launch_bounds__(256) k_join_fill(SlotDev s) {
       s.t5_etaphi[idx] = st.p_d2[j];
       s.t5_f[idx] = make_float4((float)cr.y, (float)cr.x, (float)s.t3_kd[ab.x].x, (float)s.t3_kd[ab.y].x);
       s.t5_pt[idx] = st.p_f4[j].x;
-    } else if (KIND == J_PT5) {
-      s.pt5_po[idx] = ab; s.pt5_chi2[idx] = st.p_d2[j].x;
     } else {
-      s.pt3_po[idx] = ab; s.pt3_chi2[idx] = st.p_d2[j].x;
+      // S0, same-seed rule (k_dedup.cu): the seed's minimum score, on the bit pattern of the non-negative double
+      const double c2 = st.p_d2[j].x;
+      if (KIND == J_PT5) { s.pt5_po[idx] = ab; s.pt5_chi2[idx] = c2; }
+      else { s.pt3_po[idx] = ab; s.pt3_chi2[idx] = c2; }
+      atomicMin((KIND == J_PT5 ? s.pls_min5 : s.pls_min3) + ab.x, (unsigned long long)__double_as_longlong(c2));
     }
   }
+}
+template <int KIND>
+__global__ void __launch_bounds__(256) k_join_fill(const __grid_constant__ Batch B) {
+  pdl_enter();
+  LST_SLOT(B);
+  join_fill_body<KIND>(s);
+}
+__global__ void __launch_bounds__(256) k_px_fill(const __grid_constant__ Batch B) {
+  pdl_enter();
+  LST_SLOT(B);
+  if (blockIdx.y == 0) join_fill_body<J_PT5>(s);
+  else join_fill_body<J_PT3>(s);
 }
 
 // ------------------------------------------------------------------ launchers
 template <int KIND>
-static void launch_join_t(const Ctx &c, const SlotDev &s, uint32_t row_cap, uint32_t out_cap, cudaStream_t st) {
-  const int gg = (int)((row_cap / kRowChunk + 1 + 3) / 4);   // 4 warps per block, one group per warp
-  k_join_groups<KIND><<<gg < c.n_sm * 8 ? gg : c.n_sm * 8, 128, 0, st>>>(s); LST_MARK(c, st, JoinTraits<KIND>::n_groups);
-  launch_emit(c, s, JoinTraits<KIND>::stage, JoinTraits<KIND>::rows_level, st);
-  k_join_eval<KIND><<<c.n_sm * 16, kThreads, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, JoinTraits<KIND>::n_eval);
-  k_join_decide<KIND><<<c.n_sm * 4, 128, 0, st>>>(c.geo, s, c.par); LST_MARK(c, st, JoinTraits<KIND>::n_decide);
-  launch_item_counts(c, s, JoinTraits<KIND>::stage, st);
-  launch_scan_items(c, s, JoinTraits<KIND>::stage, JoinTraits<KIND>::out_level, out_cap, st);
-  k_join_fill<KIND><<<c.n_sm * 4, 256, 0, st>>>(s); LST_MARK(c, st, JoinTraits<KIND>::n_fill);
+static void launch_join_t(const Ctx &c, const Batch &b, uint32_t row_cap, uint32_t out_cap, cudaStream_t st) {
+  const int gg = (int)((row_cap / kRowChunk + 1 + kJoinGroupWarps - 1) / kJoinGroupWarps);
+  launch_k(c, st, JoinTraits<KIND>::n_groups, k_join_groups<KIND>, dim3(gg < c.n_sm * 8 ? gg : c.n_sm * 8), 32 * kJoinGroupWarps, 0,
+           false, b);
+  launch_k(c, st, JoinTraits<KIND>::n_eval, k_join_eval<KIND>, dim3(c.n_sm * 16), kThreads, 0, false, b, c.par);
+  launch_k(c, st, JoinTraits<KIND>::n_decide, k_join_decide<KIND>, dim3(c.n_sm * 4), 128, 0, false, c.geo, b, c.par);
+  launch_counts(c, b, JoinTraits<KIND>::stage, JoinTraits<KIND>::out_level, out_cap, false, st);
+  launch_k(c, st, JoinTraits<KIND>::n_fill, k_join_fill<KIND>, dim3(c.n_sm * 4), 256, 0, false, b);
 }
 
-void launch_join(const Ctx &c, const SlotDev &s, int kind, cudaStream_t st) {
-  switch (kind) {
-    case J_T3: launch_join_t<J_T3>(c, s, s.cap_ls, s.cap_t3, st); break;
-    case J_T5: launch_join_t<J_T5>(c, s, s.cap_t3, s.cap_t5, st); break;
-    case J_PT5: launch_join_t<J_PT5>(c, s, s.cap_seeds * kPxCap, s.cap_pt5, st); break;
-    default: launch_join_t<J_PT3>(c, s, s.cap_seeds * kPxCap, s.cap_pt3, st); break;
-  }
-}
+void launch_t3(const Ctx &c, const Batch &b, cudaStream_t st) { launch_join_t<J_T3>(c, b, b.s[0].cap_ls, b.s[0].cap_t3, st); }
+void launch_t5(const Ctx &c, const Batch &b, cudaStream_t st) { launch_join_t<J_T5>(c, b, b.s[0].cap_t3, b.s[0].cap_t5, st); }
 
-void launch_t3(const Ctx &c, const SlotDev &s, cudaStream_t st) {
-  launch_join(c, s, J_T3, st);
-  launch_row_offsets(c, s, 2, st);
-}
-
-void launch_t5(const Ctx &c, const SlotDev &s, cudaStream_t st) {
-  launch_join(c, s, J_T5, st);
-  launch_row_offsets(c, s, 3, st);
+// pT5 (blockIdx.y = 0) and pT3 (1): independent of one another, the same five launches serve both
+void launch_pixel_joins(const Ctx &c, const Batch &b, cudaStream_t st) {
+  const uint32_t row_cap = b.s[0].cap_seeds * (uint32_t)kPxCap;
+  const int gg = (int)((row_cap / kRowChunk + 1 + kJoinGroupWarps - 1) / kJoinGroupWarps);
+  launch_k(c, st, "k_px_groups", k_px_groups, dim3(gg < c.n_sm * 4 ? gg : c.n_sm * 4, 2), 32 * kJoinGroupWarps, 0, false, b);
+  launch_k(c, st, "k_px_eval", k_px_eval, dim3(c.n_sm * 8, 2), kThreads, 0, false, b, c.par);
+  launch_k(c, st, "k_px_decide", k_px_decide, dim3(c.n_sm * 2, 2), 128, 0, false, c.geo, b, c.par);
+  launch_counts(c, b, S_PT5, 5, b.s[0].cap_pt5, true, st);
+  launch_k(c, st, "k_px_fill", k_px_fill, dim3(c.n_sm * 2, 2), 256, 0, false, b);
 }
 
 }  // namespace lst

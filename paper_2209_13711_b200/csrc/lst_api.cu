@@ -88,6 +88,8 @@ extern "C" void lst_default_config(lst_config *c) {
   c->cap_t5cand_per_hit = 16.0f;
   c->use_cuda_graph = 1;
   c->enum_pruning = 3;
+  c->use_pdl = 1;
+  c->batch_events = 1;
 }
 
 static void make_params(const lst_config &c, Params *p) {
@@ -226,7 +228,6 @@ struct Slot {
   bool bound = false, loaded = false, ran = false;
   cudaStream_t last_stream = nullptr;
   cudaGraphExec_t graph = nullptr;
-  bool graph_has_seeds = false;
   // pinned host staging for copy_to_host views (allocated on first use)
   uint32_t *h_hits = nullptr, *h_par = nullptr;
   float *h_f = nullptr;
@@ -245,16 +246,22 @@ struct lst_ctx {
   size_t exp_obj_cap = 0, exp_hit_words = 0;
   std::atomic<uint32_t> launches{0};   // kernels of one chain (the same for every slot)
   uint32_t map_edges = 0, map_edges_used = 0;   // module-map edges given / kept for the LS enumeration
+  // the two regions of a workspace that every run resets: [zero_off, zero_off + zero_bytes) to 0 (the
+  // slot header after n_hits / n_seeds, counters, flags, hash set) and [ff_off, + ff_bytes) to 0xFF
+  size_t zero_off = 0, zero_bytes = 0, ff_off = 0, ff_bytes = 0;
+  uint32_t batch = 1;                  // lst_config.batch_events, clamped to [1, kMaxBatch]
+  std::vector<cudaGraphExec_t> group_graph;   // one per group of `batch` consecutive slots
 };
 
 // bump allocator over the workspace; base == nullptr only measures
 struct Carver {
   char *base;
-  size_t off = 0;
+  size_t off = 0, last = 0;      // last: offset of the most recent take
   explicit Carver(void *b) : base((char *)b) {}
   template <class T>
   T *take(size_t n) {
     off = (off + 255) & ~(size_t)255;
+    last = off;
     T *p = base ? (T *)(base + off) : nullptr;
     off += sizeof(T) * (n ? n : 1);
     return p;
@@ -282,13 +289,38 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.cap_pt3 = capf(cf.cap_pt3_per_seed, nsd, 1024);
   s.cap_pt5 = capf(cf.cap_pt5_per_seed, nsd, 1024);
   s.cap_tc = s.cap_pt5 + s.cap_pt3 + s.cap_t5 + nsd;
+  // ---- the zeroed region: header (after n_hits / n_seeds), histogram, incidence counters, flags, hash set
   s.hdr = w.take<Header>(1);
+  const size_t zero_off = w.last + 2 * sizeof(uint32_t);
+  s.det_cnt = w.take<uint32_t>(n_det + 1);
+  s.inc_cnt = w.take<uint32_t>(2 * (3 * (size_t)nh + 1)); s.inc_cur = s.inc_cnt + 3 * (size_t)nh + 1;
+  s.pls_has5 = w.take<uint8_t>(3 * (size_t)nsd);
+  s.pls_has3 = s.pls_has5 + nsd; s.pls_near_t5 = s.pls_has5 + 2 * (size_t)nsd;
+  s.hit_used5 = w.take<uint8_t>(2 * (size_t)nh); s.hit_used3 = s.hit_used5 + nh;
+  s.pid_size = 64;
+  while (s.pid_size < 8 * (size_t)nsd && s.pid_size < (1u << 31)) s.pid_size <<= 1;
+  s.pid_key = w.take<unsigned long long>(s.pid_size);
+  s.pid_has5 = w.take<uint8_t>(2 * (size_t)s.pid_size); s.pid_has3 = s.pid_has5 + s.pid_size;
+  s.scan_part = w.take<uint32_t>(kScanBlocks + 2);
+  s.pls_bin_cnt = w.take<uint32_t>(2 * kEtaBins); s.pls_bin_cur = s.pls_bin_cnt + kEtaBins;
+  const size_t zero_end = (w.off + 255) & ~(size_t)255;
+  // ---- the 0xFF region: per-seed minimum scores and best objects of the same-seed rule
+  s.pls_min5 = w.take<unsigned long long>(3 * (size_t)nsd);      // min5 | min3 | best5, best3
+  const size_t ff_off = w.last;
+  s.pls_min3 = s.pls_min5 + nsd;
+  s.pls_best5 = (uint32_t *)(s.pls_min5 + 2 * (size_t)nsd);
+  s.pls_best3 = s.pls_best5 + nsd;
+  {
+    lst_ctx *mc = const_cast<lst_ctx *>(c);
+    mc->zero_off = zero_off; mc->zero_bytes = zero_end - zero_off;
+    mc->ff_off = ff_off; mc->ff_bytes = 24 * (size_t)nsd;
+  }
   s.raw_x = w.take<float>(nh); s.raw_y = w.take<float>(nh); s.raw_z = w.take<float>(nh);
   s.raw_det = w.take<uint32_t>(nh);
   s.seed_pt = w.take<float>(nsd); s.seed_eta = w.take<float>(nsd); s.seed_phi = w.take<float>(nsd);
   s.seed_z0 = w.take<float>(nsd); s.seed_q = w.take<int8_t>(nsd); s.seed_ids = w.take<uint32_t>(4 * (size_t)nsd);
-  s.det_cnt = w.take<uint32_t>(n_det + 1); s.det_off = w.take<uint32_t>(n_det + 1);
-  s.det_cur = w.take<uint32_t>(n_det + 1);
+  s.det_off = w.take<uint32_t>(n_det + 1);
+  s.tmp_slot = w.take<uint32_t>(nh);
   s.tmp_orig = w.take<uint32_t>(nh);
   s.tmp_key = w.take<float>(nh); s.hit_key = w.take<float>(nh);
   s.hit = w.take<float4>(nh); s.hit_orig = w.take<uint32_t>(nh);
@@ -317,26 +349,14 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.px_rng = w.take<uint2>((size_t)nsd * kPxCap);
   s.pt5_pls_off = w.take<uint32_t>((size_t)nsd + 1); s.pt3_pls_off = w.take<uint32_t>((size_t)nsd + 1);
   s.t5_hits = w.take<uint32_t>(10 * (size_t)s.cap_t5); s.pt3_hits = w.take<uint32_t>(6 * (size_t)s.cap_pt3);
-  s.inc_cnt = w.take<uint32_t>(2 * (3 * (size_t)nh + 1)); s.inc_cur = s.inc_cnt ? s.inc_cnt + 3 * (size_t)nh + 1 : nullptr;
   s.inc_off = w.take<uint32_t>(3 * (size_t)nh + 1);
   s.inc_ent = w.take<uint32_t>(10 * (size_t)s.cap_t5 + 10 * (size_t)s.cap_pt5 + 6 * (size_t)s.cap_pt3);
   s.pls_bin_off = w.take<uint32_t>(kEtaBins + 1); s.pls_bin_ent = w.take<uint32_t>(nsd);
   s.pls_adj_cnt = w.take<uint32_t>(nsd); s.pls_adj = w.take<uint32_t>((size_t)nsd * kAdjCap);
-  s.pid_size = 64;
-  while (s.pid_size < 8 * (size_t)nsd && s.pid_size < (1u << 31)) s.pid_size <<= 1;
-  s.pid_key = w.take<unsigned long long>(s.pid_size);
   s.pls_slot = w.take<uint32_t>(4 * (size_t)nsd);
-  s.pid_has5 = w.take<uint8_t>(2 * (size_t)s.pid_size); s.pid_has3 = s.pid_has5 ? s.pid_has5 + s.pid_size : nullptr;
-  s.pls_min5 = w.take<unsigned long long>(3 * (size_t)nsd);      // min5 | min3 | best5, best3
-  s.pls_min3 = s.pls_min5 ? s.pls_min5 + nsd : nullptr;
-  s.pls_best5 = s.pls_min5 ? (uint32_t *)(s.pls_min5 + 2 * (size_t)nsd) : nullptr;
-  s.pls_best3 = s.pls_best5 ? s.pls_best5 + nsd : nullptr;
-  s.pls_has5 = w.take<uint8_t>(3 * (size_t)nsd);
-  s.pls_has3 = s.pls_has5 ? s.pls_has5 + nsd : nullptr; s.pls_near_t5 = s.pls_has5 ? s.pls_has5 + 2 * (size_t)nsd : nullptr;
-  s.hit_used5 = w.take<uint8_t>(2 * (size_t)nh); s.hit_used3 = s.hit_used5 ? s.hit_used5 + nh : nullptr;
   s.tc_to = w.take<uint2>(s.cap_tc); s.tc_f = w.take<float4>(s.cap_tc);
   s.tc_flag = w.take<uint32_t>((size_t)s.cap_tc + 1); s.tc_pos = w.take<uint32_t>((size_t)s.cap_tc + 1);
-  s.scan_part = w.take<uint32_t>(kScanBlocks + 2);
+  s.flag_blk = w.take<uint32_t>(kFlagBlocks + 1);
   // work lists
   const uint32_t cand_cap[S_NSTAGE] = {
       capf(cf.cap_mdcand_per_hit, nh, 1 << 16), capf(cf.cap_lscand_per_hit, nh, 1 << 16),
@@ -345,15 +365,18 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   const uint32_t pair_groups = (uint32_t)(((size_t)nsd * kPxCap) / kRowChunk + 2);
   const uint32_t grp_cap[S_NSTAGE] = {n_mod, n_mod, s.cap_ls / kRowChunk + 2, s.cap_t3 / kRowChunk + 2,
                                       pair_groups, pair_groups};
+  const uint32_t row_cap[S_NSTAGE] = {0, 0, s.cap_ls, s.cap_t3, nsd * (uint32_t)kPxCap, nsd * (uint32_t)kPxCap};
   for (int k = 0; k < S_NSTAGE; ++k) {
     StageBuf &b = s.st[k];
     b.cap_groups = grp_cap[k];
     b.cap_items = grp_cap[k] + 2 * (cand_cap[k] / kItemCand) + 16;
     b.gR = w.take<uint32_t>(b.cap_groups); b.gW = w.take<uint32_t>(b.cap_groups);
     b.g_item0 = w.take<uint32_t>((size_t)b.cap_groups + 1);
-    b.g_unit0 = w.take<uint32_t>((size_t)b.cap_groups + 1);
-    b.items = w.take<Item>(b.cap_items);
-    b.unit_group = w.take<uint32_t>(b.cap_items);
+    b.gblk = w.take<uint32_t>((size_t)b.cap_groups / 4 + 2);
+    b.item_group = k == S_MD ? w.take<uint32_t>(b.cap_items) : nullptr;
+    b.row_start = row_cap[k] ? w.take<uint32_t>(row_cap[k]) : nullptr;
+    b.row_cum = row_cap[k] ? w.take<uint32_t>(row_cap[k]) : nullptr;
+    b.cblk = w.take<uint32_t>(kCountBlocks + 1);
     b.mask = w.take<uint32_t>((size_t)b.cap_items * kItemWords);
     b.wpre = w.take<uint16_t>((size_t)b.cap_items * kItemWords);
     b.item_cnt = w.take<uint32_t>(b.cap_items); b.item_base = w.take<uint32_t>(b.cap_items);
@@ -463,6 +486,9 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   }
   make_params(c->cfg, &c->k.par);
   c->k.ls_windows = (c->cfg.enum_pruning & 2) != 0;
+  c->k.pdl = c->cfg.use_pdl != 0;
+  if (c->cfg.batch_events < 1 || c->cfg.batch_events > kMaxBatch) { delete c; return einval(); }
+  c->batch = (uint32_t)c->cfg.batch_events;
   c->n_slots = n_slots; c->max_hits = max_hits; c->max_seeds = max_seeds;
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
@@ -577,6 +603,7 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   c->k.geo.start_mods = (const uint32_t *)(d + o_start);
   c->k.geo.n_start = (uint32_t)start_mods.size();
   c->slots.resize(n_slots);
+  c->group_graph.assign((n_slots + c->batch - 1) / c->batch, nullptr);
   {
     // candidate keys (item * 1024 + candidate), list positions and the TC index are 32-bit
     SlotDev probe;
@@ -606,13 +633,14 @@ extern "C" void lst_destroy(lst_ctx *c) {
   if (!c) return;
   cudaDeviceSynchronize();
   for (Slot &s : c->slots) free_slot_host(s);
+  for (cudaGraphExec_t g : c->group_graph) if (g) cudaGraphExecDestroy(g);
   if (c->d_static) cudaFree(c->d_static);
   delete c;
 }
 
 extern "C" size_t lst_workspace_bytes(const lst_ctx *c) { return c ? c->ws_bytes : 0; }
 
-static int capture_slot_graph(lst_ctx *c, Slot &s);
+static int capture_graph(lst_ctx *c, uint32_t slot0, uint32_t n, cudaGraphExec_t *out);
 
 extern "C" int lst_bind_workspace(lst_ctx *c, uint32_t slot, void *workspace, size_t bytes) {
   if (!c || slot >= c->n_slots || !workspace || ((uintptr_t)workspace & 255)) return einval();
@@ -626,8 +654,14 @@ extern "C" int lst_bind_workspace(lst_ctx *c, uint32_t slot, void *workspace, si
   s.workspace = workspace; s.ws_bytes = bytes;
   s.bound = true; s.loaded = false; s.ran = false;
   if (!s.h_hdr) CU(cudaMallocHost((void **)&s.h_hdr, sizeof(Header)));
-  if (c->cfg.use_cuda_graph) return capture_slot_graph(c, s);
-  return LST_OK;
+  if (!c->cfg.use_cuda_graph) return LST_OK;
+  int rc = capture_graph(c, slot, 1, &s.graph);
+  if (rc != LST_OK || c->batch == 1) return rc;
+  // the graph of the slot's group (lst_run_batch), once every slot of the group has a workspace
+  const uint32_t grp = slot / c->batch, s0 = grp * c->batch, s1 = std::min(c->n_slots, s0 + c->batch);
+  if (c->group_graph[grp]) { cudaGraphExecDestroy(c->group_graph[grp]); c->group_graph[grp] = nullptr; }
+  for (uint32_t k = s0; k < s1; ++k) if (!c->slots[k].bound) return LST_OK;
+  return capture_graph(c, s0, s1 - s0, &c->group_graph[grp]);
 }
 
 // ------------------------------------------------------------------ a0 upload
@@ -670,37 +704,52 @@ extern "C" int lst_load_event(lst_ctx *c, uint32_t slot, const lst_hits *hits, c
 }
 
 // ------------------------------------------------------------------ the chain
-// Enqueue a0 .. a6 of one slot on `st`; rec (may be NULL) counts / times the kernels.
-static int enqueue_chain(const lst_ctx *c, const SlotDev &d, cudaStream_t st, Recorder *rec) {
+// Enqueue a0 .. a6 of the slots [slot0, slot0 + n) on `st` as ONE chain of launches (gridDim.z = n);
+// rec (may be NULL) counts / times the kernels.  Two memsets reset what a run accumulates into, then
+// 39 kernels; with `pdl` every kernel but the first is launched with programmatic stream serialisation.
+static int enqueue_chain(const lst_ctx *c, uint32_t slot0, uint32_t n, cudaStream_t st, Recorder *rec, bool pdl) {
   Recorder count_only;
   Ctx k = c->k;                    // a private copy: the recorder pointer is per call, not per context
   k.rec = rec ? rec : &count_only;
-  launch_index(k, d, st);
-  launch_md(k, d, st);
-  launch_ls(k, d, st);
-  launch_t3(k, d, st);
-  launch_t5(k, d, st);
-  launch_pixel(k, d, st);
-  launch_dedup(k, d, st);
+  k.pdl = pdl && c->k.pdl;
+  k.nb = (int)n;
+  Batch b;
+  memset(&b, 0, sizeof(b));
+  for (uint32_t e = 0; e < n; ++e) {
+    const Slot &sl = c->slots[slot0 + e];
+    b.s[e] = sl.dev;
+    cudaMemsetAsync((char *)sl.workspace + c->zero_off, 0, c->zero_bytes, st);
+    cudaMemsetAsync((char *)sl.workspace + c->ff_off, 0xFF, c->ff_bytes, st);
+  }
+  launch_index(k, b, st);
+  launch_seed_prep(k, b, st);
+  launch_md(k, b, st);
+  launch_ls(k, b, st);
+  launch_t3(k, b, st);
+  launch_t5(k, b, st);
+  launch_seed_rows(k, b, st);
+  launch_pixel_joins(k, b, st);
+  launch_dedup(k, b, st);
   return k.rec->n;
 }
 
-// One CUDA graph per slot, captured when the workspace is bound (lst_run then only replays it: no
-// allocation, no capture, nothing shared between slots is written).
-static int capture_slot_graph(lst_ctx *c, Slot &s) {
+// One CUDA graph per slot (and one per group of lst_config.batch_events slots), captured when the
+// workspace is bound (lst_run then only replays it: no allocation, no capture, nothing shared between
+// slots is written).
+static int capture_graph(lst_ctx *c, uint32_t slot0, uint32_t n, cudaGraphExec_t *out) {
   cudaGraph_t gr = nullptr;
   cudaStream_t cap = nullptr;
   CU(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));      // the legacy default stream cannot be captured
   cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
   if (e != cudaSuccess) { cudaStreamDestroy(cap); return cuda_fail(e, "cudaStreamBeginCapture"); }
-  const int n = enqueue_chain(c, s.dev, cap, nullptr);
+  const int nk = enqueue_chain(c, slot0, n, cap, nullptr, true);
   e = cudaStreamEndCapture(cap, &gr);
   cudaStreamDestroy(cap);
   if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
-  e = cudaGraphInstantiate(&s.graph, gr, 0);
+  e = cudaGraphInstantiate(out, gr, 0);
   cudaGraphDestroy(gr);
-  if (e != cudaSuccess) { s.graph = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
-  c->launches.store((uint32_t)n);
+  if (e != cudaSuccess) { *out = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
+  c->launches.store((uint32_t)nk);
   return LST_OK;
 }
 
@@ -712,12 +761,31 @@ extern "C" int lst_run(lst_ctx *c, uint32_t slot, void *cuda_stream) {
   if (s.graph) {
     CU(cudaGraphLaunch(s.graph, st));
   } else {
-    c->launches.store((uint32_t)enqueue_chain(c, s.dev, st, nullptr));
+    c->launches.store((uint32_t)enqueue_chain(c, slot, 1, st, nullptr, true));
     CU(cudaGetLastError());
   }
   s.ran = true; s.last_stream = st;
   return LST_OK;
 }
+
+extern "C" int lst_run_batch(lst_ctx *c, uint32_t group, void *cuda_stream) {
+  if (!c || (uint64_t)group * c->batch >= c->n_slots) return einval();
+  const uint32_t s0 = group * c->batch, s1 = std::min(c->n_slots, s0 + c->batch);
+  for (uint32_t k = s0; k < s1; ++k)
+    if (!c->slots[k].bound || !c->slots[k].loaded) return LST_ESTATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaGraphExec_t g = c->batch == 1 ? c->slots[s0].graph : c->group_graph[group];
+  if (g) {
+    CU(cudaGraphLaunch(g, st));
+  } else {
+    c->launches.store((uint32_t)enqueue_chain(c, s0, s1 - s0, st, nullptr, true));
+    CU(cudaGetLastError());
+  }
+  for (uint32_t k = s0; k < s1; ++k) { c->slots[k].ran = true; c->slots[k].last_stream = st; }
+  return LST_OK;
+}
+
+extern "C" uint32_t lst_batch_events(const lst_ctx *c) { return c ? c->batch : 0; }
 
 // ------------------------------------------------------------------ results
 static int sync_header(lst_ctx *c, Slot &s) {
@@ -814,7 +882,7 @@ extern "C" int lst_run_timed(lst_ctx *c, uint32_t slot, void *cuda_stream, uint3
   r.timed = true;
   r.n = 0;
   CU(cudaEventRecord(r.ev[0], st));
-  c->launches.store((uint32_t)enqueue_chain(c, s.dev, st, &r));
+  c->launches.store((uint32_t)enqueue_chain(c, slot, 1, st, &r, false));
   CU(cudaGetLastError());
   s.ran = true; s.last_stream = st;
   CU(cudaStreamSynchronize(st));

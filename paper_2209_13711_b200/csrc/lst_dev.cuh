@@ -1,19 +1,23 @@
 // lst_dev.cuh -- device-side data layout and the work-item machinery shared by all stage kernels.
 //
 // Every stage (MD, LS, T3, T5, pT5, pT3) is a join: rows x per-row candidate lists, grouped so
-// that one group's operands fit in shared memory.  A stage runs as
-//   groups  : per group g, rows R_g and candidates per row (uniform W_g, or a per-row list)
-//   emit    : one block scans the groups (exact offsets), a multi-block kernel writes the
-//             fixed-size work ITEMS (<= 1024 candidates) and work UNITS
+// that one group's operands fit in shared memory.  A stage is FIVE launches:
+//   groups  : per group g, rows R_g and candidates per row (uniform W_g, or a per-row list); the
+//             group's candidates are cut into work ITEMS of <= 1024 candidates (one pass bit each);
+//             the last block to finish scans the per-block item counts (first item of every group)
 //   eval    : fp32 pre-filter on every candidate; the survivors (item, candidate, pair) are
 //             appended to the stage's candidate list through warp-private staging
 //   decide  : one thread per listed candidate: fp64 decision, pass BIT of the candidate, the
 //             computed quantities into the pool at the candidate's list index
-//   counts  : per-item pass counts and word prefixes from the pass bits
-//   scan    : one block scans the per-item pass counts (exact sizes, no truncation)
-//   fill    : one thread per listed candidate: the accepted ones move to item_base + bit rank
+//   counts  : per-item pass counts and word prefixes from the pass bits; per-block sums, the last
+//             block to finish scans them (exact sizes, no truncation)
+//   fill    : one thread per listed candidate: the accepted ones move to item_base + bit rank; the
+//             same kernel derives the level's CSR by first constituent from the ranks
 // Output order is canonical (ascending item, ascending candidate) whatever order the list was
 // appended in; warp ballots / prefix sums do the compaction, the atomics only order scratch lists.
+// Every kernel takes a BATCH of slots (events) and picks its own with blockIdx.z: one chain of
+// launches serves up to kMaxBatch events, and every kernel starts with
+// griddepcontrol.wait so that the chain can be launched with programmatic dependent launch.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -25,15 +29,17 @@ namespace lst {
 constexpr int kItemCand = 1024;          // candidates per work item
 constexpr int kItemWords = kItemCand / 32;
 constexpr int kThreads = 128;            // threads per block of eval / fill kernels
-constexpr int kUnitItems = 16;           // max items per work unit (same group, same column tile, consecutive rows)
 constexpr int kMaxRpi = 128;             // max rows per item
-constexpr int kUnitRows = 128;           // max rows per work unit
+constexpr int kMaxBatch = 8;             // events (slots) one chain of launches can serve
 constexpr int kRowChunk = 128;           // rows per group in the variable-width stages (T3, T5, pixel)
 constexpr int kMaxDeg = 512;             // maximum module-map degree (checked by lst_create)
 constexpr int kPxCap = 64;               // (seed, start module) rows per pixel seed ON AVERAGE (overflow -> LST_ENOMEM)
 constexpr int kAdjCap = 32;              // related pixel seeds per pixel seed (overflow -> LST_ENOMEM)
 constexpr int kEtaBins = 2048;           // eta bins of the pixel-seed lookup used by the cleaning
 constexpr int kScanBlocks = 128;         // blocks of the two-pass device-wide scan
+constexpr int kCountBlocks = 148;        // blocks of k_counts (per-item pass counts + two-level scan)
+constexpr int kCountThreads = 512;
+constexpr int kFlagBlocks = 592;         // blocks of k_s3_flags / k_tc_fill
 constexpr int kScanThreads = 512;
 constexpr int kPairLevel = 7;            // Header::n_obj slot that holds the (seed, module) pair count
 
@@ -61,31 +67,28 @@ __host__ __device__ __forceinline__ uint32_t item_rpi(uint32_t W) {
 __host__ __device__ __forceinline__ uint32_t item_nct(uint32_t W) {
   return W <= (uint32_t)kItemCand ? 1u : (W + kItemCand - 1) / kItemCand;
 }
-__host__ __device__ __forceinline__ uint32_t unit_items(uint32_t W) {
-  const uint32_t k = (uint32_t)kUnitRows / item_rpi(W);
-  return k < 1u ? 1u : (k > (uint32_t)kUnitItems ? (uint32_t)kUnitItems : k);
+// items of a group with R rows and W columns
+__host__ __device__ __forceinline__ uint32_t items_of(uint32_t R, uint32_t W) {
+  if (R == 0 || W == 0) return 0;
+  const uint32_t rpi = item_rpi(W);
+  return ((R + rpi - 1) / rpi) * item_nct(W);
 }
 
-struct Item {            // 16 bytes
-  uint32_t group;        // module (MD, LS) or row chunk (T3, T5, pixel)
-  uint32_t i0;           // first row (relative to the group's first row)
-  uint32_t j0;           // first candidate column
-  uint16_t nrows, nj;    // nrows * nj <= kItemCand
-};
+// "last block" tickets of the kernels whose final block runs a small serial epilogue
+enum Ticket { TK_HIST = 0, TK_GROUPS = 1 /* + stage */, TK_COUNTS = 7 /* + stage */, TK_SEEDS = 13, TK_FLAGS = 14, TK_N = 16 };
 
-struct Header {          // per slot, device; zeroed (except n_hits / n_seeds) at the start of lst_run
+struct Header {          // per slot, device; everything after n_seeds is zeroed at the start of lst_run
   uint32_t n_hits, n_seeds;
   uint32_t n_obj[8];                 // indexed by lst_level; [kPairLevel] = (seed, module) pairs
   uint32_t n_items[S_NSTAGE];
   uint32_t n_groups[S_NSTAGE];
-  uint32_t n_units[S_NSTAGE];        // work units (k_emit_items): item runs that share their columns
-  uint32_t next_unit[S_NSTAGE];      // dynamic work distribution: next unit to hand out
+  uint32_t next_unit[S_NSTAGE];      // dynamic work distribution: next row block to hand out
   uint32_t cl_used[S_NSTAGE];        // pre-filter survivors appended to the stage's candidate list
   uint32_t err;
-  uint32_t n_dd;                     // T5 + pT5 + pT3 objects entering the cleaning
-  uint32_t n_flag;                   // pT5 + pT3 + T5 + seeds: length of the TC keep-flag array
   uint32_t n_inc;                    // 3 * n_hits: rows of the (hit, object type) -> objects incidence
   uint32_t n_heavy;                  // objects k_s0 handed to k_s0_heavy (listed in tc_pos, free until S3)
+  uint32_t flag_chunk;               // keep flags per block of k_s3_flags / k_tc_fill
+  uint32_t ticket[TK_N];             // blocks that finished (last_block)
   unsigned long long cand[S_NSTAGE]; // candidates of the method's definition per stage (rows x connected columns)
   unsigned long long cand_eval[S_NSTAGE];   // candidates the stage's pre-filter kernel actually evaluated
 };
@@ -93,9 +96,10 @@ struct Header {          // per slot, device; zeroed (except n_hits / n_seeds) a
 struct StageBuf {        // work list of one stage
   uint32_t *gR, *gW;     // [cap_groups] rows / width (or candidate count) per group
   uint32_t *g_item0;     // [cap_groups+1] first item of a group
-  uint32_t *g_unit0;     // [cap_groups+1] first work unit of a group
-  Item *items;           // [cap_items]
-  uint32_t *unit_group;  // [cap_items] group of a work unit
+  uint32_t *gblk;        // [cap_groups / groups per block + 2] items of the groups of one block of the groups kernel
+  uint32_t *item_group;  // [cap_items] group of an item (MD only: the module)
+  uint32_t *row_start, *row_cum;   // [cap_rows] joins: first right object of a row / candidates of the group before the row
+  uint32_t *cblk;        // [kCountBlocks + 1] pass counts of the items of one block of k_counts
   uint32_t *mask;        // [cap_items * kItemWords]
   uint16_t *wpre;        // [cap_items * kItemWords] pass count of the item's words before this one
   uint32_t *item_cnt;    // [cap_items] pass count
@@ -152,7 +156,8 @@ struct SlotDev {
   float *raw_x, *raw_y, *raw_z; uint32_t *raw_det;
   float *seed_pt, *seed_eta, *seed_phi, *seed_z0; int8_t *seed_q; uint32_t *seed_ids;
   // a0: hits grouped by det
-  uint32_t *det_cnt, *det_off, *det_cur;     // [n_det+1]
+  uint32_t *det_cnt, *det_off;               // [n_det+1]
+  uint32_t *tmp_slot;                        // [cap_hits] arrival rank of a hit inside its det (k_hist)
   uint32_t *tmp_orig;                        // [cap_hits]
   float *tmp_key, *hit_key;                  // [cap_hits] azimuth relative to the module centre (sort key inside a det)
   float4 *hit;                               // [cap_hits] x, y, z, rt
@@ -203,6 +208,7 @@ struct SlotDev {
   uint32_t *inc_cnt, *inc_cur;     // [3 cap_hits+1] each, contiguous: (hit, type) -> objects incidence, row 3 h + type
   uint32_t *inc_off;               // [3 cap_hits+1]
   uint32_t *inc_ent;               // [10 cap_t5 + 10 cap_pt5 + 6 cap_pt3] object ids (T5 | pT5 | pT3)
+  uint32_t *pls_bin_cnt, *pls_bin_cur;   // [kEtaBins] each (zeroed per run): seeds per eta bin, fill cursor
   uint32_t *pls_bin_off;           // [kEtaBins+1]
   uint32_t *pls_bin_ent;           // [cap_seeds]
   uint32_t *pls_adj_cnt, *pls_adj; // [cap_seeds], [cap_seeds * kAdjCap]: seeds close in eta-phi to a seed
@@ -217,7 +223,8 @@ struct SlotDev {
   uint32_t *pls_best5, *pls_best3;              // [cap_seeds] the seed's best pT5 / pT3 (index in its collection), or ~0
                                                 // (the four arrays are contiguous: one memset)
   uint8_t *hit_used5, *hit_used3;  // [cap_hits] each, contiguous: hit belongs to a surviving pT5 / pT3 (S1, S2)
-  uint32_t *tc_flag, *tc_pos;      // [cap_tc+1]
+  uint32_t *tc_flag, *tc_pos;      // [cap_tc+1] keep flags in TC order; tc_pos: the objects k_s0 hands to k_s0_heavy
+  uint32_t *flag_blk;              // [kFlagBlocks+1] kept flags per block of k_s3_flags, then their exclusive prefix
   uint32_t *scan_part;             // [kScanBlocks+2]: block partials, total; last word = ticket
   // TC
   uint2 *tc_to;                    // type, obj
@@ -228,6 +235,26 @@ struct SlotDev {
   // export scratch
   uint32_t *exp_hits, *exp_par; float *exp_f;
 };
+
+// The slots (events) one chain of launches serves: a kernel's blocks with blockIdx.z = e work on
+// slot s[e].  Passed by value as a __grid_constant__ kernel parameter (CUDA >= 12.1 allows 32 KB).
+struct Batch {
+  SlotDev s[kMaxBatch];
+};
+#define LST_SLOT(B) const SlotDev &s = (B).s[blockIdx.z]
+
+// ------------------------------------------------------------------ programmatic dependent launch
+// Every kernel of the chain calls pdl_enter() before it touches memory: griddepcontrol.wait blocks
+// until the preceding kernel of the stream has completed and its writes are visible (a no-op when
+// the kernel was launched without the programmatic-serialisation attribute).  No kernel triggers its
+// dependents early (griddepcontrol.launch_dependents): a dependent's blocks would take SM slots from
+// blocks of this kernel that have not started yet (measured: slower); the implicit trigger at block
+// exit lets the next kernel's launch overlap this kernel's tail and its memory flush.
+__device__ __forceinline__ void pdl_enter() {
+#if defined(__CUDA_ARCH__)
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+}
 
 // ------------------------------------------------------------------ small device helpers
 __device__ __forceinline__ uint32_t warp_sum(uint32_t v) {
@@ -265,6 +292,118 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t *sh, ui
   e += sh[w];
   *total = sh[32];
   return e;
+}
+
+// "Last block" epilogue: every block calls this after its last global write; exactly one block
+// (the last to arrive) gets true, after which it sees the writes of all the others (read them with
+// __ldcg: L1 is not coherent).  ticket: a zeroed word of the slot header; nblocks = blocks that call.
+__device__ __forceinline__ bool last_block(uint32_t *ticket, uint32_t nblocks) {
+  __shared__ bool lb_last;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) lb_last = atomicAdd(ticket, 1u) == nblocks - 1u;
+  __syncthreads();
+  const bool l = lb_last;
+  if (l) __threadfence();
+  return l;
+}
+
+// Last-block scan used by the groups kernels and k_counts: exclusive scan of part[0 .. n) in place
+// (n <= a few thousand), total returned to every thread.  sh: 33 words.
+__device__ __forceinline__ uint32_t lb_scan_parts(uint32_t *part, uint32_t n, uint32_t *sh) {
+  const uint32_t chunk = (n + blockDim.x - 1) / blockDim.x;
+  const uint32_t b0 = min(n, threadIdx.x * chunk), b1 = min(n, b0 + chunk);
+  uint32_t sum = 0;
+  for (uint32_t i = b0; i < b1; ++i) sum += __ldcg(&part[i]);
+  uint32_t tot;
+  uint32_t run = block_excl_scan(sum, sh, &tot);
+  for (uint32_t i = b0; i < b1; ++i) { const uint32_t v = __ldcg(&part[i]); part[i] = run; run += v; }
+  __syncthreads();
+  return tot;
+}
+
+// Exclusive scan of in[0..n) into out[0..n], out[n] = total; one block, in and out 16-byte aligned.
+// Coalesced: per round thread t owns the four elements 4 (round * blockDim.x + t) .. + 3 (one uint4
+// load, one block scan, one uint4 store).  The input was written by other blocks of the same kernel
+// (last-block epilogue): read through L2.
+__device__ __forceinline__ void block_scan_array(const uint32_t *in, uint32_t *out, uint32_t n, uint32_t *sh) {
+  uint32_t carry = 0;
+  for (uint32_t base = 0; base < n; base += 4 * blockDim.x) {
+    const uint32_t i = base + 4 * threadIdx.x;
+    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+    if (i + 3 < n) v = __ldcg(reinterpret_cast<const uint4 *>(in + i));
+    else {
+      if (i < n) v.x = __ldcg(&in[i]);
+      if (i + 1 < n) v.y = __ldcg(&in[i + 1]);
+      if (i + 2 < n) v.z = __ldcg(&in[i + 2]);
+    }
+    uint32_t tot;
+    const uint32_t e = carry + block_excl_scan(v.x + v.y + v.z + v.w, sh, &tot);
+    const uint4 o = make_uint4(e, e + v.x, e + v.x + v.y, e + v.x + v.y + v.z);
+    if (i + 3 < n) *reinterpret_cast<uint4 *>(out + i) = o;
+    else {
+      if (i < n) out[i] = o.x;
+      if (i + 1 < n) out[i + 1] = o.y;
+      if (i + 2 < n) out[i + 2] = o.z;
+    }
+    carry += tot;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[n] = carry;
+}
+
+// Last-block epilogue of the two-level scans: arr[i] += blk[i / per_block] for i < n (arr holds the
+// exclusive prefix inside its block, blk the exclusive prefix of the block sums).  Four independent
+// loads in flight per thread (the values come from other blocks: read through L2).
+__device__ __forceinline__ void lb_add_block_prefix(uint32_t *arr, uint32_t n, const uint32_t *blk, uint32_t per_block) {
+  if (per_block == 0) return;
+  const uint32_t T = blockDim.x;
+  for (uint32_t base = threadIdx.x; base < n; base += 4 * T) {
+    uint32_t v[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { const uint32_t i = base + k * T; v[k] = i < n ? __ldcg(&arr[i]) + blk[i / per_block] : 0u; }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { const uint32_t i = base + k * T; if (i < n) arr[i] = v[k]; }
+  }
+}
+
+// eta bins of the pixel seeds ("close in eta-phi" lookups of the cleaning, reading C7)
+__device__ __forceinline__ int eta_bin(const Params &g, double eta) {
+  const double t = (eta + 4.0) * g.eta_bin_inv;
+  if (!(t >= 0.0)) return 0;
+  return t < (double)g.eta_nbins ? (int)t : g.eta_nbins - 1;
+}
+__device__ __forceinline__ bool close_eta_phi(const Params &g, double e1, double p1, double e2, double p2) {
+  const double de = e1 - e2;
+  if (fabs(de) > g.dr_eta_pre) return false;
+  const double dp = wrap_pi(p1 - p2);
+  return de * de + dp * dp < g.dr2max;
+}
+
+// One warp: the seeds b != a close to seed a in eta-phi, found through the eta bins (a close seed
+// lies in a's bin or a neighbouring one: the bin width exceeds sqrt(dr2max)).
+__device__ __forceinline__ void pls_adjacent(const SlotDev &s, const Params &g, uint32_t a) {
+  const int lane = threadIdx.x & 31;
+  const double ea = (double)s.seed_eta[a], pa = (double)s.seed_phi[a];
+  const int b0 = eta_bin(g, ea);
+  const int lo = b0 > 0 ? b0 - 1 : 0, hi = b0 + 1 < g.eta_nbins ? b0 + 1 : g.eta_nbins - 1;
+  const uint32_t e0 = s.pls_bin_off[lo], e1 = s.pls_bin_off[hi + 1];
+  uint32_t cnt = 0;
+  for (uint32_t eb = e0; eb < e1; eb += 32) {
+    const uint32_t e = eb + lane;
+    uint32_t b = 0;
+    bool close = false;
+    if (e < e1) {
+      b = s.pls_bin_ent[e];
+      close = b != a && close_eta_phi(g, ea, pa, (double)s.seed_eta[b], (double)s.seed_phi[b]);
+    }
+    const uint32_t bal = __ballot_sync(0xffffffffu, close);
+    const uint32_t pos = cnt + __popc(bal & ((1u << lane) - 1u));
+    if (close && pos < (uint32_t)kAdjCap) s.pls_adj[(size_t)a * kAdjCap + pos] = b;
+    cnt += __popc(bal);
+  }
+  if (cnt > (uint32_t)kAdjCap) { if (lane == 0) atomicOr(&s.hdr->err, (uint32_t)ERR_CAP_PIX); cnt = 0; }
+  if (lane == 0) s.pls_adj_cnt[a] = cnt;
 }
 
 // Warp-private ring queue (64 entries in shared memory; head / count are warp-uniform registers).
@@ -385,6 +524,16 @@ struct ClBufT {
 };
 typedef ClStageT<32> ClStage;
 typedef ClBufT<32> ClBuf;
+
+// Number of accepted candidates with a key below `key` (= item * kItemCand + candidate): the canonical
+// index at which the objects of a row start, given the key of the row's first candidate.  The masks
+// are cleared item by item (all 32 words), so a key past the item's last candidate is fine.
+__device__ __forceinline__ uint32_t rank_before(const StageBuf &st, uint32_t n_items, uint32_t n_total, uint32_t key) {
+  const uint32_t it = key / (uint32_t)kItemCand, c = key % (uint32_t)kItemCand;
+  if (it >= n_items) return n_total;
+  const size_t w = (size_t)it * kItemWords + (c >> 5);
+  return st.item_base[it] + st.wpre[w] + __popc(st.mask[w] & ((1u << (c & 31)) - 1u));
+}
 
 // fill: canonical index of listed candidate `key` = item * kItemCand + candidate, or 0xFFFFFFFF if
 // the decide kernel did not accept it (its pass bit is clear)

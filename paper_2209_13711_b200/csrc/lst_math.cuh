@@ -337,7 +337,9 @@ LST_HD bool ls_row_window(const Params &g, float ri, float zi, int ci, float rlo
     const float cmin = rlo - ri;
     if (cmin > 1.0f) {
       const float k = (g.f_kmax + LST_FDIV(tol, cmin)) * 1.002f;
-      if (k * rhi <= 0.6f) w = (asinf(k * rhi) - asinf(k * ri)) * 1.002f + 2e-4f;              // L2, mode R
+      // asin(b) - asin(a) = integral of 1 / sqrt(1 - x^2) over [a, b] <= (b - a) / sqrt(1 - b^2)
+      const float bq = k * rhi;
+      if (bq <= 0.6f) w = LST_FDIV(bq - k * ri, sqrtf(1.0f - bq * bq)) * 1.002f + 2e-4f;             // L2, mode R
     }
   } else {
     const float azo0 = (zlo <= 0.0f && zhi >= 0.0f) ? 0.0f : fminf(fabsf(zlo), fabsf(zhi));
@@ -345,7 +347,7 @@ LST_HD bool ls_row_window(const Params &g, float ri, float zi, int ci, float rlo
     const float den = 0.5f * (fabsf(zi) + azo0) - g.f_z0max - 0.5f * ns * g.f_sig_z[ci];
     if (den > 1.0f) {
       const float x = fminf(1.0f, g.f_kmax * (0.5f * (ri + rhi) + 0.5f * ns * (g.f_sig_r[ci] + g.f_sig_r[cB])));
-      w = (LST_FDIV((dzmax + ns * g.f_sig_z[ci]) * asinf(x), den) + tol) * 1.002f + 2e-4f;     // L2, mode Z
+      w = (LST_FDIV((dzmax + ns * g.f_sig_z[ci]) * (x + 0.5708f * x * x * x), den) + tol) * 1.002f + 2e-4f;   // L2, mode Z: asin(x) <= x + (pi/2 - 1) x^3
     }
   }
   *W = w;

@@ -711,3 +711,59 @@ def test_config4h_all_seeds_bench_configuration_sampled(B, geom_full, map_full):
     assert near <= 3
     assert cnt[O.TC] > 1000
     lst.close()
+
+
+@pytest.mark.parametrize("batch,pdl,graph", [(4, 1, 1), (3, 0, 1), (8, 1, 0)])
+def test_batched_chain_equals_single_slot_runs(B, geom_full, map_full, batch, pdl, graph):
+    """lst_run_batch runs a group of `batch_events` slots as ONE chain of launches
+    (grid over (event, work)); with or without programmatic dependent launch and CUDA graphs, every
+    level of every event is bit-identical (objects, order, floats, keep flags, TC list) to a plain
+    single-slot lst_run of the same event, which the other tests compare with the oracle.  The
+    last group of 8 slots with batch 3 is a partial one (2 slots)."""
+    import torch
+    n_slots = 8
+    evs = [lstgen.make_event(geom_full, "cfg4", seed=2000 + i) for i in range(n_slots)]
+    mh, ms = max(e.n_hits for e in evs), max(e.n_seeds for e in evs)
+    sd = lambda e: (e.seed_pt, e.seed_eta, e.seed_phi, e.seed_z0, e.seed_q, e.seed_hit_ids)
+    cfg1 = B.lst_default_config()
+    cfg1.use_pdl = 0
+    single = B.LST(geom_full, map_full[0], map_full[1], cfg=cfg1, n_slots=1, max_hits=mh, max_seeds=ms)
+    ref = []
+    for e in evs:
+        single.lst_load_event(0, e.x, e.y, e.z, e.det, sd(e))
+        single.lst_run(0)
+        ref.append((single.lst_get_counts(0)[0].copy(), [single.lst_get_objects(0, lvl) for lvl in range(7)]))
+    single.close()
+    cfg = B.lst_default_config()
+    cfg.batch_events, cfg.use_pdl, cfg.use_cuda_graph = batch, pdl, graph
+    lst = B.LST(geom_full, map_full[0], map_full[1], cfg=cfg, n_slots=n_slots, max_hits=mh, max_seeds=ms)
+    assert B.lib().lst_batch_events(lst._h) == batch
+    n_groups = (n_slots + batch - 1) // batch
+    streams = [torch.cuda.Stream() for _ in range(n_groups)]
+    for rep in range(2):                                   # the second round replays the groups' graphs on used slots
+        for sl in range(n_slots):
+            e = evs[(sl + rep) % n_slots]
+            lst.lst_load_event(sl, e.x, e.y, e.z, e.det, sd(e), stream=streams[sl // batch])
+        for grp in range(n_groups):
+            lst.lst_run_batch(grp, stream=streams[grp])
+        for sl in range(n_slots):
+            i = (sl + rep) % n_slots
+            cnt, _ = lst.lst_get_counts(sl)
+            assert np.array_equal(cnt, ref[i][0]) and cnt[O.TC] > 100, "event %d: counts differ" % i
+            for lvl in range(7):
+                got, want = lst.lst_get_objects(sl, lvl), ref[i][1][lvl]
+                for k in ("hits", "parents", "f"):
+                    assert np.array_equal(got[k], want[k]), (i, lvl, k)
+                if want["keep"] is not None:
+                    assert np.array_equal(got["keep"], want["keep"]), (i, lvl)
+    # a group with an unloaded slot is refused, never run partially
+    fresh = B.LST(geom_full, map_full[0], map_full[1], cfg=cfg, n_slots=batch, max_hits=mh, max_seeds=ms)
+    e = evs[0]
+    fresh.lst_load_event(0, e.x, e.y, e.z, e.det, sd(e))
+    with pytest.raises(B.LstError) as ei:
+        fresh.lst_run_batch(0)
+    assert ei.value.status == B.LST_ESTATE
+    with pytest.raises(B.LstError):
+        fresh.lst_run_batch(1)
+    fresh.close()
+    lst.close()
