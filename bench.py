@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cfg4", action="store_true", help="skip the second, literal config-4 (6000-particle) throughput entry")
+    ap.add_argument("--truncate", type=float, default=0.999, help="occupancy quantile of the truncated memory mode entry "
+                    "(PAPER.md:125; 0 = skip)")
     return ap.parse_args()
 
 
@@ -339,7 +341,7 @@ def as_np(t, dt):
     return a.view(dt) if a.dtype != dt else a
 
 
-def run_ours(a, rank, world, local_rank, init_dist=True):
+def run_ours(a, rank, world, local_rank, init_dist=True, cfg_override=None, events=None):
     import torch
     import torch.distributed as dist
     import lstgen
@@ -354,10 +356,11 @@ def run_ours(a, rank, world, local_rank, init_dist=True):
     geom = lstgen.build_geometry(False)
     off, cols = B.lst_build_module_map(geom)
     from paper_2209_13711_b200 import sharding
-    events = [lstgen.make_event(geom, a.workload, seed=sd) for sd in sharding.event_seeds(rank, world, a.events)]
+    if events is None:
+        events = [lstgen.make_event(geom, a.workload, seed=sd) for sd in sharding.event_seeds(rank, world, a.events)]
     max_hits = max(e.n_hits for e in events)
     max_seeds = max(max(e.n_seeds for e in events), 1)
-    cfg = B.lst_default_config()
+    cfg = cfg_override if cfg_override is not None else B.lst_default_config()
     cfg.use_pdl, cfg.batch_events = a.pdl, a.batch
     assert a.slots % a.batch == 0 and a.events % a.slots == 0
     lst = B.LST(geom, off, cols, cfg=cfg, n_slots=a.slots, max_hits=max_hits, max_seeds=max_seeds, device=str(dev))
@@ -590,6 +593,22 @@ def main():
         line["also"] = {"cfg4": {"value": val4, "unit": UNIT, "ms_per_step": ms4 / a.steps, "workload": workload_name(b),
                                  "objects_event0": dict(zip(("md", "ls", "t3", "t5", "pt3", "pt5", "tc"),
                                                             [int(c) for c in cnt4[0][0]]))}}
+    if a.truncate > 0 and world == 1 and a.events >= 8:
+        # occupancy-truncated memory mode: caps at the quantile of the per-module
+        # occupancy of the first 32 events, capacities sized from the truncated sample, same 64-event batch
+        import copy
+        from paper_2209_13711_b200 import occupancy
+        try:
+            cfg_t, rep = occupancy.calibrate(geom, mp[0], mp[1], events[:32], quantile=a.truncate)
+            b = copy.copy(a)
+            b.no_e2e = True
+            lst_t, _, _, _, _, cnt_t, ms_t, _, val_t, _, _, _ = run_ours(b, rank, world, local_rank, init_dist=False,
+                                                                         cfg_override=cfg_t, events=events)
+            rep.update({"value": val_t, "unit": UNIT, "ms_per_step": ms_t / a.steps})
+            lst_t.close()
+        except Exception as ex:          # reported, never hidden: the exact-mode line above stands on its own
+            rep = {"error": repr(ex)}
+        line.setdefault("also", {})["truncated"] = rep
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

@@ -86,6 +86,14 @@ typedef struct {
                               [g E, (g + 1) E)) and lst_run_batch runs a whole group as ONE chain of
                               launches with a grid over (event, work): SURVEY.md 8(f)1, the B200 form of
                               the paper's multi-streaming                             */
+  uint32_t trunc_cap[6][16]; /* occupancy truncation, default all 0 = exact:
+                              trunc_cap[level][L] = K > 0: a module of logical layer L keeps at most K
+                              objects of `level` (LST_MD .. LST_T5; an object belongs to the module of its
+                              first mini-doublet); trunc_cap[LST_PT3 / LST_PT5][0] = K: a pixel seed keeps
+                              at most K pT3 / pT5.  Kept are the K first in the canonical order of the
+                              level (hits of a sensor ascend in azimuth relative to the module centre,
+                              ties by caller index; candidates row-major over (left object, right object)).
+                              The cap_* factors above can then be sized from the truncated occupancies. */
 } lst_config;
 
 /* Detector description, HOST arrays of length n_modules (copied by the callee).  A module is a

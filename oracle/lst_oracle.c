@@ -59,6 +59,8 @@ struct lsto_ctx {
   VEC(t5_t) t5;
   VEC(px_t) pt3, pt5;
   VEC(tc_t) tc;
+  float *phic;                       /* [n_modules] module centre azimuth: set by lsto_set_truncation (azimuth order) */
+  uint32_t trunc[6][16];             /* occupancy caps per level and logical layer (0 = none)                         */
   uint32_t *md_mod_off;              /* [n_modules+1] MD range of a module          */
   uint32_t *ls_md_off;               /* [n_md+1]      LS range of an inner MD       */
   uint32_t *t3_md_off;               /* [n_md+1]      T3 range of a first MD        */
@@ -501,9 +503,26 @@ void lsto_destroy(lsto_ctx *c) {
   if (!c) return;
   free_event(c);
   VFREE(c->md); VFREE(c->ls); VFREE(c->t3); VFREE(c->t5); VFREE(c->pt3); VFREE(c->pt5); VFREE(c->tc);
-  free(c->category); free(c->layer); free(c->map_off); free(c->map_cols);
+  free(c->category); free(c->layer); free(c->map_off); free(c->map_cols); free(c->phic);
   free(c);
 }
+
+/* PAPER.md:125 (occupancy truncation).  Optional mode: a bucket (MD, LS, T3, T5: the
+ * module of the object's first MD; pT3 / pT5: the pixel seed) keeps at most K objects, the K FIRST in
+ * the enumeration order of the definition, where the hits of a sensor are taken in ascending azimuth
+ * relative to the module centre phic (ties: original index).  caps: 6 x 16 values, level-major (MD,
+ * LS, T3, T5, PT3, PT5) by logical layer of the bucket's module (pixel levels: entry 0), 0 = no cap.
+ * Must be called before lsto_load_event.  The all-pairs (brute) builders ignore the caps. */
+int lsto_set_truncation(lsto_ctx *c, const float *phic, const uint32_t *caps) {
+  if (!c || !phic) return -1;
+  free(c->phic);
+  c->phic = malloc(((size_t)c->n_modules + 1) * sizeof(float));
+  memcpy(c->phic, phic, (size_t)c->n_modules * sizeof(float));
+  memset(c->trunc, 0, sizeof(c->trunc));
+  if (caps) memcpy(c->trunc, caps, sizeof(c->trunc));
+  return 0;
+}
+static uint32_t trunc_cap(const lsto_ctx *c, int level, uint32_t module) { return c->trunc[level][c->layer[module] & 15]; }
 
 int lsto_load_event(lsto_ctx *c, uint32_t n_hits, const float *x, const float *y, const float *z,
                     const uint32_t *det, uint32_t n_seeds, const float *pt, const float *eta,
@@ -525,6 +544,26 @@ int lsto_load_event(lsto_ctx *c, uint32_t n_hits, const float *x, const float *y
   memcpy(fill, c->det_off, ((size_t)nd + 1) * 4);
   for (uint32_t h = 0; h < n_hits; ++h) c->det_hits[fill[det[h]]++] = h;
   free(fill);
+  if (c->phic) {
+    /* occupancy-truncation mode (lsto_set_truncation): inside a det the hits ascend in azimuth relative
+     * to the module centre (ties: original index), so that every level is enumerated in the order the
+     * truncation rule "keep the first K of a bucket" refers to.  Insertion sort: a det holds ~10 hits. */
+    for (uint32_t d = 0; d < nd; ++d) {
+      uint32_t a = c->det_off[d], b = c->det_off[d + 1];
+      for (uint32_t i = a + 1; i < b; ++i) {
+        uint32_t h = c->det_hits[i];
+        double kh = wrap_pi(atan2(c->hy[h], c->hx[h]) - (double)c->phic[d >> 1]);
+        uint32_t j = i;
+        while (j > a) {
+          uint32_t g = c->det_hits[j - 1];
+          double kg = wrap_pi(atan2(c->hy[g], c->hx[g]) - (double)c->phic[d >> 1]);
+          if (kg < kh || (kg == kh && g < h)) break;
+          c->det_hits[j] = g; --j;
+        }
+        c->det_hits[j] = h;
+      }
+    }
+  }
   c->spt = malloc(((size_t)n_seeds + 1) * 8); c->seta = malloc(((size_t)n_seeds + 1) * 8);
   c->sphi = malloc(((size_t)n_seeds + 1) * 8); c->sz0 = malloc(((size_t)n_seeds + 1) * 8);
   c->sq = malloc((size_t)n_seeds + 1); c->sids = malloc(((size_t)n_seeds + 1) * 16);
@@ -557,7 +596,8 @@ int lsto_build_md(lsto_ctx *c) {
         pt3 u = hit_pt(c, hu, cat);
         md_t md; memset(&md, 0, sizeof(md));
         cut_t r = md_eval(c, &l, &u, cat, &md);
-        if (r.pass) { md.hl = hl; md.hu = hu; md.module = m; VPUSH(c->md, md); }
+        uint32_t K = trunc_cap(c, LSTO_MD, m);
+        if (r.pass && !(K && c->md.n - c->md_mod_off[m] >= K)) { md.hl = hl; md.hu = hu; md.module = m; VPUSH(c->md, md); }
       }
     }
   }
@@ -574,9 +614,12 @@ int lsto_build_ls(lsto_ctx *c, int brute) {
   VCLEAR(c->ls);
   free(c->ls_md_off);
   c->ls_md_off = calloc((size_t)c->md.n + 1, 4);
+  uint32_t bucket = 0xFFFFFFFFu, in_bucket = 0;     /* occupancy truncation: LS kept so far in the inner MD's module */
   for (uint32_t i = 0; i < c->md.n; ++i) {
     c->ls_md_off[i] = c->ls.n;
     const md_t *mi = &c->md.v[i];
+    if (mi->module != bucket) { bucket = mi->module; in_bucket = 0; }
+    const uint32_t K = trunc_cap(c, LSTO_LS, mi->module);
     if (brute) {
       for (uint32_t o = 0; o < c->md.n; ++o) {
         const md_t *mo = &c->md.v[o];
@@ -589,7 +632,7 @@ int lsto_build_ls(lsto_ctx *c, int brute) {
         uint32_t B = c->map_cols[e];
         for (uint32_t o = c->md_mod_off[B]; o < c->md_mod_off[B + 1]; ++o) {
           ls_t ls; memset(&ls, 0, sizeof(ls));
-          if (ls_eval(c, mi, &c->md.v[o], &ls).pass) { ls.mi = i; ls.mo = o; VPUSH(c->ls, ls); }
+          if (ls_eval(c, mi, &c->md.v[o], &ls).pass && !(K && in_bucket >= K)) { ls.mi = i; ls.mo = o; VPUSH(c->ls, ls); ++in_bucket; }
         }
       }
     }
@@ -603,8 +646,11 @@ int lsto_build_t3(lsto_ctx *c, int brute) {
   free(c->t3_md_off);
   c->t3_md_off = calloc((size_t)c->md.n + 2, 4);
   uint32_t cur_md = 0;
+  uint32_t bucket = 0xFFFFFFFFu, in_bucket = 0;     /* occupancy truncation: T3 kept so far in the first MD's module */
   for (uint32_t a = 0; a < c->ls.n; ++a) {
     const ls_t *A = &c->ls.v[a];
+    const uint32_t modA = c->md.v[A->mi].module, K = brute ? 0 : trunc_cap(c, LSTO_T3, modA);
+    if (modA != bucket) { bucket = modA; in_bucket = 0; }
     while (cur_md <= A->mi) c->t3_md_off[cur_md++] = c->t3.n;   /* T3 are grouped by first MD */
     uint32_t b0 = brute ? 0 : c->ls_md_off[A->mo], b1 = brute ? c->ls.n : c->ls_md_off[A->mo + 1];
     for (uint32_t b = b0; b < b1; ++b) {
@@ -612,9 +658,9 @@ int lsto_build_t3(lsto_ctx *c, int brute) {
       if (Bq->mi != A->mo) continue;
       t3_t t; memset(&t, 0, sizeof(t));
       const md_t *m1 = &c->md.v[A->mi], *m2 = &c->md.v[A->mo], *m3 = &c->md.v[Bq->mo];
-      if (t3_eval(c, &m1->a, &m2->a, &m3->a, &t).pass) {
+      if (t3_eval(c, &m1->a, &m2->a, &m3->a, &t).pass && !(K && in_bucket >= K)) {
         t.la = a; t.lb = b; t.m[0] = A->mi; t.m[1] = A->mo; t.m[2] = Bq->mo;
-        VPUSH(c->t3, t);
+        VPUSH(c->t3, t); ++in_bucket;
       }
     }
   }
@@ -624,8 +670,11 @@ int lsto_build_t3(lsto_ctx *c, int brute) {
 
 int lsto_build_t5(lsto_ctx *c, int brute) {
   VCLEAR(c->t5);
+  uint32_t bucket = 0xFFFFFFFFu, in_bucket = 0;     /* occupancy truncation: T5 kept so far in the first MD's module */
   for (uint32_t a = 0; a < c->t3.n; ++a) {
     const t3_t *A = &c->t3.v[a];
+    const uint32_t modA = c->md.v[A->m[0]].module, K = brute ? 0 : trunc_cap(c, LSTO_T5, modA);
+    if (modA != bucket) { bucket = modA; in_bucket = 0; }
     uint32_t b0 = brute ? 0 : c->t3_md_off[A->m[2]], b1 = brute ? c->t3.n : c->t3_md_off[A->m[2] + 1];
     for (uint32_t b = b0; b < b1; ++b) {
       const t3_t *Bq = &c->t3.v[b];
@@ -634,10 +683,10 @@ int lsto_build_t5(lsto_ctx *c, int brute) {
       const pt3 *P[5];
       for (int k = 0; k < 5; ++k) P[k] = &c->md.v[mm[k]].a;
       t5_t t; memset(&t, 0, sizeof(t));
-      if (t5_eval(c, P, A->kappa3, A->sigk3, Bq->kappa3, Bq->sigk3, &t).pass) {
+      if (t5_eval(c, P, A->kappa3, A->sigk3, Bq->kappa3, Bq->sigk3, &t).pass && !(K && in_bucket >= K)) {
         t.ta = a; t.tb = b;
         for (int k = 0; k < 5; ++k) t.m[k] = mm[k];
-        VPUSH(c->t5, t);
+        VPUSH(c->t5, t); ++in_bucket;
       }
     }
   }
@@ -647,24 +696,27 @@ int lsto_build_t5(lsto_ctx *c, int brute) {
 int lsto_link_pixel(lsto_ctx *c, uint32_t s0, uint32_t s1) {
   VCLEAR(c->pt5); VCLEAR(c->pt3);
   if (s1 > c->n_seeds) s1 = c->n_seeds;
+  const uint32_t K5 = c->trunc[LSTO_PT5][0], K3 = c->trunc[LSTO_PT3][0];   /* occupancy truncation: per pixel seed */
   for (uint32_t p = s0; p < s1; ++p) {
+    uint32_t kept = 0;
     for (uint32_t o = 0; o < c->t5.n; ++o) {
       const t5_t *T = &c->t5.v[o];
       const pt3 *P[5];
       for (int k = 0; k < 5; ++k) P[k] = &c->md.v[T->m[k]].a;
       double chi2 = 0;
       cut_t r = px_eval(c, p, P, 5, c->layer[c->md.v[T->m[0]].module], &chi2, 0);
-      if (r.pass) { px_t x = {p, o, chi2, r.margin}; VPUSH(c->pt5, x); }
+      if (r.pass && !(K5 && kept >= K5)) { px_t x = {p, o, chi2, r.margin}; VPUSH(c->pt5, x); ++kept; }
     }
   }
   for (uint32_t p = s0; p < s1; ++p) {
+    uint32_t kept = 0;
     for (uint32_t o = 0; o < c->t3.n; ++o) {
       const t3_t *T = &c->t3.v[o];
       const pt3 *P[3];
       for (int k = 0; k < 3; ++k) P[k] = &c->md.v[T->m[k]].a;
       double chi2 = 0;
       cut_t r = px_eval(c, p, P, 3, c->layer[c->md.v[T->m[0]].module], &chi2, 0);
-      if (r.pass) { px_t x = {p, o, chi2, r.margin}; VPUSH(c->pt3, x); }
+      if (r.pass && !(K3 && kept >= K3)) { px_t x = {p, o, chi2, r.margin}; VPUSH(c->pt3, x); ++kept; }
     }
   }
   return 0;
@@ -747,6 +799,8 @@ int lsto_link_pixel_indexed(lsto_ctx *c, uint32_t s0, uint32_t s1) {
   for (uint32_t i = 0; i < nmd; ++i) t5_off[i + 1] += t5_off[i];
   for (int five = 1; five >= 0; --five) {
     for (uint32_t p = s0; p < s1; ++p) {
+      const uint32_t K = c->trunc[five ? LSTO_PT5 : LSTO_PT3][0];       /* occupancy truncation: per pixel seed */
+      uint32_t kept = 0;
       for (uint32_t k = 0; k < n_start; ++k) {
         uint32_t m = mods[k];
         if (!px_box_possible(c, p, &box[m], c->category[m])) continue;
@@ -759,7 +813,7 @@ int lsto_link_pixel_indexed(lsto_ctx *c, uint32_t s0, uint32_t s1) {
             for (int q = 0; q < n; ++q) P[q] = &c->md.v[mm[q]].a;
             double chi2 = 0;
             cut_t r = px_eval(c, p, P, n, c->layer[m], &chi2, 0);
-            if (r.pass) { px_t x = {p, o, chi2, r.margin}; if (five) VPUSH(c->pt5, x); else VPUSH(c->pt3, x); }
+            if (r.pass && !(K && kept >= K)) { px_t x = {p, o, chi2, r.margin}; if (five) VPUSH(c->pt5, x); else VPUSH(c->pt3, x); ++kept; }
           }
         }
       }

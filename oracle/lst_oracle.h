@@ -77,6 +77,11 @@ lsto_ctx *lsto_create(uint32_t n_modules, const uint8_t *category, const uint8_t
                       const lsto_config *cfg);
 void lsto_destroy(lsto_ctx *c);
 
+/* PAPER.md:125 occupancy truncation (optional; see the .c file): hit order inside a sensor = ascending
+ * azimuth relative to phic[module]; caps[level * 16 + logical layer] = K keeps the first K objects of a
+ * module (pixel levels: caps[level * 16] per seed); NULL caps = order only.  Call before lsto_load_event. */
+int lsto_set_truncation(lsto_ctx *c, const float *phic, const uint32_t *caps);
+
 int lsto_load_event(lsto_ctx *c, uint32_t n_hits, const float *x, const float *y, const float *z,
                     const uint32_t *det, uint32_t n_seeds, const float *pt, const float *eta,
                     const float *phi, const float *z0, const int8_t *q, const uint32_t *hit_ids);

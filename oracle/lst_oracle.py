@@ -58,6 +58,7 @@ def lib():
         L.lsto_create.argtypes = [u32, vp, vp, vp, vp, C.POINTER(Config)]
         L.lsto_destroy.argtypes = [vp]
         L.lsto_load_event.argtypes = [vp, u32, vp, vp, vp, vp, u32, vp, vp, vp, vp, vp, vp]
+        L.lsto_set_truncation.argtypes = [vp, vp, vp]
         L.lsto_build_md.argtypes = [vp]
         for f in ("lsto_build_ls", "lsto_build_t3", "lsto_build_t5", "lsto_dedup"):
             getattr(L, f).argtypes = [vp, i32]
@@ -131,6 +132,13 @@ class Oracle:
             self.close()
         except Exception:
             pass
+
+    def set_truncation(self, phic, caps=None):
+        """Occupancy-truncation mode: azimuth hit order + per-bucket caps [6, 16] (or None)."""
+        ph = np.ascontiguousarray(phic, dtype=np.float32)
+        cp = np.ascontiguousarray(caps, dtype=np.uint32).reshape(6, 16) if caps is not None else None
+        rc = lib().lsto_set_truncation(self._h, _p(ph), _p(cp) if cp is not None else None)
+        assert rc == 0
 
     def load(self, ev):
         f = lambda a, dt: np.ascontiguousarray(a, dtype=dt)

@@ -167,7 +167,73 @@ __global__ void __launch_bounds__(kCountThreads) k_counts(const __grid_constant_
     }
   }
 }
+// ------------------------------------------------------------------ occupancy truncation
+// Optional memory mode: a bucket (MD, LS, T3, T5: the module of the object's first MD; pT3 / pT5: the
+// pixel seed) keeps at most K accepted candidates, the K FIRST in canonical order ("the K smallest
+// keys": a candidate's key is its position in the enumeration of the method's definition).  A bucket's
+// candidates are one contiguous range of pass bits, so the rule is: clear every set bit after the
+// K-th one of the range.  One warp per bucket, between the decide kernel and k_counts; sizes stay
+// exact (of the truncated set).  K = Params::trunc[level][logical layer of the module] ([level][0]
+// for the per-seed caps), 0 = no cap.
+__device__ __forceinline__ uint32_t row_key(const StageBuf &st, uint32_t a, uint32_t n_rows, uint32_t n_items) {
+  return a < n_rows ? st.g_item0[a / kRowChunk] * (uint32_t)kItemCand + st.row_cum[a] : n_items * (uint32_t)kItemCand;
+}
+__global__ void __launch_bounds__(256) k_truncate(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
+                                                   const __grid_constant__ Params g, int stage0) {
+  pdl_enter();
+  LST_SLOT(B);
+  const int stage = stage0 + (int)blockIdx.y;
+  const Header *hdr = s.hdr;
+  const StageBuf &st = s.st[stage];
+  const uint32_t n_items = hdr->n_items[stage];
+  if (n_items == 0) return;
+  const int level = stage == S_PT5 ? 5 : (stage == S_PT3 ? 4 : stage);
+  const bool by_seed = stage >= S_PT5;
+  const uint32_t n_buckets = by_seed ? hdr->n_seeds : geo.n_modules;
+  const uint32_t n_rows = stage == S_T3 ? hdr->n_obj[1] : (stage == S_T5 ? hdr->n_obj[2] : hdr->n_obj[kPairLevel]);
+  const int lane = threadIdx.x & 31;
+  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+  for (uint32_t b = warp; b < n_buckets; b += nwarp) {
+    const uint32_t K = by_seed ? g.trunc[level][0] : g.trunc[level][geo.layer[b] & 15];
+    if (K == 0) continue;
+    uint32_t key_lo, key_hi;
+    if (stage <= S_LS) { key_lo = st.g_item0[b] * (uint32_t)kItemCand; key_hi = st.g_item0[b + 1] * (uint32_t)kItemCand; }
+    else {
+      uint32_t a0, a1;
+      if (by_seed) { a0 = s.px_off[b]; a1 = s.px_off[b + 1]; }
+      else {
+        const uint32_t *off = stage == S_T3 ? s.ls_md_off : s.t3_md_off;
+        a0 = off[s.md_mod_off[b]]; a1 = off[s.md_mod_off[b + 1]];
+      }
+      key_lo = row_key(st, a0, n_rows, n_items); key_hi = row_key(st, a1, n_rows, n_items);
+    }
+    if (key_lo >= key_hi) continue;
+    const uint32_t w_lo = key_lo >> 5, w_hi = (key_hi + 31u) >> 5;     // mask word of a key = key / 32 (kItemCand = 32 words)
+    uint32_t running = 0;
+    for (uint32_t wb = w_lo; wb < w_hi; wb += 32) {
+      const uint32_t w = wb + lane;
+      uint32_t mk = w < w_hi ? st.mask[w] : 0u;
+      if (w == w_lo) mk &= ~((1u << (key_lo & 31u)) - 1u);
+      if (w == (key_hi >> 5) && (key_hi & 31u)) mk &= (1u << (key_hi & 31u)) - 1u;
+      const uint32_t c = (uint32_t)__popc(mk);
+      uint32_t tot;
+      const uint32_t before = running + warp_excl_scan(c, &tot);
+      if (c && before + c > K) {
+        const uint32_t keepn = K > before ? K - before : 0u;             // the lowest keepn set bits of mk stay
+        uint32_t t = mk;
+        for (uint32_t k = 0; k < keepn; ++k) t &= t - 1u;
+        atomicAnd(&st.mask[w], ~t);                                        // edge words are shared with the neighbouring buckets
+      }
+      running += tot;
+    }
+  }
+}
+
 void launch_counts(const Ctx &c, const Batch &b, int stage, int level, uint32_t cap, bool pair, cudaStream_t st) {
+  if (c.trunc_stages & ((1u << stage) | (pair ? 1u << (stage + 1) : 0u))) {
+    const uint32_t nb = stage >= S_PT5 ? b.s[0].cap_seeds : c.geo.n_modules;
+    launch_k(c, st, "k_truncate", k_truncate, dim3(grid_for(nb, 8, c.n_sm * 4), pair ? 2 : 1), 256, 0, false, c.geo, b, c.par, stage);
+  }
   static const char *const nm[S_NSTAGE] = {"k_counts[MD]", "k_counts[LS]", "k_counts[T3]", "k_counts[T5]", "k_counts[pT5+pT3]", "k_counts[pT3]"};
   const uint32_t cap1 = pair ? b.s[0].cap_pt3 : 0u;
   launch_k(c, st, nm[stage], k_counts, dim3(kCountBlocks, pair ? 2 : 1), kCountThreads, 0, false, b, stage, level, cap, cap1);

@@ -17,7 +17,7 @@ using namespace lst;
 
 // ------------------------------------------------------------------ status text
 static thread_local char g_cuda_err[256] = "no CUDA error recorded";
-static thread_local char g_cap_err[256] = "workspace too small or object capacity exceeded";
+static thread_local char g_cap_err[640] = "workspace too small or object capacity exceeded";
 static thread_local char g_inval_err[192] = "invalid argument";
 
 static int cuda_fail(cudaError_t e, const char *where) {
@@ -90,6 +90,7 @@ extern "C" void lst_default_config(lst_config *c) {
   c->enum_pruning = 3;
   c->use_pdl = 1;
   c->batch_events = 1;
+  /* trunc_cap: all 0 (no occupancy truncation) */
 }
 
 static void make_params(const lst_config &c, Params *p) {
@@ -107,6 +108,7 @@ static void make_params(const lst_config &c, Params *p) {
   p->dup_t5 = c.dup_t5_shared; p->dup_pt5 = c.dup_pt5_shared; p->dup_pt3 = c.dup_pt3_shared;
   p->s0_enabled = c.s0_enabled;
   p->start_mask = c.start_layer_mask;
+  for (int l = 0; l < 6; ++l) for (int k = 0; k < 16; ++k) p->trunc[l][k] = c.trunc_cap[l][k];
   // bin width >= 1.25 sqrt(dr2max): two seeds closer than sqrt(dr2max) in eta are in adjacent bins
   const double sq = std::sqrt(std::max(c.dr2max, 0.0));
   const double width = std::max(1.25 * sq, 8.0 / kEtaBins);
@@ -487,6 +489,13 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   make_params(c->cfg, &c->k.par);
   c->k.ls_windows = (c->cfg.enum_pruning & 2) != 0;
   c->k.pdl = c->cfg.use_pdl != 0;
+  {
+    // stages with an occupancy cap: MD, LS, T3, T5 per logical layer; pT3 / pT5 per seed ([level][0])
+    const int stage_of_level[6] = {S_MD, S_LS, S_T3, S_T5, S_PT3, S_PT5};
+    for (int l = 0; l < 6; ++l)
+      for (int k = 0; k < (l < 4 ? 16 : 1); ++k)
+        if (c->cfg.trunc_cap[l][k]) c->k.trunc_stages |= 1u << stage_of_level[l];
+  }
   if (c->cfg.batch_events < 1 || c->cfg.batch_events > kMaxBatch) { delete c; return einval(); }
   c->batch = (uint32_t)c->cfg.batch_events;
   c->n_slots = n_slots; c->max_hits = max_hits; c->max_seeds = max_seeds;
@@ -801,11 +810,15 @@ static int sync_header(lst_ctx *c, Slot &s) {
   }
   if (s.h_hdr->err & (ERR_CAP_ITEMS | ERR_CAP_OBJ | ERR_CAP_PIX)) {
     const Header &h = *s.h_hdr;
-    snprintf(g_cap_err, sizeof(g_cap_err),
-             "capacity exceeded:%s%s%s (objects MD %u LS %u T3 %u T5 %u pT3 %u pT5 %u; raise lst_config.cap_*)",
-             (h.err & ERR_CAP_ITEMS) ? " work items" : "", (h.err & ERR_CAP_OBJ) ? " object array" : "",
-             (h.err & ERR_CAP_PIX) ? " per-seed list" : "", h.n_obj[0], h.n_obj[1], h.n_obj[2], h.n_obj[3], h.n_obj[4],
-             h.n_obj[5]);
+    int n = snprintf(g_cap_err, sizeof(g_cap_err),
+                     "capacity exceeded:%s%s%s (objects MD %u LS %u T3 %u T5 %u pT3 %u pT5 %u; raise lst_config.cap_*);",
+                     (h.err & ERR_CAP_ITEMS) ? " work items / candidate list" : "", (h.err & ERR_CAP_OBJ) ? " object array" : "",
+                     (h.err & ERR_CAP_PIX) ? " per-seed list" : "", h.n_obj[0], h.n_obj[1], h.n_obj[2], h.n_obj[3], h.n_obj[4],
+                     h.n_obj[5]);
+    static const char *const nm[S_NSTAGE] = {"MD", "LS", "T3", "T5", "pT5", "pT3"};
+    for (int k = 0; k < S_NSTAGE && n > 0 && n < (int)sizeof(g_cap_err) - 80; ++k)   // a stage whose work list overflowed shows items 0
+      n += snprintf(g_cap_err + n, sizeof(g_cap_err) - n, " %s items %u/%u list %u/%u", nm[k], h.n_items[k], s.dev.st[k].cap_items,
+                    h.cl_used[k], s.dev.st[k].cap_cl);
     return LST_ENOMEM;
   }
   return LST_OK;

@@ -24,6 +24,7 @@ struct Ctx {             // what the launchers need from a context
   int ls_windows = 1;    // lst_config.enum_pruning bit 1: per-row windows of the LS enumeration
   int pdl = 0;           // launch with programmatic stream serialisation (lst_config.use_pdl)
   int nb = 1;            // slots (events) in the batch: gridDim.z of every launch
+  unsigned trunc_stages = 0;   // bit k: stage k has an occupancy cap (k_truncate runs before its k_counts)
 };
 
 // One launch of the chain: gridDim.z = events of the batch; with c.pdl the kernel may become resident

@@ -44,6 +44,7 @@ struct Params {
   // eta binning of the pixel seeds used by the cleaning (k_dedup.cu)
   double eta_bin_inv, dr_eta_pre;
   int eta_nbins;
+  uint32_t trunc[6][16];   // occupancy truncation (lst_config.trunc_cap): per lst_level and logical layer, 0 = none
 };
 
 LST_HD bool is_endcap(int cat) { return cat >= 2; }

@@ -1,0 +1,133 @@
+"""Occupancy-truncated memory mode: "a bucket keeps the K first objects
+of its canonical order".  CPU part: the oracle's truncation mode pinned against an independent numpy
+restatement of the rule at the MD level and against properties at every level.  GPU part (-m gpu):
+the CUDA path with lst_config.trunc_cap against the oracle in the same mode, every level."""
+import numpy as np
+import pytest
+
+import lstgen
+from oracle import lst_oracle as O
+
+CAPS = np.zeros((6, 16), np.uint32)
+CAPS[O.MD, :] = 5
+CAPS[O.LS, :] = 12
+CAPS[O.T3, :] = 10
+CAPS[O.T5, :] = 6
+CAPS[O.PT3, 0] = 3
+CAPS[O.PT5, 0] = 2
+
+
+def _run(geom, mp, ev, caps, order=True, upto=O.TC):
+    o = O.Oracle(geom, mp[0], mp[1])
+    if order:
+        o.set_truncation(geom.phic, caps)
+    o.load(ev)
+    o.run(upto=upto, pixel_indexed=True)
+    return o
+
+
+def _keys(o, lvl):
+    d = o.get(lvl)
+    h = d["hits"].astype(np.int64)
+    if lvl in (O.PT3, O.PT5):
+        h = np.concatenate([d["parents"][:, :1].astype(np.int64), h], 1)
+    return [tuple(r) for r in h.tolist()]
+
+
+def test_azimuth_order_alone_changes_no_set(geom_barrel, map_barrel):
+    ev = lstgen.make_event(geom_barrel, "cfg2s")
+    a, b = _run(geom_barrel, map_barrel, ev, None, order=False), _run(geom_barrel, map_barrel, ev, None, order=True)
+    for lvl in (O.MD, O.LS, O.T3, O.T5, O.PT3, O.PT5, O.TC):
+        assert a.count(lvl) == b.count(lvl) > 0
+        if lvl != O.TC:
+            assert set(_keys(a, lvl)) == set(_keys(b, lvl))
+    # ... and the MDs of a module now ascend in the azimuth of their lower hit relative to the module centre
+    md = b.get(O.MD)
+    mod = md["parents"][:, 0].astype(np.int64)
+    lo = md["hits"][:, 0].astype(np.int64)
+    rel = np.arctan2(ev.y[lo].astype(np.float64), ev.x[lo].astype(np.float64)) - np.asarray(geom_barrel.phic, np.float64)[mod]
+    rel = np.remainder(rel + np.pi, 2 * np.pi) - np.pi
+    assert np.all(np.diff(mod) >= 0) and np.all(np.diff(rel)[np.diff(mod) == 0] >= 0)
+
+
+def test_md_cap_is_the_first_k_of_a_numpy_restatement(geom_barrel, map_barrel):
+    """MD level, typed independently: group the EXACT mini-doublets by module, order them by (azimuth
+    of the lower hit relative to the module centre, its index, the same of the upper hit), keep K."""
+    ev = lstgen.make_event(geom_barrel, "cfg2")
+    caps = np.zeros((6, 16), np.uint32)
+    caps[O.MD, :] = 2
+    exact = _run(geom_barrel, map_barrel, ev, None, order=False, upto=O.MD).get(O.MD)
+    got = set(_keys(_run(geom_barrel, map_barrel, ev, caps, upto=O.MD), O.MD))
+    phic = np.asarray(geom_barrel.phic, np.float64)
+    x, y = ev.x.astype(np.float64), ev.y.astype(np.float64)
+    want, over = set(), 0
+    mod = exact["parents"][:, 0].astype(np.int64)
+    for m in np.unique(mod):
+        rows = exact["hits"][mod == m].astype(np.int64)
+        rel = lambda h: np.remainder(np.arctan2(y[h], x[h]) - phic[m] + np.pi, 2 * np.pi) - np.pi
+        order = sorted(range(len(rows)), key=lambda k: (rel(rows[k, 0]), rows[k, 0], rel(rows[k, 1]), rows[k, 1]))
+        over += len(rows) > 2
+        want |= {tuple(rows[k].tolist()) for k in order[:2]}
+    assert over > 20, "the cap must bite for the pin to mean something"
+    assert got == want
+
+
+def test_caps_at_every_level_properties(geom_barrel, map_barrel):
+    ev = lstgen.make_event(geom_barrel, "cfg2s")
+    exact, tr = _run(geom_barrel, map_barrel, ev, None, order=False), _run(geom_barrel, map_barrel, ev, CAPS)
+    lay = np.asarray(geom_barrel.logical_layer, np.int64)
+    first_mod = None
+    for lvl in (O.MD, O.LS, O.T3, O.T5, O.PT3, O.PT5):
+        ke, kt = set(_keys(exact, lvl)), _keys(tr, lvl)
+        assert set(kt) <= ke and len(set(kt)) == len(kt), "a truncated level is a subset of the exact one"
+        assert 0 < len(kt) < len(ke), "level %s: the caps must bite" % O.LEVEL_NAMES[lvl]
+        d = tr.get(lvl)
+        if lvl in (O.PT3, O.PT5):
+            _, cnt = np.unique(d["parents"][:, 0], return_counts=True)
+            assert cnt.max() <= CAPS[lvl, 0]
+        else:
+            # bucket = module of the first MD = module of the first hit
+            m = ev.det[d["hits"][:, 0].astype(np.int64)].astype(np.int64) >> 1
+            u, cnt = np.unique(m, return_counts=True)
+            assert np.all(cnt <= CAPS[lvl, lay[u]])
+            assert np.all(np.diff(m) >= 0), "objects stay grouped by the module of their first MD"
+    assert tr.count(O.TC) > 0
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg_name", ["cfg2s", "cfg4"])
+def test_gpu_truncated_mode_matches_oracle_truncated_mode(geom_barrel, map_barrel, geom_full, map_full, cfg_name):
+    """The CUDA path with lst_config.trunc_cap against the oracle in the same mode: identical object
+    sets at every level (the objects a full bucket keeps are decided by the canonical order, i.e. by the
+    fp32 azimuth keys of the hits on the GPU and fp64 ones in the oracle: a pair of hits of one sensor
+    closer than ~1e-6 rad in azimuth could flip; none does on these seeded events), TC included."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2209_13711_b200 import binding as B
+    geom, mp = (geom_barrel, map_barrel) if cfg_name == "cfg2s" else (geom_full, map_full)
+    caps = CAPS.copy()
+    if cfg_name == "cfg4":
+        caps[O.MD, :], caps[O.LS, :], caps[O.T3, :], caps[O.T5, :] = 8, 30, 24, 8
+        caps[O.PT3, 0], caps[O.PT5, 0] = 6, 3
+    ev = lstgen.make_event(geom, cfg_name)
+    o = _run(geom, mp, ev, caps)
+    cfg = B.lst_default_config()
+    for l in range(6):
+        for k in range(16):
+            cfg.trunc_cap[l][k] = int(caps[l, k])
+    lst = B.LST(geom, mp[0], mp[1], cfg=cfg, n_slots=1, max_hits=ev.n_hits, max_seeds=max(ev.n_seeds, 1))
+    lst.lst_load_event(0, ev.x, ev.y, ev.z, ev.det, (ev.seed_pt, ev.seed_eta, ev.seed_phi, ev.seed_z0, ev.seed_q, ev.seed_hit_ids))
+    lst.lst_run(0)
+    cnt, _ = lst.lst_get_counts(0)
+    exact = _run(geom, mp, ev, None, order=False)
+    for lvl in (O.MD, O.LS, O.T3, O.T5, O.PT3, O.PT5):
+        got = lst.lst_get_objects(0, lvl)
+        h = got["hits"].astype(np.int64)
+        if lvl in (O.PT3, O.PT5):
+            h = np.concatenate([got["parents"][:, :1].astype(np.int64), h], 1)
+        kg = set(map(tuple, h.tolist()))
+        assert kg == set(_keys(o, lvl)), "level %s differs from the oracle's truncated mode" % O.LEVEL_NAMES[lvl]
+        assert 0 < len(kg) < exact.count(lvl), "level %s: the caps must bite" % O.LEVEL_NAMES[lvl]
+    assert cnt[O.TC] == o.count(O.TC) > 0
+    lst.close()
