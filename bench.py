@@ -53,6 +53,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cfg4", action="store_true", help="skip the second, literal config-4 (6000-particle) throughput entry")
+    ap.add_argument("--no-physics", action="store_true", help="skip the efficiency / fake / duplicate-rate entry")
     ap.add_argument("--truncate", type=float, default=0.999, help="occupancy quantile of the truncated memory mode entry "
                     "(PAPER.md:125; 0 = skip)")
     return ap.parse_args()
@@ -593,6 +594,24 @@ def main():
         line["also"] = {"cfg4": {"value": val4, "unit": UNIT, "ms_per_step": ms4 / a.steps, "workload": workload_name(b),
                                  "objects_event0": dict(zip(("md", "ls", "t3", "t5", "pt3", "pt5", "tc"),
                                                             [int(c) for c in cnt4[0][0]]))}}
+    if rank == 0 and not a.no_physics:
+        # physics sanity on synthetic truth: efficiency / fake rate / duplicate rate of the
+        # track candidates of the first events of the batch (the paper's figures need CMS simulation)
+        from paper_2209_13711_b200 import physics as PH
+        cfgp = B.lst_default_config()
+        lp = B.LST(geom, mp[0], mp[1], cfg=cfgp, n_slots=1, max_hits=max(e.n_hits for e in events),
+                   max_seeds=max(max(e.n_seeds for e in events), 1))
+        acc = None
+        for e in events[:4]:
+            lp.lst_load_event(0, e.x, e.y, e.z, e.det, (e.seed_pt, e.seed_eta, e.seed_phi, e.seed_z0, e.seed_q, e.seed_hit_ids)
+                              if e.n_seeds else None)
+            lp.lst_run(0)
+            tc = lp.lst_get_objects(0, B.LST_TC)
+            acc = PH.add(acc, PH.rates(e, tc["hits"], tc["parents"][:, 0], tc["f"][:, 0], tc["f"][:, 1]))
+        lp.close()
+        line.setdefault("also", {})["physics_synthetic_truth"] = dict(PH.summary(acc), events=4,
+            note="matched = >= 75 % of the candidate's hits from one particle; denominator = pT > 0.8 GeV, |eta| < 2.4, both "
+                 "sensors hit in >= 5 modules; context only (PAPER.md:95-99 quotes ~90 % / < 5 % duplicates / 15-20 % fakes on CMS tt-bar PU200)")
     if a.truncate > 0 and world == 1 and a.events >= 8:
         # occupancy-truncated memory mode: caps at the quantile of the per-module
         # occupancy of the first 32 events, capacities sized from the truncated sample, same 64-event batch
