@@ -94,6 +94,12 @@ typedef struct {
                               level (hits of a sensor ascend in azimuth relative to the module centre,
                               ties by caller index; candidates row-major over (left object, right object)).
                               The cap_* factors above can then be sized from the truncated occupancies. */
+  int32_t store_half;      /* 0 (default) | 1: reduced-precision storage (PAPER.md:147 outlook):
+                              the derived floats that no later decision reads (MD dphi; LS dphi, kappa,
+                              sigma_kappa; T3 beta; T5 R, chi2, kappa3 a / b, pT) are kept as IEEE binary16
+                              in the slot workspace (half the bytes; relative error <= 4.9e-4, values above
+                              65504 saturate) and widened again by lst_get_objects.  Object sets, keep flags
+                              and the TC list are unchanged: every decision uses the fp64 quantities. */
 } lst_config;
 
 /* Detector description, HOST arrays of length n_modules (copied by the callee).  A module is a

@@ -37,7 +37,8 @@ class lst_config(C.Structure):
             "cap_md_per_hit", "cap_ls_per_hit", "cap_t3_per_hit", "cap_t5_per_hit", "cap_pt3_per_seed",
             "cap_pt5_per_seed", "cap_mdcand_per_hit", "cap_lscand_per_hit", "cap_t3cand_per_hit",
             "cap_t5cand_per_hit")] + [("use_cuda_graph", C.c_int32), ("enum_pruning", C.c_int32), ("use_pdl", C.c_int32),
-                                   ("batch_events", C.c_int32), ("trunc_cap", (C.c_uint32 * 16) * 6)]
+                                   ("batch_events", C.c_int32), ("trunc_cap", (C.c_uint32 * 16) * 6),
+                                   ("store_half", C.c_int32)]
 
 
 class lst_geometry(C.Structure):

@@ -596,7 +596,7 @@ __global__ void __launch_bounds__(256) k_tc_fill(const __grid_constant__ Batch B
       s.tc_to[pos] = make_uint2(type, obj);
       if (type == 3) {
         const double2 ep = s.t5_etaphi[obj];
-        s.tc_f[pos] = make_float4(s.t5_pt[obj], (float)ep.x, (float)ep.y, 3.0f);
+        s.tc_f[pos] = make_float4(ld_f(s, s.t5_pt, obj), (float)ep.x, (float)ep.y, 3.0f);
       } else {
         s.tc_f[pos] = make_float4(s.seed_pt[p], s.seed_eta[p], s.seed_phi[p], (float)type);
       }

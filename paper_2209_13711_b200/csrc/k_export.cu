@@ -20,7 +20,7 @@ __global__ void k_export(SlotDev s, int level) {
         md_orig_hits(s, i, s.exp_hits + 2 * (size_t)i);
         par0 = s.md_mod[i] >> 2;
         const double2 k = s.md_kd[i];
-        f = make_float4(s.md_dphi[i], (float)k.x, (float)k.y, 0.f);
+        f = make_float4(ld_f(s, s.md_dphi, i), (float)k.x, (float)k.y, 0.f);
         break;
       }
       case 1: {
@@ -28,7 +28,7 @@ __global__ void k_export(SlotDev s, int level) {
         md_orig_hits(s, m.x, s.exp_hits + 4 * (size_t)i);
         md_orig_hits(s, m.y, s.exp_hits + 4 * (size_t)i + 2);
         par0 = m.x; par1 = m.y;
-        f = s.ls_f[i];
+        f = ld_f4(s, s.ls_f, i);
         break;
       }
       case 2: {
@@ -39,14 +39,14 @@ __global__ void k_export(SlotDev s, int level) {
         const uint2 l = s.t3_ls[i];
         par0 = l.x; par1 = l.y;
         const double2 k = s.t3_kd[i];
-        f = make_float4(s.t3_beta[i], (float)k.x, (float)k.y, 0.f);
+        f = make_float4(ld_f(s, s.t3_beta, i), (float)k.x, (float)k.y, 0.f);
         break;
       }
       case 3: {
         for (int q = 0; q < 5; ++q) md_orig_hits(s, s.t5_md[5 * (size_t)i + q], s.exp_hits + 10 * (size_t)i + 2 * q);
         const uint2 t = s.t5_t3[i];
         par0 = t.x; par1 = t.y;
-        f = s.t5_f[i];
+        f = ld_f4(s, s.t5_f, i);
         break;
       }
       case 4: {

@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(256) k_md_fill(const __grid_constant__ GeoDev 
     s.md_kf[idx] = make_float2((float)kd.x, (float)kd.y);
     s.md_hit[idx] = h;
     s.md_mod[idx] = (m << 2) | (uint32_t)geo.category[m];
-    s.md_dphi[idx] = st.p_f4[j].x;
+    st_f(s, s.md_dphi, idx, st.p_f4[j].x);
     s.md_phi[idx] = atan2f(l.y, l.x);
     s.md_prel[idx] = s.hit_key[h.x];
   }
@@ -486,7 +486,7 @@ __global__ void __launch_bounds__(256) k_ls_fill(const __grid_constant__ Batch B
     const uint32_t idx = pool_target(st, st.cl_key[j]);
     if (idx == 0xFFFFFFFFu) continue;
     s.ls_md[idx] = st.cl_ab[j];
-    s.ls_f[idx] = st.p_f4[j];
+    st_f4(s, s.ls_f, idx, st.p_f4[j]);
   }
 }
 

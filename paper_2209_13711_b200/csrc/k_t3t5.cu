@@ -476,7 +476,7 @@ __device__ __forceinline__ void join_fill_body(const SlotDev &s) {
       s.t3_md[idx] = make_uint4(la.x, la.y, lb.y, 0u);
       s.t3_ls[idx] = ab;
       s.t3_kd[idx] = st.p_d2[j];
-      s.t3_beta[idx] = st.p_f4[j].x;
+      st_f(s, s.t3_beta, idx, st.p_f4[j].x);
     } else if (KIND == J_T5) {
       const uint4 ta = s.t3_md[ab.x], tb = s.t3_md[ab.y];
       const uint32_t m[5] = {ta.x, ta.y, ta.z, tb.y, tb.z};
@@ -486,8 +486,8 @@ __device__ __forceinline__ void join_fill_body(const SlotDev &s) {
       s.t5_t3[idx] = ab;
       s.t5_chi2[idx] = cr.x;
       s.t5_etaphi[idx] = st.p_d2[j];
-      s.t5_f[idx] = make_float4((float)cr.y, (float)cr.x, (float)s.t3_kd[ab.x].x, (float)s.t3_kd[ab.y].x);
-      s.t5_pt[idx] = st.p_f4[j].x;
+      st_f4(s, s.t5_f, idx, make_float4((float)cr.y, (float)cr.x, (float)s.t3_kd[ab.x].x, (float)s.t3_kd[ab.y].x));
+      st_f(s, s.t5_pt, idx, st.p_f4[j].x);
     } else {
       // S0, same-seed rule (k_dedup.cu): the seed's minimum score, on the bit pattern of the non-negative double
       const double c2 = st.p_d2[j].x;

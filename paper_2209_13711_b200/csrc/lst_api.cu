@@ -90,7 +90,7 @@ extern "C" void lst_default_config(lst_config *c) {
   c->enum_pruning = 3;
   c->use_pdl = 1;
   c->batch_events = 1;
-  /* trunc_cap: all 0 (no occupancy truncation) */
+  /* trunc_cap: all 0 (no occupancy truncation); store_half: 0 */
 }
 
 static void make_params(const lst_config &c, Params *p) {
@@ -291,6 +291,8 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.cap_pt3 = capf(cf.cap_pt3_per_seed, nsd, 1024);
   s.cap_pt5 = capf(cf.cap_pt5_per_seed, nsd, 1024);
   s.cap_tc = s.cap_pt5 + s.cap_pt3 + s.cap_t5 + nsd;
+  s.half_store = cf.store_half != 0;
+  const auto hs = [&](size_t n) { return s.half_store ? (n + 1) / 2 : n; };   // elements of the fp32 type that hold n binary16 ones
   // ---- the zeroed region: header (after n_hits / n_seeds), histogram, incidence counters, flags, hash set
   s.hdr = w.take<Header>(1);
   const size_t zero_off = w.last + 2 * sizeof(uint32_t);
@@ -327,19 +329,19 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.tmp_key = w.take<float>(nh); s.hit_key = w.take<float>(nh);
   s.hit = w.take<float4>(nh); s.hit_orig = w.take<uint32_t>(nh);
   s.md_pos = w.take<float4>(s.cap_md); s.md_kd = w.take<double2>(s.cap_md); s.md_kf = w.take<float2>(s.cap_md);
-  s.md_hit = w.take<uint2>(s.cap_md); s.md_mod = w.take<uint32_t>(s.cap_md); s.md_dphi = w.take<float>(s.cap_md);
+  s.md_hit = w.take<uint2>(s.cap_md); s.md_mod = w.take<uint32_t>(s.cap_md); s.md_dphi = w.take<float>(hs(s.cap_md));
   s.md_phi = w.take<float>(s.cap_md); s.md_prel = w.take<float>(s.cap_md);
   s.md_mod_off = w.take<uint32_t>(n_mod + 1);
   s.mod_ev = w.take<ModEv>(n_mod);
   s.edge_col0 = w.take<uint32_t>(std::max<uint32_t>(c->map_edges_used, 1));
-  s.ls_md = w.take<uint2>(s.cap_ls); s.ls_f = w.take<float4>(s.cap_ls);
+  s.ls_md = w.take<uint2>(s.cap_ls); s.ls_f = w.take<float4>(hs(s.cap_ls));
   s.ls_md_off = w.take<uint32_t>((size_t)s.cap_md + 1);
   s.t3_md = w.take<uint4>(s.cap_t3); s.t3_ls = w.take<uint2>(s.cap_t3); s.t3_kd = w.take<double2>(s.cap_t3);
-  s.t3_beta = w.take<float>(s.cap_t3);
+  s.t3_beta = w.take<float>(hs(s.cap_t3));
   s.t3_md_off = w.take<uint32_t>((size_t)s.cap_md + 1);
   s.t5_md = w.take<uint32_t>(5 * (size_t)s.cap_t5); s.t5_t3 = w.take<uint2>(s.cap_t5);
   s.t5_chi2 = w.take<double>(s.cap_t5); s.t5_etaphi = w.take<double2>(s.cap_t5);
-  s.t5_f = w.take<float4>(s.cap_t5); s.t5_pt = w.take<float>(s.cap_t5); s.t5_keep = w.take<uint8_t>(s.cap_t5);
+  s.t5_f = w.take<float4>(hs(s.cap_t5)); s.t5_pt = w.take<float>(hs(s.cap_t5)); s.t5_keep = w.take<uint8_t>(s.cap_t5);
   s.t5_md_off = w.take<uint32_t>((size_t)s.cap_md + 1);
   s.pt5_po = w.take<uint2>(s.cap_pt5); s.pt3_po = w.take<uint2>(s.cap_pt3);
   s.pt5_chi2 = w.take<double>(s.cap_pt5); s.pt3_chi2 = w.take<double>(s.cap_pt3);

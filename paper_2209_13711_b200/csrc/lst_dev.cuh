@@ -19,6 +19,7 @@
 // launches serves up to kMaxBatch events, and every kernel starts with
 // griddepcontrol.wait so that the chain can be launched with programmatic dependent launch.
 #pragma once
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -234,7 +235,33 @@ struct SlotDev {
   uint32_t cap_hits, cap_seeds, cap_md, cap_ls, cap_t3, cap_t5, cap_pt3, cap_pt5, cap_tc;
   // export scratch
   uint32_t *exp_hits, *exp_par; float *exp_f;
+  // lst_config.store_half: the derived floats that no later decision reads
+  // (md_dphi, ls_f, t3_beta, t5_f, t5_pt) are stored as IEEE binary16; the arrays above then hold 2-byte
+  // elements (same pointers, half the bytes) and are accessed through ld_f / st_f / ld_f4 / st_f4
+  uint32_t half_store;
 };
+
+// A derived float (or float4) at index i of an array that holds fp32 or, with half_store, binary16 elements
+// (round to nearest; |v| above the binary16 range saturates to +-65504 instead of becoming infinite).
+__device__ __forceinline__ __half to_half_sat(float v) { return __float2half_rn(fminf(65504.0f, fmaxf(-65504.0f, v))); }
+__device__ __forceinline__ void st_f(const SlotDev &s, float *arr, size_t i, float v) {
+  if (s.half_store) reinterpret_cast<__half *>(arr)[i] = to_half_sat(v); else arr[i] = v;
+}
+__device__ __forceinline__ float ld_f(const SlotDev &s, const float *arr, size_t i) {
+  return s.half_store ? __half2float(reinterpret_cast<const __half *>(arr)[i]) : arr[i];
+}
+__device__ __forceinline__ void st_f4(const SlotDev &s, float4 *arr, size_t i, float4 v) {
+  if (s.half_store) {
+    const __half2 a = __halves2half2(to_half_sat(v.x), to_half_sat(v.y)), b = __halves2half2(to_half_sat(v.z), to_half_sat(v.w));
+    reinterpret_cast<uint2 *>(arr)[i] = make_uint2(*reinterpret_cast<const uint32_t *>(&a), *reinterpret_cast<const uint32_t *>(&b));
+  } else arr[i] = v;
+}
+__device__ __forceinline__ float4 ld_f4(const SlotDev &s, const float4 *arr, size_t i) {
+  if (!s.half_store) return arr[i];
+  const uint2 u = reinterpret_cast<const uint2 *>(arr)[i];
+  const float2 a = __half22float2(*reinterpret_cast<const __half2 *>(&u.x)), b = __half22float2(*reinterpret_cast<const __half2 *>(&u.y));
+  return make_float4(a.x, a.y, b.x, b.y);
+}
 
 // The slots (events) one chain of launches serves: a kernel's blocks with blockIdx.z = e work on
 // slot s[e].  Passed by value as a __grid_constant__ kernel parameter (CUDA >= 12.1 allows 32 KB).

@@ -767,3 +767,45 @@ def test_batched_chain_equals_single_slot_runs(B, geom_full, map_full, batch, pd
         fresh.lst_run_batch(1)
     fresh.close()
     lst.close()
+
+
+def test_reduced_precision_storage_changes_only_exported_floats(B, geom_full, map_full):
+    """lst_config.store_half keeps the derived floats that no later
+    decision reads as binary16.  Measured parity impact: every object, parent index, keep flag and TC
+    entry is identical to the fp32-storage run; the affected exported floats differ by at most 2^-11
+    relative (round to nearest; R saturates at 65504 cm), the others not at all; the workspace shrinks."""
+    ev = lstgen.make_event(geom_full, "cfg4")
+    sd = (ev.seed_pt, ev.seed_eta, ev.seed_phi, ev.seed_z0, ev.seed_q, ev.seed_hit_ids)
+    runs = []
+    for half in (0, 1):
+        cfg = B.lst_default_config()
+        cfg.store_half = half
+        lst = B.LST(geom_full, map_full[0], map_full[1], cfg=cfg, n_slots=1, max_hits=ev.n_hits, max_seeds=ev.n_seeds)
+        lst.lst_load_event(0, ev.x, ev.y, ev.z, ev.det, sd)
+        lst.lst_run(0)
+        runs.append(([lst.lst_get_objects(0, lvl) for lvl in range(7)], lst.workspace_bytes))
+        lst.close()
+    (full, ws_full), (half, ws_half) = runs
+    assert ws_half < ws_full
+    # columns of `f` stored in binary16 per level: MD dphi; LS all; T3 beta; T5 all; TC pt of the T5-type entries
+    half_cols = {O.MD: [0], O.LS: [0, 1, 2], O.T3: [0], O.T5: [0, 1, 2, 3], O.PT3: [], O.PT5: [], O.TC: [0]}
+    worst = 0.0
+    for lvl in range(7):
+        a, b = full[lvl], half[lvl]
+        assert np.array_equal(a["hits"], b["hits"]) and np.array_equal(a["parents"], b["parents"]) and len(a["hits"]) > 100
+        if a["keep"] is not None:
+            assert np.array_equal(a["keep"], b["keep"])
+        for c in range(4):
+            x, y = a["f"][:, c].astype(np.float64), b["f"][:, c].astype(np.float64)
+            if c not in half_cols[lvl]:
+                assert np.array_equal(x, y), (lvl, c)
+                continue
+            sat = np.abs(x) > 65504.0
+            assert np.all(np.abs(y[sat]) == 65504.0)
+            big = (np.abs(x) >= 6.2e-5) & ~sat                     # binary16 normal range
+            rel = np.abs(x - y)[big] / np.abs(x[big])
+            assert rel.size == 0 or rel.max() <= 2.0 ** -11 * 1.0001, (lvl, c, rel.max())
+            assert np.all(np.abs(x - y)[~big & ~sat] <= 2.0 ** -25)  # subnormal spacing 2^-24
+            worst = max(worst, float(rel.max()) if rel.size else 0.0)
+    assert 1e-4 < worst <= 2.0 ** -11 * 1.0001
+    print("store_half: workspace %.1f -> %.1f MB, largest relative change of an exported float %.2e" % (ws_full / 1e6, ws_half / 1e6, worst))
