@@ -100,6 +100,13 @@ typedef struct {
                               in the slot workspace (half the bytes; relative error <= 4.9e-4, values above
                               65504 saturate) and widened again by lst_get_objects.  Object sets, keep flags
                               and the TC list are unchanged: every decision uses the fp64 quantities. */
+  int32_t s0_fixpoint_passes; /* 0 (default): the non-greedy cleaning rule S0 (an object is removed iff SOME
+                              better duplicate exists).  P = 2, 4, .. 16: S0 of the T5 collection is iterated
+                              P more times towards the greedy fix-point "kept iff no KEPT better duplicate"
+                              (cleaning of PAPER.md:77-83), which keeps every T5 the non-greedy
+                              rule keeps plus those that lost only to removed objects.  After an even number of
+                              passes the kept set is a duplicate-free subset of the fix-point, equal to it when
+                              lst_get_fixpoint_unsettled reports 0 (8 passes on the 6 000-particle, 12 on the 13 500-particle synthetic events). */
 } lst_config;
 
 /* Detector description, HOST arrays of length n_modules (copied by the callee).  A module is a
@@ -219,6 +226,10 @@ int lst_run(lst_ctx *ctx, uint32_t slot, void *cuda_stream);
  * lst_run.  LST_ESTATE if a slot of the group has no workspace or no event. */
 int lst_run_batch(lst_ctx *ctx, uint32_t group, void *cuda_stream);
 uint32_t lst_batch_events(const lst_ctx *ctx);
+
+/* Number of T5 whose keep flag still changed in the last fix-point pass of the slot's last run
+ * (lst_config.s0_fixpoint_passes > 0); 0 = the greedy fix-point was reached exactly. */
+int lst_get_fixpoint_unsettled(lst_ctx *ctx, uint32_t slot, uint32_t *n_unsettled);
 
 /* Synchronise the slot's stream and return a view of one level.  LST_ENOMEM if a collection
  * overflowed its capacity, LST_EINVAL if the event was invalid (see lst_load_event). */

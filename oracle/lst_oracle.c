@@ -61,6 +61,7 @@ struct lsto_ctx {
   VEC(tc_t) tc;
   float *phic;                       /* [n_modules] module centre azimuth: set by lsto_set_truncation (azimuth order) */
   uint32_t trunc[6][16];             /* occupancy caps per level and logical layer (0 = none)                         */
+  int s0_fixpoint;                   /* lsto_set_s0_fixpoint: greedy (fix-point) S0 for the T5 collection              */
   uint32_t *md_mod_off;              /* [n_modules+1] MD range of a module          */
   uint32_t *ls_md_off;               /* [n_md+1]      LS range of an inner MD       */
   uint32_t *t3_md_off;               /* [n_md+1]      T3 range of a first MD        */
@@ -954,6 +955,49 @@ static void s0_clean(const lsto_ctx *c, const dobj_t *o, uint32_t n, int min_sha
   }
 }
 
+/* S0, fix-point variant (SURVEY.md 8(f)3 "iterated dedup"; cleaning of PAPER.md:77-83).  The non-greedy
+ * rule removes a when SOME better duplicate b exists, even a b that is itself removed by a still better c
+ * that a does not overlap: a is lost for nothing.  The fix-point is the greedy definition: take the objects
+ * from the best to the worst ("beats" is a strict total order); an object is kept iff no KEPT object is a
+ * duplicate of it (shares >= min_shared OT hits).  Every kept object of the non-greedy rule is kept here
+ * too.  Applied to the T5 collection (lsto_set_s0_fixpoint); the pixel-seeded collections keep the
+ * non-greedy rule, whose same-seed clause already leaves one object per seed. */
+static const lsto_ctx *g_sort_ctx;
+static const dobj_t *g_sort_obj;
+static int cmp_beats(const void *pa, const void *pb) {
+  uint32_t a = *(const uint32_t *)pa, b = *(const uint32_t *)pb;
+  if (a == b) return 0;
+  return beats(g_sort_ctx, &g_sort_obj[a], &g_sort_obj[b]) ? -1 : 1;
+}
+static void s0_fixpoint(const lsto_ctx *c, const dobj_t *o, uint32_t n, int min_shared, uint8_t *keep) {
+  for (uint32_t i = 0; i < n; ++i) keep[i] = 1;
+  if (!c->cfg.s0_enabled || n == 0) return;
+  uint32_t *order = malloc((size_t)n * 4), *rank = malloc((size_t)n * 4);
+  for (uint32_t i = 0; i < n; ++i) order[i] = i;
+  g_sort_ctx = c; g_sort_obj = o;
+  qsort(order, n, 4, cmp_beats);
+  for (uint32_t r = 0; r < n; ++r) rank[order[r]] = r;
+  uint32_t nh = c->n_hits;
+  uint32_t *off = calloc((size_t)nh + 2, 4);
+  for (uint32_t a = 0; a < n; ++a) for (int k = 0; k < o[a].n_ot; ++k) off[o[a].ot[k] + 1]++;
+  for (uint32_t h = 0; h < nh; ++h) off[h + 1] += off[h];
+  uint32_t *lst = malloc(((size_t)off[nh] + 1) * 4), *fill = malloc(((size_t)nh + 1) * 4);
+  memcpy(fill, off, ((size_t)nh + 1) * 4);
+  for (uint32_t a = 0; a < n; ++a) for (int k = 0; k < o[a].n_ot; ++k) lst[fill[o[a].ot[k]]++] = a;
+  for (uint32_t r = 0; r < n; ++r) {                     /* best first: every better object is already decided */
+    uint32_t a = order[r];
+    for (int k = 0; k < o[a].n_ot && keep[a]; ++k) {
+      uint32_t h = o[a].ot[k];
+      for (uint32_t e = off[h]; e < off[h + 1]; ++e) {
+        uint32_t b = lst[e];
+        if (b != a && rank[b] < r && keep[b] && shared_ot(&o[a], &o[b]) >= min_shared) { keep[a] = 0; break; }
+      }
+    }
+  }
+  free(order); free(rank); free(off); free(lst); free(fill);
+}
+int lsto_set_s0_fixpoint(lsto_ctx *c, int on) { if (!c) return -1; c->s0_fixpoint = on != 0; return 0; }
+
 int lsto_dedup(lsto_ctx *c, int brute) {
   uint32_t n5 = c->t5.n, np5 = c->pt5.n, np3 = c->pt3.n, ns = c->n_seeds;
   free(c->keep_t5); free(c->keep_pt3); free(c->keep_pt5); free(c->keep_pls);
@@ -966,7 +1010,8 @@ int lsto_dedup(lsto_ctx *c, int brute) {
   for (uint32_t i = 0; i < np3; ++i) op3[i] = dobj_px(c, &c->pt3.v[i], 0);
   double m = INFINITY;
   /* S0 intra-collection */
-  s0_clean(c, o5, n5, c->cfg.dup_t5_shared, 0, brute, c->keep_t5);
+  if (c->s0_fixpoint && !brute) s0_fixpoint(c, o5, n5, c->cfg.dup_t5_shared, c->keep_t5);
+  else s0_clean(c, o5, n5, c->cfg.dup_t5_shared, 0, brute, c->keep_t5);
   s0_clean(c, op5, np5, c->cfg.dup_pt5_shared, 1, brute, c->keep_pt5);
   s0_clean(c, op3, np3, c->cfg.dup_pt3_shared, 1, brute, c->keep_pt3);
   /* S1: pT3 vs pT5 (both S0 survivors) */

@@ -95,6 +95,9 @@ int lsto_link_pixel(lsto_ctx *c, uint32_t seed_begin, uint32_t seed_end); /* pT5
 /* the same pairs through a per-module first-anchor window (identical output; see the .c file) */
 int lsto_link_pixel_indexed(lsto_ctx *c, uint32_t seed_begin, uint32_t seed_end);
 int lsto_dedup(lsto_ctx *c, int brute);                                   /* S0-S4 -> TC    */
+/* S0 of the T5 collection as a fix-point (greedy from the best object down: kept iff no KEPT object is a
+ * duplicate) instead of the non-greedy rule; see the .c file.  Ignored by the brute mode. */
+int lsto_set_s0_fixpoint(lsto_ctx *c, int on);
 
 uint32_t lsto_count(const lsto_ctx *c, int level);
 /* copy-out: any pointer may be NULL.  hit_idx: n*arity original hit indices in layer order

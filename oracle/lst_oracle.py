@@ -59,6 +59,7 @@ def lib():
         L.lsto_destroy.argtypes = [vp]
         L.lsto_load_event.argtypes = [vp, u32, vp, vp, vp, vp, u32, vp, vp, vp, vp, vp, vp]
         L.lsto_set_truncation.argtypes = [vp, vp, vp]
+        L.lsto_set_s0_fixpoint.argtypes = [vp, i32]
         L.lsto_build_md.argtypes = [vp]
         for f in ("lsto_build_ls", "lsto_build_t3", "lsto_build_t5", "lsto_dedup"):
             getattr(L, f).argtypes = [vp, i32]
@@ -139,6 +140,10 @@ class Oracle:
         cp = np.ascontiguousarray(caps, dtype=np.uint32).reshape(6, 16) if caps is not None else None
         rc = lib().lsto_set_truncation(self._h, _p(ph), _p(cp) if cp is not None else None)
         assert rc == 0
+
+    def set_s0_fixpoint(self, on=True):
+        """Greedy (fix-point) S0 for the T5 collection instead of the non-greedy rule."""
+        assert lib().lsto_set_s0_fixpoint(self._h, int(on)) == 0
 
     def load(self, ev):
         f = lambda a, dt: np.ascontiguousarray(a, dtype=dt)

@@ -22,7 +22,7 @@ LEVEL_NAMES = ("MD", "LS", "T3", "T5", "PT3", "PT5", "TC")
 
 EXPORTS = ("lst_default_config", "lst_build_module_map", "lst_free", "lst_create", "lst_destroy",
            "lst_workspace_bytes", "lst_bind_workspace", "lst_load_event", "lst_run", "lst_get_objects",
-           "lst_get_counts", "lst_launches_per_run", "lst_run_timed", "lst_strerror", "lst_run_batch", "lst_batch_events")
+           "lst_get_counts", "lst_launches_per_run", "lst_run_timed", "lst_strerror", "lst_run_batch", "lst_batch_events", "lst_get_fixpoint_unsettled")
 TEST_EXPORTS = ("lst_host_eval", "lst_host_ls_window")      # include/lst_test.h
 
 
@@ -38,7 +38,7 @@ class lst_config(C.Structure):
             "cap_pt5_per_seed", "cap_mdcand_per_hit", "cap_lscand_per_hit", "cap_t3cand_per_hit",
             "cap_t5cand_per_hit")] + [("use_cuda_graph", C.c_int32), ("enum_pruning", C.c_int32), ("use_pdl", C.c_int32),
                                    ("batch_events", C.c_int32), ("trunc_cap", (C.c_uint32 * 16) * 6),
-                                   ("store_half", C.c_int32)]
+                                   ("store_half", C.c_int32), ("s0_fixpoint_passes", C.c_int32)]
 
 
 class lst_geometry(C.Structure):
@@ -101,6 +101,7 @@ def lib():
         L.lst_run_batch.argtypes = [vp, u32, vp]
         L.lst_batch_events.argtypes = [vp]
         L.lst_batch_events.restype = u32
+        L.lst_get_fixpoint_unsettled.argtypes = [vp, u32, C.POINTER(u32)]
         L.lst_get_objects.argtypes = [vp, u32, C.c_int, C.c_int, C.POINTER(lst_objects)]
         L.lst_get_counts.argtypes = [vp, u32, vp, vp]
         L.lst_launches_per_run.argtypes = [vp]
@@ -257,6 +258,11 @@ class LST:
 
     def lst_run_batch(self, group, stream=None):
         _check(lib().lst_run_batch(self._h, group, self._stream_ptr(stream)), "lst_run_batch")
+
+    def lst_get_fixpoint_unsettled(self, slot):
+        n = C.c_uint32(0)
+        _check(lib().lst_get_fixpoint_unsettled(self._h, slot, C.byref(n)), "lst_get_fixpoint_unsettled")
+        return int(n.value)
 
     def lst_run_timed(self, slot, stream=None):
         """-> list of (kernel name, ms) of one un-graphed, event-bracketed pass of the chain."""

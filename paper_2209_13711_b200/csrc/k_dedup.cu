@@ -188,13 +188,22 @@ __device__ __forceinline__ void pls_best_body(const SlotDev &s, uint32_t n5, uin
 constexpr int kS0Slots = 128;
 constexpr uint32_t kNoHit = 0xFFFFFFFFu;
 constexpr uint32_t kS0Light = 64;   // entries an 8-lane group looks at before it hands a longer object to k_s0_heavy
-__global__ void __launch_bounds__(128) k_s0(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
+//
+// pass > 0 (lst_config.s0_fixpoint_passes): a pass of the fix-point iteration of the T5 collection.  The
+// non-greedy rule (pass 0) keeps L1 = {no better duplicate at all}; pass p keeps {no better duplicate
+// among the objects kept by pass p - 1}.  The passes alternate between subsets (even p) and supersets
+// (odd p) of the greedy fix-point "kept iff no KEPT better duplicate" and meet it after a few steps; the
+// flags of pass p - 1 are read from one of two buffers (t5_keep, t5_keep2), those of pass p go to the other.
+__global__ void __launch_bounds__(128) k_s0(const __grid_constant__ Batch B, const __grid_constant__ Params g, int pass,
+                                            int last_pass) {
   __shared__ uint32_t sh_pre[16][12], sh_beg[16][12];
   __shared__ uint32_t sh_tab[16][kS0Slots];
   pdl_enter();
   LST_SLOT(B);
   Header *hdr = s.hdr;
   const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_dd = n5 + np5 + hdr->n_obj[4];
+  const uint8_t *alive = pass == 0 ? nullptr : ((pass & 1) ? s.t5_keep : s.t5_keep2);     // flags of the previous pass
+  uint8_t *t5_out = (pass & 1) ? s.t5_keep2 : s.t5_keep;
   const int lane = threadIdx.x & 31, gl = lane & 7, gbase = lane & ~7, gid = threadIdx.x >> 3;
   const uint32_t gmask = 0xFFu << gbase;
   const uint32_t group = (blockIdx.x * blockDim.x + threadIdx.x) >> 3, ngroup = (gridDim.x * blockDim.x) >> 3;
@@ -205,14 +214,14 @@ __global__ void __launch_bounds__(128) k_s0(const __grid_constant__ Batch B, con
   // says, so the others are flagged here and the search below runs on the T5 and on the seeds' best
   // objects only (work index: [0, n5) T5, then per seed its best pT5, then per seed its best pT3).
   const uint32_t n_seeds = hdr->n_seeds;
-  if (g.s0_enabled) {
+  if (g.s0_enabled && pass == 0) {
     const uint32_t np3 = hdr->n_obj[4];
     for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < np5 + np3; j += gridDim.x * blockDim.x) {
       if (j < np5) { if (s.pls_best5[s.pt5_po[j].x] != j) s.pt5_keep[j] = 0; }
       else { const uint32_t i = j - np5; if (s.pls_best3[s.pt3_po[i].x] != i) s.pt3_keep[i] = 0; }
     }
   }
-  const uint32_t n_work = g.s0_enabled ? n5 + 2u * n_seeds : n_dd;
+  const uint32_t n_work = pass ? n5 : (g.s0_enabled ? n5 + 2u * n_seeds : n_dd);
   for (uint32_t wk = group;; wk += ngroup) {
     if (!__any_sync(0xffffffffu, wk < n_work)) break;
     uint32_t d = wk;
@@ -276,7 +285,7 @@ __global__ void __launch_bounds__(128) k_s0(const __grid_constant__ Batch B, con
         if (active && i < total) {
           while (i >= pre[cur + 1]) ++cur;
           const uint32_t b = s.inc_ent[beg[cur] + (i - pre[cur])];
-          if (b != d && !(score_arr[b - dbase] > A.score)) {
+          if (b != d && !(score_arr[b - dbase] > A.score) && (alive == nullptr || alive[b])) {
             int cnt;
             if (!collide) {
               const uint32_t *hb = A.type == 0 ? s.t5_hits + 10 * (size_t)b
@@ -310,10 +319,13 @@ __global__ void __launch_bounds__(128) k_s0(const __grid_constant__ Batch B, con
       if (h1 != kNoHit) tab[slot1] = kNoHit;
       __syncwarp();
     }
-    if (valid && gl == 0 && defer && !beaten) s.tc_pos[atomicAdd(&hdr->n_heavy, 1u)] = d;
+    if (valid && gl == 0 && defer && !beaten) s.tc_pos[atomicAdd(&hdr->n_heavy[pass], 1u)] = d;
     if (valid && gl == 0 && !(defer && !beaten)) {
       const bool keep = !beaten;
-      if (A.type == 0) s.t5_keep[A.idx] = keep;
+      if (A.type == 0) {
+        t5_out[A.idx] = keep;
+        if (last_pass && alive && (alive[A.idx] != 0) != keep) atomicAdd(&hdr->n_unsettled, 1u);
+      }
       else if (A.type == 1) {
         s.pt5_keep[A.idx] = keep;
         if (keep) {
@@ -331,19 +343,22 @@ __global__ void __launch_bounds__(128) k_s0(const __grid_constant__ Batch B, con
 // the objects that survive): one BLOCK per object over the whole flattened list (a hit of a |eta| ~ 0
 // seed's objects is shared by thousands of pT3: the longest lists set the duration, so they get 128
 // lanes), objects handed out dynamically.  Warp 0 sets the object up, all warps stride the list.
-__global__ void __launch_bounds__(128) k_s0_heavy(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
+__global__ void __launch_bounds__(128) k_s0_heavy(const __grid_constant__ Batch B, const __grid_constant__ Params g, int pass,
+                                                  int last_pass) {
   __shared__ uint32_t pre[12], beg[12];
   __shared__ uint32_t tab[256];
   __shared__ uint32_t sh_hv, sh_collide;
   pdl_enter();
   LST_SLOT(B);
   const Header *hdr = s.hdr;
-  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_heavy = hdr->n_heavy;
+  const uint32_t n5 = hdr->n_obj[3], np5 = hdr->n_obj[5], n_heavy = hdr->n_heavy[pass];
+  const uint8_t *alive = pass == 0 ? nullptr : ((pass & 1) ? s.t5_keep : s.t5_keep2);
+  uint8_t *t5_out = (pass & 1) ? s.t5_keep2 : s.t5_keep;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   for (int k = threadIdx.x; k < 256; k += blockDim.x) tab[k] = 0xFFFFFFFFu;
   for (;;) {
     __syncthreads();                                            // the previous object is done with the shared arrays
-    if (threadIdx.x == 0) sh_hv = atomicAdd(&s.hdr->next_unit[S_T5], 1u);
+    if (threadIdx.x == 0) sh_hv = atomicAdd(&s.hdr->heavy_next[pass], 1u);
     __syncthreads();
     const uint32_t hv = sh_hv;
     if (hv >= n_heavy) break;
@@ -394,7 +409,7 @@ __global__ void __launch_bounds__(128) k_s0_heavy(const __grid_constant__ Batch 
         if (i < total) {
           while (i >= pre[cur + 1]) ++cur;
           const uint32_t b = s.inc_ent[beg[cur] + (i - pre[cur])];
-          if (b != d && !(score_arr[b - dbase] > A.score)) {
+          if (b != d && !(score_arr[b - dbase] > A.score) && (alive == nullptr || alive[b])) {
             int cnt;
             if (!collide) {
               const uint32_t *hb = A.type == 0 ? s.t5_hits + 10 * (size_t)b
@@ -428,7 +443,10 @@ __global__ void __launch_bounds__(128) k_s0_heavy(const __grid_constant__ Batch 
     }
     if (threadIdx.x == 0) {
       const bool keep = !beaten;
-      if (A.type == 0) s.t5_keep[A.idx] = keep;
+      if (A.type == 0) {
+        t5_out[A.idx] = keep;
+        if (last_pass && alive && (alive[A.idx] != 0) != keep) atomicAdd(&s.hdr->n_unsettled, 1u);
+      }
       else if (A.type == 1) {
         s.pt5_keep[A.idx] = keep;
         if (keep) {
@@ -618,8 +636,13 @@ void launch_dedup(const Ctx &c, const Batch &b, cudaStream_t st) {
   launch_k(c, st, "k_dd_count", k_dd_count, dim3(grid_of(cap_dd, 256, c.n_sm * 8)), 256, 0, false, b, c.par);
   launch_scan(c, b, 0, st);
   launch_k(c, st, "k_dd_scatter", k_dd_scatter, dim3(grid_of(cap_dd, 256, c.n_sm * 8)), 256, 0, false, b);
-  launch_k(c, st, "k_s0", k_s0, dim3(grid_of(cap_dd, 16, c.n_sm * 16)), 128, 0, false, b, c.par);
-  launch_k(c, st, "k_s0_heavy", k_s0_heavy, dim3(grid_of(cap_dd, 4, c.n_sm * 16)), 128, 0, false, b, c.par);
+  for (int pass = 0; pass <= c.fix_passes; ++pass) {      // pass 0: the non-greedy rule; further passes: T5 fix-point iteration
+    const int last = pass == c.fix_passes;
+    const uint32_t n_obj = pass ? s.cap_t5 : cap_dd;
+    launch_k(c, st, pass ? "k_s0[fix]" : "k_s0", k_s0, dim3(grid_of(n_obj, 16, c.n_sm * 16)), 128, 0, false, b, c.par, pass, last);
+    launch_k(c, st, pass ? "k_s0_heavy[fix]" : "k_s0_heavy", k_s0_heavy, dim3(grid_of(n_obj, 4, c.n_sm * 16)), 128, 0, false, b,
+             c.par, pass, last);
+  }
   launch_k(c, st, "k_s1", k_s1, dim3(grid_of(s.cap_pt3, 128, c.n_sm * 16)), 128, 0, false, b);
   launch_k(c, st, "k_s2", k_s2, dim3(grid_of(s.cap_t5, 128, c.n_sm * 8)), 128, 0, false, b, c.par);
   launch_k(c, st, "k_s3_flags", k_s3_flags, dim3(kFlagBlocks), 256, 0, false, b);

@@ -341,7 +341,7 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.t3_md_off = w.take<uint32_t>((size_t)s.cap_md + 1);
   s.t5_md = w.take<uint32_t>(5 * (size_t)s.cap_t5); s.t5_t3 = w.take<uint2>(s.cap_t5);
   s.t5_chi2 = w.take<double>(s.cap_t5); s.t5_etaphi = w.take<double2>(s.cap_t5);
-  s.t5_f = w.take<float4>(hs(s.cap_t5)); s.t5_pt = w.take<float>(hs(s.cap_t5)); s.t5_keep = w.take<uint8_t>(s.cap_t5);
+  s.t5_f = w.take<float4>(hs(s.cap_t5)); s.t5_pt = w.take<float>(hs(s.cap_t5)); s.t5_keep = w.take<uint8_t>(s.cap_t5); s.t5_keep2 = w.take<uint8_t>(s.cap_t5);
   s.t5_md_off = w.take<uint32_t>((size_t)s.cap_md + 1);
   s.pt5_po = w.take<uint2>(s.cap_pt5); s.pt3_po = w.take<uint2>(s.cap_pt3);
   s.pt5_chi2 = w.take<double>(s.cap_pt5); s.pt3_chi2 = w.take<double>(s.cap_pt3);
@@ -491,6 +491,8 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   make_params(c->cfg, &c->k.par);
   c->k.ls_windows = (c->cfg.enum_pruning & 2) != 0;
   c->k.pdl = c->cfg.use_pdl != 0;
+  if (c->cfg.s0_fixpoint_passes < 0 || c->cfg.s0_fixpoint_passes > kMaxFixPasses || (c->cfg.s0_fixpoint_passes & 1)) { delete c; return einval(); }
+  c->k.fix_passes = c->cfg.s0_fixpoint_passes;
   {
     // stages with an occupancy cap: MD, LS, T3, T5 per logical layer; pT3 / pT5 per seed ([level][0])
     const int stage_of_level[6] = {S_MD, S_LS, S_T3, S_T5, S_PT3, S_PT5};
@@ -797,6 +799,17 @@ extern "C" int lst_run_batch(lst_ctx *c, uint32_t group, void *cuda_stream) {
 }
 
 extern "C" uint32_t lst_batch_events(const lst_ctx *c) { return c ? c->batch : 0; }
+
+static int sync_header(lst_ctx *c, Slot &s);
+extern "C" int lst_get_fixpoint_unsettled(lst_ctx *c, uint32_t slot, uint32_t *n) {
+  if (!c || slot >= c->n_slots || !n) return einval();
+  Slot &s = c->slots[slot];
+  if (!s.ran) return LST_ESTATE;
+  const int rc = sync_header(c, s);
+  if (rc != LST_OK) return rc;
+  *n = s.h_hdr->n_unsettled;
+  return LST_OK;
+}
 
 // ------------------------------------------------------------------ results
 static int sync_header(lst_ctx *c, Slot &s) {

@@ -32,6 +32,7 @@ constexpr int kItemWords = kItemCand / 32;
 constexpr int kThreads = 128;            // threads per block of eval / fill kernels
 constexpr int kMaxRpi = 128;             // max rows per item
 constexpr int kMaxBatch = 8;             // events (slots) one chain of launches can serve
+constexpr int kMaxFixPasses = 16;        // lst_config.s0_fixpoint_passes (even, <= this)
 constexpr int kRowChunk = 128;           // rows per group in the variable-width stages (T3, T5, pixel)
 constexpr int kMaxDeg = 512;             // maximum module-map degree (checked by lst_create)
 constexpr int kPxCap = 64;               // (seed, start module) rows per pixel seed ON AVERAGE (overflow -> LST_ENOMEM)
@@ -87,7 +88,9 @@ struct Header {          // per slot, device; everything after n_seeds is zeroed
   uint32_t cl_used[S_NSTAGE];        // pre-filter survivors appended to the stage's candidate list
   uint32_t err;
   uint32_t n_inc;                    // 3 * n_hits: rows of the (hit, object type) -> objects incidence
-  uint32_t n_heavy;                  // objects k_s0 handed to k_s0_heavy (listed in tc_pos, free until S3)
+  uint32_t n_heavy[kMaxFixPasses + 1];     // per S0 pass: objects k_s0 handed to k_s0_heavy (listed in tc_pos, free until S3)
+  uint32_t heavy_next[kMaxFixPasses + 1];  // ... and the next one to hand out
+  uint32_t n_unsettled;              // T5 whose flag still changed in the last fix-point pass (0: the fix-point was reached)
   uint32_t flag_chunk;               // keep flags per block of k_s3_flags / k_tc_fill
   uint32_t ticket[TK_N];             // blocks that finished (last_block)
   unsigned long long cand[S_NSTAGE]; // candidates of the method's definition per stage (rows x connected columns)
@@ -193,6 +196,7 @@ struct SlotDev {
   float4 *t5_f;          // R, chi2, k3a, k3b
   float *t5_pt;
   uint8_t *t5_keep;
+  uint8_t *t5_keep2;     // second flag buffer of the S0 fix-point passes
   uint32_t *t5_md_off;   // [cap_md+1] T5 range of a first MD
   // pixel-seeded
   uint2 *pt5_po, *pt3_po;          // pls, obj

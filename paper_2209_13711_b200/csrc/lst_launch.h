@@ -9,7 +9,7 @@ namespace lst {
 // Launch recorder: counts the kernels a chain enqueues and, when `timed`, drops a CUDA event after
 // each one so that lst_run_timed can report per-kernel durations (bench.py, profiles/).
 struct Recorder {
-  static constexpr int kMax = 64;
+  static constexpr int kMax = 96;
   bool timed = false;
   int n = 0;
   const char *name[kMax];
@@ -24,6 +24,7 @@ struct Ctx {             // what the launchers need from a context
   int ls_windows = 1;    // lst_config.enum_pruning bit 1: per-row windows of the LS enumeration
   int pdl = 0;           // launch with programmatic stream serialisation (lst_config.use_pdl)
   int nb = 1;            // slots (events) in the batch: gridDim.z of every launch
+  int fix_passes = 0;    // lst_config.s0_fixpoint_passes: extra S0 passes over the T5 collection
   unsigned trunc_stages = 0;   // bit k: stage k has an occupancy cap (k_truncate runs before its k_counts)
 };
 

@@ -809,3 +809,36 @@ def test_reduced_precision_storage_changes_only_exported_floats(B, geom_full, ma
             worst = max(worst, float(rel.max()) if rel.size else 0.0)
     assert 1e-4 < worst <= 2.0 ** -11 * 1.0001
     print("store_half: workspace %.1f -> %.1f MB, largest relative change of an exported float %.2e" % (ws_full / 1e6, ws_half / 1e6, worst))
+
+
+@pytest.mark.parametrize("cfg_name,passes", [("cfg4", 8), ("cfg3", 8)])
+def test_s0_fixpoint_passes_match_the_oracle_fixpoint(B, geom_full, map_full, cfg_name, passes):
+    """lst_config.s0_fixpoint_passes iterates S0 of the T5 collection to the greedy
+    fix-point; keep flags of every collection and the TC list equal the oracle's fix-point mode, the
+    iteration has converged (0 unsettled objects), and the non-greedy survivors are a strict subset."""
+    ev = lstgen.make_event(geom_full, cfg_name)
+    sd = (ev.seed_pt, ev.seed_eta, ev.seed_phi, ev.seed_z0, ev.seed_q, ev.seed_hit_ids) if ev.n_seeds else None
+    o = O.Oracle(geom_full, map_full[0], map_full[1])
+    o.set_s0_fixpoint(True)
+    o.load(ev)
+    o.run(upto=O.TC, pixel_indexed=True)
+    keeps = {}
+    for p in (0, passes):
+        cfg = B.lst_default_config()
+        cfg.s0_fixpoint_passes = p
+        lst = B.LST(geom_full, map_full[0], map_full[1], cfg=cfg, n_slots=1, max_hits=ev.n_hits, max_seeds=max(ev.n_seeds, 1))
+        for rep in range(2):                    # second run: graph replay on a used slot
+            lst.lst_load_event(0, ev.x, ev.y, ev.z, ev.det, sd)
+            lst.lst_run(0)
+        keeps[p] = lst.lst_get_objects(0, O.T5)["keep"].copy()
+        if p:
+            assert lst.lst_get_fixpoint_unsettled(0) == 0
+            diff = {lvl: differing(o, lst, lvl) for lvl in ALL_LEVELS}
+            assert not any(diff.values()), "this event has no near-threshold object"
+            assert compare_cleaning(o, _SlotView(lst, 0), ev) > 100
+        lst.close()
+    assert np.all(keeps[passes][keeps[0]]) and keeps[passes].sum() > keeps[0].sum() > 100
+    with pytest.raises(B.LstError):             # odd or too many passes are refused by lst_create
+        cfg = B.lst_default_config()
+        cfg.s0_fixpoint_passes = 3
+        B.LST(geom_full, map_full[0], map_full[1], cfg=cfg, n_slots=1, max_hits=1000, max_seeds=10)

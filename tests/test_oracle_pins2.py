@@ -881,3 +881,66 @@ def test_pixel_linking_indexed_equals_all_pairs(geom_full, map_full):
         assert len(ga["parents"]) > 200
         assert np.array_equal(ga["parents"], gb["parents"]) and np.array_equal(ga["f"], gb["f"])
         assert np.array_equal(ga["margin"], gb["margin"])
+
+
+# ----------------------------------------------------------------------------- S0 as a fix-point
+def test_s0_fixpoint_recovers_what_lost_only_to_removed_objects(geom_barrel, map_barrel):
+    """The chain of test_s0_t5_needs_five_of_ten_shared_hits: C beats B5, B5 beats A, C and A share
+    nothing.  Non-greedy: A and B5 removed.  Fix-point (greedy from the best down): B5 is removed by C,
+    so nothing that is KEPT duplicates A: A comes back."""
+    H = Hand(geom_barrel, map_barrel)
+    md = _mds(20, extra=[(2, 101)])
+    A, B5, C = (0, 1, 2, 3, 4), (0, 1, 20, 13, 14), (5, 6, 20, 13, 14)
+    kin = lambda c, e: (c, 1.0, e, 0.0)
+    kw = dict(md_hits=md, t5_md=[A, B5, C], t5_kin=[kin(5.0, 0.0), kin(3.0, 1.0), kin(1.0, 2.0)])
+    H.o.inject(**kw); H.o.dedup()
+    assert H.o.keep(O.T5).tolist() == [0, 0, 1]
+    H.o.set_s0_fixpoint(True)
+    H.o.inject(**kw); H.o.dedup()
+    assert H.o.keep(O.T5).tolist() == [1, 0, 1]
+    # a longer chain D > C > B5 > A (D shares 5 hits with C only): C goes, B5 comes back, A goes again
+    D = (5, 6, 7, 8, 9)
+    md2 = _mds(20, extra=[(2, 101), (7, 103)])        # MD 21 = lower hit of MD 7
+    C2 = (5, 6, 21, 13, 14)                           # shares MDs 5, 6 and the lower hit of MD 7 (via MD 21) with D: 5 hits
+    B6 = (0, 6, 20, 13, 14)                           # shares MDs 6, 13, 14 with C2: 6 hits; nothing with D beyond MD 6 (2 hits)
+    A2 = (0, 20, 2, 3, 4)                             # shares MDs 0, 20 and the lower hit of MD 2 (in MD 20) with B6: 5 hits
+    kw = dict(md_hits=md2, t5_md=[A2, B6, C2, D], t5_kin=[kin(7.0, 0.0), kin(5.0, 1.0), kin(3.0, 2.0), kin(1.0, 3.0)])
+    H.o.set_s0_fixpoint(False)
+    H.o.inject(**kw); H.o.dedup()
+    assert H.o.keep(O.T5).tolist() == [0, 0, 0, 1]
+    H.o.set_s0_fixpoint(True)
+    H.o.inject(**kw); H.o.dedup()
+    assert H.o.keep(O.T5).tolist() == [0, 1, 0, 1]
+
+
+def test_s0_fixpoint_equals_a_numpy_greedy_and_contains_the_non_greedy_survivors(geom_full, map_full):
+    """On a full-detector event: the fix-point flags equal a plain Python greedy (objects by ascending
+    chi2, kept iff no kept earlier object shares >= 5 hits) typed here, and are a superset of the
+    non-greedy S0 survivors.  S1-S3 are switched off by having no pixel seeds (config 3)."""
+    ev = lstgen.make_event(geom_full, "cfg3")
+    flags = {}
+    for fx in (False, True):
+        o = O.Oracle(geom_full, map_full[0], map_full[1])
+        o.set_s0_fixpoint(fx)
+        o.load(ev)
+        o.run(upto=O.TC)
+        flags[fx] = o.keep(O.T5)
+        t5 = o.get(O.T5)
+    assert np.all(flags[True][flags[False]]) and flags[True].sum() > flags[False].sum() > 100
+    chi2 = t5["f"][:, 1]
+    # "b beats a" (reading 15): the score, then - T5 that differ only in upper hits have identical anchors, hence
+    # identical chi2 - the hit coordinates in layer order, then the hit indices
+    x, y, z = (np.asarray(v, np.float64) for v in (ev.x, ev.y, ev.z))
+    rows = t5["hits"].astype(np.int64)
+    key = [(chi2[i], tuple(np.stack([x[r], y[r], z[r]], 1).ravel().tolist()), tuple(r.tolist())) for i, r in enumerate(rows)]
+    assert len(set(chi2.tolist())) < len(chi2), "this event does exercise the tie-break"
+    hits = [set(r) for r in t5["hits"].tolist()]
+    by_hit = {}
+    for i, hs in enumerate(hits):
+        for h in hs:
+            by_hit.setdefault(h, []).append(i)
+    keep = np.zeros(len(hits), bool)
+    for a in sorted(range(len(hits)), key=key.__getitem__):
+        cand = {b for h in hits[a] for b in by_hit[h] if keep[b]}
+        keep[a] = not any(len(hits[a] & hits[b]) >= 5 for b in cand)
+    assert np.array_equal(keep, flags[True])
