@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(1024) k_hist(const __grid_constant__ GeoDev ge
   __syncthreads();
   // two modules (four dets: one uint4 of det_cnt) per thread and round; one block scan per round
   const uint32_t ng = geo.n_modules;
-  uint32_t carry = 0;
+  uint32_t carry = 0, rcarry = 0;
   unsigned long long my_cand = 0;
   for (uint32_t base = 0; base < ng; base += 2 * blockDim.x) {
     const uint32_t m = base + 2 * threadIdx.x;
@@ -55,6 +55,12 @@ __global__ void __launch_bounds__(1024) k_hist(const __grid_constant__ GeoDev ge
     my_cand += (unsigned long long)v.x * v.y + (unsigned long long)v.z * v.w;
     carry += tot;
     __syncthreads();
+    uint32_t rtot;                                                     // rows (lower-sensor hits) before the module
+    const uint32_t re = rcarry + block_excl_scan(v.x + v.z, sh, &rtot);
+    if (m < ng) s.md_row0[m] = re;
+    if (m + 1 < ng) s.md_row0[m + 1] = re + v.x;
+    rcarry += rtot;
+    __syncthreads();
   }
   const uint32_t total = carry;
 #pragma unroll
@@ -64,6 +70,7 @@ __global__ void __launch_bounds__(1024) k_hist(const __grid_constant__ GeoDev ge
   if (threadIdx.x == 0) {
     const bool overflow = total > st.cap_items;
     st.g_item0[ng] = total;
+    s.md_row0[ng] = rcarry;
     hdr->n_groups[S_MD] = ng;
     hdr->n_items[S_MD] = overflow ? 0u : total;
     hdr->cand[S_MD] = sh_cand;
@@ -111,6 +118,7 @@ __global__ void __launch_bounds__(256) k_rank(const __grid_constant__ GeoDev geo
     s.hit[b + r] = make_float4(x, y, z, sqrtf(x * x + y * y));
     s.hit_orig[b + r] = h;
     s.hit_key[b + r] = key;
+    if ((d & 1u) == 0u) s.row_mod[s.md_row0[d >> 1] + r] = d >> 1;   // MD row -> module (k_md_eval: one thread per row)
   }
 }
 

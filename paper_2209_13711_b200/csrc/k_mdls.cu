@@ -6,8 +6,10 @@ namespace lst {
 
 // =================================================================== MD
 // Work item = (module, rows of lower hits, columns of upper hits), <= 1024 pairs (typically ~100).
-// k_md_eval: one WARP per item, no staging and no barriers: every (lower, upper) pair goes through
-// the fp32 pre-filter, the survivors are appended to the stage's candidate list.
+// k_md_eval: one THREAD per row (lower-sensor hit), walking the upper-sensor hits of its module: a
+// module holds ~9 x 9 pairs, so per-module set-up by a warp cost more than the pairs themselves; every
+// pair goes through the fp32 pre-filter, the survivors are appended to the stage's candidate list.  The
+// row that starts a work item clears its pass bits (the decide kernel ORs them in).
 // k_md_decide: one thread per listed pair, fp64 decision; accepted pairs set their pass bit and
 // write kappa, sigma_kappa and dphi to the pool.
 __global__ void __launch_bounds__(256) k_md_eval(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
@@ -17,47 +19,50 @@ __global__ void __launch_bounds__(256) k_md_eval(const __grid_constant__ GeoDev 
   LST_SLOT(B);
   const StageBuf &st = s.st[S_MD];
   const bool live = s.hdr->n_items[S_MD] != 0;      // 0: nothing to do, or the work list overflowed
-  const int lane = threadIdx.x & 31;
-  const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
   ClBufT<64> cl;
   cl.init(&cl_mem[threadIdx.x >> 5]);
-  constexpr int kSlices = 8, kSliceCand = kItemCand / kSlices;   // a warp task = slice `sl` (128 candidates) of every item of a module
-  const uint32_t n_task = live ? geo.n_modules * kSlices : 0u;
-  for (uint32_t w = warp; w < n_task; w += nwarp) {
-    const uint32_t m = w / kSlices, sl = w % kSlices;
-    const uint32_t R = st.gR[m], W = st.gW[m];
-    if ((unsigned long long)sl * kSliceCand >= (unsigned long long)R * W) continue;           // also R W == 0; a module of several items has R W > kItemCand
-    const uint32_t it0 = st.g_item0[m], rpi = item_rpi(W), nct = item_nct(W);
-    const uint32_t n_it = ((R + rpi - 1) / rpi) * nct;
-    const int cat = geo.category[m];
-    const uint32_t lo_m = s.det_off[2 * m], up_m = s.det_off[2 * m + 1];
-    for (uint32_t k = 0; k < n_it; ++k) {
-      const uint32_t it = it0 + k;
-      uint32_t i0, j0;
-      int nrows, nj;
-      if (W <= (uint32_t)kItemCand) { i0 = k * rpi; j0 = 0; nrows = (int)min(rpi, R - i0); nj = (int)W; }
-      else { i0 = k / nct; j0 = (k % nct) * kItemCand; nrows = 1; nj = (int)min((uint32_t)kItemCand, W - j0); }
-      if (sl == 0) {
-        st.mask[(size_t)it * kItemWords + lane] = 0;             // the decide kernel ORs the pass bits in
-        if (lane == 0) st.item_group[it] = m;
-      }
-      const int nc = nrows * nj;
-      if ((int)(sl * kSliceCand) >= nc) continue;
-      const uint32_t lo0 = lo_m + i0, up0 = up_m + j0;
-      const uint32_t inv = (1u << 20) / (uint32_t)nj + 1u;      // c / nj == (c * inv) >> 20 for c * nj < 2^20
-      const int c_end = min(nc, (int)((sl + 1) * kSliceCand));
-      for (int base = (int)(sl * kSliceCand); base < c_end; base += 32) {
-        const int c = base + lane;
-        bool keep = false;
-        uint32_t hl = 0, hu = 0;
-        if (c < c_end) {
-          const int r = (int)(((uint32_t)c * inv) >> 20), jj = c - r * nj;
-          hl = lo0 + r; hu = up0 + jj;
-          const float4 l = s.hit[hl], u = s.hit[hu];
-          keep = md_pre_f(g, l.x, l.y, l.z, l.w, u.x, u.y, u.z, u.w, cat);
+  const uint32_t n_rows = live ? s.md_row0[geo.n_modules] : 0u;
+  const uint32_t n_round = (n_rows + 31u) & ~31u;   // whole warps: the list appends are warp-cooperative
+  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < n_round; t += gridDim.x * blockDim.x) {
+    uint32_t W = 0, hl = 0, up_m = 0, key0 = 0;
+    int cat = 0;
+    if (t < n_rows) {
+      const uint32_t m = s.row_mod[t], r = t - s.md_row0[m];
+      W = st.gW[m];
+      cat = geo.category[m];
+      hl = s.det_off[2 * m] + r;
+      up_m = s.det_off[2 * m + 1];
+      if (W) {
+        uint32_t it, n_clear;
+        if (W <= (uint32_t)kItemCand) {
+          const uint32_t rpi = item_rpi(W), q = r / rpi;
+          it = st.g_item0[m] + q;
+          key0 = it * (uint32_t)kItemCand + (r - q * rpi) * W;
+          n_clear = r == q * rpi ? 1u : 0u;
+        } else {
+          n_clear = item_nct(W);
+          it = st.g_item0[m] + r * n_clear;
+          key0 = it * (uint32_t)kItemCand;
         }
-        cl.push(s.hdr, st, S_MD, keep, it * (uint32_t)kItemCand + (uint32_t)c, make_uint2(hl, hu));
+        for (uint32_t k = 0; k < n_clear; ++k) {
+          uint4 *mw = reinterpret_cast<uint4 *>(st.mask + (size_t)(it + k) * kItemWords);
+#pragma unroll
+          for (int q4 = 0; q4 < kItemWords / 4; ++q4) mw[q4] = make_uint4(0u, 0u, 0u, 0u);
+          st.item_group[it + k] = m;
+        }
       }
+    }
+    const float4 l = s.hit[hl];
+    const uint32_t Wmax = __reduce_max_sync(0xffffffffu, W);
+    for (uint32_t j = 0; j < Wmax; ++j) {
+      bool keep = false;
+      const uint32_t hu = up_m + j;
+      if (j < W) {
+        const float4 u = s.hit[hu];
+        keep = md_pre_f(g, l.x, l.y, l.z, l.w, u.x, u.y, u.z, u.w, cat);
+      }
+      // W > kItemCand: the row's candidates continue in the next item(s): key0 + j still addresses (item + j / 1024, j % 1024)
+      cl.push(s.hdr, st, S_MD, keep, key0 + j, make_uint2(hl, hu));
     }
   }
   cl.flush_all(s.hdr, st, S_MD);
@@ -494,7 +499,7 @@ __global__ void __launch_bounds__(256) k_ls_fill(const __grid_constant__ Batch B
 static inline int persistent_grid(const Ctx &c, int per_sm) { return c.n_sm * per_sm; }
 
 void launch_md(const Ctx &c, const Batch &b, cudaStream_t st) {
-  launch_k(c, st, "k_md_eval", k_md_eval, dim3(persistent_grid(c, 8)), 256, 0, false, c.geo, b, c.par);
+  launch_k(c, st, "k_md_eval", k_md_eval, dim3(grid_for(b.s[0].cap_hits, 256, c.n_sm * 8)), 256, 0, false, c.geo, b, c.par);
   launch_k(c, st, "k_md_decide", k_md_decide, dim3(persistent_grid(c, 4)), 128, 0, false, c.geo, b, c.par);
   launch_counts(c, b, S_MD, 0, b.s[0].cap_md, false, st);
   launch_k(c, st, "k_md_fill", k_md_fill, dim3(persistent_grid(c, 4)), 256, 0, false, c.geo, b);

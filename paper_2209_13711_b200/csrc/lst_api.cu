@@ -324,6 +324,7 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.seed_pt = w.take<float>(nsd); s.seed_eta = w.take<float>(nsd); s.seed_phi = w.take<float>(nsd);
   s.seed_z0 = w.take<float>(nsd); s.seed_q = w.take<int8_t>(nsd); s.seed_ids = w.take<uint32_t>(4 * (size_t)nsd);
   s.det_off = w.take<uint32_t>(n_det + 1);
+  s.md_row0 = w.take<uint32_t>(n_mod + 1); s.row_mod = w.take<uint32_t>(nh);
   s.tmp_slot = w.take<uint32_t>(nh);
   s.tmp_orig = w.take<uint32_t>(nh);
   s.tmp_key = w.take<float>(nh); s.hit_key = w.take<float>(nh);

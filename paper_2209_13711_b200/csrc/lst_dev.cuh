@@ -161,6 +161,8 @@ struct SlotDev {
   float *seed_pt, *seed_eta, *seed_phi, *seed_z0; int8_t *seed_q; uint32_t *seed_ids;
   // a0: hits grouped by det
   uint32_t *det_cnt, *det_off;               // [n_det+1]
+  uint32_t *md_row0;                         // [n_modules+1] lower-sensor hits (rows of the MD stage) of the modules before m
+  uint32_t *row_mod;                         // [cap_hits] module of MD row t (t-th lower-sensor hit in sorted order)
   uint32_t *tmp_slot;                        // [cap_hits] arrival rank of a hit inside its det (k_hist)
   uint32_t *tmp_orig;                        // [cap_hits]
   float *tmp_key, *hit_key;                  // [cap_hits] azimuth relative to the module centre (sort key inside a det)
