@@ -92,7 +92,8 @@ def alu_peak_gops():
 
 # DRAM bytes (read + write) of one launch of the dominant kernel from the ncu --set full capture
 # summarised in profiles/ (the file is named in the roofline object); None for other kernels.
-NCU_TRAFFIC = {"k_ls_eval": (3004416, "profiles/r1d_top_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full")}
+NCU_TRAFFIC = {"k_ls_eval": (4499456, "profiles/r2g_top_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full"),
+               "k_s0": (11172864, "profiles/r2g_top_kernels.md")}
 
 
 class ClockSampler:
@@ -186,6 +187,16 @@ def algorithmic_bytes(name, n):
         "k_px_fill": (28 + B_PT) * (n["pt5"] + n["pt3"]),
         "k_s0": (40 + 8 + 1) * n["t5"] + (8 + 8 + 1) * (n["pt5"] + n["pt3"]),
         "k_tc_fill": B_TC * n["tc"] + 4 * (n["t5"] + n["pt5"] + n["pt3"] + n["seeds"]),
+        # cleaning (a6): lookup kernels; bytes = the objects' hit lists, scores and flags read once, the incidence
+        # rows (3 per hit: offset, cursor / count) and entries (4 B per (object, hit)) written / read once
+        "k_dd_count": (20 + 40) * n["t5"] + 8 * n["pt5"] + (8 + 24) * n["pt3"] + 12 * n["hits"],
+        "k_scan_sums": 12 * n["hits"],
+        "k_scan_apply": 24 * n["hits"],
+        "k_dd_scatter": (40 + 4 * 10) * (n["t5"] + n["pt5"]) + (24 + 4 * 6) * n["pt3"] + 24 * n["hits"],
+        "k_s0_heavy": (40 + 8 + 1) * n["tc"],
+        "k_s1": (24 + 8 + 1) * n["pt3"] + n["hits"],
+        "k_s2": (40 + 16 + 1) * n["t5"] + 2 * n["hits"] + 9 * n["seeds"],
+        "k_s3_flags": 5 * (n["t5"] + n["pt5"] + n["pt3"]) + (4 + 16 + 8) * n["seeds"],
     }
     return t.get(name)
 
