@@ -105,7 +105,7 @@ static inline int px_grid(const Ctx &c, const Batch &b) {
 // a side - its extrapolation tolerances diverge - so the lists are sized exactly, not capped per
 // seed.)  Dynamic shared memory: 8 warps x nw words of bits.
 template <bool FILL>
-__global__ void __launch_bounds__(256) k_px_modules(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
+__global__ void __launch_bounds__(256, FILL ? 6 : 5) k_px_modules(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
                                                      const __grid_constant__ Params g) {
   extern __shared__ uint32_t px_sh[];
   pdl_enter();

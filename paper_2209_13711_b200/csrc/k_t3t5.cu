@@ -378,13 +378,13 @@ __device__ __forceinline__ void join_eval_body(const SlotDev &s, const Params &g
   cl.flush_all(s.hdr, st, stage);
 }
 template <int KIND>
-__global__ void __launch_bounds__(kThreads) k_join_eval(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
+__global__ void __launch_bounds__(kThreads, 10) k_join_eval(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
   __shared__ JoinSh m;
   pdl_enter();
   LST_SLOT(B);
   join_eval_body<KIND>(s, g, m);
 }
-__global__ void __launch_bounds__(kThreads) k_px_eval(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
+__global__ void __launch_bounds__(kThreads, 10) k_px_eval(const __grid_constant__ Batch B, const __grid_constant__ Params g) {
   __shared__ JoinSh m;
   pdl_enter();
   LST_SLOT(B);
@@ -430,13 +430,13 @@ __device__ __forceinline__ void join_decide_body(const GeoDev &geo, const SlotDe
   }
 }
 template <int KIND>
-__global__ void __launch_bounds__(128) k_join_decide(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
+__global__ void __launch_bounds__(128, KIND == J_T3 ? 8 : 5) k_join_decide(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
                                                       const __grid_constant__ Params g) {
   pdl_enter();
   LST_SLOT(B);
   join_decide_body<KIND>(geo, s, g);
 }
-__global__ void __launch_bounds__(128) k_px_decide(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
+__global__ void __launch_bounds__(128, 8) k_px_decide(const __grid_constant__ GeoDev geo, const __grid_constant__ Batch B,
                                                     const __grid_constant__ Params g) {
   pdl_enter();
   LST_SLOT(B);

@@ -58,9 +58,9 @@ enum ErrBits {
 constexpr float kBoxTolLen = 5e-5f;   // cm: half the growth the host-side box arithmetic allows for
 constexpr float kBoxTolPhi = 5e-7f;   // rad (+ the fp32 rounding of the two azimuths, < 4e-6 in all)
 
-// Item / unit geometry of a group with R rows and W columns (shared by k_emit_items and the eval
-// kernels).  W <= kItemCand: one column tile, item_rpi(W) rows per item; else one row per item and
-// ceil(W / kItemCand) column tiles.  A unit = unit_items(W) consecutive row chunks of one column tile.
+// Item geometry of a group with R rows and W columns (MD, LS; a join group is one "row" of W flat
+// candidates).  W <= kItemCand: one column tile, item_rpi(W) rows per item; else one row per item and
+// ceil(W / kItemCand) column tiles.  Item (q, ct) of the group = g_item0 + q * n_ct + ct.
 __host__ __device__ __forceinline__ uint32_t item_rpi(uint32_t W) {
   if (W > (uint32_t)kItemCand) return 1u;
   const uint32_t r = (uint32_t)kItemCand / W;
