@@ -92,8 +92,8 @@ def alu_peak_gops():
 
 # DRAM bytes (read + write) of one launch of the dominant kernel from the ncu --set full capture
 # summarised in profiles/ (the file is named in the roofline object); None for other kernels.
-NCU_TRAFFIC = {"k_ls_eval": (4499456, "profiles/r2g_top_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full"),
-               "k_s0": (11172864, "profiles/r2g_top_kernels.md")}
+NCU_TRAFFIC = {"k_ls_eval": (4498688, "profiles/r2j_top_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full"),
+               "k_s0": (11162880, "profiles/r2j_top_kernels.md")}
 
 
 class ClockSampler:
