@@ -842,3 +842,56 @@ def test_s0_fixpoint_passes_match_the_oracle_fixpoint(B, geom_full, map_full, cf
         cfg = B.lst_default_config()
         cfg.s0_fixpoint_passes = 3
         B.LST(geom_full, map_full[0], map_full[1], cfg=cfg, n_slots=1, max_hits=1000, max_seeds=10)
+
+
+def test_all_options_on_degenerate_events(B, geom_barrel, map_barrel):
+    """Every optional mode at once (batched chain, occupancy caps, fix-point passes, binary16 storage,
+    no graph) on degenerate inputs: an empty event, a single hit, seeds without hits, and a normal
+    event in the same batch; then the slots re-used the other way round.  The normal event still
+    equals a plain run with the same caps; the degenerate ones give empty collections, except that
+    the hit-less event keeps its bare pixel seeds as track candidates."""
+    import dataclasses
+    ev = lstgen.make_event(geom_barrel, "cfg2s")
+    sd = lambda e: (e.seed_pt, e.seed_eta, e.seed_phi, e.seed_z0, e.seed_q, e.seed_hit_ids) if e.n_seeds else None
+    cut = lambda e, n: dataclasses.replace(e, x=e.x[:n], y=e.y[:n], z=e.z[:n], det=e.det[:n], pid=e.pid[:n])
+    noseed = dataclasses.replace(ev, seed_pt=ev.seed_pt[:0], seed_eta=ev.seed_eta[:0], seed_phi=ev.seed_phi[:0],
+                                 seed_z0=ev.seed_z0[:0], seed_q=ev.seed_q[:0], seed_hit_ids=ev.seed_hit_ids[:0],
+                                 seed_pid=ev.seed_pid[:0])
+    evs = [cut(noseed, 0), cut(noseed, 1), cut(ev, 0), ev]
+
+    def config(batch):
+        cfg = B.lst_default_config()
+        cfg.batch_events, cfg.s0_fixpoint_passes, cfg.store_half, cfg.use_cuda_graph = batch, 4, 1, 0
+        for l, k in ((O.MD, 4), (O.LS, 8), (O.T3, 8), (O.T5, 4)):
+            for L in range(16):
+                cfg.trunc_cap[l][L] = k
+        cfg.trunc_cap[O.PT3][0], cfg.trunc_cap[O.PT5][0] = 3, 2
+        return cfg
+
+    ref = B.LST(geom_barrel, map_barrel[0], map_barrel[1], cfg=config(1), n_slots=1, max_hits=ev.n_hits, max_seeds=ev.n_seeds)
+    ref.lst_load_event(0, ev.x, ev.y, ev.z, ev.det, sd(ev))
+    ref.lst_run(0)
+    want = [ref.lst_get_objects(0, lvl) for lvl in range(7)]
+    assert len(want[O.TC]["hits"]) > 10
+    ref.close()
+    lst = B.LST(geom_barrel, map_barrel[0], map_barrel[1], cfg=config(4), n_slots=4, max_hits=ev.n_hits, max_seeds=ev.n_seeds)
+    for order in ((0, 1, 2, 3), (3, 2, 1, 0)):
+        for sl, k in enumerate(order):
+            e = evs[k]
+            lst.lst_load_event(sl, e.x, e.y, e.z, e.det, sd(e))
+        lst.lst_run_batch(0)
+        for sl, k in enumerate(order):
+            cnt, _ = lst.lst_get_counts(sl)
+            assert lst.lst_get_fixpoint_unsettled(sl) == 0
+            if k < 2:
+                assert cnt.sum() == 0
+            elif k == 2:
+                assert cnt[:6].sum() == 0 and 0 < cnt[O.TC] <= ev.n_seeds
+                tc = lst.lst_get_objects(sl, O.TC)
+                assert np.all(tc["parents"][:, 0] == O.TC) and np.all(tc["hits"][:, :10] == 0xFFFFFFFF)
+            else:
+                for lvl in range(7):
+                    got = lst.lst_get_objects(sl, lvl)
+                    for key in ("hits", "parents", "f"):
+                        assert np.array_equal(got[key], want[lvl][key]), (lvl, key)
+    lst.close()
