@@ -223,10 +223,10 @@ __global__ void __launch_bounds__(256, FILL ? 6 : 5) k_px_modules(const __grid_c
   }
 }
 
-void launch_seed_prep(const Ctx &c, const Batch &b, cudaStream_t st) {
+void launch_seed_prep(const Ctx &c, const Batch &b, cudaStream_t st, bool first) {
   const size_t shb = px_shared_bytes(c);
   if (shb > 48 * 1024) cudaFuncSetAttribute(k_px_modules<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shb);
-  launch_k(c, st, "k_px_modules<false>", k_px_modules<false>, dim3(px_grid(c, b)), 256, shb, false, c.geo, b, c.par);
+  launch_k(c, st, "k_px_modules<false>", k_px_modules<false>, dim3(px_grid(c, b)), 256, shb, first, c.geo, b, c.par);
 }
 void launch_seed_rows(const Ctx &c, const Batch &b, cudaStream_t st) {
   const size_t shb = px_shared_bytes(c);

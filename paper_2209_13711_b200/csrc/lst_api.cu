@@ -721,7 +721,10 @@ extern "C" int lst_load_event(lst_ctx *c, uint32_t slot, const lst_hits *hits, c
 // Enqueue a0 .. a6 of the slots [slot0, slot0 + n) on `st` as ONE chain of launches (gridDim.z = n);
 // rec (may be NULL) counts / times the kernels.  Two memsets reset what a run accumulates into, then
 // 39 kernels; with `pdl` every kernel but the first is launched with programmatic stream serialisation.
-static int enqueue_chain(const lst_ctx *c, uint32_t slot0, uint32_t n, cudaStream_t st, Recorder *rec, bool pdl) {
+// side (capture only, else NULL): a second stream on which the seed-preparation kernel, which needs nothing
+// but the seeds, runs beside a0 .. a4 (a fork / join inside the graph); without it the kernel runs inline.
+static int enqueue_chain(const lst_ctx *c, uint32_t slot0, uint32_t n, cudaStream_t st, Recorder *rec, bool pdl,
+                         cudaStream_t side = nullptr, cudaEvent_t ev_fork = nullptr, cudaEvent_t ev_join = nullptr) {
   Recorder count_only;
   Ctx k = c->k;                    // a private copy: the recorder pointer is per call, not per context
   k.rec = rec ? rec : &count_only;
@@ -735,12 +738,21 @@ static int enqueue_chain(const lst_ctx *c, uint32_t slot0, uint32_t n, cudaStrea
     cudaMemsetAsync((char *)sl.workspace + c->zero_off, 0, c->zero_bytes, st);
     cudaMemsetAsync((char *)sl.workspace + c->ff_off, 0xFF, c->ff_bytes, st);
   }
-  launch_index(k, b, st);
-  launch_seed_prep(k, b, st);
+  if (side) {
+    cudaEventRecord(ev_fork, st);
+    cudaStreamWaitEvent(side, ev_fork, 0);
+    launch_seed_prep(k, b, side, true);
+    cudaEventRecord(ev_join, side);
+    launch_index(k, b, st);
+  } else {
+    launch_index(k, b, st);
+    launch_seed_prep(k, b, st, false);
+  }
   launch_md(k, b, st);
   launch_ls(k, b, st);
   launch_t3(k, b, st);
   launch_t5(k, b, st);
+  if (side) cudaStreamWaitEvent(st, ev_join, 0);
   launch_seed_rows(k, b, st);
   launch_pixel_joins(k, b, st);
   launch_dedup(k, b, st);
@@ -756,9 +768,17 @@ static int capture_graph(lst_ctx *c, uint32_t slot0, uint32_t n, cudaGraphExec_t
   CU(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));      // the legacy default stream cannot be captured
   cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
   if (e != cudaSuccess) { cudaStreamDestroy(cap); return cuda_fail(e, "cudaStreamBeginCapture"); }
-  const int nk = enqueue_chain(c, slot0, n, cap, nullptr, true);
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking);
+  cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming);
+  cudaEventCreateWithFlags(&ev_join, cudaEventDisableTiming);
+  const int nk = enqueue_chain(c, slot0, n, cap, nullptr, true, side, ev_fork, ev_join);
   e = cudaStreamEndCapture(cap, &gr);
   cudaStreamDestroy(cap);
+  cudaStreamDestroy(side);
+  cudaEventDestroy(ev_fork);
+  cudaEventDestroy(ev_join);
   if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
   e = cudaGraphInstantiate(out, gr, 0);
   cudaGraphDestroy(gr);

@@ -74,7 +74,7 @@ void launch_t3(const Ctx &c, const Batch &b, cudaStream_t st);
 void launch_t5(const Ctx &c, const Batch &b, cudaStream_t st);
 void launch_pixel_joins(const Ctx &c, const Batch &b, cudaStream_t st);  // pT5 and pT3 in the same launches (blockIdx.y)
 // k_pix.cu
-void launch_seed_prep(const Ctx &c, const Batch &b, cudaStream_t st);    // needs the seeds only
+void launch_seed_prep(const Ctx &c, const Batch &b, cudaStream_t st, bool first);   // needs the seeds only
 void launch_seed_rows(const Ctx &c, const Batch &b, cudaStream_t st);    // needs the MDs
 // k_dedup.cu
 void launch_dedup(const Ctx &c, const Batch &b, cudaStream_t st);
