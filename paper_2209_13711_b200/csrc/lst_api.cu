@@ -722,7 +722,8 @@ extern "C" int lst_load_event(lst_ctx *c, uint32_t slot, const lst_hits *hits, c
 // rec (may be NULL) counts / times the kernels.  Two memsets reset what a run accumulates into, then
 // 39 kernels; with `pdl` every kernel but the first is launched with programmatic stream serialisation.
 // side (capture only, else NULL): a second stream on which the seed-preparation kernel, which needs nothing
-// but the seeds, runs beside a0 .. a4 (a fork / join inside the graph); without it the kernel runs inline.
+// but the seeds, and the (seed, module) row kernel, which needs the MDs on top, run beside a0 .. a4 (a fork /
+// join inside the graph); without it the two kernels run inline.
 static int enqueue_chain(const lst_ctx *c, uint32_t slot0, uint32_t n, cudaStream_t st, Recorder *rec, bool pdl,
                          cudaStream_t side = nullptr, cudaEvent_t ev_fork = nullptr, cudaEvent_t ev_join = nullptr) {
   Recorder count_only;
@@ -742,18 +743,23 @@ static int enqueue_chain(const lst_ctx *c, uint32_t slot0, uint32_t n, cudaStrea
     cudaEventRecord(ev_fork, st);
     cudaStreamWaitEvent(side, ev_fork, 0);
     launch_seed_prep(k, b, side, true);
-    cudaEventRecord(ev_join, side);
     launch_index(k, b, st);
   } else {
     launch_index(k, b, st);
     launch_seed_prep(k, b, st, false);
   }
   launch_md(k, b, st);
+  if (side) {                      // the (seed, module) rows need the MDs and the seed preparation, nothing else
+    cudaEventRecord(ev_fork, st);
+    cudaStreamWaitEvent(side, ev_fork, 0);
+    launch_seed_rows(k, b, side);
+    cudaEventRecord(ev_join, side);
+  }
   launch_ls(k, b, st);
   launch_t3(k, b, st);
   launch_t5(k, b, st);
   if (side) cudaStreamWaitEvent(st, ev_join, 0);
-  launch_seed_rows(k, b, st);
+  else launch_seed_rows(k, b, st);
   launch_pixel_joins(k, b, st);
   launch_dedup(k, b, st);
   return k.rec->n;
