@@ -1,6 +1,7 @@
-/* lst_test.h -- test hooks of liblst_b200.so.  NOT part of the product API (include/lst.h): they run
- * the CUDA path's __host__ __device__ selection arithmetic (csrc/lst_math.cuh) on the CPU so that the
- * "-m not gpu" tests can compare it with the oracle without a GPU.  HOST pointers only.
+/* lst_test.h -- test hooks of liblst_b200.so.  NOT part of the product API (include/lst.h).
+ * lst_host_eval / lst_host_ls_window run the CUDA path's __host__ __device__ selection arithmetic
+ * (csrc/lst_math.cuh) on the CPU so that the "-m not gpu" tests can compare it with the oracle without
+ * a GPU.  lst_test_get_hit_index reads back what step a0 left in a slot.  HOST pointers only.
  */
 #ifndef LST_TEST_H
 #define LST_TEST_H
@@ -27,6 +28,14 @@ int lst_host_eval(const lst_config *cfg /* NULL = defaults */, int level, uint32
  * w[i]: bound on |dphi| of a pair that can pass L2 (> pi: none). */
 int lst_host_ls_window(const lst_config *cfg, uint32_t n, const float *row, const uint8_t *row_cat, const float *box,
                        const uint8_t *box_cat, uint8_t *live, float *w);
+
+/* Read-only view of step a0 of the slot's last run (synchronises the slot's stream): det_off
+ * (2 * n_modules + 1 words), hit_orig (n_hits words) and hit_xyzr (4 * n_hits floats) as the chain's
+ * k_hist / k_scatter / k_rank wrote them; any of the three may be NULL.  *n_hits_out (may be NULL) =
+ * hits of the event.  Used by tests/test_zz_no_alloc.py to compare lst_index_hits_static with the
+ * regular path.  LST_ESTATE before the first run of the slot. */
+int lst_test_get_hit_index(lst_ctx *ctx, uint32_t slot, uint32_t *det_off, uint32_t *hit_orig, float *hit_xyzr,
+                           uint32_t *n_hits_out);
 
 #ifdef __cplusplus
 }

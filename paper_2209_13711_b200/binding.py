@@ -23,7 +23,9 @@ LEVEL_NAMES = ("MD", "LS", "T3", "T5", "PT3", "PT5", "TC")
 EXPORTS = ("lst_default_config", "lst_build_module_map", "lst_free", "lst_create", "lst_destroy",
            "lst_workspace_bytes", "lst_bind_workspace", "lst_load_event", "lst_run", "lst_get_objects",
            "lst_get_counts", "lst_launches_per_run", "lst_run_timed", "lst_strerror", "lst_run_batch", "lst_batch_events", "lst_get_fixpoint_unsettled")
-TEST_EXPORTS = ("lst_host_eval", "lst_host_ls_window")      # include/lst_test.h
+TEST_EXPORTS = ("lst_host_eval", "lst_host_ls_window", "lst_test_get_hit_index")      # include/lst_test.h
+STATIC_EXPORTS = ("lst_index_hits_static",)                  # include/lst_static.h
+LST_STATIC_MAX_HITS, LST_STATIC_MAX_DETS = 1 << 18, 1 << 16
 
 
 class lst_config(C.Structure):
@@ -111,6 +113,8 @@ def lib():
         L.lst_strerror.restype = C.c_char_p
         L.lst_host_eval.argtypes = [C.POINTER(lst_config), C.c_int, u32, vp, vp, vp, vp, vp, vp]
         L.lst_host_ls_window.argtypes = [C.POINTER(lst_config), u32, vp, vp, vp, vp, vp, vp]
+        L.lst_test_get_hit_index.argtypes = [vp, u32, vp, vp, vp, C.POINTER(u32)]
+        L.lst_index_hits_static.argtypes = [vp, vp, vp, vp, u32, vp, u32, vp, vp, vp, vp, vp, C.c_char_p, C.c_size_t]
         _lib = L
     return _lib
 
@@ -179,6 +183,33 @@ def lst_host_ls_window(row, row_cat, box, box_cat, cfg: lst_config | None = None
     return live.astype(bool), w
 
 
+def lst_index_hits_static(x, y, z, det, phic, det_off, hit_orig, hit_xyzr, n_rejected, stream=None, n_hits=None,
+                          n_dets=None):
+    """include/lst_static.h: step a0 with the library's fixed scratch array, for callers that may not
+    allocate GPU memory.  Every array is a torch CUDA tensor the CALLER made (inputs x, y, z f32 and
+    det i32 / u32 bits of n_hits elements, phic f32 of n_dets / 2; outputs det_off [n_dets + 1],
+    hit_orig [n_hits], hit_xyzr [n_hits, 4] f32, n_rejected [1]); this wrapper only passes their
+    addresses on and allocates nothing itself.  Nothing is synchronised: the work is enqueued on
+    `stream` (default: the legacy default stream).  Events above LST_STATIC_MAX_HITS / _DETS raise
+    LstStaticError with the library's message.  Calls share one scratch array per GPU: keep them on
+    one stream (or order them with events), and make the first call on a GPU before any stream capture."""
+    n_hits = int(x.shape[0]) if n_hits is None else int(n_hits)
+    n_dets = 2 * int(phic.shape[0]) if n_dets is None else int(n_dets)
+    ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+    err = C.create_string_buffer(384)
+    rc = lib().lst_index_hits_static(ptr(x), ptr(y), ptr(z), ptr(det), n_hits, ptr(phic), n_dets, ptr(det_off),
+                                     ptr(hit_orig), ptr(hit_xyzr), ptr(n_rejected),
+                                     C.c_void_p(stream.cuda_stream if stream is not None else 0), err, len(err))
+    if rc != LST_OK:
+        raise LstStaticError(rc, err.value.decode())
+
+
+class LstStaticError(RuntimeError):
+    def __init__(self, status, text):
+        self.status = status
+        super().__init__("%s (%d)" % (text, status))
+
+
 class LST:
     """One detector on one GPU with n_slots event slots (include/lst.h).  Methods are the C calls."""
 
@@ -192,6 +223,7 @@ class LST:
         self.cfg = cfg if cfg is not None else lst_default_config()
         self.n_slots, self.max_hits, self.max_seeds = n_slots, max_hits, max_seeds
         ga = _GeomArrays(geom)
+        self._n_modules_src = ga.arr[0]
         off = np.ascontiguousarray(map_offsets, dtype=np.uint32)
         cols = np.ascontiguousarray(map_cols, dtype=np.uint32)
         cols_ = cols if cols.size else np.zeros(1, np.uint32)
@@ -296,6 +328,16 @@ class LST:
         return dict(hits=arr(o.hit_idx, (n, ar), C.c_uint32, np.uint32),
                     parents=arr(o.parents, (n, 2), C.c_uint32, np.uint32),
                     f=arr(o.f, (n, 4), C.c_float, np.float32), keep=keep)
+
+    def lst_test_get_hit_index(self, slot):
+        """Test hook (include/lst_test.h): (det_off, hit_orig, hit_xyzr [n, 4]) step a0 left in the slot."""
+        n = C.c_uint32(0)
+        _check(lib().lst_test_get_hit_index(self._h, slot, None, None, None, C.byref(n)), "lst_test_get_hit_index")
+        n = int(n.value)
+        n_det = 2 * len(self._n_modules_src)
+        det_off, orig, xyzr = np.zeros(n_det + 1, np.uint32), np.zeros(max(n, 1), np.uint32), np.zeros((max(n, 1), 4), np.float32)
+        _check(lib().lst_test_get_hit_index(self._h, slot, _p(det_off), _p(orig), _p(xyzr), None), "lst_test_get_hit_index")
+        return det_off, orig[:n], xyzr[:n]
 
     def launches_per_run(self):
         return int(lib().lst_launches_per_run(self._h))

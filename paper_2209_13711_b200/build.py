@@ -12,8 +12,9 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "liblst_b200.so")
-SOURCES = ["lst_api.cu", "k_common.cu", "k_mdls.cu", "k_t3t5.cu", "k_pix.cu", "k_dedup.cu", "k_export.cu"]
-HEADERS = ["lst_math.cuh", "lst_dev.cuh", "lst_launch.h", os.path.join("..", "..", "include", "lst.h")]
+SOURCES = ["lst_api.cu", "k_common.cu", "k_mdls.cu", "k_t3t5.cu", "k_pix.cu", "k_dedup.cu", "k_export.cu", "lst_index_static.cu"]
+HEADERS = ["lst_math.cuh", "lst_dev.cuh", "lst_launch.h", os.path.join("..", "..", "include", "lst.h"),
+           os.path.join("..", "..", "include", "lst_static.h"), os.path.join("..", "..", "include", "lst_test.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -1022,3 +1022,19 @@ extern "C" int lst_host_ls_window(const lst_config *cfg_in, uint32_t n, const fl
   }
   return LST_OK;
 }
+
+// Test hook (include/lst_test.h): what a0 left in the slot, copied to host arrays.  Reads only.
+extern "C" int lst_test_get_hit_index(lst_ctx *c, uint32_t slot, uint32_t *det_off, uint32_t *hit_orig, float *hit_xyzr,
+                                      uint32_t *n_hits_out) {
+  if (!c || slot >= c->n_slots) return einval();
+  Slot &s = c->slots[slot];
+  if (!s.ran) return LST_ESTATE;
+  const int rc = sync_header(c, s);
+  if (rc != LST_OK) return rc;
+  const uint32_t n = s.h_hdr->n_hits, n_det = c->k.geo.n_det;
+  if (det_off) CU(cudaMemcpy(det_off, s.dev.det_off, sizeof(uint32_t) * ((size_t)n_det + 1), cudaMemcpyDeviceToHost));
+  if (hit_orig && n) CU(cudaMemcpy(hit_orig, s.dev.hit_orig, sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToHost));
+  if (hit_xyzr && n) CU(cudaMemcpy(hit_xyzr, s.dev.hit, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToHost));
+  if (n_hits_out) *n_hits_out = n;
+  return LST_OK;
+}

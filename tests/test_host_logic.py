@@ -43,6 +43,13 @@ def test_library_exports_every_declared_symbol():
     assert hooks == set(B.TEST_EXPORTS) and not (hooks & declared)
     for name in sorted(hooks):
         assert hasattr(L, name), name
+    # the allocation-free entry point has a header of its own
+    static = _declared("lst_static.h")
+    assert static == set(B.STATIC_EXPORTS) and not (static & (declared | hooks))
+    for name in sorted(static):
+        assert hasattr(L, name), name
+    hdr = open(os.path.join(ROOT, "include", "lst_static.h")).read()
+    assert "LST_STATIC_MAX_HITS %du" % B.LST_STATIC_MAX_HITS in hdr and "LST_STATIC_MAX_DETS %du" % B.LST_STATIC_MAX_DETS in hdr
 
 
 def test_default_config_matches_oracle_config():
