@@ -647,11 +647,15 @@ def main():
                  "sensors hit in >= 5 modules; context only (PAPER.md:95-99 quotes ~90 % / < 5 % duplicates / 15-20 % fakes on CMS tt-bar PU200)")
     if a.truncate > 0 and world == 1 and a.events >= 8:
         # occupancy-truncated memory mode: caps at the quantile of the per-module
-        # occupancy of the first 32 events, capacities sized from the truncated sample, same 64-event batch
+        # occupancy of a calibration sample that is DISJOINT from the timed batch (16 events of the same workload,
+        # seeds 5000..5015), capacities sized from the truncated sample, then the same 64-event batch as above
         import copy
+        import lstgen
         from paper_2209_13711_b200 import occupancy
         try:
-            cfg_t, rep = occupancy.calibrate(geom, mp[0], mp[1], events[:32], quantile=a.truncate)
+            calib = [lstgen.make_event(geom, a.workload, seed=5000 + k) for k in range(16)]
+            cfg_t, rep = occupancy.calibrate(geom, mp[0], mp[1], calib, quantile=a.truncate)
+            rep["calibration_sample"] = "16 events, seeds 5000..5015 (disjoint from the timed batch)"
             b = copy.copy(a)
             b.no_e2e = True
             lst_t, _, _, _, _, cnt_t, ms_t, _, val_t, _, _, _ = run_ours(b, rank, world, local_rank, init_dist=False,

@@ -15,7 +15,8 @@
  *     on different CUDA streams concurrently ("multi-streaming").  Calls on
  *     one slot must be issued in order load -> run -> get from one host thread at a time;
  *     different slots may be driven from different host threads (nothing shared is written after
- *     lst_bind_workspace, which captures the slot's CUDA graph).
+ *     lst_bind_workspace, which captures the slot's CUDA graph; concurrent lst_bind_workspace calls
+ *     on one context are serialised inside the library).
  *   - the library never allocates device memory after lst_create(): each slot works inside one
  *     caller-provided workspace (lst_workspace_bytes / lst_bind_workspace).
  */
@@ -93,7 +94,12 @@ typedef struct {
                               at most K pT3 / pT5.  Kept are the K first in the canonical order of the
                               level (hits of a sensor ascend in azimuth relative to the module centre,
                               ties by caller index; candidates row-major over (left object, right object)).
-                              The cap_* factors above can then be sized from the truncated occupancies. */
+                              The cap_* factors above can then be sized from the truncated occupancies
+                              (paper_2209_13711_b200/occupancy.py).  The mode bounds what a BUCKET keeps, not the
+                              slot's memory: the capacities stay global (cap_* x max_hits) and the work lists hold
+                              the untruncated pre-filter survivors, so an event busier than the capacities allow
+                              is still refused with LST_ENOMEM (never a silently smaller result); size them on a
+                              sample that is disjoint from, and as busy as, the events to be served. */
   int32_t store_half;      /* 0 (default) | 1: reduced-precision storage (PAPER.md:147 outlook):
                               the derived floats that no later decision reads (MD dphi; LS dphi, kappa,
                               sigma_kappa; T3 beta; T5 R, chi2, kappa3 a / b, pT) are kept as IEEE binary16
@@ -203,8 +209,10 @@ void lst_destroy(lst_ctx *ctx);
 size_t lst_workspace_bytes(const lst_ctx *ctx);
 /* Give slot `slot` its workspace: DEVICE memory, 256-byte aligned, >= lst_workspace_bytes(), owned
  * by the caller and borrowed until lst_destroy or the next bind.  LST_ENOMEM if too small.  With
- * lst_config.use_cuda_graph the slot's chain is captured and instantiated here (the one call after
- * lst_create that allocates and synchronises); lst_run only replays it. */
+ * lst_config.use_cuda_graph the slot's chain is captured and instantiated here; besides lst_create this
+ * is the call that allocates (the graph, a small pinned header) and synchronises; lst_run only replays
+ * the graph.  The one later allocation is the pinned staging of lst_get_objects(copy_to_host = 1), see
+ * there. */
 int lst_bind_workspace(lst_ctx *ctx, uint32_t slot, void *workspace, size_t bytes);
 
 /* a0: copy one event into the slot (async on `cuda_stream`, a cudaStream_t passed as void*).
@@ -232,7 +240,11 @@ uint32_t lst_batch_events(const lst_ctx *ctx);
 int lst_get_fixpoint_unsettled(lst_ctx *ctx, uint32_t slot, uint32_t *n_unsettled);
 
 /* Synchronise the slot's stream and return a view of one level.  LST_ENOMEM if a collection
- * overflowed its capacity, LST_EINVAL if the event was invalid (see lst_load_event). */
+ * overflowed its capacity, LST_EINVAL if the event was invalid (see lst_load_event).
+ * Allocation: copy_to_host = 0 allocates nothing.  The FIRST copy_to_host = 1 call on a slot allocates
+ * that slot's pinned host staging (cudaMallocHost, sized for the largest level; kept until lst_destroy),
+ * so slots that only hand out device views never pay for it: make that first call during warm-up if the
+ * steady state must be allocation-free. */
 int lst_get_objects(lst_ctx *ctx, uint32_t slot, lst_level level, int copy_to_host, lst_objects *out);
 
 /* Per-level object counts of the slot's last run (synchronises); counts: uint32[LST_NLEVEL], HOST.

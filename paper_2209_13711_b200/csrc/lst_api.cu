@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -253,6 +254,7 @@ struct lst_ctx {
   size_t zero_off = 0, zero_bytes = 0, ff_off = 0, ff_bytes = 0;
   uint32_t batch = 1;                  // lst_config.batch_events, clamped to [1, kMaxBatch]
   std::vector<cudaGraphExec_t> group_graph;   // one per group of `batch` consecutive slots
+  std::mutex bind_mu;                  // lst_bind_workspace: binds of one context are serialised (group_graph is shared)
 };
 
 // bump allocator over the workspace; base == nullptr only measures
@@ -276,7 +278,9 @@ static uint32_t capf(float per, uint32_t n, uint32_t floor_) {
   return std::max<uint32_t>((uint32_t)c, floor_);
 }
 
-static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
+// record != NULL (lst_create only): the layout figures that do not depend on `base` (reset regions, export
+// capacities) are stored in the context; lst_bind_workspace passes NULL and writes nothing shared.
+static size_t carve(const lst_ctx *c, void *base, SlotDev *out, lst_ctx *record) {
   Carver w(base);
   SlotDev s;
   memset(&s, 0, sizeof(s));
@@ -314,10 +318,9 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.pls_min3 = s.pls_min5 + nsd;
   s.pls_best5 = (uint32_t *)(s.pls_min5 + 2 * (size_t)nsd);
   s.pls_best3 = s.pls_best5 + nsd;
-  {
-    lst_ctx *mc = const_cast<lst_ctx *>(c);
-    mc->zero_off = zero_off; mc->zero_bytes = zero_end - zero_off;
-    mc->ff_off = ff_off; mc->ff_bytes = 24 * (size_t)nsd;
+  if (record) {
+    record->zero_off = zero_off; record->zero_bytes = zero_end - zero_off;
+    record->ff_off = ff_off; record->ff_bytes = 24 * (size_t)nsd;
   }
   s.raw_x = w.take<float>(nh); s.raw_y = w.take<float>(nh); s.raw_z = w.take<float>(nh);
   s.raw_det = w.take<uint32_t>(nh);
@@ -404,8 +407,7 @@ static size_t carve(const lst_ctx *c, void *base, SlotDev *out) {
   s.exp_par = w.take<uint32_t>(2 * obj_cap);
   s.exp_f = w.take<float>(4 * obj_cap);
   if (out) *out = s;
-  const_cast<lst_ctx *>(c)->exp_obj_cap = obj_cap;
-  const_cast<lst_ctx *>(c)->exp_hit_words = hit_words;
+  if (record) { record->exp_obj_cap = obj_cap; record->exp_hit_words = hit_words; }
   return (w.off + 255) & ~(size_t)255;
 }
 
@@ -563,8 +565,18 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   e = cudaMalloc(&c->d_static, total);
   if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaMalloc(static)"); }
   char *d = (char *)c->d_static;
-  cudaMemcpy(d + o_cat, g->category, n, cudaMemcpyHostToDevice);
-  cudaMemcpy(d + o_lay, g->logical_layer, n, cudaMemcpyHostToDevice);
+  // every upload is checked: the first failure is kept and reported below (a synchronous cudaMemcpy that
+  // failed is not reported by the later cudaDeviceSynchronize)
+  cudaError_t up_err = cudaSuccess;
+  const char *up_what = "";
+  auto upload_as = [&](const char *what, void *dst, const void *src, size_t bytes) {
+    if (up_err != cudaSuccess || bytes == 0) return;
+    up_err = cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice);
+    if (up_err != cudaSuccess) up_what = what;
+  };
+#define upload(dst, src, bytes) upload_as("upload " #src, (dst), (src), (bytes))
+  upload(d + o_cat, g->category, n);
+  upload(d + o_lay, g->logical_layer, n);
   {
     // the LS enumeration walks the map without its dead edges (ls_edge_possible)
     std::vector<uint32_t> poff(n + 1, 0u), pcols;
@@ -576,23 +588,23 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
       poff[m + 1] = (uint32_t)pcols.size();
     }
     c->map_edges = nnz; c->map_edges_used = (uint32_t)pcols.size();
-    cudaMemcpy(d + o_off, poff.data(), (size_t)(n + 1) * 4, cudaMemcpyHostToDevice);
-    if (!pcols.empty()) cudaMemcpy(d + o_cols, pcols.data(), pcols.size() * 4, cudaMemcpyHostToDevice);
+    upload(d + o_off, poff.data(), (size_t)(n + 1) * 4);
+    if (!pcols.empty()) upload(d + o_cols, pcols.data(), pcols.size() * 4);
   }
   const float *box[6] = {g->rmin, g->rmax, g->phic, g->half_phi, g->zmin, g->zmax};
-  for (int k = 0; k < 6; ++k) cudaMemcpy(d + o_box + k * box_stride, box[k], (size_t)n * 4, cudaMemcpyHostToDevice);
+  for (int k = 0; k < 6; ++k) upload(d + o_box + k * box_stride, box[k], (size_t)n * 4);
   if (!start_mods.empty())
-    cudaMemcpy(d + o_start, start_mods.data(), start_mods.size() * 4, cudaMemcpyHostToDevice);
+    upload(d + o_start, start_mods.data(), start_mods.size() * 4);
   {
     std::vector<float> r1(4 * std::max<size_t>(n_prow, 1), 0.0f), r2(4 * std::max<size_t>(n_prow, 1), 0.0f);
     for (size_t r = 0; r < n_prow; ++r)
       for (int q = 0; q < 4; ++q) { r1[4 * r + q] = prow_b[8 * r + q]; r2[4 * r + q] = prow_b[8 * r + 4 + q]; }
-    cudaMemcpy(d + o_prow, r1.data(), r1.size() * 4, cudaMemcpyHostToDevice);
-    cudaMemcpy(d + o_prow2, r2.data(), r2.size() * 4, cudaMemcpyHostToDevice);
-    cudaMemcpy(d + o_poff, prow_off.data(), prow_off.size() * 4, cudaMemcpyHostToDevice);
+    upload(d + o_prow, r1.data(), r1.size() * 4);
+    upload(d + o_prow2, r2.data(), r2.size() * 4);
+    upload(d + o_poff, prow_off.data(), prow_off.size() * 4);
     if (!prow_k.empty()) {
-      cudaMemcpy(d + o_pk, prow_k.data(), prow_k.size() * 4, cudaMemcpyHostToDevice);
-      cudaMemcpy(d + o_pphi, prow_phic.data(), prow_phic.size() * 4, cudaMemcpyHostToDevice);
+      upload(d + o_pk, prow_k.data(), prow_k.size() * 4);
+      upload(d + o_pphi, prow_phic.data(), prow_phic.size() * 4);
     }
     c->k.geo.prow_b1 = (const float4 *)(d + o_prow); c->k.geo.prow_b2 = (const float4 *)(d + o_prow2);
     c->k.geo.prow_off = (const uint32_t *)(d + o_poff); c->k.geo.prow_k = (const uint32_t *)(d + o_pk);
@@ -601,9 +613,11 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
     std::vector<uint32_t> prow_of(std::max<size_t>(start_mods.size(), 1), 0u);
     for (size_t r = 0; r < n_prow; ++r)
       for (uint32_t i = prow_off[r]; i < prow_off[r + 1]; ++i) prow_of[prow_k[i]] = (uint32_t)r;
-    cudaMemcpy(d + o_pof, prow_of.data(), prow_of.size() * 4, cudaMemcpyHostToDevice);
+    upload(d + o_pof, prow_of.data(), prow_of.size() * 4);
     c->k.geo.prow_of = (const uint32_t *)(d + o_pof);
   }
+#undef upload
+  if (up_err != cudaSuccess) { cudaFree(c->d_static); delete c; return cuda_fail(up_err, up_what); }
   e = cudaDeviceSynchronize();
   if (e != cudaSuccess) { cudaFree(c->d_static); delete c; return cuda_fail(e, "upload geometry"); }
   c->k.geo.n_modules = n; c->k.geo.n_det = 2 * n;
@@ -621,7 +635,7 @@ extern "C" int lst_create(const lst_geometry *g, const lst_module_map *map, cons
   {
     // candidate keys (item * 1024 + candidate), list positions and the TC index are 32-bit
     SlotDev probe;
-    c->ws_bytes = carve(c, nullptr, &probe);
+    c->ws_bytes = carve(c, nullptr, &probe, c);
     bool fits = (double)c->cfg.cap_pt5_per_seed * max_seeds + (double)c->cfg.cap_pt3_per_seed * max_seeds +
                     (double)c->cfg.cap_t5_per_hit * max_hits + max_seeds < 4.0e9;
     for (int k = 0; k < S_NSTAGE; ++k)
@@ -662,9 +676,10 @@ extern "C" int lst_bind_workspace(lst_ctx *c, uint32_t slot, void *workspace, si
     snprintf(g_cap_err, sizeof(g_cap_err), "workspace too small: %zu bytes given, %zu needed", bytes, c->ws_bytes);
     return LST_ENOMEM;
   }
+  std::lock_guard<std::mutex> bind_lock(c->bind_mu);   // two threads binding slots of one group share group_graph[grp]
   Slot &s = c->slots[slot];
   if (s.graph) { cudaGraphExecDestroy(s.graph); s.graph = nullptr; }
-  carve(c, workspace, &s.dev);
+  carve(c, workspace, &s.dev, nullptr);
   s.workspace = workspace; s.ws_bytes = bytes;
   s.bound = true; s.loaded = false; s.ran = false;
   if (!s.h_hdr) CU(cudaMallocHost((void **)&s.h_hdr, sizeof(Header)));
@@ -770,21 +785,25 @@ static int enqueue_chain(const lst_ctx *c, uint32_t slot0, uint32_t n, cudaStrea
 // slots is written).
 static int capture_graph(lst_ctx *c, uint32_t slot0, uint32_t n, cudaGraphExec_t *out) {
   cudaGraph_t gr = nullptr;
-  cudaStream_t cap = nullptr;
-  CU(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));      // the legacy default stream cannot be captured
-  cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
-  if (e != cudaSuccess) { cudaStreamDestroy(cap); return cuda_fail(e, "cudaStreamBeginCapture"); }
-  cudaStream_t side = nullptr;
+  cudaStream_t cap = nullptr, side = nullptr;
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
-  cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking);
-  cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming);
-  cudaEventCreateWithFlags(&ev_join, cudaEventDisableTiming);
+  auto release = [&]() {
+    if (ev_join) cudaEventDestroy(ev_join);
+    if (ev_fork) cudaEventDestroy(ev_fork);
+    if (side) cudaStreamDestroy(side);
+    if (cap) cudaStreamDestroy(cap);
+  };
+  // everything the capture needs exists, and is checked, before the capture begins
+  cudaError_t e = cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking);   // the legacy default stream cannot be captured
+  const char *what = "cudaStreamCreateWithFlags(capture)";
+  if (e == cudaSuccess) { e = cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking); what = "cudaStreamCreateWithFlags(side)"; }
+  if (e == cudaSuccess) { e = cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming); what = "cudaEventCreateWithFlags(fork)"; }
+  if (e == cudaSuccess) { e = cudaEventCreateWithFlags(&ev_join, cudaEventDisableTiming); what = "cudaEventCreateWithFlags(join)"; }
+  if (e == cudaSuccess) { e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal); what = "cudaStreamBeginCapture"; }
+  if (e != cudaSuccess) { release(); return cuda_fail(e, what); }
   const int nk = enqueue_chain(c, slot0, n, cap, nullptr, true, side, ev_fork, ev_join);
   e = cudaStreamEndCapture(cap, &gr);
-  cudaStreamDestroy(cap);
-  cudaStreamDestroy(side);
-  cudaEventDestroy(ev_fork);
-  cudaEventDestroy(ev_join);
+  release();
   if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
   e = cudaGraphInstantiate(out, gr, 0);
   cudaGraphDestroy(gr);

@@ -86,30 +86,48 @@ def size_factors(cfg, sample, max_hits, max_seeds):
 
 
 def calibrate(geom, map_offsets, map_cols, events, quantile=0.999, device="cuda:0"):
-    """-> (cfg for the truncated mode, report dict).  `events`: the calibration sample."""
+    """-> (cfg for the truncated mode, report dict).  `events`: the calibration sample (keep it disjoint from
+    the events that are later timed or served: the capacities are fitted to this sample with HEADROOM /
+    CAND_HEADROOM, and an event that exceeds them is reported as LST_ENOMEM, see include/lst.h).
+
+    The report separates the two effects that shrink a workspace: re-sizing the capacity factors from a
+    sample (available to the exact mode as well) and the truncation itself.  It therefore holds THREE
+    workspaces: exact mode at the default factors, exact mode with sample-sized factors (the control), and
+    truncated mode with sample-sized factors.  `footprint_ratio` is control / truncated: the gain that is
+    due to truncation alone; `footprint_ratio_vs_defaults` includes the re-sizing."""
     mh, ms = max(e.n_hits for e in events), max(max(e.n_seeds for e in events), 1)
-    exact = B.LST(geom, map_offsets, map_cols, n_slots=1, max_hits=mh, max_seeds=ms, device=device)
+    mk = lambda cfg: B.LST(geom, map_offsets, map_cols, cfg=cfg, n_slots=1, max_hits=mh, max_seeds=ms, device=device)
+    same = lambda a, b: all(np.array_equal(x[0], y[0]) for x, y in zip(a, b))
+    exact = mk(None)
     ws_exact = exact.workspace_bytes
     s_exact = run_sample(exact, events)
     exact.close()
+    # control: the exact mode with capacities sized from the same sample, same headroom
+    sized = mk(size_factors(B.lst_default_config(), s_exact, mh, ms))
+    ws_exact_sized = sized.workspace_bytes
+    assert same(s_exact, run_sample(sized, events))      # (an overflow would raise LST_ENOMEM)
+    sized.close()
     caps = caps_from_sample(geom, events, s_exact, quantile)
     # pass 1: the caps with the default capacities -> truncated occupancies; pass 2: capacities sized from them
-    lst = B.LST(geom, map_offsets, map_cols, cfg=config_with_caps(caps), n_slots=1, max_hits=mh, max_seeds=ms, device=device)
+    lst = mk(config_with_caps(caps))
     s_tr = run_sample(lst, events)
     lst.close()
     cfg = size_factors(config_with_caps(caps), s_tr, mh, ms)
-    lst = B.LST(geom, map_offsets, map_cols, cfg=cfg, n_slots=1, max_hits=mh, max_seeds=ms, device=device)
+    lst = mk(cfg)
     ws_tr = lst.workspace_bytes
-    s_chk = run_sample(lst, events)              # must reproduce pass 1 (an overflow would raise LST_ENOMEM)
+    assert same(s_tr, run_sample(lst, events))           # must reproduce pass 1
     lst.close()
-    assert all(np.array_equal(a[0], b[0]) for a, b in zip(s_tr, s_chk))
     tot_e = np.stack([s[0] for s in s_exact]).astype(np.float64).sum(0)
     tot_t = np.stack([s[0] for s in s_tr]).astype(np.float64).sum(0)
     names = ("md", "ls", "t3", "t5", "pt3", "pt5", "tc")
     report = {
         "quantile": quantile, "events": len(events),
-        "workspace_bytes_exact_defaults": int(ws_exact), "workspace_bytes_truncated": int(ws_tr),
-        "footprint_ratio": round(ws_exact / ws_tr, 2),
+        "workspace_bytes_exact_defaults": int(ws_exact), "workspace_bytes_exact_sample_sized": int(ws_exact_sized),
+        "workspace_bytes_truncated": int(ws_tr),
+        "footprint_ratio": round(ws_exact_sized / ws_tr, 3),
+        "footprint_ratio_vs_defaults": round(ws_exact / ws_tr, 2),
+        "footprint_note": "footprint_ratio = exact mode with sample-sized capacities / truncated mode with sample-sized "
+                          "capacities (truncation alone); _vs_defaults also counts the re-sizing of the default factors",
         "objects_kept_fraction": {n: round(float(tot_t[k] / max(tot_e[k], 1.0)), 5) for k, n in enumerate(names)},
         "caps_per_layer": {names[l]: [int(v) for v in caps[l]] for l in range(4)},
         "caps_per_seed": {"pt3": int(caps[B.LST_PT3, 0]), "pt5": int(caps[B.LST_PT5, 0])},

@@ -131,3 +131,51 @@ def test_gpu_truncated_mode_matches_oracle_truncated_mode(geom_barrel, map_barre
         assert 0 < len(kg) < exact.count(lvl), "level %s: the caps must bite" % O.LEVEL_NAMES[lvl]
     assert cnt[O.TC] == o.count(O.TC) > 0
     lst.close()
+
+
+@pytest.mark.gpu
+def test_gpu_calibration_separates_resizing_from_truncation_and_a_busier_event_is_refused_loudly(geom_full, map_full):
+    """occupancy.calibrate on a small sample: the report holds the exact mode at the default factors, the exact
+    mode with sample-sized factors (the control) and the truncated mode with sample-sized factors, and quotes
+    control / truncated as the truncation gain.  Then an event four times busier than anything in the sample
+    runs with the calibrated capacities: the truncated mode caps a BUCKET, the capacities stay global, so the
+    event must be refused with LST_ENOMEM naming the stage (include/lst.h) - never a silently smaller result -
+    and the slot must serve the next event normally."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2209_13711_b200 import binding as B
+    from paper_2209_13711_b200 import occupancy
+    calib = [lstgen.make_event(geom_full, "cfg4", seed=7000 + k, n_particles=1500) for k in range(3)]
+    cfg_t, rep = occupancy.calibrate(geom_full, map_full[0], map_full[1], calib, quantile=0.99)
+    ws_d, ws_s, ws_t = (rep[k] for k in ("workspace_bytes_exact_defaults", "workspace_bytes_exact_sample_sized",
+                                         "workspace_bytes_truncated"))
+    assert ws_t <= ws_s < ws_d
+    assert rep["footprint_ratio"] == round(ws_s / ws_t, 3) and rep["footprint_ratio_vs_defaults"] == round(ws_d / ws_t, 2)
+    kept = rep["objects_kept_fraction"]
+    assert all(0.0 < kept[n] <= 1.0 for n in ("md", "ls", "t3", "t5", "tc")) and kept["ls"] < 1.0
+
+    busy = lstgen.make_event(geom_full, "cfg4", seed=7100)                  # 6 000 particles
+    mh_cal = max(e.n_hits for e in calib)
+    assert busy.n_hits > 3 * mh_cal
+    scale = mh_cal / busy.n_hits           # same capacities as calibrated, in a context that can load the busy event
+    for name in ("cap_md_per_hit", "cap_ls_per_hit", "cap_t3_per_hit", "cap_t5_per_hit", "cap_mdcand_per_hit",
+                 "cap_lscand_per_hit", "cap_t3cand_per_hit", "cap_t5cand_per_hit"):
+        setattr(cfg_t, name, getattr(cfg_t, name) * scale)
+    seeds = lambda e: (e.seed_pt, e.seed_eta, e.seed_phi, e.seed_z0, e.seed_q, e.seed_hit_ids)
+    ms = max(busy.n_seeds, max(e.n_seeds for e in calib))
+    lst = B.LST(geom_full, map_full[0], map_full[1], cfg=cfg_t, n_slots=1, max_hits=busy.n_hits, max_seeds=ms)
+    lst.lst_load_event(0, calib[0].x, calib[0].y, calib[0].z, calib[0].det, seeds(calib[0]))
+    lst.lst_run(0)
+    want, _ = lst.lst_get_counts(0)
+    assert want[O.TC] > 0
+    lst.lst_load_event(0, busy.x, busy.y, busy.z, busy.det, seeds(busy))
+    lst.lst_run(0)
+    with pytest.raises(B.LstError) as e:
+        lst.lst_get_counts(0)
+    assert e.value.status == B.LST_ENOMEM and "capacity exceeded" in str(e.value)
+    lst.lst_load_event(0, calib[0].x, calib[0].y, calib[0].z, calib[0].det, seeds(calib[0]))
+    lst.lst_run(0)
+    again, _ = lst.lst_get_counts(0)
+    assert np.array_equal(again, want), "the slot recovers after a refused event"
+    lst.close()
