@@ -652,6 +652,7 @@ def main():
         import copy
         import lstgen
         from paper_2209_13711_b200 import occupancy
+        rep = {}
         try:
             calib = [lstgen.make_event(geom, a.workload, seed=5000 + k) for k in range(16)]
             cfg_t, rep = occupancy.calibrate(geom, mp[0], mp[1], calib, quantile=a.truncate)
@@ -663,7 +664,7 @@ def main():
             rep.update({"value": val_t, "unit": UNIT, "ms_per_step": ms_t / a.steps})
             lst_t.close()
         except Exception as ex:          # reported, never hidden: the exact-mode line above stands on its own
-            rep = {"error": repr(ex)}
+            rep = dict(rep, error=repr(ex))      # the calibration report survives a refused batch
         line.setdefault("also", {})["truncated"] = rep
     if rank == 0:
         print(json.dumps(line))

@@ -18,6 +18,9 @@ from . import binding as B
 LEVELS = (B.LST_MD, B.LST_LS, B.LST_T3, B.LST_T5, B.LST_PT3, B.LST_PT5)
 HEADROOM = 1.3          # object capacities: largest occupancy of the sample x this
 CAND_HEADROOM = 1.6     # work-item capacities (the items of a module waste up to half of their 1024 candidates)
+LIST_HEADROOM = 2.0     # candidate lists: largest number of pre-filter survivors of the sample x this.  The survivors
+                        # of the pixel stages fluctuate far more from event to event than the object counts do (an
+                        # unseen event of the same workload reached 1.4 x the maximum of a 16-event sample)
 
 
 def _seeds(ev):
@@ -75,7 +78,7 @@ def size_factors(cfg, sample, max_hits, max_seeds):
     # an object capacity also sizes the stage's candidate list (2 x capacity + 4096 entries), which holds the
     # pre-filter survivors of the UNtruncated enumeration: cand[6 + stage], stages MD, LS, T3, T5, pT5, pT3
     surv = {B.LST_MD: cand[6], B.LST_LS: cand[7], B.LST_T3: cand[8], B.LST_T5: cand[9], B.LST_PT5: cand[10], B.LST_PT3: cand[11]}
-    f = lambda lvl, n: float(HEADROOM * max(cnt[lvl], 0.5 * surv[lvl]) / max(n, 1))
+    f = lambda lvl, n: float(max(HEADROOM * cnt[lvl], 0.5 * LIST_HEADROOM * surv[lvl]) / max(n, 1))
     cfg.cap_md_per_hit, cfg.cap_ls_per_hit = f(B.LST_MD, max_hits), f(B.LST_LS, max_hits)
     cfg.cap_t3_per_hit, cfg.cap_t5_per_hit = f(B.LST_T3, max_hits), f(B.LST_T5, max_hits)
     cfg.cap_pt3_per_seed, cfg.cap_pt5_per_seed = f(B.LST_PT3, max_seeds), f(B.LST_PT5, max_seeds)

@@ -257,3 +257,67 @@ def px(g, P, cats, pt, eta, phi, z0, q, first_layer):
         ok = ok & (s > 0) & (np.abs(dph) <= g.n_sigma * sphi) & (np.abs(dzt) <= g.n_sigma * szt)
         tot = tot + (dph / sphi) ** 2 + (dzt / szt) ** 2
     return ok, cuts, dict(chi2=tot / (2.0 * n))
+
+
+# ----------------------------------------------------------------------------- C2 module map
+# SURVEY.md 8(c) C2 (Fig. 4), typed from the survey's bullet list.  One point is derived
+# rather than copied: for an endcap target the survey takes "the hull over corners of (z_B - z0)/(z_A - z0)
+# (only where side (z_A - z0) > 0)".  Over the box z0 in [-z0', z0'] x z_A in [zlo_A, zhi_A] that ratio is
+# monotone in each variable, so its hull over the ADMISSIBLE part of the box is spanned by the admissible
+# corners -- unless a corner is inadmissible, in which case the admissible part reaches z_A - z0 -> 0+ and the
+# ratio has no upper bound there.  Hence: fewer than four admissible corners => upper end = +infinity.
+MAP_KSCALE, MAP_Z0, MAP_D0MAX = 1.25, 20.0, 2.5
+
+
+def map_next_layers(L):
+    """barrel l -> barrel l + 1 and disk 1 of either side; disk d -> disk d + 1 of the same side; no skips."""
+    if L < 6:
+        return ([L + 1] if L + 1 < 6 else []) + [6, 11]
+    if 6 <= L < 10 or 11 <= L < 15:
+        return [L + 1]
+    return []
+
+
+def module_map(geom, kscale=MAP_KSCALE, z0p=MAP_Z0, d0max=MAP_D0MAX, cfg=Cfg()):
+    """-> (row_offsets [n + 1], cols) of the C2 map, columns ascending inside a row."""
+    f = lambda a: np.asarray(a, np.float64)
+    lay = np.asarray(geom.logical_layer, np.int64)
+    rmin, rmax, phic, hphi, zmin, zmax = map(f, (geom.rmin, geom.rmax, geom.phic, geom.half_phi, geom.zmin, geom.zmax))
+    n = len(lay)
+    kp = kscale * cfg.kmax
+    by_layer = {L: np.nonzero(lay == L)[0] for L in range(16)}
+    target_is_endcap = lay >= 6
+    off, cols = np.zeros(n + 1, np.int64), []
+    for A in range(n):
+        cand = [by_layer[L] for L in map_next_layers(int(lay[A]))]
+        Bs = np.sort(np.concatenate(cand)) if cand else np.zeros(0, np.int64)
+        if Bs.size:
+            aA = np.arcsin(min(1.0, kp * rmin[A]))
+            aB = np.arcsin(np.minimum(1.0, kp * rmax[Bs]))
+            d = phic[Bs] - phic[A]
+            d = np.abs(d - 2 * np.pi * np.round(d / (2 * np.pi)))
+            ok_phi = d <= hphi[A] + hphi[Bs] + aB - aA + d0max * np.maximum(0.0, 1.0 / rmin[A] - 1.0 / rmax[Bs])
+            rho_lo, rho_hi = rmin[Bs] / rmax[A], aB / aA
+            ok_rz = np.zeros(Bs.size, bool)
+            bar = ~target_is_endcap[Bs]
+            # barrel target: hull of z0 + (z_A - z0) rho over the 8 corners against [zlo_B, zhi_B]
+            zp = np.stack([z0 + (zA - z0) * rho for z0 in (-z0p, z0p) for zA in (zmin[A], zmax[A]) for rho in (rho_lo, rho_hi)])
+            ok_rz[bar] = ((zp.min(0) <= zmax[Bs]) & (zp.max(0) >= zmin[Bs]))[bar]
+            # endcap target: hull of (z_B - z0) / (z_A - z0) over the admissible corners against [rho_lo, rho_hi]
+            zB = zmin[Bs]
+            side = np.where(zB > 0, 1.0, -1.0)
+            lo, hi, nvalid = np.full(Bs.size, np.inf), np.full(Bs.size, -np.inf), np.zeros(Bs.size, np.int64)
+            for z0 in (-z0p, z0p):
+                for zA in (zmin[A], zmax[A]):
+                    den = zA - z0
+                    adm = side * den > 0.0
+                    q = np.where(adm, (zB - z0) / (den if den != 0.0 else 1.0), np.nan)
+                    lo = np.where(adm, np.minimum(lo, q), lo)
+                    hi = np.where(adm, np.maximum(hi, q), hi)
+                    nvalid += adm
+            hi = np.where(nvalid < 4, np.inf, hi)
+            ec_ok = (nvalid > 0) & (lo <= rho_hi) & (hi >= rho_lo)
+            ok_rz[~bar] = ec_ok[~bar]
+            cols.append(Bs[ok_phi & ok_rz])
+        off[A + 1] = off[A] + (len(cols[-1]) if Bs.size else 0)
+    return off, (np.concatenate(cols) if cols else np.zeros(0, np.int64))

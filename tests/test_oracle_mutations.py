@@ -55,6 +55,16 @@ MUTANTS = [
     ("C6: endcap sigma_zeta without 1/|sinh eta|", "szt = g->seed_sig_z / fabs(sh) + g->sig_r[h->cat];",
      "szt = g->seed_sig_z + g->sig_r[h->cat];", "test_px_windows_terms"),
     ("C6: chi2_pix normalisation", "*chi2 = sum / (2.0 * n);", "*chi2 = sum / (1.0 * n);", "test_px_windows_terms"),
+    ("C2: displacement allowance dropped", " + g->d0max * max2(0.0, 1.0 / rminA - 1.0 / rmaxB))) return 0;", ")) return 0;",
+     "test_map_c2_"),
+    ("C2: curvature margin 1.0 instead of map_kscale", "double kp = g->map_kscale * g->kB / (2.0 * g->pt_min);",
+     "double kp = 1.0 * g->kB / (2.0 * g->pt_min);", "test_map_c2_"),
+    ("C2: barrel may skip a layer", "if (L < 6) { if (L + 1 < 6) out[n++] = L + 1; out[n++] = 6;",
+     "if (L < 6) { if (L + 2 < 6) out[n++] = L + 2; out[n++] = 6;", "test_map_c2_"),
+    ("C2: unbounded end applied to the lower end", "if (nvalid < 4) hi = INFINITY;", "if (nvalid < 4) lo = -INFINITY;", "test_map_c2_"),
+    ("C2: z0 margin 15 instead of map_z0", "double z0s[2] = {-g->map_z0, g->map_z0}", "double z0s[2] = {-g->z0max, g->z0max}", "test_map_c2_"),
+    ("C2: rho_lo from the wrong radii", "double rho_lo = rminB / rmaxA, rho_hi = aB / aA;", "double rho_lo = rminB / rminA, rho_hi = aB / aA;",
+     "test_map_c2_"),
     ("S0: > instead of >= (indexed)", "if (shared_ot(&o[a], &o[b]) >= min_shared && beats",
      "if (shared_ot(&o[a], &o[b]) > min_shared && beats", "test_s0_"),
     ("S0: > instead of >= (all pairs)", "|| shared_ot(&o[a], &o[b]) >= min_shared;", "|| shared_ot(&o[a], &o[b]) > min_shared;",

@@ -111,6 +111,43 @@ def assert_flip(fn, expected_thr, idx, rel=1e-9):
 
 
 # ----------------------------------------------------------------------------- constants
+# ----------------------------------------------------------------------------- C2 module map (two-sided)
+# The map is part of the LS definition (an LS needs B in map(A)) and both the oracle and the CUDA side's host
+# builder consume the same reading, so GPU parity cannot see a mistake in it.  Three pins, placed first in the
+# file so that the mutation test (test_oracle_mutations.py) sees a map mutant fail HERE:
+#   * edge for edge against the numpy transcription of SURVEY.md 8(c) C2 (tests/survey_restatement.py);
+#   * the figures the survey's probe printed for the full geometry (SURVEY.md 8(c) C2 "Probe");
+#   * structure: allowed layer transitions only, disk -> disk keeps the side.
+# (Completeness against simulated prompt tracks -- the inclusive side -- is in test_oracle_pins.py.)
+@pytest.mark.parametrize("which", ["barrel", "full"])
+def test_map_c2_equals_survey_restatement(geom_barrel, geom_full, which):
+    import survey_restatement as R
+    geom = geom_barrel if which == "barrel" else geom_full
+    off, cols = O.build_module_map(geom)
+    r_off, r_cols = R.module_map(geom)
+    assert np.array_equal(off.astype(np.int64), r_off), "row sizes differ from the SURVEY restatement"
+    assert np.array_equal(cols.astype(np.int64), r_cols), "edges differ from the SURVEY restatement"
+
+
+def test_map_c2_probe_figures_and_layer_structure(geom_full):
+    off, cols = O.build_module_map(geom_full)
+    deg = np.diff(off.astype(np.int64))
+    lay = np.asarray(geom_full.logical_layer, np.int64)
+    # SURVEY.md 8(c) C2 "Probe": 237 398 directed edges, mean degree 23.9, max 144, barrel L1 mean 64,
+    # barrel L6 and disk 5 (either side) have no outgoing edge
+    assert int(off[-1]) == 237398
+    assert deg.max() == 144
+    assert abs(deg.mean() - 23.9) < 0.05
+    assert abs(deg[lay == 0].mean() - 64.0) < 1.0
+    assert deg[(lay == 5) | (lay == 10) | (lay == 15)].max() == 0 and deg[lay == 4].min() > 0
+    src = np.repeat(np.arange(len(deg)), deg)
+    la, lb = lay[src], lay[cols.astype(np.int64)]
+    barrel_ok = (la < 6) & ((lb == la + 1) & (lb < 6) | (lb == 6) | (lb == 11))
+    disk_ok = (la >= 6) & (lb == la + 1) & (lb != 11)
+    assert np.all(barrel_ok | disk_ok), "an edge skips a layer or changes the endcap side"
+    assert np.all(np.diff(cols.astype(np.int64))[np.diff(src) == 0] > 0), "columns ascend inside a row"
+
+
 def test_chi2max_is_the_1e4_quantile_of_chi2_with_2_dof():
     """chi2max = 18.42 (p = 1e-4, 2 dof): survival of chi2(2) is exp(-x/2)."""
     c = O.default_config()
