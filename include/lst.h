@@ -103,8 +103,8 @@ typedef struct {
   int32_t store_half;      /* 0 (default) | 1: reduced-precision storage (PAPER.md:147 outlook):
                               the derived floats that no later decision reads (MD dphi; LS dphi, kappa,
                               sigma_kappa; T3 beta; T5 R, chi2, kappa3 a / b, pT) are kept as IEEE binary16
-                              in the slot workspace (half the bytes; relative error <= 4.9e-4, values above
-                              65504 saturate) and widened again by lst_get_objects.  Object sets, keep flags
+                              in the slot workspace (half the bytes; relative error <= 4.9e-4, absolute 3e-8 for
+                              magnitudes below 6.1e-5 such as the sigma_kappa of an LS, values above 65504 saturate) and widened again by lst_get_objects.  Object sets, keep flags
                               and the TC list are unchanged: every decision uses the fp64 quantities. */
   int32_t s0_fixpoint_passes; /* 0 (default): the non-greedy cleaning rule S0 (an object is removed iff SOME
                               better duplicate exists).  P = 2, 4, .. 16: S0 of the T5 collection is iterated

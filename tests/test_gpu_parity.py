@@ -38,10 +38,10 @@ def _gpu(B, geom, mp, ev, upto_tc=True, **kw):
     return lst
 
 
-def _oracle(geom, mp, ev, upto):
+def _oracle(geom, mp, ev, upto, pixel_indexed=False):
     o = O.Oracle(geom, mp[0], mp[1])
     o.load(ev)
-    o.run(upto=upto)
+    o.run(upto=upto, pixel_indexed=pixel_indexed)
     return o
 
 
@@ -391,7 +391,7 @@ class _Components:
                     self.union(h[0], self.pls0 + q)
 
 
-def compare_cleaning(o, lst, ev, slot=0, diff=None):
+def compare_cleaning(o, lst, ev, slot=0, diff=None, f_rtol=REL):
     """Keep flags object by object, the TC list entry by entry and the TC floats.  diff: per level the
     keys that exist on one side only (near-threshold differences of the object building); the
     comparison then covers every object that cannot be influenced by one of them."""
@@ -449,7 +449,7 @@ def compare_cleaning(o, lst, ev, slot=0, diff=None):
     io = {k: i for i, k in enumerate(keys_o)}
     sel = [i for i, k in enumerate(keys_g) if k in io]
     f_o, f_g = tc_o["f"][[io[keys_g[i]] for i in sel]], got["f"].astype(np.float64)[sel]
-    assert np.allclose(f_g, f_o, rtol=REL, atol=1e-6)
+    assert np.allclose(f_g, f_o, rtol=f_rtol, atol=1e-6)
     if n_diff:
         print("cleaning compared on %d objects / %d TC entries outside the components of %d near-threshold objects"
               % (n_cmp, len(so), n_diff))
@@ -756,6 +756,18 @@ def test_batched_chain_equals_single_slot_runs(B, geom_full, map_full, batch, pd
                     assert np.array_equal(got[k], want[k]), (i, lvl, k)
                 if want["keep"] is not None:
                     assert np.array_equal(got["keep"], want["keep"]), (i, lvl)
+    # ... and the batched chain itself faces the oracle (not only the single-slot CUDA run): two slots of the
+    # last round, one of them in the last (possibly partial) group, at every level incl. keep flags and TC
+    for sl in (1, n_slots - 1):
+        e = evs[(sl + 1) % n_slots]
+        o = _oracle(geom_full, map_full, e, O.TC, pixel_indexed=True)
+        view = _SlotView(lst, sl)
+        diff = {}
+        for lvl in ALL_LEVELS:
+            n, near, _, _ = compare_level(o, view, lvl)
+            assert n == o.count(lvl) and n > 100
+            diff[lvl] = differing(o, view, lvl)
+        assert compare_cleaning(o, view, e, diff=diff) > 100
     # a group with an unloaded slot is refused, never run partially
     fresh = B.LST(geom_full, map_full[0], map_full[1], cfg=cfg, n_slots=batch, max_hits=mh, max_seeds=ms)
     e = evs[0]
@@ -776,6 +788,10 @@ def test_reduced_precision_storage_changes_only_exported_floats(B, geom_full, ma
     relative (round to nearest; R saturates at 65504 cm), the others not at all; the workspace shrinks."""
     ev = lstgen.make_event(geom_full, "cfg4")
     sd = (ev.seed_pt, ev.seed_eta, ev.seed_phi, ev.seed_z0, ev.seed_q, ev.seed_hit_ids)
+    o = _oracle(geom_full, map_full, ev, O.TC, pixel_indexed=True)
+    # columns of `f` stored in binary16 per level: MD dphi; LS all; T3 beta; T5 all; TC pt of the T5-type entries
+    half_cols = {O.MD: [0], O.LS: [0, 1, 2], O.T3: [0], O.T5: [0, 1, 2, 3], O.PT3: [], O.PT5: [], O.TC: [0]}
+    HALF = 2.0 ** -11 * 1.0001
     runs = []
     for half in (0, 1):
         cfg = B.lst_default_config()
@@ -784,11 +800,27 @@ def test_reduced_precision_storage_changes_only_exported_floats(B, geom_full, ma
         lst.lst_load_event(0, ev.x, ev.y, ev.z, ev.det, sd)
         lst.lst_run(0)
         runs.append(([lst.lst_get_objects(0, lvl) for lvl in range(7)], lst.workspace_bytes))
+        if half:
+            # the binary16 mode against the ORACLE: object sets, keep flags and the TC list identical; the fp32
+            # columns within the suite's 1e-4, the binary16 columns within 1e-4 + 2^-11 of the oracle's fp64 value
+            for lvl in ALL_LEVELS:
+                n, near, ref, got = compare_level(o, lst, lvl, check_floats=False)
+                assert n == o.count(lvl) and near == 0 and n > 100
+                ir = {t: i for i, t in enumerate(_keys(lvl, ref))}
+                a = ref["f"][[ir[t] for t in _keys(lvl, got)]]
+                b = got["f"].astype(np.float64)
+                for c in range({O.MD: 3, O.LS: 3, O.T3: 3, O.T5: 4, O.PT3: 1, O.PT5: 1}[lvl]):
+                    x, y = a[:, c], b[:, c]
+                    # binary16: relative 2^-11 in its normal range, absolute 2^-25 below 6.1e-5 (subnormals; the
+                    # sigma_kappa of a line segment is ~1e-5 and lands there), saturation at 65504
+                    ok = np.abs(x) <= 6.5e4
+                    half_err = np.maximum(HALF * np.abs(x), 2.0 ** -25) if c in half_cols[lvl] else 0.0
+                    excess = np.abs(x - y) - (REL * np.abs(x) + half_err + ABS_TINY)
+                    assert ok.sum() > 0.99 * len(x) and excess[ok].max() <= 0.0, (O.LEVEL_NAMES[lvl], c, excess[ok].max())
+            assert compare_cleaning(o, lst, ev, f_rtol=REL + HALF) > 100
         lst.close()
     (full, ws_full), (half, ws_half) = runs
     assert ws_half < ws_full
-    # columns of `f` stored in binary16 per level: MD dphi; LS all; T3 beta; T5 all; TC pt of the T5-type entries
-    half_cols = {O.MD: [0], O.LS: [0, 1, 2], O.T3: [0], O.T5: [0, 1, 2, 3], O.PT3: [], O.PT5: [], O.TC: [0]}
     worst = 0.0
     for lvl in range(7):
         a, b = full[lvl], half[lvl]
@@ -811,12 +843,13 @@ def test_reduced_precision_storage_changes_only_exported_floats(B, geom_full, ma
     print("store_half: workspace %.1f -> %.1f MB, largest relative change of an exported float %.2e" % (ws_full / 1e6, ws_half / 1e6, worst))
 
 
-@pytest.mark.parametrize("cfg_name,passes", [("cfg4", 8), ("cfg3", 8)])
-def test_s0_fixpoint_passes_match_the_oracle_fixpoint(B, geom_full, map_full, cfg_name, passes):
+@pytest.mark.parametrize("cfg_name,passes,seed", [("cfg4", 8, None), ("cfg3", 8, None), ("cfg4h", 16, 1000)])
+def test_s0_fixpoint_passes_match_the_oracle_fixpoint(B, geom_full, map_full, cfg_name, passes, seed):
     """lst_config.s0_fixpoint_passes iterates S0 of the T5 collection to the greedy
     fix-point; keep flags of every collection and the TC list equal the oracle's fix-point mode, the
-    iteration has converged (0 unsettled objects), and the non-greedy survivors are a strict subset."""
-    ev = lstgen.make_event(geom_full, cfg_name)
+    iteration has converged (0 unsettled objects), and the non-greedy survivors are a strict subset.
+    The third case is the bench size: event 0 of the bench batch (cfg4h, seed 1000), 16 passes (12 leave 2 T5 unsettled)."""
+    ev = lstgen.make_event(geom_full, cfg_name, seed=seed)
     sd = (ev.seed_pt, ev.seed_eta, ev.seed_phi, ev.seed_z0, ev.seed_q, ev.seed_hit_ids) if ev.n_seeds else None
     o = O.Oracle(geom_full, map_full[0], map_full[1])
     o.set_s0_fixpoint(True)
@@ -832,7 +865,18 @@ def test_s0_fixpoint_passes_match_the_oracle_fixpoint(B, geom_full, map_full, cf
             lst.lst_run(0)
         keeps[p] = lst.lst_get_objects(0, O.T5)["keep"].copy()
         if p:
-            assert lst.lst_get_fixpoint_unsettled(0) == 0
+            unsettled = lst.lst_get_fixpoint_unsettled(0)
+            if unsettled and seed is not None:
+                # not converged within the maximum number of passes: include/lst.h then promises a duplicate-free
+                # SUBSET of the fix-point; check that against the oracle's fix-point and stop there
+                got5 = lst.lst_get_objects(0, O.T5)
+                kept_g = {k for k, f in zip(_keys(O.T5, got5), got5["keep"].tolist()) if f}
+                kept_o = {k for k, f in zip(_keys(O.T5, o.get(O.T5)), o.keep(O.T5).tolist()) if f}
+                print("fix-point: %d unsettled after %d passes; kept %d of the oracle's %d" % (unsettled, p, len(kept_g), len(kept_o)))
+                assert unsettled <= 8 and kept_g <= kept_o and len(kept_o) - len(kept_g) <= 8 * unsettled
+                lst.close()
+                continue
+            assert unsettled == 0
             diff = {lvl: differing(o, lst, lvl) for lvl in ALL_LEVELS}
             assert not any(diff.values()), "this event has no near-threshold object"
             assert compare_cleaning(o, _SlotView(lst, 0), ev) > 100
@@ -873,6 +917,23 @@ def test_all_options_on_degenerate_events(B, geom_barrel, map_barrel):
     ref.lst_run(0)
     want = [ref.lst_get_objects(0, lvl) for lvl in range(7)]
     assert len(want[O.TC]["hits"]) > 10
+    # the reference run of this test is itself compared with the oracle in the same modes (occupancy caps in
+    # azimuth order, fix-point S0): object sets at every level, keep flags and TC entries; TC pt at binary16
+    caps = np.zeros((6, 16), np.uint32)
+    cfg_c = config(1)
+    for l in range(6):
+        for L in range(16):
+            caps[l, L] = cfg_c.trunc_cap[l][L]
+    o = O.Oracle(geom_barrel, map_barrel[0], map_barrel[1])
+    o.set_truncation(geom_barrel.phic, caps)
+    o.set_s0_fixpoint(True)
+    o.load(ev)
+    o.run(upto=O.TC, pixel_indexed=True)
+    assert ref.lst_get_fixpoint_unsettled(0) == 0
+    for lvl in ALL_LEVELS:
+        n, near, _, _ = compare_level(o, ref, lvl, check_floats=False)
+        assert n == o.count(lvl) and near == 0 and n > 10
+    assert compare_cleaning(o, ref, ev, f_rtol=REL + 2.0 ** -11 * 1.0001) > 10
     ref.close()
     lst = B.LST(geom_barrel, map_barrel[0], map_barrel[1], cfg=config(4), n_slots=4, max_hits=ev.n_hits, max_seeds=ev.n_seeds)
     for order in ((0, 1, 2, 3), (3, 2, 1, 0)):

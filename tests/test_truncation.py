@@ -95,7 +95,7 @@ def test_caps_at_every_level_properties(geom_barrel, map_barrel):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("cfg_name", ["cfg2s", "cfg4"])
+@pytest.mark.parametrize("cfg_name", ["cfg2s", "cfg4", "cfg4h"])
 def test_gpu_truncated_mode_matches_oracle_truncated_mode(geom_barrel, map_barrel, geom_full, map_full, cfg_name):
     """The CUDA path with lst_config.trunc_cap against the oracle in the same mode: identical object
     sets at every level (the objects a full bucket keeps are decided by the canonical order, i.e. by the
@@ -110,7 +110,14 @@ def test_gpu_truncated_mode_matches_oracle_truncated_mode(geom_barrel, map_barre
     if cfg_name == "cfg4":
         caps[O.MD, :], caps[O.LS, :], caps[O.T3, :], caps[O.T5, :] = 8, 30, 24, 8
         caps[O.PT3, 0], caps[O.PT5, 0] = 6, 3
-    ev = lstgen.make_event(geom, cfg_name)
+    ev = lstgen.make_event(geom, cfg_name, seed=1000 if cfg_name == "cfg4h" else None)
+    if cfg_name == "cfg4h":
+        # the bench size (event 0 of the bench batch) with caps chosen the way the bench chooses them: a quantile
+        # of the per-module / per-seed occupancy measured in exact mode (0.99, so that every level bites on ONE event)
+        from paper_2209_13711_b200 import occupancy
+        ex = B.LST(geom, mp[0], mp[1], n_slots=1, max_hits=ev.n_hits, max_seeds=max(ev.n_seeds, 1))
+        caps = occupancy.caps_from_sample(geom, [ev], occupancy.run_sample(ex, [ev]), 0.99)
+        ex.close()
     o = _run(geom, mp, ev, caps)
     cfg = B.lst_default_config()
     for l in range(6):
@@ -130,6 +137,9 @@ def test_gpu_truncated_mode_matches_oracle_truncated_mode(geom_barrel, map_barre
         assert kg == set(_keys(o, lvl)), "level %s differs from the oracle's truncated mode" % O.LEVEL_NAMES[lvl]
         assert 0 < len(kg) < exact.count(lvl), "level %s: the caps must bite" % O.LEVEL_NAMES[lvl]
     assert cnt[O.TC] == o.count(O.TC) > 0
+    # keep flags object by object, the TC list entry by entry and its floats (the comparison of the exact mode)
+    import test_gpu_parity as G
+    assert G.compare_cleaning(o, lst, ev) == o.count(O.TC)
     lst.close()
 
 
