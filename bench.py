@@ -90,10 +90,20 @@ def alu_peak_gops():
     return n_sm * 128 * mhz * 1e6 / 1e9, "%d SMs x 128 fp32 lanes x %.0f MHz (%s), FMA = 1 op" % (n_sm, mhz, src)
 
 
-# DRAM bytes (read + write) of one launch of the dominant kernel from the ncu --set full capture
-# summarised in profiles/ (the file is named in the roofline object); None for other kernels.
-NCU_TRAFFIC = {"k_ls_eval": (4498688, "profiles/r2j_top_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full"),
-               "k_s0": (11162880, "profiles/r2j_top_kernels.md")}
+# DRAM bytes (read + write) of one launch of a kernel, from the ncu capture summarised under profiles/:
+# profiles/*_traffic.json (the newest round's file wins) maps kernel name -> {"dram_bytes": ..., "source": ...}
+# and is written from the ncu CSV by hand-run tooling, never by this program.
+def ncu_traffic(kernel):
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.json")))
+    if not files:
+        return None, None
+    try:
+        t = json.load(open(files[-1]))
+        e = t["kernels"].get(kernel)
+        return (int(e["dram_bytes"]), "profiles/%s: %s" % (os.path.basename(files[-1]), t["source"])) if e else (None, None)
+    except Exception:
+        return None, None
 
 
 class ClockSampler:
@@ -161,7 +171,22 @@ def algorithmic_bytes(name, n):
     """Bytes one launch of kernel `name` must move for an event with the object counts n."""
     bits = lambda k: n["cand"][k] / 8.0          # one pass bit per candidate (+ ~0.4 % item headers)
     nmod, nnz = n["n_modules"], n["nnz"]
+    # k_counts: the stage's pass-bit words read once (one bit per candidate of the definition), the 16-bit running
+    # counts per word written, count + base per item of 1024 candidates
+    counts = lambda ks: sum(1.5 * bits(k) + 8.0 * n["cand"][k] / 1024.0 for k in ks)
+    pairs, nw4 = n["px_pairs"], 4 * ((n["n_start"] + 31) // 32)
     t = {
+        # seed preparation: the seed, its 4 pixel-hit ids into the hash set, one bit per start module, the count;
+        # the box rows of the start modules once.  (seed, module) rows: the bits again, pair + MD range per row
+        "k_px_modules<false>": n["seeds"] * (B_SEED + 8 * 4 + nw4 + 4 + 8) + 32 * n["n_prow"] + 4 * n["n_start"],
+        "k_px_modules<true>": n["seeds"] * (nw4 + 16 + 4) + pairs * (8 + 8 + 8 + 4),
+        "k_counts[MD]": counts([0]), "k_counts[LS]": counts([1]), "k_counts[T3]": counts([2]), "k_counts[T5]": counts([3]),
+        "k_counts[pT5+pT3]": counts([4, 5]),
+        # row lists of the joins: per row (an LS / a T3 / a (seed, module) pair) its key, the CSR range of its right
+        # objects, first right object and running candidate count
+        "k_join_groups[T3]": (8 + 8 + 8) * n["ls"] + 12 * (n["ls"] / 128.0),
+        "k_join_groups[T5]": (8 + 8 + 8) * n["t3"] + 12 * (n["t3"] / 128.0),
+        "k_px_groups": 2 * ((8 + 8 + 8) * pairs + 12 * (pairs / 128.0)),
         "k_hist": (16 + 4) * n["hits"] + 4 * 2 * nmod * 3 + 12 * nmod,   # + det scan and MD groups in its last block
         "k_scatter": 4 * n["hits"] * 2 + 4 * 2 * nmod,
         "k_rank": (B_HIT_IN + B_HIT + 4) * n["hits"],
@@ -208,7 +233,21 @@ OPS_PER_CAND = {"k_md_eval": (0, 27), "k_ls_eval": (1, 36), "k_join_eval[T3]": (
                 "k_join_eval[T5]": (3, 4 + 128), "k_px_eval": ((4, 5), 68)}
 
 
+# Index machinery and cleaning: integer / lookup work, counted as lane-operations of the walk the method defines
+#   k_px_modules: one window test (px_row_window: ~40 operations incl. two asin or a sin and a division) per
+#     (seed, row of identical start-module boxes), resp. per (seed, module) pair;
+#   k_rank: a hit is compared with every hit of its sensor (2 operations per comparison);
+#   S0 (k_s0 + k_s0_heavy): for every object and each of its hits, the objects of the same collection on that hit
+#     are visited once (load, compare, count: 4 operations) = 4 x sum over hits of (objects on the hit)^2.
 def algorithmic_ops(name, n):
+    if name == "k_px_modules<false>":
+        return 40 * n["seeds"] * n["n_prow"]
+    if name == "k_px_modules<true>":
+        return 40 * n["px_pairs"]
+    if name == "k_rank":
+        return 2 * n["rank_cmp"]
+    if name == "k_s0":
+        return 4 * n["s0_visits"]
     if name not in OPS_PER_CAND:
         return None
     k, ops = OPS_PER_CAND[name]
@@ -529,6 +568,20 @@ def kernel_table(lst, B, devt, streams, a, geom, nnz, peak, alu_peak):
          "t5": int(cnt[3]), "pt3": int(cnt[4]), "pt5": int(cnt[5]), "tc": int(cnt[6]),
          "cand": [int(c) for c in cand[:6]], "surv": [int(c) for c in cand[6:12]], "eval": [int(c) for c in cand[12:18]],
          "n_modules": int(geom.n_modules), "nnz": int(nnz)}
+    # sizes of the index machinery (host arithmetic on the geometry and on event 0's exported objects)
+    lay = np.asarray(geom.logical_layer, np.int64)
+    start = np.isin(lay, (0, 1, 6, 7, 11, 12))
+    box = np.stack([np.asarray(getattr(geom, k), np.float64)[start] for k in ("rmin", "rmax", "half_phi", "zmin", "zmax")] +
+                   [np.asarray(geom.category, np.float64)[start]], 1)
+    n["n_start"], n["n_prow"] = int(start.sum()), int(len(np.unique(box, axis=0)))
+    n["px_pairs"] = int(6 * n["seeds"])         # (seed, start module) rows: an ESTIMATE, ~6 per seed (k_pix.cu); the count is not exported
+    det = h[3].cpu().numpy().astype(np.int64)
+    n["rank_cmp"] = int((np.bincount(det).astype(np.int64) ** 2).sum())
+    visits = 0
+    for lvl, ot in ((B.LST_T5, 10), (B.LST_PT5, 10), (B.LST_PT3, 6)):
+        hh = lst.lst_get_objects(0, lvl)["hits"][:, :ot].astype(np.int64).ravel()
+        visits += int((np.bincount(hh).astype(np.int64) ** 2).sum()) if hh.size else 0
+    n["s0_visits"] = visits
     names = [k for k, _ in runs[0]]
     med = np.median(np.array([[m for _, m in r] for r in runs]), axis=0)
     chain_ms = float(med.sum())
@@ -551,7 +604,7 @@ def roofline(top, peak, peak_src, alu_peak, alu_src):
     bound by the plain fp32 ALUs: achieved = algorithmic fp32 lane-operations per
     launch / live duration against SMs x lanes x clock; the HBM view of the same kernel is kept
     beside it because BASELINE.json's metric asks for it."""
-    traffic, traffic_src = NCU_TRAFFIC.get(top["kernel"], (None, None))
+    traffic, traffic_src = ncu_traffic(top["kernel"])
     if top["gops"] is not None:
         r = {"bound": "alu", "kernel": top["kernel"], "achieved": top["gops"], "peak": round(alu_peak, 1),
              "unit": "Gop/s", "frac": top["frac_alu"], "traffic": traffic, "traffic_source": traffic_src,
