@@ -72,6 +72,50 @@ def test_md_cap_is_the_first_k_of_a_numpy_restatement(geom_barrel, map_barrel):
     assert got == want
 
 
+def test_caps_at_every_level_keep_the_first_k_of_a_numpy_restatement(geom_barrel, map_barrel):
+    """WHICH objects a full bucket keeps, at every level, typed independently of the oracle's truncation code
+    and cascaded from the EXACT collections (acceptance depends only on the object's own constituents, so the
+    truncated level = the exact level restricted to kept constituents, then cut per bucket):
+      MD   order inside a module: (azimuth of the lower hit relative to the module centre, its index, the same of
+           the upper hit); global MD order = (module, that)
+      LS   candidates row-major over (inner MD, outer MD) in MD order; bucket = module of the inner MD
+      T3   row-major over (first LS, second LS) in LS order; T5 likewise over T3s; bucket = module of the first MD
+      pT3 / pT5: per pixel seed, the T3 / T5 in their own order."""
+    ev = lstgen.make_event(geom_barrel, "cfg2s")
+    exact, tr = _run(geom_barrel, map_barrel, ev, None, order=False), _run(geom_barrel, map_barrel, ev, CAPS)
+    lay = np.asarray(geom_barrel.logical_layer, np.int64)
+    phic = np.asarray(geom_barrel.phic, np.float64)
+    x, y, det = ev.x.astype(np.float64), ev.y.astype(np.float64), ev.det.astype(np.int64)
+    rel = lambda h: float(np.remainder(np.arctan2(y[h], x[h]) - phic[det[h] >> 1] + np.pi, 2 * np.pi) - np.pi)
+
+    def first_k(cands, key, bucket, cap):
+        """cands: tuples; keep per bucket the cap(bucket) first in key order -> (kept set, rank of every kept one)"""
+        kept, n_in = [], {}
+        for t in sorted(cands, key=key):
+            b = bucket(t)
+            if n_in.get(b, 0) < cap(b):
+                n_in[b] = n_in.get(b, 0) + 1
+                kept.append(t)
+        return {t: r for r, t in enumerate(kept)}          # ranks follow the key order: usable as the next level's order
+
+    hits = lambda lvl: [tuple(r) for r in exact.get(lvl)["hits"].astype(np.int64).tolist()]
+    mod_of = lambda t: int(det[t[0]] >> 1)
+    cap_mod = lambda lvl: (lambda m: int(CAPS[lvl, lay[m]]))
+    md = first_k(hits(O.MD), lambda t: (mod_of(t), rel(t[0]), t[0], rel(t[1]), t[1]), mod_of, cap_mod(O.MD))
+    ls = first_k([t for t in hits(O.LS) if t[0:2] in md and t[2:4] in md], lambda t: (md[t[0:2]], md[t[2:4]]), mod_of, cap_mod(O.LS))
+    t3 = first_k([t for t in hits(O.T3) if t[0:4] in ls and t[2:6] in ls], lambda t: (ls[t[0:4]], ls[t[2:6]]), mod_of, cap_mod(O.T3))
+    t5 = first_k([t for t in hits(O.T5) if t[0:6] in t3 and t[4:10] in t3], lambda t: (t3[t[0:6]], t3[t[4:10]]), mod_of, cap_mod(O.T5))
+    want = {O.MD: set(md), O.LS: set(ls), O.T3: set(t3), O.T5: set(t5)}
+    for lvl, below, cap in ((O.PT3, t3, int(CAPS[O.PT3, 0])), (O.PT5, t5, int(CAPS[O.PT5, 0]))):
+        d = exact.get(lvl)
+        cands = [(int(p), *h) for p, h in zip(d["parents"][:, 0].tolist(), d["hits"].astype(np.int64).tolist()) if tuple(h) in below]
+        want[lvl] = set(first_k(cands, lambda t: (t[0], below[t[1:]]), lambda t: t[0], lambda b: cap))
+    for lvl in (O.MD, O.LS, O.T3, O.T5, O.PT3, O.PT5):
+        got = set(_keys(tr, lvl))
+        assert len(want[lvl]) < exact.count(lvl), "level %s: the cap must bite" % O.LEVEL_NAMES[lvl]
+        assert got == want[lvl], "level %s: %d kept objects differ from the restatement" % (O.LEVEL_NAMES[lvl], len(got ^ want[lvl]))
+
+
 def test_caps_at_every_level_properties(geom_barrel, map_barrel):
     ev = lstgen.make_event(geom_barrel, "cfg2s")
     exact, tr = _run(geom_barrel, map_barrel, ev, None, order=False), _run(geom_barrel, map_barrel, ev, CAPS)
